@@ -1,0 +1,739 @@
+/*
+ * fxoracle.c -- plain, slow CPU oracle of the batched block Euler update.
+ *
+ * TEST INFRASTRUCTURE ONLY.  Only tests/, __graft_entry__.smoke() and the
+ * cpu_baseline / --impl reference legs of bench.py may load this library.  It
+ * shares no code, header, table or helper with the CUDA path under
+ * paper_2208_11630_b200/csrc/ (it re-declares its own enums; the values are
+ * compared numerically by the tests, not through a common header).
+ *
+ * What it computes: the hot path BASELINE.json's north_star names -- guard-cell
+ * fill, primitive recovery with the gamma-law EOS, PLM-minmod or WENO5-JS
+ * reconstruction, HLLE or HLLC fluxes, flux divergence, SSP-RK2/3 and the CFL
+ * time step -- block by block [PAPER.md L69, section 2: "Bulk of their code is
+ * written for block-by-block update"], explicit shock capturing [PAPER.md L71],
+ * SSP-RK of order 2 or 3 [PAPER.md L103, section 2.2], perfect gas [PAPER.md
+ * L105].  PAPER.md prints no formula; every formula below is the textbook one
+ * in the reading SURVEY.md section 8(c) fixes (tags O1..O7, A1..A27) and
+ * DESIGN.md lists.  The method is an explicit iteration, so the oracle is the
+ * algorithm itself, step by step, in fp64, with no blocking, fusion or
+ * reordering.  Built with -O2 -ffp-contract=off (no FMA contraction).
+ *
+ * Pins (tests/test_oracle_*.py, -m "not gpu"): see DESIGN.md "Oracle pins".
+ * Parity unpinned: none of the routines; the Kelvin-Helmholtz field after 100
+ * steps and the config-5 field after 10 steps have no exact solution and are
+ * pinned only through conservation, symmetry and the per-routine pins.
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+#define FXO_OK 0
+#define FXO_ERR_INVALID_ARG (-1)
+#define FXO_ERR_STATE (-2)
+#define FXO_ERR_UNSUPPORTED (-3)
+#define FXO_ERR_NOMEM (-4)
+
+#define FXO_RECON_PLM_MINMOD 0
+#define FXO_RECON_WENO5 1
+#define FXO_RIEMANN_HLLE 0
+#define FXO_RIEMANN_HLLC 1
+#define FXO_BC_OUTFLOW (-1)
+#define FXO_BC_NONE (-2)
+#define FXO_OPT_RHO_FLOOR 0
+#define FXO_OPT_P_FLOOR 1
+#define FXO_OPT_WENO_EPS 2
+#define FXO_OPT_WAVESPEED 3
+#define FXO_STATUS_NONFINITE 1u
+#define FXO_STATUS_RHO_FLOOR 2u
+#define FXO_STATUS_P_FLOOR 4u
+#define FXO_STATUS_WENO_FALLBACK 8u
+
+typedef struct fxo_plan {
+  int n[3];       /* interior zones per block, x y z */
+  int g;          /* guard depth in active dimensions */
+  int gd[3];      /* guard depth per dimension (0 if inactive) [A26] */
+  int np[3];      /* padded extent per dimension */
+  int active[3];
+  int nvars;
+  int64_t nblocks;
+  double gamma;
+  int recon, riemann, rk;
+  int64_t S_j, S_k, S_b, S_v;
+  double rho_floor, p_floor, weno_eps;
+  int wavespeed; /* 0 Einfeldt, 1 Davis [A8] */
+  const int32_t *neigh;
+  unsigned long long n_nonfinite, n_rho_floor, n_p_floor, n_weno_fb;
+} fxo_plan;
+
+typedef struct fxo_layout {
+  int32_t np[3];
+  int32_t gd[3];
+  int64_t S_j, S_k, S_b, S_v;
+  int64_t bytes_per_state;
+} fxo_layout;
+
+/* ------------------------------------------------------------------ plan */
+
+int fxo_plan_create(fxo_plan **out, const int dims[3], int nguard, int nvars, int64_t nblocks,
+                    double gamma, int recon, int riemann, int rk_order) {
+  if (!out || !dims) return FXO_ERR_INVALID_ARG;
+  *out = NULL;
+  if (nvars != 5 || nblocks < 0 || !(gamma > 1.0)) return FXO_ERR_INVALID_ARG;
+  if (recon != FXO_RECON_PLM_MINMOD && recon != FXO_RECON_WENO5) return FXO_ERR_INVALID_ARG;
+  if (riemann != FXO_RIEMANN_HLLE && riemann != FXO_RIEMANN_HLLC) return FXO_ERR_INVALID_ARG;
+  if (rk_order != 2 && rk_order != 3) return FXO_ERR_INVALID_ARG;
+  if (nguard < (recon == FXO_RECON_WENO5 ? 3 : 2)) return FXO_ERR_INVALID_ARG;
+  for (int d = 0; d < 3; ++d)
+    if (dims[d] < 1) return FXO_ERR_INVALID_ARG;
+  fxo_plan *p = (fxo_plan *)calloc(1, sizeof(fxo_plan));
+  if (!p) return FXO_ERR_NOMEM;
+  int nactive = 0;
+  for (int d = 0; d < 3; ++d) {
+    p->n[d] = dims[d];
+    p->active[d] = dims[d] > 1;
+    if (p->active[d]) {
+      ++nactive;
+      if (nguard > dims[d]) {
+        free(p);
+        return FXO_ERR_INVALID_ARG;
+      }
+    }
+    p->gd[d] = p->active[d] ? nguard : 0;
+    p->np[d] = dims[d] + 2 * p->gd[d];
+  }
+  if (nactive == 0) {
+    free(p);
+    return FXO_ERR_INVALID_ARG;
+  }
+  p->g = nguard;
+  p->nvars = nvars;
+  p->nblocks = nblocks;
+  p->gamma = gamma;
+  p->recon = recon;
+  p->riemann = riemann;
+  p->rk = rk_order;
+  p->S_j = p->np[0];
+  p->S_k = (int64_t)p->np[0] * p->np[1];
+  p->S_b = p->S_k * p->np[2];
+  p->S_v = p->S_b * nblocks;
+  p->rho_floor = 1e-12;
+  p->p_floor = 1e-12;
+  p->weno_eps = 1e-6;
+  p->wavespeed = 0;
+  *out = p;
+  return FXO_OK;
+}
+
+void fxo_plan_destroy(fxo_plan *p) { free(p); }
+
+int fxo_plan_layout(const fxo_plan *p, fxo_layout *L) {
+  if (!p || !L) return FXO_ERR_INVALID_ARG;
+  for (int d = 0; d < 3; ++d) {
+    L->np[d] = p->np[d];
+    L->gd[d] = p->gd[d];
+  }
+  L->S_j = p->S_j;
+  L->S_k = p->S_k;
+  L->S_b = p->S_b;
+  L->S_v = p->S_v;
+  L->bytes_per_state = p->S_v * p->nvars * (int64_t)sizeof(double);
+  return FXO_OK;
+}
+
+int fxo_plan_set_option(fxo_plan *p, int key, double value) {
+  if (!p) return FXO_ERR_INVALID_ARG;
+  switch (key) {
+  case FXO_OPT_RHO_FLOOR: p->rho_floor = value; return FXO_OK;
+  case FXO_OPT_P_FLOOR: p->p_floor = value; return FXO_OK;
+  case FXO_OPT_WENO_EPS: p->weno_eps = value; return FXO_OK;
+  case FXO_OPT_WAVESPEED:
+    if (value != 0.0 && value != 1.0) return FXO_ERR_INVALID_ARG;
+    p->wavespeed = (int)value;
+    return FXO_OK;
+  default: return FXO_ERR_INVALID_ARG;
+  }
+}
+
+int fxo_plan_set_topology(fxo_plan *p, const int32_t *neigh) {
+  if (!p || (!neigh && p->nblocks > 0)) return FXO_ERR_INVALID_ARG;
+  for (int64_t b = 0; b < p->nblocks; ++b)
+    for (int f = 0; f < 6; ++f) {
+      int32_t v = neigh[b * 6 + f];
+      int d = f / 2;
+      if (!p->active[d]) continue; /* entries of inactive dims are ignored [A26] */
+      if (v >= 0) {
+        if (v >= p->nblocks) return FXO_ERR_INVALID_ARG;
+      } else if (v != FXO_BC_OUTFLOW) {
+        return FXO_ERR_UNSUPPORTED; /* coarse/fine neighbours have no code [A18] */
+      }
+    }
+  p->neigh = neigh;
+  return FXO_OK;
+}
+
+int fxo_status(fxo_plan *p, uint32_t *flags, unsigned long long counts[4]) {
+  if (!p || !flags) return FXO_ERR_INVALID_ARG;
+  uint32_t f = 0;
+  if (p->n_nonfinite) f |= FXO_STATUS_NONFINITE;
+  if (p->n_rho_floor) f |= FXO_STATUS_RHO_FLOOR;
+  if (p->n_p_floor) f |= FXO_STATUS_P_FLOOR;
+  if (p->n_weno_fb) f |= FXO_STATUS_WENO_FALLBACK;
+  *flags = f;
+  if (counts) {
+    counts[0] = p->n_nonfinite;
+    counts[1] = p->n_rho_floor;
+    counts[2] = p->n_p_floor;
+    counts[3] = p->n_weno_fb;
+  }
+  return FXO_OK;
+}
+
+void fxo_status_reset(fxo_plan *p) {
+  if (p) p->n_nonfinite = p->n_rho_floor = p->n_p_floor = p->n_weno_fb = 0;
+}
+
+/* ------------------------------------------------- regular-tiling topology */
+
+static uint64_t morton3(uint32_t x, uint32_t y, uint32_t z) {
+  uint64_t m = 0;
+  for (int b = 0; b < 21; ++b) {
+    m |= (uint64_t)((x >> b) & 1u) << (3 * b);
+    m |= (uint64_t)((y >> b) & 1u) << (3 * b + 1);
+    m |= (uint64_t)((z >> b) & 1u) << (3 * b + 2);
+  }
+  return m;
+}
+
+typedef struct {
+  uint64_t key;
+  int32_t lex;
+} fxo_sortrec;
+
+static int cmp_sortrec(const void *a, const void *b) {
+  const fxo_sortrec *x = (const fxo_sortrec *)a, *y = (const fxo_sortrec *)b;
+  return (x->key > y->key) - (x->key < y->key);
+}
+
+/* bc codes: 0 periodic, 1 outflow, 2 none (inactive dimension).  order: 0 lexicographic
+ * (x fastest), 1 Morton.  neigh_out [nb][6], coords_out [nb][3] (block coordinates). */
+int fxo_topology_cartesian(const int nb[3], const int bc_lo[3], const int bc_hi[3], int order,
+                           int32_t *neigh_out, int32_t *coords_out) {
+  if (!nb || !bc_lo || !bc_hi || !neigh_out) return FXO_ERR_INVALID_ARG;
+  int64_t N = (int64_t)nb[0] * nb[1] * nb[2];
+  if (nb[0] < 1 || nb[1] < 1 || nb[2] < 1 || N > 2147483647LL) return FXO_ERR_INVALID_ARG;
+  int32_t *id_of_lex = (int32_t *)malloc((size_t)N * sizeof(int32_t));
+  fxo_sortrec *rec = (fxo_sortrec *)malloc((size_t)N * sizeof(fxo_sortrec));
+  if (!id_of_lex || !rec) {
+    free(id_of_lex);
+    free(rec);
+    return FXO_ERR_NOMEM;
+  }
+  for (int64_t l = 0; l < N; ++l) {
+    int bx = (int)(l % nb[0]), by = (int)((l / nb[0]) % nb[1]), bz = (int)(l / ((int64_t)nb[0] * nb[1]));
+    rec[l].lex = (int32_t)l;
+    rec[l].key = order == 1 ? morton3((uint32_t)bx, (uint32_t)by, (uint32_t)bz) : (uint64_t)l;
+  }
+  if (order == 1) qsort(rec, (size_t)N, sizeof(fxo_sortrec), cmp_sortrec);
+  for (int64_t id = 0; id < N; ++id) id_of_lex[rec[id].lex] = (int32_t)id;
+  for (int64_t id = 0; id < N; ++id) {
+    int64_t l = rec[id].lex;
+    int c[3] = {(int)(l % nb[0]), (int)((l / nb[0]) % nb[1]), (int)(l / ((int64_t)nb[0] * nb[1]))};
+    if (coords_out)
+      for (int d = 0; d < 3; ++d) coords_out[id * 3 + d] = c[d];
+    for (int d = 0; d < 3; ++d)
+      for (int s = 0; s < 2; ++s) {
+        int bc = s ? bc_hi[d] : bc_lo[d];
+        int32_t v;
+        if (bc == 2) {
+          v = FXO_BC_NONE;
+        } else {
+          int cc[3] = {c[0], c[1], c[2]};
+          cc[d] += s ? 1 : -1;
+          if (cc[d] < 0 || cc[d] >= nb[d]) {
+            if (bc == 0) {
+              cc[d] = (cc[d] + nb[d]) % nb[d];
+              v = id_of_lex[((int64_t)cc[2] * nb[1] + cc[1]) * nb[0] + cc[0]];
+            } else {
+              v = FXO_BC_OUTFLOW;
+            }
+          } else {
+            v = id_of_lex[((int64_t)cc[2] * nb[1] + cc[1]) * nb[0] + cc[0]];
+          }
+        }
+        neigh_out[id * 6 + 2 * d + s] = v;
+      }
+  }
+  free(id_of_lex);
+  free(rec);
+  return FXO_OK;
+}
+
+/* --------------------------------------------------------- O1 guard fill */
+
+/* Source of padded zone (i,j,k) of block b: hops in the order z, y, x [O1, A14].
+ * Returns the flat variable-0 element index of the interior zone it images. */
+static int64_t guard_source(const fxo_plan *p, int64_t b, int i, int j, int k) {
+  int c[3] = {i, j, k};
+  int64_t bs = b;
+  for (int d = 2; d >= 0; --d) {
+    if (!p->active[d]) continue;
+    int lo = p->gd[d], hi = p->gd[d] + p->n[d];
+    if (c[d] < lo) {
+      int32_t nb = p->neigh[bs * 6 + 2 * d];
+      if (nb >= 0) {
+        bs = nb;
+        c[d] += p->n[d];
+      } else {
+        c[d] = lo; /* outflow: zero-gradient clamp */
+      }
+    } else if (c[d] >= hi) {
+      int32_t nb = p->neigh[bs * 6 + 2 * d + 1];
+      if (nb >= 0) {
+        bs = nb;
+        c[d] -= p->n[d];
+      } else {
+        c[d] = hi - 1;
+      }
+    }
+  }
+  return bs * p->S_b + c[2] * p->S_k + c[1] * p->S_j + c[0];
+}
+
+int fxo_guardcell_index_map(fxo_plan *p, int64_t block_begin, int64_t block_count, int64_t *src) {
+  if (!p || !src || block_begin < 0 || block_count < 0 || block_begin + block_count > p->nblocks)
+    return FXO_ERR_INVALID_ARG;
+  if (!p->neigh && p->nblocks > 0) return FXO_ERR_STATE;
+  for (int64_t bb = 0; bb < block_count; ++bb)
+    for (int k = 0; k < p->np[2]; ++k)
+      for (int j = 0; j < p->np[1]; ++j)
+        for (int i = 0; i < p->np[0]; ++i)
+          src[bb * p->S_b + k * p->S_k + j * p->S_j + i] = guard_source(p, block_begin + bb, i, j, k);
+  return FXO_OK;
+}
+
+int fxo_fill_guardcells(fxo_plan *p, double *U) {
+  if (!p || (!U && p->nblocks > 0)) return FXO_ERR_INVALID_ARG;
+  if (!p->neigh && p->nblocks > 0) return FXO_ERR_STATE;
+  /* Sources are always interior zones, which a fill never writes: in-place is safe. */
+#pragma omp parallel for schedule(static)
+  for (int64_t b = 0; b < p->nblocks; ++b)
+    for (int k = 0; k < p->np[2]; ++k)
+      for (int j = 0; j < p->np[1]; ++j)
+        for (int i = 0; i < p->np[0]; ++i) {
+          int interior = i >= p->gd[0] && i < p->gd[0] + p->n[0] && j >= p->gd[1] &&
+                         j < p->gd[1] + p->n[1] && k >= p->gd[2] && k < p->gd[2] + p->n[2];
+          if (interior) continue;
+          int64_t s = guard_source(p, b, i, j, k);
+          int64_t t = b * p->S_b + k * p->S_k + j * p->S_j + i;
+          for (int v = 0; v < p->nvars; ++v) U[v * p->S_v + t] = U[v * p->S_v + s];
+        }
+  return FXO_OK;
+}
+
+/* ---------------------------------------------------- O2 cons -> prim */
+
+/* U = (rho, mx, my, mz, E) -> W = (rho, u, v, w, p).  Floors touch primitives only [A7]. */
+static void cons2prim(const fxo_plan *p, const double U[5], double W[5], unsigned *hit) {
+  double rho = U[0];
+  if (rho < p->rho_floor) { /* NaN compares false and stays NaN */
+    rho = p->rho_floor;
+    *hit |= FXO_STATUS_RHO_FLOOR;
+  }
+  double r = 1.0 / rho;
+  double u = U[1] * r, v = U[2] * r, w = U[3] * r;
+  double pr = (p->gamma - 1.0) * (U[4] - 0.5 * (U[1] * u + U[2] * v + U[3] * w));
+  if (pr < p->p_floor) {
+    pr = p->p_floor;
+    *hit |= FXO_STATUS_P_FLOOR;
+  }
+  W[0] = rho;
+  W[1] = u;
+  W[2] = v;
+  W[3] = w;
+  W[4] = pr;
+  if (!isfinite(rho) || !isfinite(u) || !isfinite(v) || !isfinite(w) || !isfinite(pr))
+    *hit |= FXO_STATUS_NONFINITE;
+}
+
+void fxo_cons2prim(const fxo_plan *p, const double U[5], double W[5]) {
+  unsigned hit = 0;
+  cons2prim(p, U, W, &hit);
+}
+
+/* ------------------------------------------------- O3 reconstruction */
+
+/* minmod in comparison form [A4]: no products, NaN -> 0. */
+double fxo_minmod(double a, double b) {
+  if (a > 0.0 && b > 0.0) return a < b ? a : b;
+  if (a < 0.0 && b < 0.0) return a > b ? a : b;
+  return 0.0;
+}
+
+/* WENO5-JS value at the +1/2 face of the cell holding c, from cell values a..e (textbook,
+ * Jiang & Shu 1996) [O3, A5].  eps absolute, exponent 2. */
+double fxo_weno5(double a, double b, double c, double d, double e, double eps) {
+  const double sixth = 1.0 / 6.0;
+  double p0 = (2.0 * a - 7.0 * b + 11.0 * c) * sixth;
+  double p1 = (-b + 5.0 * c + 2.0 * d) * sixth;
+  double p2 = (2.0 * c + 5.0 * d - e) * sixth;
+  double t0 = a - 2.0 * b + c, u0 = a - 4.0 * b + 3.0 * c;
+  double t1 = b - 2.0 * c + d, u1 = b - d;
+  double t2 = c - 2.0 * d + e, u2 = 3.0 * c - 4.0 * d + e;
+  double b0 = (13.0 / 12.0) * (t0 * t0) + 0.25 * (u0 * u0);
+  double b1 = (13.0 / 12.0) * (t1 * t1) + 0.25 * (u1 * u1);
+  double b2 = (13.0 / 12.0) * (t2 * t2) + 0.25 * (u2 * u2);
+  double a0 = 0.1 / ((eps + b0) * (eps + b0));
+  double a1 = 0.6 / ((eps + b1) * (eps + b1));
+  double a2 = 0.3 / ((eps + b2) * (eps + b2));
+  return (a0 * p0 + a1 * p1 + a2 * p2) / (a0 + a1 + a2);
+}
+
+/* Left and right primitive states at the face between padded cells iL and iR = iL + 1 along a
+ * line of stride s in the primitive array W (5 slabs of size slab). */
+static void reconstruct_face(const fxo_plan *p, const double *W, int64_t slab, int64_t cL, int64_t s,
+                             double WL[5], double WR[5], unsigned *hit) {
+  int64_t cR = cL + s;
+  if (p->recon == FXO_RECON_PLM_MINMOD) {
+    for (int v = 0; v < 5; ++v) {
+      const double *q = W + v * slab;
+      double dL = fxo_minmod(q[cL] - q[cL - s], q[cL + s] - q[cL]);
+      double dR = fxo_minmod(q[cR] - q[cR - s], q[cR + s] - q[cR]);
+      WL[v] = q[cL] + 0.5 * dL;
+      WR[v] = q[cR] - 0.5 * dR;
+    }
+  } else {
+    for (int v = 0; v < 5; ++v) {
+      const double *q = W + v * slab;
+      WL[v] = fxo_weno5(q[cL - 2 * s], q[cL - s], q[cL], q[cL + s], q[cL + 2 * s], p->weno_eps);
+      WR[v] = fxo_weno5(q[cR + 2 * s], q[cR + s], q[cR], q[cR - s], q[cR - 2 * s], p->weno_eps);
+    }
+    /* positivity fallback, per side [A6] */
+    if (!(WL[0] > 0.0) || !(WL[4] > 0.0)) {
+      for (int v = 0; v < 5; ++v) WL[v] = W[v * slab + cL];
+      *hit |= FXO_STATUS_WENO_FALLBACK;
+    }
+    if (!(WR[0] > 0.0) || !(WR[4] > 0.0)) {
+      for (int v = 0; v < 5; ++v) WR[v] = W[v * slab + cR];
+      *hit |= FXO_STATUS_WENO_FALLBACK;
+    }
+  }
+}
+
+/* ---------------------------------------------------- O4 Riemann flux */
+
+/* States in the face frame: W = (rho, un, ut1, ut2, p); flux F = (mass, normal momentum,
+ * t1 momentum, t2 momentum, energy).  Einfeldt (Roe-average) or Davis wave-speed bounds [A8];
+ * HLLE in branching form [A10]; Toro's HLLC with the test order of O4 [A9]. */
+static void riemann_flux(const fxo_plan *p, const double WL[5], const double WR[5], double F[5]) {
+  const double gam = p->gamma, gm1 = p->gamma - 1.0, igm1 = 1.0 / (p->gamma - 1.0);
+  double rL = WL[0], unL = WL[1], t1L = WL[2], t2L = WL[3], pL = WL[4];
+  double rR = WR[0], unR = WR[1], t1R = WR[2], t2R = WR[3], pR = WR[4];
+  double irL = 1.0 / rL, irR = 1.0 / rR;
+  double cL = sqrt(gam * pL * irL), cR = sqrt(gam * pR * irR);
+  double EL = pL * igm1 + 0.5 * rL * (unL * unL + t1L * t1L + t2L * t2L);
+  double ER = pR * igm1 + 0.5 * rR * (unR * unR + t1R * t1R + t2R * t2R);
+  double UL[5] = {rL, rL * unL, rL * t1L, rL * t2L, EL};
+  double UR[5] = {rR, rR * unR, rR * t1R, rR * t2R, ER};
+  double FL[5] = {UL[1], UL[1] * unL + pL, UL[1] * t1L, UL[1] * t2L, unL * (EL + pL)};
+  double FR[5] = {UR[1], UR[1] * unR + pR, UR[1] * t1R, UR[1] * t2R, unR * (ER + pR)};
+  double SL, SR;
+  if (p->wavespeed == 0) {
+    double HL = (EL + pL) * irL, HR = (ER + pR) * irR;
+    double sl = sqrt(rL), sr = sqrt(rR);
+    double wi = 1.0 / (sl + sr);
+    double un = (sl * unL + sr * unR) * wi;
+    double t1 = (sl * t1L + sr * t1R) * wi;
+    double t2 = (sl * t2L + sr * t2R) * wi;
+    double H = (sl * HL + sr * HR) * wi;
+    double c = sqrt(gm1 * (H - 0.5 * (un * un + t1 * t1 + t2 * t2)));
+    double a = unL - cL, b = un - c;
+    SL = a < b ? a : b;
+    a = unR + cR;
+    b = un + c;
+    SR = a > b ? a : b;
+  } else {
+    double a = unL - cL, b = unR - cR;
+    SL = a < b ? a : b;
+    a = unL + cL;
+    b = unR + cR;
+    SR = a > b ? a : b;
+  }
+  if (SL >= 0.0) {
+    for (int v = 0; v < 5; ++v) F[v] = FL[v];
+    return;
+  }
+  if (SR <= 0.0) {
+    for (int v = 0; v < 5; ++v) F[v] = FR[v];
+    return;
+  }
+  if (p->riemann == FXO_RIEMANN_HLLE) {
+    double den = SR - SL, ss = SL * SR;
+    for (int v = 0; v < 5; ++v) F[v] = (SR * FL[v] - SL * FR[v] + ss * (UR[v] - UL[v])) / den;
+    return;
+  }
+  /* HLLC */
+  double aL = rL * (SL - unL), aR = rR * (SR - unR);
+  double Ss = ((pR - pL) + (aL * unL - aR * unR)) / (aL - aR);
+  if (Ss >= 0.0) {
+    double f = aL / (SL - Ss);
+    double Us[5] = {f, f * Ss, f * t1L, f * t2L, f * (EL * irL + (Ss - unL) * (Ss + pL / aL))};
+    for (int v = 0; v < 5; ++v) F[v] = FL[v] + SL * (Us[v] - UL[v]);
+  } else {
+    double f = aR / (SR - Ss);
+    double Us[5] = {f, f * Ss, f * t1R, f * t2R, f * (ER * irR + (Ss - unR) * (Ss + pR / aR))};
+    for (int v = 0; v < 5; ++v) F[v] = FR[v] + SR * (Us[v] - UR[v]);
+  }
+}
+
+/* Public, for the per-routine pins: states and flux in the face frame (rho, un, ut1, ut2, p). */
+void fxo_riemann_flux(const fxo_plan *p, const double WL[5], const double WR[5], double F[5]) {
+  riemann_flux(p, WL, WR, F);
+}
+
+/* ------------------------------------------------ O5 spatial operator */
+
+/* Face flux in direction d at the face whose left cell has flat in-block index cL, returned in
+ * the un-rotated variable order (rho, mx, my, mz, E). */
+static void face_flux(const fxo_plan *p, const double *W, int64_t slab, int64_t cL, int d, double F[5],
+                      unsigned *hit) {
+  const int64_t stride[3] = {1, p->S_j, p->S_k};
+  /* frame of direction d: normal = d, t1 = (d+1)%3, t2 = (d+2)%3 */
+  int in = 1 + d, it1 = 1 + (d + 1) % 3, it2 = 1 + (d + 2) % 3;
+  double WLu[5], WRu[5], WLf[5], WRf[5], Ff[5];
+  reconstruct_face(p, W, slab, cL, stride[d], WLu, WRu, hit);
+  WLf[0] = WLu[0]; WLf[1] = WLu[in]; WLf[2] = WLu[it1]; WLf[3] = WLu[it2]; WLf[4] = WLu[4];
+  WRf[0] = WRu[0]; WRf[1] = WRu[in]; WRf[2] = WRu[it1]; WRf[3] = WRu[it2]; WRf[4] = WRu[4];
+  riemann_flux(p, WLf, WRf, Ff);
+  F[0] = Ff[0];
+  F[in] = Ff[1];
+  F[it1] = Ff[2];
+  F[it2] = Ff[3];
+  F[4] = Ff[4];
+  for (int v = 0; v < 5; ++v)
+    if (!isfinite(F[v])) *hit |= FXO_STATUS_NONFINITE;
+}
+
+static void count_hits(fxo_plan *p, unsigned hit, unsigned long long n) {
+  if (!hit) return;
+  if (hit & FXO_STATUS_NONFINITE) {
+#pragma omp atomic
+    p->n_nonfinite += n;
+  }
+  if (hit & FXO_STATUS_RHO_FLOOR) {
+#pragma omp atomic
+    p->n_rho_floor += n;
+  }
+  if (hit & FXO_STATUS_P_FLOOR) {
+#pragma omp atomic
+    p->n_p_floor += n;
+  }
+  if (hit & FXO_STATUS_WENO_FALLBACK) {
+#pragma omp atomic
+    p->n_weno_fb += n;
+  }
+}
+
+/* Primitives of every padded zone of block b of X into W[5][S_b] (guards must be filled). */
+static void block_prims(fxo_plan *p, const double *X, int64_t b, double *W) {
+  for (int k = 0; k < p->np[2]; ++k)
+    for (int j = 0; j < p->np[1]; ++j)
+      for (int i = 0; i < p->np[0]; ++i) {
+        int64_t c = k * p->S_k + j * p->S_j + i;
+        double U[5], Wz[5];
+        for (int v = 0; v < 5; ++v) U[v] = X[v * p->S_v + b * p->S_b + c];
+        unsigned hit = 0;
+        cons2prim(p, U, Wz, &hit);
+        for (int v = 0; v < 5; ++v) W[v * p->S_b + c] = Wz[v];
+        int interior = i >= p->gd[0] && i < p->gd[0] + p->n[0] && j >= p->gd[1] &&
+                       j < p->gd[1] + p->n[1] && k >= p->gd[2] && k < p->gd[2] + p->n[2];
+        if (interior) count_hits(p, hit, 1); /* count each zone once, where it is owned */
+      }
+}
+
+/* One RK stage on block b: out = U0 + beta*((X - U0) - S(X)), S = sum_d (dt/dx_d)(F+ - F-)
+ * summed in the order x, y, z [O5, O6].  W and Fline are per-thread scratch. */
+static void block_stage(fxo_plan *p, const double *X, const double *U0, double *out, int64_t b,
+                        const double *dx, double dt, double beta, int first, double *W, double *S,
+                        double *Fline) {
+  block_prims(p, X, b, W);
+  const int64_t stride[3] = {1, p->S_j, p->S_k};
+  memset(S, 0, sizeof(double) * 5 * (size_t)p->S_b);
+  for (int d = 0; d < 3; ++d) {
+    if (!p->active[d]) continue;
+    double r = dt / dx[b * 3 + d];
+    int d1 = (d + 1) % 3, d2 = (d + 2) % 3;
+    for (int a2 = p->gd[d2]; a2 < p->gd[d2] + p->n[d2]; ++a2)
+      for (int a1 = p->gd[d1]; a1 < p->gd[d1] + p->n[d1]; ++a1) {
+        int64_t base = a1 * stride[d1] + a2 * stride[d2];
+        unsigned hit = 0;
+        for (int f = 0; f <= p->n[d]; ++f) {
+          int64_t cL = base + (int64_t)(p->gd[d] + f - 1) * stride[d];
+          face_flux(p, W, p->S_b, cL, d, Fline + 5 * f, &hit);
+        }
+        count_hits(p, hit & (FXO_STATUS_NONFINITE | FXO_STATUS_WENO_FALLBACK), 1);
+        for (int f = 0; f < p->n[d]; ++f) {
+          int64_t c = base + (int64_t)(p->gd[d] + f) * stride[d];
+          for (int v = 0; v < 5; ++v) S[v * p->S_b + c] += r * (Fline[5 * (f + 1) + v] - Fline[5 * f + v]);
+        }
+      }
+  }
+  for (int k = p->gd[2]; k < p->gd[2] + p->n[2]; ++k)
+    for (int j = p->gd[1]; j < p->gd[1] + p->n[1]; ++j)
+      for (int i = p->gd[0]; i < p->gd[0] + p->n[0]; ++i) {
+        int64_t c = k * p->S_k + j * p->S_j + i;
+        for (int v = 0; v < 5; ++v) {
+          int64_t g = v * p->S_v + b * p->S_b + c;
+          if (first)
+            out[g] = U0[g] - S[v * p->S_b + c];
+          else
+            out[g] = U0[g] + beta * ((X[g] - U0[g]) - S[v * p->S_b + c]);
+        }
+      }
+}
+
+static int run_stage(fxo_plan *p, double *X, const double *U0, double *out, const double *dx, double dt,
+                     double beta, int first) {
+  int rc = fxo_fill_guardcells(p, X); /* O1 on the stage input before every S(.) [A15] */
+  if (rc) return rc;
+  int fail = 0;
+#pragma omp parallel
+  {
+    double *W = (double *)malloc(sizeof(double) * 5 * (size_t)p->S_b);
+    double *S = (double *)malloc(sizeof(double) * 5 * (size_t)p->S_b);
+    int nmax = p->n[0] > p->n[1] ? p->n[0] : p->n[1];
+    if (p->n[2] > nmax) nmax = p->n[2];
+    double *Fl = (double *)malloc(sizeof(double) * 5 * (size_t)(nmax + 1));
+    if (!W || !S || !Fl) {
+#pragma omp atomic write
+      fail = 1;
+    } else {
+#pragma omp for schedule(dynamic, 4)
+      for (int64_t b = 0; b < p->nblocks; ++b) block_stage(p, X, U0, out, b, dx, dt, beta, first, W, S, Fl);
+    }
+    free(W);
+    free(S);
+    free(Fl);
+  }
+  return fail ? FXO_ERR_NOMEM : FXO_OK;
+}
+
+/* Forward-Euler stage U <- U - S(U) (used by tests to compose the SSP-RK schemes). */
+int fxo_euler_step(fxo_plan *p, double *U, const double *dx, double dt) {
+  if (!p || (!U && p->nblocks) || (!dx && p->nblocks)) return FXO_ERR_INVALID_ARG;
+  if (!p->neigh && p->nblocks > 0) return FXO_ERR_STATE;
+  size_t n = (size_t)p->S_v * 5;
+  double *U1 = (double *)malloc(sizeof(double) * (n ? n : 1));
+  if (!U1) return FXO_ERR_NOMEM;
+  int rc = run_stage(p, U, U, U1, dx, dt, 1.0, 1);
+  if (!rc) {
+    /* copy interiors back (guards of U keep the fill) */
+    for (int64_t b = 0; b < p->nblocks; ++b)
+      for (int k = p->gd[2]; k < p->gd[2] + p->n[2]; ++k)
+        for (int j = p->gd[1]; j < p->gd[1] + p->n[1]; ++j)
+          for (int i = p->gd[0]; i < p->gd[0] + p->n[0]; ++i)
+            for (int v = 0; v < 5; ++v) {
+              int64_t g = v * p->S_v + b * p->S_b + k * p->S_k + j * p->S_j + i;
+              U[g] = U1[g];
+            }
+  }
+  free(U1);
+  return rc;
+}
+
+/* O6: one SSP-RK step (Shu-Osher in increment form [A12]), in place on the interior of U. */
+int fxo_hydro_advance(fxo_plan *p, double *U, const double *dx, double dt) {
+  if (!p || (!U && p->nblocks) || (!dx && p->nblocks)) return FXO_ERR_INVALID_ARG;
+  if (!(dt > 0.0) || !isfinite(dt)) return FXO_ERR_INVALID_ARG;
+  if (!p->neigh && p->nblocks > 0) return FXO_ERR_STATE;
+  if (p->nblocks == 0) return FXO_OK;
+  size_t n = (size_t)p->S_v * 5;
+  double *U1 = (double *)malloc(sizeof(double) * n);
+  double *U2 = p->rk == 3 ? (double *)malloc(sizeof(double) * n) : NULL;
+  if (!U1 || (p->rk == 3 && !U2)) {
+    free(U1);
+    free(U2);
+    return FXO_ERR_NOMEM;
+  }
+  /* guards of U1/U2 are filled by run_stage before they are read; interiors are fully written */
+  memset(U1, 0, sizeof(double) * n);
+  if (U2) memset(U2, 0, sizeof(double) * n);
+  int rc = run_stage(p, U, U, U1, dx, dt, 1.0, 1); /* U1 = U0 - S(U0) */
+  if (!rc && p->rk == 2) {
+    rc = run_stage(p, U1, U, U, dx, dt, 0.5, 0); /* U = U0 + 1/2((U1-U0) - S(U1)) */
+  } else if (!rc) {
+    rc = run_stage(p, U1, U, U2, dx, dt, 0.25, 0); /* U2 = U0 + 1/4((U1-U0) - S(U1)) */
+    if (!rc) rc = run_stage(p, U2, U, U, dx, dt, 2.0 / 3.0, 0); /* U = U0 + 2/3((U2-U0) - S(U2)) */
+  }
+  free(U1);
+  free(U2);
+  return rc;
+}
+
+/* Face fluxes of direction dir from U (guards must already be filled) [A17]:
+ * F[v][b][k][j][i] with extents (nz, ny, nx) and n_dir + 1 along dir, i fastest. */
+int fxo_debug_compute_fluxes(fxo_plan *p, const double *U, int dir, double *F) {
+  if (!p || !U || !F || dir < 0 || dir > 2 || !p->active[dir]) return FXO_ERR_INVALID_ARG;
+  int e[3] = {p->n[0], p->n[1], p->n[2]};
+  e[dir] += 1;
+  int64_t FS_j = e[0], FS_k = (int64_t)e[0] * e[1], FS_b = FS_k * e[2], FS_v = FS_b * p->nblocks;
+  const int64_t stride[3] = {1, p->S_j, p->S_k};
+  int fail = 0;
+#pragma omp parallel
+  {
+    double *W = (double *)malloc(sizeof(double) * 5 * (size_t)p->S_b);
+    if (!W) {
+#pragma omp atomic write
+      fail = 1;
+    } else {
+#pragma omp for schedule(dynamic, 4)
+      for (int64_t b = 0; b < p->nblocks; ++b) {
+        block_prims(p, U, b, W);
+        for (int k = 0; k < e[2]; ++k)
+          for (int j = 0; j < e[1]; ++j)
+            for (int i = 0; i < e[0]; ++i) {
+              int c[3] = {i + p->gd[0], j + p->gd[1], k + p->gd[2]};
+              c[dir] -= 1; /* left cell of face f is padded cell g + f - 1 */
+              int64_t cL = c[2] * p->S_k + c[1] * p->S_j + c[0];
+              (void)stride;
+              double Ff[5];
+              unsigned hit = 0;
+              face_flux(p, W, p->S_b, cL, dir, Ff, &hit);
+              for (int v = 0; v < 5; ++v) F[v * FS_v + b * FS_b + k * FS_k + j * FS_j + i] = Ff[v];
+            }
+      }
+    }
+    free(W);
+  }
+  return fail ? FXO_ERR_NOMEM : FXO_OK;
+}
+
+/* ---------------------------------------------------------------- O7 dt */
+
+int fxo_hydro_compute_dt(fxo_plan *p, const double *U, const double *dx, double cfl, double *dt_out) {
+  if (!p || !dt_out || (!U && p->nblocks) || (!dx && p->nblocks)) return FXO_ERR_INVALID_ARG;
+  double best = INFINITY;
+#pragma omp parallel for schedule(static) reduction(min : best)
+  for (int64_t b = 0; b < p->nblocks; ++b)
+    for (int k = p->gd[2]; k < p->gd[2] + p->n[2]; ++k)
+      for (int j = p->gd[1]; j < p->gd[1] + p->n[1]; ++j)
+        for (int i = p->gd[0]; i < p->gd[0] + p->n[0]; ++i) {
+          int64_t c = b * p->S_b + k * p->S_k + j * p->S_j + i;
+          double Uz[5], W[5];
+          for (int v = 0; v < 5; ++v) Uz[v] = U[v * p->S_v + c];
+          unsigned hit = 0;
+          cons2prim(p, Uz, W, &hit);
+          double cs = sqrt(p->gamma * W[4] / W[0]);
+          for (int d = 0; d < 3; ++d) {
+            if (!p->active[d]) continue;
+            double s = fabs(W[1 + d]) + cs;
+            double t = dx[b * 3 + d] / s;
+            if (!(s > 0.0) || !isfinite(s)) hit |= FXO_STATUS_NONFINITE;
+            if (t < best) best = t;
+          }
+          count_hits(p, hit & FXO_STATUS_NONFINITE, 1);
+        }
+  *dt_out = cfl * best;
+  return FXO_OK;
+}

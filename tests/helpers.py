@@ -1,0 +1,144 @@
+"""Test helpers shared by the oracle pins and the GPU parity tests (no method arithmetic beyond the
+textbook exact Riemann solver used as an external pin)."""
+import math
+
+import numpy as np
+
+from oracle import fxoracle as fxo
+from paper_2208_11630_b200 import inputs
+
+
+def golden_rows(name):
+    import os
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", name)
+    rows = []
+    with open(path) as f:
+        for line in f:
+            if line.startswith("#") or not line.strip():
+                continue
+            rows.append(line.split())
+    return rows
+
+
+def oracle_plan_for(cfg, nblocks=None, order=inputs.ORDER_LEX, bc=None, nb=None, recon=None, riemann=None, rk=None):
+    """Oracle plan + topology for a config (regular tiling nb, default cfg.nb)."""
+    nb = tuple(nb or cfg.nb)
+    bc = bc or cfg.bc
+    code = {"periodic": fxo.TOPO_PERIODIC, "outflow": fxo.TOPO_OUTFLOW}[bc]
+    bcs = [code if cfg.block_dims[d] > 1 else fxo.TOPO_NONE for d in range(3)]
+    neigh, coords = fxo.topology_cartesian(nb, bcs, bcs, order)
+    plan = fxo.OraclePlan(cfg.block_dims, cfg.nguard, neigh.shape[0], cfg.gamma,
+                          cfg.recon if recon is None else recon, cfg.riemann if riemann is None else riemann,
+                          cfg.rk_order if rk is None else rk)
+    plan.set_topology(neigh)
+    return plan, neigh, coords
+
+
+def exact_riemann(WL, WR, gamma, xi):
+    """Exact solution of the 1-D Riemann problem for a perfect gas sampled at xi = x/t (array).
+    Textbook (Toro, Riemann Solvers..., ch. 4): Newton iteration on the star pressure.  States
+    (rho, u, p).  Returns rho, u, p arrays."""
+    rl, ul, pl = WL
+    rr, ur, pr = WR
+    g = gamma
+    cl, cr = math.sqrt(g * pl / rl), math.sqrt(g * pr / rr)
+
+    def f(p, rk, pk, ck):
+        if p > pk:
+            A, B = 2.0 / ((g + 1) * rk), (g - 1) / (g + 1) * pk
+            q = math.sqrt(A / (p + B))
+            return (p - pk) * q, q * (1 - 0.5 * (p - pk) / (p + B))
+        return 2 * ck / (g - 1) * ((p / pk) ** ((g - 1) / (2 * g)) - 1), 1 / (rk * ck) * (p / pk) ** (-(g + 1) / (2 * g))
+
+    p = 0.5 * (pl + pr)
+    for _ in range(100):
+        fl, dfl = f(p, rl, pl, cl)
+        fr, dfr = f(p, rr, pr, cr)
+        dp = (fl + fr + ur - ul) / (dfl + dfr)
+        p = max(p - dp, 1e-14)
+        if abs(dp) < 1e-15 * p:
+            break
+    fl, _ = f(p, rl, pl, cl)
+    fr, _ = f(p, rr, pr, cr)
+    us = 0.5 * (ul + ur) + 0.5 * (fr - fl)
+    ps = p
+    xi = np.asarray(xi, np.float64)
+    rho, u, pp = np.empty_like(xi), np.empty_like(xi), np.empty_like(xi)
+    gm = (g - 1) / (g + 1)
+    for n, s in enumerate(xi):
+        if s <= us:  # left of contact
+            if ps > pl:  # left shock
+                sl = ul - cl * math.sqrt((g + 1) / (2 * g) * ps / pl + (g - 1) / (2 * g))
+                if s <= sl:
+                    rho[n], u[n], pp[n] = rl, ul, pl
+                else:
+                    rho[n], u[n], pp[n] = rl * ((ps / pl + gm) / (gm * ps / pl + 1)), us, ps
+            else:
+                shl = ul - cl
+                csl = cl * (ps / pl) ** ((g - 1) / (2 * g))
+                stl = us - csl
+                if s <= shl:
+                    rho[n], u[n], pp[n] = rl, ul, pl
+                elif s >= stl:
+                    rho[n], u[n], pp[n] = rl * (ps / pl) ** (1 / g), us, ps
+                else:
+                    c = 2 / (g + 1) * (cl + (g - 1) / 2 * (ul - s))
+                    rho[n] = rl * (c / cl) ** (2 / (g - 1))
+                    u[n] = 2 / (g + 1) * (cl + (g - 1) / 2 * ul + s)
+                    pp[n] = pl * (c / cl) ** (2 * g / (g - 1))
+        else:
+            if ps > pr:
+                sr = ur + cr * math.sqrt((g + 1) / (2 * g) * ps / pr + (g - 1) / (2 * g))
+                if s >= sr:
+                    rho[n], u[n], pp[n] = rr, ur, pr
+                else:
+                    rho[n], u[n], pp[n] = rr * ((ps / pr + gm) / (gm * ps / pr + 1)), us, ps
+            else:
+                shr = ur + cr
+                csr = cr * (ps / pr) ** ((g - 1) / (2 * g))
+                str_ = us + csr
+                if s >= shr:
+                    rho[n], u[n], pp[n] = rr, ur, pr
+                elif s <= str_:
+                    rho[n], u[n], pp[n] = rr * (ps / pr) ** (1 / g), us, ps
+                else:
+                    c = 2 / (g + 1) * (cr - (g - 1) / 2 * (ur - s))
+                    rho[n] = rr * (c / cr) ** (2 / (g - 1))
+                    u[n] = 2 / (g + 1) * (-cr + (g - 1) / 2 * ur + s)
+                    pp[n] = pr * (c / cr) ** (2 * g / (g - 1))
+    return rho, u, pp, ps, us
+
+
+def run_to_time(plan, U, dx, cfl, t_end=None, steps=None):
+    """O8 driver: dt from compute_dt, last step clipped at t_end."""
+    t, n = 0.0, 0
+    while True:
+        if steps is not None and n >= steps:
+            break
+        if t_end is not None and t >= t_end:
+            break
+        dt = plan.compute_dt(U, dx, cfl)
+        if t_end is not None and t + dt > t_end:
+            dt = t_end - t
+        plan.advance(U, dx, dt)
+        t += dt
+        n += 1
+    return t, n
+
+
+def rel_err(cfg, got, ref):
+    """Max relative cellwise error over interior zones [A21]: |d rho|/rho, |d E|/E,
+    |d m_d|/(rho(|u|+c)), denominators from the reference state.  got/ref: interiors [5,...]."""
+    got = np.asarray(got)
+    ref = np.asarray(ref)
+    rho, E = ref[0], ref[4]
+    m2 = ref[1] ** 2 + ref[2] ** 2 + ref[3] ** 2
+    p = np.maximum((cfg.gamma - 1.0) * (E - 0.5 * m2 / rho), 1e-300)
+    scale_m = np.sqrt(m2) + rho * np.sqrt(cfg.gamma * p / rho)
+    e = np.abs(got[0] - rho) / rho
+    e = np.maximum(e, np.abs(got[4] - E) / E)
+    for d in (1, 2, 3):
+        e = np.maximum(e, np.abs(got[d] - ref[d]) / scale_m)
+    if not np.all(np.isfinite(got)):
+        return float("inf")
+    return float(e.max())

@@ -1,0 +1,264 @@
+"""Whole-scheme pins of the oracle (O5-O8): the hand-computed 1-D step, exact Sod solution, conservation,
+uniform-state preservation, mirror symmetry, RK composition, dt closed form.  CPU only.
+Citations: BASELINE.json north_star (list of invariants), SURVEY.md 8(c)-iii."""
+import math
+
+import numpy as np
+import pytest
+
+from oracle import fxoracle as fxo
+from paper_2208_11630_b200 import inputs
+from tests.helpers import exact_riemann, golden_rows, oracle_plan_for, rel_err, run_to_time
+
+
+def sod_setup(N=256, riemann=fxo.RIEMANN_HLLE, mirror=False):
+    cfg = inputs.config(1)
+    cfg.block_dims = (N, 1, 1)
+    plan, neigh, coords = oracle_plan_for(cfg, riemann=riemann)
+    U = inputs.embed(cfg, inputs.block_interiors(cfg, coords)).numpy()
+    if mirror:
+        U = U[..., ::-1].copy()
+        U[1] *= -1
+    return cfg, plan, U, inputs.dx_array(cfg)
+
+
+# ------------------------------------------------------------ hand-computed single step
+def test_sod_single_step_golden():
+    rows = golden_rows("sod_single_step.txt")
+    dt_gold = float([r for r in rows if r[0] == "dt"][0][1])
+    assert dt_gold == pytest.approx(0.0026411070460266143, rel=1e-15)  # value printed in SURVEY.md
+    for name, solver in (("hlle", fxo.RIEMANN_HLLE), ("hllc", fxo.RIEMANN_HLLC)):
+        cfg, plan, U, dx = sod_setup(256, solver)
+        U0 = U.copy()
+        dt = plan.compute_dt(U, dx, cfg.cfl)
+        assert dt == pytest.approx(dt_gold, rel=1e-15)
+        # stage 1 alone
+        U1 = U0.copy()
+        plan.euler_step(U1, dx, dt)
+        plan.advance(U, dx, dt)
+        g = 4
+        for stage, arr in ((1, U1), (2, U)):
+            changed = [i for i in range(256) if any(arr[v, 0, 0, 0, g + i] != U0[v, 0, 0, 0, g + i] for v in (0, 1, 4))]
+            gold = [r for r in rows if r[0] == name and int(r[1]) == stage]
+            assert changed == [int(r[2]) for r in gold]
+            for r in gold:
+                z = int(r[2])
+                got = [arr[v, 0, 0, 0, g + z] for v in (0, 1, 4)]
+                np.testing.assert_allclose(got, [float(x) for x in r[3:6]], rtol=5e-15)
+        # conservation of the step: sum d rho = sum d E = 0; sum d m * dx/dt = p_L - p_R = 0.9
+        d = plan.interior(U) - plan.interior(U0)
+        assert abs(math.fsum(d[0].ravel())) < 1e-15 and abs(math.fsum(d[4].ravel())) < 4e-15
+        assert math.fsum(d[1].ravel()) * (1 / 256) / dt == pytest.approx(0.9, rel=1e-13)
+        assert np.all(U[2] [~np.isnan(U[2])] == 0) and np.all(U[3][~np.isnan(U[3])] == 0)
+
+
+# ------------------------------------------------------------ exact Riemann solution
+def test_exact_solver_reproduces_published_sod_star_values():
+    # Toro, table 4.1-style values quoted in SURVEY.md 8(c)-iii 'whole scheme, config 1'
+    rho, u, p, ps, us = exact_riemann((1, 0, 1), (0.125, 0, 0.1), 1.4, np.array([0.0, 0.8 / 0.2 - 2.5, 1.6]))
+    assert ps == pytest.approx(0.303130178051, rel=1e-10) and us == pytest.approx(0.927452620049, rel=1e-10)
+    rho2, _, _, _, _ = exact_riemann((1, 0, 1), (0.125, 0, 0.1), 1.4, np.array([0.5, 1.0]))
+    assert rho2[0] == pytest.approx(0.426319428178, rel=1e-10) and rho2[1] == pytest.approx(0.265573711705, rel=1e-10)
+
+
+def sod_l1(N):
+    cfg, plan, U, dx = sod_setup(N)
+    t, n = run_to_time(plan, U, dx, cfg.cfl, t_end=0.2)
+    assert t == 0.2
+    x = (np.arange(N) + 0.5) / N
+    rho_ex, _, _, _, _ = exact_riemann((1, 0, 1), (0.125, 0, 0.1), 1.4, (x - 0.5) / 0.2)
+    f, counts = plan.status()
+    assert f == 0  # no floors, nothing non-finite in config 1 [A7]
+    return float(np.sum(np.abs(plan.interior(U)[0, 0, 0, 0] - rho_ex)) / N), n
+
+
+def test_sod_converges_to_exact_solution():
+    Ns = [64, 128, 256, 512, 1024]
+    errs = [sod_l1(N)[0] for N in Ns]
+    assert all(errs[i + 1] < errs[i] for i in range(len(errs) - 1))
+    order = -np.polyfit(np.log(Ns[1:]), np.log(errs[1:]), 1)[0]
+    # a TVD scheme smears the contact like N^(-2/3): fitted order ~0.84, accept >= 0.8 [A23]
+    assert order >= 0.8, (errs, order)
+    assert errs[2] < 5e-3  # N = 256
+
+
+def test_sod_mirror_symmetry_bitwise():
+    for solver in (fxo.RIEMANN_HLLE, fxo.RIEMANN_HLLC):
+        cfg, plan, U, dx = sod_setup(128, solver)
+        _, planm, Um, _ = sod_setup(128, solver, mirror=True)
+        for _ in range(20):
+            dt = plan.compute_dt(U, dx, 0.8)
+            assert dt == planm.compute_dt(Um, dx, 0.8)
+            plan.advance(U, dx, dt)
+            planm.advance(Um, dx, dt)
+        a, b = plan.interior(U), planm.interior(Um)[..., ::-1]
+        assert np.array_equal(a[0], b[0]) and np.array_equal(a[4], b[4]) and np.array_equal(a[1], -b[1])
+
+
+# ------------------------------------------------------------ uniform state, conservation
+@pytest.mark.parametrize("recon,riemann,rk", [(0, 0, 2), (0, 1, 3), (1, 0, 3), (1, 1, 2)])
+def test_uniform_state_preserved_bitwise(recon, riemann, rk):
+    cfg = inputs.config(3, nb=(2, 1, 2))
+    cfg.block_dims = (6, 5, 4)
+    for bc in ("periodic", "outflow"):
+        plan, neigh, coords = oracle_plan_for(cfg, bc=bc, recon=recon, riemann=riemann, rk=rk)
+        W = (1.3, 0.7, -0.4, 0.2, 2.2)
+        E = W[4] / (cfg.gamma - 1) + 0.5 * W[0] * (W[1] ** 2 + W[2] ** 2 + W[3] ** 2)
+        U = np.full(plan.shape, np.nan)
+        for v, val in enumerate((W[0], W[0] * W[1], W[0] * W[2], W[0] * W[3], E)):
+            plan.interior(U)[v] = val
+        U0 = plan.interior(U).copy()
+        dx = np.tile([0.1, 0.2, 0.15], (plan.nblocks, 1))
+        for _ in range(10):
+            plan.advance(U, dx, 0.01)
+        assert np.array_equal(plan.interior(U), U0)
+
+
+def totals(plan, U):
+    Ui = plan.interior(U)
+    return np.array([math.fsum(Ui[v].ravel()) for v in range(5)])
+
+
+def scale_totals(cfg, plan, U):
+    Ui = plan.interior(U)
+    rho, E = Ui[0], Ui[4]
+    m2 = Ui[1] ** 2 + Ui[2] ** 2 + Ui[3] ** 2
+    p = np.maximum((cfg.gamma - 1) * (E - 0.5 * m2 / rho), 0)
+    sm = math.fsum((np.sqrt(m2) + rho * np.sqrt(cfg.gamma * p / rho)).ravel())
+    return np.array([math.fsum(rho.ravel()), sm, sm, sm, math.fsum(E.ravel())])
+
+
+@pytest.mark.parametrize("number,nb,steps", [(2, (8, 8, 1), 100), (3, (3, 3, 3), 20), (4, (2, 2, 2), 6), (5, (2, 3, 2), 10)])
+def test_conservation_on_periodic_domains(number, nb, steps):
+    cfg = inputs.config(number, nb=nb)
+    plan, neigh, coords = oracle_plan_for(cfg)
+    U = inputs.embed(cfg, inputs.block_interiors(cfg, coords)).numpy()
+    dx = inputs.dx_array(cfg)
+    T0, S0 = totals(plan, U), scale_totals(cfg, plan, U)
+    run_to_time(plan, U, dx, cfg.cfl, steps=steps)
+    T1 = totals(plan, U)
+    assert np.all(np.isfinite(T1))
+    assert np.max(np.abs(T1 - T0) / S0) <= 1e-13, (T1 - T0) / S0   # [NS] 1e-13 relative, metric [A22]
+    f, counts = plan.status()
+    assert not (f & fxo.STATUS_NONFINITE)
+    if number in (2, 4):
+        assert f == 0  # no floor hits, no WENO fallback [A6, A7]
+
+
+def test_sedov_reflection_symmetry():
+    cfg = inputs.config(3, nb=(2, 2, 2))
+    plan, neigh, coords = oracle_plan_for(cfg)
+    U = inputs.embed(cfg, inputs.block_interiors(cfg, coords)).numpy()
+    dx = inputs.dx_array(cfg)
+    run_to_time(plan, U, dx, cfg.cfl, steps=10)
+    # assemble the global field
+    n = 16
+    G = np.empty((5, 32, 32, 32))
+    Ui = plan.interior(U)
+    for b, (bx, by, bz) in enumerate(coords):
+        G[:, bz * n:(bz + 1) * n, by * n:(by + 1) * n, bx * n:(bx + 1) * n] = Ui[:, b]
+    assert G[0].max() > 1.2  # the blast has done something
+    for axis, mom in ((3, 1), (2, 2), (1, 3)):
+        R = np.flip(G, axis=axis).copy()
+        R[mom] *= -1
+        scale = np.abs(G).max(axis=(1, 2, 3), keepdims=True)
+        scale[1:4] = scale[1:4].max()
+        assert np.max(np.abs(R - G) / scale) <= 1e-12
+
+
+# ------------------------------------------------------------ RK composition, dt
+def test_rk_is_the_shu_osher_composition_of_euler_steps():
+    cfg = inputs.config(5, nb=(2, 2, 2))
+    dx = inputs.dx_array(cfg)
+    for rk in (2, 3):
+        plan, neigh, coords = oracle_plan_for(cfg, rk=rk)
+        U0 = inputs.embed(cfg, inputs.block_interiors(cfg, coords)).numpy()
+        dt = plan.compute_dt(U0, dx, 0.3)
+        U = U0.copy()
+        plan.advance(U, dx, dt)
+        E1 = U0.copy()
+        plan.euler_step(E1, dx, dt)
+        E2 = E1.copy()
+        plan.euler_step(E2, dx, dt)
+        i = plan.interior
+        if rk == 2:
+            ref = 0.5 * i(U0) + 0.5 * i(E2)
+        else:
+            U2 = U0.copy()
+            i(U2)[...] = 0.75 * i(U0) + 0.25 * i(E2)
+            plan.euler_step(U2, dx, dt)
+            ref = i(U0) / 3.0 + (2.0 / 3.0) * i(U2)
+        assert rel_err(cfg, i(U), ref) <= 1e-14
+
+
+def test_dt_closed_form_and_brute_force():
+    cfg = inputs.config(3, nb=(2, 1, 1))
+    cfg.block_dims = (5, 4, 4)
+    plan, neigh, coords = oracle_plan_for(cfg, bc="outflow")
+    W = (0.5, 0.3, -1.1, 0.4, 0.8)
+    E = W[4] / 0.4 + 0.5 * W[0] * (W[1] ** 2 + W[2] ** 2 + W[3] ** 2)
+    U = np.full(plan.shape, np.nan)
+    for v, val in enumerate((W[0], W[0] * W[1], W[0] * W[2], W[0] * W[3], E)):
+        plan.interior(U)[v] = val
+    dx = np.tile([0.1, 0.1, 0.1], (2, 1))
+    c = math.sqrt(1.4 * 0.8 / 0.5)
+    assert plan.compute_dt(U, dx, 0.3) == pytest.approx(0.3 * 0.1 / (1.1 + c), rel=1e-14)
+    # anisotropic, per-block dx: brute force over zones in python
+    rng = np.random.default_rng(11)
+    Ui = plan.interior(U)
+    Ui[0] = rng.uniform(0.5, 2, Ui[0].shape)
+    for v in (1, 2, 3):
+        Ui[v] = rng.normal(size=Ui[0].shape)
+    Ui[4] = 3 + rng.uniform(0, 1, Ui[0].shape)
+    dx = np.array([[0.1, 0.05, 0.2], [0.02, 0.3, 0.1]])
+    best = math.inf
+    for b in range(2):
+        for idx in np.ndindex(Ui[0, b].shape):
+            rho = Ui[0, b][idx]
+            u = [Ui[v, b][idx] / rho for v in (1, 2, 3)]
+            p = 0.4 * (Ui[4, b][idx] - 0.5 * rho * sum(x * x for x in u))
+            cs = math.sqrt(1.4 * p / rho)
+            for d in range(3):
+                best = min(best, dx[b, d] / (abs(u[d]) + cs))
+    assert plan.compute_dt(U, dx, 0.25) == pytest.approx(0.25 * best, rel=1e-14)
+    # 2-D plan ignores the inactive dimension's dx
+    cfg2 = inputs.config(2, nb=(2, 2, 1))
+    plan2, _, coords2 = oracle_plan_for(cfg2)
+    U2 = inputs.embed(cfg2, inputs.block_interiors(cfg2, coords2)).numpy()
+    dx2 = inputs.dx_array(cfg2)
+    dxz = dx2.copy()
+    dxz[:, 2] = 1e-9
+    assert plan2.compute_dt(U2, dx2, 0.4) == plan2.compute_dt(U2, dxz, 0.4)
+
+
+def test_block_permutation_invariance_bitwise():
+    cfg = inputs.config(5, nb=(2, 2, 2))
+    dx = inputs.dx_array(cfg)
+    plan, neigh, coords = oracle_plan_for(cfg)
+    U = inputs.embed(cfg, inputs.block_interiors(cfg, coords)).numpy()
+    perm = np.random.default_rng(3).permutation(8)
+    inv = np.argsort(perm)
+    neigh_p = neigh[perm].copy()
+    neigh_p[neigh_p >= 0] = inv[neigh_p[neigh_p >= 0]]
+    plan_p = fxo.OraclePlan(cfg.block_dims, cfg.nguard, 8, cfg.gamma, cfg.recon, cfg.riemann, cfg.rk_order)
+    plan_p.set_topology(neigh_p)
+    Up = np.ascontiguousarray(U[:, perm])
+    for _ in range(2):
+        plan.advance(U, dx, 2e-4)
+        plan_p.advance(Up, dx, 2e-4)
+    assert np.array_equal(plan.interior(U)[:, perm], plan_p.interior(Up))
+
+
+def test_advance_ignores_guard_contents_and_rejects_bad_dt():
+    cfg = inputs.config(2, nb=(2, 2, 1))
+    plan, neigh, coords = oracle_plan_for(cfg)
+    Ui = inputs.block_interiors(cfg, coords)
+    A = inputs.embed(cfg, Ui, float("nan")).numpy()
+    B = inputs.embed(cfg, Ui, 123.0).numpy()
+    dx = inputs.dx_array(cfg)
+    plan.advance(A, dx, 1e-3)
+    plan.advance(B, dx, 1e-3)
+    assert np.array_equal(plan.interior(A), plan.interior(B))
+    for bad in (0.0, -1.0, float("nan"), float("inf")):
+        with pytest.raises(ValueError):
+            plan.advance(A, dx, bad)
