@@ -209,7 +209,7 @@ def test_dt_closed_form_and_brute_force():
     Ui[0] = rng.uniform(0.5, 2, Ui[0].shape)
     for v in (1, 2, 3):
         Ui[v] = rng.normal(size=Ui[0].shape)
-    Ui[4] = 3 + rng.uniform(0, 1, Ui[0].shape)
+    Ui[4] = 30 + rng.uniform(0, 1, Ui[0].shape)
     dx = np.array([[0.1, 0.05, 0.2], [0.02, 0.3, 0.1]])
     best = math.inf
     for b in range(2):
