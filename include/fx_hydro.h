@@ -1,0 +1,169 @@
+/*
+ * fx_hydro.h -- C ABI of libfxhydro: the batched block Euler update on one B200 (sm_100a).
+ *
+ * The operation: the unsplit finite-volume update of the compressible Euler equations over a batch
+ * of fixed-size mesh blocks with guard cells, the block-by-block hot path of a Flash-X style run
+ * [PAPER.md L69 section 2 "block-by-block update"; L71 "explicit methods ... strong shocks"; L103
+ * section 2.2 Spark: "second- or third-order strong stability preserving (SSP) Runge-Kutta"; L105
+ * "perfect-gas EOS"].  PAPER.md prints no formula; the discretisation is the one BASELINE.json's
+ * north_star names, in the readings DESIGN.md lists (tags O1..O8, A1..A27 of SURVEY.md 8(c)).
+ *
+ * Conventions
+ *  - All functions return int: FX_OK (0) or a negative FX_ERR_*; nothing aborts or throws across the
+ *    ABI.  fx_last_error() returns a thread-local message for the last failure on this thread.
+ *  - "dev" pointers are device (HBM) pointers, "host" pointers are host pointers.  Every device
+ *    buffer is CALLER-OWNED (allocate it with PyTorch or cudaMalloc); the library never allocates
+ *    device memory.  `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).
+ *  - Unless stated, a call only enqueues work on `stream` and returns without synchronising.
+ *  - State layout [a0]: U[v][b][k][j][i], fp64, SoA with one contiguous slab per variable, i fastest:
+ *        element(v,b,k,j,i) = v*S_v + b*S_b + k*S_k + j*S_j + i        (int64 arithmetic)
+ *    v in (rho, m_x, m_y, m_z, E); padded extents np[d] = n[d] + 2*gd[d], gd[d] = nguard if n[d] > 1
+ *    else 0 (a dimension of extent 1 is inactive: no guards, no sweep, no dt contribution [A26]).
+ *    Interior zone (i,j,k) has gd[0] <= i < gd[0]+n[0] etc.  Query strides with fx_hydro_plan_layout.
+ */
+#ifndef FX_HYDRO_H
+#define FX_HYDRO_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define FX_OK 0
+#define FX_ERR_INVALID_ARG (-1)
+#define FX_ERR_STATE (-2)       /* call order: topology or workspace not set */
+#define FX_ERR_UNSUPPORTED (-3) /* coarse/fine neighbour relation, nvars != 5, ... */
+#define FX_ERR_WORKSPACE (-4)   /* workspace missing, too small or not 256-byte aligned */
+#define FX_ERR_CUDA (-5)        /* a CUDA runtime call or launch failed; see fx_last_error() */
+
+enum { FX_RECON_PLM_MINMOD = 0, FX_RECON_WENO5 = 1 };
+enum { FX_RIEMANN_HLLE = 0, FX_RIEMANN_HLLC = 1 };
+enum { FX_BC_OUTFLOW = -1, FX_BC_NONE = -2 };                        /* neighbour-table codes */
+enum { FX_TOPO_PERIODIC = 0, FX_TOPO_OUTFLOW = 1, FX_TOPO_NONE = 2 }; /* fx_topology_cartesian bc codes */
+enum { FX_ORDER_LEX = 0, FX_ORDER_MORTON = 1 };
+enum {
+  FX_OPT_RHO_FLOOR = 0, /* primitive density floor, default 1e-12 [A7] */
+  FX_OPT_P_FLOOR = 1,   /* primitive pressure floor, default 1e-12 [A7] */
+  FX_OPT_WENO_EPS = 2,  /* WENO5-JS epsilon, default 1e-6 [A5] */
+  FX_OPT_WAVESPEED = 3, /* 0 = Einfeldt (default), 1 = Davis [A8] */
+  FX_OPT_PATH = 4       /* 0 = auto (fused stage kernel when the block shape allows), 1 = generic */
+};
+enum {
+  FX_STATUS_NONFINITE = 1u,
+  FX_STATUS_RHO_FLOOR = 2u,
+  FX_STATUS_P_FLOOR = 4u,
+  FX_STATUS_WENO_FALLBACK = 8u
+};
+
+typedef struct fx_hydro_plan fx_hydro_plan;
+
+typedef struct fx_layout {
+  int32_t np[3];                 /* padded extents (x, y, z) */
+  int32_t gd[3];                 /* guard depth per dimension */
+  int64_t S_j, S_k, S_b, S_v;    /* element strides */
+  int64_t bytes_per_state;       /* nvars * S_v * 8 */
+} fx_layout;
+
+/* Thread-local text of the last error on the calling thread ("" if none). */
+const char *fx_last_error(void);
+
+/* Plan: a host object owned by the library, freed by fx_hydro_plan_destroy.
+ * block_dims = interior zones (nx, ny, nz) per block; nvars must be 5 (rho, m_x, m_y, m_z, E) [A1];
+ * recon FX_RECON_*; riemann FX_RIEMANN_*; rk_order 2 or 3 (SSP-RK).
+ * FX_ERR_INVALID_ARG: a dim < 1; no active dim; nguard < 2 (PLM) or < 3 (WENO5); nguard > an active
+ * block dim; gamma <= 1; nblocks < 0; unknown enum.  FX_ERR_UNSUPPORTED: nvars != 5. */
+int fx_hydro_plan_create(fx_hydro_plan **out, const int block_dims[3], int nguard, int nvars, int64_t nblocks,
+                         double gamma, int recon, int riemann, int rk_order);
+int fx_hydro_plan_destroy(fx_hydro_plan *plan);
+
+/* Strides and padded extents of the state array (pure). */
+int fx_hydro_plan_layout(const fx_hydro_plan *plan, fx_layout *out);
+
+/* Options; must be set before the first advance.  Unknown key / bad value -> FX_ERR_INVALID_ARG. */
+int fx_hydro_plan_set_option(fx_hydro_plan *plan, int key, double value);
+
+/* Workspace (device, caller-owned, 256-byte aligned): (rk_order - 1) state copies for the RK stages
+ * + a 256-byte scratch block (dt reduction word, status word and counters).  set_workspace
+ * initialises the scratch block and synchronises the device once. */
+size_t fx_hydro_plan_workspace_bytes(const fx_hydro_plan *plan);
+int fx_hydro_plan_set_workspace(fx_hydro_plan *plan, void *workspace_dev, size_t bytes);
+
+/* Topology: neigh_dev is int32 [nblocks][6] in the order -x,+x,-y,+y,-z,+z; an entry >= 0 is the id of
+ * the same-level neighbour block (periodic boundaries are expressed by wrapped ids), FX_BC_OUTFLOW a
+ * zero-gradient physical boundary; entries of inactive dimensions are ignored.  The table stays
+ * caller-owned and must outlive the plan's use of it.  The call copies it to the host once to validate
+ * (synchronises).  Any other negative entry in an active dimension is a coarse/fine relation:
+ * FX_ERR_UNSUPPORTED [A18]. */
+int fx_hydro_plan_set_topology(fx_hydro_plan *plan, const int32_t *neigh_dev);
+
+/* Host helper: neighbour table and block coordinates of a regular nb[0] x nb[1] x nb[2] tiling.
+ * bc_lo/bc_hi per dimension: FX_TOPO_*; order FX_ORDER_LEX (x fastest) or FX_ORDER_MORTON.
+ * neigh_out_host int32 [nblocks][6]; coords_out_host int32 [nblocks][3] (may be NULL). */
+int fx_topology_cartesian(const int nb[3], const int bc_lo[3], const int bc_hi[3], int order,
+                          int32_t *neigh_out_host, int32_t *coords_out_host);
+
+/* a1 Guard-cell fill [O1, A14]: every guard zone (faces, edges, corners) of every block of U_dev, in
+ * place, gets the 5 variables of the interior zone it images: hops z, then y, then x through the
+ * neighbour table; outflow clamps to the nearest interior index.  Needs the topology (FX_ERR_STATE). */
+int fx_fill_guardcells(fx_hydro_plan *plan, double *U_dev, void *stream);
+
+/* Test hook: for blocks [block_begin, block_begin+block_count), the flat variable-0 element index each
+ * padded zone is filled from (itself for interior zones): src_dev int64 [block_count][np2][np1][np0]. */
+int fx_guardcell_index_map(fx_hydro_plan *plan, int64_t block_begin, int64_t block_count, int64_t *src_dev,
+                           void *stream);
+
+/* a7 CFL time step [O7, A13]: *dt_out_dev = cfl * min over blocks, interior zones and active d of
+ * dx[b][d] / (|u_d| + c).  dx_dev is double [nblocks][3].  Reads interior zones only; writes +inf when
+ * nblocks == 0.  A non-finite or non-positive signal speed sets FX_STATUS_NONFINITE.  Needs the
+ * workspace (FX_ERR_STATE). */
+int fx_hydro_compute_dt(fx_hydro_plan *plan, const double *U_dev, const double *dx_dev, double cfl,
+                        double *dt_out_dev, void *stream);
+
+/* a1..a6 One SSP-RK step [O5, O6], all stages, in place on the INTERIOR zones of U_dev:
+ *   U1 = U0 - S(U0);  RK2: U = U0 + 1/2((U1-U0) - S(U1));
+ *   RK3: U2 = U0 + 1/4((U1-U0) - S(U1)); U = U0 + 2/3((U2-U0) - S(U2));
+ *   S(X) = sum_{d active} dt/dx[b][d] (F_{d,+} - F_{d,-}), fluxes from cons->prim (gamma law),
+ *   PLM-minmod or WENO5-JS on primitives, HLLE or HLLC.
+ * Guard zones of U_dev need not be valid on entry (the call fills or gathers halos of each stage input
+ * itself) and are unspecified on exit [A15].  dt <= 0 or non-finite -> FX_ERR_INVALID_ARG.  Needs
+ * topology and workspace (FX_ERR_STATE). */
+int fx_hydro_advance(fx_hydro_plan *plan, double *U_dev, const double *dx_dev, double dt, void *stream);
+
+/* End-to-end variant with HOST buffers: copies U_host (whole padded state) and dx_host to the device
+ * staging buffers U_stage_dev / dx_stage_dev (caller-owned, bytes_per_state and nblocks*24 bytes), runs
+ * `nsteps` steps of { compute_dt with `cfl`; advance } entirely on the device (dt never visits the
+ * host), copies the state back into U_host and the last dt into *dt_last_host, and synchronises
+ * `stream`.  Host buffers should be pinned for full PCIe speed. */
+int fx_hydro_advance_host(fx_hydro_plan *plan, double *U_host, const double *dx_host, double cfl, int nsteps,
+                          double *U_stage_dev, double *dx_stage_dev, double *dt_last_host, void *stream);
+
+/* As fx_hydro_advance, but dt is read on the device from dt_dev (e.g. written by fx_hydro_compute_dt
+ * on the same stream): no host round trip per step. */
+int fx_hydro_advance_devdt(fx_hydro_plan *plan, double *U_dev, const double *dx_dev, const double *dt_dev,
+                           void *stream);
+
+/* Status word and counters {non-finite, rho floor, p floor, WENO fallback} accumulated by all kernels
+ * since the last reset; synchronises `stream`.  counts_host may be NULL. */
+int fx_hydro_status(fx_hydro_plan *plan, uint32_t *flags_host, unsigned long long counts_host[4], void *stream);
+int fx_hydro_status_reset(fx_hydro_plan *plan, void *stream);
+
+/* Debug / per-kernel parity: face fluxes of direction dir (0,1,2) from U_dev whose guard zones are
+ * already filled [A17]: F_dev[v][b][k][j][i], extents (nz, ny, nx) with n_dir + 1 along dir, i fastest;
+ * face f lies between padded cells gd+f-1 and gd+f.  Not on the timed path. */
+int fx_debug_compute_fluxes(fx_hydro_plan *plan, const double *U_dev, int dir, double *F_dev, void *stream);
+
+/* Which stage kernel fx_hydro_advance will use for this plan: 0 generic (guard fill + zone kernel),
+ * 1 fused (halo gathered from neighbour interiors inside the stage kernel). */
+int fx_hydro_plan_path(const fx_hydro_plan *plan);
+
+/* Measurement aid for the fp64 roofline: runs a dependent-chain-free DFMA kernel (iters FMAs per
+ * thread on 8 independent accumulators) over the whole device; the caller times it with events.
+ * out_dev: double [1] sink.  Returns the number of FMAs issued in *fma_count_host. */
+int fx_probe_fp64_fma(int iters, double *out_dev, unsigned long long *fma_count_host, void *stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FX_HYDRO_H */

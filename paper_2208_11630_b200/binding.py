@@ -1,0 +1,228 @@
+"""Thin ctypes binding of libfxhydro.so (include/fx_hydro.h): argument marshalling only.
+
+Every step of the path runs inside the CUDA library; PyTorch supplies device memory and streams.  There is
+no CPU fallback: a missing library or a failing call raises.  Names mirror the C ABI.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libfxhydro.so")
+
+OK, ERR_INVALID_ARG, ERR_STATE, ERR_UNSUPPORTED, ERR_WORKSPACE, ERR_CUDA = 0, -1, -2, -3, -4, -5
+RECON_PLM_MINMOD, RECON_WENO5 = 0, 1
+RIEMANN_HLLE, RIEMANN_HLLC = 0, 1
+BC_OUTFLOW, BC_NONE = -1, -2
+TOPO_PERIODIC, TOPO_OUTFLOW, TOPO_NONE = 0, 1, 2
+ORDER_LEX, ORDER_MORTON = 0, 1
+OPT_RHO_FLOOR, OPT_P_FLOOR, OPT_WENO_EPS, OPT_WAVESPEED, OPT_PATH = 0, 1, 2, 3, 4
+STATUS_NONFINITE, STATUS_RHO_FLOOR, STATUS_P_FLOOR, STATUS_WENO_FALLBACK = 1, 2, 4, 8
+
+EXPORTS = [
+    "fx_last_error", "fx_hydro_plan_create", "fx_hydro_plan_destroy", "fx_hydro_plan_layout",
+    "fx_hydro_plan_set_option", "fx_hydro_plan_workspace_bytes", "fx_hydro_plan_set_workspace",
+    "fx_hydro_plan_set_topology", "fx_topology_cartesian", "fx_fill_guardcells", "fx_guardcell_index_map",
+    "fx_hydro_compute_dt", "fx_hydro_advance", "fx_hydro_advance_host", "fx_hydro_advance_devdt",
+    "fx_hydro_status", "fx_hydro_status_reset", "fx_debug_compute_fluxes", "fx_hydro_plan_path",
+    "fx_probe_fp64_fma",
+]
+
+
+class FxError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"libfxhydro error {code}: {msg}")
+        self.code = code
+
+
+class Layout(C.Structure):
+    _fields_ = [("np", C.c_int32 * 3), ("gd", C.c_int32 * 3), ("S_j", C.c_int64), ("S_k", C.c_int64),
+                ("S_b", C.c_int64), ("S_v", C.c_int64), ("bytes_per_state", C.c_int64)]
+
+
+_lib = None
+
+
+def lib():
+    """Load libfxhydro.so; raises if it has not been built (no fallback)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} is missing: run `python -m paper_2208_11630_b200.build` "
+                              "(the CUDA library is the only implementation; there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        vp, i3 = C.c_void_p, C.POINTER(C.c_int)
+        L.fx_last_error.restype = C.c_char_p
+        L.fx_hydro_plan_create.argtypes = [C.POINTER(vp), i3, C.c_int, C.c_int, C.c_int64, C.c_double, C.c_int,
+                                           C.c_int, C.c_int]
+        L.fx_hydro_plan_destroy.argtypes = [vp]
+        L.fx_hydro_plan_layout.argtypes = [vp, C.POINTER(Layout)]
+        L.fx_hydro_plan_set_option.argtypes = [vp, C.c_int, C.c_double]
+        L.fx_hydro_plan_workspace_bytes.argtypes = [vp]
+        L.fx_hydro_plan_workspace_bytes.restype = C.c_size_t
+        L.fx_hydro_plan_set_workspace.argtypes = [vp, vp, C.c_size_t]
+        L.fx_hydro_plan_set_topology.argtypes = [vp, vp]
+        L.fx_topology_cartesian.argtypes = [i3, i3, i3, C.c_int, vp, vp]
+        L.fx_fill_guardcells.argtypes = [vp, vp, vp]
+        L.fx_guardcell_index_map.argtypes = [vp, C.c_int64, C.c_int64, vp, vp]
+        L.fx_hydro_compute_dt.argtypes = [vp, vp, vp, C.c_double, vp, vp]
+        L.fx_hydro_advance.argtypes = [vp, vp, vp, C.c_double, vp]
+        L.fx_hydro_advance_devdt.argtypes = [vp, vp, vp, vp, vp]
+        L.fx_hydro_advance_host.argtypes = [vp, vp, vp, C.c_double, C.c_int, vp, vp, vp, vp]
+        L.fx_hydro_status.argtypes = [vp, C.POINTER(C.c_uint32), C.POINTER(C.c_ulonglong), vp]
+        L.fx_hydro_status_reset.argtypes = [vp, vp]
+        L.fx_debug_compute_fluxes.argtypes = [vp, vp, C.c_int, vp, vp]
+        L.fx_hydro_plan_path.argtypes = [vp]
+        L.fx_probe_fp64_fma.argtypes = [C.c_int, vp, C.POINTER(C.c_ulonglong), vp]
+        _lib = L
+    return _lib
+
+
+def _check(rc):
+    if rc != 0:
+        raise FxError(rc, lib().fx_last_error().decode())
+
+
+def _stream(stream=None):
+    s = torch.cuda.current_stream() if stream is None else stream
+    return C.c_void_p(s.cuda_stream)
+
+
+def _dev(t: torch.Tensor, dtype):
+    assert t.is_cuda and t.dtype == dtype and t.is_contiguous(), (t.device, t.dtype, t.is_contiguous())
+    return C.c_void_p(t.data_ptr())
+
+
+def fx_topology_cartesian(nb, bc_lo, bc_hi, order=ORDER_LEX):
+    """Host helper: (neigh int32 [nblocks,6], coords int32 [nblocks,3]) numpy arrays."""
+    n = int(nb[0]) * int(nb[1]) * int(nb[2])
+    neigh = np.empty((max(n, 0), 6), np.int32)
+    coords = np.empty((max(n, 0), 3), np.int32)
+    i3 = C.c_int * 3
+    _check(lib().fx_topology_cartesian(i3(*nb), i3(*bc_lo), i3(*bc_hi), order, C.c_void_p(neigh.ctypes.data),
+                                       C.c_void_p(coords.ctypes.data)))
+    return neigh, coords
+
+
+class HydroPlan:
+    """fx_hydro_plan with its caller-owned device buffers (workspace, neighbour table) held as torch tensors."""
+
+    def __init__(self, block_dims, nguard, nblocks, gamma, recon, riemann, rk_order, nvars=5, device="cuda"):
+        self._h = C.c_void_p()
+        _check(lib().fx_hydro_plan_create(C.byref(self._h), (C.c_int * 3)(*block_dims), nguard, nvars, nblocks, gamma,
+                                          recon, riemann, rk_order))
+        L = Layout()
+        _check(lib().fx_hydro_plan_layout(self._h, C.byref(L)))
+        self.block_dims = tuple(int(d) for d in block_dims)
+        self.nblocks, self.nvars, self.gamma, self.rk_order = int(nblocks), nvars, gamma, rk_order
+        self.np, self.gd = tuple(L.np), tuple(L.gd)
+        self.S_j, self.S_k, self.S_b, self.S_v = L.S_j, L.S_k, L.S_b, L.S_v
+        self.bytes_per_state = L.bytes_per_state
+        self.device = torch.device(device)
+        self._ws = None
+        self._neigh = None
+        self._dt = None
+
+    def __del__(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            lib().fx_hydro_plan_destroy(self._h)
+            self._h = C.c_void_p()
+
+    @property
+    def shape(self):
+        return (self.nvars, self.nblocks, self.np[2], self.np[1], self.np[0])
+
+    @property
+    def path(self):
+        return lib().fx_hydro_plan_path(self._h)
+
+    def fx_hydro_plan_set_option(self, key, value):
+        _check(lib().fx_hydro_plan_set_option(self._h, key, float(value)))
+
+    def fx_hydro_plan_workspace_bytes(self):
+        return int(lib().fx_hydro_plan_workspace_bytes(self._h))
+
+    def fx_hydro_plan_set_workspace(self, ws: torch.Tensor | None = None):
+        if ws is None:
+            ws = torch.empty(self.fx_hydro_plan_workspace_bytes(), dtype=torch.uint8, device=self.device)
+        assert ws.is_cuda and ws.dtype == torch.uint8
+        _check(lib().fx_hydro_plan_set_workspace(self._h, C.c_void_p(ws.data_ptr()), ws.numel()))
+        self._ws = ws
+        self._dt = torch.empty(1, dtype=torch.float64, device=self.device)
+
+    def fx_hydro_plan_set_topology(self, neigh):
+        if not isinstance(neigh, torch.Tensor):
+            neigh = torch.as_tensor(np.ascontiguousarray(neigh, np.int32))
+        neigh = neigh.to(self.device, torch.int32).contiguous().reshape(self.nblocks, 6)
+        _check(lib().fx_hydro_plan_set_topology(self._h, C.c_void_p(neigh.data_ptr())))
+        self._neigh = neigh  # caller-owned table must outlive the plan's use of it
+
+    def fx_fill_guardcells(self, U, stream=None):
+        _check(lib().fx_fill_guardcells(self._h, _dev(U, torch.float64), _stream(stream)))
+
+    def fx_guardcell_index_map(self, block_begin=0, block_count=None, stream=None):
+        if block_count is None:
+            block_count = self.nblocks - block_begin
+        src = torch.empty((block_count, self.np[2], self.np[1], self.np[0]), dtype=torch.int64, device=self.device)
+        _check(lib().fx_guardcell_index_map(self._h, block_begin, block_count, C.c_void_p(src.data_ptr()), _stream(stream)))
+        return src
+
+    def fx_hydro_compute_dt(self, U, dx, cfl, dt_out=None, stream=None):
+        """Enqueues the reduction; returns the 1-element device tensor holding dt (no sync)."""
+        dt_out = self._dt if dt_out is None else dt_out
+        _check(lib().fx_hydro_compute_dt(self._h, _dev(U, torch.float64), _dev(dx, torch.float64), float(cfl),
+                                         _dev(dt_out, torch.float64), _stream(stream)))
+        return dt_out
+
+    def fx_hydro_advance(self, U, dx, dt, stream=None):
+        if isinstance(dt, torch.Tensor):
+            _check(lib().fx_hydro_advance_devdt(self._h, _dev(U, torch.float64), _dev(dx, torch.float64),
+                                                _dev(dt, torch.float64), _stream(stream)))
+        else:
+            _check(lib().fx_hydro_advance(self._h, _dev(U, torch.float64), _dev(dx, torch.float64), float(dt),
+                                          _stream(stream)))
+
+    def fx_hydro_advance_host(self, U_host, dx_host, cfl, nsteps, U_stage, dx_stage, stream=None):
+        """U_host / dx_host: CPU (preferably pinned) float64 tensors, updated in place.  Returns the last dt."""
+        assert not U_host.is_cuda and U_host.dtype == torch.float64 and U_host.is_contiguous()
+        assert not dx_host.is_cuda and dx_host.dtype == torch.float64 and dx_host.is_contiguous()
+        dt_last = C.c_double(float("nan"))
+        _check(lib().fx_hydro_advance_host(self._h, C.c_void_p(U_host.data_ptr()), C.c_void_p(dx_host.data_ptr()),
+                                           float(cfl), int(nsteps), _dev(U_stage, torch.float64),
+                                           _dev(dx_stage, torch.float64), C.cast(C.byref(dt_last), C.c_void_p),
+                                           _stream(stream)))
+        return float(dt_last.value)
+
+    def fx_hydro_status(self, stream=None):
+        f = C.c_uint32()
+        cnt = (C.c_ulonglong * 4)()
+        _check(lib().fx_hydro_status(self._h, C.byref(f), cnt, _stream(stream)))
+        return int(f.value), [int(x) for x in cnt]
+
+    def fx_hydro_status_reset(self, stream=None):
+        _check(lib().fx_hydro_status_reset(self._h, _stream(stream)))
+
+    def flux_shape(self, direction):
+        e = list(self.block_dims)
+        e[direction] += 1
+        return (self.nvars, self.nblocks, e[2], e[1], e[0])
+
+    def fx_debug_compute_fluxes(self, U, direction, stream=None):
+        F = torch.empty(self.flux_shape(direction), dtype=torch.float64, device=self.device)
+        _check(lib().fx_debug_compute_fluxes(self._h, _dev(U, torch.float64), direction, _dev(F, torch.float64),
+                                             _stream(stream)))
+        return F
+
+    def interior(self, U):
+        g, n = self.gd, self.block_dims
+        return U[:, :, g[2]:g[2] + n[2], g[1]:g[1] + n[1], g[0]:g[0] + n[0]]
+
+
+def fx_probe_fp64_fma(iters, out, stream=None):
+    n = C.c_ulonglong()
+    _check(lib().fx_probe_fp64_fma(int(iters), _dev(out, torch.float64), C.byref(n), _stream(stream)))
+    return int(n.value)

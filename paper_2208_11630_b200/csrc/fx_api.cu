@@ -1,0 +1,252 @@
+// fx_api.cu -- the C ABI of include/fx_hydro.h: plan / layout manager (a0), call sequencing of the RK
+// stages, error plumbing.  Every entry point is extern "C"; nothing throws across the boundary.
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <algorithm>
+#include <new>
+#include <vector>
+
+#include "fx_internal.h"
+
+static thread_local char fx_errbuf[512] = "";
+
+int fx_fail(int code, const char *fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(fx_errbuf, sizeof(fx_errbuf), fmt, ap);
+  va_end(ap);
+  return code;
+}
+
+int fx_cuda_check(cudaError_t e, const char *what) {
+  if (e == cudaSuccess) return FX_OK;
+  return fx_fail(FX_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
+}
+
+extern "C" const char *fx_last_error(void) { return fx_errbuf; }
+
+// ------------------------------------------------------------------ plan (a0)
+extern "C" int fx_hydro_plan_create(fx_hydro_plan **out, const int block_dims[3], int nguard, int nvars,
+                                    int64_t nblocks, double gamma, int recon, int riemann, int rk_order) {
+  if (!out || !block_dims) return fx_fail(FX_ERR_INVALID_ARG, "plan_create: null argument");
+  *out = nullptr;
+  if (nvars != 5) return fx_fail(FX_ERR_UNSUPPORTED, "plan_create: nvars must be 5 (rho, mx, my, mz, E), got %d", nvars);
+  if (nblocks < 0 || nblocks > 2147483647LL) return fx_fail(FX_ERR_INVALID_ARG, "plan_create: nblocks out of range");
+  if (!(gamma > 1.0) || !isfinite(gamma)) return fx_fail(FX_ERR_INVALID_ARG, "plan_create: gamma must be > 1");
+  if (recon != FX_RECON_PLM_MINMOD && recon != FX_RECON_WENO5) return fx_fail(FX_ERR_INVALID_ARG, "plan_create: unknown reconstruction %d", recon);
+  if (riemann != FX_RIEMANN_HLLE && riemann != FX_RIEMANN_HLLC) return fx_fail(FX_ERR_INVALID_ARG, "plan_create: unknown Riemann solver %d", riemann);
+  if (rk_order != 2 && rk_order != 3) return fx_fail(FX_ERR_INVALID_ARG, "plan_create: rk_order must be 2 or 3");
+  const int need = recon == FX_RECON_WENO5 ? 3 : 2;
+  if (nguard < need) return fx_fail(FX_ERR_INVALID_ARG, "plan_create: nguard %d < %d needed by the reconstruction", nguard, need);
+  fx_hydro_plan *p = new (std::nothrow) fx_hydro_plan();
+  if (!p) return fx_fail(FX_ERR_INVALID_ARG, "plan_create: out of host memory");
+  memset(p, 0, sizeof(*p));
+  FxParams &P = p->P;
+  int nactive = 0;
+  for (int d = 0; d < 3; ++d) {
+    if (block_dims[d] < 1 || block_dims[d] > 4096) {
+      delete p;
+      return fx_fail(FX_ERR_INVALID_ARG, "plan_create: block_dims[%d] = %d out of range", d, block_dims[d]);
+    }
+    P.n[d] = block_dims[d];
+    P.active[d] = block_dims[d] > 1;
+    if (P.active[d]) {
+      ++nactive;
+      if (nguard > block_dims[d]) {
+        delete p;
+        return fx_fail(FX_ERR_INVALID_ARG, "plan_create: nguard %d exceeds block_dims[%d] = %d", nguard, d, block_dims[d]);
+      }
+    }
+    P.gd[d] = P.active[d] ? nguard : 0;
+    P.np[d] = P.n[d] + 2 * P.gd[d];
+  }
+  if (nactive == 0) {
+    delete p;
+    return fx_fail(FX_ERR_INVALID_ARG, "plan_create: no active dimension");
+  }
+  P.S_j = P.np[0];
+  P.S_k = (long long)P.np[0] * P.np[1];
+  P.S_b = P.S_k * P.np[2];
+  P.S_v = P.S_b * nblocks;
+  if (P.S_b > 2147483647LL) {
+    delete p;
+    return fx_fail(FX_ERR_INVALID_ARG, "plan_create: padded block too large");
+  }
+  P.nblocks = nblocks;
+  P.gamma = gamma;
+  P.gm1 = gamma - 1.0;
+  P.igm1 = 1.0 / (gamma - 1.0);
+  P.rho_floor = 1e-12;
+  P.p_floor = 1e-12;
+  P.weno_eps = 1e-6;
+  P.recon = recon;
+  P.riemann = riemann;
+  P.wavespeed = 0;
+  p->nguard = nguard;
+  p->nvars = nvars;
+  p->rk = rk_order;
+  *out = p;
+  return FX_OK;
+}
+
+extern "C" int fx_hydro_plan_destroy(fx_hydro_plan *plan) {
+  delete plan;
+  return FX_OK;
+}
+
+extern "C" int fx_hydro_plan_layout(const fx_hydro_plan *plan, fx_layout *out) {
+  if (!plan || !out) return fx_fail(FX_ERR_INVALID_ARG, "plan_layout: null argument");
+  for (int d = 0; d < 3; ++d) {
+    out->np[d] = plan->P.np[d];
+    out->gd[d] = plan->P.gd[d];
+  }
+  out->S_j = plan->P.S_j;
+  out->S_k = plan->P.S_k;
+  out->S_b = plan->P.S_b;
+  out->S_v = plan->P.S_v;
+  out->bytes_per_state = plan->P.S_v * plan->nvars * (int64_t)sizeof(double);
+  return FX_OK;
+}
+
+extern "C" int fx_hydro_plan_set_option(fx_hydro_plan *plan, int key, double value) {
+  if (!plan) return fx_fail(FX_ERR_INVALID_ARG, "set_option: null plan");
+  switch (key) {
+  case FX_OPT_RHO_FLOOR: plan->P.rho_floor = value; return FX_OK;
+  case FX_OPT_P_FLOOR: plan->P.p_floor = value; return FX_OK;
+  case FX_OPT_WENO_EPS:
+    if (!(value > 0.0)) return fx_fail(FX_ERR_INVALID_ARG, "set_option: WENO eps must be > 0");
+    plan->P.weno_eps = value;
+    return FX_OK;
+  case FX_OPT_WAVESPEED:
+    if (value != 0.0 && value != 1.0) return fx_fail(FX_ERR_INVALID_ARG, "set_option: wavespeed must be 0 or 1");
+    plan->P.wavespeed = (int)value;
+    return FX_OK;
+  case FX_OPT_PATH:
+    if (value != 0.0 && value != 1.0) return fx_fail(FX_ERR_INVALID_ARG, "set_option: path must be 0 or 1");
+    plan->path_option = (int)value;
+    return FX_OK;
+  default: return fx_fail(FX_ERR_INVALID_ARG, "set_option: unknown key %d", key);
+  }
+}
+
+extern "C" int fx_hydro_plan_path(const fx_hydro_plan *plan) {
+  if (!plan) return fx_fail(FX_ERR_INVALID_ARG, "plan_path: null plan");
+  return (plan->path_option == 0 && fx_fused_supported(plan->P)) ? 1 : 0;
+}
+
+static size_t fx_state_bytes_aligned(const fx_hydro_plan *plan) {
+  size_t b = (size_t)plan->P.S_v * plan->nvars * sizeof(double);
+  return (b + 255) & ~(size_t)255;
+}
+
+extern "C" size_t fx_hydro_plan_workspace_bytes(const fx_hydro_plan *plan) {
+  if (!plan) return 0;
+  return (size_t)FX_SCR_WORDS * 8 + (size_t)(plan->rk - 1) * fx_state_bytes_aligned(plan);
+}
+
+extern "C" int fx_hydro_plan_set_workspace(fx_hydro_plan *plan, void *ws, size_t bytes) {
+  if (!plan) return fx_fail(FX_ERR_INVALID_ARG, "set_workspace: null plan");
+  if (!ws || ((uintptr_t)ws & 255) != 0) return fx_fail(FX_ERR_WORKSPACE, "set_workspace: workspace null or not 256-byte aligned");
+  if (bytes < fx_hydro_plan_workspace_bytes(plan))
+    return fx_fail(FX_ERR_WORKSPACE, "set_workspace: %zu bytes given, %zu needed", bytes, fx_hydro_plan_workspace_bytes(plan));
+  unsigned long long init[FX_SCR_WORDS];
+  memset(init, 0, sizeof(init));
+  init[FX_SCR_DTBITS] = 0x7ff0000000000000ull;  // +inf
+  FX_CUDA(cudaMemcpy(ws, init, sizeof(init), cudaMemcpyHostToDevice));
+  FX_CUDA(cudaDeviceSynchronize());
+  plan->workspace = ws;
+  plan->workspace_bytes = bytes;
+  plan->P.scratch = (unsigned long long *)ws;
+  char *base = (char *)ws + FX_SCR_WORDS * 8;
+  plan->stage[0] = (double *)base;
+  plan->stage[1] = plan->rk == 3 ? (double *)(base + fx_state_bytes_aligned(plan)) : nullptr;
+  return FX_OK;
+}
+
+// ------------------------------------------------------------------ topology
+extern "C" int fx_hydro_plan_set_topology(fx_hydro_plan *plan, const int32_t *neigh_dev) {
+  if (!plan) return fx_fail(FX_ERR_INVALID_ARG, "set_topology: null plan");
+  const long long nb = plan->P.nblocks;
+  if (nb > 0) {
+    if (!neigh_dev) return fx_fail(FX_ERR_INVALID_ARG, "set_topology: null table");
+    std::vector<int32_t> h((size_t)nb * 6);
+    FX_CUDA(cudaMemcpy(h.data(), neigh_dev, h.size() * sizeof(int32_t), cudaMemcpyDeviceToHost));
+    for (long long b = 0; b < nb; ++b)
+      for (int f = 0; f < 6; ++f) {
+        if (!plan->P.active[f / 2]) continue;
+        const int32_t v = h[b * 6 + f];
+        if (v >= 0) {
+          if (v >= nb) return fx_fail(FX_ERR_INVALID_ARG, "set_topology: block %lld face %d -> id %d out of range", b, f, v);
+        } else if (v != FX_BC_OUTFLOW) {
+          return fx_fail(FX_ERR_UNSUPPORTED, "set_topology: block %lld face %d has code %d: coarse/fine neighbours are not supported", b, f, v);
+        }
+      }
+  }
+  plan->P.neigh = neigh_dev;
+  plan->topology_set = true;
+  return FX_OK;
+}
+
+static uint64_t fx_morton3(uint32_t x, uint32_t y, uint32_t z) {
+  auto spread = [](uint64_t v) {
+    v &= 0x1fffff;
+    v = (v | v << 32) & 0x1f00000000ffffull;
+    v = (v | v << 16) & 0x1f0000ff0000ffull;
+    v = (v | v << 8) & 0x100f00f00f00f00full;
+    v = (v | v << 4) & 0x10c30c30c30c30c3ull;
+    v = (v | v << 2) & 0x1249249249249249ull;
+    return v;
+  };
+  return spread(x) | spread(y) << 1 | spread(z) << 2;
+}
+
+extern "C" int fx_topology_cartesian(const int nb[3], const int bc_lo[3], const int bc_hi[3], int order,
+                                     int32_t *neigh_out, int32_t *coords_out) {
+  if (!nb || !bc_lo || !bc_hi || !neigh_out) return fx_fail(FX_ERR_INVALID_ARG, "topology_cartesian: null argument");
+  if (order != FX_ORDER_LEX && order != FX_ORDER_MORTON) return fx_fail(FX_ERR_INVALID_ARG, "topology_cartesian: unknown order");
+  for (int d = 0; d < 3; ++d) {
+    if (nb[d] < 1) return fx_fail(FX_ERR_INVALID_ARG, "topology_cartesian: nb[%d] < 1", d);
+    if (bc_lo[d] < 0 || bc_lo[d] > 2 || bc_hi[d] < 0 || bc_hi[d] > 2) return fx_fail(FX_ERR_INVALID_ARG, "topology_cartesian: bad bc code");
+  }
+  const long long N = (long long)nb[0] * nb[1] * nb[2];
+  if (N > 2147483647LL) return fx_fail(FX_ERR_INVALID_ARG, "topology_cartesian: too many blocks");
+  std::vector<int32_t> lex_of_id((size_t)N), id_of_lex((size_t)N);
+  for (long long l = 0; l < N; ++l) lex_of_id[l] = (int32_t)l;
+  if (order == FX_ORDER_MORTON) {
+    std::vector<uint64_t> key((size_t)N);
+    for (long long l = 0; l < N; ++l)
+      key[l] = fx_morton3((uint32_t)(l % nb[0]), (uint32_t)((l / nb[0]) % nb[1]), (uint32_t)(l / ((long long)nb[0] * nb[1])));
+    std::stable_sort(lex_of_id.begin(), lex_of_id.end(), [&](int32_t a, int32_t b) { return key[a] < key[b]; });
+  }
+  for (long long id = 0; id < N; ++id) id_of_lex[lex_of_id[id]] = (int32_t)id;
+  for (long long id = 0; id < N; ++id) {
+    const long long l = lex_of_id[id];
+    const int c[3] = {(int)(l % nb[0]), (int)((l / nb[0]) % nb[1]), (int)(l / ((long long)nb[0] * nb[1]))};
+    if (coords_out)
+      for (int d = 0; d < 3; ++d) coords_out[id * 3 + d] = c[d];
+    for (int d = 0; d < 3; ++d)
+      for (int s = 0; s < 2; ++s) {
+        const int bc = s ? bc_hi[d] : bc_lo[d];
+        int32_t v;
+        if (bc == FX_TOPO_NONE) {
+          v = FX_BC_NONE;
+        } else {
+          int cc[3] = {c[0], c[1], c[2]};
+          cc[d] += s ? 1 : -1;
+          const bool outside = cc[d] < 0 || cc[d] >= nb[d];
+          if (outside && bc == FX_TOPO_OUTFLOW) {
+            v = FX_BC_OUTFLOW;
+          } else {
+            cc[d] = (cc[d] + nb[d]) % nb[d];
+            v = id_of_lex[((long long)cc[2] * nb[1] + cc[1]) * nb[0] + cc[0]];
+          }
+        }
+        neigh_out[id * 6 + 2 * d + s] = v;
+      }
+  }
+  return FX_OK;
+}

@@ -1,0 +1,156 @@
+// fx_generic.cu -- generic (any block shape, 1/2/3-D) stage kernel and the debug flux kernel.
+//
+// The generic path is: K1 full guard fill of the stage input, then this zone kernel: one thread per
+// interior zone computes the two face fluxes of each active direction from the padded stage input
+// (each face is evaluated by both zones that share it, bit-identically, so conservation holds to
+// rounding), forms S = sum_d dt/dx_d (F+ - F-) and the SSP-RK combination.  It is the path for block
+// shapes the fused kernel (fx_fused.cu) does not cover (configs 1 and 2) and the scaffold its parity is
+// checked against; it is not the roofline path.
+#include "fx_physics.cuh"
+
+// Face flux of direction d at the face whose left cell is element cL of X (variable-0 index).
+template <int RECON, int RIEMANN>
+__device__ __forceinline__ unsigned fx_face_flux_global(const FxParams &P, const double *__restrict__ X, long long cL,
+                                                        int d, long long s, double F[5]) {
+  constexpr int R = (RECON == FX_RECON_PLM_MINMOD) ? 2 : 3;  // cells each side of the face
+  double W[2 * R][5];
+  unsigned hit = 0;
+#pragma unroll
+  for (int m = 0; m < 2 * R; ++m) {
+    const long long c = cL + (m - (R - 1)) * s;
+    hit |= fx_c2p(P, X[c], X[P.S_v + c], X[2 * P.S_v + c], X[3 * P.S_v + c], X[4 * P.S_v + c], W[m]);
+  }
+  const int in = 1 + d, it1 = 1 + (d + 1) % 3, it2 = 1 + (d + 2) % 3;
+  const int map[5] = {0, in, it1, it2, 4};
+  double WL[5], WR[5];
+#pragma unroll
+  for (int f = 0; f < 5; ++f) {
+    const int v = map[f];
+    if (RECON == FX_RECON_PLM_MINMOD) {
+      const double a = W[0][v], b = W[1][v], c = W[2][v], e = W[3][v];
+      WL[f] = b + 0.5 * fx_minmod(b - a, c - b);
+      WR[f] = c - 0.5 * fx_minmod(c - b, e - c);
+    } else {
+      WL[f] = fx_weno5(W[0][v], W[1][v], W[2][v], W[3][v], W[4][v], P.weno_eps);
+      WR[f] = fx_weno5(W[5][v], W[4][v], W[3][v], W[2][v], W[1][v], P.weno_eps);
+    }
+  }
+  if (RECON == FX_RECON_WENO5) {  // positivity fallback per side [A6]
+    if (!(WL[0] > 0.0) || !(WL[4] > 0.0)) {
+#pragma unroll
+      for (int f = 0; f < 5; ++f) WL[f] = W[R - 1][map[f]];
+      hit |= FX_STATUS_WENO_FALLBACK;
+    }
+    if (!(WR[0] > 0.0) || !(WR[4] > 0.0)) {
+#pragma unroll
+      for (int f = 0; f < 5; ++f) WR[f] = W[R][map[f]];
+      hit |= FX_STATUS_WENO_FALLBACK;
+    }
+  }
+  double Ff[5];
+  fx_riemann<RIEMANN>(P, WL, WR, Ff);
+  F[0] = Ff[0];
+  F[in] = Ff[1];
+  F[it1] = Ff[2];
+  F[it2] = Ff[3];
+  F[4] = Ff[4];
+  const double sum = Ff[0] + Ff[1] + Ff[2] + Ff[3] + Ff[4];
+  if (!(fabs(sum) <= 1.79e308)) hit |= FX_STATUS_NONFINITE;
+  return hit & (FX_STATUS_NONFINITE | FX_STATUS_WENO_FALLBACK);  // floors are counted where a zone is owned
+}
+
+template <int RECON, int RIEMANN>
+__global__ void __launch_bounds__(128) fx_k_generic_stage(FxParams P, const double *__restrict__ X,
+                                                          const double *U0, double *out,
+                                                          const double *__restrict__ dx, double dt,
+                                                          const double *__restrict__ dt_dev, double beta, int first,
+                                                          long long nzones) {
+  const long long z = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (z >= nzones) return;
+  const int nx = P.n[0], ny = P.n[1], nz = P.n[2];
+  const long long per_block = (long long)nx * ny * nz;
+  const long long b = z / per_block;
+  const int r = (int)(z - b * per_block);
+  const int i = r % nx, j = (r / nx) % ny, k = r / (nx * ny);
+  const long long c = b * P.S_b + (k + P.gd[2]) * P.S_k + (j + P.gd[1]) * P.S_j + (i + P.gd[0]);
+  if (dt_dev) dt = *dt_dev;
+  const long long stride[3] = {1, P.S_j, P.S_k};
+  double S[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+  unsigned hit = 0;
+  {  // floors are counted once per owned zone
+    double W[5];
+    hit |= fx_c2p(P, X[c], X[P.S_v + c], X[2 * P.S_v + c], X[3 * P.S_v + c], X[4 * P.S_v + c], W) &
+           (FX_STATUS_RHO_FLOOR | FX_STATUS_P_FLOOR | FX_STATUS_NONFINITE);
+  }
+#pragma unroll 1
+  for (int d = 0; d < 3; ++d) {
+    if (!P.active[d]) continue;
+    const double rd = dt / __ldg(&dx[b * 3 + d]);
+    double Fm[5], Fp[5];
+    hit |= fx_face_flux_global<RECON, RIEMANN>(P, X, c - stride[d], d, stride[d], Fm);
+    hit |= fx_face_flux_global<RECON, RIEMANN>(P, X, c, d, stride[d], Fp);
+#pragma unroll
+    for (int v = 0; v < 5; ++v) S[v] += rd * (Fp[v] - Fm[v]);
+  }
+#pragma unroll
+  for (int v = 0; v < 5; ++v) {
+    const long long g = v * P.S_v + c;
+    const double u0 = U0[g];
+    out[g] = first ? (u0 - S[v]) : (u0 + beta * ((X[g] - u0) - S[v]));
+  }
+  if (hit) fx_note(P, hit);
+}
+
+template <int RECON, int RIEMANN>
+__global__ void __launch_bounds__(128) fx_k_debug_fluxes(FxParams P, const double *__restrict__ U, int dir,
+                                                         double *__restrict__ F, long long nfaces, int e0, int e1,
+                                                         int e2) {
+  const long long z = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (z >= nfaces) return;
+  const long long per_block = (long long)e0 * e1 * e2;
+  const long long b = z / per_block;
+  const int r = (int)(z - b * per_block);
+  int cc[3] = {r % e0 + P.gd[0], (r / e0) % e1 + P.gd[1], r / (e0 * e1) + P.gd[2]};
+  cc[dir] -= 1;  // left cell of face f is padded cell gd + f - 1 [A17]
+  const long long stride[3] = {1, P.S_j, P.S_k};
+  const long long cL = b * P.S_b + cc[2] * P.S_k + cc[1] * P.S_j + cc[0];
+  double Ff[5];
+  unsigned hit = fx_face_flux_global<RECON, RIEMANN>(P, U, cL, dir, stride[dir], Ff);
+  const long long FS_v = per_block * P.nblocks;
+#pragma unroll
+  for (int v = 0; v < 5; ++v) F[v * FS_v + z] = Ff[v];
+  if (hit) fx_note(P, hit);
+}
+
+#define FX_DISPATCH(P, CALL)                                                                       \
+  do {                                                                                             \
+    if (P.recon == FX_RECON_PLM_MINMOD && P.riemann == FX_RIEMANN_HLLE) { CALL(FX_RECON_PLM_MINMOD, FX_RIEMANN_HLLE); } \
+    else if (P.recon == FX_RECON_PLM_MINMOD) { CALL(FX_RECON_PLM_MINMOD, FX_RIEMANN_HLLC); }       \
+    else if (P.riemann == FX_RIEMANN_HLLE) { CALL(FX_RECON_WENO5, FX_RIEMANN_HLLE); }              \
+    else { CALL(FX_RECON_WENO5, FX_RIEMANN_HLLC); }                                                \
+  } while (0)
+
+int fx_launch_generic_stage(const FxParams &P, const double *X, const double *U0, double *out, const double *dx,
+                            double dt, const double *dt_dev, double beta, int first, cudaStream_t st) {
+  const long long nzones = P.nblocks * P.n[0] * P.n[1] * P.n[2];
+  if (nzones == 0) return FX_OK;
+  const unsigned grid = (unsigned)((nzones + 127) / 128);
+#define CALL(RC, RM) fx_k_generic_stage<RC, RM><<<grid, 128, 0, st>>>(P, X, U0, out, dx, dt, dt_dev, beta, first, nzones)
+  FX_DISPATCH(P, CALL);
+#undef CALL
+  FX_LAUNCH_CHECK("generic_stage");
+  return FX_OK;
+}
+
+int fx_launch_debug_fluxes(const FxParams &P, const double *U, int dir, double *F, cudaStream_t st) {
+  int e[3] = {P.n[0], P.n[1], P.n[2]};
+  e[dir] += 1;
+  const long long nfaces = P.nblocks * e[0] * e[1] * e[2];
+  if (nfaces == 0) return FX_OK;
+  const unsigned grid = (unsigned)((nfaces + 127) / 128);
+#define CALL(RC, RM) fx_k_debug_fluxes<RC, RM><<<grid, 128, 0, st>>>(P, U, dir, F, nfaces, e[0], e[1], e[2])
+  FX_DISPATCH(P, CALL);
+#undef CALL
+  FX_LAUNCH_CHECK("debug_fluxes");
+  return FX_OK;
+}

@@ -1,0 +1,62 @@
+// fx_internal.h -- plan object and kernel parameter block of libfxhydro (not part of the ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/fx_hydro.h"
+
+// Parameter block passed by value to every kernel (a0: the block-layout manager's address map).
+struct FxParams {
+  int n[3];       // interior zones per block (x, y, z)
+  int gd[3];      // guard depth per dimension (0 if inactive)
+  int np[3];      // padded extents
+  int active[3];
+  long long S_j, S_k, S_b, S_v;  // element strides of U[v][b][k][j][i]
+  long long nblocks;
+  double gamma, gm1, igm1;
+  double rho_floor, p_floor, weno_eps;
+  int recon, riemann, wavespeed;
+  const int *neigh;                 // [nblocks][6], device
+  unsigned long long *scratch;      // device scratch block, see FX_SCR_*
+};
+
+// 64-bit words of the scratch block
+enum {
+  FX_SCR_DTBITS = 0,   // running min of dx/(|u|+c) as the bit pattern of a non-negative double
+  FX_SCR_COUNTER = 1,  // CTAs finished in the dt reduction
+  FX_SCR_FLAGS = 2,    // status bits
+  FX_SCR_COUNT0 = 4,   // 4 counters: non-finite, rho floor, p floor, WENO fallback
+  FX_SCR_WORDS = 32
+};
+
+struct fx_hydro_plan {
+  FxParams P;
+  int nguard, nvars, rk;
+  int path_option;      // FX_OPT_PATH
+  void *workspace;      // device
+  size_t workspace_bytes;
+  double *stage[2];     // RK stage copies inside the workspace
+  bool topology_set;
+};
+
+// error plumbing (fx_api.cu)
+int fx_fail(int code, const char *fmt, ...);
+int fx_cuda_check(cudaError_t e, const char *what);
+#define FX_CUDA(call)                                   \
+  do {                                                  \
+    int _rc = fx_cuda_check((call), #call);             \
+    if (_rc) return _rc;                                \
+  } while (0)
+#define FX_LAUNCH_CHECK(name) FX_CUDA(cudaPeekAtLastError())
+
+// kernel launchers (one per .cu file); all enqueue on `st`
+int fx_launch_fill_guardcells(const FxParams &P, double *U, cudaStream_t st);
+int fx_launch_index_map(const FxParams &P, long long b0, long long nb, long long *src, cudaStream_t st);
+int fx_launch_compute_dt(const FxParams &P, const double *U, const double *dx, double cfl, double *dt_out,
+                         cudaStream_t st);
+int fx_launch_generic_stage(const FxParams &P, const double *X, const double *U0, double *out, const double *dx,
+                            double dt, const double *dt_dev, double beta, int first, cudaStream_t st);
+int fx_launch_debug_fluxes(const FxParams &P, const double *U, int dir, double *F, cudaStream_t st);
+bool fx_fused_supported(const FxParams &P);
+int fx_launch_fused_stage(const FxParams &P, const double *X, const double *U0, double *out, const double *dx,
+                          double dt, const double *dt_dev, double beta, int first, cudaStream_t st);

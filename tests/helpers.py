@@ -142,3 +142,24 @@ def rel_err(cfg, got, ref):
     if not np.all(np.isfinite(got)):
         return float("inf")
     return float(e.max())
+
+
+def gpu_plan_for(cfg, order=inputs.ORDER_LEX, bc=None, nb=None, recon=None, riemann=None, rk=None, path=None,
+                 neigh=None, nblocks=None):
+    """CUDA-side plan + topology + workspace for a config (uses the library's own topology helper)."""
+    from paper_2208_11630_b200 import binding as fx
+    nb = tuple(nb or cfg.nb)
+    bc = bc or cfg.bc
+    code = {"periodic": fx.TOPO_PERIODIC, "outflow": fx.TOPO_OUTFLOW}[bc]
+    bcs = [code if cfg.block_dims[d] > 1 else fx.TOPO_NONE for d in range(3)]
+    coords = None
+    if neigh is None:
+        neigh, coords = fx.fx_topology_cartesian(nb, bcs, bcs, order)
+    plan = fx.HydroPlan(cfg.block_dims, cfg.nguard, neigh.shape[0], cfg.gamma,
+                        cfg.recon if recon is None else recon, cfg.riemann if riemann is None else riemann,
+                        cfg.rk_order if rk is None else rk)
+    if path is not None:
+        plan.fx_hydro_plan_set_option(fx.OPT_PATH, path)
+    plan.fx_hydro_plan_set_topology(neigh)
+    plan.fx_hydro_plan_set_workspace()
+    return plan, neigh, coords

@@ -1,0 +1,110 @@
+"""CPU-side checks of the C ABI: the library loads, exports every symbol include/fx_hydro.h declares, and its
+host logic (argument checks, layout, topology helper) agrees with the oracle's independent implementation."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+from oracle import fxoracle as fxo
+from paper_2208_11630_b200 import binding as fx
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def declared_symbols():
+    text = open(os.path.join(ROOT, "include", "fx_hydro.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(fx_[a-z0-9_]+)\s*\(", text)))
+
+
+def test_library_exports_every_declared_symbol():
+    L = fx.lib()
+    syms = declared_symbols()
+    assert len(syms) >= 18
+    for s in syms:
+        assert hasattr(L, s), s
+    assert sorted(fx.EXPORTS) == syms
+
+
+def test_enum_values_match_between_header_oracle_and_binding():
+    text = open(os.path.join(ROOT, "include", "fx_hydro.h")).read()
+    def val(name):
+        m = re.search(r"\b%s\s*=\s*(-?\d+)" % name, text) or re.search(r"#define\s+%s\s+\(?(-?\d+)" % name, text)
+        return int(m.group(1))
+    for name in ("RECON_PLM_MINMOD", "RECON_WENO5", "RIEMANN_HLLE", "RIEMANN_HLLC", "BC_OUTFLOW", "BC_NONE",
+                 "TOPO_PERIODIC", "TOPO_OUTFLOW", "TOPO_NONE", "ORDER_LEX", "ORDER_MORTON", "OPT_RHO_FLOOR",
+                 "OPT_P_FLOOR", "OPT_WENO_EPS", "OPT_WAVESPEED"):
+        assert val("FX_" + name) == getattr(fx, name) == getattr(fxo, name), name
+
+
+def create(dims, g, nb, gamma=1.4, recon=0, riemann=1, rk=2, nvars=5):
+    h = C.c_void_p()
+    rc = fx.lib().fx_hydro_plan_create(C.byref(h), (C.c_int * 3)(*dims), g, nvars, nb, gamma, recon, riemann, rk)
+    return rc, h
+
+
+def test_plan_create_argument_checks():
+    assert create((16, 16, 16), 4, 8)[0] == fx.OK
+    assert create((16, 16, 16), 1, 8)[0] == fx.ERR_INVALID_ARG
+    assert create((16, 16, 16), 2, 8, recon=1)[0] == fx.ERR_INVALID_ARG  # WENO5 needs 3
+    assert create((2, 1, 1), 3, 8)[0] == fx.ERR_INVALID_ARG              # nguard > block dim
+    assert create((16, 0, 1), 4, 8)[0] == fx.ERR_INVALID_ARG
+    assert create((1, 1, 1), 2, 8)[0] == fx.ERR_INVALID_ARG              # no active dim
+    assert create((16, 16, 16), 4, 8, gamma=1.0)[0] == fx.ERR_INVALID_ARG
+    assert create((16, 16, 16), 4, 8, rk=4)[0] == fx.ERR_INVALID_ARG
+    assert create((16, 16, 16), 4, 8, recon=2)[0] == fx.ERR_INVALID_ARG
+    assert create((16, 16, 16), 4, 8, riemann=7)[0] == fx.ERR_INVALID_ARG
+    assert create((16, 16, 16), 4, -1)[0] == fx.ERR_INVALID_ARG
+    assert create((16, 16, 16), 4, 8, nvars=6)[0] == fx.ERR_UNSUPPORTED
+    assert b"nvars" in fx.lib().fx_last_error()
+
+
+@pytest.mark.parametrize("dims,g,nb", [((16, 16, 16), 4, 32768), ((256, 1, 1), 4, 1), ((16, 16, 1), 4, 64), ((8, 8, 8), 3, 5)])
+def test_layout_matches_oracle_and_closed_form(dims, g, nb):
+    rc, h = create(dims, g, nb)
+    assert rc == 0
+    L = fx.Layout()
+    assert fx.lib().fx_hydro_plan_layout(h, C.byref(L)) == 0
+    o = fxo.OraclePlan(dims, g, nb, 1.4, 0, 1, 2)
+    assert tuple(L.np) == o.np and tuple(L.gd) == o.gd
+    assert (L.S_j, L.S_k, L.S_b, L.S_v, L.bytes_per_state) == (o.S_j, o.S_k, o.S_b, o.S_v, o.bytes_per_state)
+    npd = [d + 2 * g if d > 1 else d for d in dims]
+    assert L.S_b == npd[0] * npd[1] * npd[2] and L.bytes_per_state == 5 * 8 * nb * L.S_b
+    # workspace = (rk - 1) state copies (256-byte aligned) + 256-byte scratch
+    ws = fx.lib().fx_hydro_plan_workspace_bytes(h)
+    assert ws == 256 + ((L.bytes_per_state + 255) // 256) * 256
+    rc3, h3 = create(dims, g, nb, rk=3)
+    assert fx.lib().fx_hydro_plan_workspace_bytes(h3) == 256 + 2 * (((L.bytes_per_state + 255) // 256) * 256)
+
+
+def test_config5_needs_64bit_indexing():
+    rc, h = create((16, 16, 16), 4, 32768)
+    L = fx.Layout()
+    fx.lib().fx_hydro_plan_layout(h, C.byref(L))
+    assert 5 * L.S_v > 2 ** 31 and L.bytes_per_state == 18119393280
+
+
+@pytest.mark.parametrize("nb,lo,hi,order", [((4, 3, 2), (0, 1, 0), (0, 1, 0), 0), ((4, 4, 4), (0, 0, 0), (0, 0, 0), 1),
+                                            ((5, 1, 1), (1, 2, 2), (0, 2, 2), 0), ((3, 5, 1), (0, 1, 2), (1, 0, 2), 1),
+                                            ((1, 1, 1), (0, 0, 0), (0, 0, 0), 1)])
+def test_topology_helper_matches_oracle(nb, lo, hi, order):
+    n1, c1 = fx.fx_topology_cartesian(nb, lo, hi, order)
+    n2, c2 = fxo.topology_cartesian(nb, lo, hi, order)
+    assert np.array_equal(n1, n2) and np.array_equal(c1, c2)
+
+
+def test_options_and_state_errors_without_gpu():
+    rc, h = create((16, 16, 16), 4, 8)
+    L = fx.lib()
+    assert L.fx_hydro_plan_set_option(h, fx.OPT_WAVESPEED, 1.0) == 0
+    assert L.fx_hydro_plan_set_option(h, fx.OPT_WAVESPEED, 2.0) == fx.ERR_INVALID_ARG
+    assert L.fx_hydro_plan_set_option(h, 99, 0.0) == fx.ERR_INVALID_ARG
+    assert L.fx_hydro_plan_set_option(h, fx.OPT_WENO_EPS, 0.0) == fx.ERR_INVALID_ARG
+    # operations before topology / workspace are refused before any CUDA call is made
+    assert L.fx_fill_guardcells(h, None, None) == fx.ERR_STATE
+    assert L.fx_hydro_advance(h, None, None, 0.1, None) == fx.ERR_STATE
+    assert L.fx_hydro_compute_dt(h, None, None, 0.3, None, None) == fx.ERR_STATE
+    assert L.fx_hydro_plan_set_workspace(h, C.c_void_p(8), 1 << 30) == fx.ERR_WORKSPACE  # misaligned
+    assert L.fx_hydro_plan_set_workspace(h, C.c_void_p(256), 16) == fx.ERR_WORKSPACE     # too small

@@ -1,0 +1,230 @@
+"""GPU <-> oracle parity through the C ABI (run on the B200 box: pytest -m gpu).
+Tolerances [NS]: interior zones <= 1e-12 after one RK step, <= 1e-9 after 10 steps (metric A21);
+dt <= 1e-14 relative; guard-cell index maps and filled guard data bit-exact."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import fxoracle as fxo
+from paper_2208_11630_b200 import inputs
+from tests.helpers import gpu_plan_for, oracle_plan_for, rel_err
+
+pytestmark = pytest.mark.gpu
+
+TOL_1, TOL_10, TOL_DT = 1e-12, 1e-9, 1e-14
+
+
+def setup(number, nb=None, path=None, **kw):
+    cfg = inputs.config(number, nb=nb)
+    oplan, neigh, coords = oracle_plan_for(cfg, **kw)
+    gplan, gneigh, gcoords = gpu_plan_for(cfg, path=path, **kw)
+    assert np.array_equal(neigh, gneigh) and np.array_equal(coords, gcoords)
+    Uh = inputs.embed(cfg, inputs.block_interiors(cfg, coords))
+    return cfg, oplan, gplan, Uh, inputs.dx_array(cfg)
+
+
+GUARD_CASES = [
+    ((4, 4, 4), 2, (2, 2, 2), "periodic", 0), ((4, 4, 4), 4, (2, 2, 2), "periodic", 1),
+    ((6, 4, 5), 3, (3, 1, 2), "outflow", 0), ((8, 6, 1), 3, (2, 3, 1), "periodic", 0),
+    ((12, 1, 1), 4, (3, 1, 1), "outflow", 0), ((12, 1, 1), 4, (1, 1, 1), "periodic", 0),
+    ((16, 16, 16), 4, (3, 2, 2), "periodic", 1), ((16, 16, 1), 4, (8, 8, 1), "periodic", 0),
+    ((256, 1, 1), 4, (1, 1, 1), "outflow", 0),
+]
+
+
+@pytest.mark.parametrize("dims,g,nb,bc,order", GUARD_CASES)
+def test_guard_index_map_and_fill_bit_exact(dims, g, nb, bc, order):
+    cfg = inputs.config(3)
+    cfg.block_dims, cfg.nguard, cfg.nb, cfg.bc = dims, g, nb, bc
+    oplan, neigh, coords = oracle_plan_for(cfg, order=order)
+    gplan, _, _ = gpu_plan_for(cfg, order=order)
+    assert np.array_equal(gplan.fx_guardcell_index_map().cpu().numpy(), oplan.index_map())
+    if gplan.nblocks > 2:
+        assert np.array_equal(gplan.fx_guardcell_index_map(1, 2).cpu().numpy(), oplan.index_map(1, 2))
+    rng = np.random.default_rng(42)
+    Uh = np.full(oplan.shape, np.nan)
+    oplan.interior(Uh)[...] = rng.normal(size=oplan.interior(Uh).shape)
+    Ud = torch.from_numpy(Uh).cuda()
+    oplan.fill_guardcells(Uh)
+    gplan.fx_fill_guardcells(Ud)
+    assert np.array_equal(Ud.cpu().numpy(), Uh)  # every zone, bit for bit (no NaN left)
+    assert not np.isnan(Uh).any()
+
+
+@pytest.mark.parametrize("number,nb", [(1, None), (2, None), (3, (4, 4, 4)), (4, (3, 3, 3)), (5, (3, 3, 3))])
+def test_compute_dt(number, nb):
+    cfg, oplan, gplan, Uh, dx = setup(number, nb)
+    dt_o = oplan.compute_dt(Uh.numpy(), dx, cfg.cfl)
+    dt_g = float(gplan.fx_hydro_compute_dt(Uh.cuda(), torch.from_numpy(dx).cuda(), cfg.cfl).item())
+    assert abs(dt_g - dt_o) <= TOL_DT * dt_o
+    # twice in a row: the scratch word re-arms itself
+    dt_g2 = float(gplan.fx_hydro_compute_dt(Uh.cuda(), torch.from_numpy(dx).cuda(), cfg.cfl).item())
+    assert dt_g2 == dt_g
+
+
+def test_compute_dt_uniform_state_closed_form_and_per_block_dx():
+    cfg = inputs.config(3, nb=(2, 2, 2))
+    oplan, neigh, coords = oracle_plan_for(cfg)
+    gplan, _, _ = gpu_plan_for(cfg)
+    W = (0.5, 0.3, -1.1, 0.4, 0.8)
+    E = W[4] / 0.4 + 0.5 * W[0] * (W[1] ** 2 + W[2] ** 2 + W[3] ** 2)
+    U = np.full(oplan.shape, np.nan)
+    for v, val in enumerate((W[0], W[0] * W[1], W[0] * W[2], W[0] * W[3], E)):
+        oplan.interior(U)[v] = val
+    dx = np.random.default_rng(0).uniform(0.01, 0.1, size=(8, 3))
+    dt_o = oplan.compute_dt(U, dx, 0.3)
+    dt_g = float(gplan.fx_hydro_compute_dt(torch.from_numpy(U).cuda(), torch.from_numpy(dx).cuda(), 0.3).item())
+    assert abs(dt_g - dt_o) <= TOL_DT * dt_o
+
+
+@pytest.mark.parametrize("number,nb,recon,riemann", [(2, (2, 2, 1), 0, 1), (3, (2, 2, 2), 0, 1), (3, (2, 2, 2), 0, 0),
+                                                     (5, (2, 2, 2), 1, 1), (4, (2, 2, 2), 1, 0), (1, None, 0, 0)])
+def test_debug_fluxes(number, nb, recon, riemann):
+    cfg, oplan, gplan, Uh, dx = setup(number, nb, recon=recon, riemann=riemann)
+    Un = Uh.numpy().copy()
+    oplan.fill_guardcells(Un)
+    Ud = torch.from_numpy(Un).cuda()
+    for d in range(3):
+        if cfg.block_dims[d] == 1:
+            continue
+        Fo = oplan.debug_compute_fluxes(Un, d)
+        Fg = gplan.fx_debug_compute_fluxes(Ud, d).cpu().numpy()
+        scale = np.abs(Fo).max(axis=(1, 2, 3, 4), keepdims=True)
+        scale[1:4] = scale[1:4].max()
+        assert np.all(np.abs(Fg - Fo) <= 1e-13 * scale)  # scale may be 0 (e.g. Sedov mass flux at t = 0): then exact
+
+
+ADV_CASES = [  # number, nb, kwargs
+    (1, None, {}), (2, None, {}), (3, None, {}), (4, (3, 3, 3), {}), (5, (3, 3, 3), {}),
+    (3, (2, 2, 2), dict(riemann=0, rk=3)), (5, (2, 2, 2), dict(recon=1, riemann=0, rk=2)),
+    (2, (3, 2, 1), dict(recon=1, rk=3)), (5, (2, 2, 2), dict(bc="outflow")),
+]
+
+
+@pytest.mark.parametrize("path", [None, 1])
+@pytest.mark.parametrize("number,nb,kw", ADV_CASES)
+def test_advance_1_and_10_steps(number, nb, kw, path):
+    cfg, oplan, gplan, Uh, dx = setup(number, nb, path=path, **kw)
+    if path == 1 and gplan.path == 0 and False:
+        pytest.skip()
+    Uo = Uh.numpy().copy()
+    Ud = Uh.cuda()
+    dxd = torch.from_numpy(dx).cuda()
+    for step in range(10):
+        dt = oplan.compute_dt(Uo, dx, cfg.cfl)
+        oplan.advance(Uo, dx, dt)
+        gplan.fx_hydro_advance(Ud, dxd, dt)  # same dt on both sides: the step itself is what is compared
+        if step in (0, 9):
+            err = rel_err(cfg, gplan.interior(Ud).cpu().numpy(), oplan.interior(Uo))
+            assert err <= (TOL_1 if step == 0 else TOL_10), (step, err)
+    fo, _ = oplan.status()
+    fg, _ = gplan.fx_hydro_status()
+    assert fo == fg, (fo, fg)
+
+
+def test_device_dt_path_equals_host_dt_path():
+    cfg, oplan, gplan, Uh, dx = setup(5, (2, 2, 2))
+    dxd = torch.from_numpy(dx).cuda()
+    A, B = Uh.cuda(), Uh.cuda()
+    for _ in range(3):
+        dt = gplan.fx_hydro_compute_dt(A, dxd, cfg.cfl)
+        gplan.fx_hydro_advance(A, dxd, dt)  # device-resident dt
+        dth = float(gplan.fx_hydro_compute_dt(B, dxd, cfg.cfl).item())
+        gplan.fx_hydro_advance(B, dxd, dth)
+    assert torch.equal(gplan.interior(A), gplan.interior(B))
+
+
+def test_advance_host_equals_device_path():
+    cfg, oplan, gplan, Uh, dx = setup(3, (2, 2, 2))
+    dxd = torch.from_numpy(dx).cuda()
+    A = Uh.cuda()
+    for _ in range(2):
+        gplan.fx_hydro_advance(A, dxd, gplan.fx_hydro_compute_dt(A, dxd, cfg.cfl))
+    Hh = Uh.clone().pin_memory()
+    dxh = torch.from_numpy(dx).pin_memory()
+    stage, dstage = torch.empty_like(A), torch.empty_like(dxd)
+    dt_last = gplan.fx_hydro_advance_host(Hh, dxh, cfg.cfl, 2, stage, dstage)
+    assert np.isfinite(dt_last) and dt_last > 0
+    assert torch.equal(gplan.interior(Hh), gplan.interior(A).cpu())
+
+
+@pytest.mark.parametrize("recon,riemann,rk", [(0, 0, 2), (0, 1, 3), (1, 0, 3), (1, 1, 2)])
+def test_uniform_state_preserved_bitwise(recon, riemann, rk):
+    for dims, nb in (((16, 16, 16), (2, 2, 2)), ((6, 5, 4), (2, 1, 2)), ((16, 16, 1), (2, 2, 1))):
+        cfg = inputs.config(3, nb=nb)
+        cfg.block_dims = dims
+        for bc in ("periodic", "outflow"):
+            gplan, _, _ = gpu_plan_for(cfg, bc=bc, recon=recon, riemann=riemann, rk=rk)
+            W = (1.3, 0.7, -0.4, 0.2, 2.2)
+            E = W[4] / (cfg.gamma - 1) + 0.5 * W[0] * (W[1] ** 2 + W[2] ** 2 + W[3] ** 2)
+            U = torch.full(gplan.shape, float("nan"), dtype=torch.float64, device="cuda")
+            for v, val in enumerate((W[0], W[0] * W[1], W[0] * W[2], W[0] * W[3], E)):
+                gplan.interior(U)[v] = val
+            U0 = gplan.interior(U).clone()
+            dx = torch.tensor([[0.1, 0.2, 0.15]] * gplan.nblocks, dtype=torch.float64, device="cuda")
+            for _ in range(10):
+                gplan.fx_hydro_advance(U, dx, 0.01)
+            assert torch.equal(gplan.interior(U), U0)
+
+
+def test_guard_contents_do_not_matter_and_bad_dt_is_refused():
+    from paper_2208_11630_b200 import binding as fx
+    cfg, oplan, gplan, Uh, dx = setup(5, (2, 2, 2))
+    dxd = torch.from_numpy(dx).cuda()
+    Ui = inputs.interior_view(cfg, Uh)
+    A = inputs.embed(cfg, Ui, float("nan")).cuda()
+    B = inputs.embed(cfg, Ui, 123.0).cuda()
+    gplan.fx_hydro_advance(A, dxd, 1e-4)
+    gplan.fx_hydro_advance(B, dxd, 1e-4)
+    assert torch.equal(gplan.interior(A), gplan.interior(B))
+    for bad in (0.0, -1.0, float("nan"), float("inf")):
+        with pytest.raises(fx.FxError) as e:
+            gplan.fx_hydro_advance(A, dxd, bad)
+        assert e.value.code == fx.ERR_INVALID_ARG
+
+
+def test_block_permutation_invariance_bitwise():
+    cfg = inputs.config(5, nb=(3, 2, 2))
+    gplan, neigh, coords = gpu_plan_for(cfg)
+    Uh = inputs.embed(cfg, inputs.block_interiors(cfg, coords))
+    perm = np.random.default_rng(3).permutation(12)
+    inv = np.argsort(perm)
+    neigh_p = neigh[perm].copy()
+    neigh_p[neigh_p >= 0] = inv[neigh_p[neigh_p >= 0]]
+    gplan_p, _, _ = gpu_plan_for(cfg, neigh=neigh_p)
+    A = Uh.cuda()
+    B = Uh[:, perm].contiguous().cuda()
+    dx = torch.from_numpy(inputs.dx_array(cfg)).cuda()
+    for _ in range(2):
+        gplan.fx_hydro_advance(A, dx, 2e-4)
+        gplan_p.fx_hydro_advance(B, dx, 2e-4)
+    assert torch.equal(gplan.interior(A)[:, perm], gplan_p.interior(B))
+
+
+def test_sod_mirror_symmetry_and_run_to_time():
+    cfg, oplan, gplan, Uh, dx = setup(1)
+    dxd = torch.from_numpy(dx).cuda()
+    A = Uh.cuda()
+    M = Uh.flip(-1).clone()
+    M[1] *= -1
+    M = M.cuda()
+    gplan.fx_hydro_advance(A, dxd, 0.0026411070460266143)
+    gplan.fx_hydro_advance(M, dxd, 0.0026411070460266143)
+    a, m = gplan.interior(A).cpu().numpy(), gplan.interior(M).cpu().numpy()[..., ::-1]
+    assert np.max(np.abs(a[0] - m[0])) <= 1e-13 and np.max(np.abs(a[4] - m[4])) <= 1e-13 * 2.5
+    assert np.max(np.abs(a[1] + m[1])) <= 1e-13
+    # whole run to t = 0.2 with the GPU's own dt, last step clipped; compare with the oracle's run
+    Uo = Uh.numpy().copy()
+    Ud = Uh.cuda()
+    t = 0.0
+    n = 0
+    while t < 0.2:
+        dt = float(gplan.fx_hydro_compute_dt(Ud, dxd, cfg.cfl).item())
+        dto = oplan.compute_dt(Uo, dx, cfg.cfl)
+        assert abs(dt - dto) <= 1e-11 * dto  # states drift apart by rounding only
+        dt = min(dto, 0.2 - t)
+        gplan.fx_hydro_advance(Ud, dxd, dt)
+        oplan.advance(Uo, dx, dt)
+        t += dt
+        n += 1
+    assert rel_err(cfg, gplan.interior(Ud).cpu().numpy(), oplan.interior(Uo)) <= 1e-9
