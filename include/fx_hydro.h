@@ -158,6 +158,13 @@ int fx_debug_compute_fluxes(fx_hydro_plan *plan, const double *U_dev, int dir, d
  * 1 fused (halo gathered from neighbour interiors inside the stage kernel). */
 int fx_hydro_plan_path(const fx_hydro_plan *plan);
 
+/* Measurement aid: when enabled, fx_hydro_advance brackets every stage-kernel launch (the dominant
+ * kernel; excludes the guard fill of the generic path) with CUDA events on the launching stream (at most
+ * 4096 launches are recorded between two reads).  get_timing synchronises the recorded events, returns
+ * the summed kernel time in milliseconds and the number of launches, and clears the record. */
+int fx_hydro_plan_set_timing(fx_hydro_plan *plan, int enable);
+int fx_hydro_plan_get_timing(fx_hydro_plan *plan, double *stage_ms_sum_host, long long *stage_launches_host);
+
 /* Measurement aid for the fp64 roofline: runs a dependent-chain-free DFMA kernel (iters FMAs per
  * thread on 8 independent accumulators) over the whole device; the caller times it with events.
  * out_dev: double [1] sink.  Returns the number of FMAs issued in *fma_count_host. */

@@ -29,7 +29,7 @@ EXPORTS = [
     "fx_hydro_plan_set_topology", "fx_topology_cartesian", "fx_fill_guardcells", "fx_guardcell_index_map",
     "fx_hydro_compute_dt", "fx_hydro_advance", "fx_hydro_advance_host", "fx_hydro_advance_devdt",
     "fx_hydro_status", "fx_hydro_status_reset", "fx_debug_compute_fluxes", "fx_hydro_plan_path",
-    "fx_probe_fp64_fma",
+    "fx_probe_fp64_fma", "fx_hydro_plan_set_timing", "fx_hydro_plan_get_timing",
 ]
 
 
@@ -77,6 +77,8 @@ def lib():
         L.fx_hydro_status_reset.argtypes = [vp, vp]
         L.fx_debug_compute_fluxes.argtypes = [vp, vp, C.c_int, vp, vp]
         L.fx_hydro_plan_path.argtypes = [vp]
+        L.fx_hydro_plan_set_timing.argtypes = [vp, C.c_int]
+        L.fx_hydro_plan_get_timing.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
         L.fx_probe_fp64_fma.argtypes = [C.c_int, vp, C.POINTER(C.c_ulonglong), vp]
         _lib = L
     return _lib
@@ -205,6 +207,15 @@ class HydroPlan:
 
     def fx_hydro_status_reset(self, stream=None):
         _check(lib().fx_hydro_status_reset(self._h, _stream(stream)))
+
+    def fx_hydro_plan_set_timing(self, enable=True):
+        _check(lib().fx_hydro_plan_set_timing(self._h, int(bool(enable))))
+
+    def fx_hydro_plan_get_timing(self):
+        """(sum of stage-kernel milliseconds, number of launches) since the last read."""
+        ms, n = C.c_double(), C.c_longlong()
+        _check(lib().fx_hydro_plan_get_timing(self._h, C.byref(ms), C.byref(n)))
+        return float(ms.value), int(n.value)
 
     def flux_shape(self, direction):
         e = list(self.block_dims)

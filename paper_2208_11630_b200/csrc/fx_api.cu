@@ -94,6 +94,10 @@ extern "C" int fx_hydro_plan_create(fx_hydro_plan **out, const int block_dims[3]
 }
 
 extern "C" int fx_hydro_plan_destroy(fx_hydro_plan *plan) {
+  if (plan && plan->ev) {
+    for (int i = 0; i < 2 * FX_MAX_REC; ++i) cudaEventDestroy(plan->ev[i]);
+    delete[] plan->ev;
+  }
   delete plan;
   return FX_OK;
 }

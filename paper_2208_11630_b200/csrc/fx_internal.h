@@ -37,7 +37,12 @@ struct fx_hydro_plan {
   size_t workspace_bytes;
   double *stage[2];     // RK stage copies inside the workspace
   bool topology_set;
+  // optional per-launch timing of the stage kernels (fx_hydro_plan_set_timing)
+  bool timing;
+  cudaEvent_t *ev;  // 2 * FX_MAX_REC events, created on demand
+  int nrec;
 };
+enum { FX_MAX_REC = 4096 };
 
 // error plumbing (fx_api.cu)
 int fx_fail(int code, const char *fmt, ...);

@@ -3,6 +3,8 @@
 #include <math.h>
 #include <string.h>
 
+#include <new>
+
 #include "fx_internal.h"
 
 static int fx_need(const fx_hydro_plan *plan, bool topo, bool ws, const char *who) {
@@ -39,10 +41,49 @@ extern "C" int fx_hydro_compute_dt(fx_hydro_plan *plan, const double *U, const d
 // gathered from neighbour interiors inside the fused kernel.
 static int fx_stage(fx_hydro_plan *plan, double *X, const double *U0, double *out, const double *dx, double dt,
                     const double *dt_dev, double beta, int first, cudaStream_t st) {
-  if (fx_hydro_plan_path(plan) == 1) return fx_launch_fused_stage(plan->P, X, U0, out, dx, dt, dt_dev, beta, first, st);
-  int rc = fx_launch_fill_guardcells(plan->P, X, st);  // O1 on the stage input before every S(.) [A15]
+  const bool fused = fx_hydro_plan_path(plan) == 1;
+  int rc = FX_OK;
+  if (!fused) {
+    rc = fx_launch_fill_guardcells(plan->P, X, st);  // O1 on the stage input before every S(.) [A15]
+    if (rc) return rc;
+  }
+  const bool rec = plan->timing && plan->ev && plan->nrec < FX_MAX_REC;
+  if (rec) FX_CUDA(cudaEventRecord(plan->ev[2 * plan->nrec], st));
+  rc = fused ? fx_launch_fused_stage(plan->P, X, U0, out, dx, dt, dt_dev, beta, first, st)
+             : fx_launch_generic_stage(plan->P, X, U0, out, dx, dt, dt_dev, beta, first, st);
   if (rc) return rc;
-  return fx_launch_generic_stage(plan->P, X, U0, out, dx, dt, dt_dev, beta, first, st);
+  if (rec) {
+    FX_CUDA(cudaEventRecord(plan->ev[2 * plan->nrec + 1], st));
+    ++plan->nrec;
+  }
+  return FX_OK;
+}
+
+extern "C" int fx_hydro_plan_set_timing(fx_hydro_plan *plan, int enable) {
+  if (!plan) return fx_fail(FX_ERR_INVALID_ARG, "set_timing: null plan");
+  if (enable && !plan->ev) {
+    plan->ev = new (std::nothrow) cudaEvent_t[2 * FX_MAX_REC];
+    if (!plan->ev) return fx_fail(FX_ERR_INVALID_ARG, "set_timing: out of host memory");
+    for (int i = 0; i < 2 * FX_MAX_REC; ++i) FX_CUDA(cudaEventCreate(&plan->ev[i]));
+  }
+  plan->timing = enable != 0;
+  plan->nrec = 0;
+  return FX_OK;
+}
+
+extern "C" int fx_hydro_plan_get_timing(fx_hydro_plan *plan, double *ms_sum, long long *launches) {
+  if (!plan || !ms_sum || !launches) return fx_fail(FX_ERR_INVALID_ARG, "get_timing: null argument");
+  double sum = 0.0;
+  for (int i = 0; i < plan->nrec; ++i) {
+    float ms = 0.f;
+    FX_CUDA(cudaEventSynchronize(plan->ev[2 * i + 1]));
+    FX_CUDA(cudaEventElapsedTime(&ms, plan->ev[2 * i], plan->ev[2 * i + 1]));
+    sum += ms;
+  }
+  *ms_sum = sum;
+  *launches = plan->nrec;
+  plan->nrec = 0;
+  return FX_OK;
 }
 
 static int fx_advance_impl(fx_hydro_plan *plan, double *U, const double *dx, double dt, const double *dt_dev,
