@@ -1,0 +1,310 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the batched block Euler update on B200 (one JSON line on stdout).
+
+A "step" is one pass of the whole hot path over the workload: fx_hydro_compute_dt (a7) followed by
+fx_hydro_advance (a1..a6, all RK stages), dt staying on the device.  Metric: hydro zone-updates/s per RK
+stage = interior zones x stages / time.  Workload at N = 1: BASELINE.json configs[4] (32768 blocks of 16^3,
+PLM-minmod + HLLC, SSP-RK2; 18.1 GB per state copy, far larger than the 126 MB L2, so nothing is served
+from cache between timed iterations).  N > 1: N independent replicas of that workload, one per rank
+("replicas only", DESIGN.md section Multi-GPU); no data-path collective is invented.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 5] [--nb a,b,c]
+
+--impl reference times the CPU oracle (oracle/) on the box's host cores on a bounded sample of the same
+workload; it is a deliberately slow program, reported as a baseline, not a target.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "hydro zone-updates/s per RK stage (fp64)"
+UNIT = "zone-updates/s"
+FP64_FMA_LANES_PER_SM = 64  # 148 SMs x 64 DFMA lanes; confirmed by fx_probe_fp64_fma
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=5)
+    ap.add_argument("--nb", default=None, help="override blocks per dimension, e.g. 16,16,16")
+    ap.add_argument("--path", type=int, default=0, help="FX_OPT_PATH: 0 auto (fused when supported), 1 generic")
+    ap.add_argument("--order", default="morton", choices=["lex", "morton"])
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    return ap.parse_args()
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks and throttle reasons during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def stop(self, t0, t1):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, smax, reasons = [], None, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        rows = [r for (t, r) in self.rows if t0 - 0.05 <= t <= t1 + 0.05] or [r for (_, r) in self.rows]
+        for r in rows:
+            f = [x.strip() for x in r.split(",")]
+            try:
+                sm.append(float(f[0]))
+                smax = float(f[1])
+            except Exception:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": smax, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def build_workload(args, device):
+    """Config, plan, state resident in HBM (generated on the device), dx."""
+    import torch
+    from paper_2208_11630_b200 import binding as fx
+    from paper_2208_11630_b200 import inputs
+    nb = tuple(int(x) for x in args.nb.split(",")) if args.nb else None
+    cfg = inputs.config(args.config, nb=nb)
+    order = fx.ORDER_MORTON if args.order == "morton" else fx.ORDER_LEX
+    code = fx.TOPO_PERIODIC if cfg.bc == "periodic" else fx.TOPO_OUTFLOW
+    bcs = [code if cfg.block_dims[d] > 1 else fx.TOPO_NONE for d in range(3)]
+    neigh, coords = fx.fx_topology_cartesian(cfg.nb, bcs, bcs, order)
+    plan = fx.HydroPlan(cfg.block_dims, cfg.nguard, cfg.nblocks, cfg.gamma, cfg.recon, cfg.riemann, cfg.rk_order,
+                        device=device)
+    plan.fx_hydro_plan_set_option(fx.OPT_PATH, args.path)
+    plan.fx_hydro_plan_set_topology(neigh)
+    plan.fx_hydro_plan_set_workspace()
+    U = torch.full(plan.shape, float("nan"), dtype=torch.float64, device=device)
+    Ui = plan.interior(U)
+    chunk = 1024
+    for b0 in range(0, cfg.nblocks, chunk):
+        b1 = min(cfg.nblocks, b0 + chunk)
+        Ui[:, b0:b1] = inputs.block_interiors(cfg, coords[b0:b1], device)
+    dx = torch.from_numpy(inputs.dx_array(cfg)).to(device)
+    return cfg, plan, U, dx, coords
+
+
+# ------------------------------------------------------------------ CPU oracle legs
+def oracle_sample(args, target_seconds=15.0, steps=None):
+    """Times the oracle as it stands on a bounded sample of the workload: a 6x6x6-block sub-tiling of the
+    same field (periodic wrap of the sub-tiling), all host threads OpenMP gives it."""
+    import numpy as np
+    from oracle import fxoracle as fxo
+    from paper_2208_11630_b200 import inputs
+    full = inputs.config(args.config)
+    nb = tuple(min(6, full.nb[d]) for d in range(3))
+    cfg = inputs.config(args.config, nb=nb)
+    code = fxo.TOPO_PERIODIC if cfg.bc == "periodic" else fxo.TOPO_OUTFLOW
+    bcs = [code if cfg.block_dims[d] > 1 else fxo.TOPO_NONE for d in range(3)]
+    neigh, coords = fxo.topology_cartesian(cfg.nb, bcs, bcs, fxo.ORDER_LEX)
+    plan = fxo.OraclePlan(cfg.block_dims, cfg.nguard, cfg.nblocks, cfg.gamma, cfg.recon, cfg.riemann, cfg.rk_order)
+    plan.set_topology(neigh)
+    U = inputs.embed(cfg, inputs.block_interiors(cfg, coords)).numpy()
+    dx = inputs.dx_array(cfg)
+    cores = len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1)
+
+    def one_step():
+        t = time.perf_counter()
+        dt = plan.compute_dt(U, dx, cfg.cfl)
+        plan.advance(U, dx, dt)
+        return time.perf_counter() - t
+
+    t_first = one_step()  # also the warm-up
+    if steps is None:
+        steps = max(2, min(50, int(target_seconds / max(t_first, 1e-3))))
+    times = [one_step() for _ in range(steps)]
+    per_step = sum(times) / len(times)
+    zs = cfg.interior_zones * cfg.rk_order
+    return {"value": zs / per_step, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"config {args.config} field on a {nb[0]}x{nb[1]}x{nb[2]}-block periodic sub-tiling "
+                      f"({cfg.interior_zones} zones), {steps} steps of compute_dt + advance, OpenMP over blocks",
+            "ms_per_step": per_step * 1e3, "steps": steps}
+
+
+def run_reference(args, rank, world):
+    if rank != 0:
+        return
+    from paper_2208_11630_b200 import inputs
+    cfg = inputs.config(args.config)
+    # each step is one oracle step on the bounded sample; warm-up steps run first, untimed
+    r = oracle_sample(args, steps=max(1, args.steps))
+    line = {"impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": r["ms_per_step"], "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"config {args.config}: {cfg.name} (bounded sample: {r['sample']})"},
+            "cpu_baseline": {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle", "sample": r["sample"]},
+            "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------ CUDA arm
+def run_ours(args, rank, world, local_rank):
+    import torch
+    import torch.distributed as dist
+    from paper_2208_11630_b200 import binding as fx
+
+    fx.lib()  # fail loudly if the CUDA library is missing
+    torch.cuda.set_device(local_rank)
+    device = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=device)
+    cfg, plan, U, dx, coords = build_workload(args, device)
+    stages = cfg.rk_order
+    zones = cfg.interior_zones
+    fused = plan.path == 1
+    launches_per_step = 1 + stages * (1 if fused else 2)  # dt + per stage (guard fill +) stage kernel
+
+    def step():
+        dt = plan.fx_hydro_compute_dt(U, dx, cfg.cfl)  # stays on the device
+        plan.fx_hydro_advance(U, dx, dt)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    plan.fx_hydro_plan_set_timing(True)
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    time.sleep(0.3)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    t0 = time.time()
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    barrier()
+    t1 = time.time()
+    clocks = sampler.stop(t0, t1)
+    ms = e0.elapsed_time(e1)
+    stage_ms, stage_launches = plan.fx_hydro_plan_get_timing()
+    plan.fx_hydro_plan_set_timing(False)
+    flags, counts = plan.fx_hydro_status()
+    if world > 1:
+        t = torch.tensor([ms], dtype=torch.float64, device=device)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    value = world * zones * stages * args.steps / (ms * 1e-3)
+
+    # roofline of the dominant kernel (the stage kernel): algorithmic bytes per launch / its mean duration
+    peak, peak_src = measured_peaks()
+    alg_bytes_stage = [80.0] + [120.0] * (stages - 1)  # B per zone: read X (+U0), write out
+    alg_bytes_per_launch = zones * sum(alg_bytes_stage) / stages
+    stage_avg_ms = stage_ms / max(stage_launches, 1)
+    achieved = alg_bytes_per_launch / (stage_avg_ms * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": None, "peak_source": peak_src, "kernel": "fused stage kernel" if fused else "generic stage kernel",
+                "kernel_ms_avg": stage_avg_ms, "kernel_launches_timed": stage_launches,
+                "kernel_share_of_step": stage_ms / ms if ms > 0 else None,
+                "alg_bytes_per_zone_stage": sum(alg_bytes_stage) / stages}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"config {cfg.number}: {cfg.name}, {cfg.nblocks} blocks of "
+                                   f"{cfg.block_dims[0]}x{cfg.block_dims[1]}x{cfg.block_dims[2]} (+{cfg.nguard} guard), "
+                                   f"{'WENO5' if cfg.recon else 'PLM-minmod'}+{'HLLC' if cfg.riemann else 'HLLE'}, SSP-RK{stages}",
+                       "interior_zones": zones, "state_bytes": plan.bytes_per_state, "block_order": args.order,
+                       "path": "fused" if fused else "generic", "l2": "inputs (state) larger than L2; no flush needed",
+                       "multi_gpu": "replicas only" if world > 1 else "single"},
+            "clocks": clocks, "gpu_launches": launches_per_step * args.steps, "roofline": roofline,
+            "status_flags": flags}
+
+    # end to end through the C ABI with HOST buffers (H2D + steps + D2H inside the timed region)
+    if not args.no_e2e:
+        try:
+            Uh = torch.empty(plan.shape, dtype=torch.float64, pin_memory=True)
+            Uh.copy_(U)
+            dxh = dx.cpu().pin_memory()
+            stage_dev, dxs = U, torch.empty_like(dx)  # reuse the resident state buffer as the staging buffer
+            plan.fx_hydro_advance_host(Uh, dxh, cfg.cfl, 1, stage_dev, dxs)  # warm-up
+            barrier()
+            tt = time.perf_counter()
+            for _ in range(args.e2e_steps):
+                plan.fx_hydro_advance_host(Uh, dxh, cfg.cfl, 1, stage_dev, dxs)
+            torch.cuda.synchronize()
+            es = (time.perf_counter() - tt) / args.e2e_steps
+            if world > 1:
+                t = torch.tensor([es], dtype=torch.float64, device=device)
+                dist.all_reduce(t, op=dist.ReduceOp.MAX)
+                es = float(t.item())
+            line["e2e"] = {"value": world * zones * stages / es, "unit": UNIT,
+                           "h2d_bytes_per_step": plan.bytes_per_state + dx.numel() * 8,
+                           "d2h_bytes_per_step": plan.bytes_per_state + 8, "ms_per_step": es * 1e3,
+                           "steps": args.e2e_steps, "api": "fx_hydro_advance_host (pinned host buffers)"}
+            del Uh
+        except Exception as ex:  # e.g. not enough pinnable host memory
+            line["e2e"] = {"value": None, "unit": UNIT, "error": repr(ex)[:200]}
+
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        del U
+        torch.cuda.empty_cache()
+        line["cpu_baseline"] = {k: v for k, v in oracle_sample(args).items() if k in ("value", "unit", "cores", "kind", "sample")}
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+    else:
+        run_ours(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()
