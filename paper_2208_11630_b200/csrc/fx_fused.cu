@@ -43,7 +43,7 @@ __device__ __forceinline__ void cta_sync() { asm volatile("bar.sync 0, %0;" ::"n
 template <int RECON>
 __device__ __forceinline__ void recon_cell(const double *s, double eps, double &qm, double &qp) {
   if (RECON == FX_RECON_PLM_MINMOD) {
-    const double h = 0.5 * fx_minmod(s[1] - s[0], s[2] - s[1]);
+    const double h = 0.5 * fx_minmod_fast(s[1] - s[0], s[2] - s[1]);
     qm = s[1] - h;
     qp = s[1] + h;
   } else {
@@ -109,7 +109,7 @@ __device__ __forceinline__ void flux_dir(const FxParams &P, const double WL[5], 
   const double wl[5] = {WL[0], WL[in], WL[it1], WL[it2], WL[4]};
   const double wr[5] = {WR[0], WR[in], WR[it1], WR[it2], WR[4]};
   double f[5];
-  fx_riemann<RIEMANN>(P, wl, wr, f);
+  fx_riemann_fast<RIEMANN>(P, wl, wr, f);
   F[0] = f[0];
   F[in] = f[1];
   F[it1] = f[2];
@@ -164,7 +164,7 @@ fx_k_fused_stage(FxParams P, const double *__restrict__ X, const double *U0, dou
       int kp;
       z_source(P, b, nlo, nhi, k, bs, kp);
       const long long a = bs * P.S_b + (long long)kp * P.S_k + col;
-      const unsigned h = fx_c2p(P, X[a], X[a + Sv], X[a + 2 * Sv], X[a + 3 * Sv], X[a + 4 * Sv], w);
+      const unsigned h = fx_c2p_fast(P, X[a], X[a + Sv], X[a + 2 * Sv], X[a + 3 * Sv], X[a + 4 * Sv], w);
       if (k >= 0 && k < nz) hit |= h;  // a zone's floor hits are counted by its owner only
     };
 
@@ -275,7 +275,7 @@ fx_k_fused_stage(FxParams P, const double *__restrict__ X, const double *U0, dou
           if (nlo >= 0) { bs = nlo; cd += NX; } else cd = 0;
           const long long a = bs * P.S_b + plane + (long long)(cd + gdd) * sd;
           double w[5];
-          fx_c2p(P, X[a], X[a + Sv], X[a + 2 * Sv], X[a + 3 * Sv], X[a + 4 * Sv], w);
+          fx_c2p_fast(P, X[a], X[a + Sv], X[a + 2 * Sv], X[a + 3 * Sv], X[a + 4 * Sv], w);
 #pragma unroll
           for (int v = 0; v < 5; ++v) Pf[v * NP * NP + t * pd + (m + R) * pt] = w[v];
         }
@@ -285,7 +285,7 @@ fx_k_fused_stage(FxParams P, const double *__restrict__ X, const double *U0, dou
           if (nhi >= 0) { bs = nhi; cd -= NX; } else cd = NX - 1;
           const long long a = bs * P.S_b + plane + (long long)(cd + gdd) * sd;
           double w[5];
-          fx_c2p(P, X[a], X[a + Sv], X[a + 2 * Sv], X[a + 3 * Sv], X[a + 4 * Sv], w);
+          fx_c2p_fast(P, X[a], X[a + Sv], X[a + 2 * Sv], X[a + 3 * Sv], X[a + 4 * Sv], w);
 #pragma unroll
           for (int v = 0; v < 5; ++v) Pf[v * NP * NP + (NX + R + t) * pd + (m + R) * pt] = w[v];
         }
@@ -317,7 +317,7 @@ fx_k_fused_stage(FxParams P, const double *__restrict__ X, const double *U0, dou
         const double wl[5] = {WL[0], isx ? WL[1] : WL[2], isx ? WL[2] : WL[3], isx ? WL[3] : WL[1], WL[4]};
         const double wr[5] = {qm16[0], isx ? qm16[1] : qm16[2], isx ? qm16[2] : qm16[3], isx ? qm16[3] : qm16[1], qm16[4]};
         double f[5];
-        fx_riemann<RIEMANN>(P, wl, wr, f);
+        fx_riemann_fast<RIEMANN>(P, wl, wr, f);
         double F[5];
         F[0] = f[0];
         F[1] = isx ? f[1] : f[3];
