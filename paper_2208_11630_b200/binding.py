@@ -12,7 +12,7 @@ import numpy as np
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libfxhydro.so")
+LIB_PATH = os.environ.get("FXHYDRO_LIB") or os.path.join(_HERE, "libfxhydro.so")  # FXHYDRO_LIB: an alternative build
 
 OK, ERR_INVALID_ARG, ERR_STATE, ERR_UNSUPPORTED, ERR_WORKSPACE, ERR_CUDA = 0, -1, -2, -3, -4, -5
 RECON_PLM_MINMOD, RECON_WENO5 = 0, 1

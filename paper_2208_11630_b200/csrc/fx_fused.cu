@@ -15,6 +15,10 @@
 // HBM traffic is one read of the stage input (+ U0 in later stages) and one write per zone, plus halos.
 #include "fx_physics.cuh"
 
+#ifndef FX_FUSED_MINB_PLM
+#define FX_FUSED_MINB_PLM 1  // resident CTAs per SM the PLM kernels are compiled for
+#endif
+
 namespace {
 
 constexpr int NX = 16, NY = 16;
@@ -159,21 +163,34 @@ fx_k_fused_stage(FxParams P, const double *__restrict__ X, const double *U0, dou
 #pragma unroll
     for (int v = 0; v < 5; ++v) qpz[v] = Fz[v] = 0.0;
 
-    auto load_prim = [&](int k, double w[5]) {
+    auto z_addr = [&](int k) -> long long {
       long long bs;
       int kp;
       z_source(P, b, nlo, nhi, k, bs, kp);
-      const long long a = bs * P.S_b + (long long)kp * P.S_k + col;
-      const unsigned h = fx_c2p_fast(P, X[a], X[a + Sv], X[a + 2 * Sv], X[a + 3 * Sv], X[a + 4 * Sv], w);
+      return bs * P.S_b + (long long)kp * P.S_k + col;
+    };
+    auto load_raw = [&](int k, double u[5]) {
+      const long long a = z_addr(k);
+#pragma unroll
+      for (int v = 0; v < 5; ++v) u[v] = X[a + v * Sv];
+    };
+    auto to_prim = [&](int k, const double u[5], double w[5]) {
+      const unsigned h = fx_c2p_fast(P, u[0], u[1], u[2], u[3], u[4], w);
       if (k >= 0 && k < nz) hit |= h;  // a zone's floor hits are counted by its owner only
     };
 
+    double Un[5];  // raw conserved variables of the next new cell (software prefetch, one plane ahead)
 #pragma unroll
-    for (int m = 0; m < 2 * r; ++m) load_prim(-R + m, q[m]);
+    for (int m = 0; m < 2 * r; ++m) {
+      load_raw(-R + m, Un);
+      to_prim(-R + m, Un, q[m]);
+    }
+    load_raw(-1 + r, Un);
 
 #pragma unroll 1
     for (int c = -1; c <= nz; ++c) {
-      load_prim(c + r, q[2 * r]);
+      to_prim(c + r, Un, q[2 * r]);
+      if (c < nz) load_raw(c + r + 1, Un);
       const bool inplane = c >= 1;  // in-plane work for plane p = c - 1, whose primitives are q[r-1]
       const int p = c - 1;
       double qmx[5], qmy[5];
@@ -203,6 +220,16 @@ fx_k_fused_stage(FxParams P, const double *__restrict__ X, const double *U0, dou
         }
         cta_sync();  // B: plus-side states visible
       }
+      // operands of the stage combination, requested now and consumed after the Riemann solves
+      double u0[5], xs[5];
+      if (inplane) {
+        const long long a0 = b * P.S_b + (long long)(p + P.gd[2]) * P.S_k + col;
+#pragma unroll
+        for (int v = 0; v < 5; ++v) {
+          u0[v] = U0[a0 + v * Sv];
+          xs[v] = first ? 0.0 : X[a0 + v * Sv];
+        }
+      }
       // z: reconstruct cell c, flux of face c (between cells c-1 and c)
       double qmz[5], qpz_new[5], Fz_new[5];
       hit |= recon_cell5<RECON>(q, P.weno_eps, qmz, qpz_new);
@@ -229,8 +256,7 @@ fx_k_fused_stage(FxParams P, const double *__restrict__ X, const double *U0, dou
           const double dFz = Fz_new[v] - Fz[v];
           const double Sd = rx * dFx + ry * dFy + rz * dFz;
           const long long a = a0 + v * Sv;
-          const double u0 = U0[a];
-          const double res = first ? (u0 - Sd) : (u0 + beta * ((X[a] - u0) - Sd));
+          const double res = first ? (u0[v] - Sd) : (u0[v] + beta * ((xs[v] - u0[v]) - Sd));
           out[a] = res;
           chk += res;
         }
@@ -264,32 +290,42 @@ fx_k_fused_stage(FxParams P, const double *__restrict__ X, const double *U0, dou
     const int ld = isx ? 1 : NX, lt = isx ? (NX + 1) : 1;  // strides of L/G along direction / transverse
     constexpr int LV = NY * (NX + 1);                       // per-variable size of L/G arrays (272)
 
+    // global address of halo cell t (low: cell -R+t, high: cell 16+t) of row/column m in plane p
+    auto halo_addr = [&](int p, int t, bool high) -> long long {
+      const long long plane = (long long)(p + P.gd[2]) * P.S_k + (long long)(m + gdt) * st_;
+      long long bs = b;
+      int cd;
+      if (!high) {
+        cd = -R + t;
+        if (nlo >= 0) { bs = nlo; cd += NX; } else cd = 0;
+      } else {
+        cd = NX + t;
+        if (nhi >= 0) { bs = nhi; cd -= NX; } else cd = NX - 1;
+      }
+      return bs * P.S_b + plane + (long long)(cd + gdd) * sd;
+    };
+    double Hn[2 * R][5];  // raw halo cells of the next plane (software prefetch)
+    auto load_halo = [&](int p) {
+#pragma unroll
+      for (int t = 0; t < 2 * R; ++t) {
+        const long long a = halo_addr(p, t % R, t >= R);
+#pragma unroll
+        for (int v = 0; v < 5; ++v) Hn[t][v] = X[a + v * Sv];
+      }
+    };
+    load_halo(0);
+
 #pragma unroll 1
     for (int p = 0; p < nz; ++p) {
-      const long long plane = (long long)(p + P.gd[2]) * P.S_k + (long long)(m + gdt) * st_;
 #pragma unroll
-      for (int t = 0; t < R; ++t) {
-        {  // low halo cell -R+t
-          long long bs = b;
-          int cd = -R + t;
-          if (nlo >= 0) { bs = nlo; cd += NX; } else cd = 0;
-          const long long a = bs * P.S_b + plane + (long long)(cd + gdd) * sd;
-          double w[5];
-          fx_c2p_fast(P, X[a], X[a + Sv], X[a + 2 * Sv], X[a + 3 * Sv], X[a + 4 * Sv], w);
+      for (int t = 0; t < 2 * R; ++t) {
+        double w[5];
+        fx_c2p_fast(P, Hn[t][0], Hn[t][1], Hn[t][2], Hn[t][3], Hn[t][4], w);
+        const int pos = (t < R) ? t : (NX + t);  // padded position along the edge direction
 #pragma unroll
-          for (int v = 0; v < 5; ++v) Pf[v * NP * NP + t * pd + (m + R) * pt] = w[v];
-        }
-        {  // high halo cell 16+t
-          long long bs = b;
-          int cd = NX + t;
-          if (nhi >= 0) { bs = nhi; cd -= NX; } else cd = NX - 1;
-          const long long a = bs * P.S_b + plane + (long long)(cd + gdd) * sd;
-          double w[5];
-          fx_c2p_fast(P, X[a], X[a + Sv], X[a + 2 * Sv], X[a + 3 * Sv], X[a + 4 * Sv], w);
-#pragma unroll
-          for (int v = 0; v < 5; ++v) Pf[v * NP * NP + (NX + R + t) * pd + (m + R) * pt] = w[v];
-        }
+        for (int v = 0; v < 5; ++v) Pf[v * NP * NP + pos * pd + (m + R) * pt] = w[v];
       }
+      if (p + 1 < nz) load_halo(p + 1);
       cta_sync();  // A
       double qm16[5];
       {
@@ -360,8 +396,8 @@ int fx_launch_fused_stage(const FxParams &P, const double *X, const double *U0, 
   if (!fx_fused_supported(P)) return fx_fail(FX_ERR_UNSUPPORTED, "fused stage kernel: block shape not supported");
   if (P.nblocks == 0) return FX_OK;
   if (P.recon == FX_RECON_PLM_MINMOD) {
-    if (P.riemann == FX_RIEMANN_HLLE) return launch<FX_RECON_PLM_MINMOD, FX_RIEMANN_HLLE, 2>(P, X, U0, out, dx, dt, dt_dev, beta, first, st);
-    return launch<FX_RECON_PLM_MINMOD, FX_RIEMANN_HLLC, 2>(P, X, U0, out, dx, dt, dt_dev, beta, first, st);
+    if (P.riemann == FX_RIEMANN_HLLE) return launch<FX_RECON_PLM_MINMOD, FX_RIEMANN_HLLE, FX_FUSED_MINB_PLM>(P, X, U0, out, dx, dt, dt_dev, beta, first, st);
+    return launch<FX_RECON_PLM_MINMOD, FX_RIEMANN_HLLC, FX_FUSED_MINB_PLM>(P, X, U0, out, dx, dt, dt_dev, beta, first, st);
   }
   if (P.riemann == FX_RIEMANN_HLLE) return launch<FX_RECON_WENO5, FX_RIEMANN_HLLE, 1>(P, X, U0, out, dx, dt, dt_dev, beta, first, st);
   return launch<FX_RECON_WENO5, FX_RIEMANN_HLLC, 1>(P, X, U0, out, dx, dt, dt_dev, beta, first, st);
