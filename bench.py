@@ -94,6 +94,22 @@ class ClockSampler:
                 "samples": len(sm)}
 
 
+def max_over_ranks(x: float, world: int, device="cpu") -> float:
+    """Max of a per-rank scalar over all ranks (the multi-GPU timing rule); identity for one rank."""
+    if world <= 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(zones_per_rank: int, stages: int, steps: int, ms_max: float, world: int) -> float:
+    """Replicas only: every rank advances its own copy of the workload; value = all zone-updates / max time."""
+    return world * zones_per_rank * stages * steps / (ms_max * 1e-3)
+
+
 def measured_peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -229,11 +245,8 @@ def run_ours(args, rank, world, local_rank):
     stage_ms, stage_launches = plan.fx_hydro_plan_get_timing()
     plan.fx_hydro_plan_set_timing(False)
     flags, counts = plan.fx_hydro_status()
-    if world > 1:
-        t = torch.tensor([ms], dtype=torch.float64, device=device)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    value = world * zones * stages * args.steps / (ms * 1e-3)
+    ms = max_over_ranks(ms, world, device)
+    value = whole_job_value(zones, stages, args.steps, ms, world)
 
     # roofline of the dominant kernel (the stage kernel): algorithmic bytes per launch / its mean duration
     peak, peak_src = measured_peaks()
@@ -273,10 +286,7 @@ def run_ours(args, rank, world, local_rank):
                 plan.fx_hydro_advance_host(Uh, dxh, cfg.cfl, 1, stage_dev, dxs)
             torch.cuda.synchronize()
             es = (time.perf_counter() - tt) / args.e2e_steps
-            if world > 1:
-                t = torch.tensor([es], dtype=torch.float64, device=device)
-                dist.all_reduce(t, op=dist.ReduceOp.MAX)
-                es = float(t.item())
+            es = max_over_ranks(es, world, device)
             line["e2e"] = {"value": world * zones * stages / es, "unit": UNIT,
                            "h2d_bytes_per_step": plan.bytes_per_state + dx.numel() * 8,
                            "d2h_bytes_per_step": plan.bytes_per_state + 8, "ms_per_step": es * 1e3,

@@ -1,0 +1,52 @@
+"""Host-side logic of the N > 1 bench path, run as 2 gloo ranks on the CPU: the path does not shard across
+GPUs in this round ("replicas only"), so what N > 1 adds is the max-over-ranks timing, the
+whole-job aggregation and the reference arm running on rank 0 alone."""
+import json
+import os
+import socket
+import subprocess
+import sys
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+WORKER = r"""
+import os, sys, json
+sys.path.insert(0, %r)
+import torch.distributed as dist
+import bench
+dist.init_process_group("gloo", rank=int(os.environ["RANK"]), world_size=int(os.environ["WORLD_SIZE"]))
+rank, world = dist.get_rank(), dist.get_world_size()
+ms = bench.max_over_ranks(10.0 + 5.0 * rank, world, "cpu")
+val = bench.whole_job_value(1000, 2, 3, ms, world)
+dist.barrier()
+print(json.dumps({"rank": rank, "ms": ms, "value": val}), flush=True)
+dist.destroy_process_group()
+"""
+
+
+def free_port():
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    return port
+
+
+def test_max_over_ranks_and_aggregate_with_two_gloo_ranks():
+    port = free_port()
+    procs = []
+    for rank in range(2):
+        env = dict(os.environ, RANK=str(rank), WORLD_SIZE="2", MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+        procs.append(subprocess.Popen([sys.executable, "-c", WORKER % ROOT], env=env, stdout=subprocess.PIPE, text=True))
+    outs = [json.loads(p.communicate(timeout=120)[0].strip().splitlines()[-1]) for p in procs]
+    assert all(p.returncode == 0 for p in procs)
+    for o in outs:
+        assert o["ms"] == 15.0                                   # the slower rank sets the time on every rank
+        assert o["value"] == 2 * 1000 * 2 * 3 / 15.0e-3          # both replicas' zone-updates over that time
+
+
+def test_reference_arm_runs_on_rank0_only():
+    env = dict(os.environ, RANK="1", WORLD_SIZE="2", LOCAL_RANK="1")
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2", "--steps", "1",
+                        "--warmup", "0"], env=env, capture_output=True, text=True, timeout=120)
+    assert r.returncode == 0 and r.stdout.strip() == ""          # other ranks exit 0 without work
