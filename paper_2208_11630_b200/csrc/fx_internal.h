@@ -52,7 +52,7 @@ int fx_cuda_check(cudaError_t e, const char *what);
     int _rc = fx_cuda_check((call), #call);             \
     if (_rc) return _rc;                                \
   } while (0)
-#define FX_LAUNCH_CHECK(name) FX_CUDA(cudaPeekAtLastError())
+#define FX_LAUNCH_CHECK(name) FX_CUDA(cudaGetLastError())
 
 // kernel launchers (one per .cu file); all enqueue on `st`
 int fx_launch_fill_guardcells(const FxParams &P, double *U, cudaStream_t st);
@@ -63,5 +63,8 @@ int fx_launch_generic_stage(const FxParams &P, const double *X, const double *U0
                             double dt, const double *dt_dev, double beta, int first, cudaStream_t st);
 int fx_launch_debug_fluxes(const FxParams &P, const double *U, int dir, double *F, cudaStream_t st);
 bool fx_fused_supported(const FxParams &P);
+bool fx_stage_tma_supported(const FxParams &P);
+int fx_launch_stage_tma(const FxParams &P, const double *X, const double *U0, double *out, const double *dx, double dt,
+                        const double *dt_dev, double beta, int first, cudaStream_t st);
 int fx_launch_fused_stage(const FxParams &P, const double *X, const double *U0, double *out, const double *dx,
                           double dt, const double *dt_dev, double beta, int first, cudaStream_t st);

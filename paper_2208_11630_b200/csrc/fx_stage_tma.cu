@@ -1,0 +1,573 @@
+// fx_stage_tma.cu -- fused per-stage kernel for 3-D blocks with a 16 x 16 (x, y) cross-section (K1+K2+K3),
+// fed and drained by TMA.
+//
+// One 288-thread CTA per block marches the block's 16 x 16 column of zones through z; two CTAs share an SM, so
+// that one of them computes while the other waits at a barrier or for data.  Thread (i,j) of the 256 zone
+// threads owns the zones (i,j,k), k = 0..nz-1:
+//   * every plane of the stage input arrives as ONE 5-D TMA box {16,16,1,1,5} of U[v][b][k][j][i] in a
+//     2-slot shared-memory ring, two planes ahead of its use; the U0 plane (and, in later stages, the
+//     stage-input plane) of the zone being combined arrive the same way, and the finished plane leaves as
+//     one TMA box store.  No thread computes a global address inside the z loop and nothing is prefetched
+//     through registers;
+//   * z direction: a sliding window of primitive cells lives in registers; each plane is converted to
+//     primitives once and serves the z reconstruction, the z Riemann problem and, R planes later, the
+//     in-plane work of the same zone;
+//   * x and y directions: per plane the threads exchange primitives, plus-side face states and face fluxes
+//     through shared memory (three CTA barriers per plane; a face's flux overwrites the plus-side state it
+//     was computed from, in place);
+//   * a ninth "edge" warp supplies what a 16-wide row lacks: the halo cells of the plane -- TMA boxes
+//     {2|4,16,1,1,5} and {16,R,1,1,5} taken straight from the neighbour blocks' interiors through the
+//     neighbour table (or from this block's own edge at an outflow boundary; no guard cell in HBM is read or
+//     written) --, the plus-side state of cell -1 and the flux of the 17th face of every row and column.  Its
+//     lane 0 is the TMA producer.
+// HBM traffic per zone: one read of the stage input (+ U0, + the stage input again from L2 in later stages),
+// one write, plus halos.
+#include <cuda.h>
+#include <string.h>
+
+#include "fx_physics.cuh"
+
+namespace fxt {
+
+constexpr int NX = 16, NY = 16;
+constexpr int NZONE_THREADS = NX * NY;        // 256
+constexpr int NTHREADS = NZONE_THREADS + 32;  // + edge warp
+constexpr int PLANE_BYTES = 5 * NY * NX * 8;  // one TMA box of the main kind
+
+template <int RECON> struct Rc {
+  static constexpr int r = (RECON == FX_RECON_PLM_MINMOD) ? 1 : 2;  // stencil radius of one cell's reconstruction
+  static constexpr int R = r + 1;                                    // halo depth
+  static constexpr int NP = NX + 2 * R;                              // padded plane extent
+  static constexpr int BW = (R + 1) & ~1;                            // x-halo box width: TMA rows are multiples of 16 B
+  static constexpr int NREG = (RECON == FX_RECON_PLM_MINMOD) ? 96 : 168;  // registers per thread for 2 / 1 CTAs per SM: the register file is 16384 per SM sub-partition, and 18 / 9 warps put 5 / 3 on one of them
+};
+
+template <int RECON> struct alignas(128) Smem {
+  static constexpr int R = Rc<RECON>::R, NP = Rc<RECON>::NP, BW = Rc<RECON>::BW;
+  double rawX[2][5][NY][NX];   // TMA: stage-input planes, ring slot = tick & 1
+  double U0[2][5][NY][NX];     // TMA: U0 planes, slot = plane & 1
+  double Xs[5][NY][NX];        // TMA: stage-input plane of the zone being combined (later stages only)
+  double Out[5][NY][NX];       // result plane, drained by a TMA store
+  double Hx[2][2][5][NY][BW];  // TMA: [slot][lo|hi] raw x-halo cells of the plane
+  double Hy[2][2][5][R][NX];   // TMA: [slot][lo|hi] raw y-halo cells of the plane
+  double P[5][NP][NP];         // primitives of the plane incl. halo rows/columns (corners unused)
+  double Lx[5][NY][NX + 1];    // Lx[v][j][i] = plus-side x state of cell (i-1,j), then the x flux at face i-1/2
+  double Ly[5][NY + 1][NX];    // Ly[v][j][i] = plus-side y state of cell (i,j-1), then the y flux at face j-1/2
+  unsigned long long barX[2], barU[2], barH[2], barS;
+};
+
+__device__ __forceinline__ void cta_sync() { asm volatile("bar.sync 0, %0;" ::"n"(NTHREADS) : "memory"); }
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(unsigned long long *bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long *bar, int bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+// Wait for phase `parity` of the barrier.  A wait that lasts seconds means a lost TMA: trap (the launch then
+// fails with an error) rather than hang the device.
+__device__ __forceinline__ void mbar_wait(unsigned long long *bar, int parity) {
+  const unsigned a = smem_u32(bar);
+  unsigned ok;
+  int spins = 0;
+  do {
+    asm volatile(
+        "{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+        : "=r"(ok)
+        : "r"(a), "r"(parity)
+        : "memory");
+    if (!ok && ++spins > (1 << 22)) __trap();
+  } while (!ok);
+}
+__device__ __forceinline__ void tma_load(void *dst, const CUtensorMap *map, unsigned long long *bar, int c0, int c1, int c2, int c3) {
+  asm volatile(
+      "cp.async.bulk.tensor.5d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6, %7}], [%2];"
+      ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(0)
+      : "memory");
+}
+__device__ __forceinline__ void tma_store(const CUtensorMap *map, const void *src, int c0, int c1, int c2, int c3) {
+  asm volatile("cp.async.bulk.tensor.5d.global.shared::cta.tile.bulk_group [%0, {%2, %3, %4, %5, %6}], [%1];"
+               ::"l"(map), "r"(smem_u32(src)), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(0)
+               : "memory");
+}
+__device__ __forceinline__ void tma_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void tma_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void tma_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+// a3: minus/plus face states of one cell from its stencil s[0..2r] (centre s[r]).
+template <int RECON>
+__device__ __forceinline__ void recon_cell(const double *s, double eps, double &qm, double &qp) {
+  if (RECON == FX_RECON_PLM_MINMOD) {
+    fx_plm(s[0], s[1], s[2], qm, qp);
+  } else {
+    // WENO5-JS, both faces of the cell share the smoothness indicators (beta_0 <-> beta_2 under mirroring)
+    const double a = s[0], b = s[1], c = s[2], d = s[3], e = s[4];
+    const double sixth = 1.0 / 6.0;
+    const double t0 = a - 2.0 * b + c, u0 = a - 4.0 * b + 3.0 * c;
+    const double t1 = b - 2.0 * c + d, u1 = b - d;
+    const double t2 = c - 2.0 * d + e, u2 = 3.0 * c - 4.0 * d + e;
+    const double b0 = (13.0 / 12.0) * (t0 * t0) + 0.25 * (u0 * u0) + eps;
+    const double b1 = (13.0 / 12.0) * (t1 * t1) + 0.25 * (u1 * u1) + eps;
+    const double b2 = (13.0 / 12.0) * (t2 * t2) + 0.25 * (u2 * u2) + eps;
+    const double q0 = b1 * b2, q1 = b0 * b2, q2 = b0 * b1;
+    const double s0 = q0 * q0, s1 = q1 * q1, s2 = q2 * q2;  // ~ 1/b0^2, 1/b1^2, 1/b2^2 up to a common factor
+    {  // plus face: candidates from (a,b,c), (b,c,d), (c,d,e); weights 0.1, 0.6, 0.3
+      const double p0 = (2.0 * a - 7.0 * b + 11.0 * c) * sixth, p1 = (-b + 5.0 * c + 2.0 * d) * sixth,
+                   p2 = (2.0 * c + 5.0 * d - e) * sixth;
+      const double a0 = 0.1 * s0, a1 = 0.6 * s1, a2 = 0.3 * s2;
+      qp = (a0 * p0 + a1 * p1 + a2 * p2) / (a0 + a1 + a2);
+    }
+    {  // minus face: mirrored stencil (e,d,c,b,a)
+      const double p0 = (2.0 * e - 7.0 * d + 11.0 * c) * sixth, p1 = (-d + 5.0 * c + 2.0 * b) * sixth,
+                   p2 = (2.0 * c + 5.0 * b - a) * sixth;
+      const double a0 = 0.1 * s2, a1 = 0.6 * s1, a2 = 0.3 * s0;
+      qm = (a0 * p0 + a1 * p1 + a2 * p2) / (a0 + a1 + a2);
+    }
+  }
+}
+
+// Reconstruct all five primitives of one cell; st[m][v] is cell m of the stencil.  WENO positivity
+// fallback per side [A6]: a face state with rho <= 0 or p <= 0 reverts to the cell's own values.
+template <int RECON>
+__device__ __forceinline__ unsigned recon_cell5(const double (*st)[5], double eps, double qm[5], double qp[5]) {
+  constexpr int r = Rc<RECON>::r;
+#pragma unroll
+  for (int v = 0; v < 5; ++v) {
+    double s[2 * r + 1];
+#pragma unroll
+    for (int m = 0; m < 2 * r + 1; ++m) s[m] = st[m][v];
+    recon_cell<RECON>(s, eps, qm[v], qp[v]);
+  }
+  unsigned hit = 0;
+  if (RECON == FX_RECON_WENO5) {
+    if (!(qm[0] > 0.0) || !(qm[4] > 0.0)) {
+#pragma unroll
+      for (int v = 0; v < 5; ++v) qm[v] = st[r][v];
+      hit = FX_STATUS_WENO_FALLBACK;
+    }
+    if (!(qp[0] > 0.0) || !(qp[4] > 0.0)) {
+#pragma unroll
+      for (int v = 0; v < 5; ++v) qp[v] = st[r][v];
+      hit = FX_STATUS_WENO_FALLBACK;
+    }
+  }
+  return hit;
+}
+
+// Riemann flux for direction D (compile-time) from un-rotated primitive states; flux returned in the
+// un-rotated variable order (rho, mx, my, mz, E).
+template <int RIEMANN, int D>
+__device__ __forceinline__ void flux_dir(const FxParams &P, const double WL[5], const double WR[5], double F[5]) {
+  constexpr int in = 1 + D, it1 = 1 + (D + 1) % 3, it2 = 1 + (D + 2) % 3;
+  const double wl[5] = {WL[0], WL[in], WL[it1], WL[it2], WL[4]};
+  const double wr[5] = {WR[0], WR[in], WR[it1], WR[it2], WR[4]};
+  double f[5];
+  fx_riemann_v2<RIEMANN>(P, wl, wr, f);
+  F[0] = f[0];
+  F[in] = f[1];
+  F[it1] = f[2];
+  F[it2] = f[3];
+  F[4] = f[4];
+}
+
+// Where plane k (k in [-R, nz+R)) of this block's column lives: block id and padded k index.  Outflow
+// clamps to the nearest interior plane of this block [O1].
+__device__ __forceinline__ void z_source(const FxParams &P, int b, int nlo, int nhi, int k, int &bs, int &kp) {
+  const int nz = P.n[2];
+  bs = b;
+  if (k < 0) {
+    if (nlo >= 0) { bs = nlo; k += nz; } else k = 0;
+  } else if (k >= nz) {
+    if (nhi >= 0) { bs = nhi; k -= nz; } else k = nz - 1;
+  }
+  kp = k + P.gd[2];
+}
+
+template <int RECON, int RIEMANN, bool FIRST>
+__global__ void __launch_bounds__(NTHREADS) __maxnreg__(Rc<RECON>::NREG)
+fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ CUtensorMap mXx,
+               const __grid_constant__ CUtensorMap mXy, const __grid_constant__ CUtensorMap mU0,
+               const __grid_constant__ CUtensorMap mOut, const FxParams P, const double *__restrict__ X,
+               const double *__restrict__ dx, double dt, const double *__restrict__ dt_dev, double beta) {
+  constexpr int r = Rc<RECON>::r, R = Rc<RECON>::R, W = 2 * r + 1, NP = Rc<RECON>::NP, BW = Rc<RECON>::BW;
+  extern __shared__ __align__(1024) unsigned char fx_smem_raw[];  // TMA destinations need 128-byte alignment
+  Smem<RECON> &S = *reinterpret_cast<Smem<RECON> *>(fx_smem_raw);
+  const int b = blockIdx.x;
+  const int tid = threadIdx.x;
+  const int nz = P.n[2];
+  const int g0 = P.gd[0], g1 = P.gd[1], g2 = P.gd[2];
+  const int zlo = __ldg(&P.neigh[(long long)b * 6 + 4]), zhi = __ldg(&P.neigh[(long long)b * 6 + 5]);
+  unsigned hit = 0;
+
+  // ---------------------------------------------------------------- producer set-up (edge warp, lane 0)
+  const bool producer = tid == NZONE_THREADS;
+  int xlo = 0, xhi = 0, ylo = 0, yhi = 0;
+  if (tid >= NZONE_THREADS) {
+    xlo = __ldg(&P.neigh[(long long)b * 6 + 0]);
+    xhi = __ldg(&P.neigh[(long long)b * 6 + 1]);
+    ylo = __ldg(&P.neigh[(long long)b * 6 + 2]);
+    yhi = __ldg(&P.neigh[(long long)b * 6 + 3]);
+  }
+  auto issue_X = [&](int c) {  // stage-input plane consumed at tick c: z index c + r
+    int bs, kp;
+    z_source(P, b, zlo, zhi, c + r, bs, kp);
+    mbar_expect_tx(&S.barX[c & 1], PLANE_BYTES);
+    tma_load(&S.rawX[c & 1][0][0][0], &mXm, &S.barX[c & 1], g0, g1, kp, bs);
+  };
+  auto issue_H = [&](int p) {  // halo cells of interior plane p
+    const int s = p & 1, kp = p + g2;
+    mbar_expect_tx(&S.barH[s], 2 * 5 * NY * BW * 8 + 2 * 5 * R * NX * 8);
+    tma_load(&S.Hx[s][0][0][0][0], &mXx, &S.barH[s], g0 + (xlo >= 0 ? NX - BW : 0), g1, kp, xlo >= 0 ? xlo : b);
+    tma_load(&S.Hx[s][1][0][0][0], &mXx, &S.barH[s], g0 + (xhi >= 0 ? 0 : NX - BW), g1, kp, xhi >= 0 ? xhi : b);
+    tma_load(&S.Hy[s][0][0][0][0], &mXy, &S.barH[s], g0, g1 + (ylo >= 0 ? NY - R : 0), kp, ylo >= 0 ? ylo : b);
+    tma_load(&S.Hy[s][1][0][0][0], &mXy, &S.barH[s], g0, g1 + (yhi >= 0 ? 0 : NY - R), kp, yhi >= 0 ? yhi : b);
+  };
+  auto issue_U0 = [&](int p) {
+    mbar_expect_tx(&S.barU[p & 1], PLANE_BYTES);
+    tma_load(&S.U0[p & 1][0][0][0], &mU0, &S.barU[p & 1], g0, g1, p + g2, b);
+  };
+  auto issue_Xs = [&](int p) {
+    mbar_expect_tx(&S.barS, PLANE_BYTES);
+    tma_load(&S.Xs[0][0][0], &mXm, &S.barS, g0, g1, p + g2, b);
+  };
+  if (producer) {
+    mbar_init(&S.barX[0], 1); mbar_init(&S.barX[1], 1);
+    mbar_init(&S.barU[0], 1); mbar_init(&S.barU[1], 1);
+    mbar_init(&S.barH[0], 1); mbar_init(&S.barH[1], 1);
+    mbar_init(&S.barS, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    fence_async_smem();
+    issue_X(1);
+    if (nz >= 2) issue_X(2);
+    issue_H(0);
+    if (nz >= 2) issue_H(1);
+    issue_U0(0);
+    if (!FIRST) issue_Xs(0);
+  }
+  if (dt_dev) dt = __ldg(dt_dev);
+  cta_sync();  // barriers initialised before anyone waits on them
+
+  if (tid < NZONE_THREADS) {
+    // ------------------------------------------------------------ zone threads
+    const int i = tid & 15, j = tid >> 4;
+    const double rx = dt / __ldg(&dx[(long long)b * 3 + 0]), ry = dt / __ldg(&dx[(long long)b * 3 + 1]),
+                 rz = dt / __ldg(&dx[(long long)b * 3 + 2]);
+    double q[W][5];        // q[m] = primitives of cell c - r + m at tick c
+    double qpz[5], Fz[5];  // plus-side z state of cell c-1; z flux of face c-1 (between cells c-2 and c-1)
+    {
+      // prologue: cells -R .. r straight from global memory (all loads in flight together), the plus-side state
+      // of cell 0 and the flux of face 0
+      const long long col = (long long)(j + g1) * P.S_j + (i + g0);
+      double w[2 * R][5];
+#pragma unroll
+      for (int m = 0; m < 2 * R; ++m) {
+        int bs, kp;
+        z_source(P, b, zlo, zhi, m - R, bs, kp);
+        const long long a = (long long)bs * P.S_b + (long long)kp * P.S_k + col;
+#pragma unroll
+        for (int v = 0; v < 5; ++v) w[m][v] = X[a + v * P.S_v];
+      }
+#pragma unroll
+      for (int m = 0; m < 2 * R; ++m) {
+        double u[5];
+#pragma unroll
+        for (int v = 0; v < 5; ++v) u[v] = w[m][v];
+        const unsigned h = fx_c2p_v2(P, u[0], u[1], u[2], u[3], u[4], w[m]);
+        if (m >= R && m - R < nz) hit |= h;  // a zone's floor hits are counted by its owner only
+      }
+      double qm[5], qpm1[5];
+      hit |= recon_cell5<RECON>(&w[0], P.weno_eps, qm, qpm1);  // cell -1
+      hit |= recon_cell5<RECON>(&w[1], P.weno_eps, qm, qpz);   // cell 0
+      flux_dir<RIEMANN, 2>(P, qpm1, qm, Fz);
+#pragma unroll
+      for (int m = 0; m < 2 * r; ++m)
+#pragma unroll
+        for (int v = 0; v < 5; ++v) q[m][v] = w[m + 2][v];
+    }
+
+#pragma unroll 1
+    for (int c = 1; c <= nz; ++c) {
+      const int p = c - 1;  // plane of the in-plane work; its primitives are q[r-1]
+      {
+        mbar_wait(&S.barX[c & 1], ((c - 1) >> 1) & 1);
+        double u[5];
+#pragma unroll
+        for (int v = 0; v < 5; ++v) u[v] = S.rawX[c & 1][v][j][i];
+        const unsigned h = fx_c2p_v2(P, u[0], u[1], u[2], u[3], u[4], q[2 * r]);
+        if (c + r < nz) hit |= h;
+      }
+#pragma unroll
+      for (int v = 0; v < 5; ++v) S.P[v][j + R][i + R] = q[r - 1][v];
+      cta_sync();  // A: plane primitives (zone threads) and halo (edge warp) visible
+      double qmx[5], qmy[5];
+      {
+        double st[W][5], qp[5];
+#pragma unroll
+        for (int m = 0; m < W; ++m)
+#pragma unroll
+          for (int v = 0; v < 5; ++v) st[m][v] = (m == r) ? q[r - 1][v] : S.P[v][j + R][i + R + m - r];
+        hit |= recon_cell5<RECON>(st, P.weno_eps, qmx, qp);
+#pragma unroll
+        for (int v = 0; v < 5; ++v) S.Lx[v][j][i + 1] = qp[v];
+      }
+      {
+        double st[W][5], qp[5];
+#pragma unroll
+        for (int m = 0; m < W; ++m)
+#pragma unroll
+          for (int v = 0; v < 5; ++v) st[m][v] = (m == r) ? q[r - 1][v] : S.P[v][j + R + m - r][i + R];
+        hit |= recon_cell5<RECON>(st, P.weno_eps, qmy, qp);
+#pragma unroll
+        for (int v = 0; v < 5; ++v) S.Ly[v][j + 1][i] = qp[v];
+      }
+      // z: reconstruct cell c, flux of face c (between cells c-1 and c)
+      double Fz_new[5];
+      {
+        double qmz[5], qpz_new[5];
+        hit |= recon_cell5<RECON>(q, P.weno_eps, qmz, qpz_new);
+        flux_dir<RIEMANN, 2>(P, qpz, qmz, Fz_new);
+#pragma unroll
+        for (int v = 0; v < 5; ++v) qpz[v] = qpz_new[v];
+      }
+      cta_sync();  // B: plus-side states visible
+      double Fx[5], Fy[5];
+      {
+        double WL[5];
+#pragma unroll
+        for (int v = 0; v < 5; ++v) WL[v] = S.Lx[v][j][i];
+        flux_dir<RIEMANN, 0>(P, WL, qmx, Fx);
+#pragma unroll
+        for (int v = 0; v < 5; ++v) S.Lx[v][j][i] = Fx[v];  // in place: only this thread read the state
+#pragma unroll
+        for (int v = 0; v < 5; ++v) WL[v] = S.Ly[v][j][i];
+        flux_dir<RIEMANN, 1>(P, WL, qmy, Fy);
+#pragma unroll
+        for (int v = 0; v < 5; ++v) S.Ly[v][j][i] = Fy[v];
+      }
+      cta_sync();  // C: fluxes visible
+      {
+        mbar_wait(&S.barU[p & 1], (p >> 1) & 1);
+        if (!FIRST) mbar_wait(&S.barS, p & 1);
+        int hmax = 0;
+#pragma unroll
+        for (int v = 0; v < 5; ++v) {
+          const double dFx = S.Lx[v][j][i + 1] - Fx[v];
+          const double dFy = S.Ly[v][j + 1][i] - Fy[v];
+          const double dFz = Fz_new[v] - Fz[v];
+          const double u0 = S.U0[p & 1][v][j][i];
+          double res;
+          if (FIRST) {
+            res = fma(-rz, dFz, fma(-ry, dFy, fma(-rx, dFx, u0)));
+          } else {
+            const double t = fma(-rz, dFz, fma(-ry, dFy, fma(-rx, dFx, S.Xs[v][j][i] - u0)));
+            res = fma(beta, t, u0);
+          }
+          S.Out[v][j][i] = res;
+          hmax = max(hmax, __double2hiint(res) & 0x7fffffff);
+          Fz[v] = Fz_new[v];
+        }
+        if (hmax >= 0x7ff00000) hit |= FX_STATUS_NONFINITE;
+        fence_async_smem();  // the TMA store reads Out through the async proxy
+      }
+#pragma unroll
+      for (int m = 0; m < 2 * r; ++m)
+#pragma unroll
+        for (int v = 0; v < 5; ++v) q[m][v] = q[m + 1][v];
+    }
+    cta_sync();  // D: the last plane is in Out
+  } else {
+    // ------------------------------------------------------------ edge warp
+    const int lane = tid - NZONE_THREADS;
+    const bool isx = lane >= 16;
+    const int m = lane & 15;
+    const int nlo = isx ? xlo : ylo, nhi = isx ? xhi : yhi;
+    double *Pf = &S.P[0][0][0];
+    const int pd = isx ? 1 : NP, pt = isx ? NP : 1;  // smem strides of P along direction / transverse
+    double *Lf = isx ? &S.Lx[0][0][0] : &S.Ly[0][0][0];
+    const int ld = isx ? 1 : NX, lt = isx ? (NX + 1) : 1;  // strides of L along direction / transverse
+    constexpr int LV = NY * (NX + 1);                       // per-variable size of the L arrays (272)
+    // raw halo cell t of this lane's row / column: Hx[s][side][v][m][ix], Hy[s][side][v][iy][m]
+    constexpr int HXV = NY * BW, HYV = R * NX;  // per-variable sizes
+    auto halo_off = [&](int t, bool high) -> int {
+      int idx;  // cell index inside the box
+      if (isx) idx = high ? (nhi >= 0 ? t : BW - 1) : (nlo >= 0 ? BW - R + t : 0);
+      else idx = high ? (nhi >= 0 ? t : R - 1) : (nlo >= 0 ? t : 0);
+      return isx ? ((high ? 5 * HXV : 0) + m * BW + idx) : ((high ? 5 * HYV : 0) + idx * NX + m);
+    };
+    int hoff[2 * R];
+#pragma unroll
+    for (int t = 0; t < 2 * R; ++t) hoff[t] = halo_off(t % R, t >= R);
+    const int hv = isx ? HXV : HYV;
+
+#pragma unroll 1
+    for (int c = 1; c <= nz; ++c) {
+      const int p = c - 1, s = p & 1;
+      mbar_wait(&S.barH[s], (p >> 1) & 1);
+      const double *Hf = isx ? &S.Hx[s][0][0][0][0] : &S.Hy[s][0][0][0][0];
+#pragma unroll
+      for (int t = 0; t < 2 * R; ++t) {
+        double u[5], w[5];
+#pragma unroll
+        for (int v = 0; v < 5; ++v) u[v] = Hf[hoff[t] + v * hv];
+        fx_c2p_v2(P, u[0], u[1], u[2], u[3], u[4], w);
+        const int pos = (t < R) ? t : (NX + t);  // padded position along the edge direction
+#pragma unroll
+        for (int v = 0; v < 5; ++v) Pf[v * NP * NP + pos * pd + (m + R) * pt] = w[v];
+      }
+      cta_sync();  // A
+      if (lane == 0) {
+        // every slot consumed before barrier A of this tick is free again
+        if (c + 2 <= nz) issue_X(c + 2);
+        if (p + 2 < nz) issue_H(p + 2);
+        if (p >= 1) {
+          tma_store(&mOut, &S.Out[0][0][0], g0, g1, p - 1 + g2, b);
+          tma_commit();
+        }
+        if (p + 1 < nz) issue_U0(p + 1);
+        if (!FIRST && p >= 1) issue_Xs(p);
+      }
+      double qm16[5];
+      {
+        double st[W][5], qm[5], qp[5];
+        // cell -1: padded positions 0 .. 2r along the direction (cell -1 sits at R-1 = r)
+#pragma unroll
+        for (int mm = 0; mm < W; ++mm)
+#pragma unroll
+          for (int v = 0; v < 5; ++v) st[mm][v] = Pf[v * NP * NP + mm * pd + (m + R) * pt];
+        hit |= recon_cell5<RECON>(st, P.weno_eps, qm, qp);
+#pragma unroll
+        for (int v = 0; v < 5; ++v) Lf[v * LV + 0 * ld + m * lt] = qp[v];
+        // cell 16: padded positions 16+R-r .. 16+R+r
+#pragma unroll
+        for (int mm = 0; mm < W; ++mm)
+#pragma unroll
+          for (int v = 0; v < 5; ++v) st[mm][v] = Pf[v * NP * NP + (NX + R - r + mm) * pd + (m + R) * pt];
+        hit |= recon_cell5<RECON>(st, P.weno_eps, qm16, qp);
+      }
+      cta_sync();  // B
+      {
+        double WL[5];
+#pragma unroll
+        for (int v = 0; v < 5; ++v) WL[v] = Lf[v * LV + NX * ld + m * lt];
+        const double wl[5] = {WL[0], isx ? WL[1] : WL[2], isx ? WL[2] : WL[3], isx ? WL[3] : WL[1], WL[4]};
+        const double wr[5] = {qm16[0], isx ? qm16[1] : qm16[2], isx ? qm16[2] : qm16[3], isx ? qm16[3] : qm16[1], qm16[4]};
+        double f[5];
+        fx_riemann_v2<RIEMANN>(P, wl, wr, f);
+        double F[5];
+        F[0] = f[0];
+        F[1] = isx ? f[1] : f[3];
+        F[2] = isx ? f[2] : f[1];
+        F[3] = isx ? f[3] : f[2];
+        F[4] = f[4];
+#pragma unroll
+        for (int v = 0; v < 5; ++v) Lf[v * LV + NX * ld + m * lt] = F[v];
+      }
+      if (lane == 0 && p >= 1) tma_wait_read();  // Out is free for the combine after barrier C
+      cta_sync();  // C
+    }
+    cta_sync();  // D
+    if (lane == 0) {
+      tma_store(&mOut, &S.Out[0][0][0], g0, g1, nz - 1 + g2, b);
+      tma_commit();
+      tma_wait_all();
+    }
+  }
+  if (hit) fx_note(P, hit);
+}
+
+// ------------------------------------------------------------------ host side: tensor maps and launch
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                  const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static EncodeTiledFn encode_fn() {
+  static EncodeTiledFn fn = nullptr;
+  static bool tried = false;
+  if (!tried) {
+    tried = true;
+    void *p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+        q == cudaDriverEntryPointSuccess)
+      fn = (EncodeTiledFn)p;
+  }
+  return fn;
+}
+
+// 5-D view of a state array, U[v][b][k][j][i] (i fastest), with a box of bx x by zones of all five variables.
+static int make_map(CUtensorMap *m, const FxParams &P, const double *base, int bx, int by) {
+  EncodeTiledFn fn = encode_fn();
+  if (!fn) return fx_fail(FX_ERR_CUDA, "stage kernel: cuTensorMapEncodeTiled is not available from this driver");
+  const cuuint64_t dims[5] = {(cuuint64_t)P.np[0], (cuuint64_t)P.np[1], (cuuint64_t)P.np[2], (cuuint64_t)P.nblocks, 5};
+  const cuuint64_t strides[4] = {(cuuint64_t)P.S_j * 8, (cuuint64_t)P.S_k * 8, (cuuint64_t)P.S_b * 8, (cuuint64_t)P.S_v * 8};
+  const cuuint32_t box[5] = {(cuuint32_t)bx, (cuuint32_t)by, 1, 1, 5};
+  const cuuint32_t es[5] = {1, 1, 1, 1, 1};
+  const CUresult rc = fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 5, (void *)base, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                         CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (rc != CUDA_SUCCESS) return fx_fail(FX_ERR_CUDA, "stage kernel: cuTensorMapEncodeTiled failed with code %d", (int)rc);
+  return FX_OK;
+}
+
+template <int RECON, int RIEMANN, bool FIRST>
+int launch(const FxParams &P, const double *X, const double *U0, double *out, const double *dx, double dt, const double *dt_dev,
+           double beta, cudaStream_t st) {
+  constexpr int R = Rc<RECON>::R, BW = Rc<RECON>::BW;
+  CUtensorMap mXm, mXx, mXy, mU0, mOut;
+  int rc;
+  if ((rc = make_map(&mXm, P, X, NX, NY))) return rc;
+  if ((rc = make_map(&mXx, P, X, BW, NY))) return rc;
+  if ((rc = make_map(&mXy, P, X, NX, R))) return rc;
+  if ((rc = make_map(&mU0, P, U0, NX, NY))) return rc;
+  if ((rc = make_map(&mOut, P, out, NX, NY))) return rc;
+  auto kern = fx_k_stage_tma<RECON, RIEMANN, FIRST>;
+  const int smem = (int)sizeof(Smem<RECON>);
+  static bool configured = false;  // per instantiation
+  if (!configured) {
+    FX_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    configured = true;
+  }
+  kern<<<(unsigned)P.nblocks, NTHREADS, smem, st>>>(mXm, mXx, mXy, mU0, mOut, P, X, dx, dt, dt_dev, beta);
+  const cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) {
+    cudaFuncAttributes a;
+    memset(&a, 0, sizeof(a));
+    cudaFuncGetAttributes(&a, kern);
+    cudaGetLastError();
+    return fx_fail(FX_ERR_CUDA, "stage_tma launch: %s (regs %d, threads %d of max %d, smem dynamic %d of max %d + static %d)",
+                   cudaGetErrorString(e), a.numRegs, NTHREADS, a.maxThreadsPerBlock, smem, a.maxDynamicSharedSizeBytes,
+                   (int)a.sharedSizeBytes);
+  }
+  return FX_OK;
+}
+
+template <int RECON, int RIEMANN>
+int launch_rr(const FxParams &P, const double *X, const double *U0, double *out, const double *dx, double dt, const double *dt_dev,
+              double beta, int first, cudaStream_t st) {
+  return first ? launch<RECON, RIEMANN, true>(P, X, U0, out, dx, dt, dt_dev, beta, st)
+               : launch<RECON, RIEMANN, false>(P, X, U0, out, dx, dt, dt_dev, beta, st);
+}
+
+}  // namespace fxt
+
+bool fx_stage_tma_supported(const FxParams &P) {
+  const int R = P.recon == FX_RECON_WENO5 ? 3 : 2;
+  // TMA: global strides must be multiples of 16 bytes (S_j even), the arrays 16-byte aligned (checked at launch)
+  return P.n[0] == fxt::NX && P.n[1] == fxt::NY && P.n[2] >= R && P.active[2] && P.gd[0] >= R && (P.S_j % 2) == 0 &&
+         P.nblocks <= 0x7fffffffLL;
+}
+
+int fx_launch_stage_tma(const FxParams &P, const double *X, const double *U0, double *out, const double *dx, double dt,
+                        const double *dt_dev, double beta, int first, cudaStream_t st) {
+  if (!fx_stage_tma_supported(P)) return fx_fail(FX_ERR_UNSUPPORTED, "TMA stage kernel: block shape not supported");
+  if (P.nblocks == 0) return FX_OK;
+  if (((uintptr_t)X | (uintptr_t)U0 | (uintptr_t)out) & 15)
+    return fx_fail(FX_ERR_INVALID_ARG, "TMA stage kernel: state arrays must be 16-byte aligned");
+  if (P.recon == FX_RECON_PLM_MINMOD) {
+    if (P.riemann == FX_RIEMANN_HLLE) return fxt::launch_rr<FX_RECON_PLM_MINMOD, FX_RIEMANN_HLLE>(P, X, U0, out, dx, dt, dt_dev, beta, first, st);
+    return fxt::launch_rr<FX_RECON_PLM_MINMOD, FX_RIEMANN_HLLC>(P, X, U0, out, dx, dt, dt_dev, beta, first, st);
+  }
+  if (P.riemann == FX_RIEMANN_HLLE) return fxt::launch_rr<FX_RECON_WENO5, FX_RIEMANN_HLLE>(P, X, U0, out, dx, dt, dt_dev, beta, first, st);
+  return fxt::launch_rr<FX_RECON_WENO5, FX_RIEMANN_HLLC>(P, X, U0, out, dx, dt, dt_dev, beta, first, st);
+}
