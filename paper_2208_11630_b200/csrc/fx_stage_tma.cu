@@ -158,13 +158,13 @@ __device__ __forceinline__ unsigned recon_cell5(const double (*st)[5], double ep
 
 // Riemann flux for direction D (compile-time) from un-rotated primitive states; flux returned in the
 // un-rotated variable order (rho, mx, my, mz, E).
-template <int RIEMANN, int D>
+template <int RIEMANN, int WS, int D>
 __device__ __forceinline__ void flux_dir(const FxParams &P, const double WL[5], const double WR[5], double F[5]) {
   constexpr int in = 1 + D, it1 = 1 + (D + 1) % 3, it2 = 1 + (D + 2) % 3;
   const double wl[5] = {WL[0], WL[in], WL[it1], WL[it2], WL[4]};
   const double wr[5] = {WR[0], WR[in], WR[it1], WR[it2], WR[4]};
   double f[5];
-  fx_riemann_v2<RIEMANN>(P, wl, wr, f);
+  fx_riemann_v2<RIEMANN, WS>(P, wl, wr, f);
   F[0] = f[0];
   F[in] = f[1];
   F[it1] = f[2];
@@ -185,7 +185,7 @@ __device__ __forceinline__ void z_source(const FxParams &P, int b, int nlo, int 
   kp = k + P.gd[2];
 }
 
-template <int RECON, int RIEMANN, bool FIRST>
+template <int RECON, int RIEMANN, int WS, bool FIRST>
 __global__ void __launch_bounds__(NTHREADS) __maxnreg__(Rc<RECON>::NREG)
 fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ CUtensorMap mXx,
                const __grid_constant__ CUtensorMap mXy, const __grid_constant__ CUtensorMap mU0,
@@ -280,7 +280,7 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
       double qm[5], qpm1[5];
       hit |= recon_cell5<RECON>(&w[0], P.weno_eps, qm, qpm1);  // cell -1
       hit |= recon_cell5<RECON>(&w[1], P.weno_eps, qm, qpz);   // cell 0
-      flux_dir<RIEMANN, 2>(P, qpm1, qm, Fz);
+      flux_dir<RIEMANN, WS, 2>(P, qpm1, qm, Fz);
 #pragma unroll
       for (int m = 0; m < 2 * r; ++m)
 #pragma unroll
@@ -327,7 +327,7 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
       {
         double qmz[5], qpz_new[5];
         hit |= recon_cell5<RECON>(q, P.weno_eps, qmz, qpz_new);
-        flux_dir<RIEMANN, 2>(P, qpz, qmz, Fz_new);
+        flux_dir<RIEMANN, WS, 2>(P, qpz, qmz, Fz_new);
 #pragma unroll
         for (int v = 0; v < 5; ++v) qpz[v] = qpz_new[v];
       }
@@ -337,12 +337,12 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
         double WL[5];
 #pragma unroll
         for (int v = 0; v < 5; ++v) WL[v] = S.Lx[v][j][i];
-        flux_dir<RIEMANN, 0>(P, WL, qmx, Fx);
+        flux_dir<RIEMANN, WS, 0>(P, WL, qmx, Fx);
 #pragma unroll
         for (int v = 0; v < 5; ++v) S.Lx[v][j][i] = Fx[v];  // in place: only this thread read the state
 #pragma unroll
         for (int v = 0; v < 5; ++v) WL[v] = S.Ly[v][j][i];
-        flux_dir<RIEMANN, 1>(P, WL, qmy, Fy);
+        flux_dir<RIEMANN, WS, 1>(P, WL, qmy, Fy);
 #pragma unroll
         for (int v = 0; v < 5; ++v) S.Ly[v][j][i] = Fy[v];
       }
@@ -454,7 +454,7 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
         const double wl[5] = {WL[0], isx ? WL[1] : WL[2], isx ? WL[2] : WL[3], isx ? WL[3] : WL[1], WL[4]};
         const double wr[5] = {qm16[0], isx ? qm16[1] : qm16[2], isx ? qm16[2] : qm16[3], isx ? qm16[3] : qm16[1], qm16[4]};
         double f[5];
-        fx_riemann_v2<RIEMANN>(P, wl, wr, f);
+        fx_riemann_v2<RIEMANN, WS>(P, wl, wr, f);
         double F[5];
         F[0] = f[0];
         F[1] = isx ? f[1] : f[3];
@@ -510,7 +510,7 @@ static int make_map(CUtensorMap *m, const FxParams &P, const double *base, int b
   return FX_OK;
 }
 
-template <int RECON, int RIEMANN, bool FIRST>
+template <int RECON, int RIEMANN, int WS, bool FIRST>
 int launch(const FxParams &P, const double *X, const double *U0, double *out, const double *dx, double dt, const double *dt_dev,
            double beta, cudaStream_t st) {
   constexpr int R = Rc<RECON>::R, BW = Rc<RECON>::BW;
@@ -521,7 +521,7 @@ int launch(const FxParams &P, const double *X, const double *U0, double *out, co
   if ((rc = make_map(&mXy, P, X, NX, R))) return rc;
   if ((rc = make_map(&mU0, P, U0, NX, NY))) return rc;
   if ((rc = make_map(&mOut, P, out, NX, NY))) return rc;
-  auto kern = fx_k_stage_tma<RECON, RIEMANN, FIRST>;
+  auto kern = fx_k_stage_tma<RECON, RIEMANN, WS, FIRST>;
   const int smem = (int)sizeof(Smem<RECON>);
   static bool configured = false;  // per instantiation
   if (!configured) {
@@ -545,8 +545,11 @@ int launch(const FxParams &P, const double *X, const double *U0, double *out, co
 template <int RECON, int RIEMANN>
 int launch_rr(const FxParams &P, const double *X, const double *U0, double *out, const double *dx, double dt, const double *dt_dev,
               double beta, int first, cudaStream_t st) {
-  return first ? launch<RECON, RIEMANN, true>(P, X, U0, out, dx, dt, dt_dev, beta, st)
-               : launch<RECON, RIEMANN, false>(P, X, U0, out, dx, dt, dt_dev, beta, st);
+  if (P.wavespeed == 0)
+    return first ? launch<RECON, RIEMANN, 0, true>(P, X, U0, out, dx, dt, dt_dev, beta, st)
+                 : launch<RECON, RIEMANN, 0, false>(P, X, U0, out, dx, dt, dt_dev, beta, st);
+  return first ? launch<RECON, RIEMANN, 1, true>(P, X, U0, out, dx, dt, dt_dev, beta, st)
+               : launch<RECON, RIEMANN, 1, false>(P, X, U0, out, dx, dt, dt_dev, beta, st);
 }
 
 }  // namespace fxt
