@@ -40,7 +40,7 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=5)
     ap.add_argument("--nb", default=None, help="override blocks per dimension, e.g. 16,16,16")
-    ap.add_argument("--path", type=int, default=0, help="FX_OPT_PATH: 0 auto (TMA stage kernel when supported), 1 generic, 2 register/LDG fused kernel")
+    ap.add_argument("--path", type=int, default=0, help="FX_OPT_PATH: 0 auto (fused TMA stage kernel when supported), 1 generic")
     ap.add_argument("--order", default="morton", choices=["lex", "morton"])
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -271,7 +271,7 @@ def run_ours(args, rank, world, local_rank):
                                    f"{cfg.block_dims[0]}x{cfg.block_dims[1]}x{cfg.block_dims[2]} (+{cfg.nguard} guard), "
                                    f"{'WENO5' if cfg.recon else 'PLM-minmod'}+{'HLLC' if cfg.riemann else 'HLLE'}, SSP-RK{stages}",
                        "interior_zones": zones, "state_bytes": plan.bytes_per_state, "block_order": args.order,
-                       "path": {0: "generic", 1: "fused (register/LDG)", 2: "fused (TMA)"}[plan.path], "l2": "inputs (state) larger than L2; no flush needed",
+                       "path": {0: "generic", 1: "fused (TMA)"}[plan.path], "l2": "inputs (state) larger than L2; no flush needed",
                        "multi_gpu": "replicas only" if world > 1 else "single"},
             "clocks": clocks, "gpu_launches": launches_per_step * args.steps, "roofline": roofline,
             "status_flags": flags}

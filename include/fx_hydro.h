@@ -48,7 +48,7 @@ enum {
   FX_OPT_P_FLOOR = 1,   /* primitive pressure floor, default 1e-12 [A7] */
   FX_OPT_WENO_EPS = 2,  /* WENO5-JS epsilon, default 1e-6 [A5] */
   FX_OPT_WAVESPEED = 3, /* 0 = Einfeldt (default), 1 = Davis [A8] */
-  FX_OPT_PATH = 4       /* 0 = auto (fused stage kernel when the block shape allows), 1 = generic */
+  FX_OPT_PATH = 4       /* 0 = auto (fused TMA stage kernel when the block shape allows), 1 = generic */
 };
 enum {
   FX_STATUS_NONFINITE = 1u,
@@ -155,7 +155,8 @@ int fx_hydro_status_reset(fx_hydro_plan *plan, void *stream);
 int fx_debug_compute_fluxes(fx_hydro_plan *plan, const double *U_dev, int dir, double *F_dev, void *stream);
 
 /* Which stage kernel fx_hydro_advance will use for this plan: 0 generic (guard fill + zone kernel),
- * 1 fused (halo gathered from neighbour interiors inside the stage kernel). */
+ * 1 fused and TMA-fed (16 x 16 x nz blocks: halos gathered from neighbour interiors inside the stage kernel,
+ * every plane moved by TMA). */
 int fx_hydro_plan_path(const fx_hydro_plan *plan);
 
 /* Measurement aid: when enabled, fx_hydro_advance brackets every stage-kernel launch (the dominant

@@ -4,7 +4,7 @@
 // interior zone computes the two face fluxes of each active direction from the padded stage input
 // (each face is evaluated by both zones that share it, bit-identically, so conservation holds to
 // rounding), forms S = sum_d dt/dx_d (F+ - F-) and the SSP-RK combination.  It is the path for block
-// shapes the fused kernel (fx_fused.cu) does not cover (configs 1 and 2) and the scaffold its parity is
+// shapes the fused kernel (fx_stage_tma.cu) does not cover (configs 1 and 2) and the scaffold its parity is
 // checked against; it is not the roofline path.
 #include "fx_physics.cuh"
 

@@ -62,9 +62,6 @@ int fx_launch_compute_dt(const FxParams &P, const double *U, const double *dx, d
 int fx_launch_generic_stage(const FxParams &P, const double *X, const double *U0, double *out, const double *dx,
                             double dt, const double *dt_dev, double beta, int first, cudaStream_t st);
 int fx_launch_debug_fluxes(const FxParams &P, const double *U, int dir, double *F, cudaStream_t st);
-bool fx_fused_supported(const FxParams &P);
 bool fx_stage_tma_supported(const FxParams &P);
 int fx_launch_stage_tma(const FxParams &P, const double *X, const double *U0, double *out, const double *dx, double dt,
                         const double *dt_dev, double beta, int first, cudaStream_t st);
-int fx_launch_fused_stage(const FxParams &P, const double *X, const double *U0, double *out, const double *dx,
-                          double dt, const double *dt_dev, double beta, int first, cudaStream_t st);

@@ -41,8 +41,7 @@ extern "C" int fx_hydro_compute_dt(fx_hydro_plan *plan, const double *U, const d
 // gathered from neighbour interiors inside the fused kernel.
 static int fx_stage(fx_hydro_plan *plan, double *X, const double *U0, double *out, const double *dx, double dt,
                     const double *dt_dev, double beta, int first, cudaStream_t st) {
-  const int path = fx_hydro_plan_path(plan);
-  const bool fused = path >= 1;
+  const bool fused = fx_hydro_plan_path(plan) == 1;
   int rc = FX_OK;
   if (!fused) {
     rc = fx_launch_fill_guardcells(plan->P, X, st);  // O1 on the stage input before every S(.) [A15]
@@ -50,9 +49,8 @@ static int fx_stage(fx_hydro_plan *plan, double *X, const double *U0, double *ou
   }
   const bool rec = plan->timing && plan->ev && plan->nrec < FX_MAX_REC;
   if (rec) FX_CUDA(cudaEventRecord(plan->ev[2 * plan->nrec], st));
-  rc = path == 2   ? fx_launch_stage_tma(plan->P, X, U0, out, dx, dt, dt_dev, beta, first, st)
-       : path == 1 ? fx_launch_fused_stage(plan->P, X, U0, out, dx, dt, dt_dev, beta, first, st)
-                   : fx_launch_generic_stage(plan->P, X, U0, out, dx, dt, dt_dev, beta, first, st);
+  rc = fused ? fx_launch_stage_tma(plan->P, X, U0, out, dx, dt, dt_dev, beta, first, st)
+             : fx_launch_generic_stage(plan->P, X, U0, out, dx, dt, dt_dev, beta, first, st);
   if (rc) return rc;
   if (rec) {
     FX_CUDA(cudaEventRecord(plan->ev[2 * plan->nrec + 1], st));
