@@ -50,9 +50,11 @@ template <int RECON> struct alignas(128) Smem {
   double Out[5][NY][NX];       // result plane, drained by a TMA store
   double Hx[2][2][5][NY][BW];  // TMA: [slot][lo|hi] raw x-halo cells of the plane
   double Hy[2][2][5][R][NX];   // TMA: [slot][lo|hi] raw y-halo cells of the plane
-  double P[5][NP][NP];         // primitives of the plane incl. halo rows/columns (corners unused)
+  double P[5][NP][NP + 1];     // primitives of the plane incl. halo rows/columns (corners unused); the odd row
+                               // stride keeps the edge warp's column accesses free of bank conflicts
   double Lx[5][NY][NX + 1];    // Lx[v][j][i] = plus-side x state of cell (i-1,j), then the x flux at face i-1/2
   double Ly[5][NY + 1][NX];    // Ly[v][j][i] = plus-side y state of cell (i,j-1), then the y flux at face j-1/2
+  double rd[3];                // beta dt / dx_d of this block (beta = 1 in the first stage)
   unsigned long long barX[2], barU[2], barH[2], barS;
 };
 
@@ -247,13 +249,12 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
     if (!FIRST) issue_Xs(0);
   }
   if (dt_dev) dt = __ldg(dt_dev);
-  cta_sync();  // barriers initialised before anyone waits on them
+  if (tid < 3) S.rd[tid] = (FIRST ? 1.0 : beta) * dt / __ldg(&dx[(long long)b * 3 + tid]);
+  cta_sync();  // barriers initialised before anyone waits on them; rd visible
 
   if (tid < NZONE_THREADS) {
     // ------------------------------------------------------------ zone threads
     const int i = tid & 15, j = tid >> 4;
-    const double rx = dt / __ldg(&dx[(long long)b * 3 + 0]), ry = dt / __ldg(&dx[(long long)b * 3 + 1]),
-                 rz = dt / __ldg(&dx[(long long)b * 3 + 2]);
     double q[W][5];        // q[m] = primitives of cell c - r + m at tick c
     double qpz[5], Fz[5];  // plus-side z state of cell c-1; z flux of face c-1 (between cells c-2 and c-1)
     {
@@ -350,6 +351,8 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
       {
         mbar_wait(&S.barU[p & 1], (p >> 1) & 1);
         if (!FIRST) mbar_wait(&S.barS, p & 1);
+        // out = [U0 + beta (X - U0)] - sum_d (beta dt/dx_d) (F_d+ - F_d-)
+        const double rx = S.rd[0], ry = S.rd[1], rz = S.rd[2];
         int hmax = 0;
 #pragma unroll
         for (int v = 0; v < 5; ++v) {
@@ -357,13 +360,8 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
           const double dFy = S.Ly[v][j + 1][i] - Fy[v];
           const double dFz = Fz_new[v] - Fz[v];
           const double u0 = S.U0[p & 1][v][j][i];
-          double res;
-          if (FIRST) {
-            res = fma(-rz, dFz, fma(-ry, dFy, fma(-rx, dFx, u0)));
-          } else {
-            const double t = fma(-rz, dFz, fma(-ry, dFy, fma(-rx, dFx, S.Xs[v][j][i] - u0)));
-            res = fma(beta, t, u0);
-          }
+          const double a = FIRST ? u0 : fma(beta, S.Xs[v][j][i] - u0, u0);
+          const double res = fma(-rz, dFz, fma(-ry, dFy, fma(-rx, dFx, a)));
           S.Out[v][j][i] = res;
           hmax = max(hmax, __double2hiint(res) & 0x7fffffff);
           Fz[v] = Fz_new[v];
@@ -384,7 +382,8 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
     const int m = lane & 15;
     const int nlo = isx ? xlo : ylo, nhi = isx ? xhi : yhi;
     double *Pf = &S.P[0][0][0];
-    const int pd = isx ? 1 : NP, pt = isx ? NP : 1;  // smem strides of P along direction / transverse
+    constexpr int NPS = NP + 1;
+    const int pd = isx ? 1 : NPS, pt = isx ? NPS : 1;  // smem strides of P along direction / transverse
     double *Lf = isx ? &S.Lx[0][0][0] : &S.Ly[0][0][0];
     const int ld = isx ? 1 : NX, lt = isx ? (NX + 1) : 1;  // strides of L along direction / transverse
     constexpr int LV = NY * (NX + 1);                       // per-variable size of the L arrays (272)
@@ -414,7 +413,7 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
         fx_c2p_v2(P, u[0], u[1], u[2], u[3], u[4], w);
         const int pos = (t < R) ? t : (NX + t);  // padded position along the edge direction
 #pragma unroll
-        for (int v = 0; v < 5; ++v) Pf[v * NP * NP + pos * pd + (m + R) * pt] = w[v];
+        for (int v = 0; v < 5; ++v) Pf[v * NP * NPS + pos * pd + (m + R) * pt] = w[v];
       }
       cta_sync();  // A
       if (lane == 0) {
@@ -435,7 +434,7 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
 #pragma unroll
         for (int mm = 0; mm < W; ++mm)
 #pragma unroll
-          for (int v = 0; v < 5; ++v) st[mm][v] = Pf[v * NP * NP + mm * pd + (m + R) * pt];
+          for (int v = 0; v < 5; ++v) st[mm][v] = Pf[v * NP * NPS + mm * pd + (m + R) * pt];
         hit |= recon_cell5<RECON>(st, P.weno_eps, qm, qp);
 #pragma unroll
         for (int v = 0; v < 5; ++v) Lf[v * LV + 0 * ld + m * lt] = qp[v];
@@ -443,7 +442,7 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
 #pragma unroll
         for (int mm = 0; mm < W; ++mm)
 #pragma unroll
-          for (int v = 0; v < 5; ++v) st[mm][v] = Pf[v * NP * NP + (NX + R - r + mm) * pd + (m + R) * pt];
+          for (int v = 0; v < 5; ++v) st[mm][v] = Pf[v * NP * NPS + (NX + R - r + mm) * pd + (m + R) * pt];
         hit |= recon_cell5<RECON>(st, P.weno_eps, qm16, qp);
       }
       cta_sync();  // B
