@@ -55,7 +55,7 @@ template <int RECON> struct alignas(128) Smem {
   double Lx[5][NY][NX + 1];    // Lx[v][j][i] = plus-side x state of cell (i-1,j), then the x flux at face i-1/2
   double Ly[5][NY + 1][NX];    // Ly[v][j][i] = plus-side y state of cell (i,j-1), then the y flux at face j-1/2
   double rd[3];                // beta dt / dx_d of this block (beta = 1 in the first stage)
-  unsigned long long barX[2], barU[2], barH[2], barS;
+  unsigned long long barX[2], barH[2], barS;  // barX[c & 1]: stage-input plane of tick c AND the U0 plane of plane c - 1
 };
 
 __device__ __forceinline__ void cta_sync() { asm volatile("bar.sync 0, %0;" ::"n"(NTHREADS) : "memory"); }
@@ -227,16 +227,16 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
     tma_load(&S.Hy[s][1][0][0][0], &mXy, &S.barH[s], g0, g1 + (yhi >= 0 ? 0 : NY - R), kp, yhi >= 0 ? yhi : b);
   };
   auto issue_U0 = [&](int p) {
-    mbar_expect_tx(&S.barU[p & 1], PLANE_BYTES);
-    tma_load(&S.U0[p & 1][0][0][0], &mU0, &S.barU[p & 1], g0, g1, p + g2, b);
+    // completes on the barrier of tick p + 1, the tick that combines plane p: one wait per tick covers both loads
+    mbar_expect_tx(&S.barX[(p + 1) & 1], PLANE_BYTES);
+    tma_load(&S.U0[p & 1][0][0][0], &mU0, &S.barX[(p + 1) & 1], g0, g1, p + g2, b);
   };
   auto issue_Xs = [&](int p) {
     mbar_expect_tx(&S.barS, PLANE_BYTES);
     tma_load(&S.Xs[0][0][0], &mXm, &S.barS, g0, g1, p + g2, b);
   };
   if (producer) {
-    mbar_init(&S.barX[0], 1); mbar_init(&S.barX[1], 1);
-    mbar_init(&S.barU[0], 1); mbar_init(&S.barU[1], 1);
+    mbar_init(&S.barX[0], 2); mbar_init(&S.barX[1], 2);  // two arrivals per tick: issue_X(c) and issue_U0(c - 1)
     mbar_init(&S.barH[0], 1); mbar_init(&S.barH[1], 1);
     mbar_init(&S.barS, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -349,7 +349,6 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
       }
       cta_sync();  // C: fluxes visible
       {
-        mbar_wait(&S.barU[p & 1], (p >> 1) & 1);
         if (!FIRST) mbar_wait(&S.barS, p & 1);
         // out = [U0 + beta (X - U0)] - sum_d (beta dt/dx_d) (F_d+ - F_d-)
         const double rx = S.rd[0], ry = S.rd[1], rz = S.rd[2];
