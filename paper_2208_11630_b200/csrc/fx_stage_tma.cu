@@ -288,6 +288,10 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
         for (int v = 0; v < 5; ++v) q[m][v] = w[m + 2][v];
     }
 
+#pragma unroll
+    for (int v = 0; v < 5; ++v) S.P[v][j + R][i + R] = q[r - 1][v];  // plane 0
+    cta_sync();  // A0: plane 0 and its halo (edge warp) visible
+
 #pragma unroll 1
     for (int c = 1; c <= nz; ++c) {
       const int p = c - 1;  // plane of the in-plane work; its primitives are q[r-1]
@@ -299,9 +303,6 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
         const unsigned h = fx_c2p_v2(P, u[0], u[1], u[2], u[3], u[4], q[2 * r]);
         if (c + r < nz) hit |= h;
       }
-#pragma unroll
-      for (int v = 0; v < 5; ++v) S.P[v][j + R][i + R] = q[r - 1][v];
-      cta_sync();  // A: plane primitives (zone threads) and halo (edge warp) visible
       double qmx[5], qmy[5];
       {
         double st[W][5], qp[5];
@@ -347,7 +348,11 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
 #pragma unroll
         for (int v = 0; v < 5; ++v) S.Ly[v][j][i] = Fy[v];
       }
-      cta_sync();  // C: fluxes visible
+      if (c < nz) {  // primitives of plane p + 1 (cell c of the window): nobody reads P between barriers B and C
+#pragma unroll
+        for (int v = 0; v < 5; ++v) S.P[v][j + R][i + R] = q[r][v];
+      }
+      cta_sync();  // C: fluxes and the next plane's primitives visible
       {
         if (!FIRST) mbar_wait(&S.barS, p & 1);
         // out = [U0 + beta (X - U0)] - sum_d (beta dt/dx_d) (F_d+ - F_d-)
@@ -399,10 +404,9 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
     for (int t = 0; t < 2 * R; ++t) hoff[t] = halo_off(t % R, t >= R);
     const int hv = isx ? HXV : HYV;
 
-#pragma unroll 1
-    for (int c = 1; c <= nz; ++c) {
-      const int p = c - 1, s = p & 1;
-      mbar_wait(&S.barH[s], (p >> 1) & 1);
+    auto halo_plane = [&](int pl) {  // primitives of the halo cells of plane pl into P
+      const int s = pl & 1;
+      mbar_wait(&S.barH[s], (pl >> 1) & 1);
       const double *Hf = isx ? &S.Hx[s][0][0][0][0] : &S.Hy[s][0][0][0][0];
 #pragma unroll
       for (int t = 0; t < 2 * R; ++t) {
@@ -414,18 +418,13 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
 #pragma unroll
         for (int v = 0; v < 5; ++v) Pf[v * NP * NPS + pos * pd + (m + R) * pt] = w[v];
       }
-      cta_sync();  // A
-      if (lane == 0) {
-        // every slot consumed before barrier A of this tick is free again
-        if (c + 2 <= nz) issue_X(c + 2);
-        if (p + 2 < nz) issue_H(p + 2);
-        if (p >= 1) {
-          tma_store(&mOut, &S.Out[0][0][0], g0, g1, p - 1 + g2, b);
-          tma_commit();
-        }
-        if (p + 1 < nz) issue_U0(p + 1);
-        if (!FIRST && p >= 1) issue_Xs(p);
-      }
+    };
+    halo_plane(0);
+    cta_sync();  // A0
+
+#pragma unroll 1
+    for (int c = 1; c <= nz; ++c) {
+      const int p = c - 1;
       double qm16[5];
       {
         double st[W][5], qm[5], qp[5];
@@ -445,6 +444,17 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
         hit |= recon_cell5<RECON>(st, P.weno_eps, qm16, qp);
       }
       cta_sync();  // B
+      if (lane == 0) {
+        // every slot consumed before barrier B of this tick is free again
+        if (c + 2 <= nz) issue_X(c + 2);
+        if (p + 2 < nz) issue_H(p + 2);
+        if (p >= 1) {
+          tma_store(&mOut, &S.Out[0][0][0], g0, g1, p - 1 + g2, b);
+          tma_commit();
+        }
+        if (p + 1 < nz) issue_U0(p + 1);
+        if (!FIRST && p >= 1) issue_Xs(p);
+      }
       {
         double WL[5];
 #pragma unroll
@@ -462,6 +472,7 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
 #pragma unroll
         for (int v = 0; v < 5; ++v) Lf[v * LV + NX * ld + m * lt] = F[v];
       }
+      if (c < nz) halo_plane(c);                  // halo of plane p + 1: nobody reads P between barriers B and C
       if (lane == 0 && p >= 1) tma_wait_read();  // Out is free for the combine after barrier C
       cta_sync();  // C
     }
