@@ -159,7 +159,7 @@ extern "C" int fx_hydro_plan_set_workspace(fx_hydro_plan *plan, void *ws, size_t
     return fx_fail(FX_ERR_WORKSPACE, "set_workspace: %zu bytes given, %zu needed", bytes, fx_hydro_plan_workspace_bytes(plan));
   unsigned long long init[FX_SCR_WORDS];
   memset(init, 0, sizeof(init));
-  init[FX_SCR_DTBITS] = 0x7ff0000000000000ull;  // +inf
+  init[FX_SCR_DTBITS] = 0ull;  // running max of (|u|+c)/dx: 0
   FX_CUDA(cudaMemcpy(ws, init, sizeof(init), cudaMemcpyHostToDevice));
   FX_CUDA(cudaDeviceSynchronize());
   plan->workspace = ws;

@@ -72,43 +72,65 @@ int fx_launch_index_map(const FxParams &P, long long b0, long long nb, long long
 }
 
 // ------------------------------------------------------------------ a7 CFL reduction
-// Each thread folds several interior zones; warp-shuffle min; one atomicMin per CTA on the bit pattern
-// (non-negative doubles order like unsigned integers); the last CTA to finish writes cfl*min and re-arms
-// the scratch words for the next call.
+// dt = cfl * min over zones and active d of dx_d / (|u_d| + c)  =  cfl / max (|u_d| + c) (1 / dx_d).
+// One CTA walks whole blocks (1/dx_d once per block, 32-bit index arithmetic inside a block); every thread keeps
+// four zones' loads in flight; the per-zone work is 1/rho and sqrt by one cubic Newton step on the MUFU seeds (a few
+// ulp: the tolerance on dt is 1e-14 relative) and no division.  Warp-shuffle max, one atomicMax per CTA on the bit
+// pattern (non-negative doubles order like unsigned integers); the last CTA to finish writes cfl / max and re-arms
+// the scratch words for the next call.  HBM-bound: one 40 B/zone read pass.
 __global__ void __launch_bounds__(256) fx_k_compute_dt(FxParams P, const double *__restrict__ U,
                                                        const double *__restrict__ dx, double cfl,
-                                                       double *__restrict__ dt_out, long long nzones) {
-  const int nx = P.n[0], ny = P.n[1], nz = P.n[2];
-  const long long per_block = (long long)nx * ny * nz;
-  double best = __longlong_as_double(0x7ff0000000000000ll);  // +inf
+                                                       double *__restrict__ dt_out) {
+  const unsigned nx = P.n[0], ny = P.n[1];
+  const unsigned per_block = nx * ny * (unsigned)P.n[2];
+  double rate = 0.0;  // max of (|u_d| + c) / dx_d
   unsigned hit = 0;
-  for (long long z = (long long)blockIdx.x * blockDim.x + threadIdx.x; z < nzones; z += (long long)gridDim.x * blockDim.x) {
-    const long long b = z / per_block;
-    const int r = (int)(z - b * per_block);
-    const int i = r % nx, j = (r / nx) % ny, k = r / (nx * ny);
-    const long long c = b * P.S_b + (k + P.gd[2]) * P.S_k + (j + P.gd[1]) * P.S_j + (i + P.gd[0]);
-    double W[5];
-    fx_c2p(P, U[c], U[P.S_v + c], U[2 * P.S_v + c], U[3 * P.S_v + c], U[4 * P.S_v + c], W);
-    const double cs = sqrt(P.gamma * W[4] / W[0]);
+  for (long long b = blockIdx.x; b < P.nblocks; b += gridDim.x) {
+    double idx[3];
 #pragma unroll
-    for (int d = 0; d < 3; ++d) {
-      if (!P.active[d]) continue;
-      const double s = fabs(W[1 + d]) + cs;
-      if (!(s > 0.0) || !(s <= 1.79e308)) hit |= FX_STATUS_NONFINITE;
-      best = fmin(best, __ldg(&dx[b * 3 + d]) / s);
+    for (int d = 0; d < 3; ++d) idx[d] = P.active[d] ? 1.0 / __ldg(&dx[b * 3 + d]) : 0.0;
+    const double *Ub = U + b * P.S_b;
+    for (unsigned r0 = threadIdx.x; r0 < per_block; r0 += 4 * 256) {
+      double u[4][5];
+      bool on[4];
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        const unsigned r = r0 + q * 256;
+        on[q] = r < per_block;
+        const unsigned rr = on[q] ? r : r0;
+        const unsigned i = rr % nx, t = rr / nx, j = t % ny, k = t / ny;
+        const long long c = (long long)(k + P.gd[2]) * P.S_k + (long long)(j + P.gd[1]) * P.S_j + (i + P.gd[0]);
+#pragma unroll
+        for (int v = 0; v < 5; ++v) u[q][v] = Ub[v * P.S_v + c];
+      }
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        double W[5];
+        fx_c2p_v2(P, u[q][0], u[q][1], u[q][2], u[q][3], u[q][4], W);
+        const double cs = fx_sqrt3(P.gamma * W[4] * fx_rcp3(W[0]));
+        double m = 0.0;
+#pragma unroll
+        for (int d = 0; d < 3; ++d) m = fmax(m, (fabs(W[1 + d]) + cs) * idx[d]);
+        // a NaN anywhere reaches cs or a velocity; fmax would drop it, so test the sum
+        const double chk = (fabs(W[1]) + fabs(W[2])) + (fabs(W[3]) + cs);
+        if (on[q]) {
+          if (fx_hi_nonfinite(__double2hiint(chk)) || !(cs > 0.0)) hit |= FX_STATUS_NONFINITE;
+          rate = fmax(rate, m);
+        }
+      }
     }
   }
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) best = fmin(best, __shfl_xor_sync(0xffffffffu, best, o));
-  __shared__ double wmin[8];
+  for (int o = 16; o > 0; o >>= 1) rate = fmax(rate, __shfl_xor_sync(0xffffffffu, rate, o));
+  __shared__ double wmax[8];
   __shared__ bool last;
-  if ((threadIdx.x & 31) == 0) wmin[threadIdx.x >> 5] = best;
+  if ((threadIdx.x & 31) == 0) wmax[threadIdx.x >> 5] = rate;
   if (hit) fx_note(P, hit);
   __syncthreads();
   if (threadIdx.x == 0) {
-    double m = wmin[0];
-    for (int w = 1; w < (int)(blockDim.x >> 5); ++w) m = fmin(m, wmin[w]);
-    atomicMin(&P.scratch[FX_SCR_DTBITS], (unsigned long long)__double_as_longlong(m));
+    double m = wmax[0];
+    for (int w = 1; w < (int)(blockDim.x >> 5); ++w) m = fmax(m, wmax[w]);
+    atomicMax(&P.scratch[FX_SCR_DTBITS], (unsigned long long)__double_as_longlong(m));
     __threadfence();
     unsigned long long done = atomicAdd(&P.scratch[FX_SCR_COUNTER], 1ull);
     last = (done == gridDim.x - 1);
@@ -116,18 +138,17 @@ __global__ void __launch_bounds__(256) fx_k_compute_dt(FxParams P, const double 
   __syncthreads();
   if (last && threadIdx.x == 0) {
     __threadfence();
-    unsigned long long bits = atomicExch(&P.scratch[FX_SCR_DTBITS], 0x7ff0000000000000ull);
+    unsigned long long bits = atomicExch(&P.scratch[FX_SCR_DTBITS], 0ull);
     P.scratch[FX_SCR_COUNTER] = 0ull;
-    *dt_out = cfl * __longlong_as_double((long long)bits);
+    *dt_out = cfl / __longlong_as_double((long long)bits);  // +inf for an empty batch
   }
 }
 
 int fx_launch_compute_dt(const FxParams &P, const double *U, const double *dx, double cfl, double *dt_out,
                          cudaStream_t st) {
-  const long long nzones = P.nblocks * P.n[0] * P.n[1] * P.n[2];
-  long long want = (nzones + 256 * 8 - 1) / (256 * 8);
-  int grid = (int)(want < 1 ? 1 : (want > 148 * 16 ? 148 * 16 : want));
-  fx_k_compute_dt<<<grid, 256, 0, st>>>(P, U, dx, cfl, dt_out, nzones);
+  const long long want = P.nblocks < 1 ? 1 : P.nblocks;
+  const int grid = (int)(want > 148 * 8 ? 148 * 8 : want);
+  fx_k_compute_dt<<<grid, 256, 0, st>>>(P, U, dx, cfl, dt_out);
   FX_LAUNCH_CHECK("compute_dt");
   return FX_OK;
 }

@@ -22,7 +22,7 @@ struct FxParams {
 
 // 64-bit words of the scratch block
 enum {
-  FX_SCR_DTBITS = 0,   // running min of dx/(|u|+c) as the bit pattern of a non-negative double
+  FX_SCR_DTBITS = 0,   // running max of (|u|+c)/dx as the bit pattern of a non-negative double
   FX_SCR_COUNTER = 1,  // CTAs finished in the dt reduction
   FX_SCR_FLAGS = 2,    // status bits
   FX_SCR_COUNT0 = 4,   // 4 counters: non-finite, rho floor, p floor, WENO fallback
