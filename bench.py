@@ -1,8 +1,9 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the batched block Euler update on B200 (one JSON line on stdout).
 
-A "step" is one pass of the whole hot path over the workload: fx_hydro_compute_dt (a7) followed by
-fx_hydro_advance (a1..a6, all RK stages), dt staying on the device.  Metric: hydro zone-updates/s per RK
+A "step" is one pass of the whole hot path over the workload: fx_hydro_step = all RK stages (a1..a6) with the
+device-resident dt, and the CFL reduction (a7) of the advanced state, which the fused path forms inside the last
+stage; the first dt comes from fx_hydro_compute_dt before the warm-up.  Metric: hydro zone-updates/s per RK
 stage = interior zones x stages / time.  Workload at N = 1: BASELINE.json configs[4] (32768 blocks of 16^3,
 PLM-minmod + HLLC, SSP-RK2; 18.1 GB per state copy, far larger than the 126 MB L2, so nothing is served
 from cache between timed iterations).  N > 1: N independent replicas of that workload, one per rank
@@ -213,11 +214,13 @@ def run_ours(args, rank, world, local_rank):
     stages = cfg.rk_order
     zones = cfg.interior_zones
     fused = plan.path >= 1
-    launches_per_step = 1 + stages * (1 if fused else 2)  # dt + per stage (guard fill +) stage kernel
+    # fused path: one launch per RK stage, the CFL reduction (a7) rides in the last one; generic path: guard fill +
+    # stage kernel per stage, then the reduction pass
+    launches_per_step = stages if fused else 2 * stages + 1
+    dt = plan.fx_hydro_compute_dt(U, dx, cfg.cfl).clone()  # the first step's dt; stays on the device from here on
 
     def step():
-        dt = plan.fx_hydro_compute_dt(U, dx, cfg.cfl)  # stays on the device
-        plan.fx_hydro_advance(U, dx, dt)
+        plan.fx_hydro_step(U, dx, cfg.cfl, dt)  # a1..a6 with this dt, a7 of the advanced state into dt
 
     def barrier():
         if world > 1:

@@ -144,6 +144,16 @@ int fx_hydro_advance_host(fx_hydro_plan *plan, double *U_host, const double *dx_
 int fx_hydro_advance_devdt(fx_hydro_plan *plan, double *U_dev, const double *dx_dev, const double *dt_dev,
                            void *stream);
 
+/* One step with the time step kept on the device and the next one formed on the way [O6 + O7]: advances U_dev by
+ * *dt_inout_dev exactly as fx_hydro_advance_devdt does, and replaces *dt_inout_dev by cfl * min dx/(|u_d| + c) of
+ * the ADVANCED state -- on the fused path the reduction rides in the last RK stage (each zone's rate is formed from
+ * the values just computed, before they leave the SM), so a time loop is fx_hydro_compute_dt once, then one
+ * fx_hydro_step per step with no separate reduction pass and no host round trip.  The value equals what
+ * fx_hydro_compute_dt would return for the advanced state to rounding (a few ulp).  cfl <= 0 or non-finite ->
+ * FX_ERR_INVALID_ARG.  Needs topology and workspace (FX_ERR_STATE). */
+int fx_hydro_step(fx_hydro_plan *plan, double *U_dev, const double *dx_dev, double cfl, double *dt_inout_dev,
+                  void *stream);
+
 /* Status word and counters {non-finite, rho floor, p floor, WENO fallback} accumulated by all kernels
  * since the last reset; synchronises `stream`.  counts_host may be NULL. */
 int fx_hydro_status(fx_hydro_plan *plan, uint32_t *flags_host, unsigned long long counts_host[4], void *stream);

@@ -27,7 +27,7 @@ EXPORTS = [
     "fx_last_error", "fx_hydro_plan_create", "fx_hydro_plan_destroy", "fx_hydro_plan_layout",
     "fx_hydro_plan_set_option", "fx_hydro_plan_workspace_bytes", "fx_hydro_plan_set_workspace",
     "fx_hydro_plan_set_topology", "fx_topology_cartesian", "fx_fill_guardcells", "fx_guardcell_index_map",
-    "fx_hydro_compute_dt", "fx_hydro_advance", "fx_hydro_advance_host", "fx_hydro_advance_devdt",
+    "fx_hydro_compute_dt", "fx_hydro_advance", "fx_hydro_advance_host", "fx_hydro_advance_devdt", "fx_hydro_step",
     "fx_hydro_status", "fx_hydro_status_reset", "fx_debug_compute_fluxes", "fx_hydro_plan_path",
     "fx_probe_fp64_fma", "fx_hydro_plan_set_timing", "fx_hydro_plan_get_timing",
 ]
@@ -72,6 +72,7 @@ def lib():
         L.fx_hydro_compute_dt.argtypes = [vp, vp, vp, C.c_double, vp, vp]
         L.fx_hydro_advance.argtypes = [vp, vp, vp, C.c_double, vp]
         L.fx_hydro_advance_devdt.argtypes = [vp, vp, vp, vp, vp]
+        L.fx_hydro_step.argtypes = [vp, vp, vp, C.c_double, vp, vp]
         L.fx_hydro_advance_host.argtypes = [vp, vp, vp, C.c_double, C.c_int, vp, vp, vp, vp]
         L.fx_hydro_status.argtypes = [vp, C.POINTER(C.c_uint32), C.POINTER(C.c_ulonglong), vp]
         L.fx_hydro_status_reset.argtypes = [vp, vp]
@@ -187,6 +188,11 @@ class HydroPlan:
         else:
             _check(lib().fx_hydro_advance(self._h, _dev(U, torch.float64), _dev(dx, torch.float64), float(dt),
                                           _stream(stream)))
+
+    def fx_hydro_step(self, U, dx, cfl, dt, stream=None):
+        """Advance by the device-resident dt (a 1-element float64 CUDA tensor) and overwrite it with the next step's dt."""
+        _check(lib().fx_hydro_step(self._h, _dev(U, torch.float64), _dev(dx, torch.float64), float(cfl),
+                                   _dev(dt, torch.float64), _stream(stream)))
 
     def fx_hydro_advance_host(self, U_host, dx_host, cfl, nsteps, U_stage, dx_stage, stream=None):
         """U_host / dx_host: CPU (preferably pinned) float64 tensors, updated in place.  Returns the last dt."""

@@ -40,7 +40,8 @@ extern "C" int fx_hydro_compute_dt(fx_hydro_plan *plan, const double *U, const d
 // One stage: out = U0 + beta((X - U0) - S(X)); halos of X come from a K1 fill (generic path) or are
 // gathered from neighbour interiors inside the fused kernel.
 static int fx_stage(fx_hydro_plan *plan, double *X, const double *U0, double *out, const double *dx, double dt,
-                    const double *dt_dev, double beta, int first, cudaStream_t st) {
+                    const double *dt_dev, double beta, int first, cudaStream_t st, double cfl_next = 0.0,
+                    double *dt_next = nullptr) {
   const bool fused = fx_hydro_plan_path(plan) == 1;
   int rc = FX_OK;
   if (!fused) {
@@ -49,9 +50,13 @@ static int fx_stage(fx_hydro_plan *plan, double *X, const double *U0, double *ou
   }
   const bool rec = plan->timing && plan->ev && plan->nrec < FX_MAX_REC;
   if (rec) FX_CUDA(cudaEventRecord(plan->ev[2 * plan->nrec], st));
-  rc = fused ? fx_launch_stage_tma(plan->P, X, U0, out, dx, dt, dt_dev, beta, first, st)
+  rc = fused ? fx_launch_stage_tma(plan->P, X, U0, out, dx, dt, dt_dev, beta, first, cfl_next, dt_next, st)
              : fx_launch_generic_stage(plan->P, X, U0, out, dx, dt, dt_dev, beta, first, st);
   if (rc) return rc;
+  if (!fused && dt_next) {  // the generic path has no fused reduction: a7 as its own pass over the finished state
+    rc = fx_launch_compute_dt(plan->P, out, dx, cfl_next, dt_next, st);
+    if (rc) return rc;
+  }
   if (rec) {
     FX_CUDA(cudaEventRecord(plan->ev[2 * plan->nrec + 1], st));
     ++plan->nrec;
@@ -87,16 +92,16 @@ extern "C" int fx_hydro_plan_get_timing(fx_hydro_plan *plan, double *ms_sum, lon
 }
 
 static int fx_advance_impl(fx_hydro_plan *plan, double *U, const double *dx, double dt, const double *dt_dev,
-                           cudaStream_t st) {
+                           cudaStream_t st, double cfl_next = 0.0, double *dt_next = nullptr) {
   if (plan->P.nblocks == 0) return FX_OK;
   double *U1 = plan->stage[0], *U2 = plan->stage[1];
   // The last stage may overwrite U0 in place: its halos come from U1 (RK2) / U2 (RK3), never from U0.
   int rc = fx_stage(plan, U, U, U1, dx, dt, dt_dev, 1.0, 1, st);  // U1 = U0 - S(U0)
   if (rc) return rc;
-  if (plan->rk == 2) return fx_stage(plan, U1, U, U, dx, dt, dt_dev, 0.5, 0, st);
+  if (plan->rk == 2) return fx_stage(plan, U1, U, U, dx, dt, dt_dev, 0.5, 0, st, cfl_next, dt_next);
   rc = fx_stage(plan, U1, U, U2, dx, dt, dt_dev, 0.25, 0, st);
   if (rc) return rc;
-  return fx_stage(plan, U2, U, U, dx, dt, dt_dev, 2.0 / 3.0, 0, st);
+  return fx_stage(plan, U2, U, U, dx, dt, dt_dev, 2.0 / 3.0, 0, st, cfl_next, dt_next);
 }
 
 extern "C" int fx_hydro_advance(fx_hydro_plan *plan, double *U, const double *dx, double dt, void *stream) {
@@ -115,6 +120,17 @@ extern "C" int fx_hydro_advance_devdt(fx_hydro_plan *plan, double *U, const doub
   return fx_advance_impl(plan, U, dx, 0.0, dt_dev, (cudaStream_t)stream);
 }
 
+extern "C" int fx_hydro_step(fx_hydro_plan *plan, double *U, const double *dx, double cfl, double *dt_inout_dev,
+                             void *stream) {
+  int rc = fx_need(plan, true, true, "step");
+  if (rc) return rc;
+  if (!dt_inout_dev || ((!U || !dx) && plan->P.nblocks > 0)) return fx_fail(FX_ERR_INVALID_ARG, "step: null argument");
+  if (!(cfl > 0.0) || !isfinite(cfl)) return fx_fail(FX_ERR_INVALID_ARG, "step: cfl must be positive and finite");
+  if (plan->P.nblocks == 0) return FX_OK;
+  // every stage reads dt from dt_inout_dev when it starts; the last CTA of the last stage to finish overwrites it
+  return fx_advance_impl(plan, U, dx, 0.0, dt_inout_dev, (cudaStream_t)stream, cfl, dt_inout_dev);
+}
+
 extern "C" int fx_hydro_advance_host(fx_hydro_plan *plan, double *U_host, const double *dx_host, double cfl, int nsteps,
                                      double *U_stage, double *dx_stage, double *dt_last_host, void *stream) {
   int rc = fx_need(plan, true, true, "advance_host");
@@ -127,14 +143,18 @@ extern "C" int fx_hydro_advance_host(fx_hydro_plan *plan, double *U_host, const 
   FX_CUDA(cudaMemcpyAsync(U_stage, U_host, ub, cudaMemcpyHostToDevice, st));
   FX_CUDA(cudaMemcpyAsync(dx_stage, dx_host, db, cudaMemcpyHostToDevice, st));
   double *dt_dev = (double *)&plan->P.scratch[FX_SCR_WORDS - 1];  // last scratch word holds the step's dt
-  for (int s = 0; s < nsteps; ++s) {
+  double *dt_used = dt_dev - 1;  // the dt the last step was taken with (what the caller gets back)
+  if (nsteps > 0) {
     rc = fx_launch_compute_dt(plan->P, U_stage, dx_stage, cfl, dt_dev, st);
     if (rc) return rc;
-    rc = fx_advance_impl(plan, U_stage, dx_stage, 0.0, dt_dev, st);
+  }
+  for (int s = 0; s < nsteps; ++s) {
+    FX_CUDA(cudaMemcpyAsync(dt_used, dt_dev, sizeof(double), cudaMemcpyDeviceToDevice, st));
+    rc = fx_advance_impl(plan, U_stage, dx_stage, 0.0, dt_dev, st, cfl, dt_dev);  // leaves the next step's dt in dt_dev
     if (rc) return rc;
   }
   FX_CUDA(cudaMemcpyAsync(U_host, U_stage, ub, cudaMemcpyDeviceToHost, st));
-  if (dt_last_host && nsteps > 0) FX_CUDA(cudaMemcpyAsync(dt_last_host, dt_dev, sizeof(double), cudaMemcpyDeviceToHost, st));
+  if (dt_last_host && nsteps > 0) FX_CUDA(cudaMemcpyAsync(dt_last_host, dt_used, sizeof(double), cudaMemcpyDeviceToHost, st));
   FX_CUDA(cudaStreamSynchronize(st));
   return FX_OK;
 }

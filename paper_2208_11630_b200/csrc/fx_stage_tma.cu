@@ -13,13 +13,17 @@
 //     primitives once and serves the z reconstruction, the z Riemann problem and, R planes later, the
 //     in-plane work of the same zone;
 //   * x and y directions: per plane the threads exchange primitives, plus-side face states and face fluxes
-//     through shared memory (three CTA barriers per plane; a face's flux overwrites the plus-side state it
-//     was computed from, in place);
+//     through shared memory with TWO CTA barriers per plane: (B) plus-side states published -> Riemann solves,
+//     each face's flux overwriting, in place, the plus-side state it was computed from, and the primitives of the
+//     NEXT plane written (nobody reads them in that phase); (C) fluxes visible -> flux divergence and RK
+//     combination, which runs on into the next plane's reconstruction without a barrier;
 //   * a ninth "edge" warp supplies what a 16-wide row lacks: the halo cells of the plane -- TMA boxes
 //     {2|4,16,1,1,5} and {16,R,1,1,5} taken straight from the neighbour blocks' interiors through the
 //     neighbour table (or from this block's own edge at an outflow boundary; no guard cell in HBM is read or
 //     written) --, the plus-side state of cell -1 and the flux of the 17th face of every row and column.  Its
 //     lane 0 is the TMA producer.
+// In the last stage of fx_hydro_step (DTOUT) each finished zone also contributes (|u_d| + c)/dx_d to a running
+// maximum, reduced per warp, per CTA and with one atomicMax per CTA: the CFL step of the advanced state costs no pass.
 // HBM traffic per zone: one read of the stage input (+ U0, + the stage input again from L2 in later stages),
 // one write, plus halos.
 #include <cuda.h>
@@ -55,6 +59,8 @@ template <int RECON> struct alignas(128) Smem {
   double Lx[5][NY][NX + 1];    // Lx[v][j][i] = plus-side x state of cell (i-1,j), then the x flux at face i-1/2
   double Ly[5][NY + 1][NX];    // Ly[v][j][i] = plus-side y state of cell (i,j-1), then the y flux at face j-1/2
   double rd[3];                // beta dt / dx_d of this block (beta = 1 in the first stage)
+  double idx[3];               // 1 / dx_d (DTOUT: the CFL rate of the finished state is formed in the last stage)
+  double wmax[8];              // DTOUT: per-warp maximum of (|u_d| + c) / dx_d
   unsigned long long barX[2], barH[2], barS;  // barX[c & 1]: stage-input plane of tick c AND the U0 plane of plane c - 1
 };
 
@@ -187,12 +193,13 @@ __device__ __forceinline__ void z_source(const FxParams &P, int b, int nlo, int 
   kp = k + P.gd[2];
 }
 
-template <int RECON, int RIEMANN, int WS, bool FIRST>
+template <int RECON, int RIEMANN, int WS, bool FIRST, bool DTOUT>
 __global__ void __launch_bounds__(NTHREADS) __maxnreg__(Rc<RECON>::NREG)
 fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ CUtensorMap mXx,
                const __grid_constant__ CUtensorMap mXy, const __grid_constant__ CUtensorMap mU0,
                const __grid_constant__ CUtensorMap mOut, const FxParams P, const double *__restrict__ X,
-               const double *__restrict__ dx, double dt, const double *__restrict__ dt_dev, double beta) {
+               const double *__restrict__ dx, double dt, const double *__restrict__ dt_dev, double beta,
+               double cfl_next, double *__restrict__ dt_next) {
   constexpr int r = Rc<RECON>::r, R = Rc<RECON>::R, W = 2 * r + 1, NP = Rc<RECON>::NP, BW = Rc<RECON>::BW;
   extern __shared__ __align__(1024) unsigned char fx_smem_raw[];  // TMA destinations need 128-byte alignment
   Smem<RECON> &S = *reinterpret_cast<Smem<RECON> *>(fx_smem_raw);
@@ -249,12 +256,17 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
     if (!FIRST) issue_Xs(0);
   }
   if (dt_dev) dt = __ldg(dt_dev);
-  if (tid < 3) S.rd[tid] = (FIRST ? 1.0 : beta) * dt / __ldg(&dx[(long long)b * 3 + tid]);
+  if (tid < 3) {
+    const double dxd = __ldg(&dx[(long long)b * 3 + tid]);
+    S.rd[tid] = (FIRST ? 1.0 : beta) * dt / dxd;
+    S.idx[tid] = 1.0 / dxd;
+  }
   cta_sync();  // barriers initialised before anyone waits on them; rd visible
 
   if (tid < NZONE_THREADS) {
     // ------------------------------------------------------------ zone threads
     const int i = tid & 15, j = tid >> 4;
+    double rate = 0.0;     // DTOUT: running maximum of (|u_d| + c) / dx_d over this thread's finished zones
     double q[W][5];        // q[m] = primitives of cell c - r + m at tick c
     double qpz[5], Fz[5];  // plus-side z state of cell c-1; z flux of face c-1 (between cells c-2 and c-1)
     {
@@ -358,6 +370,7 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
         // out = [U0 + beta (X - U0)] - sum_d (beta dt/dx_d) (F_d+ - F_d-)
         const double rx = S.rd[0], ry = S.rd[1], rz = S.rd[2];
         int hmax = 0;
+        double res5[5];
 #pragma unroll
         for (int v = 0; v < 5; ++v) {
           const double dFx = S.Lx[v][j][i + 1] - Fx[v];
@@ -367,16 +380,28 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
           const double a = FIRST ? u0 : fma(beta, S.Xs[v][j][i] - u0, u0);
           const double res = fma(-rz, dFz, fma(-ry, dFy, fma(-rx, dFx, a)));
           S.Out[v][j][i] = res;
+          res5[v] = res;
           hmax = max(hmax, __double2hiint(res) & 0x7fffffff);
           Fz[v] = Fz_new[v];
         }
         if (hmax >= 0x7ff00000) hit |= FX_STATUS_NONFINITE;
+        if (DTOUT) {  // a7 on the finished zone: (|u_d| + c) / dx_d, folded into a running maximum [O7]
+          double w[5];
+          fx_c2p_v2(P, res5[0], res5[1], res5[2], res5[3], res5[4], w);
+          const double cs = fx_sqrt3(P.gamma * w[4] * fx_rcp3(w[0]));
+          rate = fmax(rate, fmax((fabs(w[1]) + cs) * S.idx[0], fmax((fabs(w[2]) + cs) * S.idx[1], (fabs(w[3]) + cs) * S.idx[2])));
+        }
         fence_async_smem();  // the TMA store reads Out through the async proxy
       }
 #pragma unroll
       for (int m = 0; m < 2 * r; ++m)
 #pragma unroll
         for (int v = 0; v < 5; ++v) q[m][v] = q[m + 1][v];
+    }
+    if (DTOUT) {
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) rate = fmax(rate, __shfl_xor_sync(0xffffffffu, rate, o));
+      if ((tid & 31) == 0) S.wmax[tid >> 5] = rate;
     }
     cta_sync();  // D: the last plane is in Out
   } else {
@@ -480,6 +505,22 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
     if (lane == 0) {
       tma_store(&mOut, &S.Out[0][0][0], g0, g1, nz - 1 + g2, b);
       tma_commit();
+      if (DTOUT) {
+        // CTA maximum -> scratch word (non-negative doubles order like unsigned integers); the last CTA to finish
+        // writes the next time step cfl / max and re-arms the scratch words, as fx_k_compute_dt does
+        double mx = S.wmax[0];
+#pragma unroll
+        for (int w8 = 1; w8 < 8; ++w8) mx = fmax(mx, S.wmax[w8]);
+        atomicMax(&P.scratch[FX_SCR_DTBITS], (unsigned long long)__double_as_longlong(mx));
+        __threadfence();
+        const unsigned long long done = atomicAdd(&P.scratch[FX_SCR_COUNTER], 1ull);
+        if (done == gridDim.x - 1) {
+          __threadfence();
+          const unsigned long long bits = atomicExch(&P.scratch[FX_SCR_DTBITS], 0ull);
+          P.scratch[FX_SCR_COUNTER] = 0ull;
+          *dt_next = cfl_next / __longlong_as_double((long long)bits);
+        }
+      }
       tma_wait_all();
     }
   }
@@ -519,9 +560,9 @@ static int make_map(CUtensorMap *m, const FxParams &P, const double *base, int b
   return FX_OK;
 }
 
-template <int RECON, int RIEMANN, int WS, bool FIRST>
+template <int RECON, int RIEMANN, int WS, bool FIRST, bool DTOUT>
 int launch(const FxParams &P, const double *X, const double *U0, double *out, const double *dx, double dt, const double *dt_dev,
-           double beta, cudaStream_t st) {
+           double beta, double cfl_next, double *dt_next, cudaStream_t st) {
   constexpr int R = Rc<RECON>::R, BW = Rc<RECON>::BW;
   CUtensorMap mXm, mXx, mXy, mU0, mOut;
   int rc;
@@ -530,14 +571,14 @@ int launch(const FxParams &P, const double *X, const double *U0, double *out, co
   if ((rc = make_map(&mXy, P, X, NX, R))) return rc;
   if ((rc = make_map(&mU0, P, U0, NX, NY))) return rc;
   if ((rc = make_map(&mOut, P, out, NX, NY))) return rc;
-  auto kern = fx_k_stage_tma<RECON, RIEMANN, WS, FIRST>;
+  auto kern = fx_k_stage_tma<RECON, RIEMANN, WS, FIRST, DTOUT>;
   const int smem = (int)sizeof(Smem<RECON>);
   static bool configured = false;  // per instantiation
   if (!configured) {
     FX_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     configured = true;
   }
-  kern<<<(unsigned)P.nblocks, NTHREADS, smem, st>>>(mXm, mXx, mXy, mU0, mOut, P, X, dx, dt, dt_dev, beta);
+  kern<<<(unsigned)P.nblocks, NTHREADS, smem, st>>>(mXm, mXx, mXy, mU0, mOut, P, X, dx, dt, dt_dev, beta, cfl_next, dt_next);
   const cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) {
     cudaFuncAttributes a;
@@ -551,14 +592,19 @@ int launch(const FxParams &P, const double *X, const double *U0, double *out, co
   return FX_OK;
 }
 
+template <int RECON, int RIEMANN, int WS>
+int launch_ws(const FxParams &P, const double *X, const double *U0, double *out, const double *dx, double dt, const double *dt_dev,
+              double beta, int first, double cfl_next, double *dt_next, cudaStream_t st) {
+  if (first) return launch<RECON, RIEMANN, WS, true, false>(P, X, U0, out, dx, dt, dt_dev, beta, 0.0, nullptr, st);
+  if (dt_next) return launch<RECON, RIEMANN, WS, false, true>(P, X, U0, out, dx, dt, dt_dev, beta, cfl_next, dt_next, st);
+  return launch<RECON, RIEMANN, WS, false, false>(P, X, U0, out, dx, dt, dt_dev, beta, 0.0, nullptr, st);
+}
+
 template <int RECON, int RIEMANN>
 int launch_rr(const FxParams &P, const double *X, const double *U0, double *out, const double *dx, double dt, const double *dt_dev,
-              double beta, int first, cudaStream_t st) {
-  if (P.wavespeed == 0)
-    return first ? launch<RECON, RIEMANN, 0, true>(P, X, U0, out, dx, dt, dt_dev, beta, st)
-                 : launch<RECON, RIEMANN, 0, false>(P, X, U0, out, dx, dt, dt_dev, beta, st);
-  return first ? launch<RECON, RIEMANN, 1, true>(P, X, U0, out, dx, dt, dt_dev, beta, st)
-               : launch<RECON, RIEMANN, 1, false>(P, X, U0, out, dx, dt, dt_dev, beta, st);
+              double beta, int first, double cfl_next, double *dt_next, cudaStream_t st) {
+  return P.wavespeed == 0 ? launch_ws<RECON, RIEMANN, 0>(P, X, U0, out, dx, dt, dt_dev, beta, first, cfl_next, dt_next, st)
+                          : launch_ws<RECON, RIEMANN, 1>(P, X, U0, out, dx, dt, dt_dev, beta, first, cfl_next, dt_next, st);
 }
 
 }  // namespace fxt
@@ -570,16 +616,17 @@ bool fx_stage_tma_supported(const FxParams &P) {
          P.nblocks <= 0x7fffffffLL;
 }
 
+// dt_next != nullptr (a later stage only): also form cfl_next * min dx/(|u|+c) of the finished state and write it there.
 int fx_launch_stage_tma(const FxParams &P, const double *X, const double *U0, double *out, const double *dx, double dt,
-                        const double *dt_dev, double beta, int first, cudaStream_t st) {
+                        const double *dt_dev, double beta, int first, double cfl_next, double *dt_next, cudaStream_t st) {
   if (!fx_stage_tma_supported(P)) return fx_fail(FX_ERR_UNSUPPORTED, "TMA stage kernel: block shape not supported");
   if (P.nblocks == 0) return FX_OK;
   if (((uintptr_t)X | (uintptr_t)U0 | (uintptr_t)out) & 15)
     return fx_fail(FX_ERR_INVALID_ARG, "TMA stage kernel: state arrays must be 16-byte aligned");
   if (P.recon == FX_RECON_PLM_MINMOD) {
-    if (P.riemann == FX_RIEMANN_HLLE) return fxt::launch_rr<FX_RECON_PLM_MINMOD, FX_RIEMANN_HLLE>(P, X, U0, out, dx, dt, dt_dev, beta, first, st);
-    return fxt::launch_rr<FX_RECON_PLM_MINMOD, FX_RIEMANN_HLLC>(P, X, U0, out, dx, dt, dt_dev, beta, first, st);
+    if (P.riemann == FX_RIEMANN_HLLE) return fxt::launch_rr<FX_RECON_PLM_MINMOD, FX_RIEMANN_HLLE>(P, X, U0, out, dx, dt, dt_dev, beta, first, cfl_next, dt_next, st);
+    return fxt::launch_rr<FX_RECON_PLM_MINMOD, FX_RIEMANN_HLLC>(P, X, U0, out, dx, dt, dt_dev, beta, first, cfl_next, dt_next, st);
   }
-  if (P.riemann == FX_RIEMANN_HLLE) return fxt::launch_rr<FX_RECON_WENO5, FX_RIEMANN_HLLE>(P, X, U0, out, dx, dt, dt_dev, beta, first, st);
-  return fxt::launch_rr<FX_RECON_WENO5, FX_RIEMANN_HLLC>(P, X, U0, out, dx, dt, dt_dev, beta, first, st);
+  if (P.riemann == FX_RIEMANN_HLLE) return fxt::launch_rr<FX_RECON_WENO5, FX_RIEMANN_HLLE>(P, X, U0, out, dx, dt, dt_dev, beta, first, cfl_next, dt_next, st);
+  return fxt::launch_rr<FX_RECON_WENO5, FX_RIEMANN_HLLC>(P, X, U0, out, dx, dt, dt_dev, beta, first, cfl_next, dt_next, st);
 }

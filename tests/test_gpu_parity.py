@@ -134,6 +134,27 @@ def test_device_dt_path_equals_host_dt_path():
     assert torch.equal(gplan.interior(A), gplan.interior(B))
 
 
+@pytest.mark.parametrize("number,nb,kw", [(5, (2, 2, 2), {}), (4, (2, 2, 2), {}), (3, (2, 2, 2), dict(rk=3, bc="outflow")), (2, None, {})])
+def test_step_with_fused_dt_equals_compute_dt_then_advance(number, nb, kw):
+    """fx_hydro_step: same state as advance with the same dt (bitwise), and the dt it leaves behind is the CFL step of
+    the advanced state (<= 1e-14 relative to the oracle's, and to the library's own reduction pass)."""
+    cfg, oplan, gplan, Uh, dx = setup(number, nb, **kw)
+    dxd = torch.from_numpy(dx).cuda()
+    A, B = Uh.cuda(), Uh.cuda()
+    dt = gplan.fx_hydro_compute_dt(A, dxd, cfg.cfl).clone()
+    for _ in range(3):
+        dt_used = dt.clone()
+        gplan.fx_hydro_step(A, dxd, cfg.cfl, dt)
+        gplan.fx_hydro_advance(B, dxd, dt_used)
+        assert torch.equal(gplan.interior(A), gplan.interior(B))
+        dt_lib = float(gplan.fx_hydro_compute_dt(B, dxd, cfg.cfl).item())
+        dt_ora = oplan.compute_dt(B.cpu().numpy(), dx, cfg.cfl)
+        assert abs(float(dt.item()) - dt_lib) <= TOL_DT * dt_lib
+        assert abs(float(dt.item()) - dt_ora) <= TOL_DT * dt_ora
+    fg, _ = gplan.fx_hydro_status()
+    assert fg == 0
+
+
 def test_advance_host_equals_device_path():
     cfg, oplan, gplan, Uh, dx = setup(3, (2, 2, 2))
     dxd = torch.from_numpy(dx).cuda()
