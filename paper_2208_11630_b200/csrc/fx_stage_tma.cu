@@ -125,13 +125,13 @@ __device__ __forceinline__ void recon_cell(const double *s, double eps, double &
       const double p0 = (2.0 * a - 7.0 * b + 11.0 * c) * sixth, p1 = (-b + 5.0 * c + 2.0 * d) * sixth,
                    p2 = (2.0 * c + 5.0 * d - e) * sixth;
       const double a0 = 0.1 * s0, a1 = 0.6 * s1, a2 = 0.3 * s2;
-      qp = (a0 * p0 + a1 * p1 + a2 * p2) / (a0 + a1 + a2);
+      qp = (a0 * p0 + a1 * p1 + a2 * p2) * fx_rcp3(a0 + a1 + a2);  // the weights' sum is positive and far from the subnormal range
     }
     {  // minus face: mirrored stencil (e,d,c,b,a)
       const double p0 = (2.0 * e - 7.0 * d + 11.0 * c) * sixth, p1 = (-d + 5.0 * c + 2.0 * b) * sixth,
                    p2 = (2.0 * c + 5.0 * b - a) * sixth;
       const double a0 = 0.1 * s2, a1 = 0.6 * s1, a2 = 0.3 * s0;
-      qm = (a0 * p0 + a1 * p1 + a2 * p2) / (a0 + a1 + a2);
+      qm = (a0 * p0 + a1 * p1 + a2 * p2) * fx_rcp3(a0 + a1 + a2);
     }
   }
 }
