@@ -611,9 +611,10 @@ int launch_rr(const FxParams &P, const double *X, const double *U0, double *out,
 
 bool fx_stage_tma_supported(const FxParams &P) {
   const int R = P.recon == FX_RECON_WENO5 ? 3 : 2;
-  // TMA: global strides must be multiples of 16 bytes (S_j even), the arrays 16-byte aligned (checked at launch)
+  // TMA: global strides must be multiples of 16 bytes (S_j even), every box must start on a 16-byte boundary (guard
+  // depth even: measured, a box starting at an odd element faults), the arrays 16-byte aligned (checked at launch)
   return P.n[0] == fxt::NX && P.n[1] == fxt::NY && P.n[2] >= R && P.active[2] && P.gd[0] >= R && (P.S_j % 2) == 0 &&
-         P.nblocks <= 0x7fffffffLL;
+         (P.gd[0] % 2) == 0 && P.nblocks <= 0x7fffffffLL;
 }
 
 // dt_next != nullptr (a later stage only): also form cfl_next * min dx/(|u|+c) of the finished state and write it there.

@@ -155,6 +155,33 @@ def test_step_with_fused_dt_equals_compute_dt_then_advance(number, nb, kw):
     assert fg == 0
 
 
+@pytest.mark.parametrize("nguard,recon,dims", [(2, 0, (16, 16, 16)), (3, 0, (16, 16, 16)), (3, 1, (16, 16, 16)), (4, 0, (16, 16, 6)),
+                                               (4, 1, (16, 16, 5))])
+def test_fused_kernel_other_guard_depths_and_block_heights(nguard, recon, dims):
+    """Guard depths other than 4 and block heights other than 16: the fused kernel where it applies (a TMA box must start
+    on a 16-byte boundary, so an odd guard depth goes to the generic path), parity with the oracle either way."""
+    for bc in ("periodic", "outflow"):
+        cfg = inputs.config(5, nb=(2, 2, 2))
+        cfg.nguard, cfg.block_dims = nguard, dims
+        oplan, neigh, coords = oracle_plan_for(cfg, bc=bc, recon=recon)
+        gplan, _, _ = gpu_plan_for(cfg, bc=bc, recon=recon)
+        assert gplan.path == (1 if nguard % 2 == 0 else 0)
+        rng = np.random.default_rng(11)
+        shape = (8,) + tuple(reversed(dims))
+        rho = 1.0 + 0.3 * rng.random(shape)
+        vel = 0.4 * rng.standard_normal((3,) + shape)
+        p = 1.0 + 0.3 * rng.random(shape)
+        Ui = np.stack([rho, rho * vel[0], rho * vel[1], rho * vel[2], p / (cfg.gamma - 1) + 0.5 * rho * (vel ** 2).sum(0)])
+        Uh = inputs.embed(cfg, torch.from_numpy(Ui))
+        dx = np.full((8, 3), 1.0 / 32)
+        Uo, Ud, dxd = Uh.numpy().copy(), Uh.cuda(), torch.from_numpy(dx).cuda()
+        for step in range(3):
+            dt = oplan.compute_dt(Uo, dx, 0.3)
+            oplan.advance(Uo, dx, dt)
+            gplan.fx_hydro_advance(Ud, dxd, dt)
+        assert rel_err(cfg, gplan.interior(Ud).cpu().numpy(), oplan.interior(Uo)) <= 1e-11
+
+
 def test_advance_host_equals_device_path():
     cfg, oplan, gplan, Uh, dx = setup(3, (2, 2, 2))
     dxd = torch.from_numpy(dx).cuda()
