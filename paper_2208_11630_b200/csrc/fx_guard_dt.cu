@@ -106,8 +106,9 @@ __global__ void __launch_bounds__(256) fx_k_compute_dt(FxParams P, const double 
 #pragma unroll
       for (int q = 0; q < 4; ++q) {
         double W[5];
-        fx_c2p_v2(P, u[q][0], u[q][1], u[q][2], u[q][3], u[q][4], W);
-        const double cs = fx_sqrt3(P.gamma * W[4] * fx_rcp3(W[0]));
+        double ir;
+        fx_c2p_v2(P, u[q][0], u[q][1], u[q][2], u[q][3], u[q][4], W, &ir);
+        const double cs = fx_sqrt3(P.gamma * W[4] * ir);
         double m = 0.0;
 #pragma unroll
         for (int d = 0; d < 3; ++d) m = fmax(m, (fabs(W[1 + d]) + cs) * idx[d]);

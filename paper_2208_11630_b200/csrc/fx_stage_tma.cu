@@ -381,14 +381,15 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
           const double res = fma(-rz, dFz, fma(-ry, dFy, fma(-rx, dFx, a)));
           S.Out[v][j][i] = res;
           res5[v] = res;
-          hmax = max(hmax, __double2hiint(res) & 0x7fffffff);
+          if (!DTOUT) hmax = max(hmax, __double2hiint(res) & 0x7fffffff);
           Fz[v] = Fz_new[v];
         }
-        if (hmax >= 0x7ff00000) hit |= FX_STATUS_NONFINITE;
+        if (!DTOUT && hmax >= 0x7ff00000) hit |= FX_STATUS_NONFINITE;
         if (DTOUT) {  // a7 on the finished zone: (|u_d| + c) / dx_d, folded into a running maximum [O7]
-          double w[5];
-          fx_c2p_v2(P, res5[0], res5[1], res5[2], res5[3], res5[4], w);
-          const double cs = fx_sqrt3(P.gamma * w[4] * fx_rcp3(w[0]));
+          double w[5], ir;
+          // (a non-finite result reaches the pressure or the density: the conversion's own test stands in for hmax)
+          hit |= fx_c2p_v2(P, res5[0], res5[1], res5[2], res5[3], res5[4], w, &ir) & FX_STATUS_NONFINITE;
+          const double cs = fx_sqrt3(P.gamma * w[4] * ir);
           rate = fmax(rate, fmax((fabs(w[1]) + cs) * S.idx[0], fmax((fabs(w[2]) + cs) * S.idx[1], (fabs(w[3]) + cs) * S.idx[2])));
         }
         fence_async_smem();  // the TMA store reads Out through the async proxy
