@@ -307,14 +307,6 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
 #pragma unroll 1
     for (int c = 1; c <= nz; ++c) {
       const int p = c - 1;  // plane of the in-plane work; its primitives are q[r-1]
-      {
-        mbar_wait(&S.barX[c & 1], ((c - 1) >> 1) & 1);
-        double u[5];
-#pragma unroll
-        for (int v = 0; v < 5; ++v) u[v] = S.rawX[c & 1][v][j][i];
-        const unsigned h = fx_c2p_v2(P, u[0], u[1], u[2], u[3], u[4], q[2 * r]);
-        if (c + r < nz) hit |= h;
-      }
       double qmx[5], qmy[5];
       {
         double st[W][5], qp[5];
@@ -336,6 +328,15 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
 #pragma unroll
         for (int v = 0; v < 5; ++v) S.Ly[v][j + 1][i] = qp[v];
       }
+      cta_sync();  // B: plus-side states visible; this tick's TMA planes have landed (the producer waited for them)
+      {  // new cell of the z window.  No mbarrier poll here: the producer observed the completion of this tick's loads
+         // before it arrived at barrier B, and the barrier orders that observation before these reads
+        double u[5];
+#pragma unroll
+        for (int v = 0; v < 5; ++v) u[v] = S.rawX[c & 1][v][j][i];
+        const unsigned h = fx_c2p_v2(P, u[0], u[1], u[2], u[3], u[4], q[2 * r]);
+        if (c + r < nz) hit |= h;
+      }
       // z: reconstruct cell c, flux of face c (between cells c-1 and c)
       double Fz_new[5];
       {
@@ -345,7 +346,6 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
 #pragma unroll
         for (int v = 0; v < 5; ++v) qpz[v] = qpz_new[v];
       }
-      cta_sync();  // B: plus-side states visible
       double Fx[5], Fy[5];
       {
         double WL[5];
@@ -366,7 +366,6 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
       }
       cta_sync();  // C: fluxes and the next plane's primitives visible
       {
-        if (!FIRST) mbar_wait(&S.barS, p & 1);
         // out = [U0 + beta (X - U0)] - sum_d (beta dt/dx_d) (F_d+ - F_d-)
         const double rx = S.rd[0], ry = S.rd[1], rz = S.rd[2];
         int hmax = 0;
@@ -469,10 +468,12 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
           for (int v = 0; v < 5; ++v) st[mm][v] = Pf[v * NP * NPS + (NX + R - r + mm) * pd + (m + R) * pt];
         hit |= recon_cell5<RECON>(st, P.weno_eps, qm16, qp);
       }
+      // this tick's stage-input plane (requested two ticks ago) and U0 plane (one tick ago): the zone threads read them
+      // after barrier B without polling the mbarrier themselves
+      mbar_wait(&S.barX[c & 1], ((c - 1) >> 1) & 1);
       cta_sync();  // B
       if (lane == 0) {
         // every slot consumed before barrier B of this tick is free again
-        if (c + 2 <= nz) issue_X(c + 2);
         if (p + 2 < nz) issue_H(p + 2);
         if (p >= 1) {
           tma_store(&mOut, &S.Out[0][0][0], g0, g1, p - 1 + g2, b);
@@ -500,7 +501,10 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
       }
       if (c < nz) halo_plane(c);                  // halo of plane p + 1: nobody reads P between barriers B and C
       if (lane == 0 && p >= 1) tma_wait_read();  // Out is free for the combine after barrier C
+      if (!FIRST) mbar_wait(&S.barS, p & 1);     // the combine's stage-input plane has landed
       cta_sync();  // C
+      // the zone threads read this tick's stage-input plane between barriers B and C: its slot is free only now
+      if (lane == 0 && c + 2 <= nz) issue_X(c + 2);
     }
     cta_sync();  // D
     if (lane == 0) {
