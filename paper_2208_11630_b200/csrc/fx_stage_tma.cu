@@ -198,8 +198,8 @@ __global__ void __launch_bounds__(NTHREADS) __maxnreg__(Rc<RECON>::NREG)
 fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ CUtensorMap mXx,
                const __grid_constant__ CUtensorMap mXy, const __grid_constant__ CUtensorMap mU0,
                const __grid_constant__ CUtensorMap mOut, const FxParams P, const double *__restrict__ X,
-               const double *__restrict__ dx, double dt, const double *__restrict__ dt_dev, double beta,
-               double cfl_next, double *__restrict__ dt_next) {
+               const double *__restrict__ dx, double dt, const double *dt_dev, double beta,
+               double cfl_next, double *dt_next) {  // dt_next may be dt_dev (fx_hydro_step): read at the start, written by the last CTA
   constexpr int r = Rc<RECON>::r, R = Rc<RECON>::R, W = 2 * r + 1, NP = Rc<RECON>::NP, BW = Rc<RECON>::BW;
   extern __shared__ __align__(1024) unsigned char fx_smem_raw[];  // TMA destinations need 128-byte alignment
   Smem<RECON> &S = *reinterpret_cast<Smem<RECON> *>(fx_smem_raw);
@@ -255,7 +255,7 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
     issue_U0(0);
     if (!FIRST) issue_Xs(0);
   }
-  if (dt_dev) dt = __ldg(dt_dev);
+  if (dt_dev) dt = *dt_dev;
   if (tid < 3) {
     const double dxd = __ldg(&dx[(long long)b * 3 + tid]);
     S.rd[tid] = (FIRST ? 1.0 : beta) * dt / dxd;
