@@ -182,6 +182,39 @@ def test_fused_kernel_other_guard_depths_and_block_heights(nguard, recon, dims):
         assert rel_err(cfg, gplan.interior(Ud).cpu().numpy(), oplan.interior(Uo)) <= 1e-11
 
 
+@pytest.mark.parametrize("path", [None, 1])
+def test_status_flags_floors_and_nonfinite(path):
+    """A7/A27: primitive floors and non-finite states raise the same status bits as in the oracle, the floored step
+    still agrees with it, and nothing traps or hangs."""
+    from paper_2208_11630_b200 import binding as fx
+    cfg, oplan, gplan, Uh, dx = setup(5, (2, 2, 2), path=path)
+    Ui = inputs.interior_view(cfg, Uh)
+    Ui[4, 3, 5, 6, 7] = 1e-3          # energy below the kinetic energy: negative pressure -> p floor
+    Ui[0, 5, 9, 2, 11] = -0.5         # negative density (at rest, so that the floored state stays finite) -> rho floor
+    Ui[1:4, 5, 9, 2, 11] = 0.0
+    Uo, Ud, dxd = Uh.numpy().copy(), Uh.cuda(), torch.from_numpy(dx).cuda()
+    oplan.advance(Uo, dx, 1e-6)
+    gplan.fx_hydro_advance(Ud, dxd, 1e-6)
+    fo, _ = oplan.status()
+    fg, _ = gplan.fx_hydro_status()
+    assert fo == fg and (fg & fx.STATUS_P_FLOOR) and (fg & fx.STATUS_RHO_FLOOR) and not (fg & fx.STATUS_NONFINITE)
+    got, ref = gplan.interior(Ud).cpu().numpy(), oplan.interior(Uo)
+    ok = np.ones(got.shape[1:], dtype=bool)
+    ok[3, 3:8, 4:9, 5:10] = False     # the neighbourhoods of the two bad zones hold huge floored-state values
+    ok[5, 7:12, 0:5, 9:14] = False
+    scale = np.abs(ref[:, ok]).max()
+    assert np.max(np.abs(got[:, ok] - ref[:, ok])) <= 1e-12 * scale
+    assert np.all(np.isfinite(got[:, ~ok]) == np.isfinite(ref[:, ~ok]))
+    # a NaN zone: flagged, not trapped
+    gplan.fx_hydro_status_reset()
+    Ud2 = Uh.cuda()
+    gplan.interior(Ud2)[1, 2, 4, 4, 4] = float("nan")
+    gplan.fx_hydro_advance(Ud2, dxd, 1e-6)
+    torch.cuda.synchronize()
+    fg2, _ = gplan.fx_hydro_status()
+    assert fg2 & fx.STATUS_NONFINITE
+
+
 def test_advance_host_equals_device_path():
     cfg, oplan, gplan, Uh, dx = setup(3, (2, 2, 2))
     dxd = torch.from_numpy(dx).cuda()
