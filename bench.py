@@ -266,6 +266,12 @@ def run_ours(args, rank, world, local_rank):
                 "kernel_ms_avg": stage_avg_ms, "kernel_launches_timed": stage_launches,
                 "kernel_share_of_step": stage_ms / ms if ms > 0 else None,
                 "alg_bytes_per_zone_stage": sum(alg_bytes_stage) / stages}
+    if fused and cfg.recon == 0 and cfg.riemann == 1:
+        # the other roof [NS]: the fp64 pipe.  437 fp64-pipe lane-instructions per zone-update (ncu)
+        # against 148 SMs x 64 lanes x the SM clock (nominal; 17 T/s measured with fx_probe_fp64_fma)
+        fp64_peak = 148 * FP64_FMA_LANES_PER_SM * 1.965e9
+        roofline["fp64_pipe"] = {"lane_instr_per_zone_update": 437, "peak_lane_instr_per_s": fp64_peak,
+                                 "frac": 437 * zones / (stage_avg_ms * 1e-3) / fp64_peak}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
