@@ -4,11 +4,12 @@
 // One 288-thread CTA per block marches the block's 16 x 16 column of zones through z; two CTAs share an SM, so
 // that one of them computes while the other waits at a barrier or for data.  Thread (i,j) of the 256 zone
 // threads owns the zones (i,j,k), k = 0..nz-1:
-//   * every plane of the stage input arrives as ONE 5-D TMA box {16,16,1,1,5} of U[v][b][k][j][i] in a
-//     2-slot shared-memory ring, two planes ahead of its use; the U0 plane (and, in later stages, the
-//     stage-input plane) of the zone being combined arrive the same way, and the finished plane leaves as
-//     one TMA box store.  No thread computes a global address inside the z loop and nothing is prefetched
-//     through registers;
+//   * every plane of the stage input arrives as ONE 5-D TMA box {16,16,1,1,5} of U[v][b][k][j][i] in a ring of r + 3
+//     shared-memory slots, a tick ahead of its use, and stays there until the zones of that plane are combined
+//     (the combine needs the stage input again: it is U0 in the first stage, X in the later ones -- no second
+//     load); in the later stages the U0 plane arrives the same way (2 slots), and the finished plane leaves as one
+//     TMA box store.  No thread computes a global address inside the z loop and nothing is prefetched through
+//     registers;
 //   * z direction: a sliding window of primitive cells lives in registers; each plane is converted to
 //     primitives once and serves the z reconstruction, the z Riemann problem and, R planes later, the
 //     in-plane work of the same zone;
@@ -24,8 +25,7 @@
 //     lane 0 is the TMA producer.
 // In the last stage of fx_hydro_step (DTOUT) each finished zone also contributes (|u_d| + c)/dx_d to a running
 // maximum, reduced per warp, per CTA and with one atomicMax per CTA: the CFL step of the advanced state costs no pass.
-// HBM traffic per zone: one read of the stage input (+ U0, + the stage input again from L2 in later stages),
-// one write, plus halos.
+// HBM traffic per zone: one read of the stage input (+ U0 in later stages), one write, plus halos.
 #include <cuda.h>
 #include <string.h>
 
@@ -43,17 +43,19 @@ template <int RECON> struct Rc {
   static constexpr int R = r + 1;                                    // halo depth
   static constexpr int NP = NX + 2 * R;                              // padded plane extent
   static constexpr int BW = (R + 1) & ~1;                            // x-halo box width: TMA rows are multiples of 16 B
+  static constexpr int NRING = r + 3;  // a stage-input plane stays in shared memory from its conversion (tick z - r) to the
+                                       // combination of its zones (until barrier B of tick z + 2) while the next one loads
   static constexpr int NREG = (RECON == FX_RECON_PLM_MINMOD) ? 96 : 168;  // registers per thread for 2 / 1 CTAs per SM: the register file is 16384 per SM sub-partition, and 18 / 9 warps put 5 / 3 on one of them
 };
 
 template <int RECON> struct alignas(128) Smem {
-  static constexpr int R = Rc<RECON>::R, NP = Rc<RECON>::NP, BW = Rc<RECON>::BW;
-  double rawX[2][5][NY][NX];   // TMA: stage-input planes, ring slot = tick & 1
-  double U0[2][5][NY][NX];     // TMA: U0 planes, slot = plane & 1
-  double Xs[5][NY][NX];        // TMA: stage-input plane of the zone being combined (later stages only)
+  static constexpr int R = Rc<RECON>::R, NP = Rc<RECON>::NP, BW = Rc<RECON>::BW, NRING = Rc<RECON>::NRING;
+  double ring[NRING][5][NY][NX];  // TMA: stage-input planes, plane z in slot z mod NRING; read twice: converted to
+                                  // primitives for the fluxes, and again as X (or, in the first stage, U0 = X) by the combine
+  double U0[2][5][NY][NX];     // TMA: U0 planes, slot = plane & 1 (later stages; in the first stage U0 is the stage input)
   double Out[5][NY][NX];       // result plane, drained by a TMA store
-  double Hx[2][2][5][NY][BW];  // TMA: [slot][lo|hi] raw x-halo cells of the plane
-  double Hy[2][2][5][R][NX];   // TMA: [slot][lo|hi] raw y-halo cells of the plane
+  double Hx[2][5][NY][BW];     // TMA: [lo|hi] raw x-halo cells of the plane (one slot: the edge warp alone reads it)
+  double Hy[2][5][R][NX];      // TMA: [lo|hi] raw y-halo cells of the plane
   double P[5][NP][NP + 1];     // primitives of the plane incl. halo rows/columns (corners unused); the odd row
                                // stride keeps the edge warp's column accesses free of bank conflicts
   double Lx[5][NY][NX + 1];    // Lx[v][j][i] = plus-side x state of cell (i-1,j), then the x flux at face i-1/2
@@ -61,7 +63,7 @@ template <int RECON> struct alignas(128) Smem {
   double rd[3];                // beta dt / dx_d of this block (beta = 1 in the first stage)
   double idx[3];               // 1 / dx_d (DTOUT: the CFL rate of the finished state is formed in the last stage)
   double wmax[8];              // DTOUT: per-warp maximum of (|u_d| + c) / dx_d
-  unsigned long long barX[2], barH[2], barS;  // barX[c & 1]: stage-input plane of tick c AND the U0 plane of plane c - 1
+  unsigned long long barX[2], barH;  // barX[c & 1]: stage-input plane of tick c AND (later stages) the U0 plane of plane c - 1
 };
 
 __device__ __forceinline__ void cta_sync() { asm volatile("bar.sync 0, %0;" ::"n"(NTHREADS) : "memory"); }
@@ -201,6 +203,7 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
                const double *__restrict__ dx, double dt, const double *dt_dev, double beta,
                double cfl_next, double *dt_next) {  // dt_next may be dt_dev (fx_hydro_step): read at the start, written by the last CTA
   constexpr int r = Rc<RECON>::r, R = Rc<RECON>::R, W = 2 * r + 1, NP = Rc<RECON>::NP, BW = Rc<RECON>::BW;
+  constexpr int NRING = Rc<RECON>::NRING;
   extern __shared__ __align__(1024) unsigned char fx_smem_raw[];  // TMA destinations need 128-byte alignment
   Smem<RECON> &S = *reinterpret_cast<Smem<RECON> *>(fx_smem_raw);
   const int b = blockIdx.x;
@@ -223,37 +226,30 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
     int bs, kp;
     z_source(P, b, zlo, zhi, c + r, bs, kp);
     mbar_expect_tx(&S.barX[c & 1], PLANE_BYTES);
-    tma_load(&S.rawX[c & 1][0][0][0], &mXm, &S.barX[c & 1], g0, g1, kp, bs);
+    tma_load(&S.ring[(c + r) % NRING][0][0][0], &mXm, &S.barX[c & 1], g0, g1, kp, bs);
   };
   auto issue_H = [&](int p) {  // halo cells of interior plane p
-    const int s = p & 1, kp = p + g2;
-    mbar_expect_tx(&S.barH[s], 2 * 5 * NY * BW * 8 + 2 * 5 * R * NX * 8);
-    tma_load(&S.Hx[s][0][0][0][0], &mXx, &S.barH[s], g0 + (xlo >= 0 ? NX - BW : 0), g1, kp, xlo >= 0 ? xlo : b);
-    tma_load(&S.Hx[s][1][0][0][0], &mXx, &S.barH[s], g0 + (xhi >= 0 ? 0 : NX - BW), g1, kp, xhi >= 0 ? xhi : b);
-    tma_load(&S.Hy[s][0][0][0][0], &mXy, &S.barH[s], g0, g1 + (ylo >= 0 ? NY - R : 0), kp, ylo >= 0 ? ylo : b);
-    tma_load(&S.Hy[s][1][0][0][0], &mXy, &S.barH[s], g0, g1 + (yhi >= 0 ? 0 : NY - R), kp, yhi >= 0 ? yhi : b);
+    const int kp = p + g2;
+    mbar_expect_tx(&S.barH, 2 * 5 * NY * BW * 8 + 2 * 5 * R * NX * 8);
+    tma_load(&S.Hx[0][0][0][0], &mXx, &S.barH, g0 + (xlo >= 0 ? NX - BW : 0), g1, kp, xlo >= 0 ? xlo : b);
+    tma_load(&S.Hx[1][0][0][0], &mXx, &S.barH, g0 + (xhi >= 0 ? 0 : NX - BW), g1, kp, xhi >= 0 ? xhi : b);
+    tma_load(&S.Hy[0][0][0][0], &mXy, &S.barH, g0, g1 + (ylo >= 0 ? NY - R : 0), kp, ylo >= 0 ? ylo : b);
+    tma_load(&S.Hy[1][0][0][0], &mXy, &S.barH, g0, g1 + (yhi >= 0 ? 0 : NY - R), kp, yhi >= 0 ? yhi : b);
   };
   auto issue_U0 = [&](int p) {
     // completes on the barrier of tick p + 1, the tick that combines plane p: one wait per tick covers both loads
     mbar_expect_tx(&S.barX[(p + 1) & 1], PLANE_BYTES);
     tma_load(&S.U0[p & 1][0][0][0], &mU0, &S.barX[(p + 1) & 1], g0, g1, p + g2, b);
   };
-  auto issue_Xs = [&](int p) {
-    mbar_expect_tx(&S.barS, PLANE_BYTES);
-    tma_load(&S.Xs[0][0][0], &mXm, &S.barS, g0, g1, p + g2, b);
-  };
   if (producer) {
-    mbar_init(&S.barX[0], 2); mbar_init(&S.barX[1], 2);  // two arrivals per tick: issue_X(c) and issue_U0(c - 1)
-    mbar_init(&S.barH[0], 1); mbar_init(&S.barH[1], 1);
-    mbar_init(&S.barS, 1);
+    // arrivals per tick: issue_X(c) and, in the later stages, issue_U0(c - 1)
+    mbar_init(&S.barX[0], FIRST ? 1 : 2); mbar_init(&S.barX[1], FIRST ? 1 : 2);
+    mbar_init(&S.barH, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     fence_async_smem();
     issue_X(1);
-    if (nz >= 2) issue_X(2);
     issue_H(0);
-    if (nz >= 2) issue_H(1);
-    issue_U0(0);
-    if (!FIRST) issue_Xs(0);
+    if (!FIRST) issue_U0(0);
   }
   if (dt_dev) dt = *dt_dev;
   if (tid < 3) {
@@ -287,6 +283,10 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
         double u[5];
 #pragma unroll
         for (int v = 0; v < 5; ++v) u[v] = w[m][v];
+        if (m >= R) {  // this block's planes 0 .. r do not come through the TMA ring: keep them there for the combine
+#pragma unroll
+          for (int v = 0; v < 5; ++v) S.ring[(m - R) % NRING][v][j][i] = u[v];
+        }
         const unsigned h = fx_c2p_v2(P, u[0], u[1], u[2], u[3], u[4], w[m]);
         if (m >= R && m - R < nz) hit |= h;  // a zone's floor hits are counted by its owner only
       }
@@ -333,7 +333,7 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
          // before it arrived at barrier B, and the barrier orders that observation before these reads
         double u[5];
 #pragma unroll
-        for (int v = 0; v < 5; ++v) u[v] = S.rawX[c & 1][v][j][i];
+        for (int v = 0; v < 5; ++v) u[v] = S.ring[(c + r) % NRING][v][j][i];
         const unsigned h = fx_c2p_v2(P, u[0], u[1], u[2], u[3], u[4], q[2 * r]);
         if (c + r < nz) hit |= h;
       }
@@ -375,8 +375,9 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
           const double dFx = S.Lx[v][j][i + 1] - Fx[v];
           const double dFy = S.Ly[v][j + 1][i] - Fy[v];
           const double dFz = Fz_new[v] - Fz[v];
-          const double u0 = S.U0[p & 1][v][j][i];
-          const double a = FIRST ? u0 : fma(beta, S.Xs[v][j][i] - u0, u0);
+          const double xs = S.ring[p % NRING][v][j][i];  // the zone's stage input; in the first stage it is U0
+          const double u0 = FIRST ? xs : S.U0[p & 1][v][j][i];
+          const double a = FIRST ? u0 : fma(beta, xs - u0, u0);
           const double res = fma(-rz, dFz, fma(-ry, dFy, fma(-rx, dFx, a)));
           S.Out[v][j][i] = res;
           res5[v] = res;
@@ -430,9 +431,8 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
     const int hv = isx ? HXV : HYV;
 
     auto halo_plane = [&](int pl) {  // primitives of the halo cells of plane pl into P
-      const int s = pl & 1;
-      mbar_wait(&S.barH[s], (pl >> 1) & 1);
-      const double *Hf = isx ? &S.Hx[s][0][0][0][0] : &S.Hy[s][0][0][0][0];
+      mbar_wait(&S.barH, pl & 1);
+      const double *Hf = isx ? &S.Hx[0][0][0][0] : &S.Hy[0][0][0][0];
 #pragma unroll
       for (int t = 0; t < 2 * R; ++t) {
         double u[5], w[5];
@@ -443,6 +443,8 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
 #pragma unroll
         for (int v = 0; v < 5; ++v) Pf[v * NP * NPS + pos * pd + (m + R) * pt] = w[v];
       }
+      __syncwarp();  // every lane has read its raw halo cells: the (single) slot can take the next plane's
+      if (lane == 0 && pl + 1 < nz) issue_H(pl + 1);
     };
     halo_plane(0);
     cta_sync();  // A0
@@ -473,14 +475,14 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
       mbar_wait(&S.barX[c & 1], ((c - 1) >> 1) & 1);
       cta_sync();  // B
       if (lane == 0) {
-        // every slot consumed before barrier B of this tick is free again
-        if (p + 2 < nz) issue_H(p + 2);
+        // every slot whose last reader finished before barrier B of this tick is free again: the ring slot of plane p - 1
+        // (combined in the phase that just ended) takes the plane of the next tick
+        if (c + 1 <= nz) issue_X(c + 1);
         if (p >= 1) {
           tma_store(&mOut, &S.Out[0][0][0], g0, g1, p - 1 + g2, b);
           tma_commit();
         }
-        if (p + 1 < nz) issue_U0(p + 1);
-        if (!FIRST && p >= 1) issue_Xs(p);
+        if (!FIRST && p + 1 < nz) issue_U0(p + 1);
       }
       {
         double WL[5];
@@ -501,10 +503,7 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
       }
       if (c < nz) halo_plane(c);                  // halo of plane p + 1: nobody reads P between barriers B and C
       if (lane == 0 && p >= 1) tma_wait_read();  // Out is free for the combine after barrier C
-      if (!FIRST) mbar_wait(&S.barS, p & 1);     // the combine's stage-input plane has landed
       cta_sync();  // C
-      // the zone threads read this tick's stage-input plane between barriers B and C: its slot is free only now
-      if (lane == 0 && c + 2 <= nz) issue_X(c + 2);
     }
     cta_sync();  // D
     if (lane == 0) {
@@ -627,6 +626,7 @@ int fx_launch_stage_tma(const FxParams &P, const double *X, const double *U0, do
                         const double *dt_dev, double beta, int first, double cfl_next, double *dt_next, cudaStream_t st) {
   if (!fx_stage_tma_supported(P)) return fx_fail(FX_ERR_UNSUPPORTED, "TMA stage kernel: block shape not supported");
   if (P.nblocks == 0) return FX_OK;
+  if (first && X != U0) return fx_fail(FX_ERR_INVALID_ARG, "TMA stage kernel: the first stage takes U0 from its stage input (X must be U0)");
   if (((uintptr_t)X | (uintptr_t)U0 | (uintptr_t)out) & 15)
     return fx_fail(FX_ERR_INVALID_ARG, "TMA stage kernel: state arrays must be 16-byte aligned");
   if (P.recon == FX_RECON_PLM_MINMOD) {
