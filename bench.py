@@ -42,6 +42,7 @@ def parse_args():
     ap.add_argument("--config", type=int, default=5)
     ap.add_argument("--nb", default=None, help="override blocks per dimension, e.g. 16,16,16")
     ap.add_argument("--path", type=int, default=0, help="FX_OPT_PATH: 0 auto (fused TMA stage kernel when supported), 1 generic")
+    ap.add_argument("--zchain", type=int, default=0, help="FX_OPT_ZCHAIN: z-neighbour blocks per CTA of the fused kernel (0 = library default)")
     ap.add_argument("--order", default="morton", choices=["lex", "morton"])
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -133,6 +134,8 @@ def build_workload(args, device):
     plan = fx.HydroPlan(cfg.block_dims, cfg.nguard, cfg.nblocks, cfg.gamma, cfg.recon, cfg.riemann, cfg.rk_order,
                         device=device)
     plan.fx_hydro_plan_set_option(fx.OPT_PATH, args.path)
+    if args.zchain:
+        plan.fx_hydro_plan_set_option(fx.OPT_ZCHAIN, args.zchain)
     plan.fx_hydro_plan_set_topology(neigh)
     plan.fx_hydro_plan_set_workspace()
     U = torch.full(plan.shape, float("nan"), dtype=torch.float64, device=device)

@@ -48,7 +48,9 @@ enum {
   FX_OPT_P_FLOOR = 1,   /* primitive pressure floor, default 1e-12 [A7] */
   FX_OPT_WENO_EPS = 2,  /* WENO5-JS epsilon, default 1e-6 [A5] */
   FX_OPT_WAVESPEED = 3, /* 0 = Einfeldt (default), 1 = Davis [A8] */
-  FX_OPT_PATH = 4       /* 0 = auto (fused TMA stage kernel when the block shape allows), 1 = generic */
+  FX_OPT_PATH = 4,      /* 0 = auto (fused TMA stage kernel when the block shape allows), 1 = generic */
+  FX_OPT_ZCHAIN = 5     /* fused path: longest chain of z-neighbour blocks one CTA marches through, 1..8 (default 8);
+                           set before fx_hydro_plan_set_topology.  Results do not depend on it. */
 };
 enum {
   FX_STATUS_NONFINITE = 1u,
@@ -84,9 +86,10 @@ int fx_hydro_plan_layout(const fx_hydro_plan *plan, fx_layout *out);
 /* Options; must be set before the first advance.  Unknown key / bad value -> FX_ERR_INVALID_ARG. */
 int fx_hydro_plan_set_option(fx_hydro_plan *plan, int key, double value);
 
-/* Workspace (device, caller-owned, 256-byte aligned): (rk_order - 1) state copies for the RK stages
- * + a 256-byte scratch block (dt reduction word, status word and counters).  set_workspace
- * initialises the scratch block and synchronises the device once. */
+/* Workspace (device, caller-owned, 256-byte aligned): a 256-byte scratch block (dt reduction word,
+ * status word and counters) + (rk_order - 1) state copies for the RK stages + the z-segment table
+ * (12 int32 per block, see FX_OPT_ZCHAIN).  set_workspace initialises the scratch block and
+ * synchronises the device once. */
 size_t fx_hydro_plan_workspace_bytes(const fx_hydro_plan *plan);
 int fx_hydro_plan_set_workspace(fx_hydro_plan *plan, void *workspace_dev, size_t bytes);
 

@@ -20,7 +20,7 @@ RIEMANN_HLLE, RIEMANN_HLLC = 0, 1
 BC_OUTFLOW, BC_NONE = -1, -2
 TOPO_PERIODIC, TOPO_OUTFLOW, TOPO_NONE = 0, 1, 2
 ORDER_LEX, ORDER_MORTON = 0, 1
-OPT_RHO_FLOOR, OPT_P_FLOOR, OPT_WENO_EPS, OPT_WAVESPEED, OPT_PATH = 0, 1, 2, 3, 4
+OPT_RHO_FLOOR, OPT_P_FLOOR, OPT_WENO_EPS, OPT_WAVESPEED, OPT_PATH, OPT_ZCHAIN = 0, 1, 2, 3, 4, 5
 STATUS_NONFINITE, STATUS_RHO_FLOOR, STATUS_P_FLOOR, STATUS_WENO_FALLBACK = 1, 2, 4, 8
 
 EXPORTS = [

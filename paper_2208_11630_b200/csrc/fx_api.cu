@@ -86,6 +86,7 @@ extern "C" int fx_hydro_plan_create(fx_hydro_plan **out, const int block_dims[3]
   P.recon = recon;
   P.riemann = riemann;
   P.wavespeed = 0;
+  p->zchain = FX_SEG_MAX;
   p->nguard = nguard;
   p->nvars = nvars;
   p->rk = rk_order;
@@ -94,6 +95,7 @@ extern "C" int fx_hydro_plan_create(fx_hydro_plan **out, const int block_dims[3]
 }
 
 extern "C" int fx_hydro_plan_destroy(fx_hydro_plan *plan) {
+  if (plan) delete[] plan->seg_host;
   if (plan && plan->ev) {
     for (int i = 0; i < 2 * FX_MAX_REC; ++i) cudaEventDestroy(plan->ev[i]);
     delete[] plan->ev;
@@ -129,6 +131,10 @@ extern "C" int fx_hydro_plan_set_option(fx_hydro_plan *plan, int key, double val
     if (value != 0.0 && value != 1.0) return fx_fail(FX_ERR_INVALID_ARG, "set_option: wavespeed must be 0 or 1");
     plan->P.wavespeed = (int)value;
     return FX_OK;
+  case FX_OPT_ZCHAIN:
+    if (!(value >= 1.0 && value <= (double)FX_SEG_MAX)) return fx_fail(FX_ERR_INVALID_ARG, "set_option: zchain must be 1..%d", (int)FX_SEG_MAX);
+    plan->zchain = (int)value;
+    return FX_OK;
   case FX_OPT_PATH:
     if (value != 0.0 && value != 1.0) return fx_fail(FX_ERR_INVALID_ARG, "set_option: path must be 0 or 1");
     plan->path_option = (int)value;
@@ -147,9 +153,25 @@ static size_t fx_state_bytes_aligned(const fx_hydro_plan *plan) {
   return (b + 255) & ~(size_t)255;
 }
 
+static size_t fx_seg_bytes(const fx_hydro_plan *plan) {  // room for one segment per block
+  return (((size_t)plan->P.nblocks * FX_SEG_STRIDE * sizeof(int)) + 255) & ~(size_t)255;
+}
+
 extern "C" size_t fx_hydro_plan_workspace_bytes(const fx_hydro_plan *plan) {
   if (!plan) return 0;
-  return (size_t)FX_SCR_WORDS * 8 + (size_t)(plan->rk - 1) * fx_state_bytes_aligned(plan);
+  return (size_t)FX_SCR_WORDS * 8 + (size_t)(plan->rk - 1) * fx_state_bytes_aligned(plan) + fx_seg_bytes(plan);
+}
+
+// Upload the segment table into its place behind the stage copies (needs both the workspace and the topology).
+static int fx_seg_upload(fx_hydro_plan *plan) {
+  if (!plan->workspace || !plan->seg_host) return FX_OK;
+  int *dst = (int *)((char *)plan->workspace + FX_SCR_WORDS * 8 + (size_t)(plan->rk - 1) * fx_state_bytes_aligned(plan));
+  if (plan->nseg_host > 0)
+    FX_CUDA(cudaMemcpy(dst, plan->seg_host, (size_t)plan->nseg_host * FX_SEG_STRIDE * sizeof(int), cudaMemcpyHostToDevice));
+  plan->P.seg = dst;
+  plan->P.nseg = plan->nseg_host;
+  plan->seg_uploaded = true;
+  return FX_OK;
 }
 
 extern "C" int fx_hydro_plan_set_workspace(fx_hydro_plan *plan, void *ws, size_t bytes) {
@@ -168,7 +190,7 @@ extern "C" int fx_hydro_plan_set_workspace(fx_hydro_plan *plan, void *ws, size_t
   char *base = (char *)ws + FX_SCR_WORDS * 8;
   plan->stage[0] = (double *)base;
   plan->stage[1] = plan->rk == 3 ? (double *)(base + fx_state_bytes_aligned(plan)) : nullptr;
-  return FX_OK;
+  return fx_seg_upload(plan);
 }
 
 // ------------------------------------------------------------------ topology
@@ -192,7 +214,59 @@ extern "C" int fx_hydro_plan_set_topology(fx_hydro_plan *plan, const int32_t *ne
   }
   plan->P.neigh = neigh_dev;
   plan->topology_set = true;
-  return FX_OK;
+  // z-chain segments: walk down (-z) from every unvisited block to the start of its chain (or once around a periodic
+  // ring), then up (+z), cutting every `zchain` blocks and wherever the two blocks do not name each other
+  delete[] plan->seg_host;
+  plan->seg_host = nullptr;
+  plan->nseg_host = 0;
+  plan->seg_uploaded = false;
+  if (nb > 0) {
+    std::vector<int32_t> h((size_t)nb * 6);
+    FX_CUDA(cudaMemcpy(h.data(), neigh_dev, h.size() * sizeof(int32_t), cudaMemcpyDeviceToHost));
+    const bool zact = plan->P.active[2] != 0;
+    auto up = [&](long long b) -> long long {  // the block above b if the link is mutual, else -1
+      if (!zact) return -1;
+      const long long a = h[b * 6 + 5];
+      return (a >= 0 && a != b && h[a * 6 + 4] == b) ? a : -1;
+    };
+    auto down = [&](long long b) -> long long {
+      if (!zact) return -1;
+      const long long a = h[b * 6 + 4];
+      return (a >= 0 && a != b && h[a * 6 + 5] == b) ? a : -1;
+    };
+    std::vector<char> seen((size_t)nb, 0);
+    plan->seg_host = new (std::nothrow) int[(size_t)nb * FX_SEG_STRIDE];
+    if (!plan->seg_host) return fx_fail(FX_ERR_INVALID_ARG, "set_topology: out of host memory");
+    // (blocks taller than 64 planes are not chained: the kernel's plane -> block map is exact up to 2^20 / nz planes)
+    const int M = (plan->zchain < 1 || plan->P.n[2] > 64) ? 1 : (plan->zchain > FX_SEG_MAX ? FX_SEG_MAX : plan->zchain);
+    for (long long b0 = 0; b0 < nb; ++b0) {
+      if (seen[b0]) continue;
+      long long start = b0;
+      for (long long steps = 0; steps < nb; ++steps) {
+        const long long d = down(start);
+        if (d < 0 || seen[d] || d == b0) break;
+        start = d;
+      }
+      long long b = start;
+      while (b >= 0 && !seen[b]) {
+        int *row = plan->seg_host + (size_t)plan->nseg_host * FX_SEG_STRIDE;
+        for (int q = 0; q < FX_SEG_STRIDE; ++q) row[q] = -1;
+        int cnt = 0;
+        row[1] = zact ? h[b * 6 + 4] : -1;
+        long long last = b;
+        while (b >= 0 && !seen[b] && cnt < M) {
+          seen[b] = 1;
+          row[2 + cnt++] = (int)b;
+          last = b;
+          b = up(b);
+        }
+        row[0] = cnt;
+        row[2 + cnt] = zact ? h[last * 6 + 5] : -1;
+        ++plan->nseg_host;
+      }
+    }
+  }
+  return fx_seg_upload(plan);
 }
 
 static uint64_t fx_morton3(uint32_t x, uint32_t y, uint32_t z) {

@@ -17,8 +17,15 @@ struct FxParams {
   double rho_floor, p_floor, weno_eps;
   int recon, riemann, wavespeed;
   const int *neigh;                 // [nblocks][6], device
+  const int *seg;                   // z-chain segments of the fused kernel: [nseg][FX_SEG_STRIDE], device (in the workspace)
+  int nseg;
   unsigned long long *scratch;      // device scratch block, see FX_SCR_*
 };
+
+// A segment = up to FX_SEG_MAX blocks that follow one another in +z (each the other's z neighbour both ways); one CTA
+// of the fused stage kernel marches through a whole segment.  Row: {count, below, id_0 .. id_{count-1}, above}, where
+// below / above are the z neighbours of the first / last block as the neighbour table gives them (id or FX_BC_OUTFLOW).
+enum { FX_SEG_MAX = 8, FX_SEG_STRIDE = 12 };
 
 // 64-bit words of the scratch block
 enum {
@@ -37,6 +44,10 @@ struct fx_hydro_plan {
   size_t workspace_bytes;
   double *stage[2];     // RK stage copies inside the workspace
   bool topology_set;
+  int zchain;           // FX_OPT_ZCHAIN: longest segment (1 .. FX_SEG_MAX)
+  int *seg_host;        // segment table built by set_topology (new[]), nseg_host rows
+  int nseg_host;
+  bool seg_uploaded;
   // optional per-launch timing of the stage kernels (fx_hydro_plan_set_timing)
   bool timing;
   cudaEvent_t *ev;  // 2 * FX_MAX_REC events, created on demand

@@ -60,8 +60,10 @@ template <int RECON> struct alignas(128) Smem {
                                // stride keeps the edge warp's column accesses free of bank conflicts
   double Lx[5][NY][NX + 1];    // Lx[v][j][i] = plus-side x state of cell (i-1,j), then the x flux at face i-1/2
   double Ly[5][NY + 1][NX];    // Ly[v][j][i] = plus-side y state of cell (i,j-1), then the y flux at face j-1/2
-  double rd[3];                // beta dt / dx_d of this block (beta = 1 in the first stage)
+  double rd[3];                // beta dt / dx_d (beta = 1 in the first stage) of the block whose planes are being combined;
+                               // rewritten by the edge warp between barriers B and C of a block's first tick
   double idx[3];               // 1 / dx_d (DTOUT: the CFL rate of the finished state is formed in the last stage)
+  int chain[FX_SEG_STRIDE];    // this CTA's segment: {count, below, id_0 .. id_{count-1}, above}
   double wmax[8];              // DTOUT: per-warp maximum of (|u_d| + c) / dx_d
   unsigned long long barX[2], barH;  // barX[c & 1]: stage-input plane of tick c AND (later stages) the U0 plane of plane c - 1
 };
@@ -114,26 +116,33 @@ __device__ __forceinline__ void recon_cell(const double *s, double eps, double &
   } else {
     // WENO5-JS, both faces of the cell share the smoothness indicators (beta_0 <-> beta_2 under mirroring)
     const double a = s[0], b = s[1], c = s[2], d = s[3], e = s[4];
+    // Every product and sum is written out (fma / _rn intrinsics): the compiler may not contract these expressions one
+    // way in one inlined copy and another way in the next, so a face value does not depend on which part of the kernel
+    // (prologue or z loop) evaluated it, and the result is bit for bit the same whatever the z-chain length.
+    const double t0 = fma(-2.0, b, __dadd_rn(a, c)), u0 = fma(3.0, c, fma(-4.0, b, a));
+    const double t1 = fma(-2.0, c, __dadd_rn(b, d)), u1 = __dsub_rn(b, d);
+    const double t2 = fma(-2.0, d, __dadd_rn(c, e)), u2 = fma(3.0, c, fma(-4.0, d, e));
+    const double b0 = fma(13.0 / 12.0, __dmul_rn(t0, t0), fma(0.25, __dmul_rn(u0, u0), eps));
+    const double b1 = fma(13.0 / 12.0, __dmul_rn(t1, t1), fma(0.25, __dmul_rn(u1, u1), eps));
+    const double b2 = fma(13.0 / 12.0, __dmul_rn(t2, t2), fma(0.25, __dmul_rn(u2, u2), eps));
+    const double q0 = __dmul_rn(b1, b2), q1 = __dmul_rn(b0, b2), q2 = __dmul_rn(b0, b1);
+    // ~ 1/b0^2, 1/b1^2, 1/b2^2 up to a common factor
+    const double s0 = __dmul_rn(q0, q0), s1 = __dmul_rn(q1, q1), s2 = __dmul_rn(q2, q2);
     const double sixth = 1.0 / 6.0;
-    const double t0 = a - 2.0 * b + c, u0 = a - 4.0 * b + 3.0 * c;
-    const double t1 = b - 2.0 * c + d, u1 = b - d;
-    const double t2 = c - 2.0 * d + e, u2 = 3.0 * c - 4.0 * d + e;
-    const double b0 = (13.0 / 12.0) * (t0 * t0) + 0.25 * (u0 * u0) + eps;
-    const double b1 = (13.0 / 12.0) * (t1 * t1) + 0.25 * (u1 * u1) + eps;
-    const double b2 = (13.0 / 12.0) * (t2 * t2) + 0.25 * (u2 * u2) + eps;
-    const double q0 = b1 * b2, q1 = b0 * b2, q2 = b0 * b1;
-    const double s0 = q0 * q0, s1 = q1 * q1, s2 = q2 * q2;  // ~ 1/b0^2, 1/b1^2, 1/b2^2 up to a common factor
-    {  // plus face: candidates from (a,b,c), (b,c,d), (c,d,e); weights 0.1, 0.6, 0.3
-      const double p0 = (2.0 * a - 7.0 * b + 11.0 * c) * sixth, p1 = (-b + 5.0 * c + 2.0 * d) * sixth,
-                   p2 = (2.0 * c + 5.0 * d - e) * sixth;
-      const double a0 = 0.1 * s0, a1 = 0.6 * s1, a2 = 0.3 * s2;
-      qp = (a0 * p0 + a1 * p1 + a2 * p2) * fx_rcp3(a0 + a1 + a2);  // the weights' sum is positive and far from the subnormal range
+    {  // plus face: candidates (times 6) from (a,b,c), (b,c,d), (c,d,e); weights 0.1, 0.6, 0.3
+      const double p0 = fma(2.0, a, fma(-7.0, b, __dmul_rn(11.0, c))), p1 = fma(2.0, d, fma(5.0, c, -b)),
+                   p2 = fma(2.0, c, fma(5.0, d, -e));
+      const double a0 = __dmul_rn(0.1, s0), a1 = __dmul_rn(0.6, s1), a2 = __dmul_rn(0.3, s2);
+      const double num = fma(a0, p0, fma(a1, p1, __dmul_rn(a2, p2)));
+      // the weights' sum is positive and far from the subnormal range
+      qp = __dmul_rn(num, __dmul_rn(sixth, fx_rcp3(__dadd_rn(__dadd_rn(a0, a1), a2))));
     }
     {  // minus face: mirrored stencil (e,d,c,b,a)
-      const double p0 = (2.0 * e - 7.0 * d + 11.0 * c) * sixth, p1 = (-d + 5.0 * c + 2.0 * b) * sixth,
-                   p2 = (2.0 * c + 5.0 * b - a) * sixth;
-      const double a0 = 0.1 * s2, a1 = 0.6 * s1, a2 = 0.3 * s0;
-      qm = (a0 * p0 + a1 * p1 + a2 * p2) * fx_rcp3(a0 + a1 + a2);
+      const double p0 = fma(2.0, e, fma(-7.0, d, __dmul_rn(11.0, c))), p1 = fma(2.0, b, fma(5.0, c, -d)),
+                   p2 = fma(2.0, c, fma(5.0, b, -a));
+      const double a0 = __dmul_rn(0.1, s2), a1 = __dmul_rn(0.6, s1), a2 = __dmul_rn(0.3, s0);
+      const double num = fma(a0, p0, fma(a1, p1, __dmul_rn(a2, p2)));
+      qm = __dmul_rn(num, __dmul_rn(sixth, fx_rcp3(__dadd_rn(__dadd_rn(a0, a1), a2))));
     }
   }
 }
@@ -182,19 +191,6 @@ __device__ __forceinline__ void flux_dir(const FxParams &P, const double WL[5], 
   F[4] = f[4];
 }
 
-// Where plane k (k in [-R, nz+R)) of this block's column lives: block id and padded k index.  Outflow
-// clamps to the nearest interior plane of this block [O1].
-__device__ __forceinline__ void z_source(const FxParams &P, int b, int nlo, int nhi, int k, int &bs, int &kp) {
-  const int nz = P.n[2];
-  bs = b;
-  if (k < 0) {
-    if (nlo >= 0) { bs = nlo; k += nz; } else k = 0;
-  } else if (k >= nz) {
-    if (nhi >= 0) { bs = nhi; k -= nz; } else k = nz - 1;
-  }
-  kp = k + P.gd[2];
-}
-
 template <int RECON, int RIEMANN, int WS, bool FIRST, bool DTOUT>
 __global__ void __launch_bounds__(NTHREADS) __maxnreg__(Rc<RECON>::NREG)
 fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ CUtensorMap mXx,
@@ -206,40 +202,62 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
   constexpr int NRING = Rc<RECON>::NRING;
   extern __shared__ __align__(1024) unsigned char fx_smem_raw[];  // TMA destinations need 128-byte alignment
   Smem<RECON> &S = *reinterpret_cast<Smem<RECON> *>(fx_smem_raw);
-  const int b = blockIdx.x;
   const int tid = threadIdx.x;
-  const int nz = P.n[2];
+  const int nzb = P.n[2];  // planes per block
   const int g0 = P.gd[0], g1 = P.gd[1], g2 = P.gd[2];
-  const int zlo = __ldg(&P.neigh[(long long)b * 6 + 4]), zhi = __ldg(&P.neigh[(long long)b * 6 + 5]);
   unsigned hit = 0;
+  // This CTA marches through a SEGMENT: M blocks that follow one another in +z, as one column of nz = M nzb planes.
+  // A block's top halo is then the next block's first planes, already on their way through the ring: they are
+  // neither loaded nor converted twice, and the pipeline is filled once per segment instead of once per block.
+  if (tid < FX_SEG_STRIDE) S.chain[tid] = __ldg(&P.seg[(long long)blockIdx.x * FX_SEG_STRIDE + tid]);
+  __syncthreads();
+  const int M = S.chain[0];
+  const int nz = M * nzb;
+  // where plane Z of the column (Z in [-R, nz + R)) lives: block id and padded k.  Outflow below / above the segment
+  // clamps to the nearest interior plane [O1].
+  // Z / nzb without a division: exact for Z < 2^20 / nzb, and the host only chains blocks of at most 64 planes
+  const unsigned zmagic = ((1u << 20) + (unsigned)nzb - 1u) / (unsigned)nzb;
+  auto zmap = [&](int Z, int &bs, int &kp) {
+    int qb = Z < 0 ? -1 : (M == 1 ? (int)(Z >= nzb) : (int)(((unsigned)Z * zmagic) >> 20));
+    int k = Z - qb * nzb;
+    int id = S.chain[2 + qb];
+    if (id < 0) {
+      if (qb < 0) { id = S.chain[2]; k = 0; } else { id = S.chain[1 + M]; k = nzb - 1; }
+    }
+    bs = id;
+    kp = k + g2;
+  };
 
   // ---------------------------------------------------------------- producer set-up (edge warp, lane 0)
   const bool producer = tid == NZONE_THREADS;
-  int xlo = 0, xhi = 0, ylo = 0, yhi = 0;
-  if (tid >= NZONE_THREADS) {
-    xlo = __ldg(&P.neigh[(long long)b * 6 + 0]);
-    xhi = __ldg(&P.neigh[(long long)b * 6 + 1]);
-    ylo = __ldg(&P.neigh[(long long)b * 6 + 2]);
-    yhi = __ldg(&P.neigh[(long long)b * 6 + 3]);
-  }
   auto issue_X = [&](int c) {  // stage-input plane consumed at tick c: z index c + r
     int bs, kp;
-    z_source(P, b, zlo, zhi, c + r, bs, kp);
+    zmap(c + r, bs, kp);
     mbar_expect_tx(&S.barX[c & 1], PLANE_BYTES);
     tma_load(&S.ring[(c + r) % NRING][0][0][0], &mXm, &S.barX[c & 1], g0, g1, kp, bs);
   };
-  auto issue_H = [&](int p) {  // halo cells of interior plane p
-    const int kp = p + g2;
+  // edge warp: the block the next halo plane is in (plane hk of block hq of the segment) and its x / y neighbours
+  int hk = 0, hq = 0, hb = 0, xlo = 0, xhi = 0, ylo = 0, yhi = 0;
+  auto halo_block = [&]() {
+    hb = S.chain[2 + hq];
+    xlo = __ldg(&P.neigh[(long long)hb * 6 + 0]);
+    xhi = __ldg(&P.neigh[(long long)hb * 6 + 1]);
+    ylo = __ldg(&P.neigh[(long long)hb * 6 + 2]);
+    yhi = __ldg(&P.neigh[(long long)hb * 6 + 3]);
+  };
+  if (tid >= NZONE_THREADS) halo_block();
+  auto issue_H = [&]() {  // halo cells of interior plane hk of block hb, from the block's x and y neighbours
+    const int b = hb, kp = hk + g2;
     mbar_expect_tx(&S.barH, 2 * 5 * NY * BW * 8 + 2 * 5 * R * NX * 8);
     tma_load(&S.Hx[0][0][0][0], &mXx, &S.barH, g0 + (xlo >= 0 ? NX - BW : 0), g1, kp, xlo >= 0 ? xlo : b);
     tma_load(&S.Hx[1][0][0][0], &mXx, &S.barH, g0 + (xhi >= 0 ? 0 : NX - BW), g1, kp, xhi >= 0 ? xhi : b);
     tma_load(&S.Hy[0][0][0][0], &mXy, &S.barH, g0, g1 + (ylo >= 0 ? NY - R : 0), kp, ylo >= 0 ? ylo : b);
     tma_load(&S.Hy[1][0][0][0], &mXy, &S.barH, g0, g1 + (yhi >= 0 ? 0 : NY - R), kp, yhi >= 0 ? yhi : b);
   };
-  auto issue_U0 = [&](int p) {
+  auto issue_U0 = [&](int p, int b, int k) {  // plane p of the column = plane k of block b
     // completes on the barrier of tick p + 1, the tick that combines plane p: one wait per tick covers both loads
     mbar_expect_tx(&S.barX[(p + 1) & 1], PLANE_BYTES);
-    tma_load(&S.U0[p & 1][0][0][0], &mU0, &S.barX[(p + 1) & 1], g0, g1, p + g2, b);
+    tma_load(&S.U0[p & 1][0][0][0], &mU0, &S.barX[(p + 1) & 1], g0, g1, k + g2, b);
   };
   if (producer) {
     // arrivals per tick: issue_X(c) and, in the later stages, issue_U0(c - 1)
@@ -248,16 +266,11 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     fence_async_smem();
     issue_X(1);
-    issue_H(0);
-    if (!FIRST) issue_U0(0);
+    issue_H();
+    if (!FIRST) issue_U0(0, S.chain[2], 0);
   }
   if (dt_dev) dt = *dt_dev;
-  if (tid < 3) {
-    const double dxd = __ldg(&dx[(long long)b * 3 + tid]);
-    S.rd[tid] = (FIRST ? 1.0 : beta) * dt / dxd;
-    S.idx[tid] = 1.0 / dxd;
-  }
-  cta_sync();  // barriers initialised before anyone waits on them; rd visible
+  cta_sync();  // barriers initialised before anyone waits on them
 
   if (tid < NZONE_THREADS) {
     // ------------------------------------------------------------ zone threads
@@ -273,7 +286,7 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
 #pragma unroll
       for (int m = 0; m < 2 * R; ++m) {
         int bs, kp;
-        z_source(P, b, zlo, zhi, m - R, bs, kp);
+        zmap(m - R, bs, kp);
         const long long a = (long long)bs * P.S_b + (long long)kp * P.S_k + col;
 #pragma unroll
         for (int v = 0; v < 5; ++v) w[m][v] = X[a + v * P.S_v];
@@ -410,7 +423,6 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
     const int lane = tid - NZONE_THREADS;
     const bool isx = lane >= 16;
     const int m = lane & 15;
-    const int nlo = isx ? xlo : ylo, nhi = isx ? xhi : yhi;
     double *Pf = &S.P[0][0][0];
     constexpr int NPS = NP + 1;
     const int pd = isx ? 1 : NPS, pt = isx ? NPS : 1;  // smem strides of P along direction / transverse
@@ -419,6 +431,7 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
     constexpr int LV = NY * (NX + 1);                       // per-variable size of the L arrays (272)
     // raw halo cell t of this lane's row / column: Hx[s][side][v][m][ix], Hy[s][side][v][iy][m]
     constexpr int HXV = NY * BW, HYV = R * NX;  // per-variable sizes
+    int nlo = isx ? xlo : ylo, nhi = isx ? xhi : yhi;  // this lane's pair of neighbours of the block the halo plane is in
     auto halo_off = [&](int t, bool high) -> int {
       int idx;  // cell index inside the box
       if (isx) idx = high ? (nhi >= 0 ? t : BW - 1) : (nlo >= 0 ? BW - R + t : 0);
@@ -430,7 +443,7 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
     for (int t = 0; t < 2 * R; ++t) hoff[t] = halo_off(t % R, t >= R);
     const int hv = isx ? HXV : HYV;
 
-    auto halo_plane = [&](int pl) {  // primitives of the halo cells of plane pl into P
+    auto halo_plane = [&](int pl) {  // primitives of the halo cells of plane pl into P (called for pl = 0, 1, 2, ... in turn)
       mbar_wait(&S.barH, pl & 1);
       const double *Hf = isx ? &S.Hx[0][0][0][0] : &S.Hy[0][0][0][0];
 #pragma unroll
@@ -444,10 +457,22 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
         for (int v = 0; v < 5; ++v) Pf[v * NP * NPS + pos * pd + (m + R) * pt] = w[v];
       }
       __syncwarp();  // every lane has read its raw halo cells: the (single) slot can take the next plane's
-      if (lane == 0 && pl + 1 < nz) issue_H(pl + 1);
+      if (pl + 1 < nz) {
+        if (++hk == nzb) {  // a new block: where its halo cells sit inside the boxes depends on which neighbours exist
+          hk = 0;
+          ++hq;
+          halo_block();
+          nlo = isx ? xlo : ylo;
+          nhi = isx ? xhi : yhi;
+#pragma unroll
+          for (int t = 0; t < 2 * R; ++t) hoff[t] = halo_off(t % R, t >= R);
+        }
+        if (lane == 0) issue_H();
+      }
     };
     halo_plane(0);
     cta_sync();  // A0
+    int pk = 0, pq = 0, pb = S.chain[2], pb_prev = pb;  // plane p is plane pk of block pb, the pq-th of the segment
 
 #pragma unroll 1
     for (int c = 1; c <= nz; ++c) {
@@ -479,10 +504,13 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
         // (combined in the phase that just ended) takes the plane of the next tick
         if (c + 1 <= nz) issue_X(c + 1);
         if (p >= 1) {
-          tma_store(&mOut, &S.Out[0][0][0], g0, g1, p - 1 + g2, b);
+          tma_store(&mOut, &S.Out[0][0][0], g0, g1, (pk >= 1 ? pk - 1 : nzb - 1) + g2, pk >= 1 ? pb : pb_prev);
           tma_commit();
         }
-        if (!FIRST && p + 1 < nz) issue_U0(p + 1);
+        if (!FIRST && p + 1 < nz) {
+          if (pk + 1 < nzb) issue_U0(p + 1, pb, pk + 1);
+          else issue_U0(p + 1, S.chain[3 + pq], 0);
+        }
       }
       {
         double WL[5];
@@ -501,13 +529,25 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
 #pragma unroll
         for (int v = 0; v < 5; ++v) Lf[v * LV + NX * ld + m * lt] = F[v];
       }
+      if (pk == 0 && lane < 3) {
+        // a block's first plane: the combines of the block below ended before barrier B, this tick's starts after C
+        const double dxd = __ldg(&dx[(long long)pb * 3 + lane]);
+        S.rd[lane] = (FIRST ? 1.0 : beta) * dt / dxd;
+        if (DTOUT) S.idx[lane] = 1.0 / dxd;
+      }
+      if (++pk == nzb) {
+        pk = 0;
+        ++pq;
+        pb_prev = pb;
+        pb = S.chain[2 + pq];
+      }
       if (c < nz) halo_plane(c);                  // halo of plane p + 1: nobody reads P between barriers B and C
       if (lane == 0 && p >= 1) tma_wait_read();  // Out is free for the combine after barrier C
       cta_sync();  // C
     }
     cta_sync();  // D
     if (lane == 0) {
-      tma_store(&mOut, &S.Out[0][0][0], g0, g1, nz - 1 + g2, b);
+      tma_store(&mOut, &S.Out[0][0][0], g0, g1, nzb - 1 + g2, S.chain[1 + M]);
       tma_commit();
       if (DTOUT) {
         // CTA maximum -> scratch word (non-negative doubles order like unsigned integers); the last CTA to finish
@@ -582,7 +622,7 @@ int launch(const FxParams &P, const double *X, const double *U0, double *out, co
     FX_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     configured = true;
   }
-  kern<<<(unsigned)P.nblocks, NTHREADS, smem, st>>>(mXm, mXx, mXy, mU0, mOut, P, X, dx, dt, dt_dev, beta, cfl_next, dt_next);
+  kern<<<(unsigned)P.nseg, NTHREADS, smem, st>>>(mXm, mXx, mXy, mU0, mOut, P, X, dx, dt, dt_dev, beta, cfl_next, dt_next);
   const cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) {
     cudaFuncAttributes a;
@@ -618,7 +658,7 @@ bool fx_stage_tma_supported(const FxParams &P) {
   // TMA: global strides must be multiples of 16 bytes (S_j even), every box must start on a 16-byte boundary (guard
   // depth even: measured, a box starting at an odd element faults), the arrays 16-byte aligned (checked at launch)
   return P.n[0] == fxt::NX && P.n[1] == fxt::NY && P.n[2] >= R && P.active[2] && P.gd[0] >= R && (P.S_j % 2) == 0 &&
-         (P.gd[0] % 2) == 0 && P.nblocks <= 0x7fffffffLL;
+         (P.gd[0] % 2) == 0 && P.nblocks <= 0x7fffffffLL && P.seg != nullptr && P.nseg > 0;
 }
 
 // dt_next != nullptr (a later stage only): also form cfl_next * min dx/(|u|+c) of the finished state and write it there.

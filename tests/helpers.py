@@ -145,7 +145,7 @@ def rel_err(cfg, got, ref):
 
 
 def gpu_plan_for(cfg, order=inputs.ORDER_LEX, bc=None, nb=None, recon=None, riemann=None, rk=None, path=None,
-                 neigh=None, nblocks=None):
+                 neigh=None, nblocks=None, zchain=None):
     """CUDA-side plan + topology + workspace for a config (uses the library's own topology helper)."""
     from paper_2208_11630_b200 import binding as fx
     nb = tuple(nb or cfg.nb)
@@ -160,6 +160,8 @@ def gpu_plan_for(cfg, order=inputs.ORDER_LEX, bc=None, nb=None, recon=None, riem
                         cfg.rk_order if rk is None else rk)
     if path is not None:
         plan.fx_hydro_plan_set_option(fx.OPT_PATH, path)
+    if zchain is not None:
+        plan.fx_hydro_plan_set_option(fx.OPT_ZCHAIN, zchain)
     plan.fx_hydro_plan_set_topology(neigh)
     plan.fx_hydro_plan_set_workspace()
     return plan, neigh, coords

@@ -182,6 +182,58 @@ def test_fused_kernel_other_guard_depths_and_block_heights(nguard, recon, dims):
         assert rel_err(cfg, gplan.interior(Ud).cpu().numpy(), oplan.interior(Uo)) <= 1e-11
 
 
+@pytest.mark.parametrize("recon,rk,nzb", [(0, 2, 16), (1, 3, 16), (0, 3, 4)])
+def test_z_chains_irregular_topology_bitwise_and_parity(recon, rk, nzb):
+    """The fused kernel marches one CTA through up to FX_OPT_ZCHAIN z-neighbour blocks.  On a topology whose chains are a
+    periodic ring of 5, with one block's +x link cut (outflow on one side only), one z link that is not mutual (the chain
+    must break there) and a different dx per block: the result does not depend on the chain length, bit for bit, the
+    fused time step neither, and both agree with the oracle on the same neighbour table."""
+    from paper_2208_11630_b200 import binding as fx
+    cfg = inputs.config(5, nb=(2, 1, 5))
+    cfg.block_dims = (16, 16, nzb)
+    per, out = fx.TOPO_PERIODIC, fx.TOPO_OUTFLOW
+    neigh, coords = fx.fx_topology_cartesian((2, 1, 5), (out, per, per), (out, per, per), inputs.ORDER_LEX)
+    neigh = np.array(neigh, np.int32).copy()
+    nbk = neigh.shape[0]
+    mid = int(np.flatnonzero((coords[:, 0] == 0) & (coords[:, 2] == 2))[0])
+    neigh[mid, 1] = fx.BC_OUTFLOW                       # x = 0 column: block 2 of the chain has no +x neighbour
+    a = int(np.flatnonzero((coords[:, 0] == 1) & (coords[:, 2] == 1))[0])
+    c = int(np.flatnonzero((coords[:, 0] == 1) & (coords[:, 2] == 3))[0])
+    neigh[a, 5] = c                                     # x = 1 column: block 1 sees block 3 above it, block 2 still names 1 below
+    neigh[c, 2] = fx.BC_OUTFLOW                         # and block 3 has outflow at -y
+    oplan = fxo.OraclePlan(cfg.block_dims, cfg.nguard, nbk, cfg.gamma, recon, cfg.riemann, rk)
+    oplan.set_topology(neigh)
+    rng = np.random.default_rng(5)
+    shape = (nbk, nzb, 16, 16)
+    rho = 1.0 + 0.3 * rng.random(shape)
+    vel = 0.4 * rng.standard_normal((3,) + shape)
+    pr = 1.0 + 0.3 * rng.random(shape)
+    Ui = np.stack([rho, rho * vel[0], rho * vel[1], rho * vel[2], pr / (cfg.gamma - 1) + 0.5 * rho * (vel ** 2).sum(0)])
+    Uh = inputs.embed(cfg, torch.from_numpy(Ui))
+    dx = rng.uniform(1.0 / 40, 1.0 / 24, size=(nbk, 3))
+    Uo = Uh.numpy().copy()
+    dts_o = []
+    for step in range(2):
+        dts_o.append(oplan.compute_dt(Uo, dx, 0.3))
+        oplan.advance(Uo, dx, dts_o[-1])
+    dts_o.append(oplan.compute_dt(Uo, dx, 0.3))
+    results = []
+    for zc in (1, 2, 3, 8):
+        gplan, _, _ = gpu_plan_for(cfg, recon=recon, rk=rk, neigh=neigh, zchain=zc)
+        assert gplan.path == 1
+        Ud, dxd = Uh.cuda(), torch.from_numpy(dx).cuda()
+        dt = gplan.fx_hydro_compute_dt(Ud, dxd, 0.3).clone()
+        dts = [float(dt.item())]
+        for step in range(2):
+            gplan.fx_hydro_step(Ud, dxd, 0.3, dt)
+            dts.append(float(dt.item()))
+        results.append((gplan.interior(Ud).cpu().numpy(), dts))
+    for got, dts in results[1:]:
+        assert np.array_equal(got, results[0][0]) and dts == results[0][1]
+    assert rel_err(cfg, results[0][0], oplan.interior(Uo)) <= 1e-11
+    assert all(abs(g - o) <= 1e-12 * o for g, o in zip(results[0][1], dts_o))
+
+
 @pytest.mark.parametrize("path", [None, 1])
 def test_status_flags_floors_and_nonfinite(path):
     """A7/A27: primitive floors and non-finite states raise the same status bits as in the oracle, the floored step
