@@ -35,7 +35,7 @@ namespace fxt {
 
 constexpr int NX = 16, NY = 16;
 constexpr int NZONE_THREADS = NX * NY;        // 256
-constexpr int NTHREADS = NZONE_THREADS + 32;  // + edge warp
+constexpr int NTHREADS = NZONE_THREADS + 64;  // + edge warp + producer warp
 constexpr int PLANE_BYTES = 5 * NY * NX * 8;  // one TMA box of the main kind
 
 template <int RECON> struct Rc {
@@ -69,6 +69,9 @@ template <int RECON> struct alignas(128) Smem {
 };
 
 __device__ __forceinline__ void cta_sync() { asm volatile("bar.sync 0, %0;" ::"n"(NTHREADS) : "memory"); }
+// edge warp -> producer warp: "the raw halo cells have been read" (named barrier 1, the two warps only)
+__device__ __forceinline__ void halo_arrive() { asm volatile("bar.arrive 1, 64;" ::: "memory"); }
+__device__ __forceinline__ void halo_sync() { asm volatile("bar.sync 1, 64;" ::: "memory"); }
 __device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
 
 __device__ __forceinline__ void mbar_init(unsigned long long *bar, int count) {
@@ -228,15 +231,15 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
     kp = k + g2;
   };
 
-  // ---------------------------------------------------------------- producer set-up (edge warp, lane 0)
-  const bool producer = tid == NZONE_THREADS;
+  // ---------------------------------------------------------------- producer set-up (producer warp, lane 0)
+  const bool producer = tid == NZONE_THREADS + 32;
   auto issue_X = [&](int c) {  // stage-input plane consumed at tick c: z index c + r
     int bs, kp;
     zmap(c + r, bs, kp);
     mbar_expect_tx(&S.barX[c & 1], PLANE_BYTES);
     tma_load(&S.ring[(c + r) % NRING][0][0][0], &mXm, &S.barX[c & 1], g0, g1, kp, bs);
   };
-  // edge warp: the block the next halo plane is in (plane hk of block hq of the segment) and its x / y neighbours
+  // edge and producer warps: the block the next halo plane is in (plane hk of block hq of the segment) and its x / y neighbours
   int hk = 0, hq = 0, hb = 0, xlo = 0, xhi = 0, ylo = 0, yhi = 0;
   auto halo_block = [&]() {
     hb = S.chain[2 + hq];
@@ -418,7 +421,7 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
       if ((tid & 31) == 0) S.wmax[tid >> 5] = rate;
     }
     cta_sync();  // D: the last plane is in Out
-  } else {
+  } else if (tid < NZONE_THREADS + 32) {
     // ------------------------------------------------------------ edge warp
     const int lane = tid - NZONE_THREADS;
     const bool isx = lane >= 16;
@@ -456,8 +459,8 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
 #pragma unroll
         for (int v = 0; v < 5; ++v) Pf[v * NP * NPS + pos * pd + (m + R) * pt] = w[v];
       }
-      __syncwarp();  // every lane has read its raw halo cells: the (single) slot can take the next plane's
       if (pl + 1 < nz) {
+        halo_arrive();  // this lane has read its raw halo cells: the (single) slot can take the next plane's
         if (++hk == nzb) {  // a new block: where its halo cells sit inside the boxes depends on which neighbours exist
           hk = 0;
           ++hq;
@@ -467,16 +470,14 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
 #pragma unroll
           for (int t = 0; t < 2 * R; ++t) hoff[t] = halo_off(t % R, t >= R);
         }
-        if (lane == 0) issue_H();
       }
     };
     halo_plane(0);
     cta_sync();  // A0
-    int pk = 0, pq = 0, pb = S.chain[2], pb_prev = pb;  // plane p is plane pk of block pb, the pq-th of the segment
+    int pk = 0, pq = 0, pb = S.chain[2];  // plane p is plane pk of block pb, the pq-th of the segment
 
 #pragma unroll 1
     for (int c = 1; c <= nz; ++c) {
-      const int p = c - 1;
       double qm16[5];
       {
         double st[W][5], qm[5], qp[5];
@@ -495,23 +496,7 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
           for (int v = 0; v < 5; ++v) st[mm][v] = Pf[v * NP * NPS + (NX + R - r + mm) * pd + (m + R) * pt];
         hit |= recon_cell5<RECON>(st, P.weno_eps, qm16, qp);
       }
-      // this tick's stage-input plane (requested two ticks ago) and U0 plane (one tick ago): the zone threads read them
-      // after barrier B without polling the mbarrier themselves
-      mbar_wait(&S.barX[c & 1], ((c - 1) >> 1) & 1);
       cta_sync();  // B
-      if (lane == 0) {
-        // every slot whose last reader finished before barrier B of this tick is free again: the ring slot of plane p - 1
-        // (combined in the phase that just ended) takes the plane of the next tick
-        if (c + 1 <= nz) issue_X(c + 1);
-        if (p >= 1) {
-          tma_store(&mOut, &S.Out[0][0][0], g0, g1, (pk >= 1 ? pk - 1 : nzb - 1) + g2, pk >= 1 ? pb : pb_prev);
-          tma_commit();
-        }
-        if (!FIRST && p + 1 < nz) {
-          if (pk + 1 < nzb) issue_U0(p + 1, pb, pk + 1);
-          else issue_U0(p + 1, S.chain[3 + pq], 0);
-        }
-      }
       {
         double WL[5];
 #pragma unroll
@@ -538,10 +523,54 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
       if (++pk == nzb) {
         pk = 0;
         ++pq;
+        pb = S.chain[2 + pq];
+      }
+      if (c < nz) halo_plane(c);  // halo of plane p + 1: nobody reads P between barriers B and C
+      cta_sync();  // C
+    }
+    cta_sync();  // D
+  } else {
+    // ------------------------------------------------------------ producer warp (lane 0 issues; the warp stays together)
+    const int lane = tid - NZONE_THREADS - 32;
+    auto next_halo = [&]() {  // the edge warp is done with the halo slot: request the next plane's halo
+      halo_sync();
+      if (++hk == nzb) {
+        hk = 0;
+        ++hq;
+        halo_block();
+      }
+      if (lane == 0) issue_H();
+    };
+    if (1 < nz) next_halo();
+    cta_sync();  // A0
+    int pk = 0, pq = 0, pb = S.chain[2], pb_prev = pb;  // plane p is plane pk of block pb, the pq-th of the segment
+#pragma unroll 1
+    for (int c = 1; c <= nz; ++c) {
+      const int p = c - 1;
+      // this tick's stage-input plane (requested two ticks ago) and U0 plane (one tick ago): the zone threads read them
+      // after barrier B without polling the mbarrier themselves
+      mbar_wait(&S.barX[c & 1], ((c - 1) >> 1) & 1);
+      cta_sync();  // B
+      if (lane == 0) {
+        // every slot whose last reader finished before barrier B of this tick is free again: the ring slot of plane p - 1
+        // (combined in the phase that just ended) takes the plane of the next tick
+        if (c + 1 <= nz) issue_X(c + 1);
+        if (p >= 1) {
+          tma_store(&mOut, &S.Out[0][0][0], g0, g1, (pk >= 1 ? pk - 1 : nzb - 1) + g2, pk >= 1 ? pb : pb_prev);
+          tma_commit();
+        }
+        if (!FIRST && p + 1 < nz) {
+          if (pk + 1 < nzb) issue_U0(p + 1, pb, pk + 1);
+          else issue_U0(p + 1, S.chain[3 + pq], 0);
+        }
+      }
+      if (++pk == nzb) {
+        pk = 0;
+        ++pq;
         pb_prev = pb;
         pb = S.chain[2 + pq];
       }
-      if (c < nz) halo_plane(c);                  // halo of plane p + 1: nobody reads P between barriers B and C
+      if (c + 1 < nz) next_halo();
       if (lane == 0 && p >= 1) tma_wait_read();  // Out is free for the combine after barrier C
       cta_sync();  // C
     }
