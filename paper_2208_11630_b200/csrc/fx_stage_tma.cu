@@ -69,9 +69,6 @@ template <int RECON> struct alignas(128) Smem {
 };
 
 __device__ __forceinline__ void cta_sync() { asm volatile("bar.sync 0, %0;" ::"n"(NTHREADS) : "memory"); }
-// edge warp -> producer warp: "the raw halo cells have been read" (named barrier 1, the two warps only)
-__device__ __forceinline__ void halo_arrive() { asm volatile("bar.arrive 1, 64;" ::: "memory"); }
-__device__ __forceinline__ void halo_sync() { asm volatile("bar.sync 1, 64;" ::: "memory"); }
 __device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
 
 __device__ __forceinline__ void mbar_init(unsigned long long *bar, int count) {
@@ -239,7 +236,7 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
     mbar_expect_tx(&S.barX[c & 1], PLANE_BYTES);
     tma_load(&S.ring[(c + r) % NRING][0][0][0], &mXm, &S.barX[c & 1], g0, g1, kp, bs);
   };
-  // edge and producer warps: the block the next halo plane is in (plane hk of block hq of the segment) and its x / y neighbours
+  // producer warp: the block the next halo plane is in (plane hk of block hq of the segment) and its x / y neighbours
   int hk = 0, hq = 0, hb = 0, xlo = 0, xhi = 0, ylo = 0, yhi = 0;
   auto halo_block = [&]() {
     hb = S.chain[2 + hq];
@@ -248,7 +245,7 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
     ylo = __ldg(&P.neigh[(long long)hb * 6 + 2]);
     yhi = __ldg(&P.neigh[(long long)hb * 6 + 3]);
   };
-  if (tid >= NZONE_THREADS) halo_block();
+  if (tid >= NZONE_THREADS + 32) halo_block();
   auto issue_H = [&]() {  // halo cells of interior plane hk of block hb, from the block's x and y neighbours
     const int b = hb, kp = hk + g2;
     mbar_expect_tx(&S.barH, 2 * 5 * NY * BW * 8 + 2 * 5 * R * NX * 8);
@@ -432,47 +429,6 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
     double *Lf = isx ? &S.Lx[0][0][0] : &S.Ly[0][0][0];
     const int ld = isx ? 1 : NX, lt = isx ? (NX + 1) : 1;  // strides of L along direction / transverse
     constexpr int LV = NY * (NX + 1);                       // per-variable size of the L arrays (272)
-    // raw halo cell t of this lane's row / column: Hx[s][side][v][m][ix], Hy[s][side][v][iy][m]
-    constexpr int HXV = NY * BW, HYV = R * NX;  // per-variable sizes
-    int nlo = isx ? xlo : ylo, nhi = isx ? xhi : yhi;  // this lane's pair of neighbours of the block the halo plane is in
-    auto halo_off = [&](int t, bool high) -> int {
-      int idx;  // cell index inside the box
-      if (isx) idx = high ? (nhi >= 0 ? t : BW - 1) : (nlo >= 0 ? BW - R + t : 0);
-      else idx = high ? (nhi >= 0 ? t : R - 1) : (nlo >= 0 ? t : 0);
-      return isx ? ((high ? 5 * HXV : 0) + m * BW + idx) : ((high ? 5 * HYV : 0) + idx * NX + m);
-    };
-    int hoff[2 * R];
-#pragma unroll
-    for (int t = 0; t < 2 * R; ++t) hoff[t] = halo_off(t % R, t >= R);
-    const int hv = isx ? HXV : HYV;
-
-    auto halo_plane = [&](int pl) {  // primitives of the halo cells of plane pl into P (called for pl = 0, 1, 2, ... in turn)
-      mbar_wait(&S.barH, pl & 1);
-      const double *Hf = isx ? &S.Hx[0][0][0][0] : &S.Hy[0][0][0][0];
-#pragma unroll
-      for (int t = 0; t < 2 * R; ++t) {
-        double u[5], w[5];
-#pragma unroll
-        for (int v = 0; v < 5; ++v) u[v] = Hf[hoff[t] + v * hv];
-        fx_c2p_v2(P, u[0], u[1], u[2], u[3], u[4], w);
-        const int pos = (t < R) ? t : (NX + t);  // padded position along the edge direction
-#pragma unroll
-        for (int v = 0; v < 5; ++v) Pf[v * NP * NPS + pos * pd + (m + R) * pt] = w[v];
-      }
-      if (pl + 1 < nz) {
-        halo_arrive();  // this lane has read its raw halo cells: the (single) slot can take the next plane's
-        if (++hk == nzb) {  // a new block: where its halo cells sit inside the boxes depends on which neighbours exist
-          hk = 0;
-          ++hq;
-          halo_block();
-          nlo = isx ? xlo : ylo;
-          nhi = isx ? xhi : yhi;
-#pragma unroll
-          for (int t = 0; t < 2 * R; ++t) hoff[t] = halo_off(t % R, t >= R);
-        }
-      }
-    };
-    halo_plane(0);
     cta_sync();  // A0
     int pk = 0, pq = 0, pb = S.chain[2];  // plane p is plane pk of block pb, the pq-th of the segment
 
@@ -525,23 +481,60 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
         ++pq;
         pb = S.chain[2 + pq];
       }
-      if (c < nz) halo_plane(c);  // halo of plane p + 1: nobody reads P between barriers B and C
       cta_sync();  // C
     }
     cta_sync();  // D
   } else {
-    // ------------------------------------------------------------ producer warp (lane 0 issues; the warp stays together)
+    // ------------------------------------------------------------ producer warp: lane 0 issues the bulk copies, all
+    // lanes convert the halo cells (lanes 0..15 the y edges of column m, lanes 16..31 the x edges of row m)
     const int lane = tid - NZONE_THREADS - 32;
-    auto next_halo = [&]() {  // the edge warp is done with the halo slot: request the next plane's halo
-      halo_sync();
-      if (++hk == nzb) {
-        hk = 0;
-        ++hq;
-        halo_block();
-      }
-      if (lane == 0) issue_H();
+    const bool isx = lane >= 16;
+    const int m = lane & 15;
+    double *Pf = &S.P[0][0][0];
+    constexpr int NPS = NP + 1;
+    const int pd = isx ? 1 : NPS, pt = isx ? NPS : 1;  // smem strides of P along direction / transverse
+    // raw halo cell t of this lane's row / column: Hx[s][side][v][m][ix], Hy[s][side][v][iy][m]
+    constexpr int HXV = NY * BW, HYV = R * NX;  // per-variable sizes
+    int nlo = isx ? xlo : ylo, nhi = isx ? xhi : yhi;  // this lane's pair of neighbours of the block the halo plane is in
+    auto halo_off = [&](int t, bool high) -> int {
+      int idx;  // cell index inside the box
+      if (isx) idx = high ? (nhi >= 0 ? t : BW - 1) : (nlo >= 0 ? BW - R + t : 0);
+      else idx = high ? (nhi >= 0 ? t : R - 1) : (nlo >= 0 ? t : 0);
+      return isx ? ((high ? 5 * HXV : 0) + m * BW + idx) : ((high ? 5 * HYV : 0) + idx * NX + m);
     };
-    if (1 < nz) next_halo();
+    int hoff[2 * R];
+#pragma unroll
+    for (int t = 0; t < 2 * R; ++t) hoff[t] = halo_off(t % R, t >= R);
+    const int hv = isx ? HXV : HYV;
+
+    auto halo_plane = [&](int pl) {  // primitives of the halo cells of plane pl into P (called for pl = 0, 1, 2, ... in turn)
+      mbar_wait(&S.barH, pl & 1);
+      const double *Hf = isx ? &S.Hx[0][0][0][0] : &S.Hy[0][0][0][0];
+#pragma unroll
+      for (int t = 0; t < 2 * R; ++t) {
+        double u[5], w[5];
+#pragma unroll
+        for (int v = 0; v < 5; ++v) u[v] = Hf[hoff[t] + v * hv];
+        fx_c2p_v2(P, u[0], u[1], u[2], u[3], u[4], w);
+        const int pos = (t < R) ? t : (NX + t);  // padded position along the edge direction
+#pragma unroll
+        for (int v = 0; v < 5; ++v) Pf[v * NP * NPS + pos * pd + (m + R) * pt] = w[v];
+      }
+      __syncwarp();  // every lane has read its raw halo cells: the (single) slot can take the next plane's
+      if (pl + 1 < nz) {
+        if (++hk == nzb) {  // a new block: where its halo cells sit inside the boxes depends on which neighbours exist
+          hk = 0;
+          ++hq;
+          halo_block();
+          nlo = isx ? xlo : ylo;
+          nhi = isx ? xhi : yhi;
+#pragma unroll
+          for (int t = 0; t < 2 * R; ++t) hoff[t] = halo_off(t % R, t >= R);
+        }
+        if (lane == 0) issue_H();
+      }
+    };
+    halo_plane(0);
     cta_sync();  // A0
     int pk = 0, pq = 0, pb = S.chain[2], pb_prev = pb;  // plane p is plane pk of block pb, the pq-th of the segment
 #pragma unroll 1
@@ -570,7 +563,7 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
         pb_prev = pb;
         pb = S.chain[2 + pq];
       }
-      if (c + 1 < nz) next_halo();
+      if (c < nz) halo_plane(c);  // halo of plane p + 1: nobody reads P between barriers B and C
       if (lane == 0 && p >= 1) tma_wait_read();  // Out is free for the combine after barrier C
       cta_sync();  // C
     }
