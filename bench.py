@@ -261,20 +261,20 @@ def run_ours(args, rank, world, local_rank):
     stage_avg_ms = stage_ms / max(stage_launches, 1)
     achieved = alg_bytes_per_launch / (stage_avg_ms * 1e-3) / 1e9
     # traffic: dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture of
-    # this command (profiles/r1_ncu_tma_raw.csv: mean of the stage-1 and stage-2 launches); null for other workloads
-    traffic = 21.03e9 if (cfg.number == 5 and args.nb is None and fused and stages == 2) else None
+    # this command (profiles/r1_ncu_chain_raw.csv: mean of the stage-1 and stage-2 launches); null for other workloads
+    traffic = 20.33e9 if (cfg.number == 5 and args.nb is None and fused and stages == 2) else None
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": traffic, "traffic_source": "ncu capture profiles/r1_ncu_tma_raw.csv (GB per launch, mean of both stages)"
+                "traffic": traffic, "traffic_source": "ncu capture profiles/r1_ncu_chain_raw.csv (GB per launch, mean of both stages)"
                 if traffic else None, "alg_bytes_per_launch": alg_bytes_per_launch, "peak_source": peak_src, "kernel": "fused stage kernel" if fused else "generic stage kernel",
                 "kernel_ms_avg": stage_avg_ms, "kernel_launches_timed": stage_launches,
                 "kernel_share_of_step": stage_ms / ms if ms > 0 else None,
                 "alg_bytes_per_zone_stage": sum(alg_bytes_stage) / stages}
     if fused and cfg.recon == 0 and cfg.riemann == 1:
-        # the other roof [NS]: the fp64 pipe.  437 fp64-pipe lane-instructions per zone-update (ncu)
+        # the other roof [NS]: the fp64 pipe.  438 fp64-pipe lane-instructions per zone-update (ncu: 419 in stage 1, 458 in stage 2 with the CFL rate)
         # against 148 SMs x 64 lanes x the SM clock (nominal; 17 T/s measured with fx_probe_fp64_fma)
         fp64_peak = 148 * FP64_FMA_LANES_PER_SM * 1.965e9
-        roofline["fp64_pipe"] = {"lane_instr_per_zone_update": 437, "peak_lane_instr_per_s": fp64_peak,
-                                 "frac": 437 * zones / (stage_avg_ms * 1e-3) / fp64_peak}
+        roofline["fp64_pipe"] = {"lane_instr_per_zone_update": 438, "peak_lane_instr_per_s": fp64_peak,
+                                 "frac": 438 * zones / (stage_avg_ms * 1e-3) / fp64_peak}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
