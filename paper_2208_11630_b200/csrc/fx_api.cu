@@ -86,7 +86,7 @@ extern "C" int fx_hydro_plan_create(fx_hydro_plan **out, const int block_dims[3]
   P.recon = recon;
   P.riemann = riemann;
   P.wavespeed = 0;
-  p->zchain = FX_SEG_MAX;
+  p->zchain = 0;  // auto
   p->nguard = nguard;
   p->nvars = nvars;
   p->rk = rk_order;
@@ -132,7 +132,7 @@ extern "C" int fx_hydro_plan_set_option(fx_hydro_plan *plan, int key, double val
     plan->P.wavespeed = (int)value;
     return FX_OK;
   case FX_OPT_ZCHAIN:
-    if (!(value >= 1.0 && value <= (double)FX_SEG_MAX)) return fx_fail(FX_ERR_INVALID_ARG, "set_option: zchain must be 1..%d", (int)FX_SEG_MAX);
+    if (!(value >= 0.0 && value <= (double)FX_SEG_MAX)) return fx_fail(FX_ERR_INVALID_ARG, "set_option: zchain must be 0 (auto) or 1..%d", (int)FX_SEG_MAX);
     plan->zchain = (int)value;
     return FX_OK;
   case FX_OPT_PATH:
@@ -238,7 +238,24 @@ extern "C" int fx_hydro_plan_set_topology(fx_hydro_plan *plan, const int32_t *ne
     plan->seg_host = new (std::nothrow) int[(size_t)nb * FX_SEG_STRIDE];
     if (!plan->seg_host) return fx_fail(FX_ERR_INVALID_ARG, "set_topology: out of host memory");
     // (blocks taller than 64 planes are not chained: the kernel's plane -> block map is exact up to 2^20 / nz planes)
-    const int M = (plan->zchain < 1 || plan->P.n[2] > 64) ? 1 : (plan->zchain > FX_SEG_MAX ? FX_SEG_MAX : plan->zchain);
+    int M = plan->zchain > FX_SEG_MAX ? FX_SEG_MAX : plan->zchain;
+    if (M <= 0) {
+      // auto: a segment of M blocks costs about M + 0.09 block times (measured: the start-up of a CTA and the z halo of
+      // a segment are 9 % of a block), and the launch takes ceil(segments / resident CTAs) rounds of them
+      int dev = 0, sms = 148;
+      if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+      const long long slots = (long long)sms * (plan->P.recon == FX_RECON_WENO5 ? 1 : 2);
+      double best = 0.0;
+      for (int m = 1; m <= FX_SEG_MAX; m *= 2) {
+        const long long nseg = (nb + m - 1) / m;
+        const double cost = (double)((nseg + slots - 1) / slots) * (m + 0.09);
+        if (M <= 0 || cost < best) {
+          best = cost;
+          M = m;
+        }
+      }
+    }
+    if (plan->P.n[2] > 64) M = 1;
     for (long long b0 = 0; b0 < nb; ++b0) {
       if (seen[b0]) continue;
       long long start = b0;
