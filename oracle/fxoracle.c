@@ -41,6 +41,7 @@
 #define FXO_RIEMANN_HLLC 1
 #define FXO_BC_OUTFLOW (-1)
 #define FXO_BC_NONE (-2)
+#define FXO_BC_REFLECT (-3) /* reflecting wall [B9]: mirror image of the interior, normal momentum negated */
 #define FXO_OPT_RHO_FLOOR 0
 #define FXO_OPT_P_FLOOR 1
 #define FXO_OPT_WENO_EPS 2
@@ -165,7 +166,7 @@ int fxo_plan_set_topology(fxo_plan *p, const int32_t *neigh) {
       if (!p->active[d]) continue; /* entries of inactive dims are ignored [A26] */
       if (v >= 0) {
         if (v >= p->nblocks) return FXO_ERR_INVALID_ARG;
-      } else if (v != FXO_BC_OUTFLOW) {
+      } else if (v != FXO_BC_OUTFLOW && v != FXO_BC_REFLECT) {
         return FXO_ERR_UNSUPPORTED; /* coarse/fine neighbours have no code [A18] */
       }
     }
@@ -216,7 +217,7 @@ static int cmp_sortrec(const void *a, const void *b) {
   return (x->key > y->key) - (x->key < y->key);
 }
 
-/* bc codes: 0 periodic, 1 outflow, 2 none (inactive dimension).  order: 0 lexicographic
+/* bc codes: 0 periodic, 1 outflow, 2 none (inactive dimension), 3 reflecting.  order: 0 lexicographic
  * (x fastest), 1 Morton.  neigh_out [nb][6], coords_out [nb][3] (block coordinates). */
 int fxo_topology_cartesian(const int nb[3], const int bc_lo[3], const int bc_hi[3], int order,
                            int32_t *neigh_out, int32_t *coords_out) {
@@ -256,7 +257,7 @@ int fxo_topology_cartesian(const int nb[3], const int bc_lo[3], const int bc_hi[
               cc[d] = (cc[d] + nb[d]) % nb[d];
               v = id_of_lex[((int64_t)cc[2] * nb[1] + cc[1]) * nb[0] + cc[0]];
             } else {
-              v = FXO_BC_OUTFLOW;
+              v = bc == 3 ? FXO_BC_REFLECT : FXO_BC_OUTFLOW;
             }
           } else {
             v = id_of_lex[((int64_t)cc[2] * nb[1] + cc[1]) * nb[0] + cc[0]];
@@ -273,8 +274,11 @@ int fxo_topology_cartesian(const int nb[3], const int bc_lo[3], const int bc_hi[
 /* --------------------------------------------------------- O1 guard fill */
 
 /* Source of padded zone (i,j,k) of block b: hops in the order z, y, x [O1, A14].
- * Returns the flat variable-0 element index of the interior zone it images. */
-static int64_t guard_source(const fxo_plan *p, int64_t b, int i, int j, int k) {
+ * Returns the flat variable-0 element index of the interior zone it images.  At a reflecting wall [B9] guard
+ * zone -1-m images interior zone m (16+m images 15-m) and bit d of *flip is set: the momentum component
+ * normal to that wall changes sign in the image. */
+static int64_t guard_source(const fxo_plan *p, int64_t b, int i, int j, int k, unsigned *flip) {
+  *flip = 0;
   int c[3] = {i, j, k};
   int64_t bs = b;
   for (int d = 2; d >= 0; --d) {
@@ -285,6 +289,9 @@ static int64_t guard_source(const fxo_plan *p, int64_t b, int i, int j, int k) {
       if (nb >= 0) {
         bs = nb;
         c[d] += p->n[d];
+      } else if (nb == FXO_BC_REFLECT) {
+        c[d] = 2 * lo - 1 - c[d];
+        *flip |= 1u << d;
       } else {
         c[d] = lo; /* outflow: zero-gradient clamp */
       }
@@ -293,6 +300,9 @@ static int64_t guard_source(const fxo_plan *p, int64_t b, int i, int j, int k) {
       if (nb >= 0) {
         bs = nb;
         c[d] -= p->n[d];
+      } else if (nb == FXO_BC_REFLECT) {
+        c[d] = 2 * hi - 1 - c[d];
+        *flip |= 1u << d;
       } else {
         c[d] = hi - 1;
       }
@@ -309,7 +319,10 @@ int fxo_guardcell_index_map(fxo_plan *p, int64_t block_begin, int64_t block_coun
     for (int k = 0; k < p->np[2]; ++k)
       for (int j = 0; j < p->np[1]; ++j)
         for (int i = 0; i < p->np[0]; ++i)
-          src[bb * p->S_b + k * p->S_k + j * p->S_j + i] = guard_source(p, block_begin + bb, i, j, k);
+        {
+          unsigned flip;
+          src[bb * p->S_b + k * p->S_k + j * p->S_j + i] = guard_source(p, block_begin + bb, i, j, k, &flip);
+        }
   return FXO_OK;
 }
 
@@ -325,9 +338,13 @@ int fxo_fill_guardcells(fxo_plan *p, double *U) {
           int interior = i >= p->gd[0] && i < p->gd[0] + p->n[0] && j >= p->gd[1] &&
                          j < p->gd[1] + p->n[1] && k >= p->gd[2] && k < p->gd[2] + p->n[2];
           if (interior) continue;
-          int64_t s = guard_source(p, b, i, j, k);
+          unsigned flip;
+          int64_t s = guard_source(p, b, i, j, k, &flip);
           int64_t t = b * p->S_b + k * p->S_k + j * p->S_j + i;
-          for (int v = 0; v < p->nvars; ++v) U[v * p->S_v + t] = U[v * p->S_v + s];
+          for (int v = 0; v < p->nvars; ++v) {
+            double x = U[v * p->S_v + s];
+            U[v * p->S_v + t] = (v >= 1 && v <= 3 && ((flip >> (v - 1)) & 1u)) ? -x : x;
+          }
         }
   return FXO_OK;
 }

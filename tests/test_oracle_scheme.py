@@ -166,6 +166,49 @@ def test_sedov_reflection_symmetry():
         assert np.max(np.abs(R - G) / scale) <= 1e-12
 
 
+def test_reflecting_wall_equals_half_of_a_symmetric_domain():
+    """[B9] A block with a reflecting wall at +x evolves exactly like the left half of a domain twice as wide whose
+    right half is the mirror image (rho, E, m_y, m_z even, m_x odd about the wall): the wall's guard cells hold what the
+    mirrored neighbour block would hold.  The filled guard zones agree bit for bit; from the second RK stage on the two
+    runs differ by how exactly the scheme's arithmetic commutes with the reflection (a few ulp per step for general
+    2-D data), so the states are compared to 2e-15 after one step and 1e-13 after ten."""
+    for recon, riemann, rk in ((0, 1, 2), (1, 0, 3)):
+        dims, g = (16, 8, 1), 4
+        o, r, per, none = fxo.TOPO_OUTFLOW, fxo.TOPO_REFLECT, fxo.TOPO_PERIODIC, fxo.TOPO_NONE
+        nh, _ = fxo.topology_cartesian((1, 1, 1), [o, per, none], [r, per, none], fxo.ORDER_LEX)
+        nf, cf = fxo.topology_cartesian((2, 1, 1), [o, per, none], [o, per, none], fxo.ORDER_LEX)
+        half = fxo.OraclePlan(dims, g, 1, 1.4, recon, riemann, rk)
+        half.set_topology(nh)
+        full = fxo.OraclePlan(dims, g, 2, 1.4, recon, riemann, rk)
+        full.set_topology(nf)
+        rng = np.random.default_rng(17)
+        rho = 1.0 + 0.4 * rng.random((1, 8, 16))
+        vel = 0.5 * rng.standard_normal((3, 1, 8, 16))
+        pr = 1.0 + 0.4 * rng.random((1, 8, 16))
+        L = np.stack([rho, rho * vel[0], rho * vel[1], rho * vel[2], pr / 0.4 + 0.5 * rho * (vel ** 2).sum(0)])
+        Rm = L[..., ::-1].copy()
+        Rm[1] = -Rm[1]
+        Uh = np.full(half.shape, np.nan)
+        half.interior(Uh)[:, 0] = L
+        Uf = np.full(full.shape, np.nan)
+        assert tuple(cf[0]) == (0, 0, 0) and tuple(cf[1]) == (1, 0, 0)
+        full.interior(Uf)[:, 0] = L
+        full.interior(Uf)[:, 1] = Rm
+        A, B = Uh.copy(), Uf.copy()
+        half.fill_guardcells(A)
+        full.fill_guardcells(B)
+        assert np.array_equal(A[:, 0], B[:, 0])  # the wall's guard zones ARE the mirrored neighbour's zones
+        dxh, dxf = np.full((1, 3), 1.0 / 32), np.full((2, 3), 1.0 / 32)
+        for step in range(10):
+            dt = full.compute_dt(Uf, dxf, 0.3)
+            assert abs(dt - half.compute_dt(Uh, dxh, 0.3)) <= 1e-14 * dt
+            half.advance(Uh, dxh, dt)
+            full.advance(Uf, dxf, dt)
+            a, b = half.interior(Uh)[:, 0], full.interior(Uf)[:, 0]
+            assert np.max(np.abs(a - b)) <= (2e-15 if step == 0 else 1e-13) * np.abs(b).max(), (recon, step)
+        assert np.abs(half.interior(Uh)[1, 0, 0, :, -1]).max() > 1e-3  # something moves next to the wall
+
+
 # ------------------------------------------------------------ RK composition, dt
 def test_rk_is_the_shu_osher_composition_of_euler_steps():
     cfg = inputs.config(5, nb=(2, 2, 2))
