@@ -40,8 +40,8 @@ extern "C" {
 
 enum { FX_RECON_PLM_MINMOD = 0, FX_RECON_WENO5 = 1 };
 enum { FX_RIEMANN_HLLE = 0, FX_RIEMANN_HLLC = 1 };
-enum { FX_BC_OUTFLOW = -1, FX_BC_NONE = -2 };                        /* neighbour-table codes */
-enum { FX_TOPO_PERIODIC = 0, FX_TOPO_OUTFLOW = 1, FX_TOPO_NONE = 2 }; /* fx_topology_cartesian bc codes */
+enum { FX_BC_OUTFLOW = -1, FX_BC_NONE = -2, FX_BC_REFLECT = -3 };    /* neighbour-table codes */
+enum { FX_TOPO_PERIODIC = 0, FX_TOPO_OUTFLOW = 1, FX_TOPO_NONE = 2, FX_TOPO_REFLECT = 3 }; /* fx_topology_cartesian bc codes */
 enum { FX_ORDER_LEX = 0, FX_ORDER_MORTON = 1 };
 enum {
   FX_OPT_RHO_FLOOR = 0, /* primitive density floor, default 1e-12 [A7] */
@@ -96,7 +96,8 @@ int fx_hydro_plan_set_workspace(fx_hydro_plan *plan, void *workspace_dev, size_t
 
 /* Topology: neigh_dev is int32 [nblocks][6] in the order -x,+x,-y,+y,-z,+z; an entry >= 0 is the id of
  * the same-level neighbour block (periodic boundaries are expressed by wrapped ids), FX_BC_OUTFLOW a
- * zero-gradient physical boundary; entries of inactive dimensions are ignored.  The table stays
+ * zero-gradient physical boundary, FX_BC_REFLECT a reflecting wall (guard zone -1-m images interior zone m
+ * with the momentum normal to the wall negated; reading B9); entries of inactive dimensions are ignored.  The table stays
  * caller-owned and must outlive the plan's use of it.  The call copies it to the host once to validate
  * (synchronises).  Any other negative entry in an active dimension is a coarse/fine relation:
  * FX_ERR_UNSUPPORTED [A18]. */
@@ -110,7 +111,8 @@ int fx_topology_cartesian(const int nb[3], const int bc_lo[3], const int bc_hi[3
 
 /* a1 Guard-cell fill [O1, A14]: every guard zone (faces, edges, corners) of every block of U_dev, in
  * place, gets the 5 variables of the interior zone it images: hops z, then y, then x through the
- * neighbour table; outflow clamps to the nearest interior index.  Needs the topology (FX_ERR_STATE). */
+ * neighbour table; outflow clamps to the nearest interior index, a reflecting wall mirrors the index and
+ * negates the normal momentum.  Needs the topology (FX_ERR_STATE). */
 int fx_fill_guardcells(fx_hydro_plan *plan, double *U_dev, void *stream);
 
 /* Test hook: for blocks [block_begin, block_begin+block_count), the flat variable-0 element index each

@@ -17,8 +17,8 @@ LIB_PATH = os.environ.get("FXHYDRO_LIB") or os.path.join(_HERE, "libfxhydro.so")
 OK, ERR_INVALID_ARG, ERR_STATE, ERR_UNSUPPORTED, ERR_WORKSPACE, ERR_CUDA = 0, -1, -2, -3, -4, -5
 RECON_PLM_MINMOD, RECON_WENO5 = 0, 1
 RIEMANN_HLLE, RIEMANN_HLLC = 0, 1
-BC_OUTFLOW, BC_NONE = -1, -2
-TOPO_PERIODIC, TOPO_OUTFLOW, TOPO_NONE = 0, 1, 2
+BC_OUTFLOW, BC_NONE, BC_REFLECT = -1, -2, -3
+TOPO_PERIODIC, TOPO_OUTFLOW, TOPO_NONE, TOPO_REFLECT = 0, 1, 2, 3
 ORDER_LEX, ORDER_MORTON = 0, 1
 OPT_RHO_FLOOR, OPT_P_FLOOR, OPT_WENO_EPS, OPT_WAVESPEED, OPT_PATH, OPT_ZCHAIN = 0, 1, 2, 3, 4, 5
 STATUS_NONFINITE, STATUS_RHO_FLOOR, STATUS_P_FLOOR, STATUS_WENO_FALLBACK = 1, 2, 4, 8

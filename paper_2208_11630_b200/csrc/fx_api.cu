@@ -207,13 +207,14 @@ extern "C" int fx_hydro_plan_set_topology(fx_hydro_plan *plan, const int32_t *ne
         const int32_t v = h[b * 6 + f];
         if (v >= 0) {
           if (v >= nb) return fx_fail(FX_ERR_INVALID_ARG, "set_topology: block %lld face %d -> id %d out of range", b, f, v);
-        } else if (v != FX_BC_OUTFLOW) {
+        } else if (v != FX_BC_OUTFLOW && v != FX_BC_REFLECT) {
           return fx_fail(FX_ERR_UNSUPPORTED, "set_topology: block %lld face %d has code %d: coarse/fine neighbours are not supported", b, f, v);
         }
       }
   }
   plan->P.neigh = neigh_dev;
   plan->topology_set = true;
+  plan->P.walls = 0;
   // z-chain segments: walk down (-z) from every unvisited block to the start of its chain (or once around a periodic
   // ring), then up (+z), cutting every `zchain` blocks and wherever the two blocks do not name each other
   delete[] plan->seg_host;
@@ -234,6 +235,9 @@ extern "C" int fx_hydro_plan_set_topology(fx_hydro_plan *plan, const int32_t *ne
       const long long a = h[b * 6 + 4];
       return (a >= 0 && a != b && h[a * 6 + 5] == b) ? a : -1;
     };
+    for (long long b = 0; b < nb; ++b)
+      for (int f = 0; f < 6; ++f)
+        if (plan->P.active[f / 2] && h[b * 6 + f] == FX_BC_REFLECT) plan->P.walls = 1;
     std::vector<char> seen((size_t)nb, 0);
     plan->seg_host = new (std::nothrow) int[(size_t)nb * FX_SEG_STRIDE];
     if (!plan->seg_host) return fx_fail(FX_ERR_INVALID_ARG, "set_topology: out of host memory");
@@ -305,7 +309,7 @@ extern "C" int fx_topology_cartesian(const int nb[3], const int bc_lo[3], const 
   if (order != FX_ORDER_LEX && order != FX_ORDER_MORTON) return fx_fail(FX_ERR_INVALID_ARG, "topology_cartesian: unknown order");
   for (int d = 0; d < 3; ++d) {
     if (nb[d] < 1) return fx_fail(FX_ERR_INVALID_ARG, "topology_cartesian: nb[%d] < 1", d);
-    if (bc_lo[d] < 0 || bc_lo[d] > 2 || bc_hi[d] < 0 || bc_hi[d] > 2) return fx_fail(FX_ERR_INVALID_ARG, "topology_cartesian: bad bc code");
+    if (bc_lo[d] < 0 || bc_lo[d] > 3 || bc_hi[d] < 0 || bc_hi[d] > 3) return fx_fail(FX_ERR_INVALID_ARG, "topology_cartesian: bad bc code");
   }
   const long long N = (long long)nb[0] * nb[1] * nb[2];
   if (N > 2147483647LL) return fx_fail(FX_ERR_INVALID_ARG, "topology_cartesian: too many blocks");
@@ -333,8 +337,8 @@ extern "C" int fx_topology_cartesian(const int nb[3], const int bc_lo[3], const 
           int cc[3] = {c[0], c[1], c[2]};
           cc[d] += s ? 1 : -1;
           const bool outside = cc[d] < 0 || cc[d] >= nb[d];
-          if (outside && bc == FX_TOPO_OUTFLOW) {
-            v = FX_BC_OUTFLOW;
+          if (outside && (bc == FX_TOPO_OUTFLOW || bc == FX_TOPO_REFLECT)) {
+            v = bc == FX_TOPO_REFLECT ? FX_BC_REFLECT : FX_BC_OUTFLOW;
           } else {
             cc[d] = (cc[d] + nb[d]) % nb[d];
             v = id_of_lex[((long long)cc[2] * nb[1] + cc[1]) * nb[0] + cc[0]];

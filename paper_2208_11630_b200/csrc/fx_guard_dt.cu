@@ -2,8 +2,10 @@
 #include "fx_physics.cuh"
 
 // ------------------------------------------------------------------ a1 guard fill
-// Source of padded zone (i,j,k) of block b: hops z, y, x through the neighbour table [O1, A14].
-__device__ __forceinline__ long long fx_guard_source(const FxParams &P, long long b, int i, int j, int k) {
+// Source of padded zone (i,j,k) of block b: hops z, y, x through the neighbour table [O1, A14].  Bit d of flip is set
+// when the zone lies behind a reflecting wall of dimension d [B9]: its image carries the negated d-momentum.
+__device__ __forceinline__ long long fx_guard_source(const FxParams &P, long long b, int i, int j, int k, unsigned &flip) {
+  flip = 0;
   int c[3] = {i, j, k};
   long long bs = b;
 #pragma unroll
@@ -12,10 +14,14 @@ __device__ __forceinline__ long long fx_guard_source(const FxParams &P, long lon
     const int lo = P.gd[d], hi = P.gd[d] + P.n[d];
     if (c[d] < lo) {
       int nb = __ldg(&P.neigh[bs * 6 + 2 * d]);
-      if (nb >= 0) { bs = nb; c[d] += P.n[d]; } else c[d] = lo;
+      if (nb >= 0) { bs = nb; c[d] += P.n[d]; }
+      else if (nb == FX_BC_REFLECT) { c[d] = 2 * lo - 1 - c[d]; flip |= 1u << d; }
+      else c[d] = lo;
     } else if (c[d] >= hi) {
       int nb = __ldg(&P.neigh[bs * 6 + 2 * d + 1]);
-      if (nb >= 0) { bs = nb; c[d] -= P.n[d]; } else c[d] = hi - 1;
+      if (nb >= 0) { bs = nb; c[d] -= P.n[d]; }
+      else if (nb == FX_BC_REFLECT) { c[d] = 2 * hi - 1 - c[d]; flip |= 1u << d; }
+      else c[d] = hi - 1;
     }
   }
   return bs * P.S_b + c[2] * P.S_k + c[1] * P.S_j + c[0];
@@ -31,10 +37,14 @@ __global__ void __launch_bounds__(256) fx_k_fill_guardcells(FxParams P, double *
   const bool interior = i >= P.gd[0] && i < P.gd[0] + P.n[0] && j >= P.gd[1] && j < P.gd[1] + P.n[1] &&
                         k >= P.gd[2] && k < P.gd[2] + P.n[2];
   if (interior) return;
-  const long long s = fx_guard_source(P, b, i, j, k);
+  unsigned flip;
+  const long long s = fx_guard_source(P, b, i, j, k, flip);
   const long long t = b * P.S_b + z;
 #pragma unroll
-  for (int v = 0; v < 5; ++v) U[v * P.S_v + t] = U[v * P.S_v + s];
+  for (int v = 0; v < 5; ++v) {
+    const double x = U[v * P.S_v + s];
+    U[v * P.S_v + t] = (v >= 1 && v <= 3 && ((flip >> (v - 1)) & 1u)) ? -x : x;
+  }
 }
 
 __global__ void __launch_bounds__(256) fx_k_index_map(FxParams P, long long b0, long long nb, long long *__restrict__ src) {
@@ -43,7 +53,8 @@ __global__ void __launch_bounds__(256) fx_k_index_map(FxParams P, long long b0, 
   const int z = blockIdx.x * blockDim.x + threadIdx.x;
   if (z >= P.S_b) return;
   const int i = z % P.np[0], j = (z / P.np[0]) % P.np[1], k = z / (P.np[0] * P.np[1]);
-  src[bb * P.S_b + z] = fx_guard_source(P, b0 + bb, i, j, k);
+  unsigned flip;
+  src[bb * P.S_b + z] = fx_guard_source(P, b0 + bb, i, j, k, flip);
 }
 
 static void fx_block_grid(long long nblocks, long long per_block_threads, dim3 &grid) {

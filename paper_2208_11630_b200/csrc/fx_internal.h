@@ -19,6 +19,7 @@ struct FxParams {
   const int *neigh;                 // [nblocks][6], device
   const int *seg;                   // z-chain segments of the fused kernel: [nseg][FX_SEG_STRIDE], device (in the workspace)
   int nseg;
+  int walls;                        // some block has a reflecting wall in an active dimension [B9]
   unsigned long long *scratch;      // device scratch block, see FX_SCR_*
 };
 

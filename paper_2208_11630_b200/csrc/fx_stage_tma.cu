@@ -191,7 +191,8 @@ __device__ __forceinline__ void flux_dir(const FxParams &P, const double WL[5], 
   F[4] = f[4];
 }
 
-template <int RECON, int RIEMANN, int WS, bool FIRST, bool DTOUT>
+// WALLS: some block of the launch has a reflecting wall [B9] (the image cells' sign flips are compiled in only then)
+template <int RECON, int RIEMANN, int WS, bool FIRST, bool DTOUT, bool WALLS>
 __global__ void __launch_bounds__(NTHREADS) __maxnreg__(Rc<RECON>::NREG)
 fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ CUtensorMap mXx,
                const __grid_constant__ CUtensorMap mXy, const __grid_constant__ CUtensorMap mU0,
@@ -214,7 +215,8 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
   const int M = S.chain[0];
   const int nz = M * nzb;
   // where plane Z of the column (Z in [-R, nz + R)) lives: block id and padded k.  Outflow below / above the segment
-  // clamps to the nearest interior plane [O1].
+  // clamps to the nearest interior plane [O1]; a reflecting wall [B9] mirrors the plane index (plane -1-m is plane m, its
+  // z momentum negated by whoever converts it: the prologue below the segment, the z loop above it).
   // Z / nzb without a division: exact for Z < 2^20 / nzb, and the host only chains blocks of at most 64 planes
   const unsigned zmagic = ((1u << 20) + (unsigned)nzb - 1u) / (unsigned)nzb;
   auto zmap = [&](int Z, int &bs, int &kp) {
@@ -222,11 +224,14 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
     int k = Z - qb * nzb;
     int id = S.chain[2 + qb];
     if (id < 0) {
-      if (qb < 0) { id = S.chain[2]; k = 0; } else { id = S.chain[1 + M]; k = nzb - 1; }
+      const bool wall = WALLS && id == FX_BC_REFLECT;
+      if (qb < 0) { id = S.chain[2]; k = wall ? -1 - Z : 0; } else { id = S.chain[1 + M]; k = wall ? nzb - 1 - (Z - nz) : nzb - 1; }
     }
     bs = id;
     kp = k + g2;
   };
+  const bool wall_below = WALLS && S.chain[1] == FX_BC_REFLECT;
+  const int zflip_from = (WALLS && S.chain[2 + M] == FX_BC_REFLECT) ? nz : 0x7fffffff;  // planes >= this carry a negated z momentum
 
   // ---------------------------------------------------------------- producer set-up (producer warp, lane 0)
   const bool producer = tid == NZONE_THREADS + 32;
@@ -290,6 +295,7 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
         const long long a = (long long)bs * P.S_b + (long long)kp * P.S_k + col;
 #pragma unroll
         for (int v = 0; v < 5; ++v) w[m][v] = X[a + v * P.S_v];
+        if (m < R && wall_below) w[m][3] = -w[m][3];
       }
 #pragma unroll
       for (int m = 0; m < 2 * R; ++m) {
@@ -347,6 +353,7 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
         double u[5];
 #pragma unroll
         for (int v = 0; v < 5; ++v) u[v] = S.ring[(c + r) % NRING][v][j][i];
+        if (WALLS && c + r >= zflip_from) u[3] = -u[3];  // image planes above a reflecting wall
         const unsigned h = fx_c2p_v2(P, u[0], u[1], u[2], u[3], u[4], q[2 * r]);
         if (c + r < nz) hit |= h;
       }
@@ -498,8 +505,9 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
     int nlo = isx ? xlo : ylo, nhi = isx ? xhi : yhi;  // this lane's pair of neighbours of the block the halo plane is in
     auto halo_off = [&](int t, bool high) -> int {
       int idx;  // cell index inside the box
-      if (isx) idx = high ? (nhi >= 0 ? t : BW - 1) : (nlo >= 0 ? BW - R + t : 0);
-      else idx = high ? (nhi >= 0 ? t : R - 1) : (nlo >= 0 ? t : 0);
+      // a neighbour's cells; at a reflecting wall this block's own cells in mirrored order [B9]; at outflow its edge cell
+      if (isx) idx = high ? (nhi >= 0 ? t : ((WALLS && nhi == FX_BC_REFLECT) ? BW - 1 - t : BW - 1)) : (nlo >= 0 ? BW - R + t : ((WALLS && nlo == FX_BC_REFLECT) ? R - 1 - t : 0));
+      else idx = high ? (nhi >= 0 ? t : ((WALLS && nhi == FX_BC_REFLECT) ? R - 1 - t : R - 1)) : (nlo >= 0 ? t : ((WALLS && nlo == FX_BC_REFLECT) ? R - 1 - t : 0));
       return isx ? ((high ? 5 * HXV : 0) + m * BW + idx) : ((high ? 5 * HYV : 0) + idx * NX + m);
     };
     int hoff[2 * R];
@@ -515,6 +523,9 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
         double u[5], w[5];
 #pragma unroll
         for (int v = 0; v < 5; ++v) u[v] = Hf[hoff[t] + v * hv];
+        if (WALLS && (t < R ? nlo : nhi) == FX_BC_REFLECT) {  // image cells behind a wall: normal momentum negated
+          if (isx) u[1] = -u[1]; else u[2] = -u[2];
+        }
         fx_c2p_v2(P, u[0], u[1], u[2], u[3], u[4], w);
         const int pos = (t < R) ? t : (NX + t);  // padded position along the edge direction
 #pragma unroll
@@ -626,7 +637,7 @@ static int make_map(CUtensorMap *m, const FxParams &P, const double *base, int b
   return FX_OK;
 }
 
-template <int RECON, int RIEMANN, int WS, bool FIRST, bool DTOUT>
+template <int RECON, int RIEMANN, int WS, bool FIRST, bool DTOUT, bool WALLS>
 int launch(const FxParams &P, const double *X, const double *U0, double *out, const double *dx, double dt, const double *dt_dev,
            double beta, double cfl_next, double *dt_next, cudaStream_t st) {
   constexpr int R = Rc<RECON>::R, BW = Rc<RECON>::BW;
@@ -637,7 +648,7 @@ int launch(const FxParams &P, const double *X, const double *U0, double *out, co
   if ((rc = make_map(&mXy, P, X, NX, R))) return rc;
   if ((rc = make_map(&mU0, P, U0, NX, NY))) return rc;
   if ((rc = make_map(&mOut, P, out, NX, NY))) return rc;
-  auto kern = fx_k_stage_tma<RECON, RIEMANN, WS, FIRST, DTOUT>;
+  auto kern = fx_k_stage_tma<RECON, RIEMANN, WS, FIRST, DTOUT, WALLS>;
   const int smem = (int)sizeof(Smem<RECON>);
   static bool configured = false;  // per instantiation
   if (!configured) {
@@ -661,9 +672,14 @@ int launch(const FxParams &P, const double *X, const double *U0, double *out, co
 template <int RECON, int RIEMANN, int WS>
 int launch_ws(const FxParams &P, const double *X, const double *U0, double *out, const double *dx, double dt, const double *dt_dev,
               double beta, int first, double cfl_next, double *dt_next, cudaStream_t st) {
-  if (first) return launch<RECON, RIEMANN, WS, true, false>(P, X, U0, out, dx, dt, dt_dev, beta, 0.0, nullptr, st);
-  if (dt_next) return launch<RECON, RIEMANN, WS, false, true>(P, X, U0, out, dx, dt, dt_dev, beta, cfl_next, dt_next, st);
-  return launch<RECON, RIEMANN, WS, false, false>(P, X, U0, out, dx, dt, dt_dev, beta, 0.0, nullptr, st);
+  if (P.walls) {
+    if (first) return launch<RECON, RIEMANN, WS, true, false, true>(P, X, U0, out, dx, dt, dt_dev, beta, 0.0, nullptr, st);
+    if (dt_next) return launch<RECON, RIEMANN, WS, false, true, true>(P, X, U0, out, dx, dt, dt_dev, beta, cfl_next, dt_next, st);
+    return launch<RECON, RIEMANN, WS, false, false, true>(P, X, U0, out, dx, dt, dt_dev, beta, 0.0, nullptr, st);
+  }
+  if (first) return launch<RECON, RIEMANN, WS, true, false, false>(P, X, U0, out, dx, dt, dt_dev, beta, 0.0, nullptr, st);
+  if (dt_next) return launch<RECON, RIEMANN, WS, false, true, false>(P, X, U0, out, dx, dt, dt_dev, beta, cfl_next, dt_next, st);
+  return launch<RECON, RIEMANN, WS, false, false, false>(P, X, U0, out, dx, dt, dt_dev, beta, 0.0, nullptr, st);
 }
 
 template <int RECON, int RIEMANN>

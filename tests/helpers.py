@@ -24,7 +24,7 @@ def oracle_plan_for(cfg, nblocks=None, order=inputs.ORDER_LEX, bc=None, nb=None,
     """Oracle plan + topology for a config (regular tiling nb, default cfg.nb)."""
     nb = tuple(nb or cfg.nb)
     bc = bc or cfg.bc
-    code = {"periodic": fxo.TOPO_PERIODIC, "outflow": fxo.TOPO_OUTFLOW}[bc]
+    code = {"periodic": fxo.TOPO_PERIODIC, "outflow": fxo.TOPO_OUTFLOW, "reflect": fxo.TOPO_REFLECT}[bc]
     bcs = [code if cfg.block_dims[d] > 1 else fxo.TOPO_NONE for d in range(3)]
     neigh, coords = fxo.topology_cartesian(nb, bcs, bcs, order)
     plan = fxo.OraclePlan(cfg.block_dims, cfg.nguard, neigh.shape[0], cfg.gamma,
@@ -150,7 +150,7 @@ def gpu_plan_for(cfg, order=inputs.ORDER_LEX, bc=None, nb=None, recon=None, riem
     from paper_2208_11630_b200 import binding as fx
     nb = tuple(nb or cfg.nb)
     bc = bc or cfg.bc
-    code = {"periodic": fx.TOPO_PERIODIC, "outflow": fx.TOPO_OUTFLOW}[bc]
+    code = {"periodic": fx.TOPO_PERIODIC, "outflow": fx.TOPO_OUTFLOW, "reflect": fx.TOPO_REFLECT}[bc]
     bcs = [code if cfg.block_dims[d] > 1 else fx.TOPO_NONE for d in range(3)]
     coords = None
     if neigh is None:

@@ -29,6 +29,7 @@ GUARD_CASES = [
     ((12, 1, 1), 4, (3, 1, 1), "outflow", 0), ((12, 1, 1), 4, (1, 1, 1), "periodic", 0),
     ((16, 16, 16), 4, (3, 2, 2), "periodic", 1), ((16, 16, 1), 4, (8, 8, 1), "periodic", 0),
     ((256, 1, 1), 4, (1, 1, 1), "outflow", 0),
+    ((6, 4, 5), 3, (2, 1, 2), "reflect", 0), ((16, 16, 16), 4, (2, 2, 1), "reflect", 1), ((12, 1, 1), 4, (2, 1, 1), "reflect", 0),
 ]
 
 
@@ -98,6 +99,8 @@ ADV_CASES = [  # number, nb, kwargs
     (1, None, {}), (2, None, {}), (3, None, {}), (4, (3, 3, 3), {}), (5, (3, 3, 3), {}),
     (3, (2, 2, 2), dict(riemann=0, rk=3)), (5, (2, 2, 2), dict(recon=1, riemann=0, rk=2)),
     (2, (3, 2, 1), dict(recon=1, rk=3)), (5, (2, 2, 2), dict(bc="outflow")),
+    (5, (2, 2, 2), dict(bc="reflect")), (5, (1, 1, 3), dict(bc="reflect", recon=1, rk=3)), (2, (2, 2, 1), dict(bc="reflect")),
+    (1, None, dict(bc="reflect")),
 ]
 
 
@@ -232,6 +235,41 @@ def test_z_chains_irregular_topology_bitwise_and_parity(recon, rk, nzb):
         assert np.array_equal(got, results[0][0]) and dts == results[0][1]
     assert rel_err(cfg, results[0][0], oplan.interior(Uo)) <= 1e-11
     assert all(abs(g - o) <= 1e-12 * o for g, o in zip(results[0][1], dts_o))
+
+
+@pytest.mark.parametrize("recon,rk", [(0, 2), (1, 3)])
+def test_walls_all_round_chain_lengths_bitwise_and_conservation(recon, rk):
+    """[B9] A closed box (reflecting walls on all six sides, 1 x 2 x 3 blocks): the fused kernel's image cells (x / y
+    halos in the producer warp, z image planes in the prologue and the z loop) against the oracle's filled guard cells;
+    the same bits for chain lengths 1, 2 and 8; and nothing leaves a closed box: total mass and energy are conserved
+    to rounding."""
+    cfg = inputs.config(5, nb=(1, 2, 3))
+    oplan, neigh, coords = oracle_plan_for(cfg, bc="reflect", recon=recon, rk=rk)
+    rng = np.random.default_rng(23)
+    shape = (6, 16, 16, 16)
+    rho = 1.0 + 0.3 * rng.random(shape)
+    vel = 0.4 * rng.standard_normal((3,) + shape)
+    pr = 1.0 + 0.3 * rng.random(shape)
+    Ui = np.stack([rho, rho * vel[0], rho * vel[1], rho * vel[2], pr / (cfg.gamma - 1) + 0.5 * rho * (vel ** 2).sum(0)])
+    Uh = inputs.embed(cfg, torch.from_numpy(Ui))
+    dx = np.full((6, 3), 1.0 / 32)
+    Uo = Uh.numpy().copy()
+    dts = []
+    for step in range(3):
+        dts.append(oplan.compute_dt(Uo, dx, 0.3))
+        oplan.advance(Uo, dx, dts[-1])
+    results = []
+    for zc in (1, 2, 8):
+        gplan, _, _ = gpu_plan_for(cfg, bc="reflect", recon=recon, rk=rk, zchain=zc)
+        assert gplan.path == 1
+        Ud, dxd = Uh.cuda(), torch.from_numpy(dx).cuda()
+        for dt in dts:
+            gplan.fx_hydro_advance(Ud, dxd, dt)
+        results.append(gplan.interior(Ud).cpu().numpy())
+    assert np.array_equal(results[1], results[0]) and np.array_equal(results[2], results[0])
+    assert rel_err(cfg, results[0], oplan.interior(Uo)) <= 1e-11
+    for v in (0, 4):
+        assert abs(results[0][v].sum() - Ui[v].sum()) <= 1e-12 * Ui[v].sum()
 
 
 @pytest.mark.parametrize("path", [None, 1])
