@@ -46,6 +46,9 @@
 #define FXO_OPT_P_FLOOR 1
 #define FXO_OPT_WENO_EPS 2
 #define FXO_OPT_WAVESPEED 3
+#define FXO_OPT_GRAVITY_X 6 /* constant acceleration g_d [B10]; 4 and 5 are options of the CUDA library only */
+#define FXO_OPT_GRAVITY_Y 7
+#define FXO_OPT_GRAVITY_Z 8
 #define FXO_STATUS_NONFINITE 1u
 #define FXO_STATUS_RHO_FLOOR 2u
 #define FXO_STATUS_P_FLOOR 4u
@@ -63,6 +66,7 @@ typedef struct fxo_plan {
   int recon, riemann, rk;
   int64_t S_j, S_k, S_b, S_v;
   double rho_floor, p_floor, weno_eps;
+  double grav[3];
   int wavespeed; /* 0 Einfeldt, 1 Davis [A8] */
   const int32_t *neigh;
   unsigned long long n_nonfinite, n_rho_floor, n_p_floor, n_weno_fb;
@@ -149,6 +153,9 @@ int fxo_plan_set_option(fxo_plan *p, int key, double value) {
   case FXO_OPT_RHO_FLOOR: p->rho_floor = value; return FXO_OK;
   case FXO_OPT_P_FLOOR: p->p_floor = value; return FXO_OK;
   case FXO_OPT_WENO_EPS: p->weno_eps = value; return FXO_OK;
+  case FXO_OPT_GRAVITY_X: p->grav[0] = value; return FXO_OK;
+  case FXO_OPT_GRAVITY_Y: p->grav[1] = value; return FXO_OK;
+  case FXO_OPT_GRAVITY_Z: p->grav[2] = value; return FXO_OK;
   case FXO_OPT_WAVESPEED:
     if (value != 0.0 && value != 1.0) return FXO_ERR_INVALID_ARG;
     p->wavespeed = (int)value;
@@ -570,7 +577,8 @@ static void block_prims(fxo_plan *p, const double *X, int64_t b, double *W) {
 }
 
 /* One RK stage on block b: out = U0 + beta*((X - U0) - S(X)), S = sum_d (dt/dx_d)(F+ - F-)
- * summed in the order x, y, z [O5, O6].  W and Fline are per-thread scratch. */
+ * summed in the order x, y, z [O5, O6], minus dt times the constant-gravity source of the stage input [B10]:
+ * (0, rho g_x, rho g_y, rho g_z, g . m) from the zone's conserved values.  W and Fline are per-thread scratch. */
 static void block_stage(fxo_plan *p, const double *X, const double *U0, double *out, int64_t b,
                         const double *dx, double dt, double beta, int first, double *W, double *S,
                         double *Fline) {
@@ -600,6 +608,15 @@ static void block_stage(fxo_plan *p, const double *X, const double *U0, double *
     for (int j = p->gd[1]; j < p->gd[1] + p->n[1]; ++j)
       for (int i = p->gd[0]; i < p->gd[0] + p->n[0]; ++i) {
         int64_t c = k * p->S_k + j * p->S_j + i;
+        if (p->grav[0] != 0.0 || p->grav[1] != 0.0 || p->grav[2] != 0.0) {
+          int64_t z = b * p->S_b + c;
+          double rho = X[z], gm = 0.0;
+          for (int d = 0; d < 3; ++d) {
+            S[(1 + d) * p->S_b + c] -= dt * (rho * p->grav[d]);
+            gm += p->grav[d] * X[(1 + d) * p->S_v + z];
+          }
+          S[4 * p->S_b + c] -= dt * gm;
+        }
         for (int v = 0; v < 5; ++v) {
           int64_t g = v * p->S_v + b * p->S_b + c;
           if (first)

@@ -19,6 +19,7 @@ _LIB = os.path.join(_HERE, "libfxoracle.so")
 RECON_PLM_MINMOD, RECON_WENO5 = 0, 1
 RIEMANN_HLLE, RIEMANN_HLLC = 0, 1
 BC_OUTFLOW, BC_NONE, BC_REFLECT = -1, -2, -3
+OPT_GRAVITY_X, OPT_GRAVITY_Y, OPT_GRAVITY_Z = 6, 7, 8
 TOPO_PERIODIC, TOPO_OUTFLOW, TOPO_NONE, TOPO_REFLECT = 0, 1, 2, 3
 ORDER_LEX, ORDER_MORTON = 0, 1
 OPT_RHO_FLOOR, OPT_P_FLOOR, OPT_WENO_EPS, OPT_WAVESPEED = 0, 1, 2, 3

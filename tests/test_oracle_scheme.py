@@ -4,6 +4,7 @@ Citations: BASELINE.json north_star (list of invariants), SURVEY.md 8(c)-iii."""
 import math
 
 import numpy as np
+import torch
 import pytest
 
 from oracle import fxoracle as fxo
@@ -207,6 +208,68 @@ def test_reflecting_wall_equals_half_of_a_symmetric_domain():
             a, b = half.interior(Uh)[:, 0], full.interior(Uf)[:, 0]
             assert np.max(np.abs(a - b)) <= (2e-15 if step == 0 else 1e-13) * np.abs(b).max(), (recon, step)
         assert np.abs(half.interior(Uh)[1, 0, 0, :, -1]).max() > 1e-3  # something moves next to the wall
+
+
+def test_constant_gravity_free_fall_closed_form():
+    """[B10] A uniform gas in a periodic box under a constant acceleration g falls freely: fluxes are uniform, so
+    d m/dt = rho g and dE/dt = g . m exactly, i.e. m(t) = m0 + rho g t and E(t) = E0 + g . m0 t + rho |g|^2 t^2 / 2
+    with rho constant.  SSP-RK2/3 integrate a linear m and a quadratic E exactly, so the closed form holds to
+    rounding after any number of steps of any size."""
+    for rk, recon in ((2, 0), (3, 1)):
+        dims, g = (8, 8, 8), 4
+        per = fxo.TOPO_PERIODIC
+        neigh, _ = fxo.topology_cartesian((2, 1, 2), [per] * 3, [per] * 3, fxo.ORDER_LEX)
+        plan = fxo.OraclePlan(dims, g, 4, 1.4, recon, 1, rk)
+        plan.set_topology(neigh)
+        grav = np.array([0.3, -0.2, 0.5])
+        for d in range(3):
+            plan.set_option(fxo.OPT_GRAVITY_X + d, grav[d])
+        rho, vel, pr = 1.3, np.array([0.2, 0.1, -0.4]), 0.9
+        m0 = rho * vel
+        E0 = pr / 0.4 + 0.5 * rho * (vel ** 2).sum()
+        U = np.full(plan.shape, np.nan)
+        I = plan.interior(U)
+        I[0], I[1], I[2], I[3], I[4] = rho, m0[0], m0[1], m0[2], E0
+        dx = np.full((4, 3), 1.0 / 16)
+        t = 0.0
+        for dt in (0.01, 0.003, 0.02, 0.007):
+            plan.advance(U, dx, dt)
+            t += dt
+            I = plan.interior(U)
+            assert np.max(np.abs(I[0] - rho)) <= 1e-15
+            for d in range(3):
+                assert np.max(np.abs(I[1 + d] - (m0[d] + rho * grav[d] * t))) <= 1e-14
+            assert np.max(np.abs(I[4] - (E0 + grav @ m0 * t + 0.5 * rho * (grav ** 2).sum() * t * t))) <= 1e-14
+
+
+def test_constant_gravity_source_is_rho_g_and_g_dot_m():
+    """[B10] For general data the difference between a step with and a step without gravity, divided by dt, tends to
+    the source (0, rho g, g . m) of the zone's own conserved values as dt -> 0 (the flux terms cancel to O(dt))."""
+    cfg = inputs.config(5, nb=(2, 1, 1))
+    cfg.block_dims = (8, 8, 8)
+    plan0, neigh, coords = oracle_plan_for(cfg)
+    plang, _, _ = oracle_plan_for(cfg)
+    grav = np.array([0.7, -1.1, 0.4])
+    for d in range(3):
+        plang.set_option(fxo.OPT_GRAVITY_X + d, grav[d])
+    rng = np.random.default_rng(9)
+    shape = (2, 8, 8, 8)
+    rho = 1.0 + 0.3 * rng.random(shape)
+    vel = 0.4 * rng.standard_normal((3,) + shape)
+    pr = 1.0 + 0.3 * rng.random(shape)
+    Ui = np.stack([rho, rho * vel[0], rho * vel[1], rho * vel[2], pr / (cfg.gamma - 1) + 0.5 * rho * (vel ** 2).sum(0)])
+    U0 = inputs.embed(cfg, torch.from_numpy(Ui)).numpy()
+    dx = np.full((2, 3), 1.0 / 16)
+    errs = []
+    for dt in (1e-4, 1e-5):
+        A, B = U0.copy(), U0.copy()
+        plan0.advance(A, dx, dt)
+        plang.advance(B, dx, dt)
+        D = (plang.interior(B) - plan0.interior(A)) / dt
+        ref = np.stack([np.zeros_like(rho), rho * grav[0], rho * grav[1], rho * grav[2],
+                        grav[0] * Ui[1] + grav[1] * Ui[2] + grav[2] * Ui[3]])
+        errs.append(np.max(np.abs(D - ref)))
+    assert errs[0] <= 2e-2 and errs[1] <= 0.2 * errs[0] + 1e-8  # first order in dt
 
 
 # ------------------------------------------------------------ RK composition, dt
