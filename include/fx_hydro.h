@@ -49,9 +49,12 @@ enum {
   FX_OPT_WENO_EPS = 2,  /* WENO5-JS epsilon, default 1e-6 [A5] */
   FX_OPT_WAVESPEED = 3, /* 0 = Einfeldt (default), 1 = Davis [A8] */
   FX_OPT_PATH = 4,      /* 0 = auto (fused TMA stage kernel when the block shape allows), 1 = generic */
-  FX_OPT_ZCHAIN = 5     /* fused path: longest chain of z-neighbour blocks one CTA marches through, 1..8; 0 (default) =
+  FX_OPT_ZCHAIN = 5,    /* fused path: longest chain of z-neighbour blocks one CTA marches through, 1..8; 0 (default) =
                            chosen from the number of blocks and of SMs so that the launch still fills the GPU.
                            Set before fx_hydro_plan_set_topology.  Results do not depend on it (bit for bit). */
+  FX_OPT_GRAVITY_X = 6, /* constant acceleration g_x (default 0): every stage adds beta dt (0, rho g, g.m) [B10] */
+  FX_OPT_GRAVITY_Y = 7,
+  FX_OPT_GRAVITY_Z = 8
 };
 enum {
   FX_STATUS_NONFINITE = 1u,

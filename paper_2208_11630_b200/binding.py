@@ -21,6 +21,7 @@ BC_OUTFLOW, BC_NONE, BC_REFLECT = -1, -2, -3
 TOPO_PERIODIC, TOPO_OUTFLOW, TOPO_NONE, TOPO_REFLECT = 0, 1, 2, 3
 ORDER_LEX, ORDER_MORTON = 0, 1
 OPT_RHO_FLOOR, OPT_P_FLOOR, OPT_WENO_EPS, OPT_WAVESPEED, OPT_PATH, OPT_ZCHAIN = 0, 1, 2, 3, 4, 5
+OPT_GRAVITY_X, OPT_GRAVITY_Y, OPT_GRAVITY_Z = 6, 7, 8
 STATUS_NONFINITE, STATUS_RHO_FLOOR, STATUS_P_FLOOR, STATUS_WENO_FALLBACK = 1, 2, 4, 8
 
 EXPORTS = [

@@ -131,6 +131,13 @@ extern "C" int fx_hydro_plan_set_option(fx_hydro_plan *plan, int key, double val
     if (value != 0.0 && value != 1.0) return fx_fail(FX_ERR_INVALID_ARG, "set_option: wavespeed must be 0 or 1");
     plan->P.wavespeed = (int)value;
     return FX_OK;
+  case FX_OPT_GRAVITY_X:
+  case FX_OPT_GRAVITY_Y:
+  case FX_OPT_GRAVITY_Z:
+    if (!(value == value) || value > 1e300 || value < -1e300) return fx_fail(FX_ERR_INVALID_ARG, "set_option: gravity must be finite");
+    plan->P.grav[key - FX_OPT_GRAVITY_X] = value;
+    plan->P.grav_on = plan->P.grav[0] != 0.0 || plan->P.grav[1] != 0.0 || plan->P.grav[2] != 0.0;
+    return FX_OK;
   case FX_OPT_ZCHAIN:
     if (!(value >= 0.0 && value <= (double)FX_SEG_MAX)) return fx_fail(FX_ERR_INVALID_ARG, "set_option: zchain must be 0 (auto) or 1..%d", (int)FX_SEG_MAX);
     plan->zchain = (int)value;

@@ -92,6 +92,16 @@ __global__ void __launch_bounds__(128) fx_k_generic_stage(FxParams P, const doub
 #pragma unroll
     for (int v = 0; v < 5; ++v) S[v] += rd * (Fp[v] - Fm[v]);
   }
+  if (P.grav_on) {  // constant-gravity source of the stage input's own zone [B10]
+    const double rho = X[c];
+    double gm = 0.0;
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+      S[1 + d] -= dt * (rho * P.grav[d]);
+      gm += P.grav[d] * X[(1 + d) * P.S_v + c];
+    }
+    S[4] -= dt * gm;
+  }
 #pragma unroll
   for (int v = 0; v < 5; ++v) {
     const long long g = v * P.S_v + c;

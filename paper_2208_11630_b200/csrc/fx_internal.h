@@ -20,6 +20,8 @@ struct FxParams {
   const int *seg;                   // z-chain segments of the fused kernel: [nseg][FX_SEG_STRIDE], device (in the workspace)
   int nseg;
   int walls;                        // some block has a reflecting wall in an active dimension [B9]
+  int grav_on;                      // any component of grav is non-zero [B10]
+  double grav[3];
   unsigned long long *scratch;      // device scratch block, see FX_SCR_*
 };
 

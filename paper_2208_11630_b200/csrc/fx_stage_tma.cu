@@ -191,8 +191,9 @@ __device__ __forceinline__ void flux_dir(const FxParams &P, const double WL[5], 
   F[4] = f[4];
 }
 
-// WALLS: some block of the launch has a reflecting wall [B9] (the image cells' sign flips are compiled in only then)
-template <int RECON, int RIEMANN, int WS, bool FIRST, bool DTOUT, bool WALLS>
+// EXTRAS: some block of the launch has a reflecting wall [B9] or gravity is on [B10]: the image cells' sign flips
+// and the source term are compiled in only then
+template <int RECON, int RIEMANN, int WS, bool FIRST, bool DTOUT, bool EXTRAS>
 __global__ void __launch_bounds__(NTHREADS) __maxnreg__(Rc<RECON>::NREG)
 fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ CUtensorMap mXx,
                const __grid_constant__ CUtensorMap mXy, const __grid_constant__ CUtensorMap mU0,
@@ -224,14 +225,14 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
     int k = Z - qb * nzb;
     int id = S.chain[2 + qb];
     if (id < 0) {
-      const bool wall = WALLS && id == FX_BC_REFLECT;
+      const bool wall = EXTRAS && id == FX_BC_REFLECT;
       if (qb < 0) { id = S.chain[2]; k = wall ? -1 - Z : 0; } else { id = S.chain[1 + M]; k = wall ? nzb - 1 - (Z - nz) : nzb - 1; }
     }
     bs = id;
     kp = k + g2;
   };
-  const bool wall_below = WALLS && S.chain[1] == FX_BC_REFLECT;
-  const int zflip_from = (WALLS && S.chain[2 + M] == FX_BC_REFLECT) ? nz : 0x7fffffff;  // planes >= this carry a negated z momentum
+  const bool wall_below = EXTRAS && S.chain[1] == FX_BC_REFLECT;
+  const int zflip_from = (EXTRAS && S.chain[2 + M] == FX_BC_REFLECT) ? nz : 0x7fffffff;  // planes >= this carry a negated z momentum
 
   // ---------------------------------------------------------------- producer set-up (producer warp, lane 0)
   const bool producer = tid == NZONE_THREADS + 32;
@@ -353,7 +354,7 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
         double u[5];
 #pragma unroll
         for (int v = 0; v < 5; ++v) u[v] = S.ring[(c + r) % NRING][v][j][i];
-        if (WALLS && c + r >= zflip_from) u[3] = -u[3];  // image planes above a reflecting wall
+        if (EXTRAS && c + r >= zflip_from) u[3] = -u[3];  // image planes above a reflecting wall
         const unsigned h = fx_c2p_v2(P, u[0], u[1], u[2], u[3], u[4], q[2 * r]);
         if (c + r < nz) hit |= h;
       }
@@ -389,7 +390,7 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
         // out = [U0 + beta (X - U0)] - sum_d (beta dt/dx_d) (F_d+ - F_d-)
         const double rx = S.rd[0], ry = S.rd[1], rz = S.rd[2];
         int hmax = 0;
-        double res5[5];
+        double res5[5], xs5[5];
 #pragma unroll
         for (int v = 0; v < 5; ++v) {
           const double dFx = S.Lx[v][j][i + 1] - Fx[v];
@@ -399,10 +400,26 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
           const double u0 = FIRST ? xs : S.U0[p & 1][v][j][i];
           const double a = FIRST ? u0 : fma(beta, xs - u0, u0);
           const double res = fma(-rz, dFz, fma(-ry, dFy, fma(-rx, dFx, a)));
-          S.Out[v][j][i] = res;
+          if (!EXTRAS) {  // (the plain kernel keeps its one-pass form: splitting the loop costs it 2 %)
+            S.Out[v][j][i] = res;
+            if (!DTOUT) hmax = max(hmax, __double2hiint(res) & 0x7fffffff);
+          }
           res5[v] = res;
-          if (!DTOUT) hmax = max(hmax, __double2hiint(res) & 0x7fffffff);
+          if (EXTRAS) xs5[v] = xs;
           Fz[v] = Fz_new[v];
+        }
+        if (EXTRAS) {
+          if (P.grav_on) {  // + beta dt (0, rho g, g . m) of the stage input's own zone [B10]
+            const double bdt = (FIRST ? 1.0 : beta) * dt;
+            res5[4] = fma(bdt, fma(P.grav[2], xs5[3], fma(P.grav[1], xs5[2], P.grav[0] * xs5[1])), res5[4]);
+#pragma unroll
+            for (int d = 0; d < 3; ++d) res5[1 + d] = fma(bdt * P.grav[d], xs5[0], res5[1 + d]);
+          }
+#pragma unroll
+          for (int v = 0; v < 5; ++v) {
+            S.Out[v][j][i] = res5[v];
+            if (!DTOUT) hmax = max(hmax, __double2hiint(res5[v]) & 0x7fffffff);
+          }
         }
         if (!DTOUT && hmax >= 0x7ff00000) hit |= FX_STATUS_NONFINITE;
         if (DTOUT) {  // a7 on the finished zone: (|u_d| + c) / dx_d, folded into a running maximum [O7]
@@ -506,8 +523,8 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
     auto halo_off = [&](int t, bool high) -> int {
       int idx;  // cell index inside the box
       // a neighbour's cells; at a reflecting wall this block's own cells in mirrored order [B9]; at outflow its edge cell
-      if (isx) idx = high ? (nhi >= 0 ? t : ((WALLS && nhi == FX_BC_REFLECT) ? BW - 1 - t : BW - 1)) : (nlo >= 0 ? BW - R + t : ((WALLS && nlo == FX_BC_REFLECT) ? R - 1 - t : 0));
-      else idx = high ? (nhi >= 0 ? t : ((WALLS && nhi == FX_BC_REFLECT) ? R - 1 - t : R - 1)) : (nlo >= 0 ? t : ((WALLS && nlo == FX_BC_REFLECT) ? R - 1 - t : 0));
+      if (isx) idx = high ? (nhi >= 0 ? t : ((EXTRAS && nhi == FX_BC_REFLECT) ? BW - 1 - t : BW - 1)) : (nlo >= 0 ? BW - R + t : ((EXTRAS && nlo == FX_BC_REFLECT) ? R - 1 - t : 0));
+      else idx = high ? (nhi >= 0 ? t : ((EXTRAS && nhi == FX_BC_REFLECT) ? R - 1 - t : R - 1)) : (nlo >= 0 ? t : ((EXTRAS && nlo == FX_BC_REFLECT) ? R - 1 - t : 0));
       return isx ? ((high ? 5 * HXV : 0) + m * BW + idx) : ((high ? 5 * HYV : 0) + idx * NX + m);
     };
     int hoff[2 * R];
@@ -523,7 +540,7 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
         double u[5], w[5];
 #pragma unroll
         for (int v = 0; v < 5; ++v) u[v] = Hf[hoff[t] + v * hv];
-        if (WALLS && (t < R ? nlo : nhi) == FX_BC_REFLECT) {  // image cells behind a wall: normal momentum negated
+        if (EXTRAS && (t < R ? nlo : nhi) == FX_BC_REFLECT) {  // image cells behind a wall: normal momentum negated
           if (isx) u[1] = -u[1]; else u[2] = -u[2];
         }
         fx_c2p_v2(P, u[0], u[1], u[2], u[3], u[4], w);
@@ -637,7 +654,7 @@ static int make_map(CUtensorMap *m, const FxParams &P, const double *base, int b
   return FX_OK;
 }
 
-template <int RECON, int RIEMANN, int WS, bool FIRST, bool DTOUT, bool WALLS>
+template <int RECON, int RIEMANN, int WS, bool FIRST, bool DTOUT, bool EXTRAS>
 int launch(const FxParams &P, const double *X, const double *U0, double *out, const double *dx, double dt, const double *dt_dev,
            double beta, double cfl_next, double *dt_next, cudaStream_t st) {
   constexpr int R = Rc<RECON>::R, BW = Rc<RECON>::BW;
@@ -648,7 +665,7 @@ int launch(const FxParams &P, const double *X, const double *U0, double *out, co
   if ((rc = make_map(&mXy, P, X, NX, R))) return rc;
   if ((rc = make_map(&mU0, P, U0, NX, NY))) return rc;
   if ((rc = make_map(&mOut, P, out, NX, NY))) return rc;
-  auto kern = fx_k_stage_tma<RECON, RIEMANN, WS, FIRST, DTOUT, WALLS>;
+  auto kern = fx_k_stage_tma<RECON, RIEMANN, WS, FIRST, DTOUT, EXTRAS>;
   const int smem = (int)sizeof(Smem<RECON>);
   static bool configured = false;  // per instantiation
   if (!configured) {
@@ -672,7 +689,7 @@ int launch(const FxParams &P, const double *X, const double *U0, double *out, co
 template <int RECON, int RIEMANN, int WS>
 int launch_ws(const FxParams &P, const double *X, const double *U0, double *out, const double *dx, double dt, const double *dt_dev,
               double beta, int first, double cfl_next, double *dt_next, cudaStream_t st) {
-  if (P.walls) {
+  if (P.walls || P.grav_on) {
     if (first) return launch<RECON, RIEMANN, WS, true, false, true>(P, X, U0, out, dx, dt, dt_dev, beta, 0.0, nullptr, st);
     if (dt_next) return launch<RECON, RIEMANN, WS, false, true, true>(P, X, U0, out, dx, dt, dt_dev, beta, cfl_next, dt_next, st);
     return launch<RECON, RIEMANN, WS, false, false, true>(P, X, U0, out, dx, dt, dt_dev, beta, 0.0, nullptr, st);

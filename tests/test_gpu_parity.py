@@ -273,6 +273,57 @@ def test_walls_all_round_chain_lengths_bitwise_and_conservation(recon, rk):
 
 
 @pytest.mark.parametrize("path", [None, 1])
+@pytest.mark.parametrize("recon,rk,bc", [(0, 2, "periodic"), (1, 3, "reflect")])
+def test_constant_gravity_parity_and_free_fall(recon, rk, bc, path):
+    """[B10] The gravity source in both stage kernels: parity with the oracle on general data (fused dt included), and
+    the free-fall closed form m = m0 + rho g t, E = E0 + g.m0 t + rho |g|^2 t^2 / 2 for a uniform gas."""
+    from paper_2208_11630_b200 import binding as fx
+    cfg = inputs.config(5, nb=(2, 2, 2))
+    grav = (0.7, -1.1, 0.4)
+    oplan, neigh, coords = oracle_plan_for(cfg, bc=bc, recon=recon, rk=rk)
+    gplan, _, _ = gpu_plan_for(cfg, bc=bc, recon=recon, rk=rk, path=path)
+    assert gplan.path == (1 if path is None else 0)
+    for d in range(3):
+        oplan.set_option(fxo.OPT_GRAVITY_X + d, grav[d])
+        gplan.fx_hydro_plan_set_option(fx.OPT_GRAVITY_X + d, grav[d])
+    rng = np.random.default_rng(31)
+    shape = (8, 16, 16, 16)
+    rho = 1.0 + 0.3 * rng.random(shape)
+    vel = 0.4 * rng.standard_normal((3,) + shape)
+    pr = 1.0 + 0.3 * rng.random(shape)
+    Ui = np.stack([rho, rho * vel[0], rho * vel[1], rho * vel[2], pr / (cfg.gamma - 1) + 0.5 * rho * (vel ** 2).sum(0)])
+    Uh = inputs.embed(cfg, torch.from_numpy(Ui))
+    dx = np.full((8, 3), 1.0 / 32)
+    Uo, Ud, dxd = Uh.numpy().copy(), Uh.cuda(), torch.from_numpy(dx).cuda()
+    dt = gplan.fx_hydro_compute_dt(Ud, dxd, 0.3).clone()
+    for step in range(3):
+        dto = oplan.compute_dt(Uo, dx, 0.3)
+        assert abs(float(dt.item()) - dto) <= 1e-12 * dto
+        oplan.advance(Uo, dx, dto)
+        gplan.fx_hydro_step(Ud, dxd, 0.3, dt)
+    assert rel_err(cfg, gplan.interior(Ud).cpu().numpy(), oplan.interior(Uo)) <= 1e-11
+    # free fall (periodic box only: a wall would stop the gas)
+    if bc == "periodic":
+        r0, v0, p0 = 1.3, np.array([0.2, 0.1, -0.4]), 0.9
+        m0, E0 = r0 * v0, p0 / (cfg.gamma - 1) + 0.5 * r0 * (v0 ** 2).sum()
+        U = torch.full(Uh.shape, float("nan"), dtype=torch.float64)
+        I = inputs.interior_view(cfg, U)
+        for v, val in enumerate((r0, m0[0], m0[1], m0[2], E0)):
+            I[v] = val
+        U = U.cuda()
+        t = 0.0
+        for dts in (0.01, 0.003, 0.02):
+            gplan.fx_hydro_advance(U, dxd, dts)
+            t += dts
+        I = gplan.interior(U).cpu().numpy()
+        g = np.array(grav)
+        assert np.max(np.abs(I[0] - r0)) <= 1e-15
+        for d in range(3):
+            assert np.max(np.abs(I[1 + d] - (m0[d] + r0 * g[d] * t))) <= 1e-14
+        assert np.max(np.abs(I[4] - (E0 + g @ m0 * t + 0.5 * r0 * (g ** 2).sum() * t * t))) <= 1e-14
+
+
+@pytest.mark.parametrize("path", [None, 1])
 def test_status_flags_floors_and_nonfinite(path):
     """A7/A27: primitive floors and non-finite states raise the same status bits as in the oracle, the floored step
     still agrees with it, and nothing traps or hangs."""
