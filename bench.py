@@ -43,6 +43,8 @@ def parse_args():
     ap.add_argument("--nb", default=None, help="override blocks per dimension, e.g. 16,16,16")
     ap.add_argument("--path", type=int, default=0, help="FX_OPT_PATH: 0 auto (fused TMA stage kernel when supported), 1 generic")
     ap.add_argument("--zchain", type=int, default=0, help="FX_OPT_ZCHAIN: z-neighbour blocks per CTA of the fused kernel (0 = library default)")
+    ap.add_argument("--guard-x", type=int, default=-1, help="FX_OPT_GUARD_X: x guard depth (layout); -1 = 8 for 16-wide blocks with 4 guard zones "
+                    "(256-byte row pitch, interior rows on 128-byte lines), else the config's nguard")
     ap.add_argument("--order", default="morton", choices=["lex", "morton"])
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -134,11 +136,14 @@ def build_workload(args, device):
     plan = fx.HydroPlan(cfg.block_dims, cfg.nguard, cfg.nblocks, cfg.gamma, cfg.recon, cfg.riemann, cfg.rk_order,
                         device=device)
     plan.fx_hydro_plan_set_option(fx.OPT_PATH, args.path)
+    guard_x = args.guard_x if args.guard_x >= 0 else (8 if (cfg.block_dims[0] == 16 and cfg.nguard == 4) else cfg.nguard)
+    if guard_x != cfg.nguard:
+        plan.fx_hydro_plan_set_option(fx.OPT_GUARD_X, guard_x)
     if args.zchain:
         plan.fx_hydro_plan_set_option(fx.OPT_ZCHAIN, args.zchain)
     plan.fx_hydro_plan_set_topology(neigh)
     plan.fx_hydro_plan_set_workspace()
-    U = torch.full(plan.shape, float("nan"), dtype=torch.float64, device=device)
+    U = plan.alloc_state(fill=float("nan"))  # interior rows on 128-byte lines where the pitch allows it
     Ui = plan.interior(U)
     chunk = 1024
     for b0 in range(0, cfg.nblocks, chunk):
@@ -262,9 +267,10 @@ def run_ours(args, rank, world, local_rank):
     achieved = alg_bytes_per_launch / (stage_avg_ms * 1e-3) / 1e9
     # traffic: dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture of
     # this command (profiles/r1_ncu_chain_raw.csv: mean of the stage-1 and stage-2 launches); null for other workloads
-    traffic = 20.35e9 if (cfg.number == 5 and args.nb is None and fused and stages == 2) else None
+    gx8 = plan.gd[0] == 8
+    traffic = ((15.97e9 if gx8 else 20.35e9) if (cfg.number == 5 and args.nb is None and fused and stages == 2) else None)
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": traffic, "traffic_source": "ncu capture profiles/r1_ncu_chain_raw.csv (GB per launch, mean of both stages)"
+                "traffic": traffic, "traffic_source": "ncu capture profiles/r1_ncu_gx8_raw.csv (x guard depth 8) / r1_ncu_chain_raw.csv (x guard depth 4): GB per launch, mean of both stages"
                 if traffic else None, "alg_bytes_per_launch": alg_bytes_per_launch, "peak_source": peak_src, "kernel": "fused stage kernel" if fused else "generic stage kernel",
                 "kernel_ms_avg": stage_avg_ms, "kernel_launches_timed": stage_launches,
                 "kernel_share_of_step": stage_ms / ms if ms > 0 else None,
@@ -283,6 +289,7 @@ def run_ours(args, rank, world, local_rank):
                                    f"{cfg.block_dims[0]}x{cfg.block_dims[1]}x{cfg.block_dims[2]} (+{cfg.nguard} guard), "
                                    f"{'WENO5' if cfg.recon else 'PLM-minmod'}+{'HLLC' if cfg.riemann else 'HLLE'}, SSP-RK{stages}",
                        "interior_zones": zones, "state_bytes": plan.bytes_per_state, "block_order": args.order,
+                       "layout": f"x guard depth {plan.gd[0]} (row pitch {plan.S_j * 8} B), y/z guard depth {plan.gd[1]}/{plan.gd[2]}",
                        "path": {0: "generic", 1: "fused (TMA)"}[plan.path], "l2": "inputs (state) larger than L2; no flush needed",
                        "multi_gpu": "replicas only" if world > 1 else "single"},
             "clocks": clocks, "gpu_launches": launches_per_step * args.steps, "roofline": roofline,

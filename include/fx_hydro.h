@@ -54,7 +54,10 @@ enum {
                            Set before fx_hydro_plan_set_topology.  Results do not depend on it (bit for bit). */
   FX_OPT_GRAVITY_X = 6, /* constant acceleration g_x (default 0): every stage adds beta dt (0, rho g, g.m) [B10] */
   FX_OPT_GRAVITY_Y = 7,
-  FX_OPT_GRAVITY_Z = 8
+  FX_OPT_GRAVITY_Z = 8,
+  FX_OPT_GUARD_X = 9    /* guard depth of the x dimension alone, an integer in [nguard, nx] (default nguard).  CHANGES THE
+                           LAYOUT (np[0], strides: query fx_hydro_plan_layout again); set it before workspace and
+                           topology.  See "Layout and DRAM lines" below: 8 with nx = 16 makes the row pitch 256 bytes. */
 };
 enum {
   FX_STATUS_NONFINITE = 1u,
@@ -84,14 +87,19 @@ int fx_hydro_plan_create(fx_hydro_plan **out, const int block_dims[3], int nguar
                          double gamma, int recon, int riemann, int rk_order);
 int fx_hydro_plan_destroy(fx_hydro_plan *plan);
 
-/* Strides and padded extents of the state array (pure). */
+/* Strides and padded extents of the state array (pure).
+ * Layout and DRAM lines: DRAM is read in whole 128-byte lines.  With nx = 16 and 4 guard zones an interior row is 128
+ * bytes inside a 192-byte padded row, so reading the interior rows of a plane fetches the x guard columns as well
+ * (1.5x the bytes).  With FX_OPT_GUARD_X = 8 the pitch is 256 bytes, and if the array is placed so that
+ * U_dev + 8*gd[0] is a multiple of 128 every interior row is exactly one line (1.0x; measured).  Any 16-byte aligned
+ * placement is correct; only the traffic differs.  The library places its own stage copies that way. */
 int fx_hydro_plan_layout(const fx_hydro_plan *plan, fx_layout *out);
 
 /* Options; must be set before the first advance.  Unknown key / bad value -> FX_ERR_INVALID_ARG. */
 int fx_hydro_plan_set_option(fx_hydro_plan *plan, int key, double value);
 
 /* Workspace (device, caller-owned, 256-byte aligned): a 256-byte scratch block (dt reduction word,
- * status word and counters) + (rk_order - 1) state copies for the RK stages + the z-segment table
+ * status word and counters) + a 256-byte pad + (rk_order - 1) state copies for the RK stages + the z-segment table
  * (12 int32 per block, see FX_OPT_ZCHAIN).  set_workspace initialises the scratch block and
  * synchronises the device once. */
 size_t fx_hydro_plan_workspace_bytes(const fx_hydro_plan *plan);

@@ -21,7 +21,7 @@ BC_OUTFLOW, BC_NONE, BC_REFLECT = -1, -2, -3
 TOPO_PERIODIC, TOPO_OUTFLOW, TOPO_NONE, TOPO_REFLECT = 0, 1, 2, 3
 ORDER_LEX, ORDER_MORTON = 0, 1
 OPT_RHO_FLOOR, OPT_P_FLOOR, OPT_WENO_EPS, OPT_WAVESPEED, OPT_PATH, OPT_ZCHAIN = 0, 1, 2, 3, 4, 5
-OPT_GRAVITY_X, OPT_GRAVITY_Y, OPT_GRAVITY_Z = 6, 7, 8
+OPT_GRAVITY_X, OPT_GRAVITY_Y, OPT_GRAVITY_Z, OPT_GUARD_X = 6, 7, 8, 9
 STATUS_NONFINITE, STATUS_RHO_FLOOR, STATUS_P_FLOOR, STATUS_WENO_FALLBACK = 1, 2, 4, 8
 
 EXPORTS = [
@@ -119,13 +119,9 @@ class HydroPlan:
         self._h = C.c_void_p()
         _check(lib().fx_hydro_plan_create(C.byref(self._h), (C.c_int * 3)(*block_dims), nguard, nvars, nblocks, gamma,
                                           recon, riemann, rk_order))
-        L = Layout()
-        _check(lib().fx_hydro_plan_layout(self._h, C.byref(L)))
         self.block_dims = tuple(int(d) for d in block_dims)
         self.nblocks, self.nvars, self.gamma, self.rk_order = int(nblocks), nvars, gamma, rk_order
-        self.np, self.gd = tuple(L.np), tuple(L.gd)
-        self.S_j, self.S_k, self.S_b, self.S_v = L.S_j, L.S_k, L.S_b, L.S_v
-        self.bytes_per_state = L.bytes_per_state
+        self._read_layout()
         self.device = torch.device(device)
         self._ws = None
         self._neigh = None
@@ -135,6 +131,33 @@ class HydroPlan:
         if getattr(self, "_h", None) is not None and self._h.value:
             lib().fx_hydro_plan_destroy(self._h)
             self._h = C.c_void_p()
+
+    def _read_layout(self):
+        L = Layout()
+        _check(lib().fx_hydro_plan_layout(self._h, C.byref(L)))
+        self.np, self.gd = tuple(L.np), tuple(L.gd)
+        self.S_j, self.S_k, self.S_b, self.S_v = L.S_j, L.S_k, L.S_b, L.S_v
+        self.bytes_per_state = L.bytes_per_state
+
+    def alloc_state(self, fill=None, device=None, pin_memory=False):
+        """A state array `shape` placed so that its interior rows start on a 128-byte boundary where the row pitch allows
+        it (include/fx_hydro.h, "Layout and DRAM lines"): any placement is correct, this one reads no guard bytes."""
+        n = int(np.prod(self.shape))
+        off = ((128 - (8 * self.gd[0]) % 128) % 128) // 8
+        dev = self.device if device is None else torch.device(device)
+        buf = torch.empty(n + 16, dtype=torch.float64, device=dev, pin_memory=pin_memory)
+        assert buf.data_ptr() % 128 == 0
+        U = buf[off:off + n].view(self.shape)
+        if fill is not None:
+            U.fill_(fill)
+        return U
+
+    def embed(self, interior, guard_value=float("nan")):
+        """Device state array (alloc_state placement) holding `interior` [5][nblocks][nz][ny][nx]; guard zones get
+        guard_value (NaN: the advance must not depend on them)."""
+        U = self.alloc_state(fill=guard_value)
+        self.interior(U).copy_(torch.as_tensor(interior).to(self.device))
+        return U
 
     @property
     def shape(self):
@@ -146,6 +169,8 @@ class HydroPlan:
 
     def fx_hydro_plan_set_option(self, key, value):
         _check(lib().fx_hydro_plan_set_option(self._h, key, float(value)))
+        if key == OPT_GUARD_X:
+            self._read_layout()  # the option changes np[0] and the strides
 
     def fx_hydro_plan_workspace_bytes(self):
         return int(lib().fx_hydro_plan_workspace_bytes(self._h))

@@ -30,6 +30,17 @@ int fx_cuda_check(cudaError_t e, const char *what) {
 extern "C" const char *fx_last_error(void) { return fx_errbuf; }
 
 // ------------------------------------------------------------------ plan (a0)
+// Padded extents and strides from the guard depths.
+static int fx_relayout(fx_hydro_plan *p) {
+  FxParams &P = p->P;
+  for (int d = 0; d < 3; ++d) P.np[d] = P.n[d] + 2 * P.gd[d];
+  P.S_j = P.np[0];
+  P.S_k = (long long)P.np[0] * P.np[1];
+  P.S_b = P.S_k * P.np[2];
+  P.S_v = P.S_b * P.nblocks;
+  return P.S_b > 2147483647LL ? -1 : 0;
+}
+
 extern "C" int fx_hydro_plan_create(fx_hydro_plan **out, const int block_dims[3], int nguard, int nvars,
                                     int64_t nblocks, double gamma, int recon, int riemann, int rk_order) {
   if (!out || !block_dims) return fx_fail(FX_ERR_INVALID_ARG, "plan_create: null argument");
@@ -62,21 +73,16 @@ extern "C" int fx_hydro_plan_create(fx_hydro_plan **out, const int block_dims[3]
       }
     }
     P.gd[d] = P.active[d] ? nguard : 0;
-    P.np[d] = P.n[d] + 2 * P.gd[d];
   }
   if (nactive == 0) {
     delete p;
     return fx_fail(FX_ERR_INVALID_ARG, "plan_create: no active dimension");
   }
-  P.S_j = P.np[0];
-  P.S_k = (long long)P.np[0] * P.np[1];
-  P.S_b = P.S_k * P.np[2];
-  P.S_v = P.S_b * nblocks;
-  if (P.S_b > 2147483647LL) {
+  P.nblocks = nblocks;
+  if (fx_relayout(p)) {
     delete p;
     return fx_fail(FX_ERR_INVALID_ARG, "plan_create: padded block too large");
   }
-  P.nblocks = nblocks;
   P.gamma = gamma;
   P.gm1 = gamma - 1.0;
   P.igm1 = 1.0 / (gamma - 1.0);
@@ -138,6 +144,21 @@ extern "C" int fx_hydro_plan_set_option(fx_hydro_plan *plan, int key, double val
     plan->P.grav[key - FX_OPT_GRAVITY_X] = value;
     plan->P.grav_on = plan->P.grav[0] != 0.0 || plan->P.grav[1] != 0.0 || plan->P.grav[2] != 0.0;
     return FX_OK;
+  case FX_OPT_GUARD_X: {
+    if (plan->workspace || plan->topology_set)
+      return fx_fail(FX_ERR_STATE, "set_option: the x guard depth changes the layout and must be set before workspace and topology");
+    const int g = (int)value;
+    if (!plan->P.active[0] || (double)g != value || g < plan->nguard || g > plan->P.n[0])
+      return fx_fail(FX_ERR_INVALID_ARG, "set_option: x guard depth must be an integer in [nguard, nx] of an active x dimension");
+    const int old = plan->P.gd[0];
+    plan->P.gd[0] = g;
+    if (fx_relayout(plan)) {
+      plan->P.gd[0] = old;
+      fx_relayout(plan);
+      return fx_fail(FX_ERR_INVALID_ARG, "set_option: padded block too large");
+    }
+    return FX_OK;
+  }
   case FX_OPT_ZCHAIN:
     if (!(value >= 0.0 && value <= (double)FX_SEG_MAX)) return fx_fail(FX_ERR_INVALID_ARG, "set_option: zchain must be 0 (auto) or 1..%d", (int)FX_SEG_MAX);
     plan->zchain = (int)value;
@@ -164,15 +185,19 @@ static size_t fx_seg_bytes(const fx_hydro_plan *plan) {  // room for one segment
   return (((size_t)plan->P.nblocks * FX_SEG_STRIDE * sizeof(int)) + 255) & ~(size_t)255;
 }
 
+// The stage copies start `fx_stage_pad` bytes into a 256-byte pad block, so that their interior rows start on a
+// 128-byte boundary like the caller's array should (include/fx_hydro.h, "Layout and DRAM lines").
+static size_t fx_stage_pad(const fx_hydro_plan *plan) { return (128 - ((size_t)plan->P.gd[0] * 8) % 128) % 128; }
+
 extern "C" size_t fx_hydro_plan_workspace_bytes(const fx_hydro_plan *plan) {
   if (!plan) return 0;
-  return (size_t)FX_SCR_WORDS * 8 + (size_t)(plan->rk - 1) * fx_state_bytes_aligned(plan) + fx_seg_bytes(plan);
+  return (size_t)FX_SCR_WORDS * 8 + 256 + (size_t)(plan->rk - 1) * fx_state_bytes_aligned(plan) + fx_seg_bytes(plan);
 }
 
 // Upload the segment table into its place behind the stage copies (needs both the workspace and the topology).
 static int fx_seg_upload(fx_hydro_plan *plan) {
   if (!plan->workspace || !plan->seg_host) return FX_OK;
-  int *dst = (int *)((char *)plan->workspace + FX_SCR_WORDS * 8 + (size_t)(plan->rk - 1) * fx_state_bytes_aligned(plan));
+  int *dst = (int *)((char *)plan->workspace + FX_SCR_WORDS * 8 + 256 + (size_t)(plan->rk - 1) * fx_state_bytes_aligned(plan));
   if (plan->nseg_host > 0)
     FX_CUDA(cudaMemcpy(dst, plan->seg_host, (size_t)plan->nseg_host * FX_SEG_STRIDE * sizeof(int), cudaMemcpyHostToDevice));
   plan->P.seg = dst;
@@ -194,7 +219,7 @@ extern "C" int fx_hydro_plan_set_workspace(fx_hydro_plan *plan, void *ws, size_t
   plan->workspace = ws;
   plan->workspace_bytes = bytes;
   plan->P.scratch = (unsigned long long *)ws;
-  char *base = (char *)ws + FX_SCR_WORDS * 8;
+  char *base = (char *)ws + FX_SCR_WORDS * 8 + fx_stage_pad(plan);
   plan->stage[0] = (double *)base;
   plan->stage[1] = plan->rk == 3 ? (double *)(base + fx_state_bytes_aligned(plan)) : nullptr;
   return fx_seg_upload(plan);

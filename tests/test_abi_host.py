@@ -72,11 +72,11 @@ def test_layout_matches_oracle_and_closed_form(dims, g, nb):
     assert (L.S_j, L.S_k, L.S_b, L.S_v, L.bytes_per_state) == (o.S_j, o.S_k, o.S_b, o.S_v, o.bytes_per_state)
     npd = [d + 2 * g if d > 1 else d for d in dims]
     assert L.S_b == npd[0] * npd[1] * npd[2] and L.bytes_per_state == 5 * 8 * nb * L.S_b
-    # workspace = 256-byte scratch + (rk - 1) state copies (256-byte aligned) + z-segment table (12 ints per block)
+    # workspace = 256-byte scratch + 256-byte pad + (rk - 1) state copies (256-byte aligned) + z-segment table (12 ints per block)
     ws = fx.lib().fx_hydro_plan_workspace_bytes(h)
-    assert ws == 256 + ((L.bytes_per_state + 255) // 256) * 256 + ((nb * 12 * 4 + 255) // 256) * 256
+    assert ws == 512 + ((L.bytes_per_state + 255) // 256) * 256 + ((nb * 12 * 4 + 255) // 256) * 256
     rc3, h3 = create(dims, g, nb, rk=3)
-    assert fx.lib().fx_hydro_plan_workspace_bytes(h3) == 256 + 2 * (((L.bytes_per_state + 255) // 256) * 256) + ((nb * 12 * 4 + 255) // 256) * 256
+    assert fx.lib().fx_hydro_plan_workspace_bytes(h3) == 512 + 2 * (((L.bytes_per_state + 255) // 256) * 256) + ((nb * 12 * 4 + 255) // 256) * 256
 
 
 def test_config5_needs_64bit_indexing():

@@ -323,6 +323,61 @@ def test_constant_gravity_parity_and_free_fall(recon, rk, bc, path):
         assert np.max(np.abs(I[4] - (E0 + g @ m0 * t + 0.5 * r0 * (g ** 2).sum() * t * t))) <= 1e-14
 
 
+@pytest.mark.parametrize("recon,rk,bc,path", [(0, 2, "periodic", None), (1, 3, "outflow", None), (0, 3, "reflect", None), (0, 2, "periodic", 1)])
+def test_x_guard_depth_8_layout(recon, rk, bc, path):
+    """FX_OPT_GUARD_X = 8: 256-byte row pitch.  Same interiors as the oracle (which keeps its own 4-deep layout) after
+    three fused steps, on an array placed by alloc_state and on one deliberately misplaced by 16 bytes (placement
+    changes the DRAM traffic, never the result: the two agree bit for bit); the filled guard zones equal the oracle's
+    8-deep fill cropped to (8, 4, 4); and the option is refused once the workspace exists."""
+    from paper_2208_11630_b200 import binding as fx
+    cfg = inputs.config(5, nb=(2, 2, 2))
+    oplan, neigh, coords = oracle_plan_for(cfg, bc=bc, recon=recon, rk=rk)
+    code = {"periodic": fx.TOPO_PERIODIC, "outflow": fx.TOPO_OUTFLOW, "reflect": fx.TOPO_REFLECT}[bc]
+    gplan = fx.HydroPlan(cfg.block_dims, cfg.nguard, 8, cfg.gamma, recon, cfg.riemann, rk)
+    if path is not None:
+        gplan.fx_hydro_plan_set_option(fx.OPT_PATH, path)
+    gplan.fx_hydro_plan_set_option(fx.OPT_GUARD_X, 8)
+    assert gplan.np == (32, 24, 24) and gplan.gd == (8, 4, 4) and gplan.S_j == 32
+    gplan.fx_hydro_plan_set_topology(neigh)
+    gplan.fx_hydro_plan_set_workspace()
+    assert gplan.path == (1 if path is None else 0)
+    with pytest.raises(fx.FxError):
+        gplan.fx_hydro_plan_set_option(fx.OPT_GUARD_X, 4)
+    rng = np.random.default_rng(41)
+    shape = (8, 16, 16, 16)
+    rho = 1.0 + 0.3 * rng.random(shape)
+    vel = 0.4 * rng.standard_normal((3,) + shape)
+    pr = 1.0 + 0.3 * rng.random(shape)
+    Ui = np.stack([rho, rho * vel[0], rho * vel[1], rho * vel[2], pr / (cfg.gamma - 1) + 0.5 * rho * (vel ** 2).sum(0)])
+    Uo = inputs.embed(cfg, torch.from_numpy(Ui)).numpy()
+    Ud = gplan.embed(Ui)
+    assert (Ud.data_ptr() + 8 * 8) % 128 == 0
+    n = int(np.prod(gplan.shape))
+    buf = torch.full((n + 16,), float("nan"), dtype=torch.float64, device="cuda")
+    Um = buf[2:2 + n].view(gplan.shape)  # interior rows at 80 mod 128
+    gplan.interior(Um).copy_(torch.from_numpy(Ui))
+    dx = np.full((8, 3), 1.0 / 32)
+    dxd = torch.from_numpy(dx).cuda()
+    dt = gplan.fx_hydro_compute_dt(Ud, dxd, 0.3).clone()
+    dtm = dt.clone()
+    for step in range(3):
+        dto = oplan.compute_dt(Uo, dx, 0.3)
+        assert abs(float(dt.item()) - dto) <= 1e-12 * dto
+        oplan.advance(Uo, dx, dto)
+        gplan.fx_hydro_step(Ud, dxd, 0.3, dt)
+        gplan.fx_hydro_step(Um, dxd, 0.3, dtm)
+    assert torch.equal(gplan.interior(Ud), gplan.interior(Um)) and torch.equal(dt, dtm)
+    assert rel_err(cfg, gplan.interior(Ud).cpu().numpy(), oplan.interior(Uo)) <= 1e-11
+    # guard fill in the wide layout against the oracle with 8 guard zones everywhere
+    o8 = fxo.OraclePlan(cfg.block_dims, 8, 8, cfg.gamma, recon, cfg.riemann, rk)
+    o8.set_topology(neigh)
+    V = np.full(o8.shape, np.nan)
+    o8.interior(V)[...] = gplan.interior(Ud).cpu().numpy()
+    o8.fill_guardcells(V)
+    gplan.fx_fill_guardcells(Ud)
+    assert np.array_equal(Ud.cpu().numpy(), V[:, :, 4:-4, 4:-4, :])
+
+
 @pytest.mark.parametrize("path", [None, 1])
 def test_status_flags_floors_and_nonfinite(path):
     """A7/A27: primitive floors and non-finite states raise the same status bits as in the oracle, the floored step
