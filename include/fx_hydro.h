@@ -156,6 +156,15 @@ int fx_hydro_advance(fx_hydro_plan *plan, double *U_dev, const double *dx_dev, d
 int fx_hydro_advance_host(fx_hydro_plan *plan, double *U_host, const double *dx_host, double cfl, int nsteps,
                           double *U_stage_dev, double *dx_stage_dev, double *dt_last_host, void *stream);
 
+/* The same with the host holding INTERIOR zones only: Uint_host is double [5][nblocks][nz][ny][nx] (no guard zones:
+ * they carry no information, and the padded state is 3.4x the bytes of a 16^3 block's interior).  The call copies it
+ * to packed_stage_dev (same size, caller-owned), scatters it into the padded staging state U_stage_dev
+ * (bytes_per_state, caller-owned; its guard zones need not be initialised), runs the steps as above, gathers the
+ * interiors and copies them back into Uint_host.  PCIe carries interior bytes only, each way. */
+int fx_hydro_advance_host_interior(fx_hydro_plan *plan, double *Uint_host, const double *dx_host, double cfl, int nsteps,
+                                   double *U_stage_dev, double *packed_stage_dev, double *dx_stage_dev,
+                                   double *dt_last_host, void *stream);
+
 /* As fx_hydro_advance, but dt is read on the device from dt_dev (e.g. written by fx_hydro_compute_dt
  * on the same stream): no host round trip per step. */
 int fx_hydro_advance_devdt(fx_hydro_plan *plan, double *U_dev, const double *dx_dev, const double *dt_dev,

@@ -28,7 +28,7 @@ EXPORTS = [
     "fx_last_error", "fx_hydro_plan_create", "fx_hydro_plan_destroy", "fx_hydro_plan_layout",
     "fx_hydro_plan_set_option", "fx_hydro_plan_workspace_bytes", "fx_hydro_plan_set_workspace",
     "fx_hydro_plan_set_topology", "fx_topology_cartesian", "fx_fill_guardcells", "fx_guardcell_index_map",
-    "fx_hydro_compute_dt", "fx_hydro_advance", "fx_hydro_advance_host", "fx_hydro_advance_devdt", "fx_hydro_step",
+    "fx_hydro_compute_dt", "fx_hydro_advance", "fx_hydro_advance_host", "fx_hydro_advance_host_interior", "fx_hydro_advance_devdt", "fx_hydro_step",
     "fx_hydro_status", "fx_hydro_status_reset", "fx_debug_compute_fluxes", "fx_hydro_plan_path",
     "fx_probe_fp64_fma", "fx_hydro_plan_set_timing", "fx_hydro_plan_get_timing",
 ]
@@ -75,6 +75,7 @@ def lib():
         L.fx_hydro_advance_devdt.argtypes = [vp, vp, vp, vp, vp]
         L.fx_hydro_step.argtypes = [vp, vp, vp, C.c_double, vp, vp]
         L.fx_hydro_advance_host.argtypes = [vp, vp, vp, C.c_double, C.c_int, vp, vp, vp, vp]
+        L.fx_hydro_advance_host_interior.argtypes = [vp, vp, vp, C.c_double, C.c_int, vp, vp, vp, vp, vp]
         L.fx_hydro_status.argtypes = [vp, C.POINTER(C.c_uint32), C.POINTER(C.c_ulonglong), vp]
         L.fx_hydro_status_reset.argtypes = [vp, vp]
         L.fx_debug_compute_fluxes.argtypes = [vp, vp, C.c_int, vp, vp]
@@ -219,6 +220,24 @@ class HydroPlan:
         """Advance by the device-resident dt (a 1-element float64 CUDA tensor) and overwrite it with the next step's dt."""
         _check(lib().fx_hydro_step(self._h, _dev(U, torch.float64), _dev(dx, torch.float64), float(cfl),
                                    _dev(dt, torch.float64), _stream(stream)))
+
+    @property
+    def interior_shape(self):
+        n = self.block_dims
+        return (self.nvars, self.nblocks, n[2], n[1], n[0])
+
+    def fx_hydro_advance_host_interior(self, Uint_host, dx_host, cfl, nsteps, U_stage, packed_stage, dx_stage, stream=None):
+        """Uint_host: CPU (preferably pinned) float64 tensor of interior zones [5][nblocks][nz][ny][nx], updated in place;
+        U_stage: device padded state; packed_stage: device tensor of Uint_host's size.  Returns the last dt."""
+        assert not Uint_host.is_cuda and Uint_host.dtype == torch.float64 and Uint_host.is_contiguous()
+        assert tuple(Uint_host.shape) == self.interior_shape and packed_stage.numel() == Uint_host.numel()
+        assert not dx_host.is_cuda and dx_host.dtype == torch.float64 and dx_host.is_contiguous()
+        dt_last = C.c_double(float("nan"))
+        _check(lib().fx_hydro_advance_host_interior(self._h, C.c_void_p(Uint_host.data_ptr()), C.c_void_p(dx_host.data_ptr()),
+                                                    float(cfl), int(nsteps), _dev(U_stage, torch.float64),
+                                                    _dev(packed_stage, torch.float64), _dev(dx_stage, torch.float64),
+                                                    C.cast(C.byref(dt_last), C.c_void_p), _stream(stream)))
+        return float(dt_last.value)
 
     def fx_hydro_advance_host(self, U_host, dx_host, cfl, nsteps, U_stage, dx_stage, stream=None):
         """U_host / dx_host: CPU (preferably pinned) float64 tensors, updated in place.  Returns the last dt."""

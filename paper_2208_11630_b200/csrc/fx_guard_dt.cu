@@ -73,6 +73,34 @@ int fx_launch_fill_guardcells(const FxParams &P, double *U, cudaStream_t st) {
   return FX_OK;
 }
 
+// ------------------------------------------------------------------ interior <-> padded state (host-buffer path)
+// packed[v][b][k][j][i] over interior zones only  <->  U[v][b][k+g2][j+g1][i+g0].  One thread per interior zone and
+// variable; rows of nx doubles are contiguous on both sides.  TO_PACKED: gather, else scatter (guard zones untouched).
+template <bool TO_PACKED>
+__global__ void __launch_bounds__(256) fx_k_pack_interior(FxParams P, double *__restrict__ U, double *__restrict__ packed,
+                                                          long long n) {
+  const int nx = P.n[0], ny = P.n[1], nz = P.n[2];
+  const long long per_block = (long long)nx * ny * nz;
+  for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (long long)gridDim.x * blockDim.x) {
+    const long long vb = e / per_block;  // v * nblocks + b: S_v = nblocks * S_b, so the padded offset is vb * S_b
+    const int r = (int)(e - vb * per_block);
+    const int i = r % nx, j = (r / nx) % ny, k = r / (nx * ny);
+    const long long a = vb * P.S_b + (long long)(k + P.gd[2]) * P.S_k + (long long)(j + P.gd[1]) * P.S_j + (i + P.gd[0]);
+    if (TO_PACKED) packed[e] = U[a]; else U[a] = packed[e];
+  }
+}
+
+int fx_launch_pack_interior(const FxParams &P, double *U, double *packed, int to_packed, cudaStream_t st) {
+  const long long n = 5LL * P.nblocks * P.n[0] * P.n[1] * P.n[2];
+  if (n == 0) return FX_OK;
+  const long long want = (n + 255) / 256;
+  const unsigned grid = (unsigned)(want < 148LL * 32 ? want : 148LL * 32);
+  if (to_packed) fx_k_pack_interior<true><<<grid, 256, 0, st>>>(P, U, packed, n);
+  else fx_k_pack_interior<false><<<grid, 256, 0, st>>>(P, U, packed, n);
+  FX_LAUNCH_CHECK("pack_interior");
+  return FX_OK;
+}
+
 int fx_launch_index_map(const FxParams &P, long long b0, long long nb, long long *src, cudaStream_t st) {
   if (nb == 0) return FX_OK;
   dim3 grid;

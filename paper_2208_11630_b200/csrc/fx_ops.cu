@@ -159,6 +159,34 @@ extern "C" int fx_hydro_advance_host(fx_hydro_plan *plan, double *U_host, const 
   return FX_OK;
 }
 
+extern "C" int fx_hydro_advance_host_interior(fx_hydro_plan *plan, double *Uint_host, const double *dx_host, double cfl,
+                                              int nsteps, double *U_stage, double *packed_stage, double *dx_stage,
+                                              double *dt_last_host, void *stream) {
+  int rc = fx_need(plan, true, true, "advance_host_interior");
+  if (rc) return rc;
+  if (nsteps < 0 || !Uint_host || !dx_host || !U_stage || !packed_stage || !dx_stage)
+    return fx_fail(FX_ERR_INVALID_ARG, "advance_host_interior: null argument or negative nsteps");
+  cudaStream_t st = (cudaStream_t)stream;
+  const FxParams &P = plan->P;
+  const size_t ib = (size_t)plan->nvars * P.nblocks * P.n[0] * P.n[1] * P.n[2] * sizeof(double);
+  const size_t db = (size_t)P.nblocks * 3 * sizeof(double);
+  FX_CUDA(cudaMemcpyAsync(packed_stage, Uint_host, ib, cudaMemcpyHostToDevice, st));
+  FX_CUDA(cudaMemcpyAsync(dx_stage, dx_host, db, cudaMemcpyHostToDevice, st));
+  if ((rc = fx_launch_pack_interior(P, U_stage, packed_stage, 0, st))) return rc;
+  double *dt_dev = (double *)&plan->P.scratch[FX_SCR_WORDS - 1];
+  double *dt_used = dt_dev - 1;
+  if (nsteps > 0 && (rc = fx_launch_compute_dt(P, U_stage, dx_stage, cfl, dt_dev, st))) return rc;
+  for (int s = 0; s < nsteps; ++s) {
+    FX_CUDA(cudaMemcpyAsync(dt_used, dt_dev, sizeof(double), cudaMemcpyDeviceToDevice, st));
+    if ((rc = fx_advance_impl(plan, U_stage, dx_stage, 0.0, dt_dev, st, cfl, dt_dev))) return rc;
+  }
+  if ((rc = fx_launch_pack_interior(P, U_stage, packed_stage, 1, st))) return rc;
+  FX_CUDA(cudaMemcpyAsync(Uint_host, packed_stage, ib, cudaMemcpyDeviceToHost, st));
+  if (dt_last_host && nsteps > 0) FX_CUDA(cudaMemcpyAsync(dt_last_host, dt_used, sizeof(double), cudaMemcpyDeviceToHost, st));
+  FX_CUDA(cudaStreamSynchronize(st));
+  return FX_OK;
+}
+
 extern "C" int fx_hydro_status(fx_hydro_plan *plan, uint32_t *flags, unsigned long long counts[4], void *stream) {
   int rc = fx_need(plan, false, true, "status");
   if (rc) return rc;

@@ -423,6 +423,28 @@ def test_advance_host_equals_device_path():
     dt_last = gplan.fx_hydro_advance_host(Hh, dxh, cfg.cfl, 2, stage, dstage)
     assert np.isfinite(dt_last) and dt_last > 0
     assert torch.equal(gplan.interior(Hh), gplan.interior(A).cpu())
+    # the interior-only host call: same bits, a staging state whose guard zones are NaN, both layouts
+    for gx, number in ((4, 3), (8, 5), (4, 2)):
+        cfg2, _, g2, Uh2, dx2 = setup(number, (2, 2, 2) if number != 2 else None)
+        if gx == 8:
+            from paper_2208_11630_b200 import binding as fx
+            g2 = fx.HydroPlan(cfg2.block_dims, cfg2.nguard, g2.nblocks, cfg2.gamma, cfg2.recon, cfg2.riemann, cfg2.rk_order)
+            g2.fx_hydro_plan_set_option(fx.OPT_GUARD_X, 8)
+            g2.fx_hydro_plan_set_topology(gpu_plan_for(cfg2)[1])
+            g2.fx_hydro_plan_set_workspace()
+        Ui = inputs.interior_view(cfg2, Uh2).contiguous()
+        B = g2.embed(Ui)
+        dxd2 = torch.from_numpy(dx2).cuda()
+        for _ in range(2):
+            g2.fx_hydro_advance(B, dxd2, g2.fx_hydro_compute_dt(B, dxd2, cfg2.cfl))
+        Hi = Ui.clone().pin_memory()
+        assert tuple(Hi.shape) == g2.interior_shape
+        stage = g2.alloc_state(fill=float("nan"))
+        packed = torch.empty(Hi.numel(), dtype=torch.float64, device="cuda")
+        dt2 = g2.fx_hydro_advance_host_interior(Hi, torch.from_numpy(dx2).pin_memory(), cfg2.cfl, 2, stage, packed,
+                                                torch.empty_like(dxd2))
+        assert np.isfinite(dt2) and dt2 > 0
+        assert torch.equal(Hi, g2.interior(B).cpu())
 
 
 @pytest.mark.parametrize("recon,riemann,rk", [(0, 0, 2), (0, 1, 3), (1, 0, 3), (1, 1, 2)])
