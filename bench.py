@@ -268,7 +268,7 @@ def run_ours(args, rank, world, local_rank):
     # traffic: dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture of
     # this command (profiles/r1_ncu_chain_raw.csv: mean of the stage-1 and stage-2 launches); null for other workloads
     gx8 = plan.gd[0] == 8
-    traffic = ((15.97e9 if gx8 else 20.35e9) if (cfg.number == 5 and args.nb is None and fused and stages == 2) else None)
+    traffic = ((16.31e9 if gx8 else 20.35e9) if (cfg.number == 5 and args.nb is None and fused and stages == 2) else None)
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": traffic, "traffic_source": "ncu capture profiles/r1_ncu_gx8_raw.csv (x guard depth 8) / r1_ncu_chain_raw.csv (x guard depth 4): GB per launch, mean of both stages"
                 if traffic else None, "alg_bytes_per_launch": alg_bytes_per_launch, "peak_source": peak_src, "kernel": "fused stage kernel" if fused else "generic stage kernel",
