@@ -5,8 +5,10 @@ A "step" is one pass of the whole hot path over the workload: fx_hydro_step = al
 device-resident dt, and the CFL reduction (a7) of the advanced state, which the fused path forms inside the last
 stage; the first dt comes from fx_hydro_compute_dt before the warm-up.  Metric: hydro zone-updates/s per RK
 stage = interior zones x stages / time.  Workload at N = 1: BASELINE.json configs[4] (32768 blocks of 16^3,
-PLM-minmod + HLLC, SSP-RK2; 18.1 GB per state copy, far larger than the 126 MB L2, so nothing is served
-from cache between timed iterations).  N > 1: N independent replicas of that workload, one per rank
+PLM-minmod + HLLC, SSP-RK2; 24.2 GB per state copy in the wide layout bench.py picks for 16-wide blocks
+(--guard-x, FX_OPT_GUARD_X; 18.1 GB in the compact one), far larger than the 126 MB L2, so nothing is served
+from cache between timed iterations).  e2e: the same step through fx_hydro_advance_host_interior, the host
+holding the interior zones in a pinned buffer (5.37 GB each way per step inside the timed region).  N > 1: N independent replicas of that workload, one per rank
 ("replicas only", DESIGN.md section Multi-GPU); no data-path collective is invented.
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 5] [--nb a,b,c]
