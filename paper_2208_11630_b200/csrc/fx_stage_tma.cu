@@ -1,9 +1,10 @@
 // fx_stage_tma.cu -- fused per-stage kernel for 3-D blocks with a 16 x 16 (x, y) cross-section (K1+K2+K3),
 // fed and drained by TMA.
 //
-// One 288-thread CTA per block marches the block's 16 x 16 column of zones through z; two CTAs share an SM, so
-// that one of them computes while the other waits at a barrier or for data.  Thread (i,j) of the 256 zone
-// threads owns the zones (i,j,k), k = 0..nz-1:
+// One 320-thread CTA per SEGMENT -- up to 8 blocks that follow one another in +z (fx_hydro_plan_set_topology builds
+// the table) -- marches a 16 x 16 column of zones through the segment's planes; two CTAs share an SM, so that one
+// of them computes while the other waits at a barrier or for data.  Thread (i,j) of the 256 zone threads owns the
+// zones (i,j,k) of every block of the segment (a block's top halo is the next block's first planes, already in the ring):
 //   * every plane of the stage input arrives as ONE 5-D TMA box {16,16,1,1,5} of U[v][b][k][j][i] in a ring of r + 3
 //     shared-memory slots, a tick ahead of its use, and stays there until the zones of that plane are combined
 //     (the combine needs the stage input again: it is U0 in the first stage, X in the later ones -- no second
@@ -18,11 +19,13 @@
 //     each face's flux overwriting, in place, the plus-side state it was computed from, and the primitives of the
 //     NEXT plane written (nobody reads them in that phase); (C) fluxes visible -> flux divergence and RK
 //     combination, which runs on into the next plane's reconstruction without a barrier;
-//   * a ninth "edge" warp supplies what a 16-wide row lacks: the halo cells of the plane -- TMA boxes
-//     {2|4,16,1,1,5} and {16,R,1,1,5} taken straight from the neighbour blocks' interiors through the
-//     neighbour table (or from this block's own edge at an outflow boundary; no guard cell in HBM is read or
-//     written) --, the plus-side state of cell -1 and the flux of the 17th face of every row and column.  Its
-//     lane 0 is the TMA producer.
+//   * two more warps supply what a 16-wide row lacks.  The "edge" warp reconstructs cell -1 (its plus-side state) and
+//     cell 16 of every row and column and solves their 17th face.  The "producer" warp issues every TMA operation
+//     (lane 0) and converts the halo cells of the plane -- TMA boxes {2|4,16,1,1,5} and {16,R,1,1,5} taken straight
+//     from the neighbour blocks' interiors through the neighbour table (or from this block's own edge cells at an
+//     outflow boundary or, mirrored and with the normal momentum negated, at a reflecting wall; no guard cell in HBM
+//     is read or written).  They are two warps because the per-plane dependent chain of one warp doing both was as
+//     long as a zone warp's and delayed the CTA barriers.
 // In the last stage of fx_hydro_step (DTOUT) each finished zone also contributes (|u_d| + c)/dx_d to a running
 // maximum, reduced per warp, per CTA and with one atomicMax per CTA: the CFL step of the advanced state costs no pass.
 // HBM traffic per zone: one read of the stage input (+ U0 in later stages), one write, plus halos.
@@ -45,7 +48,7 @@ template <int RECON> struct Rc {
   static constexpr int BW = (R + 1) & ~1;                            // x-halo box width: TMA rows are multiples of 16 B
   static constexpr int NRING = r + 3;  // a stage-input plane stays in shared memory from its conversion (tick z - r) to the
                                        // combination of its zones (until barrier B of tick z + 2) while the next one loads
-  static constexpr int NREG = (RECON == FX_RECON_PLM_MINMOD) ? 96 : 168;  // registers per thread for 2 / 1 CTAs per SM: the register file is 16384 per SM sub-partition, and 18 / 9 warps put 5 / 3 on one of them
+  static constexpr int NREG = (RECON == FX_RECON_PLM_MINMOD) ? 96 : 168;  // registers per thread for 2 / 1 CTAs per SM: the register file is 16384 per SM sub-partition, and 20 / 10 warps put 5 / 3 on one of them
 };
 
 template <int RECON> struct alignas(128) Smem {
