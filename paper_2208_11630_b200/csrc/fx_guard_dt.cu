@@ -124,39 +124,67 @@ __global__ void __launch_bounds__(256) fx_k_compute_dt(FxParams P, const double 
   const unsigned per_block = nx * ny * (unsigned)P.n[2];
   double rate = 0.0;  // max of (|u_d| + c) / dx_d
   unsigned hit = 0;
+  // 16-byte loads need every zone pair (i even) on a 16-byte boundary: even nx, guard depth and strides, aligned base
+  const bool pairs = (nx % 2 == 0) && (P.gd[0] % 2 == 0) && (P.S_j % 2 == 0) && (P.S_v % 2 == 0) &&
+                     ((reinterpret_cast<unsigned long long>(U) & 15ull) == 0);
   for (long long b = blockIdx.x; b < P.nblocks; b += gridDim.x) {
     double idx[3];
 #pragma unroll
     for (int d = 0; d < 3; ++d) idx[d] = P.active[d] ? 1.0 / __ldg(&dx[b * 3 + d]) : 0.0;
     const double *Ub = U + b * P.S_b;
-    for (unsigned r0 = threadIdx.x; r0 < per_block; r0 += 4 * 256) {
-      double u[4][5];
-      bool on[4];
+    auto zone_rate = [&](double u0, double u1, double u2, double u3, double u4, bool live) {
+      double W[5];
+      double ir;
+      fx_c2p_v2(P, u0, u1, u2, u3, u4, W, &ir);
+      const double cs = fx_sqrt3(P.gamma * W[4] * ir);
+      double m = 0.0;
 #pragma unroll
-      for (int q = 0; q < 4; ++q) {
-        const unsigned r = r0 + q * 256;
-        on[q] = r < per_block;
-        const unsigned rr = on[q] ? r : r0;
-        const unsigned i = rr % nx, t = rr / nx, j = t % ny, k = t / ny;
-        const long long c = (long long)(k + P.gd[2]) * P.S_k + (long long)(j + P.gd[1]) * P.S_j + (i + P.gd[0]);
-#pragma unroll
-        for (int v = 0; v < 5; ++v) u[q][v] = Ub[v * P.S_v + c];
+      for (int d = 0; d < 3; ++d) m = fx_max_sel((fabs(W[1 + d]) + cs) * idx[d], m);  // (a > b ? a : b: a NaN candidate loses)
+      // a NaN anywhere reaches cs or a velocity; the maxima drop it, so test the sum
+      const double chk = (fabs(W[1]) + fabs(W[2])) + (fabs(W[3]) + cs);
+      if (live) {
+        if (fx_hi_nonfinite(__double2hiint(chk)) || !(cs > 0.0)) hit |= FX_STATUS_NONFINITE;
+        rate = fx_max_sel(m, rate);
       }
+    };
+    if (pairs) {
+      // two x-adjacent zones per 16-byte load, two such pairs in flight per thread
+      const unsigned hx = nx / 2, per_half = per_block / 2;
+      for (unsigned r0 = threadIdx.x; r0 < per_half; r0 += 2 * 256) {
+        double2 u[2][5];
+        bool on[2];
 #pragma unroll
-      for (int q = 0; q < 4; ++q) {
-        double W[5];
-        double ir;
-        fx_c2p_v2(P, u[q][0], u[q][1], u[q][2], u[q][3], u[q][4], W, &ir);
-        const double cs = fx_sqrt3(P.gamma * W[4] * ir);
-        double m = 0.0;
+        for (int q = 0; q < 2; ++q) {
+          const unsigned r = r0 + q * 256;
+          on[q] = r < per_half;
+          const unsigned rr = on[q] ? r : r0;
+          const unsigned i = 2 * (rr % hx), t = rr / hx, j = t % ny, k = t / ny;
+          const long long c = (long long)(k + P.gd[2]) * P.S_k + (long long)(j + P.gd[1]) * P.S_j + (i + P.gd[0]);
 #pragma unroll
-        for (int d = 0; d < 3; ++d) m = fmax(m, (fabs(W[1 + d]) + cs) * idx[d]);
-        // a NaN anywhere reaches cs or a velocity; fmax would drop it, so test the sum
-        const double chk = (fabs(W[1]) + fabs(W[2])) + (fabs(W[3]) + cs);
-        if (on[q]) {
-          if (fx_hi_nonfinite(__double2hiint(chk)) || !(cs > 0.0)) hit |= FX_STATUS_NONFINITE;
-          rate = fmax(rate, m);
+          for (int v = 0; v < 5; ++v) u[q][v] = *reinterpret_cast<const double2 *>(Ub + v * P.S_v + c);
         }
+#pragma unroll
+        for (int q = 0; q < 2; ++q) {
+          zone_rate(u[q][0].x, u[q][1].x, u[q][2].x, u[q][3].x, u[q][4].x, on[q]);
+          zone_rate(u[q][0].y, u[q][1].y, u[q][2].y, u[q][3].y, u[q][4].y, on[q]);
+        }
+      }
+    } else {
+      for (unsigned r0 = threadIdx.x; r0 < per_block; r0 += 4 * 256) {
+        double u[4][5];
+        bool on[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+          const unsigned r = r0 + q * 256;
+          on[q] = r < per_block;
+          const unsigned rr = on[q] ? r : r0;
+          const unsigned i = rr % nx, t = rr / nx, j = t % ny, k = t / ny;
+          const long long c = (long long)(k + P.gd[2]) * P.S_k + (long long)(j + P.gd[1]) * P.S_j + (i + P.gd[0]);
+#pragma unroll
+          for (int v = 0; v < 5; ++v) u[q][v] = Ub[v * P.S_v + c];
+        }
+#pragma unroll
+        for (int q = 0; q < 4; ++q) zone_rate(u[q][0], u[q][1], u[q][2], u[q][3], u[q][4], on[q]);
       }
     }
   }

@@ -430,8 +430,10 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
           // (a non-finite result reaches the pressure or the density: the conversion's own test stands in for hmax)
           hit |= fx_c2p_v2(P, res5[0], res5[1], res5[2], res5[3], res5[4], w, &ir) & FX_STATUS_NONFINITE;
           const double cs = fx_sqrt3(P.gamma * w[4] * ir);
-          // (compare-selects: a NaN rate loses every comparison, and the state it came from is already flagged)
-          rate = fx_max_sel(rate, fx_max_sel((fabs(w[1]) + cs) * S.idx[0], fx_max_sel((fabs(w[2]) + cs) * S.idx[1], (fabs(w[3]) + cs) * S.idx[2])));
+          // (compare-selects a > b ? a : b with the running value second: a NaN candidate loses, and the state it came
+          // from is already flagged)
+          const double r01 = fx_max_sel((fabs(w[1]) + cs) * S.idx[0], (fabs(w[2]) + cs) * S.idx[1]);
+          rate = fx_max_sel(fx_max_sel((fabs(w[3]) + cs) * S.idx[2], r01), rate);
         }
         fence_async_smem();  // the TMA store reads Out through the async proxy
       }
