@@ -64,9 +64,48 @@ static void fx_block_grid(long long nblocks, long long per_block_threads, dim3 &
   grid = dim3(gx, gy, gz ? gz : 1);
 }
 
+// The same with one thread per PAIR of x-adjacent padded zones (i even) and 16-byte accesses.  With nx, the x guard
+// depth and the strides even a pair lies wholly in the interior or wholly in one guard region and takes the same hops,
+// so its two sources are adjacent unless the x hop clamps (outflow) or mirrors (wall): those pairs go zone by zone.
+__global__ void __launch_bounds__(256) fx_k_fill_guardcells_pairs(FxParams P, double *__restrict__ U) {
+  const long long b = blockIdx.y + (long long)blockIdx.z * gridDim.y;
+  if (b >= P.nblocks) return;
+  const int zp = blockIdx.x * blockDim.x + threadIdx.x;
+  if (2LL * zp >= P.S_b) return;
+  const int hp = P.np[0] / 2;
+  const int i = 2 * (zp % hp), j = (zp / hp) % P.np[1], k = zp / (hp * P.np[1]);
+  const bool interior = i >= P.gd[0] && i < P.gd[0] + P.n[0] && j >= P.gd[1] && j < P.gd[1] + P.n[1] &&
+                        k >= P.gd[2] && k < P.gd[2] + P.n[2];
+  if (interior) return;
+  unsigned f0, f1;
+  const long long s0 = fx_guard_source(P, b, i, j, k, f0), s1 = fx_guard_source(P, b, i + 1, j, k, f1);
+  const long long t = b * P.S_b + (long long)k * P.S_k + (long long)j * P.S_j + i;
+  if (s1 == s0 + 1 && f0 == f1 && (s0 & 1) == 0) {
+#pragma unroll
+    for (int v = 0; v < 5; ++v) {
+      double2 x = *reinterpret_cast<const double2 *>(U + v * P.S_v + s0);
+      if (v >= 1 && v <= 3 && ((f0 >> (v - 1)) & 1u)) { x.x = -x.x; x.y = -x.y; }
+      *reinterpret_cast<double2 *>(U + v * P.S_v + t) = x;
+    }
+  } else {
+#pragma unroll
+    for (int v = 0; v < 5; ++v) {
+      const double x0 = U[v * P.S_v + s0], x1 = U[v * P.S_v + s1];
+      const bool n0 = v >= 1 && v <= 3 && ((f0 >> (v - 1)) & 1u), n1 = v >= 1 && v <= 3 && ((f1 >> (v - 1)) & 1u);
+      *reinterpret_cast<double2 *>(U + v * P.S_v + t) = make_double2(n0 ? -x0 : x0, n1 ? -x1 : x1);
+    }
+  }
+}
+
 int fx_launch_fill_guardcells(const FxParams &P, double *U, cudaStream_t st) {
   if (P.nblocks == 0) return FX_OK;
   dim3 grid;
+  if (P.active[0] && P.n[0] % 2 == 0 && P.gd[0] % 2 == 0 && P.S_v % 2 == 0 && ((uintptr_t)U & 15) == 0) {
+    fx_block_grid(P.nblocks, P.S_b / 2, grid);
+    fx_k_fill_guardcells_pairs<<<grid, 256, 0, st>>>(P, U);
+    FX_LAUNCH_CHECK("fill_guardcells");
+    return FX_OK;
+  }
   fx_block_grid(P.nblocks, P.S_b, grid);
   fx_k_fill_guardcells<<<grid, 256, 0, st>>>(P, U);
   FX_LAUNCH_CHECK("fill_guardcells");
