@@ -129,8 +129,11 @@ class HydroPlan:
         self._dt = None
 
     def __del__(self):
-        if getattr(self, "_h", None) is not None and self._h.value:
-            lib().fx_hydro_plan_destroy(self._h)
+        if getattr(self, "_h", None) is not None and self._h.value and _lib is not None:
+            try:  # at interpreter shutdown module globals may already be gone
+                _lib.fx_hydro_plan_destroy(self._h)
+            except Exception:
+                pass
             self._h = C.c_void_p()
 
     def _read_layout(self):
