@@ -378,6 +378,37 @@ def test_x_guard_depth_8_layout(recon, rk, bc, path):
     assert np.array_equal(Ud.cpu().numpy(), V[:, :, 4:-4, 4:-4, :])
 
 
+@pytest.mark.parametrize("number,nb", [(2, None), (5, (2, 2, 2))])
+def test_step_is_capturable_in_a_cuda_graph(number, nb):
+    """fx_hydro_step only enqueues work on the caller's stream (tensor maps travel as kernel parameters, dt stays on the
+    device), so a loop of steps can be captured once and replayed: same bits as the eager loop, on the generic path
+    (5 launches per step: launch-bound on small problems) and on the fused one."""
+    cfg, oplan, gplan, Uh, dx = setup(number, nb)
+    dxd = torch.from_numpy(dx).cuda()
+    A, B = Uh.cuda(), Uh.cuda()
+    dta = gplan.fx_hydro_compute_dt(A, dxd, cfg.cfl).clone()
+    dtb = dta.clone()
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(s):
+        gplan.fx_hydro_step(A, dxd, cfg.cfl, dta, stream=s)  # warm-up outside the capture (first-launch set-up)
+        s.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            for _ in range(4):
+                gplan.fx_hydro_step(A, dxd, cfg.cfl, dta, stream=torch.cuda.current_stream())
+    torch.cuda.synchronize()
+    g.replay()
+    g.replay()
+    torch.cuda.synchronize()
+    for _ in range(1 + 8):
+        gplan.fx_hydro_step(B, dxd, cfg.cfl, dtb)
+    torch.cuda.synchronize()
+    assert torch.equal(gplan.interior(A), gplan.interior(B)) and torch.equal(dta, dtb)
+    fg, _ = gplan.fx_hydro_status()
+    assert fg == 0
+
+
 @pytest.mark.parametrize("path", [None, 1])
 def test_status_flags_floors_and_nonfinite(path):
     """A7/A27: primitive floors and non-finite states raise the same status bits as in the oracle, the floored step
