@@ -223,10 +223,10 @@ def run_ours(args, rank, world, local_rank):
     cfg, plan, U, dx, coords = build_workload(args, device)
     stages = cfg.rk_order
     zones = cfg.interior_zones
-    fused = plan.path >= 1
+    fused = plan.path == 1
     # fused path: one launch per RK stage, the CFL reduction (a7) rides in the last one; generic path: guard fill +
     # stage kernel per stage, then the reduction pass
-    launches_per_step = stages if fused else 2 * stages + 1
+    launches_per_step = stages if fused else (stages + 1 if plan.path == 2 else 2 * stages + 1)
     dt = plan.fx_hydro_compute_dt(U, dx, cfg.cfl).clone()  # the first step's dt; stays on the device from here on
 
     def step():
@@ -292,7 +292,7 @@ def run_ours(args, rank, world, local_rank):
                                    f"{'WENO5' if cfg.recon else 'PLM-minmod'}+{'HLLC' if cfg.riemann else 'HLLE'}, SSP-RK{stages}",
                        "interior_zones": zones, "state_bytes": plan.bytes_per_state, "block_order": args.order,
                        "layout": f"x guard depth {plan.gd[0]} (row pitch {plan.S_j * 8} B), y/z guard depth {plan.gd[1]}/{plan.gd[2]}",
-                       "path": {0: "generic", 1: "fused (TMA)"}[plan.path], "l2": "inputs (state) larger than L2; no flush needed",
+                       "path": {0: "generic", 1: "fused (TMA)", 2: "tile (shared-memory block)"}[plan.path], "l2": "inputs (state) larger than L2; no flush needed",
                        "multi_gpu": "replicas only" if world > 1 else "single"},
             "clocks": clocks, "gpu_launches": launches_per_step * args.steps, "roofline": roofline,
             "status_flags": flags}

@@ -48,7 +48,10 @@ enum {
   FX_OPT_P_FLOOR = 1,   /* primitive pressure floor, default 1e-12 [A7] */
   FX_OPT_WENO_EPS = 2,  /* WENO5-JS epsilon, default 1e-6 [A5] */
   FX_OPT_WAVESPEED = 3, /* 0 = Einfeldt (default), 1 = Davis [A8] */
-  FX_OPT_PATH = 4,      /* 0 = auto (fused TMA stage kernel when the block shape allows), 1 = generic */
+  FX_OPT_PATH = 4,      /* 0 = auto: the fused TMA stage kernel for 16 x 16 x nz blocks, else the shared-memory tile kernel
+                           when the padded block fits a CTA's shared memory (8^3 blocks, 2-D, 1-D), else the generic
+                           zone kernel; 1 = generic; 2 = tile kernel where it fits, else generic.
+                           fx_hydro_plan_path reports the choice (1 fused, 2 tile, 0 generic). */
   FX_OPT_ZCHAIN = 5,    /* fused path: longest chain of z-neighbour blocks one CTA marches through, 1..8; 0 (default) =
                            chosen from the number of blocks and of SMs so that the launch still fills the GPU.
                            Set before fx_hydro_plan_set_topology.  Results do not depend on it (bit for bit). */
@@ -197,7 +200,8 @@ int fx_debug_compute_fluxes(fx_hydro_plan *plan, const double *U_dev, int dir, d
 
 /* Which stage kernel fx_hydro_advance will use for this plan: 0 generic (guard fill + zone kernel),
  * 1 fused and TMA-fed (16 x 16 x nz blocks: halos gathered from neighbour interiors inside the stage kernel,
- * every plane moved by TMA). */
+ * every plane moved by TMA), 2 shared-memory tile kernel (one CTA per block whose padded zones fit its shared
+ * memory: halos gathered through the neighbour table, each zone converted once, one Riemann solve per face). */
 int fx_hydro_plan_path(const fx_hydro_plan *plan);
 
 /* Measurement aid: when enabled, fx_hydro_advance brackets every stage-kernel launch (the dominant

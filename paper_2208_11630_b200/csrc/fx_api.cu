@@ -164,7 +164,7 @@ extern "C" int fx_hydro_plan_set_option(fx_hydro_plan *plan, int key, double val
     plan->zchain = (int)value;
     return FX_OK;
   case FX_OPT_PATH:
-    if (value != 0.0 && value != 1.0) return fx_fail(FX_ERR_INVALID_ARG, "set_option: path must be 0 or 1");
+    if (value != 0.0 && value != 1.0 && value != 2.0) return fx_fail(FX_ERR_INVALID_ARG, "set_option: path must be 0, 1 or 2");
     plan->path_option = (int)value;
     return FX_OK;
   default: return fx_fail(FX_ERR_INVALID_ARG, "set_option: unknown key %d", key);
@@ -173,7 +173,9 @@ extern "C" int fx_hydro_plan_set_option(fx_hydro_plan *plan, int key, double val
 
 extern "C" int fx_hydro_plan_path(const fx_hydro_plan *plan) {
   if (!plan) return fx_fail(FX_ERR_INVALID_ARG, "plan_path: null plan");
-  return (plan->path_option == 0 && fx_stage_tma_supported(plan->P)) ? 1 : 0;
+  if (plan->path_option == 0 && fx_stage_tma_supported(plan->P)) return 1;
+  if (plan->path_option != 1 && fx_stage_tile_supported(plan->P)) return 2;
+  return 0;
 }
 
 static size_t fx_state_bytes_aligned(const fx_hydro_plan *plan) {

@@ -2,31 +2,6 @@
 #include "fx_physics.cuh"
 
 // ------------------------------------------------------------------ a1 guard fill
-// Source of padded zone (i,j,k) of block b: hops z, y, x through the neighbour table [O1, A14].  Bit d of flip is set
-// when the zone lies behind a reflecting wall of dimension d [B9]: its image carries the negated d-momentum.
-__device__ __forceinline__ long long fx_guard_source(const FxParams &P, long long b, int i, int j, int k, unsigned &flip) {
-  flip = 0;
-  int c[3] = {i, j, k};
-  long long bs = b;
-#pragma unroll
-  for (int d = 2; d >= 0; --d) {
-    if (!P.active[d]) continue;
-    const int lo = P.gd[d], hi = P.gd[d] + P.n[d];
-    if (c[d] < lo) {
-      int nb = __ldg(&P.neigh[bs * 6 + 2 * d]);
-      if (nb >= 0) { bs = nb; c[d] += P.n[d]; }
-      else if (nb == FX_BC_REFLECT) { c[d] = 2 * lo - 1 - c[d]; flip |= 1u << d; }
-      else c[d] = lo;
-    } else if (c[d] >= hi) {
-      int nb = __ldg(&P.neigh[bs * 6 + 2 * d + 1]);
-      if (nb >= 0) { bs = nb; c[d] -= P.n[d]; }
-      else if (nb == FX_BC_REFLECT) { c[d] = 2 * hi - 1 - c[d]; flip |= 1u << d; }
-      else c[d] = hi - 1;
-    }
-  }
-  return bs * P.S_b + c[2] * P.S_k + c[1] * P.S_j + c[0];
-}
-
 // One thread per padded zone of one block (blockIdx.y, folded with gridDim.z for > 65535 blocks).
 __global__ void __launch_bounds__(256) fx_k_fill_guardcells(FxParams P, double *__restrict__ U) {
   const long long b = blockIdx.y + (long long)blockIdx.z * gridDim.y;

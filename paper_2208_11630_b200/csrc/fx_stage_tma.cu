@@ -111,73 +111,6 @@ __device__ __forceinline__ void tma_wait_read() { asm volatile("cp.async.bulk.wa
 __device__ __forceinline__ void tma_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
-// a3: minus/plus face states of one cell from its stencil s[0..2r] (centre s[r]).
-template <int RECON>
-__device__ __forceinline__ void recon_cell(const double *s, double eps, double &qm, double &qp) {
-  if (RECON == FX_RECON_PLM_MINMOD) {
-    fx_plm(s[0], s[1], s[2], qm, qp);
-  } else {
-    // WENO5-JS, both faces of the cell share the smoothness indicators (beta_0 <-> beta_2 under mirroring)
-    const double a = s[0], b = s[1], c = s[2], d = s[3], e = s[4];
-    // Every product and sum is written out (fma / _rn intrinsics): the compiler may not contract these expressions one
-    // way in one inlined copy and another way in the next, so a face value does not depend on which part of the kernel
-    // (prologue or z loop) evaluated it, and the result is bit for bit the same whatever the z-chain length.
-    const double t0 = fma(-2.0, b, __dadd_rn(a, c)), u0 = fma(3.0, c, fma(-4.0, b, a));
-    const double t1 = fma(-2.0, c, __dadd_rn(b, d)), u1 = __dsub_rn(b, d);
-    const double t2 = fma(-2.0, d, __dadd_rn(c, e)), u2 = fma(3.0, c, fma(-4.0, d, e));
-    const double b0 = fma(13.0 / 12.0, __dmul_rn(t0, t0), fma(0.25, __dmul_rn(u0, u0), eps));
-    const double b1 = fma(13.0 / 12.0, __dmul_rn(t1, t1), fma(0.25, __dmul_rn(u1, u1), eps));
-    const double b2 = fma(13.0 / 12.0, __dmul_rn(t2, t2), fma(0.25, __dmul_rn(u2, u2), eps));
-    const double q0 = __dmul_rn(b1, b2), q1 = __dmul_rn(b0, b2), q2 = __dmul_rn(b0, b1);
-    // ~ 1/b0^2, 1/b1^2, 1/b2^2 up to a common factor
-    const double s0 = __dmul_rn(q0, q0), s1 = __dmul_rn(q1, q1), s2 = __dmul_rn(q2, q2);
-    const double sixth = 1.0 / 6.0;
-    {  // plus face: candidates (times 6) from (a,b,c), (b,c,d), (c,d,e); weights 0.1, 0.6, 0.3
-      const double p0 = fma(2.0, a, fma(-7.0, b, __dmul_rn(11.0, c))), p1 = fma(2.0, d, fma(5.0, c, -b)),
-                   p2 = fma(2.0, c, fma(5.0, d, -e));
-      const double a0 = __dmul_rn(0.1, s0), a1 = __dmul_rn(0.6, s1), a2 = __dmul_rn(0.3, s2);
-      const double num = fma(a0, p0, fma(a1, p1, __dmul_rn(a2, p2)));
-      // the weights' sum is positive and far from the subnormal range
-      qp = __dmul_rn(num, __dmul_rn(sixth, fx_rcp3(__dadd_rn(__dadd_rn(a0, a1), a2))));
-    }
-    {  // minus face: mirrored stencil (e,d,c,b,a)
-      const double p0 = fma(2.0, e, fma(-7.0, d, __dmul_rn(11.0, c))), p1 = fma(2.0, b, fma(5.0, c, -d)),
-                   p2 = fma(2.0, c, fma(5.0, b, -a));
-      const double a0 = __dmul_rn(0.1, s2), a1 = __dmul_rn(0.6, s1), a2 = __dmul_rn(0.3, s0);
-      const double num = fma(a0, p0, fma(a1, p1, __dmul_rn(a2, p2)));
-      qm = __dmul_rn(num, __dmul_rn(sixth, fx_rcp3(__dadd_rn(__dadd_rn(a0, a1), a2))));
-    }
-  }
-}
-
-// Reconstruct all five primitives of one cell; st[m][v] is cell m of the stencil.  WENO positivity
-// fallback per side [A6]: a face state with rho <= 0 or p <= 0 reverts to the cell's own values.
-template <int RECON>
-__device__ __forceinline__ unsigned recon_cell5(const double (*st)[5], double eps, double qm[5], double qp[5]) {
-  constexpr int r = Rc<RECON>::r;
-#pragma unroll
-  for (int v = 0; v < 5; ++v) {
-    double s[2 * r + 1];
-#pragma unroll
-    for (int m = 0; m < 2 * r + 1; ++m) s[m] = st[m][v];
-    recon_cell<RECON>(s, eps, qm[v], qp[v]);
-  }
-  unsigned hit = 0;
-  if (RECON == FX_RECON_WENO5) {
-    if (!(qm[0] > 0.0) || !(qm[4] > 0.0)) {
-#pragma unroll
-      for (int v = 0; v < 5; ++v) qm[v] = st[r][v];
-      hit = FX_STATUS_WENO_FALLBACK;
-    }
-    if (!(qp[0] > 0.0) || !(qp[4] > 0.0)) {
-#pragma unroll
-      for (int v = 0; v < 5; ++v) qp[v] = st[r][v];
-      hit = FX_STATUS_WENO_FALLBACK;
-    }
-  }
-  return hit;
-}
-
 // Riemann flux for direction D (compile-time) from un-rotated primitive states; flux returned in the
 // un-rotated variable order (rho, mx, my, mz, E).
 template <int RIEMANN, int WS, int D>
@@ -314,8 +247,8 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
         if (m >= R && m - R < nz) hit |= h;  // a zone's floor hits are counted by its owner only
       }
       double qm[5], qpm1[5];
-      hit |= recon_cell5<RECON>(&w[0], P.weno_eps, qm, qpm1);  // cell -1
-      hit |= recon_cell5<RECON>(&w[1], P.weno_eps, qm, qpz);   // cell 0
+      hit |= fx_recon_cell5<RECON>(&w[0], P.weno_eps, qm, qpm1);  // cell -1
+      hit |= fx_recon_cell5<RECON>(&w[1], P.weno_eps, qm, qpz);   // cell 0
       flux_dir<RIEMANN, WS, 2>(P, qpm1, qm, Fz);
 #pragma unroll
       for (int m = 0; m < 2 * r; ++m)
@@ -337,7 +270,7 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
         for (int m = 0; m < W; ++m)
 #pragma unroll
           for (int v = 0; v < 5; ++v) st[m][v] = (m == r) ? q[r - 1][v] : S.P[v][j + R][i + R + m - r];
-        hit |= recon_cell5<RECON>(st, P.weno_eps, qmx, qp);
+        hit |= fx_recon_cell5<RECON>(st, P.weno_eps, qmx, qp);
 #pragma unroll
         for (int v = 0; v < 5; ++v) S.Lx[v][j][i + 1] = qp[v];
       }
@@ -347,7 +280,7 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
         for (int m = 0; m < W; ++m)
 #pragma unroll
           for (int v = 0; v < 5; ++v) st[m][v] = (m == r) ? q[r - 1][v] : S.P[v][j + R + m - r][i + R];
-        hit |= recon_cell5<RECON>(st, P.weno_eps, qmy, qp);
+        hit |= fx_recon_cell5<RECON>(st, P.weno_eps, qmy, qp);
 #pragma unroll
         for (int v = 0; v < 5; ++v) S.Ly[v][j + 1][i] = qp[v];
       }
@@ -365,7 +298,7 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
       double Fz_new[5];
       {
         double qmz[5], qpz_new[5];
-        hit |= recon_cell5<RECON>(q, P.weno_eps, qmz, qpz_new);
+        hit |= fx_recon_cell5<RECON>(q, P.weno_eps, qmz, qpz_new);
         flux_dir<RIEMANN, WS, 2>(P, qpz, qmz, Fz_new);
 #pragma unroll
         for (int v = 0; v < 5; ++v) qpz[v] = qpz_new[v];
@@ -472,7 +405,7 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
         for (int mm = 0; mm < W; ++mm)
 #pragma unroll
           for (int v = 0; v < 5; ++v) st[mm][v] = Pf[v * NP * NPS + mm * pd + (m + R) * pt];
-        hit |= recon_cell5<RECON>(st, P.weno_eps, qm, qp);
+        hit |= fx_recon_cell5<RECON>(st, P.weno_eps, qm, qp);
 #pragma unroll
         for (int v = 0; v < 5; ++v) Lf[v * LV + 0 * ld + m * lt] = qp[v];
         // cell 16: padded positions 16+R-r .. 16+R+r
@@ -480,7 +413,7 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
         for (int mm = 0; mm < W; ++mm)
 #pragma unroll
           for (int v = 0; v < 5; ++v) st[mm][v] = Pf[v * NP * NPS + (NX + R - r + mm) * pd + (m + R) * pt];
-        hit |= recon_cell5<RECON>(st, P.weno_eps, qm16, qp);
+        hit |= fx_recon_cell5<RECON>(st, P.weno_eps, qm16, qp);
       }
       cta_sync();  // B
       {

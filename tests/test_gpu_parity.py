@@ -434,6 +434,57 @@ def test_repeated_runs_are_bitwise_identical(recon, rk, bc):
     assert torch.isfinite(ref[0]).all()
 
 
+@pytest.mark.parametrize("dims,nb,nguard,recon,rk,bc,grav", [
+    ((8, 8, 8), (3, 2, 2), 4, 0, 2, "periodic", False), ((8, 8, 8), (2, 2, 3), 4, 1, 3, "reflect", True),
+    ((8, 8, 8), (2, 3, 2), 2, 0, 3, "outflow", False), ((8, 6, 5), (2, 2, 2), 3, 1, 2, "periodic", False),
+    ((32, 32, 1), (2, 2, 1), 4, 0, 2, "reflect", True), ((256, 1, 1), (2, 1, 1), 4, 1, 3, "outflow", False)])
+def test_tile_kernel_small_blocks(dims, nb, nguard, recon, rk, bc, grav):
+    """The shared-memory tile kernel (path 2: blocks whose padded zones fit a CTA's shared memory -- 8^3 blocks, 2-D and
+    1-D blocks): parity with the oracle after 1 and 5 steps, the same status flags, agreement with the generic kernel to
+    rounding, walls, gravity, odd guard depths and non-cubic blocks included."""
+    from paper_2208_11630_b200 import binding as fx
+    cfg = inputs.config(5, nb=nb)
+    cfg.block_dims, cfg.nguard = dims, nguard
+    oplan, neigh, coords = oracle_plan_for(cfg, bc=bc, recon=recon, rk=rk)
+    gplan, _, _ = gpu_plan_for(cfg, bc=bc, recon=recon, rk=rk)
+    gen, _, _ = gpu_plan_for(cfg, bc=bc, recon=recon, rk=rk, path=1)
+    assert gplan.path == 2 and gen.path == 0
+    g = (0.7, -1.1 if dims[1] > 1 else 0.0, 0.4 if dims[2] > 1 else 0.0)
+    if grav:
+        for d in range(3):
+            oplan.set_option(fxo.OPT_GRAVITY_X + d, g[d])
+            gplan.fx_hydro_plan_set_option(fx.OPT_GRAVITY_X + d, g[d])
+            gen.fx_hydro_plan_set_option(fx.OPT_GRAVITY_X + d, g[d])
+    nblk = nb[0] * nb[1] * nb[2]
+    rng = np.random.default_rng(77)
+    shape = (nblk, dims[2], dims[1], dims[0])
+    rho = 1.0 + 0.3 * rng.random(shape)
+    vel = 0.4 * rng.standard_normal((3,) + shape)
+    for d in (1, 2):
+        if dims[d] == 1:
+            vel[d] = 0.0
+    pr = 1.0 + 0.3 * rng.random(shape)
+    Ui = np.stack([rho, rho * vel[0], rho * vel[1], rho * vel[2], pr / (cfg.gamma - 1) + 0.5 * rho * (vel ** 2).sum(0)])
+    Uh = inputs.embed(cfg, torch.from_numpy(Ui))
+    dx = np.full((nblk, 3), 1.0 / 64)
+    Uo, Ud, Ug, dxd = Uh.numpy().copy(), Uh.cuda(), Uh.cuda(), torch.from_numpy(dx).cuda()
+    for step in range(5):
+        dt = oplan.compute_dt(Uo, dx, 0.3)
+        oplan.advance(Uo, dx, dt)
+        gplan.fx_hydro_advance(Ud, dxd, dt)
+        gen.fx_hydro_advance(Ug, dxd, dt)
+        err = rel_err(cfg, gplan.interior(Ud).cpu().numpy(), oplan.interior(Uo))
+        assert err <= (1e-12 if step == 0 else 1e-10), (step, err)
+    assert rel_err(cfg, gplan.interior(Ud).cpu().numpy(), gen.interior(Ug).cpu().numpy()) <= 1e-11
+    assert oplan.status()[0] == gplan.fx_hydro_status()[0]
+    # the step call (dt of the advanced state by the reduction pass) on the tile path
+    dtd = gplan.fx_hydro_compute_dt(Ud, dxd, 0.3).clone()
+    gplan.fx_hydro_step(Ud, dxd, 0.3, dtd)
+    dto = oplan.compute_dt(Uo, dx, 0.3)
+    oplan.advance(Uo, dx, dto)
+    assert abs(float(dtd.item()) - oplan.compute_dt(Uo, dx, 0.3)) <= 1e-12 * dto
+
+
 @pytest.mark.parametrize("path", [None, 1])
 def test_status_flags_floors_and_nonfinite(path):
     """A7/A27: primitive floors and non-finite states raise the same status bits as in the oracle, the floored step
