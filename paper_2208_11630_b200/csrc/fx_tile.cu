@@ -17,7 +17,6 @@
 
 namespace fxtile {
 
-constexpr int NT = 256;
 
 struct Geo {
   int e[3];          // extents of the primitive tile: n_d + 2R in active dimensions (R = reach of the reconstruction)
@@ -53,7 +52,7 @@ struct Tile {  // what the direction passes need, in registers
 };
 
 // Direction D (compile-time): one Riemann solve per face into Ff, then S += (dt/dx_D)(F+ - F-) for every interior zone.
-template <int RECON, int RIEMANN, int WS, int D>
+template <int RECON, int RIEMANN, int WS, int NT, int D>
 __device__ __forceinline__ unsigned tile_direction(const FxParams &P, const Tile &T, double rd, int tid) {
   constexpr int r = (RECON == FX_RECON_PLM_MINMOD) ? 1 : 2, W5 = 2 * r + 1;
   constexpr int d1 = (D + 1) % 3, d2 = (D + 2) % 3;      // momentum rotation of the face frame (as in the fused kernel)
@@ -111,7 +110,7 @@ __device__ __forceinline__ unsigned tile_direction(const FxParams &P, const Tile
   return hit;
 }
 
-template <int RECON, int RIEMANN, int WS>
+template <int RECON, int RIEMANN, int WS, int NT>
 __global__ void __launch_bounds__(NT) fx_k_stage_tile(const FxParams P, const double *__restrict__ X, const double *U0,
                                                       double *out, const double *__restrict__ dx, double dt,
                                                       const double *__restrict__ dt_dev, double beta, int first,
@@ -160,9 +159,9 @@ __global__ void __launch_bounds__(NT) fx_k_stage_tile(const FxParams P, const do
   __syncthreads();
 
   // ---- 2. per direction (order x, y, z [O5]): one Riemann solve per face, then the divergence
-  if (P.active[0]) hit |= tile_direction<RECON, RIEMANN, WS, 0>(P, T, dt / __ldg(&dx[b * 3 + 0]), tid);
-  if (P.active[1]) hit |= tile_direction<RECON, RIEMANN, WS, 1>(P, T, dt / __ldg(&dx[b * 3 + 1]), tid);
-  if (P.active[2]) hit |= tile_direction<RECON, RIEMANN, WS, 2>(P, T, dt / __ldg(&dx[b * 3 + 2]), tid);
+  if (P.active[0]) hit |= tile_direction<RECON, RIEMANN, WS, NT, 0>(P, T, dt / __ldg(&dx[b * 3 + 0]), tid);
+  if (P.active[1]) hit |= tile_direction<RECON, RIEMANN, WS, NT, 1>(P, T, dt / __ldg(&dx[b * 3 + 1]), tid);
+  if (P.active[2]) hit |= tile_direction<RECON, RIEMANN, WS, NT, 2>(P, T, dt / __ldg(&dx[b * 3 + 2]), tid);
 
   // ---- 3. out = U0 + beta((X - U0) - S), minus S's gravity part [B10]
   for (int e = tid; e < nint; e += NT) {
@@ -191,11 +190,11 @@ __global__ void __launch_bounds__(NT) fx_k_stage_tile(const FxParams P, const do
   if (hit) fx_note(P, hit);
 }
 
-template <int RECON, int RIEMANN, int WS>
-static int launch(const FxParams &P, const double *X, const double *U0, double *out, const double *dx, double dt,
-                  const double *dt_dev, double beta, int first, cudaStream_t st) {
+template <int RECON, int RIEMANN, int WS, int NT>
+static int launch_nt(const FxParams &P, const double *X, const double *U0, double *out, const double *dx, double dt,
+                     const double *dt_dev, double beta, int first, cudaStream_t st) {
   const Geo g = geometry(P);
-  auto kern = fx_k_stage_tile<RECON, RIEMANN, WS>;
+  auto kern = fx_k_stage_tile<RECON, RIEMANN, WS, NT>;
   static bool configured = false;  // per instantiation
   if (!configured) {
     FX_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
@@ -204,6 +203,17 @@ static int launch(const FxParams &P, const double *X, const double *U0, double *
   kern<<<(unsigned)P.nblocks, NT, g.smem, st>>>(P, X, U0, out, dx, dt, dt_dev, beta, first, g.ntile, g.faces_max, g.nint);
   FX_LAUNCH_CHECK("stage_tile");
   return FX_OK;
+}
+
+// Threads per CTA (measured): 256 for blocks of a few hundred zones (8^3 with PLM: two CTAs per SM; 16 x 16 in 2-D),
+// 512 for 1024 zones and more and for WENO5 on 512 (one CTA per SM either way: more warps hide more latency).
+template <int RECON, int RIEMANN, int WS>
+static int launch(const FxParams &P, const double *X, const double *U0, double *out, const double *dx, double dt,
+                  const double *dt_dev, double beta, int first, cudaStream_t st) {
+  const int nint = P.n[0] * P.n[1] * P.n[2];
+  if (nint >= 1024 || (RECON == FX_RECON_WENO5 && nint >= 512))
+    return launch_nt<RECON, RIEMANN, WS, 512>(P, X, U0, out, dx, dt, dt_dev, beta, first, st);
+  return launch_nt<RECON, RIEMANN, WS, 256>(P, X, U0, out, dx, dt, dt_dev, beta, first, st);
 }
 
 }  // namespace fxtile
