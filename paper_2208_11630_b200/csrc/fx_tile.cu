@@ -43,12 +43,25 @@ static Geo geometry(const FxParams &P) {
   return g;
 }
 
+// x / d for 0 <= x < 2^15 and 1 <= d <= 2^10 through a float reciprocal: (x + 0.5) / d is at least 0.5/d away from an
+// integer and the float error is below x 2^-22, so truncation gives the exact quotient (an integer division is ~20
+// instructions, and index arithmetic was a third of this kernel's instructions)
+struct Div {
+  int d;
+  float inv;
+  __host__ __device__ Div() : d(1), inv(1.0f) {}
+  __host__ __device__ explicit Div(int dd) : d(dd), inv(1.0f / (float)dd) {}
+  __device__ __forceinline__ int quot(int x) const { return __float2int_rz(((float)x + 0.5f) * inv); }
+  __device__ __forceinline__ void divmod(int x, int &q, int &rem) const { q = quot(x); rem = x - q * d; }
+};
+
 struct Tile {  // what the direction passes need, in registers
   double *Wp, *Ff, *Sa;
   int ntile, faces_max, nint;
   int e0, e1;        // tile extents in x and y
   int n[3];
   int off[3];        // tile coordinate of interior zone 0 in each dimension (R if active, else 0)
+  Div dn0, dn1;      // divisors n0, n1 (interior decode)
 };
 
 // Direction D (compile-time): one Riemann solve per face into Ff, then S += (dt/dx_D)(F+ - F-) for every interior zone.
@@ -63,10 +76,11 @@ __device__ __forceinline__ unsigned tile_direction(const FxParams &P, const Tile
   // face order: x runs fastest in every direction (for D = 0 that is the face's own coordinate), so that a warp reads
   // W along rows; fs = distance between the two faces of a zone in that order
   const int fs = D == 0 ? 1 : nta;
+  const Div dnf(nf), dnta(nta);
   for (int f = tid; f < nfaces; f += NT) {
-    int fd, ca, cb;
-    if (D == 0) { fd = f % nf; ca = (f / nf) % nta; cb = f / (nf * nta); }
-    else { ca = f % nta; fd = (f / nta) % nf; cb = f / (nta * nf); }
+    int fd, ca, cb, t;
+    if (D == 0) { dnf.divmod(f, t, fd); dnta.divmod(t, cb, ca); }
+    else { dnta.divmod(f, t, ca); dnf.divmod(t, cb, fd); }
     int cc[3];
     cc[D] = T.off[D] + fd;  // the cell on the plus side of the face
     cc[ta] = T.off[ta] + ca;
@@ -98,10 +112,9 @@ __device__ __forceinline__ unsigned tile_direction(const FxParams &P, const Tile
   }
   __syncthreads();
   for (int e = tid; e < T.nint; e += NT) {
-    int ci[3];
-    ci[0] = e % T.n[0];
-    ci[1] = (e / T.n[0]) % T.n[1];
-    ci[2] = e / (T.n[0] * T.n[1]);
+    int ci[3], t;
+    T.dn0.divmod(e, t, ci[0]);
+    T.dn1.divmod(t, ci[2], ci[1]);
     const int f = D == 0 ? ci[0] + nf * (ci[ta] + nta * ci[tb]) : ci[ta] + nta * (ci[D] + nf * ci[tb]);
 #pragma unroll
     for (int v = 0; v < 5; ++v) T.Sa[v * T.nint + e] += rd * (T.Ff[v * T.faces_max + f + fs] - T.Ff[v * T.faces_max + f]);
@@ -110,8 +123,10 @@ __device__ __forceinline__ unsigned tile_direction(const FxParams &P, const Tile
   return hit;
 }
 
-template <int RECON, int RIEMANN, int WS, int NT>
-__global__ void __launch_bounds__(NT) fx_k_stage_tile(const FxParams P, const double *__restrict__ X, const double *U0,
+// GB: zones per thread and gather round (their loads are in flight together; 4 for big tiles, 1 for tiles of a few
+// hundred zones, where the registers are better spent on more resident CTAs)
+template <int RECON, int RIEMANN, int WS, int NT, int GB>
+__global__ void __launch_bounds__(NT, (GB == 1 && NT == 256) ? 4 : 1) fx_k_stage_tile(const FxParams P, const double *__restrict__ X, const double *U0,
                                                       double *out, const double *__restrict__ dx, double dt,
                                                       const double *__restrict__ dt_dev, double beta, int first,
                                                       int ntile, int faces_max, int nint) {
@@ -131,28 +146,43 @@ __global__ void __launch_bounds__(NT) fx_k_stage_tile(const FxParams P, const do
     T.n[0] = P.n[0]; T.n[1] = P.n[1]; T.n[2] = P.n[2];
     T.off[0] = P.active[0] ? R : 0; T.off[1] = P.active[1] ? R : 0; T.off[2] = P.active[2] ? R : 0;
     T.e0 = T.n[0] + 2 * T.off[0]; T.e1 = T.n[1] + 2 * T.off[1]; e2 = T.n[2] + 2 * T.off[2];
+    T.dn0 = Div(T.n[0]); T.dn1 = Div(T.n[1]);
   }
+  const Div de0(T.e0), de1(T.e1);
 
   // ---- 1. gather + cons -> prim, once per zone of the block and of its R-deep face slabs
-  for (int z = tid; z < ntile; z += NT) {
-    const int t0 = z % T.e0, t1 = (z / T.e0) % T.e1, t2 = z / (T.e0 * T.e1);
-    // offsets from the interior box: how many coordinates lie outside it
-    const int outside = (t0 < T.off[0] || t0 >= T.off[0] + T.n[0]) + (t1 < T.off[1] || t1 >= T.off[1] + T.n[1]) +
-                        (t2 < T.off[2] || t2 >= T.off[2] + T.n[2]);
-    if (outside > 1) continue;  // 1-D stencils never look at edge or corner zones
-    unsigned flip;
-    const long long s = fx_guard_source(P, b, t0 - T.off[0] + P.gd[0], t1 - T.off[1] + P.gd[1], t2 - T.off[2] + P.gd[2], flip);
-    double u[5];
+  for (int z0 = tid; z0 < ntile; z0 += GB * NT) {
+    double u[GB][5];
+    int outside[GB];
 #pragma unroll
-    for (int v = 0; v < 5; ++v) u[v] = X[v * P.S_v + s];
-    if (flip & 1u) u[1] = -u[1];
-    if (flip & 2u) u[2] = -u[2];
-    if (flip & 4u) u[3] = -u[3];
-    double w[5];
-    const unsigned h = fx_c2p_v2(P, u[0], u[1], u[2], u[3], u[4], w);
-    if (outside == 0) hit |= h;  // floors and non-finite states are counted where a zone is owned
+    for (int q = 0; q < GB; ++q) {
+      const int z = z0 + q * NT;
+      outside[q] = 3;  // "skip"
+      if (z >= ntile) continue;
+      int t, t0, t1, t2;
+      de0.divmod(z, t, t0);
+      de1.divmod(t, t2, t1);
+      // how many coordinates lie outside the interior box: 1-D stencils never look at edge or corner zones
+      outside[q] = (t0 < T.off[0] || t0 >= T.off[0] + T.n[0]) + (t1 < T.off[1] || t1 >= T.off[1] + T.n[1]) +
+                   (t2 < T.off[2] || t2 >= T.off[2] + T.n[2]);
+      if (outside[q] > 1) continue;
+      unsigned flip;
+      const long long s = fx_guard_source(P, b, t0 - T.off[0] + P.gd[0], t1 - T.off[1] + P.gd[1], t2 - T.off[2] + P.gd[2], flip);
 #pragma unroll
-    for (int v = 0; v < 5; ++v) T.Wp[v * ntile + z] = w[v];
+      for (int v = 0; v < 5; ++v) u[q][v] = X[v * P.S_v + s];
+      if (flip & 1u) u[q][1] = -u[q][1];
+      if (flip & 2u) u[q][2] = -u[q][2];
+      if (flip & 4u) u[q][3] = -u[q][3];
+    }
+#pragma unroll
+    for (int q = 0; q < GB; ++q) {
+      if (outside[q] > 1) continue;
+      double w[5];
+      const unsigned h = fx_c2p_v2(P, u[q][0], u[q][1], u[q][2], u[q][3], u[q][4], w);
+      if (outside[q] == 0) hit |= h;  // floors and non-finite states are counted where a zone is owned
+#pragma unroll
+      for (int v = 0; v < 5; ++v) T.Wp[v * ntile + z0 + q * NT] = w[v];
+    }
   }
   (void)e2;
   for (int e = tid; e < 5 * nint; e += NT) T.Sa[e] = 0.0;
@@ -165,7 +195,9 @@ __global__ void __launch_bounds__(NT) fx_k_stage_tile(const FxParams P, const do
 
   // ---- 3. out = U0 + beta((X - U0) - S), minus S's gravity part [B10]
   for (int e = tid; e < nint; e += NT) {
-    const int c0 = e % T.n[0], c1 = (e / T.n[0]) % T.n[1], c2 = e / (T.n[0] * T.n[1]);
+    int c0, c1, c2, t;
+    T.dn0.divmod(e, t, c0);
+    T.dn1.divmod(t, c2, c1);
     const long long c = b * P.S_b + (long long)(c2 + P.gd[2]) * P.S_k + (long long)(c1 + P.gd[1]) * P.S_j + (c0 + P.gd[0]);
     double S5[5];
 #pragma unroll
@@ -190,11 +222,11 @@ __global__ void __launch_bounds__(NT) fx_k_stage_tile(const FxParams P, const do
   if (hit) fx_note(P, hit);
 }
 
-template <int RECON, int RIEMANN, int WS, int NT>
+template <int RECON, int RIEMANN, int WS, int NT, int GB>
 static int launch_nt(const FxParams &P, const double *X, const double *U0, double *out, const double *dx, double dt,
                      const double *dt_dev, double beta, int first, cudaStream_t st) {
   const Geo g = geometry(P);
-  auto kern = fx_k_stage_tile<RECON, RIEMANN, WS, NT>;
+  auto kern = fx_k_stage_tile<RECON, RIEMANN, WS, NT, GB>;
   static bool configured = false;  // per instantiation
   if (!configured) {
     FX_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
@@ -212,8 +244,9 @@ static int launch(const FxParams &P, const double *X, const double *U0, double *
                   const double *dt_dev, double beta, int first, cudaStream_t st) {
   const int nint = P.n[0] * P.n[1] * P.n[2];
   if (nint >= 1024 || (RECON == FX_RECON_WENO5 && nint >= 512))
-    return launch_nt<RECON, RIEMANN, WS, 512>(P, X, U0, out, dx, dt, dt_dev, beta, first, st);
-  return launch_nt<RECON, RIEMANN, WS, 256>(P, X, U0, out, dx, dt, dt_dev, beta, first, st);
+    return launch_nt<RECON, RIEMANN, WS, 512, 4>(P, X, U0, out, dx, dt, dt_dev, beta, first, st);
+  if (geometry(P).ntile >= 1024) return launch_nt<RECON, RIEMANN, WS, 256, 4>(P, X, U0, out, dx, dt, dt_dev, beta, first, st);
+  return launch_nt<RECON, RIEMANN, WS, 256, 1>(P, X, U0, out, dx, dt, dt_dev, beta, first, st);
 }
 
 }  // namespace fxtile
