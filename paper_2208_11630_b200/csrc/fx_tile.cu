@@ -123,8 +123,7 @@ __device__ __forceinline__ unsigned tile_direction(const FxParams &P, const Tile
   return hit;
 }
 
-// GB: zones per thread and gather round (their loads are in flight together; 4 for big tiles, 1 for tiles of a few
-// hundred zones, where the registers are better spent on more resident CTAs)
+// GB: (kept as a tuning handle of the launch: 1 caps the registers so that four CTAs of small tiles share an SM)
 template <int RECON, int RIEMANN, int WS, int NT, int GB>
 __global__ void __launch_bounds__(NT, (GB == 1 && NT == 256) ? 4 : 1) fx_k_stage_tile(const FxParams P, const double *__restrict__ X, const double *U0,
                                                       double *out, const double *__restrict__ dx, double dt,
@@ -151,37 +150,50 @@ __global__ void __launch_bounds__(NT, (GB == 1 && NT == 256) ? 4 : 1) fx_k_stage
   const Div de0(T.e0), de1(T.e1);
 
   // ---- 1. gather + cons -> prim, once per zone of the block and of its R-deep face slabs
-  for (int z0 = tid; z0 < ntile; z0 += GB * NT) {
-    double u[GB][5];
-    int outside[GB];
-#pragma unroll
-    for (int q = 0; q < GB; ++q) {
-      const int z = z0 + q * NT;
-      outside[q] = 3;  // "skip"
-      if (z >= ntile) continue;
+  // Pass A: every zone's five conserved values travel global -> shared by cp.async (no registers: all of a thread's
+  // loads, up to 60, are in flight together -- the gather is latency-bound); 5 bits per zone remember what pass B needs.
+  unsigned long long tag = 0;  // per zone of this thread: bit 0-1 = coordinates outside the interior (3 = skip), 2-4 = flip
+  {
+    int q = 0;
+    for (int z = tid; z < ntile; z += NT, ++q) {
       int t, t0, t1, t2;
       de0.divmod(z, t, t0);
       de1.divmod(t, t2, t1);
       // how many coordinates lie outside the interior box: 1-D stencils never look at edge or corner zones
-      outside[q] = (t0 < T.off[0] || t0 >= T.off[0] + T.n[0]) + (t1 < T.off[1] || t1 >= T.off[1] + T.n[1]) +
-                   (t2 < T.off[2] || t2 >= T.off[2] + T.n[2]);
-      if (outside[q] > 1) continue;
+      const int outside = (t0 < T.off[0] || t0 >= T.off[0] + T.n[0]) + (t1 < T.off[1] || t1 >= T.off[1] + T.n[1]) +
+                          (t2 < T.off[2] || t2 >= T.off[2] + T.n[2]);
+      if (outside > 1) {
+        tag |= 3ull << (5 * q);
+        continue;
+      }
       unsigned flip;
       const long long s = fx_guard_source(P, b, t0 - T.off[0] + P.gd[0], t1 - T.off[1] + P.gd[1], t2 - T.off[2] + P.gd[2], flip);
+      tag |= (unsigned long long)(outside | (flip << 2)) << (5 * q);
 #pragma unroll
-      for (int v = 0; v < 5; ++v) u[q][v] = X[v * P.S_v + s];
-      if (flip & 1u) u[q][1] = -u[q][1];
-      if (flip & 2u) u[q][2] = -u[q][2];
-      if (flip & 4u) u[q][3] = -u[q][3];
+      for (int v = 0; v < 5; ++v) {
+        const unsigned dst = (unsigned)__cvta_generic_to_shared(&T.Wp[v * ntile + z]);
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(X + v * P.S_v + s) : "memory");
+      }
     }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
+  }
+  // Pass B: each thread converts the zones it fetched, in place
+  {
+    int q = 0;
+    for (int z = tid; z < ntile; z += NT, ++q) {
+      const unsigned tg = (unsigned)(tag >> (5 * q)) & 31u;
+      if ((tg & 3u) == 3u) continue;
+      double u[5], w[5];
 #pragma unroll
-    for (int q = 0; q < GB; ++q) {
-      if (outside[q] > 1) continue;
-      double w[5];
-      const unsigned h = fx_c2p_v2(P, u[q][0], u[q][1], u[q][2], u[q][3], u[q][4], w);
-      if (outside[q] == 0) hit |= h;  // floors and non-finite states are counted where a zone is owned
+      for (int v = 0; v < 5; ++v) u[v] = T.Wp[v * ntile + z];
+      if (tg & 4u) u[1] = -u[1];
+      if (tg & 8u) u[2] = -u[2];
+      if (tg & 16u) u[3] = -u[3];
+      const unsigned h = fx_c2p_v2(P, u[0], u[1], u[2], u[3], u[4], w);
+      if ((tg & 3u) == 0u) hit |= h;  // floors and non-finite states are counted where a zone is owned
 #pragma unroll
-      for (int v = 0; v < 5; ++v) T.Wp[v * ntile + z0 + q * NT] = w[v];
+      for (int v = 0; v < 5; ++v) T.Wp[v * ntile + z] = w[v];
     }
   }
   (void)e2;
@@ -254,7 +266,11 @@ static int launch(const FxParams &P, const double *X, const double *U0, double *
 // Blocks whose primitives (padded block), one direction's fluxes and the accumulators fit the 227 KB of a CTA.
 bool fx_stage_tile_supported(const FxParams &P) {
   if (P.nblocks > 0x7fffffffLL || P.nblocks < 1) return false;
-  return fxtile::geometry(P).smem <= (size_t)227 * 1024;
+  const fxtile::Geo g = fxtile::geometry(P);
+  const int nint = P.n[0] * P.n[1] * P.n[2];
+  const int nt = (nint >= 1024 || (P.recon == FX_RECON_WENO5 && nint >= 512)) ? 512 : 256;
+  // (the gather keeps 5 bits per zone of a thread in one 64-bit word: at most 12 zones per thread)
+  return g.smem <= (size_t)227 * 1024 && g.ntile <= 12 * nt;
 }
 
 int fx_launch_stage_tile(const FxParams &P, const double *X, const double *U0, double *out, const double *dx, double dt,
