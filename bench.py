@@ -43,6 +43,8 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=5)
     ap.add_argument("--nb", default=None, help="override blocks per dimension, e.g. 16,16,16")
+    ap.add_argument("--block", default=None, help="override zones per block and dimension, e.g. 8,8,8 (with --nb 64,64,64: config 5's field "
+                    "on 8^3 blocks; not a BASELINE config: the small-block workload of the tile kernel)")
     ap.add_argument("--path", type=int, default=0, help="FX_OPT_PATH: 0 auto (fused TMA stage kernel when supported), 1 generic")
     ap.add_argument("--zchain", type=int, default=0, help="FX_OPT_ZCHAIN: z-neighbour blocks per CTA of the fused kernel (0 = library default)")
     ap.add_argument("--guard-x", type=int, default=-1, help="FX_OPT_GUARD_X: x guard depth (layout); -1 = 8 for 16-wide blocks with 4 guard zones "
@@ -131,6 +133,9 @@ def build_workload(args, device):
     from paper_2208_11630_b200 import inputs
     nb = tuple(int(x) for x in args.nb.split(",")) if args.nb else None
     cfg = inputs.config(args.config, nb=nb)
+    if args.block:
+        import dataclasses
+        cfg = dataclasses.replace(cfg, block_dims=tuple(int(x) for x in args.block.split(",")))
     order = fx.ORDER_MORTON if args.order == "morton" else fx.ORDER_LEX
     code = fx.TOPO_PERIODIC if cfg.bc == "periodic" else fx.TOPO_OUTFLOW
     bcs = [code if cfg.block_dims[d] > 1 else fx.TOPO_NONE for d in range(3)]
