@@ -18,7 +18,8 @@
  *  - State layout [a0]: U[v][b][k][j][i], fp64, SoA with one contiguous slab per variable, i fastest:
  *        element(v,b,k,j,i) = v*S_v + b*S_b + k*S_k + j*S_j + i        (int64 arithmetic)
  *    v in (rho, m_x, m_y, m_z, E); padded extents np[d] = n[d] + 2*gd[d], gd[d] = nguard if n[d] > 1
- *    else 0 (a dimension of extent 1 is inactive: no guards, no sweep, no dt contribution [A26]).
+ *    else 0 (a dimension of extent 1 is inactive: no guards, no sweep, no dt contribution [A26]);
+ *    FX_OPT_GUARD_X may deepen gd[0] alone (a layout choice: wider row pitch, same results).
  *    Interior zone (i,j,k) has gd[0] <= i < gd[0]+n[0] etc.  Query strides with fx_hydro_plan_layout.
  */
 #ifndef FX_HYDRO_H
