@@ -123,9 +123,10 @@ __device__ __forceinline__ unsigned tile_direction(const FxParams &P, const Tile
   return hit;
 }
 
-// GB: (kept as a tuning handle of the launch: 1 caps the registers so that four CTAs of small tiles share an SM)
-template <int RECON, int RIEMANN, int WS, int NT, int GB>
-__global__ void __launch_bounds__(NT, (GB == 1 && NT == 256) ? 4 : 1) fx_k_stage_tile(const FxParams P, const double *__restrict__ X, const double *U0,
+// MINB: resident CTAs per SM the register allocation aims at (4 for tiles of a few hundred zones, whose shared memory
+// would allow it; 1 otherwise: shared memory limits those to one or two CTAs anyway)
+template <int RECON, int RIEMANN, int WS, int NT, int MINB>
+__global__ void __launch_bounds__(NT, MINB) fx_k_stage_tile(const FxParams P, const double *__restrict__ X, const double *U0,
                                                       double *out, const double *__restrict__ dx, double dt,
                                                       const double *__restrict__ dt_dev, double beta, int first,
                                                       int ntile, int faces_max, int nint) {
@@ -234,11 +235,11 @@ __global__ void __launch_bounds__(NT, (GB == 1 && NT == 256) ? 4 : 1) fx_k_stage
   if (hit) fx_note(P, hit);
 }
 
-template <int RECON, int RIEMANN, int WS, int NT, int GB>
+template <int RECON, int RIEMANN, int WS, int NT, int MINB>
 static int launch_nt(const FxParams &P, const double *X, const double *U0, double *out, const double *dx, double dt,
                      const double *dt_dev, double beta, int first, cudaStream_t st) {
   const Geo g = geometry(P);
-  auto kern = fx_k_stage_tile<RECON, RIEMANN, WS, NT, GB>;
+  auto kern = fx_k_stage_tile<RECON, RIEMANN, WS, NT, MINB>;
   static bool configured = false;  // per instantiation
   if (!configured) {
     FX_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
@@ -256,9 +257,9 @@ static int launch(const FxParams &P, const double *X, const double *U0, double *
                   const double *dt_dev, double beta, int first, cudaStream_t st) {
   const int nint = P.n[0] * P.n[1] * P.n[2];
   if (nint >= 1024 || (RECON == FX_RECON_WENO5 && nint >= 512))
-    return launch_nt<RECON, RIEMANN, WS, 512, 4>(P, X, U0, out, dx, dt, dt_dev, beta, first, st);
-  if (geometry(P).ntile >= 1024) return launch_nt<RECON, RIEMANN, WS, 256, 4>(P, X, U0, out, dx, dt, dt_dev, beta, first, st);
-  return launch_nt<RECON, RIEMANN, WS, 256, 1>(P, X, U0, out, dx, dt, dt_dev, beta, first, st);
+    return launch_nt<RECON, RIEMANN, WS, 512, 1>(P, X, U0, out, dx, dt, dt_dev, beta, first, st);
+  if (geometry(P).ntile >= 1024) return launch_nt<RECON, RIEMANN, WS, 256, 1>(P, X, U0, out, dx, dt, dt_dev, beta, first, st);
+  return launch_nt<RECON, RIEMANN, WS, 256, 4>(P, X, U0, out, dx, dt, dt_dev, beta, first, st);
 }
 
 }  // namespace fxtile
