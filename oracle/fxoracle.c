@@ -19,6 +19,10 @@
  * algorithm itself, step by step, in fp64, with no blocking, fusion or
  * reordering.  Built with -O2 -ffp-contract=off (no FMA contraction).
  *
+ * Passive mass scalars (nvars = 5 + ns, reading B11 of DESIGN.md; "multispecies variant"): carried as
+ * rho X_s, reconstructed as X_s, and given by each Riemann solver the flux it gives a transverse velocity.  Pinned in
+ * tests/test_oracle_scalars.py.
+ *
  * Pins (tests/test_oracle_*.py, -m "not gpu"): see DESIGN.md "Oracle pins".
  * Parity unpinned: none of the routines; the Kelvin-Helmholtz field after 100
  * steps and the config-5 field after 10 steps have no exact solution and are
@@ -49,6 +53,7 @@
 #define FXO_OPT_GRAVITY_X 6 /* constant acceleration g_d [B10]; 4 and 5 are options of the CUDA library only */
 #define FXO_OPT_GRAVITY_Y 7
 #define FXO_OPT_GRAVITY_Z 8
+#define FXO_MAXV 32 /* 5 hydro variables + up to 27 passive mass scalars [B11] */
 #define FXO_STATUS_NONFINITE 1u
 #define FXO_STATUS_RHO_FLOOR 2u
 #define FXO_STATUS_P_FLOOR 4u
@@ -85,7 +90,7 @@ int fxo_plan_create(fxo_plan **out, const int dims[3], int nguard, int nvars, in
                     double gamma, int recon, int riemann, int rk_order) {
   if (!out || !dims) return FXO_ERR_INVALID_ARG;
   *out = NULL;
-  if (nvars != 5 || nblocks < 0 || !(gamma > 1.0)) return FXO_ERR_INVALID_ARG;
+  if (nvars < 5 || nvars > FXO_MAXV || nblocks < 0 || !(gamma > 1.0)) return FXO_ERR_INVALID_ARG;
   if (recon != FXO_RECON_PLM_MINMOD && recon != FXO_RECON_WENO5) return FXO_ERR_INVALID_ARG;
   if (riemann != FXO_RIEMANN_HLLE && riemann != FXO_RIEMANN_HLLC) return FXO_ERR_INVALID_ARG;
   if (rk_order != 2 && rk_order != 3) return FXO_ERR_INVALID_ARG;
@@ -358,8 +363,9 @@ int fxo_fill_guardcells(fxo_plan *p, double *U) {
 
 /* ---------------------------------------------------- O2 cons -> prim */
 
-/* U = (rho, mx, my, mz, E) -> W = (rho, u, v, w, p).  Floors touch primitives only [A7]. */
-static void cons2prim(const fxo_plan *p, const double U[5], double W[5], unsigned *hit) {
+/* U = (rho, mx, my, mz, E, rho X_1 ..) -> W = (rho, u, v, w, p, X_1 ..).  Floors touch primitives only [A7].
+ * Passive mass scalars [B11]: X_s = (rho X_s) / rho with the same (floored) density the velocities use; nv = 5 + ns. */
+static void cons2prim(const fxo_plan *p, int nv, const double *U, double *W, unsigned *hit) {
   double rho = U[0];
   if (rho < p->rho_floor) { /* NaN compares false and stays NaN */
     rho = p->rho_floor;
@@ -379,11 +385,21 @@ static void cons2prim(const fxo_plan *p, const double U[5], double W[5], unsigne
   W[4] = pr;
   if (!isfinite(rho) || !isfinite(u) || !isfinite(v) || !isfinite(w) || !isfinite(pr))
     *hit |= FXO_STATUS_NONFINITE;
+  for (int s = 5; s < nv; ++s) {
+    W[s] = U[s] * r;
+    if (!isfinite(W[s])) *hit |= FXO_STATUS_NONFINITE;
+  }
 }
 
 void fxo_cons2prim(const fxo_plan *p, const double U[5], double W[5]) {
   unsigned hit = 0;
-  cons2prim(p, U, W, &hit);
+  cons2prim(p, 5, U, W, &hit);
+}
+
+/* The same with the plan's passive scalars: U and W hold p->nvars entries [B11]. */
+void fxo_cons2prim_nv(const fxo_plan *p, const double *U, double *W) {
+  unsigned hit = 0;
+  cons2prim(p, p->nvars, U, W, &hit);
 }
 
 /* ------------------------------------------------- O3 reconstruction */
@@ -415,12 +431,13 @@ double fxo_weno5(double a, double b, double c, double d, double e, double eps) {
 }
 
 /* Left and right primitive states at the face between padded cells iL and iR = iL + 1 along a
- * line of stride s in the primitive array W (5 slabs of size slab). */
-static void reconstruct_face(const fxo_plan *p, const double *W, int64_t slab, int64_t cL, int64_t s,
-                             double WL[5], double WR[5], unsigned *hit) {
+ * line of stride s in the primitive array W (nv slabs of size slab; every component, passive scalars
+ * included [B11], is reconstructed the same way and the positivity fallback replaces all of them). */
+static void reconstruct_face(const fxo_plan *p, int nv, const double *W, int64_t slab, int64_t cL, int64_t s,
+                             double *WL, double *WR, unsigned *hit) {
   int64_t cR = cL + s;
   if (p->recon == FXO_RECON_PLM_MINMOD) {
-    for (int v = 0; v < 5; ++v) {
+    for (int v = 0; v < nv; ++v) {
       const double *q = W + v * slab;
       double dL = fxo_minmod(q[cL] - q[cL - s], q[cL + s] - q[cL]);
       double dR = fxo_minmod(q[cR] - q[cR - s], q[cR + s] - q[cR]);
@@ -428,18 +445,18 @@ static void reconstruct_face(const fxo_plan *p, const double *W, int64_t slab, i
       WR[v] = q[cR] - 0.5 * dR;
     }
   } else {
-    for (int v = 0; v < 5; ++v) {
+    for (int v = 0; v < nv; ++v) {
       const double *q = W + v * slab;
       WL[v] = fxo_weno5(q[cL - 2 * s], q[cL - s], q[cL], q[cL + s], q[cL + 2 * s], p->weno_eps);
       WR[v] = fxo_weno5(q[cR + 2 * s], q[cR + s], q[cR], q[cR - s], q[cR - 2 * s], p->weno_eps);
     }
     /* positivity fallback, per side [A6] */
     if (!(WL[0] > 0.0) || !(WL[4] > 0.0)) {
-      for (int v = 0; v < 5; ++v) WL[v] = W[v * slab + cL];
+      for (int v = 0; v < nv; ++v) WL[v] = W[v * slab + cL];
       *hit |= FXO_STATUS_WENO_FALLBACK;
     }
     if (!(WR[0] > 0.0) || !(WR[4] > 0.0)) {
-      for (int v = 0; v < 5; ++v) WR[v] = W[v * slab + cR];
+      for (int v = 0; v < nv; ++v) WR[v] = W[v * slab + cR];
       *hit |= FXO_STATUS_WENO_FALLBACK;
     }
   }
@@ -450,7 +467,10 @@ static void reconstruct_face(const fxo_plan *p, const double *W, int64_t slab, i
 /* States in the face frame: W = (rho, un, ut1, ut2, p); flux F = (mass, normal momentum,
  * t1 momentum, t2 momentum, energy).  Einfeldt (Roe-average) or Davis wave-speed bounds [A8];
  * HLLE in branching form [A10]; Toro's HLLC with the test order of O4 [A9]. */
-static void riemann_flux(const fxo_plan *p, const double WL[5], const double WR[5], double F[5]) {
+/* Passive scalars [B11]: W[5 + s] = X_s, U = rho X_s, F = (rho un) X_s -- each solver treats X_s exactly as it
+ * treats a transverse velocity (an advected quantity): upwind flux when supersonic, the HLL average for HLLE,
+ * rho* X_K in the star state of HLLC (which makes the flux X_K times the mass flux). */
+static void riemann_flux(const fxo_plan *p, int nv, const double *WL, const double *WR, double *F) {
   const double gam = p->gamma, gm1 = p->gamma - 1.0, igm1 = 1.0 / (p->gamma - 1.0);
   double rL = WL[0], unL = WL[1], t1L = WL[2], t2L = WL[3], pL = WL[4];
   double rR = WR[0], unR = WR[1], t1R = WR[2], t2R = WR[3], pR = WR[4];
@@ -458,10 +478,16 @@ static void riemann_flux(const fxo_plan *p, const double WL[5], const double WR[
   double cL = sqrt(gam * pL * irL), cR = sqrt(gam * pR * irR);
   double EL = pL * igm1 + 0.5 * rL * (unL * unL + t1L * t1L + t2L * t2L);
   double ER = pR * igm1 + 0.5 * rR * (unR * unR + t1R * t1R + t2R * t2R);
-  double UL[5] = {rL, rL * unL, rL * t1L, rL * t2L, EL};
-  double UR[5] = {rR, rR * unR, rR * t1R, rR * t2R, ER};
-  double FL[5] = {UL[1], UL[1] * unL + pL, UL[1] * t1L, UL[1] * t2L, unL * (EL + pL)};
-  double FR[5] = {UR[1], UR[1] * unR + pR, UR[1] * t1R, UR[1] * t2R, unR * (ER + pR)};
+  double UL[FXO_MAXV] = {rL, rL * unL, rL * t1L, rL * t2L, EL};
+  double UR[FXO_MAXV] = {rR, rR * unR, rR * t1R, rR * t2R, ER};
+  double FL[FXO_MAXV] = {UL[1], UL[1] * unL + pL, UL[1] * t1L, UL[1] * t2L, unL * (EL + pL)};
+  double FR[FXO_MAXV] = {UR[1], UR[1] * unR + pR, UR[1] * t1R, UR[1] * t2R, unR * (ER + pR)};
+  for (int s = 5; s < nv; ++s) {
+    UL[s] = rL * WL[s];
+    UR[s] = rR * WR[s];
+    FL[s] = UL[1] * WL[s];
+    FR[s] = UR[1] * WR[s];
+  }
   double SL, SR;
   if (p->wavespeed == 0) {
     double HL = (EL + pL) * irL, HR = (ER + pR) * irR;
@@ -485,16 +511,16 @@ static void riemann_flux(const fxo_plan *p, const double WL[5], const double WR[
     SR = a > b ? a : b;
   }
   if (SL >= 0.0) {
-    for (int v = 0; v < 5; ++v) F[v] = FL[v];
+    for (int v = 0; v < nv; ++v) F[v] = FL[v];
     return;
   }
   if (SR <= 0.0) {
-    for (int v = 0; v < 5; ++v) F[v] = FR[v];
+    for (int v = 0; v < nv; ++v) F[v] = FR[v];
     return;
   }
   if (p->riemann == FXO_RIEMANN_HLLE) {
     double den = SR - SL, ss = SL * SR;
-    for (int v = 0; v < 5; ++v) F[v] = (SR * FL[v] - SL * FR[v] + ss * (UR[v] - UL[v])) / den;
+    for (int v = 0; v < nv; ++v) F[v] = (SR * FL[v] - SL * FR[v] + ss * (UR[v] - UL[v])) / den;
     return;
   }
   /* HLLC */
@@ -502,40 +528,53 @@ static void riemann_flux(const fxo_plan *p, const double WL[5], const double WR[
   double Ss = ((pR - pL) + (aL * unL - aR * unR)) / (aL - aR);
   if (Ss >= 0.0) {
     double f = aL / (SL - Ss);
-    double Us[5] = {f, f * Ss, f * t1L, f * t2L, f * (EL * irL + (Ss - unL) * (Ss + pL / aL))};
-    for (int v = 0; v < 5; ++v) F[v] = FL[v] + SL * (Us[v] - UL[v]);
+    double Us[FXO_MAXV] = {f, f * Ss, f * t1L, f * t2L, f * (EL * irL + (Ss - unL) * (Ss + pL / aL))};
+    for (int s = 5; s < nv; ++s) Us[s] = f * WL[s];
+    for (int v = 0; v < nv; ++v) F[v] = FL[v] + SL * (Us[v] - UL[v]);
   } else {
     double f = aR / (SR - Ss);
-    double Us[5] = {f, f * Ss, f * t1R, f * t2R, f * (ER * irR + (Ss - unR) * (Ss + pR / aR))};
-    for (int v = 0; v < 5; ++v) F[v] = FR[v] + SR * (Us[v] - UR[v]);
+    double Us[FXO_MAXV] = {f, f * Ss, f * t1R, f * t2R, f * (ER * irR + (Ss - unR) * (Ss + pR / aR))};
+    for (int s = 5; s < nv; ++s) Us[s] = f * WR[s];
+    for (int v = 0; v < nv; ++v) F[v] = FR[v] + SR * (Us[v] - UR[v]);
   }
 }
 
 /* Public, for the per-routine pins: states and flux in the face frame (rho, un, ut1, ut2, p). */
 void fxo_riemann_flux(const fxo_plan *p, const double WL[5], const double WR[5], double F[5]) {
-  riemann_flux(p, WL, WR, F);
+  riemann_flux(p, 5, WL, WR, F);
+}
+
+/* The same with the plan's passive scalars: WL, WR, F hold p->nvars entries [B11]. */
+void fxo_riemann_flux_nv(const fxo_plan *p, const double *WL, const double *WR, double *F) {
+  riemann_flux(p, p->nvars, WL, WR, F);
 }
 
 /* ------------------------------------------------ O5 spatial operator */
 
 /* Face flux in direction d at the face whose left cell has flat in-block index cL, returned in
- * the un-rotated variable order (rho, mx, my, mz, E). */
-static void face_flux(const fxo_plan *p, const double *W, int64_t slab, int64_t cL, int d, double F[5],
+ * the un-rotated variable order (rho, mx, my, mz, E, scalars). */
+static void face_flux(const fxo_plan *p, const double *W, int64_t slab, int64_t cL, int d, double *F,
                       unsigned *hit) {
+  const int nv = p->nvars;
   const int64_t stride[3] = {1, p->S_j, p->S_k};
   /* frame of direction d: normal = d, t1 = (d+1)%3, t2 = (d+2)%3 */
   int in = 1 + d, it1 = 1 + (d + 1) % 3, it2 = 1 + (d + 2) % 3;
-  double WLu[5], WRu[5], WLf[5], WRf[5], Ff[5];
-  reconstruct_face(p, W, slab, cL, stride[d], WLu, WRu, hit);
+  double WLu[FXO_MAXV], WRu[FXO_MAXV], WLf[FXO_MAXV], WRf[FXO_MAXV], Ff[FXO_MAXV];
+  reconstruct_face(p, nv, W, slab, cL, stride[d], WLu, WRu, hit);
   WLf[0] = WLu[0]; WLf[1] = WLu[in]; WLf[2] = WLu[it1]; WLf[3] = WLu[it2]; WLf[4] = WLu[4];
   WRf[0] = WRu[0]; WRf[1] = WRu[in]; WRf[2] = WRu[it1]; WRf[3] = WRu[it2]; WRf[4] = WRu[4];
-  riemann_flux(p, WLf, WRf, Ff);
+  for (int s = 5; s < nv; ++s) {
+    WLf[s] = WLu[s];
+    WRf[s] = WRu[s];
+  }
+  riemann_flux(p, nv, WLf, WRf, Ff);
+  for (int s = 5; s < nv; ++s) F[s] = Ff[s];
   F[0] = Ff[0];
   F[in] = Ff[1];
   F[it1] = Ff[2];
   F[it2] = Ff[3];
   F[4] = Ff[4];
-  for (int v = 0; v < 5; ++v)
+  for (int v = 0; v < nv; ++v)
     if (!isfinite(F[v])) *hit |= FXO_STATUS_NONFINITE;
 }
 
@@ -559,17 +598,17 @@ static void count_hits(fxo_plan *p, unsigned hit, unsigned long long n) {
   }
 }
 
-/* Primitives of every padded zone of block b of X into W[5][S_b] (guards must be filled). */
+/* Primitives of every padded zone of block b of X into W[nvars][S_b] (guards must be filled). */
 static void block_prims(fxo_plan *p, const double *X, int64_t b, double *W) {
   for (int k = 0; k < p->np[2]; ++k)
     for (int j = 0; j < p->np[1]; ++j)
       for (int i = 0; i < p->np[0]; ++i) {
         int64_t c = k * p->S_k + j * p->S_j + i;
-        double U[5], Wz[5];
-        for (int v = 0; v < 5; ++v) U[v] = X[v * p->S_v + b * p->S_b + c];
+        double U[FXO_MAXV], Wz[FXO_MAXV];
+        for (int v = 0; v < p->nvars; ++v) U[v] = X[v * p->S_v + b * p->S_b + c];
         unsigned hit = 0;
-        cons2prim(p, U, Wz, &hit);
-        for (int v = 0; v < 5; ++v) W[v * p->S_b + c] = Wz[v];
+        cons2prim(p, p->nvars, U, Wz, &hit);
+        for (int v = 0; v < p->nvars; ++v) W[v * p->S_b + c] = Wz[v];
         int interior = i >= p->gd[0] && i < p->gd[0] + p->n[0] && j >= p->gd[1] &&
                        j < p->gd[1] + p->n[1] && k >= p->gd[2] && k < p->gd[2] + p->n[2];
         if (interior) count_hits(p, hit, 1); /* count each zone once, where it is owned */
@@ -578,13 +617,15 @@ static void block_prims(fxo_plan *p, const double *X, int64_t b, double *W) {
 
 /* One RK stage on block b: out = U0 + beta*((X - U0) - S(X)), S = sum_d (dt/dx_d)(F+ - F-)
  * summed in the order x, y, z [O5, O6], minus dt times the constant-gravity source of the stage input [B10]:
- * (0, rho g_x, rho g_y, rho g_z, g . m) from the zone's conserved values.  W and Fline are per-thread scratch. */
+ * (0, rho g_x, rho g_y, rho g_z, g . m) from the zone's conserved values (none for the scalars [B11]).  W and Fline
+ * are per-thread scratch. */
 static void block_stage(fxo_plan *p, const double *X, const double *U0, double *out, int64_t b,
                         const double *dx, double dt, double beta, int first, double *W, double *S,
                         double *Fline) {
+  const int nv = p->nvars;
   block_prims(p, X, b, W);
   const int64_t stride[3] = {1, p->S_j, p->S_k};
-  memset(S, 0, sizeof(double) * 5 * (size_t)p->S_b);
+  memset(S, 0, sizeof(double) * (size_t)nv * (size_t)p->S_b);
   for (int d = 0; d < 3; ++d) {
     if (!p->active[d]) continue;
     double r = dt / dx[b * 3 + d];
@@ -595,12 +636,12 @@ static void block_stage(fxo_plan *p, const double *X, const double *U0, double *
         unsigned hit = 0;
         for (int f = 0; f <= p->n[d]; ++f) {
           int64_t cL = base + (int64_t)(p->gd[d] + f - 1) * stride[d];
-          face_flux(p, W, p->S_b, cL, d, Fline + 5 * f, &hit);
+          face_flux(p, W, p->S_b, cL, d, Fline + nv * f, &hit);
         }
         count_hits(p, hit & (FXO_STATUS_NONFINITE | FXO_STATUS_WENO_FALLBACK), 1);
         for (int f = 0; f < p->n[d]; ++f) {
           int64_t c = base + (int64_t)(p->gd[d] + f) * stride[d];
-          for (int v = 0; v < 5; ++v) S[v * p->S_b + c] += r * (Fline[5 * (f + 1) + v] - Fline[5 * f + v]);
+          for (int v = 0; v < nv; ++v) S[v * p->S_b + c] += r * (Fline[nv * (f + 1) + v] - Fline[nv * f + v]);
         }
       }
   }
@@ -617,7 +658,7 @@ static void block_stage(fxo_plan *p, const double *X, const double *U0, double *
           }
           S[4 * p->S_b + c] -= dt * gm;
         }
-        for (int v = 0; v < 5; ++v) {
+        for (int v = 0; v < nv; ++v) {
           int64_t g = v * p->S_v + b * p->S_b + c;
           if (first)
             out[g] = U0[g] - S[v * p->S_b + c];
@@ -634,11 +675,11 @@ static int run_stage(fxo_plan *p, double *X, const double *U0, double *out, cons
   int fail = 0;
 #pragma omp parallel
   {
-    double *W = (double *)malloc(sizeof(double) * 5 * (size_t)p->S_b);
-    double *S = (double *)malloc(sizeof(double) * 5 * (size_t)p->S_b);
+    double *W = (double *)malloc(sizeof(double) * (size_t)p->nvars * (size_t)p->S_b);
+    double *S = (double *)malloc(sizeof(double) * (size_t)p->nvars * (size_t)p->S_b);
     int nmax = p->n[0] > p->n[1] ? p->n[0] : p->n[1];
     if (p->n[2] > nmax) nmax = p->n[2];
-    double *Fl = (double *)malloc(sizeof(double) * 5 * (size_t)(nmax + 1));
+    double *Fl = (double *)malloc(sizeof(double) * (size_t)p->nvars * (size_t)(nmax + 1));
     if (!W || !S || !Fl) {
 #pragma omp atomic write
       fail = 1;
@@ -657,7 +698,7 @@ static int run_stage(fxo_plan *p, double *X, const double *U0, double *out, cons
 int fxo_euler_step(fxo_plan *p, double *U, const double *dx, double dt) {
   if (!p || (!U && p->nblocks) || (!dx && p->nblocks)) return FXO_ERR_INVALID_ARG;
   if (!p->neigh && p->nblocks > 0) return FXO_ERR_STATE;
-  size_t n = (size_t)p->S_v * 5;
+  size_t n = (size_t)p->S_v * (size_t)p->nvars;
   double *U1 = (double *)malloc(sizeof(double) * (n ? n : 1));
   if (!U1) return FXO_ERR_NOMEM;
   int rc = run_stage(p, U, U, U1, dx, dt, 1.0, 1);
@@ -667,7 +708,7 @@ int fxo_euler_step(fxo_plan *p, double *U, const double *dx, double dt) {
       for (int k = p->gd[2]; k < p->gd[2] + p->n[2]; ++k)
         for (int j = p->gd[1]; j < p->gd[1] + p->n[1]; ++j)
           for (int i = p->gd[0]; i < p->gd[0] + p->n[0]; ++i)
-            for (int v = 0; v < 5; ++v) {
+            for (int v = 0; v < p->nvars; ++v) {
               int64_t g = v * p->S_v + b * p->S_b + k * p->S_k + j * p->S_j + i;
               U[g] = U1[g];
             }
@@ -682,7 +723,7 @@ int fxo_hydro_advance(fxo_plan *p, double *U, const double *dx, double dt) {
   if (!(dt > 0.0) || !isfinite(dt)) return FXO_ERR_INVALID_ARG;
   if (!p->neigh && p->nblocks > 0) return FXO_ERR_STATE;
   if (p->nblocks == 0) return FXO_OK;
-  size_t n = (size_t)p->S_v * 5;
+  size_t n = (size_t)p->S_v * (size_t)p->nvars;
   double *U1 = (double *)malloc(sizeof(double) * n);
   double *U2 = p->rk == 3 ? (double *)malloc(sizeof(double) * n) : NULL;
   if (!U1 || (p->rk == 3 && !U2)) {
@@ -716,7 +757,7 @@ int fxo_debug_compute_fluxes(fxo_plan *p, const double *U, int dir, double *F) {
   int fail = 0;
 #pragma omp parallel
   {
-    double *W = (double *)malloc(sizeof(double) * 5 * (size_t)p->S_b);
+    double *W = (double *)malloc(sizeof(double) * (size_t)p->nvars * (size_t)p->S_b);
     if (!W) {
 #pragma omp atomic write
       fail = 1;
@@ -731,10 +772,10 @@ int fxo_debug_compute_fluxes(fxo_plan *p, const double *U, int dir, double *F) {
               c[dir] -= 1; /* left cell of face f is padded cell g + f - 1 */
               int64_t cL = c[2] * p->S_k + c[1] * p->S_j + c[0];
               (void)stride;
-              double Ff[5];
+              double Ff[FXO_MAXV];
               unsigned hit = 0;
               face_flux(p, W, p->S_b, cL, dir, Ff, &hit);
-              for (int v = 0; v < 5; ++v) F[v * FS_v + b * FS_b + k * FS_k + j * FS_j + i] = Ff[v];
+              for (int v = 0; v < p->nvars; ++v) F[v * FS_v + b * FS_b + k * FS_k + j * FS_j + i] = Ff[v];
             }
       }
     }
@@ -757,7 +798,7 @@ int fxo_hydro_compute_dt(fxo_plan *p, const double *U, const double *dx, double 
           double Uz[5], W[5];
           for (int v = 0; v < 5; ++v) Uz[v] = U[v * p->S_v + c];
           unsigned hit = 0;
-          cons2prim(p, Uz, W, &hit);
+          cons2prim(p, 5, Uz, W, &hit); /* the scalars do not enter the time step [B11] */
           double cs = sqrt(p->gamma * W[4] / W[0]);
           for (int d = 0; d < 3; ++d) {
             if (!p->active[d]) continue;

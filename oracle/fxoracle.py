@@ -30,7 +30,7 @@ def build(force: bool = False) -> str:
     """Compile the oracle with gcc (no FMA contraction, no fast-math)."""
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
         subprocess.check_call(
-            ["gcc", "-O2", "-ffp-contract=off", "-fopenmp", "-std=c99", "-Wall", "-shared", "-fPIC",
+            ["gcc", "-O2", "-ffp-contract=off", "-fopenmp", "-std=c99", "-Wall", "-Wno-maybe-uninitialized", "-shared", "-fPIC",
              "-o", _LIB, _SRC, "-lm"])
     return _LIB
 
@@ -69,6 +69,10 @@ def lib():
         L.fxo_weno5.restype = C.c_double
         L.fxo_riemann_flux.argtypes = [C.c_void_p, dp, dp, dp]
         L.fxo_riemann_flux.restype = None
+        L.fxo_cons2prim_nv.argtypes = [C.c_void_p, dp, dp]
+        L.fxo_cons2prim_nv.restype = None
+        L.fxo_riemann_flux_nv.argtypes = [C.c_void_p, dp, dp, dp]
+        L.fxo_riemann_flux_nv.restype = None
         L.fxo_euler_step.argtypes = [C.c_void_p, dp, dp, C.c_double]
         L.fxo_hydro_advance.argtypes = [C.c_void_p, dp, dp, C.c_double]
         L.fxo_debug_compute_fluxes.argtypes = [C.c_void_p, dp, C.c_int, dp]
@@ -174,6 +178,23 @@ class OraclePlan:
         W = np.empty(5)
         lib().fxo_cons2prim(self._h, _dptr(U5), _dptr(W))
         return W
+
+    def cons2prim_nv(self, U):
+        """All nvars entries (hydro variables + passive scalars, reading B11)."""
+        U = np.ascontiguousarray(U, np.float64)
+        assert U.shape == (self.nvars,)
+        W = np.empty(self.nvars)
+        lib().fxo_cons2prim_nv(self._h, _dptr(U), _dptr(W))
+        return W
+
+    def riemann_flux_nv(self, WL, WR):
+        """Face-frame states (rho, un, ut1, ut2, p, X_1..) of nvars entries -> flux of nvars entries (B11)."""
+        WL = np.ascontiguousarray(WL, np.float64)
+        WR = np.ascontiguousarray(WR, np.float64)
+        assert WL.shape == (self.nvars,) and WR.shape == (self.nvars,)
+        F = np.empty(self.nvars)
+        lib().fxo_riemann_flux_nv(self._h, _dptr(WL), _dptr(WR), _dptr(F))
+        return F
 
     def riemann_flux(self, WL, WR):
         WL = np.ascontiguousarray(WL, np.float64)

@@ -117,18 +117,18 @@ def dx_array(cfg: Config, nblocks=None) -> np.ndarray:
     return np.ascontiguousarray(np.tile(np.asarray(cfg.dx, np.float64), (n, 1)))
 
 
-def padded_shape(cfg: Config, nblocks=None):
+def padded_shape(cfg: Config, nblocks=None, nvars=5):
     g = [cfg.nguard if d > 1 else 0 for d in cfg.block_dims]
     n = cfg.nblocks if nblocks is None else nblocks
-    return (5, n, cfg.block_dims[2] + 2 * g[2], cfg.block_dims[1] + 2 * g[1], cfg.block_dims[0] + 2 * g[0])
+    return (nvars, n, cfg.block_dims[2] + 2 * g[2], cfg.block_dims[1] + 2 * g[1], cfg.block_dims[0] + 2 * g[0])
 
 
 def embed(cfg: Config, interior: torch.Tensor, guard_value=float("nan")) -> torch.Tensor:
-    """Place interiors [5][nsel][nz][ny][nx] into a padded state array; guard zones get guard_value
+    """Place interiors [nvars][nsel][nz][ny][nx] into a padded state array; guard zones get guard_value
     (NaN by default: fx_hydro_advance must not depend on them [A15])."""
     g = [cfg.nguard if d > 1 else 0 for d in cfg.block_dims]
     nx, ny, nz = cfg.block_dims
-    U = torch.full(padded_shape(cfg, interior.shape[1]), guard_value, dtype=torch.float64, device=interior.device)
+    U = torch.full(padded_shape(cfg, interior.shape[1], interior.shape[0]), guard_value, dtype=torch.float64, device=interior.device)
     U[:, :, g[2]:g[2] + nz, g[1]:g[1] + ny, g[0]:g[0] + nx] = interior
     return U
 
@@ -264,6 +264,42 @@ def block_interiors(cfg: Config, coords, device="cpu") -> torch.Tensor:
         rho = torch.exp(s - 0.5 * sigma * sigma)
         return _prim_to_cons(rho, vel[0], vel[1], vel[2], ones, cfg.gamma)
     raise ValueError(n)
+
+
+def with_scalars(cfg: Config, coords, interior: torch.Tensor, ns: int) -> torch.Tensor:
+    """Append ns passive mass scalars rho*X_s to interiors [5][nsel][nz][ny][nx] -> [5+ns][...] (reading B11; the
+    stand-in for a multispecies composition).  Even s: a smooth abundance X_s = 0.5 + 0.4 cos(2 pi
+    k_s.x + phi_s), integer k_s with 1 <= |k_s|_inf <= 3 in the active dimensions, seeded; odd s: a composition
+    interface, X_s = 1 where N/4 <= I_d < 3N/4 along the active dimension d = (s // 2) % ndim, else 0.
+    N_d counts the zones of the tiling cfg.nb (not of the full-size field), so reduced tilings keep both features."""
+    if ns == 0:
+        return interior
+    coords = np.asarray(coords)
+    dev = interior.device
+    idx = _global_index(cfg, coords, dev)
+    N = tuple(cfg.block_dims[d] * cfg.nb[d] for d in range(3))  # the tiling actually run (periodic on it)
+    active = [d for d in range(3) if cfg.block_dims[d] > 1]
+    rho = interior[0]
+    view = [(slice(None), None, None, slice(None)), (slice(None), None, slice(None), None),
+            (slice(None), slice(None), None, None)]
+    out = [interior]
+    rng = np.random.default_rng([BASE_SEED, cfg.number, 100])
+    for s in range(ns):
+        k = rng.integers(-3, 4, size=3)
+        phi = rng.random()
+        if s % 2 == 0:
+            if all(k[d] == 0 for d in active):
+                k[active[0]] = 1
+            theta = torch.zeros(rho.shape, dtype=torch.float64, device=dev)
+            for d in active:
+                theta = theta + (int(k[d]) * (2 * idx[d] + 1) % (2 * N[d])).to(torch.float64)[view[d]] / N[d]
+            X = 0.5 + 0.4 * torch.cos(math.pi * theta + 2.0 * math.pi * phi)
+        else:
+            d = active[(s // 2) % len(active)]
+            inside = ((4 * idx[d] >= N[d]) & (4 * idx[d] < 3 * N[d]))[view[d]]
+            X = torch.where(inside, torch.ones_like(rho), torch.zeros_like(rho))
+        out.append((rho * X)[None])
+    return torch.cat(out, dim=0)
 
 
 def initial_state(cfg: Config, order=ORDER_LEX, device="cpu", chunk_blocks=2048, guard_value=float("nan")):

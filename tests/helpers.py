@@ -20,7 +20,8 @@ def golden_rows(name):
     return rows
 
 
-def oracle_plan_for(cfg, nblocks=None, order=inputs.ORDER_LEX, bc=None, nb=None, recon=None, riemann=None, rk=None):
+def oracle_plan_for(cfg, nblocks=None, order=inputs.ORDER_LEX, bc=None, nb=None, recon=None, riemann=None, rk=None,
+                    nvars=5):
     """Oracle plan + topology for a config (regular tiling nb, default cfg.nb)."""
     nb = tuple(nb or cfg.nb)
     bc = bc or cfg.bc
@@ -29,7 +30,7 @@ def oracle_plan_for(cfg, nblocks=None, order=inputs.ORDER_LEX, bc=None, nb=None,
     neigh, coords = fxo.topology_cartesian(nb, bcs, bcs, order)
     plan = fxo.OraclePlan(cfg.block_dims, cfg.nguard, neigh.shape[0], cfg.gamma,
                           cfg.recon if recon is None else recon, cfg.riemann if riemann is None else riemann,
-                          cfg.rk_order if rk is None else rk)
+                          cfg.rk_order if rk is None else rk, nvars=nvars)
     plan.set_topology(neigh)
     return plan, neigh, coords
 
@@ -145,7 +146,7 @@ def rel_err(cfg, got, ref):
 
 
 def gpu_plan_for(cfg, order=inputs.ORDER_LEX, bc=None, nb=None, recon=None, riemann=None, rk=None, path=None,
-                 neigh=None, nblocks=None, zchain=None):
+                 neigh=None, nblocks=None, zchain=None, nvars=5):
     """CUDA-side plan + topology + workspace for a config (uses the library's own topology helper)."""
     from paper_2208_11630_b200 import binding as fx
     nb = tuple(nb or cfg.nb)
@@ -157,7 +158,7 @@ def gpu_plan_for(cfg, order=inputs.ORDER_LEX, bc=None, nb=None, recon=None, riem
         neigh, coords = fx.fx_topology_cartesian(nb, bcs, bcs, order)
     plan = fx.HydroPlan(cfg.block_dims, cfg.nguard, neigh.shape[0], cfg.gamma,
                         cfg.recon if recon is None else recon, cfg.riemann if riemann is None else riemann,
-                        cfg.rk_order if rk is None else rk)
+                        cfg.rk_order if rk is None else rk, nvars=nvars)
     if path is not None:
         plan.fx_hydro_plan_set_option(fx.OPT_PATH, path)
     if zchain is not None:

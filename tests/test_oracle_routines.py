@@ -177,4 +177,6 @@ def test_plan_argument_checks():
     with pytest.raises(ValueError):
         fxo.OraclePlan((8, 1, 1), 4, 1, 1.4, 0, 0, 4)  # rk order
     with pytest.raises(ValueError):
-        fxo.OraclePlan((8, 1, 1), 4, 1, 1.4, 0, 0, 2, nvars=6)
+        fxo.OraclePlan((8, 1, 1), 4, 1, 1.4, 0, 0, 2, nvars=4)
+    with pytest.raises(ValueError):
+        fxo.OraclePlan((8, 1, 1), 4, 1, 1.4, 0, 0, 2, nvars=33)  # more than 27 passive scalars [B11]
