@@ -35,7 +35,8 @@ extern "C" {
 #define FX_OK 0
 #define FX_ERR_INVALID_ARG (-1)
 #define FX_ERR_STATE (-2)       /* call order: topology or workspace not set */
-#define FX_ERR_UNSUPPORTED (-3) /* coarse/fine neighbour relation, nvars != 5, ... */
+#define FX_ERR_UNSUPPORTED (-3) /* coarse/fine neighbour relation, nvars > FX_MAX_NVARS, ... */
+#define FX_MAX_NVARS 32     /* 5 hydro variables + at most 27 passive mass scalars [B11] */
 #define FX_ERR_WORKSPACE (-4)   /* workspace missing, too small or not 256-byte aligned */
 #define FX_ERR_CUDA (-5)        /* a CUDA runtime call or launch failed; see fx_last_error() */
 
@@ -88,10 +89,14 @@ typedef struct fx_layout {
 const char *fx_last_error(void);
 
 /* Plan: a host object owned by the library, freed by fx_hydro_plan_destroy.
- * block_dims = interior zones (nx, ny, nz) per block; nvars must be 5 (rho, m_x, m_y, m_z, E) [A1];
+ * block_dims = interior zones (nx, ny, nz) per block; nvars = 5 + ns: (rho, m_x, m_y, m_z, E) [A1] followed by ns
+ * passive mass scalars rho*X_s ("a perfect-gas EOS with a multispecies variant"; reading B11):
+ * X_s = rho X_s / rho is reconstructed like the other primitives and gets from the Riemann solver the flux of an
+ * advected quantity (for HLLC: the upwind X_s times the mass flux); no floor, no source term, not in the time step;
+ * copied unchanged into guard zones (walls included).  Plans with ns > 0 run on the generic path (fx_hydro_plan_path = 0);
  * recon FX_RECON_*; riemann FX_RIEMANN_*; rk_order 2 or 3 (SSP-RK).
  * FX_ERR_INVALID_ARG: a dim < 1; no active dim; nguard < 2 (PLM) or < 3 (WENO5); nguard > an active
- * block dim; gamma <= 1; nblocks < 0; unknown enum.  FX_ERR_UNSUPPORTED: nvars != 5. */
+ * block dim; gamma <= 1; nblocks < 0; unknown enum; nvars < 5.  FX_ERR_UNSUPPORTED: nvars > FX_MAX_NVARS. */
 int fx_hydro_plan_create(fx_hydro_plan **out, const int block_dims[3], int nguard, int nvars, int64_t nblocks,
                          double gamma, int recon, int riemann, int rk_order);
 int fx_hydro_plan_destroy(fx_hydro_plan *plan);

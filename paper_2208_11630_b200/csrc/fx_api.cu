@@ -45,7 +45,10 @@ extern "C" int fx_hydro_plan_create(fx_hydro_plan **out, const int block_dims[3]
                                     int64_t nblocks, double gamma, int recon, int riemann, int rk_order) {
   if (!out || !block_dims) return fx_fail(FX_ERR_INVALID_ARG, "plan_create: null argument");
   *out = nullptr;
-  if (nvars != 5) return fx_fail(FX_ERR_UNSUPPORTED, "plan_create: nvars must be 5 (rho, mx, my, mz, E), got %d", nvars);
+  if (nvars < 5) return fx_fail(FX_ERR_INVALID_ARG, "plan_create: nvars must be at least 5 (rho, mx, my, mz, E), got %d", nvars);
+  if (nvars > FX_MAX_NVARS)
+    return fx_fail(FX_ERR_UNSUPPORTED, "plan_create: nvars = %d: at most %d passive scalars after the 5 hydro variables",
+                   nvars, FX_MAX_NVARS - 5);
   if (nblocks < 0 || nblocks > 2147483647LL) return fx_fail(FX_ERR_INVALID_ARG, "plan_create: nblocks out of range");
   if (!(gamma > 1.0) || !isfinite(gamma)) return fx_fail(FX_ERR_INVALID_ARG, "plan_create: gamma must be > 1");
   if (recon != FX_RECON_PLM_MINMOD && recon != FX_RECON_WENO5) return fx_fail(FX_ERR_INVALID_ARG, "plan_create: unknown reconstruction %d", recon);
@@ -95,6 +98,7 @@ extern "C" int fx_hydro_plan_create(fx_hydro_plan **out, const int block_dims[3]
   p->zchain = 0;  // auto
   p->nguard = nguard;
   p->nvars = nvars;
+  p->P.nvars = nvars;
   p->rk = rk_order;
   *out = p;
   return FX_OK;
@@ -173,6 +177,7 @@ extern "C" int fx_hydro_plan_set_option(fx_hydro_plan *plan, int key, double val
 
 extern "C" int fx_hydro_plan_path(const fx_hydro_plan *plan) {
   if (!plan) return fx_fail(FX_ERR_INVALID_ARG, "plan_path: null plan");
+  if (plan->nvars > 5) return 0;  // passive scalars [B11] are carried by the generic path only
   if (plan->path_option == 0 && fx_stage_tma_supported(plan->P)) return 1;
   if (plan->path_option != 1 && fx_stage_tile_supported(plan->P)) return 2;
   return 0;

@@ -8,10 +8,11 @@
 // checked against; it is not the roofline path.
 #include "fx_physics.cuh"
 
-// Face flux of direction d at the face whose left cell is element cL of X (variable-0 index).
+// Face flux of direction d at the face whose left cell is element cL of X (variable-0 index).  Aq: what the passive
+// scalars need from the solve (fx_riemann); fb: which sides took the WENO5 positivity fallback (bit 0 left, bit 1 right).
 template <int RECON, int RIEMANN>
 __device__ __forceinline__ unsigned fx_face_flux_global(const FxParams &P, const double *__restrict__ X, long long cL,
-                                                        int d, long long s, double F[5]) {
+                                                        int d, long long s, double F[5], double &Aq, unsigned &fb) {
   constexpr int R = (RECON == FX_RECON_PLM_MINMOD) ? 2 : 3;  // cells each side of the face
   double W[2 * R][5];
   unsigned hit = 0;
@@ -35,20 +36,23 @@ __device__ __forceinline__ unsigned fx_face_flux_global(const FxParams &P, const
       WR[f] = fx_weno5(W[5][v], W[4][v], W[3][v], W[2][v], W[1][v], P.weno_eps);
     }
   }
+  fb = 0;
   if (RECON == FX_RECON_WENO5) {  // positivity fallback per side [A6]
     if (!(WL[0] > 0.0) || !(WL[4] > 0.0)) {
 #pragma unroll
       for (int f = 0; f < 5; ++f) WL[f] = W[R - 1][map[f]];
       hit |= FX_STATUS_WENO_FALLBACK;
+      fb |= 1u;
     }
     if (!(WR[0] > 0.0) || !(WR[4] > 0.0)) {
 #pragma unroll
       for (int f = 0; f < 5; ++f) WR[f] = W[R][map[f]];
       hit |= FX_STATUS_WENO_FALLBACK;
+      fb |= 2u;
     }
   }
   double Ff[5];
-  fx_riemann<RIEMANN>(P, WL, WR, Ff);
+  fx_riemann<RIEMANN>(P, WL, WR, Ff, Aq);
   F[0] = Ff[0];
   F[in] = Ff[1];
   F[it1] = Ff[2];
@@ -57,6 +61,39 @@ __device__ __forceinline__ unsigned fx_face_flux_global(const FxParams &P, const
   const double sum = Ff[0] + Ff[1] + Ff[2] + Ff[3] + Ff[4];
   if (!(fabs(sum) <= 1.79e308)) hit |= FX_STATUS_NONFINITE;
   return hit & (FX_STATUS_NONFINITE | FX_STATUS_WENO_FALLBACK);  // floors are counted where a zone is owned
+}
+
+template <int RECON, int RIEMANN>
+__device__ __forceinline__ unsigned fx_face_flux_global(const FxParams &P, const double *__restrict__ X, long long cL,
+                                                        int d, long long s, double F[5]) {
+  double Aq;
+  unsigned fb;
+  return fx_face_flux_global<RECON, RIEMANN>(P, X, cL, d, s, F, Aq, fb);
+}
+
+// Passive scalar [B11]: left / right abundances X = (rho X) / rho at the face whose left cell is cL, reconstructed like
+// every other primitive (Q = the scalar's slab, X = the density's); a side that took the positivity fallback keeps
+// its cell value.
+template <int RECON>
+__device__ __forceinline__ void fx_scalar_face(const FxParams &P, const double *__restrict__ X,
+                                               const double *__restrict__ Q, long long cL, long long s, unsigned fb,
+                                               double &qL, double &qR) {
+  constexpr int R = (RECON == FX_RECON_PLM_MINMOD) ? 2 : 3;
+  double x[2 * R];
+#pragma unroll
+  for (int m = 0; m < 2 * R; ++m) {
+    const long long c = cL + (m - (R - 1)) * s;
+    double rho = X[c];
+    if (rho < P.rho_floor) rho = P.rho_floor;
+    x[m] = Q[c] * (1.0 / rho);
+  }
+  if (RECON == FX_RECON_PLM_MINMOD) {
+    qL = x[1] + 0.5 * fx_minmod(x[1] - x[0], x[2] - x[1]);
+    qR = x[2] - 0.5 * fx_minmod(x[2] - x[1], x[3] - x[2]);
+  } else {
+    qL = (fb & 1u) ? x[R - 1] : fx_weno5(x[0], x[1], x[2], x[3], x[4], P.weno_eps);
+    qR = (fb & 2u) ? x[R] : fx_weno5(x[5], x[4], x[3], x[2], x[1], P.weno_eps);
+  }
 }
 
 template <int RECON, int RIEMANN>
@@ -76,6 +113,8 @@ __global__ void __launch_bounds__(128) fx_k_generic_stage(FxParams P, const doub
   if (dt_dev) dt = *dt_dev;
   const long long stride[3] = {1, P.S_j, P.S_k};
   double S[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+  double qA[3][2], qF[3][2];  // per direction and face (low, high): scalar coefficient and mass flux [B11]
+  unsigned qfb = 0;           // 4 bits per direction: fallback sides of the low and the high face
   unsigned hit = 0;
   {  // floors are counted once per owned zone
     double W[5];
@@ -87,10 +126,14 @@ __global__ void __launch_bounds__(128) fx_k_generic_stage(FxParams P, const doub
     if (!P.active[d]) continue;
     const double rd = dt / __ldg(&dx[b * 3 + d]);
     double Fm[5], Fp[5];
-    hit |= fx_face_flux_global<RECON, RIEMANN>(P, X, c - stride[d], d, stride[d], Fm);
-    hit |= fx_face_flux_global<RECON, RIEMANN>(P, X, c, d, stride[d], Fp);
+    unsigned fbm, fbp;
+    hit |= fx_face_flux_global<RECON, RIEMANN>(P, X, c - stride[d], d, stride[d], Fm, qA[d][0], fbm);
+    hit |= fx_face_flux_global<RECON, RIEMANN>(P, X, c, d, stride[d], Fp, qA[d][1], fbp);
 #pragma unroll
     for (int v = 0; v < 5; ++v) S[v] += rd * (Fp[v] - Fm[v]);
+    qF[d][0] = Fm[0];
+    qF[d][1] = Fp[0];
+    qfb |= (fbm | (fbp << 2)) << (4 * d);
   }
   if (P.grav_on) {  // constant-gravity source of the stage input's own zone [B10]
     const double rho = X[c];
@@ -108,6 +151,28 @@ __global__ void __launch_bounds__(128) fx_k_generic_stage(FxParams P, const doub
     const double u0 = U0[g];
     out[g] = first ? (u0 - S[v]) : (u0 + beta * ((X[g] - u0) - S[v]));
   }
+  // passive scalars [B11]: flux = Aq X_L + (mass flux - Aq) X_R at each of the zone's faces, same divergence and
+  // combination, no source term
+#pragma unroll 1
+  for (int sv = 5; sv < P.nvars; ++sv) {
+    const double *Q = X + sv * P.S_v;
+    double Ss = 0.0;
+#pragma unroll 1
+    for (int d = 0; d < 3; ++d) {
+      if (!P.active[d]) continue;
+      const double rd = dt / __ldg(&dx[b * 3 + d]);
+      double mL, mR, pL, pR;
+      fx_scalar_face<RECON>(P, X, Q, c - stride[d], stride[d], (qfb >> (4 * d)) & 3u, mL, mR);
+      fx_scalar_face<RECON>(P, X, Q, c, stride[d], (qfb >> (4 * d + 2)) & 3u, pL, pR);
+      const double Fm = qA[d][0] * mL + (qF[d][0] - qA[d][0]) * mR;
+      const double Fp = qA[d][1] * pL + (qF[d][1] - qA[d][1]) * pR;
+      if (!(fabs(Fm + Fp) <= 1.79e308)) hit |= FX_STATUS_NONFINITE;
+      Ss += rd * (Fp - Fm);
+    }
+    const long long g = sv * P.S_v + c;
+    const double u0 = U0[g];
+    out[g] = first ? (u0 - Ss) : (u0 + beta * ((Q[c] - u0) - Ss));
+  }
   if (hit) fx_note(P, hit);
 }
 
@@ -124,11 +189,19 @@ __global__ void __launch_bounds__(128) fx_k_debug_fluxes(FxParams P, const doubl
   cc[dir] -= 1;  // left cell of face f is padded cell gd + f - 1 [A17]
   const long long stride[3] = {1, P.S_j, P.S_k};
   const long long cL = b * P.S_b + cc[2] * P.S_k + cc[1] * P.S_j + cc[0];
-  double Ff[5];
-  unsigned hit = fx_face_flux_global<RECON, RIEMANN>(P, U, cL, dir, stride[dir], Ff);
+  double Ff[5], Aq;
+  unsigned fb;
+  unsigned hit = fx_face_flux_global<RECON, RIEMANN>(P, U, cL, dir, stride[dir], Ff, Aq, fb);
   const long long FS_v = per_block * P.nblocks;
 #pragma unroll
   for (int v = 0; v < 5; ++v) F[v * FS_v + z] = Ff[v];
+  for (int sv = 5; sv < P.nvars; ++sv) {  // passive scalars [B11]
+    double qL, qR;
+    fx_scalar_face<RECON>(P, U, U + sv * P.S_v, cL, stride[dir], fb, qL, qR);
+    const double Fs = Aq * qL + (Ff[0] - Aq) * qR;
+    if (!(fabs(Fs) <= 1.79e308)) hit |= FX_STATUS_NONFINITE;
+    F[sv * FS_v + z] = Fs;
+  }
   if (hit) fx_note(P, hit);
 }
 

@@ -20,6 +20,7 @@ __global__ void __launch_bounds__(256) fx_k_fill_guardcells(FxParams P, double *
     const double x = U[v * P.S_v + s];
     U[v * P.S_v + t] = (v >= 1 && v <= 3 && ((flip >> (v - 1)) & 1u)) ? -x : x;
   }
+  for (int v = 5; v < P.nvars; ++v) U[v * P.S_v + t] = U[v * P.S_v + s];  // passive scalars: copied, never negated [B11]
 }
 
 __global__ void __launch_bounds__(256) fx_k_index_map(FxParams P, long long b0, long long nb, long long *__restrict__ src) {
@@ -62,6 +63,8 @@ __global__ void __launch_bounds__(256) fx_k_fill_guardcells_pairs(FxParams P, do
       if (v >= 1 && v <= 3 && ((f0 >> (v - 1)) & 1u)) { x.x = -x.x; x.y = -x.y; }
       *reinterpret_cast<double2 *>(U + v * P.S_v + t) = x;
     }
+    for (int v = 5; v < P.nvars; ++v)  // passive scalars [B11]
+      *reinterpret_cast<double2 *>(U + v * P.S_v + t) = *reinterpret_cast<const double2 *>(U + v * P.S_v + s0);
   } else {
 #pragma unroll
     for (int v = 0; v < 5; ++v) {
@@ -69,6 +72,8 @@ __global__ void __launch_bounds__(256) fx_k_fill_guardcells_pairs(FxParams P, do
       const bool n0 = v >= 1 && v <= 3 && ((f0 >> (v - 1)) & 1u), n1 = v >= 1 && v <= 3 && ((f1 >> (v - 1)) & 1u);
       *reinterpret_cast<double2 *>(U + v * P.S_v + t) = make_double2(n0 ? -x0 : x0, n1 ? -x1 : x1);
     }
+    for (int v = 5; v < P.nvars; ++v)
+      *reinterpret_cast<double2 *>(U + v * P.S_v + t) = make_double2(U[v * P.S_v + s0], U[v * P.S_v + s1]);
   }
 }
 
@@ -105,7 +110,7 @@ __global__ void __launch_bounds__(256) fx_k_pack_interior(FxParams P, double *__
 }
 
 int fx_launch_pack_interior(const FxParams &P, double *U, double *packed, int to_packed, cudaStream_t st) {
-  const long long n = 5LL * P.nblocks * P.n[0] * P.n[1] * P.n[2];
+  const long long n = (long long)P.nvars * P.nblocks * P.n[0] * P.n[1] * P.n[2];
   if (n == 0) return FX_OK;
   const long long want = (n + 255) / 256;
   const unsigned grid = (unsigned)(want < 148LL * 32 ? want : 148LL * 32);

@@ -11,6 +11,7 @@ struct FxParams {
   int gd[3];      // guard depth per dimension (0 if inactive)
   int np[3];      // padded extents
   int active[3];
+  int nvars;      // 5 hydro variables + passive mass scalars [B11]
   long long S_j, S_k, S_b, S_v;  // element strides of U[v][b][k][j][i]
   long long nblocks;
   double gamma, gm1, igm1;

@@ -57,8 +57,14 @@ def test_plan_create_argument_checks():
     assert create((16, 16, 16), 4, 8, recon=2)[0] == fx.ERR_INVALID_ARG
     assert create((16, 16, 16), 4, 8, riemann=7)[0] == fx.ERR_INVALID_ARG
     assert create((16, 16, 16), 4, -1)[0] == fx.ERR_INVALID_ARG
-    assert create((16, 16, 16), 4, 8, nvars=6)[0] == fx.ERR_UNSUPPORTED
+    assert create((16, 16, 16), 4, 8, nvars=4)[0] == fx.ERR_INVALID_ARG
+    assert create((16, 16, 16), 4, 8, nvars=33)[0] == fx.ERR_UNSUPPORTED   # more than 27 passive scalars [B11]
     assert b"nvars" in fx.lib().fx_last_error()
+    rc, h = create((16, 16, 16), 4, 8, nvars=9)
+    assert rc == 0 and fx.lib().fx_hydro_plan_path(h) == 0                  # scalars ride on the generic path
+    L = fx.Layout()
+    assert fx.lib().fx_hydro_plan_layout(h, C.byref(L)) == 0 and L.bytes_per_state == 9 * 8 * 24 ** 3 * 8
+    fx.lib().fx_hydro_plan_destroy(h)
 
 
 @pytest.mark.parametrize("dims,g,nb", [((16, 16, 16), 4, 32768), ((256, 1, 1), 4, 1), ((16, 16, 1), 4, 64), ((8, 8, 8), 3, 5)])

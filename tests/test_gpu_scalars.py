@@ -1,0 +1,135 @@
+"""GPU <-> oracle parity of the passive mass scalars (reading B11; run on the B200 box: pytest -m gpu).
+Tolerances as for the hydro variables [NS]: <= 1e-12 after one RK step, <= 1e-9 after 10 steps; the error of a
+scalar zone is |d(rho X_s)| / rho with the oracle's density (X_s is of order one), the hydro variables keep the
+metric A21.  Guard-cell fill of all nvars variables bit-exact."""
+import numpy as np
+import pytest
+import torch
+
+from paper_2208_11630_b200 import inputs
+from tests.helpers import gpu_plan_for, oracle_plan_for, rel_err
+
+pytestmark = pytest.mark.gpu
+
+TOL_1, TOL_10 = 1e-12, 1e-9
+
+
+def setup(number, nb, ns, **kw):
+    cfg = inputs.config(number, nb=nb)
+    oplan, neigh, coords = oracle_plan_for(cfg, nvars=5 + ns, **kw)
+    gplan, gneigh, gcoords = gpu_plan_for(cfg, nvars=5 + ns, **kw)
+    assert np.array_equal(neigh, gneigh) and np.array_equal(coords, gcoords)
+    Ui = inputs.with_scalars(cfg, coords, inputs.block_interiors(cfg, coords), ns)
+    return cfg, oplan, gplan, inputs.embed(cfg, Ui), inputs.dx_array(cfg)
+
+
+def scalar_err(got, ref):
+    """got / ref: interiors [5 + ns, ...]."""
+    if not np.all(np.isfinite(got)):
+        return float("inf")
+    return float((np.abs(got[5:] - ref[5:]) / ref[0]).max())
+
+
+CASES = [  # number, nb, ns, kwargs
+    (1, None, 2, {}), (2, None, 3, {}), (3, (2, 2, 2), 1, {}), (4, (2, 2, 2), 2, {}), (5, (3, 3, 3), 4, {}),
+    (5, (2, 2, 2), 2, dict(riemann=0, rk=3)), (5, (2, 2, 2), 3, dict(recon=1, riemann=0)),
+    (2, (3, 2, 1), 2, dict(recon=1, rk=3)), (5, (2, 2, 2), 2, dict(bc="outflow")),
+    (5, (2, 2, 2), 2, dict(bc="reflect")), (2, (2, 2, 1), 27, dict(bc="reflect", riemann=0)),
+    (1, None, 1, dict(bc="reflect", riemann=1)),
+]
+
+
+@pytest.mark.parametrize("number,nb,ns,kw", CASES)
+def test_advance_1_and_10_steps(number, nb, ns, kw):
+    cfg, oplan, gplan, Uh, dx = setup(number, nb, ns, **kw)
+    assert gplan.path == 0  # scalars ride on the generic path
+    Uo = Uh.numpy().copy()
+    Ud = Uh.cuda()
+    dxd = torch.from_numpy(dx).cuda()
+    for step in range(10):
+        dt = oplan.compute_dt(Uo, dx, cfg.cfl)
+        if step == 0:
+            dt_g = float(gplan.fx_hydro_compute_dt(Ud, dxd, cfg.cfl).item())
+            assert abs(dt_g - dt) <= 1e-14 * dt
+        oplan.advance(Uo, dx, dt)
+        gplan.fx_hydro_advance(Ud, dxd, dt)
+        if step in (0, 9):
+            got, ref = gplan.interior(Ud).cpu().numpy(), oplan.interior(Uo)
+            tol = TOL_1 if step == 0 else TOL_10
+            assert rel_err(cfg, got[:5], ref[:5]) <= tol
+            assert scalar_err(got, ref) <= tol, (step, scalar_err(got, ref))
+    assert not np.array_equal(oplan.interior(Uo)[5:], gplan.interior(Uh).numpy()[5:])  # the scalars moved
+    fo, _ = oplan.status()
+    fg, _ = gplan.fx_hydro_status()
+    assert fo == fg, (fo, fg)
+
+
+def test_hydro_variables_do_not_see_the_scalars_and_paths_agree():
+    """The hydro variables of a run with scalars are bit for bit those of the generic path without them, and within
+    rounding those of the fused path."""
+    cfg, oplan, gplan, Uh, dx = setup(5, (2, 2, 2), 3)
+    g5, _, _ = gpu_plan_for(cfg, path=1)
+    gf, _, _ = gpu_plan_for(cfg)
+    assert g5.path == 0 and gf.path == 1
+    dxd = torch.from_numpy(dx).cuda()
+    A, B, C = Uh.cuda(), Uh[:5].contiguous().cuda(), Uh[:5].contiguous().cuda()
+    for _ in range(3):
+        dt = float(g5.fx_hydro_compute_dt(B, dxd, cfg.cfl).item())
+        gplan.fx_hydro_advance(A, dxd, dt)
+        g5.fx_hydro_advance(B, dxd, dt)
+        gf.fx_hydro_advance(C, dxd, dt)
+    assert torch.equal(gplan.interior(A)[:5], g5.interior(B))
+    assert rel_err(cfg, gf.interior(C).cpu().numpy(), g5.interior(B).cpu().numpy()) <= 1e-12
+
+
+@pytest.mark.parametrize("dims,g,nb,bc", [((6, 4, 5), 3, (2, 1, 2), "reflect"), ((16, 16, 16), 4, (2, 2, 1), "periodic"),
+                                          ((12, 1, 1), 4, (2, 1, 1), "outflow"), ((7, 6, 1), 3, (2, 2, 1), "reflect")])
+def test_guard_fill_of_all_variables_bit_exact(dims, g, nb, bc):
+    cfg = inputs.config(3)
+    cfg.block_dims, cfg.nguard, cfg.nb, cfg.bc = dims, g, nb, bc
+    oplan, neigh, coords = oracle_plan_for(cfg, nvars=8)
+    gplan, _, _ = gpu_plan_for(cfg, nvars=8)
+    rng = np.random.default_rng(7)
+    Uh = np.full(oplan.shape, np.nan)
+    oplan.interior(Uh)[...] = rng.normal(size=oplan.interior(Uh).shape)
+    Ud = torch.from_numpy(Uh).cuda()
+    oplan.fill_guardcells(Uh)
+    gplan.fx_fill_guardcells(Ud)
+    assert np.array_equal(Ud.cpu().numpy(), Uh)
+    assert not np.isnan(Uh).any()
+
+
+@pytest.mark.parametrize("number,nb,recon,riemann", [(2, (2, 2, 1), 0, 1), (5, (2, 2, 2), 1, 1), (4, (2, 2, 2), 1, 0),
+                                                     (5, (2, 2, 2), 0, 0)])
+def test_debug_fluxes(number, nb, recon, riemann):
+    cfg, oplan, gplan, Uh, dx = setup(number, nb, 3, recon=recon, riemann=riemann)
+    Un = Uh.numpy().copy()
+    oplan.fill_guardcells(Un)
+    Ud = torch.from_numpy(Un).cuda()
+    for d in range(3):
+        if cfg.block_dims[d] == 1:
+            continue
+        Fo = oplan.debug_compute_fluxes(Un, d)
+        Fg = gplan.fx_debug_compute_fluxes(Ud, d).cpu().numpy()
+        assert Fg.shape == Fo.shape and Fo.shape[0] == 8
+        # rounding scale of an advected flux: density times the fastest signal speed
+        W = oplan.interior(Un)
+        scale = float((np.abs(W[1:4]).sum(axis=0) + np.sqrt(cfg.gamma * W[0] * W[4])).max())
+        assert np.all(np.abs(Fg[5:] - Fo[5:]) <= 1e-13 * scale)
+        assert np.abs(Fo[5:]).max() > 0
+
+
+def test_host_interior_call_carries_the_scalars():
+    """fx_hydro_advance_host_interior with nvars = 7: the packed host buffer holds all seven variables."""
+    cfg, oplan, gplan, Uh, dx = setup(2, (2, 2, 1), 2)
+    Uo = Uh.numpy().copy()
+    nsteps = 3
+    for _ in range(nsteps):
+        oplan.advance(Uo, dx, oplan.compute_dt(Uo, dx, cfg.cfl))
+    Uint = gplan.interior(Uh).contiguous().pin_memory()
+    U_stage = gplan.alloc_state()
+    packed = torch.empty(gplan.interior_shape, dtype=torch.float64, device="cuda")
+    dx_stage = torch.empty((gplan.nblocks, 3), dtype=torch.float64, device="cuda")
+    gplan.fx_hydro_advance_host_interior(Uint, torch.from_numpy(dx), cfg.cfl, nsteps, U_stage, packed, dx_stage)
+    got, ref = Uint.numpy(), oplan.interior(Uo)
+    assert rel_err(cfg, got[:5], ref[:5]) <= 1e-11 and scalar_err(got, ref) <= 1e-11
