@@ -50,6 +50,8 @@ def parse_args():
     ap.add_argument("--guard-x", type=int, default=-1, help="FX_OPT_GUARD_X: x guard depth (layout); -1 = 8 for 16-wide blocks with 4 guard zones "
                     "(256-byte row pitch, interior rows on 128-byte lines), else the config's nguard")
     ap.add_argument("--order", default="morton", choices=["lex", "morton"])
+    ap.add_argument("--scalars", type=int, default=0, help="passive mass scalars carried with the 5 hydro variables (DESIGN.md B11; "
+                    "nvars = 5 + this; generic path)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=2)
@@ -141,7 +143,7 @@ def build_workload(args, device):
     bcs = [code if cfg.block_dims[d] > 1 else fx.TOPO_NONE for d in range(3)]
     neigh, coords = fx.fx_topology_cartesian(cfg.nb, bcs, bcs, order)
     plan = fx.HydroPlan(cfg.block_dims, cfg.nguard, cfg.nblocks, cfg.gamma, cfg.recon, cfg.riemann, cfg.rk_order,
-                        device=device)
+                        nvars=5 + args.scalars, device=device)
     plan.fx_hydro_plan_set_option(fx.OPT_PATH, args.path)
     guard_x = args.guard_x if args.guard_x >= 0 else (8 if (cfg.block_dims[0] == 16 and cfg.nguard == 4) else cfg.nguard)
     if guard_x != cfg.nguard:
@@ -155,7 +157,7 @@ def build_workload(args, device):
     chunk = 1024
     for b0 in range(0, cfg.nblocks, chunk):
         b1 = min(cfg.nblocks, b0 + chunk)
-        Ui[:, b0:b1] = inputs.block_interiors(cfg, coords[b0:b1], device)
+        Ui[:, b0:b1] = inputs.with_scalars(cfg, coords[b0:b1], inputs.block_interiors(cfg, coords[b0:b1], device), args.scalars)
     dx = torch.from_numpy(inputs.dx_array(cfg)).to(device)
     return cfg, plan, U, dx, coords
 
@@ -173,9 +175,10 @@ def oracle_sample(args, target_seconds=15.0, steps=None):
     code = fxo.TOPO_PERIODIC if cfg.bc == "periodic" else fxo.TOPO_OUTFLOW
     bcs = [code if cfg.block_dims[d] > 1 else fxo.TOPO_NONE for d in range(3)]
     neigh, coords = fxo.topology_cartesian(cfg.nb, bcs, bcs, fxo.ORDER_LEX)
-    plan = fxo.OraclePlan(cfg.block_dims, cfg.nguard, cfg.nblocks, cfg.gamma, cfg.recon, cfg.riemann, cfg.rk_order)
+    plan = fxo.OraclePlan(cfg.block_dims, cfg.nguard, cfg.nblocks, cfg.gamma, cfg.recon, cfg.riemann, cfg.rk_order,
+                          nvars=5 + args.scalars)
     plan.set_topology(neigh)
-    U = inputs.embed(cfg, inputs.block_interiors(cfg, coords)).numpy()
+    U = inputs.embed(cfg, inputs.with_scalars(cfg, coords, inputs.block_interiors(cfg, coords), args.scalars)).numpy()
     dx = inputs.dx_array(cfg)
     cores = len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1)
 
@@ -268,7 +271,8 @@ def run_ours(args, rank, world, local_rank):
 
     # roofline of the dominant kernel (the stage kernel): algorithmic bytes per launch / its mean duration
     peak, peak_src = measured_peaks()
-    alg_bytes_stage = [80.0] + [120.0] * (stages - 1)  # B per zone: read X (+U0), write out
+    # B per zone: read X (+U0), write out, 8 B each per variable
+    alg_bytes_stage = [16.0 * (5 + args.scalars)] + [24.0 * (5 + args.scalars)] * (stages - 1)
     alg_bytes_per_launch = zones * sum(alg_bytes_stage) / stages
     stage_avg_ms = stage_ms / max(stage_launches, 1)
     achieved = alg_bytes_per_launch / (stage_avg_ms * 1e-3) / 1e9
@@ -294,7 +298,8 @@ def run_ours(args, rank, world, local_rank):
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": f"config {cfg.number}: {cfg.name}, {cfg.nblocks} blocks of "
                                    f"{cfg.block_dims[0]}x{cfg.block_dims[1]}x{cfg.block_dims[2]} (+{cfg.nguard} guard), "
-                                   f"{'WENO5' if cfg.recon else 'PLM-minmod'}+{'HLLC' if cfg.riemann else 'HLLE'}, SSP-RK{stages}",
+                                   f"{'WENO5' if cfg.recon else 'PLM-minmod'}+{'HLLC' if cfg.riemann else 'HLLE'}, SSP-RK{stages}"
+                                   + (f", {args.scalars} passive mass scalars" if args.scalars else ""),
                        "interior_zones": zones, "state_bytes": plan.bytes_per_state, "block_order": args.order,
                        "layout": f"x guard depth {plan.gd[0]} (row pitch {plan.S_j * 8} B), y/z guard depth {plan.gd[1]}/{plan.gd[2]}",
                        "path": {0: "generic", 1: "fused (TMA)", 2: "tile (shared-memory block)"}[plan.path], "l2": "inputs (state) larger than L2; no flush needed",

@@ -96,6 +96,26 @@ __device__ __forceinline__ void fx_scalar_face(const FxParams &P, const double *
   }
 }
 
+// The same for the two faces of one zone from the 2R+1 abundances x[0..2R] centred on it (x[R] is the zone): low face
+// between x[R-1] and x[R], high face between x[R] and x[R+1].
+template <int RECON>
+__device__ __forceinline__ void fx_scalar_faces_of_zone(const double *x, double eps, unsigned fbm, unsigned fbp,
+                                                        double &mL, double &mR, double &pL, double &pR) {
+  if (RECON == FX_RECON_PLM_MINMOD) {
+    const double s0 = fx_minmod(x[1] - x[0], x[2] - x[1]), s1 = fx_minmod(x[2] - x[1], x[3] - x[2]),
+                 s2 = fx_minmod(x[3] - x[2], x[4] - x[3]);
+    mL = x[1] + 0.5 * s0;
+    mR = x[2] - 0.5 * s1;
+    pL = x[2] + 0.5 * s1;
+    pR = x[3] - 0.5 * s2;
+  } else {
+    mL = (fbm & 1u) ? x[2] : fx_weno5(x[0], x[1], x[2], x[3], x[4], eps);
+    mR = (fbm & 2u) ? x[3] : fx_weno5(x[5], x[4], x[3], x[2], x[1], eps);
+    pL = (fbp & 1u) ? x[3] : fx_weno5(x[1], x[2], x[3], x[4], x[5], eps);
+    pR = (fbp & 2u) ? x[4] : fx_weno5(x[6], x[5], x[4], x[3], x[2], eps);
+  }
+}
+
 template <int RECON, int RIEMANN>
 __global__ void __launch_bounds__(128) fx_k_generic_stage(FxParams P, const double *__restrict__ X,
                                                           const double *U0, double *out,
@@ -113,7 +133,9 @@ __global__ void __launch_bounds__(128) fx_k_generic_stage(FxParams P, const doub
   if (dt_dev) dt = *dt_dev;
   const long long stride[3] = {1, P.S_j, P.S_k};
   double S[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+  constexpr int RS = (RECON == FX_RECON_PLM_MINMOD) ? 2 : 3;
   double qA[3][2], qF[3][2];  // per direction and face (low, high): scalar coefficient and mass flux [B11]
+  double qri[3][2 * RS + 1];  // 1 / rho of the zone's stencil cells per direction (scalars only)
   unsigned qfb = 0;           // 4 bits per direction: fallback sides of the low and the high face
   unsigned hit = 0;
   {  // floors are counted once per owned zone
@@ -134,6 +156,14 @@ __global__ void __launch_bounds__(128) fx_k_generic_stage(FxParams P, const doub
     qF[d][0] = Fm[0];
     qF[d][1] = Fp[0];
     qfb |= (fbm | (fbp << 2)) << (4 * d);
+    if (P.nvars > 5) {
+#pragma unroll
+      for (int m = 0; m <= 2 * RS; ++m) {
+        double rho = X[c + (m - RS) * stride[d]];
+        if (rho < P.rho_floor) rho = P.rho_floor;
+        qri[d][m] = 1.0 / rho;
+      }
+    }
   }
   if (P.grav_on) {  // constant-gravity source of the stage input's own zone [B10]
     const double rho = X[c];
@@ -161,9 +191,10 @@ __global__ void __launch_bounds__(128) fx_k_generic_stage(FxParams P, const doub
     for (int d = 0; d < 3; ++d) {
       if (!P.active[d]) continue;
       const double rd = dt / __ldg(&dx[b * 3 + d]);
-      double mL, mR, pL, pR;
-      fx_scalar_face<RECON>(P, X, Q, c - stride[d], stride[d], (qfb >> (4 * d)) & 3u, mL, mR);
-      fx_scalar_face<RECON>(P, X, Q, c, stride[d], (qfb >> (4 * d + 2)) & 3u, pL, pR);
+      double mL, mR, pL, pR, x[2 * RS + 1];
+#pragma unroll
+      for (int m = 0; m <= 2 * RS; ++m) x[m] = Q[c + (m - RS) * stride[d]] * qri[d][m];
+      fx_scalar_faces_of_zone<RECON>(x, P.weno_eps, (qfb >> (4 * d)) & 3u, (qfb >> (4 * d + 2)) & 3u, mL, mR, pL, pR);
       const double Fm = qA[d][0] * mL + (qF[d][0] - qA[d][0]) * mR;
       const double Fp = qA[d][1] * pL + (qF[d][1] - qA[d][1]) * pR;
       if (!(fabs(Fm + Fp) <= 1.79e308)) hit |= FX_STATUS_NONFINITE;
