@@ -3,7 +3,9 @@
 // The generic path is: K1 full guard fill of the stage input, then this zone kernel: one thread per
 // interior zone computes the two face fluxes of each active direction from the padded stage input
 // (each face is evaluated by both zones that share it, bit-identically, so conservation holds to
-// rounding), forms S = sum_d dt/dx_d (F+ - F-) and the SSP-RK combination.  It is the path for block
+// rounding; the 2R+1 stencil cells of a direction are converted once and serve both faces), forms
+// S = sum_d dt/dx_d (F+ - F-) and the SSP-RK combination; then, for plans with passive scalars [B11], the same for
+// every scalar from the mass fluxes and coefficients the hydro part left in shared memory.  It is the path for block
 // shapes the fused kernel (fx_stage_tma.cu) does not cover (configs 1 and 2) and the scaffold its parity is
 // checked against; it is not the roofline path.
 #include "fx_physics.cuh"
@@ -116,12 +118,122 @@ __device__ __forceinline__ void fx_scalar_faces_of_zone(const double *x, double 
   }
 }
 
-template <int RECON, int RIEMANN>
-__global__ void __launch_bounds__(128) fx_k_generic_stage(FxParams P, const double *__restrict__ X,
+// Flux at the face between cells W[0 .. R-1] (left) and W[R .. 2R-1] (right) of a line of primitives along the
+// compile-time direction D, in the un-rotated variable order; the arithmetic of fx_face_flux_global, face by face.
+template <int RECON, int RIEMANN, int D>
+__device__ __forceinline__ unsigned fx_face_from_prims(const FxParams &P, const double (*W)[5], double F[5], double &Aq,
+                                                       unsigned &fb) {
+  constexpr int R = (RECON == FX_RECON_PLM_MINMOD) ? 2 : 3;
+  constexpr int in = 1 + D, it1 = 1 + (D + 1) % 3, it2 = 1 + (D + 2) % 3;
+  constexpr int map[5] = {0, in, it1, it2, 4};
+  unsigned hit = 0;
+  double WL[5], WR[5];
+#pragma unroll
+  for (int f = 0; f < 5; ++f) {
+    const int v = map[f];
+    if (RECON == FX_RECON_PLM_MINMOD) {
+      const double a = W[0][v], b = W[1][v], c = W[2][v], e = W[3][v];
+      WL[f] = b + 0.5 * fx_minmod(b - a, c - b);
+      WR[f] = c - 0.5 * fx_minmod(c - b, e - c);
+    } else {
+      WL[f] = fx_weno5(W[0][v], W[1][v], W[2][v], W[3][v], W[4][v], P.weno_eps);
+      WR[f] = fx_weno5(W[5][v], W[4][v], W[3][v], W[2][v], W[1][v], P.weno_eps);
+    }
+  }
+  fb = 0;
+  if (RECON == FX_RECON_WENO5) {  // positivity fallback per side [A6]
+    if (!(WL[0] > 0.0) || !(WL[4] > 0.0)) {
+#pragma unroll
+      for (int f = 0; f < 5; ++f) WL[f] = W[R - 1][map[f]];
+      hit |= FX_STATUS_WENO_FALLBACK;
+      fb |= 1u;
+    }
+    if (!(WR[0] > 0.0) || !(WR[4] > 0.0)) {
+#pragma unroll
+      for (int f = 0; f < 5; ++f) WR[f] = W[R][map[f]];
+      hit |= FX_STATUS_WENO_FALLBACK;
+      fb |= 2u;
+    }
+  }
+  double Ff[5];
+  fx_riemann<RIEMANN>(P, WL, WR, Ff, Aq);
+  F[0] = Ff[0];
+  F[in] = Ff[1];
+  F[it1] = Ff[2];
+  F[it2] = Ff[3];
+  F[4] = Ff[4];
+  const double sum = Ff[0] + Ff[1] + Ff[2] + Ff[3] + Ff[4];
+  if (!(fabs(sum) <= 1.79e308)) hit |= FX_STATUS_NONFINITE;
+  return hit;
+}
+
+// What the scalar loop of a zone needs from its hydro part, per direction, kept in shared memory (one column per
+// thread: conflict-free) so that it costs the hydro part no registers.
+template <int RECON> struct FxScalarShared {
+  static constexpr int RS = (RECON == FX_RECON_PLM_MINMOD) ? 2 : 3;
+  double A[3][2][128], F[3][2][128];  // per direction and face (low, high): scalar coefficient Aq and mass flux [B11]
+  double ri[3][2 * RS + 1][128];      // 1 / rho of the zone's stencil cells
+};
+
+// Direction D of one zone: the 2R+1 stencil cells are converted once and serve both faces.
+template <int RECON, int RIEMANN, int D, bool SCALARS>
+__device__ __forceinline__ unsigned fx_zone_direction(const FxParams &P, const double *__restrict__ X, long long c,
+                                                      long long s, double rd, double S[5], unsigned &qfb,
+                                                      FxScalarShared<RECON> *sh) {
+  constexpr int R = (RECON == FX_RECON_PLM_MINMOD) ? 2 : 3;
+  double W[2 * R + 1][5];
+  unsigned hit = 0;
+#pragma unroll
+  for (int m = 0; m <= 2 * R; ++m) {
+    const long long e = c + (m - R) * s;
+    hit |= fx_c2p(P, X[e], X[P.S_v + e], X[2 * P.S_v + e], X[3 * P.S_v + e], X[4 * P.S_v + e], W[m]);
+    if (SCALARS) sh->ri[D][m][threadIdx.x] = 1.0 / W[m][0];
+  }
+  hit &= FX_STATUS_NONFINITE;  // floors are counted where a zone is owned
+  double Fm[5], Fp[5], Am, Ap;
+  unsigned fbm, fbp;
+  hit |= fx_face_from_prims<RECON, RIEMANN, D>(P, &W[0], Fm, Am, fbm);
+  hit |= fx_face_from_prims<RECON, RIEMANN, D>(P, &W[1], Fp, Ap, fbp);
+#pragma unroll
+  for (int v = 0; v < 5; ++v) S[v] += rd * (Fp[v] - Fm[v]);
+  if (SCALARS) {
+    sh->A[D][0][threadIdx.x] = Am;
+    sh->A[D][1][threadIdx.x] = Ap;
+    sh->F[D][0][threadIdx.x] = Fm[0];
+    sh->F[D][1][threadIdx.x] = Fp[0];
+    qfb |= (fbm | (fbp << 2)) << (4 * D);
+  }
+  return hit;
+}
+
+// One scalar, direction D: r dt/dx (F+ - F-) with flux = Aq X_L + (mass flux - Aq) X_R [B11].
+template <int RECON, int D>
+__device__ __forceinline__ double fx_zone_scalar_direction(const FxParams &P, const double *__restrict__ Q, long long c,
+                                                           long long s, double rd, unsigned qfb,
+                                                           const FxScalarShared<RECON> *sh, unsigned &hit) {
+  constexpr int RS = (RECON == FX_RECON_PLM_MINMOD) ? 2 : 3;
+  double mL, mR, pL, pR, x[2 * RS + 1];
+#pragma unroll
+  for (int m = 0; m <= 2 * RS; ++m) x[m] = Q[c + (m - RS) * s] * sh->ri[D][m][threadIdx.x];
+  fx_scalar_faces_of_zone<RECON>(x, P.weno_eps, (qfb >> (4 * D)) & 3u, (qfb >> (4 * D + 2)) & 3u, mL, mR, pL, pR);
+  const double Am = sh->A[D][0][threadIdx.x], Ap = sh->A[D][1][threadIdx.x];
+  const double Fm = Am * mL + (sh->F[D][0][threadIdx.x] - Am) * mR;
+  const double Fp = Ap * pL + (sh->F[D][1][threadIdx.x] - Ap) * pR;
+  if (!(fabs(Fm + Fp) <= 1.79e308)) hit |= FX_STATUS_NONFINITE;
+  return rd * (Fp - Fm);
+}
+
+// Resident CTAs aimed at (measured at config 5 / config 4 on the generic path, ms per stage launch): PLM uncapped (150
+// registers, 3 CTAs) 38.3, 4 CTAs 34.0, 6 CTAs 31.3, 8 CTAs (64 registers) 30.0; WENO5 uncapped (246 registers) 15.2,
+// 4 CTAs 8.2, 5 CTAs 8.8, 6 CTAs 9.3 -- the kernel is latency-bound, the spills are cheaper than the lost warps.
+template <int RECON, int RIEMANN, bool SCALARS>
+__global__ void __launch_bounds__(128, RECON == FX_RECON_PLM_MINMOD ? 8 : 4) fx_k_generic_stage(FxParams P, const double *__restrict__ X,
                                                           const double *U0, double *out,
                                                           const double *__restrict__ dx, double dt,
                                                           const double *__restrict__ dt_dev, double beta, int first,
                                                           long long nzones) {
+  extern __shared__ __align__(16) unsigned char fx_generic_smem[];
+  FxScalarShared<RECON> *sh = reinterpret_cast<FxScalarShared<RECON> *>(fx_generic_smem);  // SCALARS only
   const long long z = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (z >= nzones) return;
   const int nx = P.n[0], ny = P.n[1], nz = P.n[2];
@@ -131,40 +243,20 @@ __global__ void __launch_bounds__(128) fx_k_generic_stage(FxParams P, const doub
   const int i = r % nx, j = (r / nx) % ny, k = r / (nx * ny);
   const long long c = b * P.S_b + (k + P.gd[2]) * P.S_k + (j + P.gd[1]) * P.S_j + (i + P.gd[0]);
   if (dt_dev) dt = *dt_dev;
-  const long long stride[3] = {1, P.S_j, P.S_k};
   double S[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
-  constexpr int RS = (RECON == FX_RECON_PLM_MINMOD) ? 2 : 3;
-  double qA[3][2], qF[3][2];  // per direction and face (low, high): scalar coefficient and mass flux [B11]
-  double qri[3][2 * RS + 1];  // 1 / rho of the zone's stencil cells per direction (scalars only)
-  unsigned qfb = 0;           // 4 bits per direction: fallback sides of the low and the high face
+  unsigned qfb = 0;  // 4 bits per direction: fallback sides of the low and the high face
   unsigned hit = 0;
   {  // floors are counted once per owned zone
     double W[5];
     hit |= fx_c2p(P, X[c], X[P.S_v + c], X[2 * P.S_v + c], X[3 * P.S_v + c], X[4 * P.S_v + c], W) &
            (FX_STATUS_RHO_FLOOR | FX_STATUS_P_FLOOR | FX_STATUS_NONFINITE);
   }
-#pragma unroll 1
-  for (int d = 0; d < 3; ++d) {
-    if (!P.active[d]) continue;
-    const double rd = dt / __ldg(&dx[b * 3 + d]);
-    double Fm[5], Fp[5];
-    unsigned fbm, fbp;
-    hit |= fx_face_flux_global<RECON, RIEMANN>(P, X, c - stride[d], d, stride[d], Fm, qA[d][0], fbm);
-    hit |= fx_face_flux_global<RECON, RIEMANN>(P, X, c, d, stride[d], Fp, qA[d][1], fbp);
-#pragma unroll
-    for (int v = 0; v < 5; ++v) S[v] += rd * (Fp[v] - Fm[v]);
-    qF[d][0] = Fm[0];
-    qF[d][1] = Fp[0];
-    qfb |= (fbm | (fbp << 2)) << (4 * d);
-    if (P.nvars > 5) {
-#pragma unroll
-      for (int m = 0; m <= 2 * RS; ++m) {
-        double rho = X[c + (m - RS) * stride[d]];
-        if (rho < P.rho_floor) rho = P.rho_floor;
-        qri[d][m] = 1.0 / rho;
-      }
-    }
-  }
+  const double rd0 = P.active[0] ? dt / __ldg(&dx[b * 3 + 0]) : 0.0;
+  const double rd1 = P.active[1] ? dt / __ldg(&dx[b * 3 + 1]) : 0.0;
+  const double rd2 = P.active[2] ? dt / __ldg(&dx[b * 3 + 2]) : 0.0;
+  if (P.active[0]) hit |= fx_zone_direction<RECON, RIEMANN, 0, SCALARS>(P, X, c, 1, rd0, S, qfb, sh);
+  if (P.active[1]) hit |= fx_zone_direction<RECON, RIEMANN, 1, SCALARS>(P, X, c, P.S_j, rd1, S, qfb, sh);
+  if (P.active[2]) hit |= fx_zone_direction<RECON, RIEMANN, 2, SCALARS>(P, X, c, P.S_k, rd2, S, qfb, sh);
   if (P.grav_on) {  // constant-gravity source of the stage input's own zone [B10]
     const double rho = X[c];
     double gm = 0.0;
@@ -181,28 +273,19 @@ __global__ void __launch_bounds__(128) fx_k_generic_stage(FxParams P, const doub
     const double u0 = U0[g];
     out[g] = first ? (u0 - S[v]) : (u0 + beta * ((X[g] - u0) - S[v]));
   }
-  // passive scalars [B11]: flux = Aq X_L + (mass flux - Aq) X_R at each of the zone's faces, same divergence and
-  // combination, no source term
+  if (SCALARS) {
+    // passive scalars [B11]: same divergence and combination, no source term
 #pragma unroll 1
-  for (int sv = 5; sv < P.nvars; ++sv) {
-    const double *Q = X + sv * P.S_v;
-    double Ss = 0.0;
-#pragma unroll 1
-    for (int d = 0; d < 3; ++d) {
-      if (!P.active[d]) continue;
-      const double rd = dt / __ldg(&dx[b * 3 + d]);
-      double mL, mR, pL, pR, x[2 * RS + 1];
-#pragma unroll
-      for (int m = 0; m <= 2 * RS; ++m) x[m] = Q[c + (m - RS) * stride[d]] * qri[d][m];
-      fx_scalar_faces_of_zone<RECON>(x, P.weno_eps, (qfb >> (4 * d)) & 3u, (qfb >> (4 * d + 2)) & 3u, mL, mR, pL, pR);
-      const double Fm = qA[d][0] * mL + (qF[d][0] - qA[d][0]) * mR;
-      const double Fp = qA[d][1] * pL + (qF[d][1] - qA[d][1]) * pR;
-      if (!(fabs(Fm + Fp) <= 1.79e308)) hit |= FX_STATUS_NONFINITE;
-      Ss += rd * (Fp - Fm);
+    for (int sv = 5; sv < P.nvars; ++sv) {
+      const double *Q = X + sv * P.S_v;
+      double Ss = 0.0;
+      if (P.active[0]) Ss += fx_zone_scalar_direction<RECON, 0>(P, Q, c, 1, rd0, qfb, sh, hit);
+      if (P.active[1]) Ss += fx_zone_scalar_direction<RECON, 1>(P, Q, c, P.S_j, rd1, qfb, sh, hit);
+      if (P.active[2]) Ss += fx_zone_scalar_direction<RECON, 2>(P, Q, c, P.S_k, rd2, qfb, sh, hit);
+      const long long g = sv * P.S_v + c;
+      const double u0 = U0[g];
+      out[g] = first ? (u0 - Ss) : (u0 + beta * ((Q[c] - u0) - Ss));
     }
-    const long long g = sv * P.S_v + c;
-    const double u0 = U0[g];
-    out[g] = first ? (u0 - Ss) : (u0 + beta * ((Q[c] - u0) - Ss));
   }
   if (hit) fx_note(P, hit);
 }
@@ -249,9 +332,15 @@ int fx_launch_generic_stage(const FxParams &P, const double *X, const double *U0
   const long long nzones = P.nblocks * P.n[0] * P.n[1] * P.n[2];
   if (nzones == 0) return FX_OK;
   const unsigned grid = (unsigned)((nzones + 127) / 128);
-#define CALL(RC, RM) fx_k_generic_stage<RC, RM><<<grid, 128, 0, st>>>(P, X, U0, out, dx, dt, dt_dev, beta, first, nzones)
-  FX_DISPATCH(P, CALL);
+  if (P.nvars > 5) {
+#define CALL(RC, RM) fx_k_generic_stage<RC, RM, true><<<grid, 128, sizeof(FxScalarShared<RC>), st>>>(P, X, U0, out, dx, dt, dt_dev, beta, first, nzones)
+    FX_DISPATCH(P, CALL);
 #undef CALL
+  } else {
+#define CALL(RC, RM) fx_k_generic_stage<RC, RM, false><<<grid, 128, 0, st>>>(P, X, U0, out, dx, dt, dt_dev, beta, first, nzones)
+    FX_DISPATCH(P, CALL);
+#undef CALL
+  }
   FX_LAUNCH_CHECK("generic_stage");
   return FX_OK;
 }
