@@ -118,55 +118,6 @@ __device__ __forceinline__ void fx_scalar_faces_of_zone(const double *x, double 
   }
 }
 
-// Flux at the face between cells W[0 .. R-1] (left) and W[R .. 2R-1] (right) of a line of primitives along the
-// compile-time direction D, in the un-rotated variable order; the arithmetic of fx_face_flux_global, face by face.
-template <int RECON, int RIEMANN, int D>
-__device__ __forceinline__ unsigned fx_face_from_prims(const FxParams &P, const double (*W)[5], double F[5], double &Aq,
-                                                       unsigned &fb) {
-  constexpr int R = (RECON == FX_RECON_PLM_MINMOD) ? 2 : 3;
-  constexpr int in = 1 + D, it1 = 1 + (D + 1) % 3, it2 = 1 + (D + 2) % 3;
-  constexpr int map[5] = {0, in, it1, it2, 4};
-  unsigned hit = 0;
-  double WL[5], WR[5];
-#pragma unroll
-  for (int f = 0; f < 5; ++f) {
-    const int v = map[f];
-    if (RECON == FX_RECON_PLM_MINMOD) {
-      const double a = W[0][v], b = W[1][v], c = W[2][v], e = W[3][v];
-      WL[f] = b + 0.5 * fx_minmod(b - a, c - b);
-      WR[f] = c - 0.5 * fx_minmod(c - b, e - c);
-    } else {
-      WL[f] = fx_weno5(W[0][v], W[1][v], W[2][v], W[3][v], W[4][v], P.weno_eps);
-      WR[f] = fx_weno5(W[5][v], W[4][v], W[3][v], W[2][v], W[1][v], P.weno_eps);
-    }
-  }
-  fb = 0;
-  if (RECON == FX_RECON_WENO5) {  // positivity fallback per side [A6]
-    if (!(WL[0] > 0.0) || !(WL[4] > 0.0)) {
-#pragma unroll
-      for (int f = 0; f < 5; ++f) WL[f] = W[R - 1][map[f]];
-      hit |= FX_STATUS_WENO_FALLBACK;
-      fb |= 1u;
-    }
-    if (!(WR[0] > 0.0) || !(WR[4] > 0.0)) {
-#pragma unroll
-      for (int f = 0; f < 5; ++f) WR[f] = W[R][map[f]];
-      hit |= FX_STATUS_WENO_FALLBACK;
-      fb |= 2u;
-    }
-  }
-  double Ff[5];
-  fx_riemann<RIEMANN>(P, WL, WR, Ff, Aq);
-  F[0] = Ff[0];
-  F[in] = Ff[1];
-  F[it1] = Ff[2];
-  F[it2] = Ff[3];
-  F[4] = Ff[4];
-  const double sum = Ff[0] + Ff[1] + Ff[2] + Ff[3] + Ff[4];
-  if (!(fabs(sum) <= 1.79e308)) hit |= FX_STATUS_NONFINITE;
-  return hit;
-}
-
 // What the scalar loop of a zone needs from its hydro part, per direction, kept in shared memory (one column per
 // thread: conflict-free) so that it costs the hydro part no registers.
 template <int RECON> struct FxScalarShared {
@@ -175,27 +126,67 @@ template <int RECON> struct FxScalarShared {
   double ri[3][2 * RS + 1][128];      // 1 / rho of the zone's stencil cells
 };
 
-// Direction D of one zone: the 2R+1 stencil cells are converted once and serve both faces.
-template <int RECON, int RIEMANN, int D, bool SCALARS>
+// Direction D of one zone, in the lean arithmetic of the fused kernel (fx_c2p_v2, fx_recon_cell, fx_riemann_v2: one
+// Newton step on the MUFU seeds instead of IEEE division and square root; same formulas, rounding differs): the 2R+1
+// stencil cells are converted once, cells -1, 0, +1 are reconstructed once each, and the zone's two faces are solved.
+template <int RECON, int RIEMANN, int WS, int D, bool SCALARS>
 __device__ __forceinline__ unsigned fx_zone_direction(const FxParams &P, const double *__restrict__ X, long long c,
                                                       long long s, double rd, double S[5], unsigned &qfb,
                                                       FxScalarShared<RECON> *sh) {
-  constexpr int R = (RECON == FX_RECON_PLM_MINMOD) ? 2 : 3;
+  constexpr int R = (RECON == FX_RECON_PLM_MINMOD) ? 2 : 3, r = R - 1;
+  constexpr int in = 1 + D, it1 = 1 + (D + 1) % 3, it2 = 1 + (D + 2) % 3;
+  constexpr int map[5] = {0, in, it1, it2, 4};
   double W[2 * R + 1][5];
   unsigned hit = 0;
 #pragma unroll
   for (int m = 0; m <= 2 * R; ++m) {
     const long long e = c + (m - R) * s;
-    hit |= fx_c2p(P, X[e], X[P.S_v + e], X[2 * P.S_v + e], X[3 * P.S_v + e], X[4 * P.S_v + e], W[m]);
-    if (SCALARS) sh->ri[D][m][threadIdx.x] = 1.0 / W[m][0];
+    double ri;
+    hit |= fx_c2p_v2(P, X[e], X[P.S_v + e], X[2 * P.S_v + e], X[3 * P.S_v + e], X[4 * P.S_v + e], W[m], &ri);
+    if (SCALARS) sh->ri[D][m][threadIdx.x] = ri;
   }
   hit &= FX_STATUS_NONFINITE;  // floors are counted where a zone is owned
-  double Fm[5], Fp[5], Am, Ap;
-  unsigned fbm, fbp;
-  hit |= fx_face_from_prims<RECON, RIEMANN, D>(P, &W[0], Fm, Am, fbm);
-  hit |= fx_face_from_prims<RECON, RIEMANN, D>(P, &W[1], Fp, Ap, fbp);
+  // face states of cells -1, 0, +1 in the face frame; fb bit 2n: minus side of cell n-1 fell back, bit 2n+1: plus side
+  double qm[3][5], qp[3][5];
+  unsigned fb = 0;
 #pragma unroll
-  for (int v = 0; v < 5; ++v) S[v] += rd * (Fp[v] - Fm[v]);
+  for (int n = 0; n < 3; ++n) {
+    double am[5], ap[5];
+#pragma unroll
+    for (int v = 0; v < 5; ++v) {
+      double st[2 * r + 1];
+#pragma unroll
+      for (int m = 0; m <= 2 * r; ++m) st[m] = W[n + m][v];  // cell n - 1 sits at index n + r
+      fx_recon_cell<RECON>(st, P.weno_eps, am[v], ap[v]);
+    }
+    if (RECON == FX_RECON_WENO5) {  // positivity fallback per side [A6]
+      if (!(am[0] > 0.0) || !(am[4] > 0.0)) {
+#pragma unroll
+        for (int v = 0; v < 5; ++v) am[v] = W[n + R - 1][v];
+        fb |= 1u << (2 * n);
+      }
+      if (!(ap[0] > 0.0) || !(ap[4] > 0.0)) {
+#pragma unroll
+        for (int v = 0; v < 5; ++v) ap[v] = W[n + R - 1][v];
+        fb |= 2u << (2 * n);
+      }
+    }
+#pragma unroll
+    for (int f = 0; f < 5; ++f) {
+      qm[n][f] = am[map[f]];
+      qp[n][f] = ap[map[f]];
+    }
+  }
+  // the faces see: low = (plus of cell -1, minus of cell 0), high = (plus of cell 0, minus of cell +1)
+  const unsigned fbm = ((fb >> 1) & 1u) | (((fb >> 2) & 1u) << 1), fbp = ((fb >> 3) & 1u) | (((fb >> 4) & 1u) << 1);
+  if (fbm | fbp) hit |= FX_STATUS_WENO_FALLBACK;
+  double Fm[5], Fp[5], Am, Ap;
+  fx_riemann_v2<RIEMANN, WS, true>(P, qp[0], qm[1], Fm, &Am);
+  fx_riemann_v2<RIEMANN, WS, true>(P, qp[1], qm[2], Fp, &Ap);
+  const double sum = (Fm[0] + Fm[1] + Fm[2] + Fm[3] + Fm[4]) + (Fp[0] + Fp[1] + Fp[2] + Fp[3] + Fp[4]);
+  if (!(fabs(sum) <= 1.79e308)) hit |= FX_STATUS_NONFINITE;
+#pragma unroll
+  for (int f = 0; f < 5; ++f) S[map[f]] += rd * (Fp[f] - Fm[f]);
   if (SCALARS) {
     sh->A[D][0][threadIdx.x] = Am;
     sh->A[D][1][threadIdx.x] = Ap;
@@ -212,10 +203,15 @@ __device__ __forceinline__ double fx_zone_scalar_direction(const FxParams &P, co
                                                            long long s, double rd, unsigned qfb,
                                                            const FxScalarShared<RECON> *sh, unsigned &hit) {
   constexpr int RS = (RECON == FX_RECON_PLM_MINMOD) ? 2 : 3;
-  double mL, mR, pL, pR, x[2 * RS + 1];
+  double x[2 * RS + 1];
 #pragma unroll
   for (int m = 0; m <= 2 * RS; ++m) x[m] = Q[c + (m - RS) * s] * sh->ri[D][m][threadIdx.x];
-  fx_scalar_faces_of_zone<RECON>(x, P.weno_eps, (qfb >> (4 * D)) & 3u, (qfb >> (4 * D + 2)) & 3u, mL, mR, pL, pR);
+  double am[3], ap[3];  // minus / plus face abundances of cells -1, 0, +1
+#pragma unroll
+  for (int n = 0; n < 3; ++n) fx_recon_cell<RECON>(&x[n], P.weno_eps, am[n], ap[n]);
+  const unsigned fbm = (qfb >> (4 * D)) & 3u, fbp = (qfb >> (4 * D + 2)) & 3u;
+  const double mL = (fbm & 1u) ? x[RS - 1] : ap[0], mR = (fbm & 2u) ? x[RS] : am[1];
+  const double pL = (fbp & 1u) ? x[RS] : ap[1], pR = (fbp & 2u) ? x[RS + 1] : am[2];
   const double Am = sh->A[D][0][threadIdx.x], Ap = sh->A[D][1][threadIdx.x];
   const double Fm = Am * mL + (sh->F[D][0][threadIdx.x] - Am) * mR;
   const double Fp = Ap * pL + (sh->F[D][1][threadIdx.x] - Ap) * pR;
@@ -226,7 +222,7 @@ __device__ __forceinline__ double fx_zone_scalar_direction(const FxParams &P, co
 // Resident CTAs aimed at (measured at config 5 / config 4 on the generic path, ms per stage launch): PLM uncapped (150
 // registers, 3 CTAs) 38.3, 4 CTAs 34.0, 6 CTAs 31.3, 8 CTAs (64 registers) 30.0; WENO5 uncapped (246 registers) 15.2,
 // 4 CTAs 8.2, 5 CTAs 8.8, 6 CTAs 9.3 -- the kernel is latency-bound, the spills are cheaper than the lost warps.
-template <int RECON, int RIEMANN, bool SCALARS>
+template <int RECON, int RIEMANN, int WS, bool SCALARS>
 __global__ void __launch_bounds__(128, RECON == FX_RECON_PLM_MINMOD ? 8 : 4) fx_k_generic_stage(FxParams P, const double *__restrict__ X,
                                                           const double *U0, double *out,
                                                           const double *__restrict__ dx, double dt,
@@ -248,15 +244,15 @@ __global__ void __launch_bounds__(128, RECON == FX_RECON_PLM_MINMOD ? 8 : 4) fx_
   unsigned hit = 0;
   {  // floors are counted once per owned zone
     double W[5];
-    hit |= fx_c2p(P, X[c], X[P.S_v + c], X[2 * P.S_v + c], X[3 * P.S_v + c], X[4 * P.S_v + c], W) &
+    hit |= fx_c2p_v2(P, X[c], X[P.S_v + c], X[2 * P.S_v + c], X[3 * P.S_v + c], X[4 * P.S_v + c], W) &
            (FX_STATUS_RHO_FLOOR | FX_STATUS_P_FLOOR | FX_STATUS_NONFINITE);
   }
   const double rd0 = P.active[0] ? dt / __ldg(&dx[b * 3 + 0]) : 0.0;
   const double rd1 = P.active[1] ? dt / __ldg(&dx[b * 3 + 1]) : 0.0;
   const double rd2 = P.active[2] ? dt / __ldg(&dx[b * 3 + 2]) : 0.0;
-  if (P.active[0]) hit |= fx_zone_direction<RECON, RIEMANN, 0, SCALARS>(P, X, c, 1, rd0, S, qfb, sh);
-  if (P.active[1]) hit |= fx_zone_direction<RECON, RIEMANN, 1, SCALARS>(P, X, c, P.S_j, rd1, S, qfb, sh);
-  if (P.active[2]) hit |= fx_zone_direction<RECON, RIEMANN, 2, SCALARS>(P, X, c, P.S_k, rd2, S, qfb, sh);
+  if (P.active[0]) hit |= fx_zone_direction<RECON, RIEMANN, WS, 0, SCALARS>(P, X, c, 1, rd0, S, qfb, sh);
+  if (P.active[1]) hit |= fx_zone_direction<RECON, RIEMANN, WS, 1, SCALARS>(P, X, c, P.S_j, rd1, S, qfb, sh);
+  if (P.active[2]) hit |= fx_zone_direction<RECON, RIEMANN, WS, 2, SCALARS>(P, X, c, P.S_k, rd2, S, qfb, sh);
   if (P.grav_on) {  // constant-gravity source of the stage input's own zone [B10]
     const double rho = X[c];
     double gm = 0.0;
@@ -332,15 +328,18 @@ int fx_launch_generic_stage(const FxParams &P, const double *X, const double *U0
   const long long nzones = P.nblocks * P.n[0] * P.n[1] * P.n[2];
   if (nzones == 0) return FX_OK;
   const unsigned grid = (unsigned)((nzones + 127) / 128);
-  if (P.nvars > 5) {
-#define CALL(RC, RM) fx_k_generic_stage<RC, RM, true><<<grid, 128, sizeof(FxScalarShared<RC>), st>>>(P, X, U0, out, dx, dt, dt_dev, beta, first, nzones)
-    FX_DISPATCH(P, CALL);
+#define CALL(RC, RM)                                                                                              \
+  do {                                                                                                          \
+    if (P.nvars > 5) {                                                                                          \
+      if (P.wavespeed == 0) fx_k_generic_stage<RC, RM, 0, true><<<grid, 128, sizeof(FxScalarShared<RC>), st>>>(P, X, U0, out, dx, dt, dt_dev, beta, first, nzones); \
+      else fx_k_generic_stage<RC, RM, 1, true><<<grid, 128, sizeof(FxScalarShared<RC>), st>>>(P, X, U0, out, dx, dt, dt_dev, beta, first, nzones); \
+    } else {                                                                                                    \
+      if (P.wavespeed == 0) fx_k_generic_stage<RC, RM, 0, false><<<grid, 128, 0, st>>>(P, X, U0, out, dx, dt, dt_dev, beta, first, nzones); \
+      else fx_k_generic_stage<RC, RM, 1, false><<<grid, 128, 0, st>>>(P, X, U0, out, dx, dt, dt_dev, beta, first, nzones); \
+    }                                                                                                           \
+  } while (0)
+  FX_DISPATCH(P, CALL);
 #undef CALL
-  } else {
-#define CALL(RC, RM) fx_k_generic_stage<RC, RM, false><<<grid, 128, 0, st>>>(P, X, U0, out, dx, dt, dt_dev, beta, first, nzones)
-    FX_DISPATCH(P, CALL);
-#undef CALL
-  }
   FX_LAUNCH_CHECK("generic_stage");
   return FX_OK;
 }
