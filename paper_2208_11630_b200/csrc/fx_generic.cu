@@ -219,11 +219,19 @@ __device__ __forceinline__ double fx_zone_scalar_direction(const FxParams &P, co
   return rd * (Fp - Fm);
 }
 
-// Resident CTAs aimed at (measured at config 5 / config 4 on the generic path, ms per stage launch): PLM uncapped (150
-// registers, 3 CTAs) 38.3, 4 CTAs 34.0, 6 CTAs 31.3, 8 CTAs (64 registers) 30.0; WENO5 uncapped (246 registers) 15.2,
-// 4 CTAs 8.2, 5 CTAs 8.8, 6 CTAs 9.3 -- the kernel is latency-bound, the spills are cheaper than the lost warps.
+#ifndef FX_GENERIC_MINB_PLM
+#define FX_GENERIC_MINB_PLM 6
+#endif
+#ifndef FX_GENERIC_MINB_WENO
+#define FX_GENERIC_MINB_WENO 4
+#endif
+// Resident CTAs aimed at (measured on the generic path, ms per stage launch; the kernel is latency-bound, so up to a
+// point the spills are cheaper than the lost warps).  PLM at config 5 without / with 4 scalars: 4 CTAs 15.4 / 29.9,
+// 5 CTAs 13.9 / 25.9, 6 CTAs (80 registers) 13.5 / 24.7, 8 CTAs (64 registers; its spills reach DRAM: 28.6 GB written
+// for 9.7 GB) 16.3 / 31.0.  WENO5 at config 4 without / with 2 scalars: 3 CTAs 5.5 / 7.8, 4 CTAs 5.5 / 7.4, 5 CTAs
+// 5.6 / 7.3.  (The IEEE-arithmetic version of this kernel: PLM uncapped 38.3, 8 CTAs 30.0; WENO5 uncapped 15.2, 4 CTAs 8.2.)
 template <int RECON, int RIEMANN, int WS, bool SCALARS>
-__global__ void __launch_bounds__(128, RECON == FX_RECON_PLM_MINMOD ? 8 : 4) fx_k_generic_stage(FxParams P, const double *__restrict__ X,
+__global__ void __launch_bounds__(128, RECON == FX_RECON_PLM_MINMOD ? FX_GENERIC_MINB_PLM : FX_GENERIC_MINB_WENO) fx_k_generic_stage(FxParams P, const double *__restrict__ X,
                                                           const double *U0, double *out,
                                                           const double *__restrict__ dx, double dt,
                                                           const double *__restrict__ dt_dev, double beta, int first,
