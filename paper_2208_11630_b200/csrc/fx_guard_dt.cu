@@ -92,6 +92,58 @@ int fx_launch_fill_guardcells(const FxParams &P, double *U, cudaStream_t st) {
   return FX_OK;
 }
 
+// The generic path's per-stage fill: only what its stencil reads.  The spatial operator is dimension by dimension [A11],
+// so a stage reads the R zones behind each FACE of a block and no edge or corner zone; fx_hydro_advance leaves guard
+// zones unspecified [A15], so nothing else has to be written (fx_fill_guardcells, the user's call, fills everything
+// [A14]).  One thread per face guard zone; the layer index runs fastest on the x faces, i on the y and z faces.
+__global__ void __launch_bounds__(256) fx_k_fill_faces(FxParams P, double *__restrict__ U, int R, int c0, int c1, int c2) {
+  const long long b = blockIdx.y + (long long)blockIdx.z * gridDim.y;
+  if (b >= P.nblocks) return;
+  int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= c0 + c1 + c2) return;
+  const int nx = P.n[0], ny = P.n[1], nz = P.n[2];
+  int i, j, k;
+  if (t < c0) {  // x faces: (layer, j, k, side)
+    const int l = t % R, jj = (t / R) % ny, kk = (t / (R * ny)) % nz, side = t / (R * ny * nz);
+    i = side ? P.gd[0] + nx + l : P.gd[0] - 1 - l;
+    j = P.gd[1] + jj;
+    k = P.gd[2] + kk;
+  } else if (t < c0 + c1) {  // y faces: (i, layer, k, side)
+    t -= c0;
+    const int ii = t % nx, l = (t / nx) % R, kk = (t / (nx * R)) % nz, side = t / (nx * R * nz);
+    i = P.gd[0] + ii;
+    j = side ? P.gd[1] + ny + l : P.gd[1] - 1 - l;
+    k = P.gd[2] + kk;
+  } else {  // z faces: (i, j, layer, side)
+    t -= c0 + c1;
+    const int ii = t % nx, jj = (t / nx) % ny, l = (t / (nx * ny)) % R, side = t / (nx * ny * R);
+    i = P.gd[0] + ii;
+    j = P.gd[1] + jj;
+    k = side ? P.gd[2] + nz + l : P.gd[2] - 1 - l;
+  }
+  unsigned flip;
+  const long long s = fx_guard_source(P, b, i, j, k, flip);
+  const long long d = b * P.S_b + (long long)k * P.S_k + (long long)j * P.S_j + i;
+#pragma unroll
+  for (int v = 0; v < 5; ++v) {
+    const double x = U[v * P.S_v + s];
+    U[v * P.S_v + d] = (v >= 1 && v <= 3 && ((flip >> (v - 1)) & 1u)) ? -x : x;
+  }
+  for (int v = 5; v < P.nvars; ++v) U[v * P.S_v + d] = U[v * P.S_v + s];
+}
+
+int fx_launch_fill_faces(const FxParams &P, double *U, cudaStream_t st) {
+  if (P.nblocks == 0) return FX_OK;
+  const int R = (P.recon == FX_RECON_PLM_MINMOD) ? 2 : 3;
+  const int c0 = P.active[0] ? 2 * R * P.n[1] * P.n[2] : 0, c1 = P.active[1] ? 2 * R * P.n[0] * P.n[2] : 0,
+            c2 = P.active[2] ? 2 * R * P.n[0] * P.n[1] : 0;
+  dim3 grid;
+  fx_block_grid(P.nblocks, (long long)c0 + c1 + c2, grid);
+  fx_k_fill_faces<<<grid, 256, 0, st>>>(P, U, R, c0, c1, c2);
+  FX_LAUNCH_CHECK("fill_faces");
+  return FX_OK;
+}
+
 // ------------------------------------------------------------------ interior <-> padded state (host-buffer path)
 // packed[v][b][k][j][i] over interior zones only  <->  U[v][b][k+g2][j+g1][i+g0].  One thread per interior zone and
 // variable; rows of nx doubles are contiguous on both sides.  TO_PACKED: gather, else scatter (guard zones untouched).

@@ -46,7 +46,7 @@ static int fx_stage(fx_hydro_plan *plan, double *X, const double *U0, double *ou
   const bool fused = path == 1;
   int rc = FX_OK;
   if (path == 0) {
-    rc = fx_launch_fill_guardcells(plan->P, X, st);  // O1 on the stage input before every S(.) [A15]
+    rc = fx_launch_fill_faces(plan->P, X, st);  // O1 on the stage input before every S(.) [A15]: the face zones S(.) reads
     if (rc) return rc;
   }
   const bool rec = plan->timing && plan->ev && plan->nrec < FX_MAX_REC;
