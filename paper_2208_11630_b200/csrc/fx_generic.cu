@@ -1,6 +1,6 @@
 // fx_generic.cu -- generic (any block shape, 1/2/3-D) stage kernel and the debug flux kernel.
 //
-// The generic path is: K1 full guard fill of the stage input, then this zone kernel: one thread per
+// The generic path is: a fill of the face guard zones of the stage input (fx_k_fill_faces), then this zone kernel: one thread per
 // interior zone computes the two face fluxes of each active direction from the padded stage input
 // (each face is evaluated by both zones that share it, bit-identically, so conservation holds to
 // rounding; the 2R+1 stencil cells of a direction are converted once and serve both faces), forms
@@ -73,7 +73,7 @@ __device__ __forceinline__ unsigned fx_face_flux_global(const FxParams &P, const
   return fx_face_flux_global<RECON, RIEMANN>(P, X, cL, d, s, F, Aq, fb);
 }
 
-// Passive scalar [B11]: left / right abundances X = (rho X) / rho at the face whose left cell is cL, reconstructed like
+// Passive scalar [B11] (debug flux kernel): left / right abundances X = (rho X) / rho at the face whose left cell is cL, reconstructed like
 // every other primitive (Q = the scalar's slab, X = the density's); a side that took the positivity fallback keeps
 // its cell value.
 template <int RECON>
@@ -95,26 +95,6 @@ __device__ __forceinline__ void fx_scalar_face(const FxParams &P, const double *
   } else {
     qL = (fb & 1u) ? x[R - 1] : fx_weno5(x[0], x[1], x[2], x[3], x[4], P.weno_eps);
     qR = (fb & 2u) ? x[R] : fx_weno5(x[5], x[4], x[3], x[2], x[1], P.weno_eps);
-  }
-}
-
-// The same for the two faces of one zone from the 2R+1 abundances x[0..2R] centred on it (x[R] is the zone): low face
-// between x[R-1] and x[R], high face between x[R] and x[R+1].
-template <int RECON>
-__device__ __forceinline__ void fx_scalar_faces_of_zone(const double *x, double eps, unsigned fbm, unsigned fbp,
-                                                        double &mL, double &mR, double &pL, double &pR) {
-  if (RECON == FX_RECON_PLM_MINMOD) {
-    const double s0 = fx_minmod(x[1] - x[0], x[2] - x[1]), s1 = fx_minmod(x[2] - x[1], x[3] - x[2]),
-                 s2 = fx_minmod(x[3] - x[2], x[4] - x[3]);
-    mL = x[1] + 0.5 * s0;
-    mR = x[2] - 0.5 * s1;
-    pL = x[2] + 0.5 * s1;
-    pR = x[3] - 0.5 * s2;
-  } else {
-    mL = (fbm & 1u) ? x[2] : fx_weno5(x[0], x[1], x[2], x[3], x[4], eps);
-    mR = (fbm & 2u) ? x[3] : fx_weno5(x[5], x[4], x[3], x[2], x[1], eps);
-    pL = (fbp & 1u) ? x[3] : fx_weno5(x[1], x[2], x[3], x[4], x[5], eps);
-    pR = (fbp & 2u) ? x[4] : fx_weno5(x[6], x[5], x[4], x[3], x[2], eps);
   }
 }
 
@@ -244,6 +224,7 @@ __global__ void __launch_bounds__(128, RECON == FX_RECON_PLM_MINMOD ? FX_GENERIC
   const long long per_block = (long long)nx * ny * nz;
   const long long b = z / per_block;
   const int r = (int)(z - b * per_block);
+  // (a CTA of 16 x 4 x 2 zones instead of 8 rows of one plane, for L1 reuse of the y and z neighbours: measured, no gain)
   const int i = r % nx, j = (r / nx) % ny, k = r / (nx * ny);
   const long long c = b * P.S_b + (k + P.gd[2]) * P.S_k + (j + P.gd[1]) * P.S_j + (i + P.gd[0]);
   if (dt_dev) dt = *dt_dev;
