@@ -478,10 +478,30 @@ static void riemann_flux(const fxo_plan *p, int nv, const double *WL, const doub
   double cL = sqrt(gam * pL * irL), cR = sqrt(gam * pR * irR);
   double EL = pL * igm1 + 0.5 * rL * (unL * unL + t1L * t1L + t2L * t2L);
   double ER = pR * igm1 + 0.5 * rR * (unR * unR + t1R * t1R + t2R * t2R);
-  double UL[FXO_MAXV] = {rL, rL * unL, rL * t1L, rL * t2L, EL};
-  double UR[FXO_MAXV] = {rR, rR * unR, rR * t1R, rR * t2R, ER};
-  double FL[FXO_MAXV] = {UL[1], UL[1] * unL + pL, UL[1] * t1L, UL[1] * t2L, unL * (EL + pL)};
-  double FR[FXO_MAXV] = {UR[1], UR[1] * unR + pR, UR[1] * t1R, UR[1] * t2R, unR * (ER + pR)};
+  double UL[FXO_MAXV]; /* entries 5.. are the scalars, set below */
+  UL[0] = rL;
+  UL[1] = rL * unL;
+  UL[2] = rL * t1L;
+  UL[3] = rL * t2L;
+  UL[4] = EL;
+  double UR[FXO_MAXV]; /* entries 5.. are the scalars, set below */
+  UR[0] = rR;
+  UR[1] = rR * unR;
+  UR[2] = rR * t1R;
+  UR[3] = rR * t2R;
+  UR[4] = ER;
+  double FL[FXO_MAXV]; /* entries 5.. are the scalars, set below */
+  FL[0] = UL[1];
+  FL[1] = UL[1] * unL + pL;
+  FL[2] = UL[1] * t1L;
+  FL[3] = UL[1] * t2L;
+  FL[4] = unL * (EL + pL);
+  double FR[FXO_MAXV]; /* entries 5.. are the scalars, set below */
+  FR[0] = UR[1];
+  FR[1] = UR[1] * unR + pR;
+  FR[2] = UR[1] * t1R;
+  FR[3] = UR[1] * t2R;
+  FR[4] = unR * (ER + pR);
   for (int s = 5; s < nv; ++s) {
     UL[s] = rL * WL[s];
     UR[s] = rR * WR[s];
@@ -528,12 +548,22 @@ static void riemann_flux(const fxo_plan *p, int nv, const double *WL, const doub
   double Ss = ((pR - pL) + (aL * unL - aR * unR)) / (aL - aR);
   if (Ss >= 0.0) {
     double f = aL / (SL - Ss);
-    double Us[FXO_MAXV] = {f, f * Ss, f * t1L, f * t2L, f * (EL * irL + (Ss - unL) * (Ss + pL / aL))};
+    double Us[FXO_MAXV]; /* entries 5.. are the scalars, set below */
+    Us[0] = f;
+    Us[1] = f * Ss;
+    Us[2] = f * t1L;
+    Us[3] = f * t2L;
+    Us[4] = f * (EL * irL + (Ss - unL) * (Ss + pL / aL));
     for (int s = 5; s < nv; ++s) Us[s] = f * WL[s];
     for (int v = 0; v < nv; ++v) F[v] = FL[v] + SL * (Us[v] - UL[v]);
   } else {
     double f = aR / (SR - Ss);
-    double Us[FXO_MAXV] = {f, f * Ss, f * t1R, f * t2R, f * (ER * irR + (Ss - unR) * (Ss + pR / aR))};
+    double Us[FXO_MAXV]; /* entries 5.. are the scalars, set below */
+    Us[0] = f;
+    Us[1] = f * Ss;
+    Us[2] = f * t1R;
+    Us[3] = f * t2R;
+    Us[4] = f * (ER * irR + (Ss - unR) * (Ss + pR / aR));
     for (int s = 5; s < nv; ++s) Us[s] = f * WR[s];
     for (int v = 0; v < nv; ++v) F[v] = FR[v] + SR * (Us[v] - UR[v]);
   }
