@@ -1,6 +1,7 @@
 // fx_generic.cu -- generic (any block shape, 1/2/3-D) stage kernel and the debug flux kernel.
 //
-// The generic path is: a fill of the face guard zones of the stage input (fx_k_fill_faces), then this zone kernel: one thread per
+// The generic path is this zone kernel (the hydro variables' stencil cells beyond a face are read from where O1 would copy
+// them from: no fill pass for them; the passive scalars' face guard zones are filled by fx_k_fill_faces first): one thread per
 // interior zone computes the two face fluxes of each active direction from the padded stage input
 // (each face is evaluated by both zones that share it, bit-identically, so conservation holds to
 // rounding; the 2R+1 stencil cells of a direction are converted once and serve both faces), forms
@@ -98,6 +99,26 @@ __device__ __forceinline__ void fx_scalar_face(const FxParams &P, const double *
   }
 }
 
+// Where the stencil cell o zones along direction D from zone idx (interior coordinate along D) of block b lives, as an
+// offset from the zone's own element c: inside the block it is c + o s; beyond a face it is the neighbour block's
+// interior zone, this block's own edge zone (outflow) or its mirror zone with the normal momentum negated (wall) --
+// the single hop of O1 [A14], taken while reading: the generic path fills no guard zone.
+template <int D>
+__device__ __forceinline__ long long fx_stencil_cell(const FxParams &P, long long b, long long c, int idx, int o,
+                                                     long long s, bool &flip) {
+  flip = false;
+  const int n = P.n[D], t = idx + o;
+  if (t >= 0 && t < n) return c + o * s;
+  const int side = t >= n;
+  const int nb = __ldg(&P.neigh[b * 6 + 2 * D + side]);
+  if (nb >= 0) return c + (nb - b) * P.S_b + (long long)(o + (side ? -n : n)) * s;
+  if (nb == FX_BC_REFLECT) {
+    flip = true;
+    return c + (long long)((side ? 2 * n - 1 - t : -1 - t) - idx) * s;
+  }
+  return c + (long long)((side ? n - 1 : 0) - idx) * s;  // outflow: zero-gradient clamp
+}
+
 // What the scalar loop of a zone needs from its hydro part, per direction, kept in shared memory (one column per
 // thread: conflict-free) so that it costs the hydro part no registers.
 template <int RECON> struct FxScalarShared {
@@ -110,9 +131,9 @@ template <int RECON> struct FxScalarShared {
 // Newton step on the MUFU seeds instead of IEEE division and square root; same formulas, rounding differs): the 2R+1
 // stencil cells are converted once, cells -1, 0, +1 are reconstructed once each, and the zone's two faces are solved.
 template <int RECON, int RIEMANN, int WS, int D, bool SCALARS>
-__device__ __forceinline__ unsigned fx_zone_direction(const FxParams &P, const double *__restrict__ X, long long c,
-                                                      long long s, double rd, double S[5], unsigned &qfb,
-                                                      FxScalarShared<RECON> *sh) {
+__device__ __forceinline__ unsigned fx_zone_direction(const FxParams &P, const double *__restrict__ X, long long b,
+                                                      long long c, int idx, long long s, double rd, double S[5],
+                                                      unsigned &qfb, FxScalarShared<RECON> *sh) {
   constexpr int R = (RECON == FX_RECON_PLM_MINMOD) ? 2 : 3, r = R - 1;
   constexpr int in = 1 + D, it1 = 1 + (D + 1) % 3, it2 = 1 + (D + 2) % 3;
   constexpr int map[5] = {0, in, it1, it2, 4};
@@ -120,9 +141,11 @@ __device__ __forceinline__ unsigned fx_zone_direction(const FxParams &P, const d
   unsigned hit = 0;
 #pragma unroll
   for (int m = 0; m <= 2 * R; ++m) {
-    const long long e = c + (m - R) * s;
-    double ri;
-    hit |= fx_c2p_v2(P, X[e], X[P.S_v + e], X[2 * P.S_v + e], X[3 * P.S_v + e], X[4 * P.S_v + e], W[m], &ri);
+    bool flip;
+    const long long e = fx_stencil_cell<D>(P, b, c, idx, m - R, s, flip);
+    double u[5] = {X[e], X[P.S_v + e], X[2 * P.S_v + e], X[3 * P.S_v + e], X[4 * P.S_v + e]}, ri;
+    if (flip) u[1 + D] = -u[1 + D];
+    hit |= fx_c2p_v2(P, u[0], u[1], u[2], u[3], u[4], W[m], &ri);
     if (SCALARS) sh->ri[D][m][threadIdx.x] = ri;
   }
   hit &= FX_STATUS_NONFINITE;  // floors are counted where a zone is owned
@@ -185,6 +208,8 @@ __device__ __forceinline__ double fx_zone_scalar_direction(const FxParams &P, co
   constexpr int RS = (RECON == FX_RECON_PLM_MINMOD) ? 2 : 3;
   double x[2 * RS + 1];
 #pragma unroll
+  // (the scalars' face guard zones were filled by fx_k_fill_faces: looking every cell of every scalar up through the
+  // neighbour table as the hydro part does cost 25 % of the step with 4 scalars)
   for (int m = 0; m <= 2 * RS; ++m) x[m] = Q[c + (m - RS) * s] * sh->ri[D][m][threadIdx.x];
   double am[3], ap[3];  // minus / plus face abundances of cells -1, 0, +1
 #pragma unroll
@@ -239,9 +264,9 @@ __global__ void __launch_bounds__(128, RECON == FX_RECON_PLM_MINMOD ? FX_GENERIC
   const double rd0 = P.active[0] ? dt / __ldg(&dx[b * 3 + 0]) : 0.0;
   const double rd1 = P.active[1] ? dt / __ldg(&dx[b * 3 + 1]) : 0.0;
   const double rd2 = P.active[2] ? dt / __ldg(&dx[b * 3 + 2]) : 0.0;
-  if (P.active[0]) hit |= fx_zone_direction<RECON, RIEMANN, WS, 0, SCALARS>(P, X, c, 1, rd0, S, qfb, sh);
-  if (P.active[1]) hit |= fx_zone_direction<RECON, RIEMANN, WS, 1, SCALARS>(P, X, c, P.S_j, rd1, S, qfb, sh);
-  if (P.active[2]) hit |= fx_zone_direction<RECON, RIEMANN, WS, 2, SCALARS>(P, X, c, P.S_k, rd2, S, qfb, sh);
+  if (P.active[0]) hit |= fx_zone_direction<RECON, RIEMANN, WS, 0, SCALARS>(P, X, b, c, i, 1, rd0, S, qfb, sh);
+  if (P.active[1]) hit |= fx_zone_direction<RECON, RIEMANN, WS, 1, SCALARS>(P, X, b, c, j, P.S_j, rd1, S, qfb, sh);
+  if (P.active[2]) hit |= fx_zone_direction<RECON, RIEMANN, WS, 2, SCALARS>(P, X, b, c, k, P.S_k, rd2, S, qfb, sh);
   if (P.grav_on) {  // constant-gravity source of the stage input's own zone [B10]
     const double rho = X[c];
     double gm = 0.0;

@@ -92,11 +92,13 @@ int fx_launch_fill_guardcells(const FxParams &P, double *U, cudaStream_t st) {
   return FX_OK;
 }
 
-// The generic path's per-stage fill: only what its stencil reads.  The spatial operator is dimension by dimension [A11],
+// The generic path's per-stage fill of the passive scalars (variables v0 = 5 and up; the hydro variables' halo cells
+// are read through the neighbour table by the zone kernel itself): only what its stencil reads.  The spatial operator is dimension by dimension [A11],
 // so a stage reads the R zones behind each FACE of a block and no edge or corner zone; fx_hydro_advance leaves guard
 // zones unspecified [A15], so nothing else has to be written (fx_fill_guardcells, the user's call, fills everything
 // [A14]).  One thread per face guard zone; the layer index runs fastest on the x faces, i on the y and z faces.
-__global__ void __launch_bounds__(256) fx_k_fill_faces(FxParams P, double *__restrict__ U, int R, int c0, int c1, int c2) {
+__global__ void __launch_bounds__(256) fx_k_fill_faces(FxParams P, double *__restrict__ U, int R, int c0, int c1, int c2,
+                                                       int v0) {
   const long long b = blockIdx.y + (long long)blockIdx.z * gridDim.y;
   if (b >= P.nblocks) return;
   int t = blockIdx.x * blockDim.x + threadIdx.x;
@@ -124,22 +126,20 @@ __global__ void __launch_bounds__(256) fx_k_fill_faces(FxParams P, double *__res
   unsigned flip;
   const long long s = fx_guard_source(P, b, i, j, k, flip);
   const long long d = b * P.S_b + (long long)k * P.S_k + (long long)j * P.S_j + i;
-#pragma unroll
-  for (int v = 0; v < 5; ++v) {
+  for (int v = v0; v < P.nvars; ++v) {  // variables v0 .. nvars-1
     const double x = U[v * P.S_v + s];
     U[v * P.S_v + d] = (v >= 1 && v <= 3 && ((flip >> (v - 1)) & 1u)) ? -x : x;
   }
-  for (int v = 5; v < P.nvars; ++v) U[v * P.S_v + d] = U[v * P.S_v + s];
 }
 
-int fx_launch_fill_faces(const FxParams &P, double *U, cudaStream_t st) {
-  if (P.nblocks == 0) return FX_OK;
+int fx_launch_fill_faces(const FxParams &P, double *U, int v0, cudaStream_t st) {
+  if (P.nblocks == 0 || v0 >= P.nvars) return FX_OK;
   const int R = (P.recon == FX_RECON_PLM_MINMOD) ? 2 : 3;
   const int c0 = P.active[0] ? 2 * R * P.n[1] * P.n[2] : 0, c1 = P.active[1] ? 2 * R * P.n[0] * P.n[2] : 0,
             c2 = P.active[2] ? 2 * R * P.n[0] * P.n[1] : 0;
   dim3 grid;
   fx_block_grid(P.nblocks, (long long)c0 + c1 + c2, grid);
-  fx_k_fill_faces<<<grid, 256, 0, st>>>(P, U, R, c0, c1, c2);
+  fx_k_fill_faces<<<grid, 256, 0, st>>>(P, U, R, c0, c1, c2, v0);
   FX_LAUNCH_CHECK("fill_faces");
   return FX_OK;
 }

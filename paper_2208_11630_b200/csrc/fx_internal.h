@@ -71,7 +71,7 @@ int fx_cuda_check(cudaError_t e, const char *what);
 
 // kernel launchers (one per .cu file); all enqueue on `st`
 int fx_launch_fill_guardcells(const FxParams &P, double *U, cudaStream_t st);
-int fx_launch_fill_faces(const FxParams &P, double *U, cudaStream_t st);  // face guard zones of depth R only
+int fx_launch_fill_faces(const FxParams &P, double *U, int v0, cudaStream_t st);  // face guard zones of depth R, variables >= v0
 int fx_launch_index_map(const FxParams &P, long long b0, long long nb, long long *src, cudaStream_t st);
 int fx_launch_pack_interior(const FxParams &P, double *U, double *packed, int to_packed, cudaStream_t st);
 int fx_launch_compute_dt(const FxParams &P, const double *U, const double *dx, double cfl, double *dt_out,

@@ -45,8 +45,10 @@ static int fx_stage(fx_hydro_plan *plan, double *X, const double *U0, double *ou
   const int path = fx_hydro_plan_path(plan);  // 1 fused TMA kernel, 2 shared-memory tile kernel, 0 generic
   const bool fused = path == 1;
   int rc = FX_OK;
-  if (path == 0) {
-    rc = fx_launch_fill_faces(plan->P, X, st);  // O1 on the stage input before every S(.) [A15]: the face zones S(.) reads
+  if (path == 0 && plan->nvars > 5) {
+    // the generic zone kernel reads the hydro variables' halo cells through the neighbour table, like the other two
+    // paths; only the passive scalars' face guard zones are filled [A15]
+    rc = fx_launch_fill_faces(plan->P, X, 5, st);
     if (rc) return rc;
   }
   const bool rec = plan->timing && plan->ev && plan->nrec < FX_MAX_REC;
