@@ -204,8 +204,8 @@ int fx_hydro_status_reset(fx_hydro_plan *plan, void *stream);
  * face f lies between padded cells gd+f-1 and gd+f.  Not on the timed path. */
 int fx_debug_compute_fluxes(fx_hydro_plan *plan, const double *U_dev, int dir, double *F_dev, void *stream);
 
-/* Which stage kernel fx_hydro_advance will use for this plan: 0 generic (fill of the face guard zones the stencil
- * reads + zone kernel; the only path for plans with passive scalars),
+/* Which stage kernel fx_hydro_advance will use for this plan: 0 generic (zone kernel that reads its halo cells through
+ * the neighbour table; the only path for plans with passive scalars, whose face guard zones it fills first),
  * 1 fused and TMA-fed (16 x 16 x nz blocks: halos gathered from neighbour interiors inside the stage kernel,
  * every plane moved by TMA), 2 shared-memory tile kernel (one CTA per block whose padded zones fit its shared
  * memory: halos gathered through the neighbour table, each zone converted once, one Riemann solve per face). */
