@@ -232,9 +232,9 @@ def run_ours(args, rank, world, local_rank):
     stages = cfg.rk_order
     zones = cfg.interior_zones
     fused = plan.path == 1
-    # fused path: one launch per RK stage, the CFL reduction (a7) rides in the last one; generic path: guard fill +
-    # stage kernel per stage, then the reduction pass
-    launches_per_step = stages if fused else (stages + 1 if plan.path == 2 else 2 * stages + 1)
+    # fused path: one launch per RK stage, the CFL reduction (a7) rides in the last one; tile and generic paths: one
+    # stage kernel per stage, then the reduction pass; with passive scalars also their face fill per stage
+    launches_per_step = stages if fused else (stages + 1 + (stages if args.scalars else 0))
     dt = plan.fx_hydro_compute_dt(U, dx, cfg.cfl).clone()  # the first step's dt; stays on the device from here on
 
     def step():

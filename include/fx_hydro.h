@@ -51,8 +51,9 @@ enum {
   FX_OPT_WENO_EPS = 2,  /* WENO5-JS epsilon, default 1e-6 [A5] */
   FX_OPT_WAVESPEED = 3, /* 0 = Einfeldt (default), 1 = Davis [A8] */
   FX_OPT_PATH = 4,      /* 0 = auto: the fused TMA stage kernel for 16 x 16 x nz blocks, else the shared-memory tile kernel
-                           when the padded block fits a CTA's shared memory (8^3 blocks, 2-D, 1-D), else the generic
-                           zone kernel; 1 = generic; 2 = tile kernel where it fits, else generic.
+                           when the padded block fits a CTA's shared memory (8^3 blocks with WENO5, 2-D, 1-D), else
+                           the generic zone kernel (also 3-D PLM blocks that would fit: it is the faster one there, measured);
+                           1 = generic; 2 = tile kernel where it fits, else generic.
                            fx_hydro_plan_path reports the choice (1 fused, 2 tile, 0 generic). */
   FX_OPT_ZCHAIN = 5,    /* fused path: longest chain of z-neighbour blocks one CTA marches through, 1..8; 0 (default) =
                            chosen from the number of blocks and of SMs so that the launch still fills the GPU.

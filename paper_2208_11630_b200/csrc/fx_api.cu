@@ -179,7 +179,11 @@ extern "C" int fx_hydro_plan_path(const fx_hydro_plan *plan) {
   if (!plan) return fx_fail(FX_ERR_INVALID_ARG, "plan_path: null plan");
   if (plan->nvars > 5) return 0;  // passive scalars [B11] are carried by the generic path only
   if (plan->path_option == 0 && fx_stage_tma_supported(plan->P)) return 1;
-  if (plan->path_option != 1 && fx_stage_tile_supported(plan->P)) return 2;
+  // 3-D blocks with PLM: the generic zone kernel, which gathers its halo cells itself, is ahead of the tile kernel
+  // (8^3 blocks: 34.6 against 41.2 ms per step, measured); FX_OPT_PATH = 2 still selects the tile kernel
+  const bool generic_ahead = plan->path_option == 0 && plan->P.active[0] && plan->P.active[1] && plan->P.active[2] &&
+                             plan->P.recon == FX_RECON_PLM_MINMOD;
+  if (plan->path_option != 1 && !generic_ahead && fx_stage_tile_supported(plan->P)) return 2;
   return 0;
 }
 

@@ -446,9 +446,10 @@ def test_tile_kernel_small_blocks(dims, nb, nguard, recon, rk, bc, grav):
     cfg = inputs.config(5, nb=nb)
     cfg.block_dims, cfg.nguard = dims, nguard
     oplan, neigh, coords = oracle_plan_for(cfg, bc=bc, recon=recon, rk=rk)
-    gplan, _, _ = gpu_plan_for(cfg, bc=bc, recon=recon, rk=rk)
+    gplan, _, _ = gpu_plan_for(cfg, bc=bc, recon=recon, rk=rk, path=2)  # 2: prefer the tile kernel (3-D PLM blocks default to the generic one)
     gen, _, _ = gpu_plan_for(cfg, bc=bc, recon=recon, rk=rk, path=1)
-    assert gplan.path == 2 and gen.path == 0
+    auto, _, _ = gpu_plan_for(cfg, bc=bc, recon=recon, rk=rk)
+    assert gplan.path == 2 and gen.path == 0 and auto.path == (0 if (recon == 0 and min(dims) > 1) else 2)
     g = (0.7, -1.1 if dims[1] > 1 else 0.0, 0.4 if dims[2] > 1 else 0.0)
     if grav:
         for d in range(3):
