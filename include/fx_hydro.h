@@ -219,11 +219,6 @@ int fx_hydro_plan_path(const fx_hydro_plan *plan);
 int fx_hydro_plan_set_timing(fx_hydro_plan *plan, int enable);
 int fx_hydro_plan_get_timing(fx_hydro_plan *plan, double *stage_ms_sum_host, long long *stage_launches_host);
 
-/* Measurement aid for the fp64 roofline: runs a dependent-chain-free DFMA kernel (iters FMAs per
- * thread on 8 independent accumulators) over the whole device; the caller times it with events.
- * out_dev: double [1] sink.  Returns the number of FMAs issued in *fma_count_host. */
-int fx_probe_fp64_fma(int iters, double *out_dev, unsigned long long *fma_count_host, void *stream);
-
 #ifdef __cplusplus
 }
 #endif

@@ -462,6 +462,14 @@ static void reconstruct_face(const fxo_plan *p, int nv, const double *W, int64_t
   }
 }
 
+/* Test hook: the face states [O3, A6] at the face between cells cL and cL + s of a line of primitives
+ * W[v * slab + cell] (a call of reconstruct_face, nothing else); *hit receives the status bits it raises. */
+void fxo_face_states(const fxo_plan *p, const double *W, int64_t slab, int64_t cL, int64_t s, double *WL, double *WR,
+                     unsigned *hit) {
+  *hit = 0;
+  reconstruct_face(p, p->nvars, W, slab, cL, s, WL, WR, hit);
+}
+
 /* ---------------------------------------------------- O4 Riemann flux */
 
 /* States in the face frame: W = (rho, un, ut1, ut2, p); flux F = (mass, normal momentum,

@@ -67,6 +67,8 @@ def lib():
         L.fxo_minmod.restype = C.c_double
         L.fxo_weno5.argtypes = [C.c_double] * 6
         L.fxo_weno5.restype = C.c_double
+        L.fxo_face_states.argtypes = [C.c_void_p, dp, C.c_int64, C.c_int64, C.c_int64, dp, dp, C.POINTER(C.c_uint32)]
+        L.fxo_face_states.restype = None
         L.fxo_riemann_flux.argtypes = [C.c_void_p, dp, dp, dp]
         L.fxo_riemann_flux.restype = None
         L.fxo_cons2prim_nv.argtypes = [C.c_void_p, dp, dp]
@@ -186,6 +188,16 @@ class OraclePlan:
         W = np.empty(self.nvars)
         lib().fxo_cons2prim_nv(self._h, _dptr(U), _dptr(W))
         return W
+
+    def face_states(self, W, cL):
+        """Face states [O3, A6] between cells cL and cL + 1 of a line of primitives W[nvars][ncells]; returns
+        (WL, WR, status bits raised)."""
+        W = np.ascontiguousarray(W, np.float64)
+        assert W.ndim == 2 and W.shape[0] == self.nvars
+        WL, WR = np.empty(self.nvars), np.empty(self.nvars)
+        hit = C.c_uint32()
+        lib().fxo_face_states(self._h, _dptr(W), W.shape[1], int(cL), 1, _dptr(WL), _dptr(WR), C.byref(hit))
+        return WL, WR, int(hit.value)
 
     def riemann_flux_nv(self, WL, WR):
         """Face-frame states (rho, un, ut1, ut2, p, X_1..) of nvars entries -> flux of nvars entries (B11)."""

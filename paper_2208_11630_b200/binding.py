@@ -12,7 +12,7 @@ import numpy as np
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.environ.get("FXHYDRO_LIB") or os.path.join(_HERE, "libfxhydro.so")  # FXHYDRO_LIB: an alternative build
+LIB_PATH = os.path.join(_HERE, "libfxhydro.so")
 
 OK, ERR_INVALID_ARG, ERR_STATE, ERR_UNSUPPORTED, ERR_WORKSPACE, ERR_CUDA = 0, -1, -2, -3, -4, -5
 RECON_PLM_MINMOD, RECON_WENO5 = 0, 1
@@ -30,7 +30,7 @@ EXPORTS = [
     "fx_hydro_plan_set_topology", "fx_topology_cartesian", "fx_fill_guardcells", "fx_guardcell_index_map",
     "fx_hydro_compute_dt", "fx_hydro_advance", "fx_hydro_advance_host", "fx_hydro_advance_host_interior", "fx_hydro_advance_devdt", "fx_hydro_step",
     "fx_hydro_status", "fx_hydro_status_reset", "fx_debug_compute_fluxes", "fx_hydro_plan_path",
-    "fx_probe_fp64_fma", "fx_hydro_plan_set_timing", "fx_hydro_plan_get_timing",
+    "fx_hydro_plan_set_timing", "fx_hydro_plan_get_timing",
 ]
 
 
@@ -82,7 +82,6 @@ def lib():
         L.fx_hydro_plan_path.argtypes = [vp]
         L.fx_hydro_plan_set_timing.argtypes = [vp, C.c_int]
         L.fx_hydro_plan_get_timing.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
-        L.fx_probe_fp64_fma.argtypes = [C.c_int, vp, C.POINTER(C.c_ulonglong), vp]
         _lib = L
     return _lib
 
@@ -285,9 +284,3 @@ class HydroPlan:
     def interior(self, U):
         g, n = self.gd, self.block_dims
         return U[:, :, g[2]:g[2] + n[2], g[1]:g[1] + n[1], g[0]:g[0] + n[0]]
-
-
-def fx_probe_fp64_fma(iters, out, stream=None):
-    n = C.c_ulonglong()
-    _check(lib().fx_probe_fp64_fma(int(iters), _dev(out, torch.float64), C.byref(n), _stream(stream)))
-    return int(n.value)

@@ -26,13 +26,8 @@ def _stale() -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False, defines=(), out: str | None = None) -> str:
-    """Build libfxhydro.so.  `defines` (e.g. ["FX_FUSED_MINB_PLM=1"]) and `out` make a tuning variant that
-    binding.py loads when FXHYDRO_LIB points at it."""
-    global LIB
-    if out:
-        LIB = os.path.abspath(out)
-        force = True
+def build(force: bool = False, verbose: bool = False) -> str:
+    """Build libfxhydro.so in-tree (only when a source is newer than the library, unless `force`)."""
     if not force and not _stale():
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
@@ -43,7 +38,7 @@ def build(force: bool = False, verbose: bool = False, defines=(), out: str | Non
     for src in sources():
         obj = os.path.join(bdir, os.path.basename(src)[:-3] + ".o")
         objs.append(obj)
-        procs.append((src, subprocess.Popen([nvcc, *NVCC_FLAGS, *[f"-D{d}" for d in defines], "-c", src, "-o", obj], stdout=subprocess.PIPE,
+        procs.append((src, subprocess.Popen([nvcc, *NVCC_FLAGS, "-c", src, "-o", obj], stdout=subprocess.PIPE,
                                             stderr=subprocess.STDOUT, text=True)))
     log = []
     for src, p in procs:
@@ -61,6 +56,4 @@ def build(force: bool = False, verbose: bool = False, defines=(), out: str | Non
 
 
 if __name__ == "__main__":
-    defs = [a[2:] for a in sys.argv if a.startswith("-D")]
-    outs = [a[6:] for a in sys.argv if a.startswith("--out=")]
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv, defines=defs, out=outs[0] if outs else None))
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))

@@ -27,6 +27,15 @@ int fx_cuda_check(cudaError_t e, const char *what) {
   return fx_fail(FX_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
 }
 
+int fx_sm_count() {
+  int dev = 0, sms = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms < 1) {
+    cudaGetLastError();
+    return 148;  // no device visible (host-only use of the library): B200's count, used for sizing heuristics only
+  }
+  return sms;
+}
+
 extern "C" const char *fx_last_error(void) { return fx_errbuf; }
 
 // ------------------------------------------------------------------ plan (a0)
@@ -131,8 +140,12 @@ extern "C" int fx_hydro_plan_layout(const fx_hydro_plan *plan, fx_layout *out) {
 extern "C" int fx_hydro_plan_set_option(fx_hydro_plan *plan, int key, double value) {
   if (!plan) return fx_fail(FX_ERR_INVALID_ARG, "set_option: null plan");
   switch (key) {
-  case FX_OPT_RHO_FLOOR: plan->P.rho_floor = value; return FX_OK;
-  case FX_OPT_P_FLOOR: plan->P.p_floor = value; return FX_OK;
+  case FX_OPT_RHO_FLOOR:
+  case FX_OPT_P_FLOOR:
+    // a floor <= 0 or non-finite would let 1/rho or sqrt(p/rho) produce Inf/NaN where the floor is meant to prevent it
+    if (!(value > 0.0) || !isfinite(value)) return fx_fail(FX_ERR_INVALID_ARG, "set_option: a floor must be positive and finite");
+    if (key == FX_OPT_RHO_FLOOR) plan->P.rho_floor = value; else plan->P.p_floor = value;
+    return FX_OK;
   case FX_OPT_WENO_EPS:
     if (!(value > 0.0)) return fx_fail(FX_ERR_INVALID_ARG, "set_option: WENO eps must be > 0");
     plan->P.weno_eps = value;
@@ -289,8 +302,7 @@ extern "C" int fx_hydro_plan_set_topology(fx_hydro_plan *plan, const int32_t *ne
     if (M <= 0) {
       // auto: a segment of M blocks costs about M + 0.09 block times (measured: the start-up of a CTA and the z halo of
       // a segment are 9 % of a block), and the launch takes ceil(segments / resident CTAs) rounds of them
-      int dev = 0, sms = 148;
-      if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+      const int sms = fx_sm_count();
       const long long slots = (long long)sms * (plan->P.recon == FX_RECON_WENO5 ? 1 : 2);
       double best = 0.0;
       for (int m = 1; m <= FX_SEG_MAX; m *= 2) {

@@ -165,7 +165,8 @@ int fx_launch_pack_interior(const FxParams &P, double *U, double *packed, int to
   const long long n = (long long)P.nvars * P.nblocks * P.n[0] * P.n[1] * P.n[2];
   if (n == 0) return FX_OK;
   const long long want = (n + 255) / 256;
-  const unsigned grid = (unsigned)(want < 148LL * 32 ? want : 148LL * 32);
+  const long long cap = (long long)fx_sm_count() * 32;
+  const unsigned grid = (unsigned)(want < cap ? want : cap);
   if (to_packed) fx_k_pack_interior<true><<<grid, 256, 0, st>>>(P, U, packed, n);
   else fx_k_pack_interior<false><<<grid, 256, 0, st>>>(P, U, packed, n);
   FX_LAUNCH_CHECK("pack_interior");
@@ -286,7 +287,8 @@ __global__ void __launch_bounds__(256) fx_k_compute_dt(FxParams P, const double 
 int fx_launch_compute_dt(const FxParams &P, const double *U, const double *dx, double cfl, double *dt_out,
                          cudaStream_t st) {
   const long long want = P.nblocks < 1 ? 1 : P.nblocks;
-  const int grid = (int)(want > 148 * 8 ? 148 * 8 : want);
+  const long long cap = (long long)fx_sm_count() * 8;
+  const int grid = (int)(want > cap ? cap : want);
   fx_k_compute_dt<<<grid, 256, 0, st>>>(P, U, dx, cfl, dt_out);
   FX_LAUNCH_CHECK("compute_dt");
   return FX_OK;

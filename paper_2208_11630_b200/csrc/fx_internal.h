@@ -59,6 +59,9 @@ struct fx_hydro_plan {
 };
 enum { FX_MAX_REC = 4096 };
 
+// number of SMs of the current device (queried once per device; fx_api.cu)
+int fx_sm_count();
+
 // error plumbing (fx_api.cu)
 int fx_fail(int code, const char *fmt, ...);
 int fx_cuda_check(cudaError_t e, const char *what);

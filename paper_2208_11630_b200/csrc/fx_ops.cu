@@ -1,5 +1,5 @@
 // fx_ops.cu -- the operations of the C ABI: guard fill, index map, dt, advance (stage sequencing),
-// host-buffer end-to-end variant, status, debug fluxes, fp64 probe.
+// host-buffer end-to-end variant, status, debug fluxes.
 #include <math.h>
 #include <string.h>
 
@@ -57,13 +57,13 @@ static int fx_stage(fx_hydro_plan *plan, double *X, const double *U0, double *ou
              : (path == 2 ? fx_launch_stage_tile(plan->P, X, U0, out, dx, dt, dt_dev, beta, first, st)
                           : fx_launch_generic_stage(plan->P, X, U0, out, dx, dt, dt_dev, beta, first, st));
   if (rc) return rc;
-  if (!fused && dt_next) {  // the generic path has no fused reduction: a7 as its own pass over the finished state
-    rc = fx_launch_compute_dt(plan->P, out, dx, cfl_next, dt_next, st);
-    if (rc) return rc;
-  }
-  if (rec) {
+  if (rec) {  // the pair brackets the stage kernel alone (fx_hydro.h), not the reduction pass below
     FX_CUDA(cudaEventRecord(plan->ev[2 * plan->nrec + 1], st));
     ++plan->nrec;
+  }
+  if (!fused && dt_next) {  // the generic and tile paths have no fused reduction: a7 as its own pass over the finished state
+    rc = fx_launch_compute_dt(plan->P, out, dx, cfl_next, dt_next, st);
+    if (rc) return rc;
   }
   return FX_OK;
 }
@@ -217,29 +217,4 @@ extern "C" int fx_debug_compute_fluxes(fx_hydro_plan *plan, const double *U, int
   if (dir < 0 || dir > 2 || !plan->P.active[dir]) return fx_fail(FX_ERR_INVALID_ARG, "debug_compute_fluxes: inactive or bad direction %d", dir);
   if ((!U || !F) && plan->P.nblocks > 0) return fx_fail(FX_ERR_INVALID_ARG, "debug_compute_fluxes: null argument");
   return fx_launch_debug_fluxes(plan->P, U, dir, F, (cudaStream_t)stream);
-}
-
-// ------------------------------------------------------------------ fp64 probe
-__global__ void __launch_bounds__(256) fx_k_probe_fma(int iters, double *out) {
-  double a[8];
-  const double x = 1.0 + 1e-9 * threadIdx.x, y = 1e-12 * (blockIdx.x + 1);
-#pragma unroll
-  for (int q = 0; q < 8; ++q) a[q] = q * 0.125;
-  for (int it = 0; it < iters; ++it) {
-#pragma unroll
-    for (int q = 0; q < 8; ++q) a[q] = fma(a[q], x, y);
-  }
-  double s = 0.0;
-#pragma unroll
-  for (int q = 0; q < 8; ++q) s += a[q];
-  if (s == 123.456) *out = s;  // never true; keeps the chain alive
-}
-
-extern "C" int fx_probe_fp64_fma(int iters, double *out_dev, unsigned long long *fma_count, void *stream) {
-  if (iters < 1 || !out_dev) return fx_fail(FX_ERR_INVALID_ARG, "probe_fp64_fma: bad argument");
-  const int grid = 148 * 8;
-  fx_k_probe_fma<<<grid, 256, 0, (cudaStream_t)stream>>>(iters, out_dev);
-  FX_LAUNCH_CHECK("probe");
-  if (fma_count) *fma_count = (unsigned long long)grid * 256ull * 8ull * (unsigned long long)iters;
-  return FX_OK;
 }

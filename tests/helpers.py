@@ -21,7 +21,7 @@ def golden_rows(name):
 
 
 def oracle_plan_for(cfg, nblocks=None, order=inputs.ORDER_LEX, bc=None, nb=None, recon=None, riemann=None, rk=None,
-                    nvars=5):
+                    nvars=5, wavespeed=None):
     """Oracle plan + topology for a config (regular tiling nb, default cfg.nb)."""
     nb = tuple(nb or cfg.nb)
     bc = bc or cfg.bc
@@ -32,6 +32,8 @@ def oracle_plan_for(cfg, nblocks=None, order=inputs.ORDER_LEX, bc=None, nb=None,
                           cfg.recon if recon is None else recon, cfg.riemann if riemann is None else riemann,
                           cfg.rk_order if rk is None else rk, nvars=nvars)
     plan.set_topology(neigh)
+    if wavespeed is not None:
+        plan.set_option(fxo.OPT_WAVESPEED, wavespeed)
     return plan, neigh, coords
 
 
@@ -146,7 +148,7 @@ def rel_err(cfg, got, ref):
 
 
 def gpu_plan_for(cfg, order=inputs.ORDER_LEX, bc=None, nb=None, recon=None, riemann=None, rk=None, path=None,
-                 neigh=None, nblocks=None, zchain=None, nvars=5):
+                 neigh=None, nblocks=None, zchain=None, nvars=5, wavespeed=None):
     """CUDA-side plan + topology + workspace for a config (uses the library's own topology helper)."""
     from paper_2208_11630_b200 import binding as fx
     nb = tuple(nb or cfg.nb)
@@ -163,6 +165,30 @@ def gpu_plan_for(cfg, order=inputs.ORDER_LEX, bc=None, nb=None, recon=None, riem
         plan.fx_hydro_plan_set_option(fx.OPT_PATH, path)
     if zchain is not None:
         plan.fx_hydro_plan_set_option(fx.OPT_ZCHAIN, zchain)
+    if wavespeed is not None:
+        plan.fx_hydro_plan_set_option(fx.OPT_WAVESPEED, wavespeed)
     plan.fx_hydro_plan_set_topology(neigh)
     plan.fx_hydro_plan_set_workspace()
     return plan, neigh, coords
+
+
+def cliff_state(cfg, coords, axis, high=1e6):
+    """Conserved block interiors [5, nb, nz, ny, nx] of the config's own field with a density cliff and a pressure cliff
+    along `axis` in every block -- a ramp (5.5, 3, 0.5) running into a plateau `high`, the profile whose WENO5 face
+    value is negative on the ramp side (tests/test_oracle_pins_r2.py) -- so that the positivity fallback [A6] is taken
+    on one side of some faces, in rho at one place and in p at another."""
+    Ui = inputs.block_interiors(cfg, coords).numpy().copy()
+    g = cfg.gamma
+    rho = Ui[0]
+    vel = Ui[1:4] / rho
+    p = (g - 1) * (Ui[4] - 0.5 * rho * (vel ** 2).sum(0))
+    ax = 3 - axis  # axis of rho[b, k, j, i]
+    n = rho.shape[ax]
+    lo_r, lo_p = (1, n - 7) if n >= 14 else (1, 1)
+    for lo, arr, vals in ((lo_r, rho, (5.5, 3.0, 0.5, high, high, high)), (lo_p, p, (high, high, high, 0.5, 3.0, 5.5))):
+        s = [slice(None)] * 4
+        s[ax] = slice(lo, lo + 6)
+        shape = [1, 1, 1, 1]
+        shape[ax] = 6
+        arr[tuple(s)] = np.array(vals).reshape(shape)
+    return np.stack([rho, rho * vel[0], rho * vel[1], rho * vel[2], p / (g - 1) + 0.5 * rho * (vel ** 2).sum(0)])

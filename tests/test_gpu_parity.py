@@ -101,6 +101,9 @@ ADV_CASES = [  # number, nb, kwargs
     (2, (3, 2, 1), dict(recon=1, rk=3)), (5, (2, 2, 2), dict(bc="outflow")),
     (5, (2, 2, 2), dict(bc="reflect")), (5, (1, 1, 3), dict(bc="reflect", recon=1, rk=3)), (2, (2, 2, 1), dict(bc="reflect")),
     (1, None, dict(bc="reflect")),
+    # Davis wave speeds [A8] (FX_OPT_WAVESPEED = 1: its own template instantiation) on every path's shape
+    (5, (2, 2, 2), dict(wavespeed=1)), (3, (2, 2, 2), dict(wavespeed=1, riemann=0)), (4, (2, 2, 2), dict(wavespeed=1)),
+    (2, (3, 2, 1), dict(wavespeed=1)), (1, None, dict(wavespeed=1)),
 ]
 
 
@@ -123,6 +126,67 @@ def test_advance_1_and_10_steps(number, nb, kw, path):
     fo, _ = oplan.status()
     fg, _ = gplan.fx_hydro_status()
     assert fo == fg, (fo, fg)
+
+
+@pytest.mark.parametrize("dims,path", [((16, 16, 16), None), ((16, 16, 16), 1), ((8, 8, 8), 2), ((8, 8, 8), 1), ((16, 16, 1), None)])
+@pytest.mark.parametrize("rk", [2, 3])
+def test_weno_positivity_fallback_taken_on_every_path(dims, path, rk):
+    """[A6] A field with density and pressure cliffs (tests.helpers.cliff_state; the oracle's branch is pinned on the
+    same profile in tests/test_oracle_pins_r2.py) along each axis: the fallback IS taken (non-zero count on both
+    sides), the status bits agree, and the states agree to the one-step tolerance on the fused, generic and tile
+    kernels.  The reverted side's WENO value is -0.75 against cell values of order 1, so rounding cannot flip the
+    decision."""
+    from tests.helpers import cliff_state
+    ndim = sum(1 for d in dims if d > 1)
+    for axis in range(ndim):
+        cfg = inputs.config(4, nb=(2, 2, 2) if ndim == 3 else (2, 2, 1))
+        cfg.block_dims = dims
+        oplan, neigh, coords = oracle_plan_for(cfg, rk=rk)
+        gplan, _, _ = gpu_plan_for(cfg, rk=rk, path=path)
+        assert gplan.path == {None: (1 if dims == (16, 16, 16) else 2), 1: 0, 2: 2}[path]
+        Uh = inputs.embed(cfg, torch.from_numpy(cliff_state(cfg, coords, axis, high=1e3)))
+        dx = inputs.dx_array(cfg)
+        Uo, Ud, dxd = Uh.numpy().copy(), Uh.cuda(), torch.from_numpy(dx).cuda()
+        dt = oplan.compute_dt(Uo, dx, 0.1)
+        oplan.advance(Uo, dx, dt)
+        gplan.fx_hydro_advance(Ud, dxd, dt)
+        fo, co = oplan.status()
+        fg, cg = gplan.fx_hydro_status()
+        assert fo & fxo.STATUS_WENO_FALLBACK and co[3] > 0 and cg[3] > 0
+        assert fo == fg, (fo, fg)
+        err = rel_err(cfg, gplan.interior(Ud).cpu().numpy(), oplan.interior(Uo))
+        assert err <= TOL_1, (axis, err)
+
+
+@pytest.mark.parametrize("path", [None, 1])
+@pytest.mark.parametrize("recon,riemann,rk", [(0, 0, 2), (1, 1, 3)])
+def test_sod_along_y_and_z(recon, riemann, rk, path):
+    """Config 1 laid along x, y and z (the oracle's three runs are bit for bit the same: tests/test_oracle_pins_r2.py):
+    each GPU run matches the oracle's, so the kernels' frame rotation is the oracle's."""
+    from paper_2208_11630_b200 import binding as fx
+    from tests.test_oracle_pins_r2 import _sod_along
+    for axis in range(3):
+        oplan, Uo, dx = _sod_along(axis, riemann, recon, rk)
+        dims = [1, 1, 1]
+        dims[axis] = 256
+        neigh = np.full((1, 6), fx.BC_NONE, np.int32)
+        neigh[0, 2 * axis] = neigh[0, 2 * axis + 1] = fx.BC_OUTFLOW
+        gplan = fx.HydroPlan(tuple(dims), 4, 1, 1.4, recon, riemann, rk)
+        if path is not None:
+            gplan.fx_hydro_plan_set_option(fx.OPT_PATH, path)
+        gplan.fx_hydro_plan_set_topology(neigh)
+        gplan.fx_hydro_plan_set_workspace()
+        Ud, dxd = torch.from_numpy(Uo).cuda(), torch.from_numpy(dx).cuda()
+        cfg = inputs.config(1)
+        for step in range(10):
+            dt = oplan.compute_dt(Uo, dx, 0.8)
+            dtg = float(gplan.fx_hydro_compute_dt(Ud, dxd, 0.8).item())
+            assert abs(dtg - dt) <= TOL_DT * dt
+            oplan.advance(Uo, dx, dt)
+            gplan.fx_hydro_advance(Ud, dxd, dt)
+            if step in (0, 9):
+                err = rel_err(cfg, gplan.interior(Ud).cpu().numpy(), oplan.interior(Uo))
+                assert err <= (TOL_1 if step == 0 else TOL_10), (axis, step, err)
 
 
 def test_device_dt_path_equals_host_dt_path():
