@@ -45,7 +45,7 @@ def parse_args():
     ap.add_argument("--nb", default=None, help="override blocks per dimension, e.g. 16,16,16")
     ap.add_argument("--block", default=None, help="override zones per block and dimension, e.g. 8,8,8 (with --nb 64,64,64: config 5's field "
                     "on 8^3 blocks; not a BASELINE config: the small-block workload of the tile kernel)")
-    ap.add_argument("--path", type=int, default=0, help="FX_OPT_PATH: 0 auto (fused TMA stage kernel when supported), 1 generic")
+    ap.add_argument("--path", type=int, default=0, help="FX_OPT_PATH: 0 auto (fused TMA stage kernel when supported), 1 generic, 2 tile, 3 the fused kernel's two-zones-per-thread variant")
     ap.add_argument("--zchain", type=int, default=0, help="FX_OPT_ZCHAIN: z-neighbour blocks per CTA of the fused kernel (0 = library default)")
     ap.add_argument("--guard-x", type=int, default=-1, help="FX_OPT_GUARD_X: x guard depth (layout); -1 = 8 for 16-wide blocks with 4 guard zones "
                     "(256-byte row pitch, interior rows on 128-byte lines), else the config's nguard")
@@ -231,7 +231,7 @@ def run_ours(args, rank, world, local_rank):
     cfg, plan, U, dx, coords = build_workload(args, device)
     stages = cfg.rk_order
     zones = cfg.interior_zones
-    fused = plan.path == 1
+    fused = plan.path in (1, 3)
     # fused path: one launch per RK stage, the CFL reduction (a7) rides in the last one; tile and generic paths: one
     # stage kernel per stage, then the reduction pass; with passive scalars also their face fill per stage
     launches_per_step = stages if fused else (stages + 1 + (stages if args.scalars else 0))
@@ -302,7 +302,7 @@ def run_ours(args, rank, world, local_rank):
                                    + (f", {args.scalars} passive mass scalars" if args.scalars else ""),
                        "interior_zones": zones, "state_bytes": plan.bytes_per_state, "block_order": args.order,
                        "layout": f"x guard depth {plan.gd[0]} (row pitch {plan.S_j * 8} B), y/z guard depth {plan.gd[1]}/{plan.gd[2]}",
-                       "path": {0: "generic", 1: "fused (TMA)", 2: "tile (shared-memory block)"}[plan.path], "l2": "inputs (state) larger than L2; no flush needed",
+                       "path": {0: "generic", 1: "fused (TMA)", 2: "tile (shared-memory block)", 3: "fused (TMA), two zones per thread"}[plan.path], "l2": "inputs (state) larger than L2; no flush needed",
                        "multi_gpu": "replicas only" if world > 1 else "single"},
             "clocks": clocks, "gpu_launches": launches_per_step * args.steps, "roofline": roofline,
             "status_flags": flags}

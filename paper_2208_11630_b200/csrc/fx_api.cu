@@ -181,7 +181,7 @@ extern "C" int fx_hydro_plan_set_option(fx_hydro_plan *plan, int key, double val
     plan->zchain = (int)value;
     return FX_OK;
   case FX_OPT_PATH:
-    if (value != 0.0 && value != 1.0 && value != 2.0) return fx_fail(FX_ERR_INVALID_ARG, "set_option: path must be 0, 1 or 2");
+    if (value != 0.0 && value != 1.0 && value != 2.0 && value != 3.0) return fx_fail(FX_ERR_INVALID_ARG, "set_option: path must be 0, 1, 2 or 3");
     plan->path_option = (int)value;
     return FX_OK;
   default: return fx_fail(FX_ERR_INVALID_ARG, "set_option: unknown key %d", key);
@@ -191,12 +191,13 @@ extern "C" int fx_hydro_plan_set_option(fx_hydro_plan *plan, int key, double val
 extern "C" int fx_hydro_plan_path(const fx_hydro_plan *plan) {
   if (!plan) return fx_fail(FX_ERR_INVALID_ARG, "plan_path: null plan");
   if (plan->nvars > 5) return 0;  // passive scalars [B11] are carried by the generic path only
-  if (plan->path_option == 0 && fx_stage_tma_supported(plan->P)) return 1;
+  if ((plan->path_option == 0 || plan->path_option == 3) && fx_stage_tma_supported(plan->P))
+    return (plan->path_option == 3 && fx_stage_pair_supported(plan->P)) ? 3 : 1;
   // 3-D blocks with PLM: the generic zone kernel, which gathers its halo cells itself, is ahead of the tile kernel
   // (8^3 blocks: 34.6 against 41.2 ms per step, measured); FX_OPT_PATH = 2 still selects the tile kernel
   const bool generic_ahead = plan->path_option == 0 && plan->P.active[0] && plan->P.active[1] && plan->P.active[2] &&
                              plan->P.recon == FX_RECON_PLM_MINMOD;
-  if (plan->path_option != 1 && !generic_ahead && fx_stage_tile_supported(plan->P)) return 2;
+  if (plan->path_option != 1 && plan->path_option != 3 && !generic_ahead && fx_stage_tile_supported(plan->P)) return 2;
   return 0;
 }
 

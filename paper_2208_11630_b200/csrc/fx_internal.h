@@ -83,8 +83,11 @@ int fx_launch_generic_stage(const FxParams &P, const double *X, const double *U0
                             double dt, const double *dt_dev, double beta, int first, cudaStream_t st);
 int fx_launch_debug_fluxes(const FxParams &P, const double *U, int dir, double *F, cudaStream_t st);
 bool fx_stage_tma_supported(const FxParams &P);
+bool fx_stage_pair_supported(const FxParams &P);  // the two-zones-per-thread variant: PLM, no wall, no gravity
 bool fx_stage_tile_supported(const FxParams &P);
 int fx_launch_stage_tile(const FxParams &P, const double *X, const double *U0, double *out, const double *dx, double dt,
                          const double *dt_dev, double beta, int first, cudaStream_t st);
+int fx_launch_stage_pair(const FxParams &P, const double *X, const double *U0, double *out, const double *dx, double dt,
+                         const double *dt_dev, double beta, int first, double cfl_next, double *dt_next, cudaStream_t st);
 int fx_launch_stage_tma(const FxParams &P, const double *X, const double *U0, double *out, const double *dx, double dt,
                         const double *dt_dev, double beta, int first, double cfl_next, double *dt_next, cudaStream_t st);

@@ -189,6 +189,48 @@ def test_sod_along_y_and_z(recon, riemann, rk, path):
                 assert err <= (TOL_1 if step == 0 else TOL_10), (axis, step, err)
 
 
+@pytest.mark.parametrize("kw", [dict(), dict(riemann=0, rk=3), dict(wavespeed=1), dict(bc="outflow", rk=3)])
+def test_pair_variant_of_the_fused_kernel(kw):
+    """FX_OPT_PATH = 3: the fused kernel with two zones per thread (csrc/fx_stage_pair.cu; slower, kept for comparison).
+    Same parity bar as every path, the fused dt included; uniform state bit for bit; results independent of the chain
+    length; with a wall in the table the plan falls back to the default fused kernel."""
+    from paper_2208_11630_b200 import binding as fx
+    cfg, oplan, gplan, Uh, dx = setup(5, (2, 2, 3), path=3, **kw)
+    assert gplan.path == 3
+    Uo, Ud, dxd = Uh.numpy().copy(), Uh.cuda(), torch.from_numpy(dx).cuda()
+    dt = gplan.fx_hydro_compute_dt(Ud, dxd, cfg.cfl).clone()
+    for step in range(10):
+        dto = oplan.compute_dt(Uo, dx, cfg.cfl)
+        assert abs(float(dt.item()) - dto) <= 1e-13 * dto
+        oplan.advance(Uo, dx, dto)
+        gplan.fx_hydro_step(Ud, dxd, cfg.cfl, dt)
+        if step in (0, 9):
+            err = rel_err(cfg, gplan.interior(Ud).cpu().numpy(), oplan.interior(Uo))
+            assert err <= (TOL_1 if step == 0 else TOL_10), (step, err)
+    fo, _ = oplan.status()
+    fg, _ = gplan.fx_hydro_status()
+    assert fo == fg
+    # chain length 1 gives the same bits
+    g1, _, _ = gpu_plan_for(cfg, path=3, zchain=1, **kw)
+    A, B = Uh.cuda(), Uh.cuda()
+    for _ in range(2):
+        gplan.fx_hydro_advance(A, dxd, 1e-3)
+        g1.fx_hydro_advance(B, dxd, 1e-3)
+    assert torch.equal(gplan.interior(A), g1.interior(B))
+    # uniform state
+    U = torch.full(Uh.shape, float("nan"), dtype=torch.float64)
+    I = inputs.interior_view(cfg, U)
+    for v, val in enumerate((1.3, 0.4, -0.7, 0.2, 5.9485)):
+        I[v] = val
+    U = U.cuda()
+    U0 = gplan.interior(U).clone()
+    for _ in range(5):
+        gplan.fx_hydro_advance(U, dxd, 0.01)
+    assert torch.equal(gplan.interior(U), U0)
+    wall, _, _ = gpu_plan_for(cfg, path=3, bc="reflect")
+    assert wall.path == 1
+
+
 def test_device_dt_path_equals_host_dt_path():
     cfg, oplan, gplan, Uh, dx = setup(5, (2, 2, 2))
     dxd = torch.from_numpy(dx).cuda()
