@@ -32,7 +32,7 @@ if ROOT not in sys.path:
 
 METRIC = "hydro zone-updates/s per RK stage (fp64)"
 UNIT = "zone-updates/s"
-FP64_FMA_LANES_PER_SM = 64  # 148 SMs x 64 DFMA lanes; confirmed by fx_probe_fp64_fma
+FP64_FMA_LANES_PER_SM = 64  # 64 DFMA lanes per SM (a warp-wide fp64 instruction per 2 cycles per sub-partition, measured)
 
 
 def parse_args():
@@ -52,6 +52,7 @@ def parse_args():
     ap.add_argument("--order", default="morton", choices=["lex", "morton"])
     ap.add_argument("--scalars", type=int, default=0, help="passive mass scalars carried with the 5 hydro variables (DESIGN.md B11; "
                     "nvars = 5 + this; generic path)")
+    ap.add_argument("--wavespeed", type=int, default=0, help="FX_OPT_WAVESPEED: 0 Einfeldt (the reading the configs are run with [A8]), 1 Davis")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=2)
@@ -145,6 +146,8 @@ def build_workload(args, device):
     plan = fx.HydroPlan(cfg.block_dims, cfg.nguard, cfg.nblocks, cfg.gamma, cfg.recon, cfg.riemann, cfg.rk_order,
                         nvars=5 + args.scalars, device=device)
     plan.fx_hydro_plan_set_option(fx.OPT_PATH, args.path)
+    if args.wavespeed:
+        plan.fx_hydro_plan_set_option(fx.OPT_WAVESPEED, args.wavespeed)
     guard_x = args.guard_x if args.guard_x >= 0 else (8 if (cfg.block_dims[0] == 16 and cfg.nguard == 4) else cfg.nguard)
     if guard_x != cfg.nguard:
         plan.fx_hydro_plan_set_option(fx.OPT_GUARD_X, guard_x)
@@ -163,7 +166,7 @@ def build_workload(args, device):
 
 
 # ------------------------------------------------------------------ CPU oracle legs
-def oracle_sample(args, target_seconds=15.0, steps=None):
+def oracle_sample(args, target_seconds=15.0, steps=None, steps_single=0):
     """Times the oracle as it stands on a bounded sample of the workload: a 6x6x6-block sub-tiling of the
     same field (periodic wrap of the sub-tiling), all host threads OpenMP gives it."""
     import numpy as np
@@ -194,7 +197,18 @@ def oracle_sample(args, target_seconds=15.0, steps=None):
     times = [one_step() for _ in range(steps)]
     per_step = sum(times) / len(times)
     zs = cfg.interior_zones * cfg.rk_order
-    return {"value": zs / per_step, "unit": UNIT, "cores": cores, "kind": "oracle",
+    single = None
+    if steps_single:
+        try:  # the same sample on ONE thread (SURVEY.md 8(d) asks for both figures)
+            import ctypes
+            gomp = ctypes.CDLL("libgomp.so.1")
+            gomp.omp_set_num_threads(1)
+            ts = [one_step() for _ in range(steps_single)]
+            gomp.omp_set_num_threads(cores)
+            single = {"value": zs / (sum(ts) / len(ts)), "unit": UNIT, "cores": 1, "steps": steps_single}
+        except Exception:
+            single = None
+    return {"value": zs / per_step, "unit": UNIT, "cores": cores, "kind": "oracle", "single_thread": single,
             "sample": f"config {args.config} field on a {nb[0]}x{nb[1]}x{nb[2]}-block periodic sub-tiling "
                       f"({cfg.interior_zones} zones), {steps} steps of compute_dt + advance, OpenMP over blocks",
             "ms_per_step": per_step * 1e3, "steps": steps}
@@ -215,6 +229,51 @@ def run_reference(args, rank, world):
             "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------ roofline inputs (files only; nothing under oracle/ runs here)
+def algorithmic_flops(cfg, args):
+    """Exact fp64 operations per zone and RK stage of this scheme from oracle/flop_counts.json, or None."""
+    try:
+        counts = json.load(open(os.path.join(ROOT, "oracle", "flop_counts.json")))["per_zone_stage"]
+    except Exception:
+        return None
+    key = f"{cfg.ndim}d_{'weno5' if cfg.recon else 'plm'}_{'hllc' if cfg.riemann else 'hlle'}_rk{cfg.rk_order}"
+    if args.wavespeed:
+        key += "_davis"
+    if cfg.ndim == 3 and cfg.block_dims == (8, 8, 8):
+        key += "_8cubed"
+    elif cfg.ndim == 3 and cfg.block_dims != (16, 16, 16):
+        return None
+    if args.scalars:
+        return None  # the counts are for the five hydro variables
+    return counts.get(key, {}).get("flops")
+
+
+def committed_traffic(cfg, args, plan):
+    """dram__bytes_read.sum + dram__bytes_write.sum per stage launch (mean over the stages of a step) from the committed
+    `ncu --set full` capture of this workload and path under profiles/, read by metric name; (None, None) if there is none."""
+    if args.nb or args.block or args.scalars or args.wavespeed or args.zchain or plan.gd[0] != 8:
+        return None, None
+    name = f"r2_ncu_config{cfg.number}_path{plan.path}_raw.csv"
+    path = os.path.join(ROOT, "profiles", name)
+    if not os.path.exists(path):
+        return None, None
+    import csv
+    rd = wr = None
+    for row in csv.reader(open(path)):
+        if not row:
+            continue
+        if row[0] in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
+            scale = {"Gbyte": 1e9, "Mbyte": 1e6, "Kbyte": 1e3, "byte": 1.0}.get(row[1], None)
+            vals = [float(x) * scale for x in row[2:] if x]
+            if row[0].startswith("dram__bytes_read"):
+                rd = sum(vals) / len(vals)
+            else:
+                wr = sum(vals) / len(vals)
+    if rd is None or wr is None:
+        return None, None
+    return rd + wr, f"profiles/{name}: dram__bytes_read.sum + dram__bytes_write.sum, mean over the captured stage launches"
 
 
 # ------------------------------------------------------------------ CUDA arm
@@ -269,29 +328,40 @@ def run_ours(args, rank, world, local_rank):
     ms = max_over_ranks(ms, world, device)
     value = whole_job_value(zones, stages, args.steps, ms, world)
 
-    # roofline of the dominant kernel (the stage kernel): algorithmic bytes per launch / its mean duration
+    # roofline of the dominant kernel (the stage kernel) [NS]: the slower of the minimum HBM bytes at the measured copy
+    # bandwidth and the method's fp64 operations at the fp64 peak.  Both sides are ALGORITHMIC: bytes = read X (+ U0 in the
+    # later stages) and write the result, 8 B per variable; flops = the exact count of the oracle built with a counting
+    # number type (oracle/flop_counts.json, written by oracle/count_flops.py; + - * / sqrt compare = 1 each).
     peak, peak_src = measured_peaks()
-    # B per zone: read X (+U0), write out, 8 B each per variable
     alg_bytes_stage = [16.0 * (5 + args.scalars)] + [24.0 * (5 + args.scalars)] * (stages - 1)
-    alg_bytes_per_launch = zones * sum(alg_bytes_stage) / stages
+    bytes_per_zone = sum(alg_bytes_stage) / stages
+    alg_bytes_per_launch = zones * bytes_per_zone
     stage_avg_ms = stage_ms / max(stage_launches, 1)
-    achieved = alg_bytes_per_launch / (stage_avg_ms * 1e-3) / 1e9
-    # traffic: dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture of
-    # this command (profiles/r1_ncu_chain_raw.csv: mean of the stage-1 and stage-2 launches); null for other workloads
-    gx8 = plan.gd[0] == 8
-    traffic = ((16.31e9 if gx8 else 20.35e9) if (cfg.number == 5 and args.nb is None and fused and stages == 2) else None)
-    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": traffic, "traffic_source": "ncu capture profiles/r1_ncu_gx8_raw.csv (x guard depth 8) / r1_ncu_chain_raw.csv (x guard depth 4): GB per launch, mean of both stages"
-                if traffic else None, "alg_bytes_per_launch": alg_bytes_per_launch, "peak_source": peak_src, "kernel": "fused stage kernel" if fused else "generic stage kernel",
+    stage_s = stage_avg_ms * 1e-3
+    hbm = {"achieved": alg_bytes_per_launch / stage_s / 1e9, "peak": peak, "unit": "GB/s", "peak_source": peak_src,
+           "alg_bytes_per_zone_stage": bytes_per_zone, "alg_bytes_per_launch": alg_bytes_per_launch}
+    hbm["frac"] = hbm["achieved"] / peak
+    props = torch.cuda.get_device_properties(device)
+    sm_max_mhz = clocks.get("sm_max_mhz") or 1965.0
+    # fp64 peak: SMs x 64 fp64 lanes x 2 flops (FMA) x the maximum SM clock (the guide's unit counts)
+    fp64_peak = props.multi_processor_count * FP64_FMA_LANES_PER_SM * 2 * sm_max_mhz * 1e6
+    flops = algorithmic_flops(cfg, args)
+    fp64 = None
+    if flops is not None:
+        fp64 = {"achieved": zones * flops / stage_s / 1e12, "peak": fp64_peak / 1e12, "unit": "TFLOP/s",
+                "peak_source": f"nominal: {props.multi_processor_count} SMs x {FP64_FMA_LANES_PER_SM} lanes x 2 x {sm_max_mhz:.0f} MHz",
+                "flops_per_zone_stage": flops, "flops_source": "oracle/flop_counts.json (counting build of the oracle, no FMA)"}
+        fp64["frac"] = fp64["achieved"] / fp64["peak"]
+    t_hbm, t_fp = bytes_per_zone / (peak * 1e9), (flops / fp64_peak if flops is not None else 0.0)
+    traffic, traffic_src = committed_traffic(cfg, args, plan)
+    side = fp64 if t_fp > t_hbm else hbm
+    roofline = {"bound": "alu" if side is fp64 else "hbm", "achieved": side["achieved"], "peak": side["peak"], "unit": side["unit"],
+                "frac": side["frac"], "traffic": traffic, "traffic_source": traffic_src,
+                "roof_ps_per_zone_stage": {"hbm": t_hbm * 1e12, "fp64": t_fp * 1e12 if flops is not None else None},
+                "hbm": hbm, "fp64": fp64,
+                "kernel": {1: "fused stage kernel", 3: "fused stage kernel, pair variant", 2: "tile stage kernel", 0: "generic stage kernel"}[plan.path],
                 "kernel_ms_avg": stage_avg_ms, "kernel_launches_timed": stage_launches,
-                "kernel_share_of_step": stage_ms / ms if ms > 0 else None,
-                "alg_bytes_per_zone_stage": sum(alg_bytes_stage) / stages}
-    if fused and cfg.recon == 0 and cfg.riemann == 1:
-        # the other roof [NS]: the fp64 pipe.  438 fp64-pipe lane-instructions per zone-update (ncu: 419 in stage 1, 458 in stage 2 with the CFL rate)
-        # against 148 SMs x 64 lanes x the SM clock (nominal; 17 T/s measured with fx_probe_fp64_fma)
-        fp64_peak = 148 * FP64_FMA_LANES_PER_SM * 1.965e9
-        roofline["fp64_pipe"] = {"lane_instr_per_zone_update": 438, "peak_lane_instr_per_s": fp64_peak,
-                                 "frac": 438 * zones / (stage_avg_ms * 1e-3) / fp64_peak}
+                "kernel_share_of_step": stage_ms / ms if ms > 0 else None}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
@@ -299,7 +369,8 @@ def run_ours(args, rank, world, local_rank):
             "config": {"workload": f"config {cfg.number}: {cfg.name}, {cfg.nblocks} blocks of "
                                    f"{cfg.block_dims[0]}x{cfg.block_dims[1]}x{cfg.block_dims[2]} (+{cfg.nguard} guard), "
                                    f"{'WENO5' if cfg.recon else 'PLM-minmod'}+{'HLLC' if cfg.riemann else 'HLLE'}, SSP-RK{stages}"
-                                   + (f", {args.scalars} passive mass scalars" if args.scalars else ""),
+                                   + (f", {args.scalars} passive mass scalars" if args.scalars else "")
+                                   + (", Davis wave speeds" if args.wavespeed else ""),
                        "interior_zones": zones, "state_bytes": plan.bytes_per_state, "block_order": args.order,
                        "layout": f"x guard depth {plan.gd[0]} (row pitch {plan.S_j * 8} B), y/z guard depth {plan.gd[1]}/{plan.gd[2]}",
                        "path": {0: "generic", 1: "fused (TMA)", 2: "tile (shared-memory block)", 3: "fused (TMA), two zones per thread"}[plan.path], "l2": "inputs (state) larger than L2; no flush needed",
@@ -337,7 +408,8 @@ def run_ours(args, rank, world, local_rank):
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         del U
         torch.cuda.empty_cache()
-        line["cpu_baseline"] = {k: v for k, v in oracle_sample(args).items() if k in ("value", "unit", "cores", "kind", "sample")}
+        line["cpu_baseline"] = {k: v for k, v in oracle_sample(args, steps_single=2).items()
+                                if k in ("value", "unit", "cores", "kind", "sample", "single_thread")}
     if rank == 0:
         print(json.dumps(line), flush=True)
     if world > 1:
