@@ -8,8 +8,11 @@ stage = interior zones x stages / time.  Workload at N = 1: BASELINE.json config
 PLM-minmod + HLLC, SSP-RK2; 24.2 GB per state copy in the wide layout bench.py picks for 16-wide blocks
 (--guard-x, FX_OPT_GUARD_X; 18.1 GB in the compact one), far larger than the 126 MB L2, so nothing is served
 from cache between timed iterations).  e2e: the same step through fx_hydro_advance_host_interior, the host
-holding the interior zones in a pinned buffer (5.37 GB each way per step inside the timed region).  N > 1: N independent replicas of that workload, one per rank
-("replicas only", DESIGN.md section Multi-GPU); no data-path collective is invented.
+holding the interior zones in a pinned buffer (5.37 GB each way per step inside the timed region).  N > 1 (weak scaling):
+the config's tiling grown N-fold (z, then y, then x doubled), cut into N contiguous Morton runs, one per rank
+(paper_2208_11630_b200/sharded.py): before every stage the cut-face slabs of its input are packed,
+exchanged (grouped NCCL send/recv) and unpacked into ghost blocks; dt is the all-reduced minimum.  Started plainly with
+--gpus N (no WORLD_SIZE in the environment) bench.py launches its N ranks itself.
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 5] [--nb a,b,c]
 
@@ -53,6 +56,8 @@ def parse_args():
     ap.add_argument("--scalars", type=int, default=0, help="passive mass scalars carried with the 5 hydro variables (DESIGN.md B11; "
                     "nvars = 5 + this; generic path)")
     ap.add_argument("--wavespeed", type=int, default=0, help="FX_OPT_WAVESPEED: 0 Einfeldt (the reading the configs are run with [A8]), 1 Davis")
+    ap.add_argument("--shard", action="store_true", help="drive the step through ShardedHydro even on one rank (the N > 1 code path with an "
+                    "empty exchange; N > 1 always uses it)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=2)
@@ -163,6 +168,48 @@ def build_workload(args, device):
         Ui[:, b0:b1] = inputs.with_scalars(cfg, coords[b0:b1], inputs.block_interiors(cfg, coords[b0:b1], device), args.scalars)
     dx = torch.from_numpy(inputs.dx_array(cfg)).to(device)
     return cfg, plan, U, dx, coords
+
+
+def shard_factors(world):
+    """How the config's tiling grows with the number of ranks (weak scaling): powers of two double z, then y, then x."""
+    f, d, w = [1, 1, 1], 2, world
+    while w % 2 == 0 and w > 1:
+        f[d] *= 2
+        d = (d - 1) % 3
+        w //= 2
+    f[2] *= w  # an odd remainder goes to z
+    return tuple(f)
+
+
+def build_sharded_workload(args, device, rank, world):
+    """N > 1: the config's tiling grown by shard_factors(world) (its field continued periodically), cut into `world`
+    contiguous Morton runs, one per rank; every rank holds its run plus the ghost blocks behind its cuts."""
+    import numpy as np
+    import torch
+    from paper_2208_11630_b200 import binding as fx
+    from paper_2208_11630_b200 import inputs
+    from paper_2208_11630_b200.sharded import ShardedHydro
+    base = inputs.config(args.config, nb=tuple(int(x) for x in args.nb.split(",")) if args.nb else None)
+    f = shard_factors(world)
+    cfg = inputs.config(args.config, nb=tuple(base.nb[d] * f[d] for d in range(3)))
+    if args.block:
+        import dataclasses
+        cfg = dataclasses.replace(cfg, block_dims=tuple(int(x) for x in args.block.split(",")))
+    code = fx.TOPO_PERIODIC if cfg.bc == "periodic" else fx.TOPO_OUTFLOW
+    bcs = [code if cfg.block_dims[d] > 1 else fx.TOPO_NONE for d in range(3)]
+    neigh, coords = fx.fx_topology_cartesian(cfg.nb, bcs, bcs, fx.ORDER_MORTON if args.order == "morton" else fx.ORDER_LEX)
+    guard_x = args.guard_x if args.guard_x >= 0 else (8 if (cfg.block_dims[0] == 16 and cfg.nguard == 4) else cfg.nguard)
+    sh = ShardedHydro(cfg.block_dims, cfg.nguard, cfg.gamma, cfg.recon, cfg.riemann, cfg.rk_order, neigh, rank, world, device=device,
+                      guard_x=guard_x, nvars=5 + args.scalars, zchain=args.zchain, wavespeed=args.wavespeed)
+    U = sh.alloc_state(fill=float("nan"))
+    gid = sh.shard.global_id
+    Ui = sh.interior(U)
+    for b0 in range(0, sh.n_owned, 1024):
+        b1 = min(sh.n_owned, b0 + 1024)
+        c = coords[gid[b0:b1]]
+        Ui[:, b0:b1] = inputs.with_scalars(cfg, c, inputs.block_interiors(cfg, c, device), args.scalars)
+    dx = torch.from_numpy(np.ascontiguousarray(inputs.dx_array(cfg)[:sh.n_local])).to(device)
+    return cfg, sh, U, dx
 
 
 # ------------------------------------------------------------------ CPU oracle legs
@@ -287,17 +334,30 @@ def run_ours(args, rank, world, local_rank):
     device = torch.device("cuda", local_rank)
     if world > 1:
         dist.init_process_group("nccl", device_id=device)
-    cfg, plan, U, dx, coords = build_workload(args, device)
+    sh = None
+    if world > 1 or args.shard:
+        cfg, sh, U, dx = build_sharded_workload(args, device, rank, world)
+        plan = sh.plan
+        zones = sh.n_owned * cfg.block_dims[0] * cfg.block_dims[1] * cfg.block_dims[2]  # this rank's share
+    else:
+        cfg, plan, U, dx, coords = build_workload(args, device)
+        zones = cfg.interior_zones
     stages = cfg.rk_order
-    zones = cfg.interior_zones
     fused = plan.path in (1, 3)
     # fused path: one launch per RK stage, the CFL reduction (a7) rides in the last one; tile and generic paths: one
     # stage kernel per stage, then the reduction pass; with passive scalars also their face fill per stage
     launches_per_step = stages if fused else (stages + 1 + (stages if args.scalars else 0))
-    dt = plan.fx_hydro_compute_dt(U, dx, cfg.cfl).clone()  # the first step's dt; stays on the device from here on
+    if sh is not None:
+        launches_per_step += (int(sh.send_elems > 0) + int(sh.recv_elems > 0)) * stages  # pack + unpack of the cut-face slabs before every stage
+        dt = sh.compute_dt(U, dx, cfg.cfl)  # the minimum over the ranks
 
-    def step():
-        plan.fx_hydro_step(U, dx, cfg.cfl, dt)  # a1..a6 with this dt, a7 of the advanced state into dt
+        def step():
+            sh.step(U, dx, cfg.cfl, dt)  # per stage: slab exchange, then the stage on the owned blocks; dt <- min over ranks
+    else:
+        dt = plan.fx_hydro_compute_dt(U, dx, cfg.cfl).clone()  # the first step's dt; stays on the device from here on
+
+        def step():
+            plan.fx_hydro_step(U, dx, cfg.cfl, dt)  # a1..a6 with this dt, a7 of the advanced state into dt
 
     def barrier():
         if world > 1:
@@ -326,6 +386,7 @@ def run_ours(args, rank, world, local_rank):
     plan.fx_hydro_plan_set_timing(False)
     flags, counts = plan.fx_hydro_status()
     ms = max_over_ranks(ms, world, device)
+    # whole job: every rank's owned zone-updates over the slowest rank's time (ranks own equal shares of the grown tiling)
     value = whole_job_value(zones, stages, args.steps, ms, world)
 
     # roofline of the dominant kernel (the stage kernel) [NS]: the slower of the minimum HBM bytes at the measured copy
@@ -374,12 +435,42 @@ def run_ours(args, rank, world, local_rank):
                        "interior_zones": zones, "state_bytes": plan.bytes_per_state, "block_order": args.order,
                        "layout": f"x guard depth {plan.gd[0]} (row pitch {plan.S_j * 8} B), y/z guard depth {plan.gd[1]}/{plan.gd[2]}",
                        "path": {0: "generic", 1: "fused (TMA)", 2: "tile (shared-memory block)", 3: "fused (TMA), two zones per thread"}[plan.path], "l2": "inputs (state) larger than L2; no flush needed",
-                       "multi_gpu": "replicas only" if world > 1 else "single"},
+                       "multi_gpu": (f"sharded: tiling {cfg.nb[0]}x{cfg.nb[1]}x{cfg.nb[2]} blocks in {world} contiguous Morton runs, "
+                                     f"{sh.shard.n_ghost} ghost blocks on rank 0, cut-face slabs exchanged before every stage "
+                                     f"(grouped NCCL send/recv, {sh.send_elems * 8} B sent by rank 0 per stage), dt = all-reduce(min)")
+                       if sh is not None else "single"},
             "clocks": clocks, "gpu_launches": launches_per_step * args.steps, "roofline": roofline,
             "status_flags": flags}
 
     # end to end through the C ABI with HOST buffers (H2D + steps + D2H inside the timed region)
-    if not args.no_e2e:
+    if not args.no_e2e and sh is not None:
+        try:  # H2D of the owned interiors from pinned memory, one sharded step, D2H of the result, per step
+            Uh = torch.empty(tuple(sh.interior(U).shape), dtype=torch.float64, pin_memory=True)
+            Uh.copy_(sh.interior(U))
+            dth = torch.empty(1, dtype=torch.float64, pin_memory=True)
+
+            def e2e_step():
+                sh.interior(U).copy_(Uh, non_blocking=True)
+                d = sh.compute_dt(U, dx, cfg.cfl)
+                sh.step(U, dx, cfg.cfl, d)
+                Uh.copy_(sh.interior(U), non_blocking=True)
+                dth.copy_(d, non_blocking=True)
+                torch.cuda.synchronize()
+
+            e2e_step()
+            barrier()
+            tt = time.perf_counter()
+            for _ in range(args.e2e_steps):
+                e2e_step()
+            es = max_over_ranks((time.perf_counter() - tt) / args.e2e_steps, world, device)
+            line["e2e"] = {"value": world * zones * stages / es, "unit": UNIT, "h2d_bytes_per_step": Uh.numel() * 8,
+                           "d2h_bytes_per_step": Uh.numel() * 8 + 8, "ms_per_step": es * 1e3, "steps": args.e2e_steps,
+                           "api": "ShardedHydro: copy of the owned interiors from pinned host memory into the padded device state, "
+                                  "compute_dt + step (exchange, stages, all-reduce), copy back; per rank, max over ranks"}
+            del Uh
+        except Exception as ex:
+            line["e2e"] = {"value": None, "unit": UNIT, "error": repr(ex)[:200]}
+    elif not args.no_e2e:
         try:
             # the host holds the interior zones (guard zones carry no information): [5][nblocks][nz][ny][nx], pinned
             Uh = torch.empty(plan.interior_shape, dtype=torch.float64, pin_memory=True)
@@ -421,6 +512,16 @@ def main():
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.impl != "reference":
+        # started plainly with --gpus N: launch the N ranks ourselves (one process per GPU, NCCL), as the driver's torchrun would
+        import socket
+        sk = socket.socket()
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+        sk.close()
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1",
+               "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+        sys.exit(subprocess.call(cmd))
     if args.impl == "reference":
         run_reference(args, rank, world)
     else:

@@ -63,9 +63,12 @@ enum {
   FX_OPT_GRAVITY_X = 6, /* constant acceleration g_x (default 0): every stage adds beta dt (0, rho g, g.m) [B10] */
   FX_OPT_GRAVITY_Y = 7,
   FX_OPT_GRAVITY_Z = 8,
-  FX_OPT_GUARD_X = 9    /* guard depth of the x dimension alone, an integer in [nguard, nx] (default nguard).  CHANGES THE
+  FX_OPT_GUARD_X = 9,   /* guard depth of the x dimension alone, an integer in [nguard, nx] (default nguard).  CHANGES THE
                            LAYOUT (np[0], strides: query fx_hydro_plan_layout again); set it before workspace and
                            topology.  See "Layout and DRAM lines" below: 8 with nx = 16 makes the row pitch 256 bytes. */
+  FX_OPT_OWNED_BLOCKS = 10 /* sharded runs [SURVEY 8(e)]: blocks [0, value) are advanced, blocks [value, nblocks) are
+                           GHOST blocks -- copies of other ranks' blocks, read as halo sources and never written by a stage
+                           (fx_shard_* builds the numbering).  Default nblocks.  Set before fx_hydro_plan_set_topology. */
 };
 enum {
   FX_STATUS_NONFINITE = 1u,
@@ -206,6 +209,46 @@ int fx_hydro_status_reset(fx_hydro_plan *plan, void *stream);
  * already filled [A17]: F_dev[v][b][k][j][i], extents (nz, ny, nx) with n_dir + 1 along dir, i fastest;
  * face f lies between padded cells gd+f-1 and gd+f.  Not on the timed path. */
 int fx_debug_compute_fluxes(fx_hydro_plan *plan, const double *U_dev, int dir, double *F_dev, void *stream);
+
+/* ---- Sharded runs over several GPUs, one process per GPU [SURVEY.md 8(e); PAPER.md L75 (MPI between ranks), L69 (blocks
+ * are independent within a stage once their boundaries are resolved)].  The library itself talks to no other process:
+ * it provides the partition (host index logic), the owned/ghost split of a plan (FX_OPT_OWNED_BLOCKS), one RK stage at a
+ * time, and the pack / unpack kernels of the face slabs; the caller moves the packed buffers between ranks (the Python
+ * binding: torch.distributed all_to_all over NCCL) and takes the minimum of the ranks' time steps.
+ *
+ * Partition: rank r owns the contiguous run [N r / nranks, N (r+1) / nranks) of the global block order (Morton runs if
+ * the table came from fx_topology_cartesian(..., FX_ORDER_MORTON)).  Local numbering: the owned blocks in global order,
+ * then one ghost block per foreign block an owned block names, ascending global id.  neigh_global_host: the global table
+ * [N][6] on the host, the same on every rank.  Items: (local block, side 0..5 = -x +x -y +y -z +z) = the slab of depth R
+ * (2 PLM, 3 WENO5) of that block's INTERIOR behind that face, all variables, packed [v][k][j][i] over the slab's extents;
+ * send items name owned blocks, receive items ghost blocks; both are grouped by peer rank (counts per peer) and ordered
+ * by (global block id, side) inside a group, so that the two ends of an exchange agree without talking. */
+typedef struct fx_shard fx_shard;
+int fx_shard_create(fx_shard **out, int64_t nblocks_global, const int32_t *neigh_global_host, int nranks, int rank);
+int fx_shard_destroy(fx_shard *shard);
+int fx_shard_sizes(const fx_shard *shard, int64_t *owned_begin, int64_t *n_owned, int64_t *n_ghost, int64_t *n_send_items,
+                   int64_t *n_recv_items);
+/* neigh_local_host [n_owned + n_ghost][6] (ghost rows: FX_BC_OUTFLOW, never resolved by a stage), global_id_host [n_owned + n_ghost] */
+int fx_shard_tables(const fx_shard *shard, int32_t *neigh_local_host, int64_t *global_id_host);
+/* send_items_host [n_send][2], recv_items_host [n_recv][2] (either may be NULL), *_counts_host [nranks] */
+int fx_shard_items(const fx_shard *shard, int32_t *send_items_host, int64_t *send_counts_host, int32_t *recv_items_host,
+                   int64_t *recv_counts_host);
+/* Elements (doubles) of one item on `side` for this plan: nvars x R x the two other extents (0 for an inactive dimension). */
+int64_t fx_halo_item_elems(const fx_hydro_plan *plan, int side);
+/* Gather the items' slabs of U into buf / scatter buf into the items' slabs of U.  items_dev int32 [n][2], offsets_dev int64
+ * [n] (element offset of each item in buf); all device pointers, caller-owned; enqueue only. */
+int fx_halo_pack(fx_hydro_plan *plan, const double *U, const int32_t *items_dev, const int64_t *offsets_dev, int64_t n, double *buf,
+                 void *stream);
+int fx_halo_unpack(fx_hydro_plan *plan, double *U, const int32_t *items_dev, const int64_t *offsets_dev, int64_t n, const double *buf,
+                   void *stream);
+/* One RK stage (stage = 0 .. rk_order - 1, to be called in order) of the step fx_hydro_advance takes [O6]: the caller acts
+ * between stages (exchange of the ghost slabs of the stage's input).  dt_dev != NULL: dt is read on the device.  dt_next_dev
+ * (last stage only, may be NULL): receives cfl_next times the CFL minimum over the OWNED blocks of the advanced state.
+ * fx_hydro_stage_arrays: the array stage `stage` reads (whose ghosts must be current) and the one it writes -- U or a stage
+ * copy inside the workspace. */
+int fx_hydro_advance_stage(fx_hydro_plan *plan, double *U, const double *dx_dev, double dt, const double *dt_dev, int stage,
+                           double cfl_next, double *dt_next_dev, void *stream);
+int fx_hydro_stage_arrays(fx_hydro_plan *plan, double *U, int stage, double **stage_input, double **stage_output);
 
 /* Which stage kernel fx_hydro_advance will use for this plan: 0 generic (zone kernel that reads its halo cells through
  * the neighbour table; the only path for plans with passive scalars, whose face guard zones it fills first),

@@ -134,9 +134,12 @@ class OraclePlan:
         self._neigh = None
 
     def __del__(self):
-        if getattr(self, "_h", None) and self._h.value:
-            lib().fxo_plan_destroy(self._h)
-            self._h = C.c_void_p()
+        try:
+            if getattr(self, "_h", None) and self._h.value:
+                lib().fxo_plan_destroy(self._h)
+                self._h = C.c_void_p()
+        except Exception:  # interpreter shutdown
+            pass
 
     @property
     def shape(self):

@@ -21,7 +21,7 @@ BC_OUTFLOW, BC_NONE, BC_REFLECT = -1, -2, -3
 TOPO_PERIODIC, TOPO_OUTFLOW, TOPO_NONE, TOPO_REFLECT = 0, 1, 2, 3
 ORDER_LEX, ORDER_MORTON = 0, 1
 OPT_RHO_FLOOR, OPT_P_FLOOR, OPT_WENO_EPS, OPT_WAVESPEED, OPT_PATH, OPT_ZCHAIN = 0, 1, 2, 3, 4, 5
-OPT_GRAVITY_X, OPT_GRAVITY_Y, OPT_GRAVITY_Z, OPT_GUARD_X = 6, 7, 8, 9
+OPT_GRAVITY_X, OPT_GRAVITY_Y, OPT_GRAVITY_Z, OPT_GUARD_X, OPT_OWNED_BLOCKS = 6, 7, 8, 9, 10
 STATUS_NONFINITE, STATUS_RHO_FLOOR, STATUS_P_FLOOR, STATUS_WENO_FALLBACK = 1, 2, 4, 8
 
 EXPORTS = [
@@ -31,6 +31,8 @@ EXPORTS = [
     "fx_hydro_compute_dt", "fx_hydro_advance", "fx_hydro_advance_host", "fx_hydro_advance_host_interior", "fx_hydro_advance_devdt", "fx_hydro_step",
     "fx_hydro_status", "fx_hydro_status_reset", "fx_debug_compute_fluxes", "fx_hydro_plan_path",
     "fx_hydro_plan_set_timing", "fx_hydro_plan_get_timing",
+    "fx_shard_create", "fx_shard_destroy", "fx_shard_sizes", "fx_shard_tables", "fx_shard_items", "fx_halo_item_elems",
+    "fx_halo_pack", "fx_halo_unpack", "fx_hydro_advance_stage", "fx_hydro_stage_arrays",
 ]
 
 
@@ -82,6 +84,18 @@ def lib():
         L.fx_hydro_plan_path.argtypes = [vp]
         L.fx_hydro_plan_set_timing.argtypes = [vp, C.c_int]
         L.fx_hydro_plan_get_timing.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
+        p64 = C.POINTER(C.c_int64)
+        L.fx_shard_create.argtypes = [C.POINTER(vp), C.c_int64, vp, C.c_int, C.c_int]
+        L.fx_shard_destroy.argtypes = [vp]
+        L.fx_shard_sizes.argtypes = [vp, p64, p64, p64, p64, p64]
+        L.fx_shard_tables.argtypes = [vp, vp, vp]
+        L.fx_shard_items.argtypes = [vp, vp, vp, vp, vp]
+        L.fx_halo_item_elems.argtypes = [vp, C.c_int]
+        L.fx_halo_item_elems.restype = C.c_int64
+        L.fx_halo_pack.argtypes = [vp, vp, vp, vp, C.c_int64, vp, vp]
+        L.fx_halo_unpack.argtypes = [vp, vp, vp, vp, C.c_int64, vp, vp]
+        L.fx_hydro_advance_stage.argtypes = [vp, vp, vp, C.c_double, vp, C.c_int, C.c_double, vp, vp]
+        L.fx_hydro_stage_arrays.argtypes = [vp, vp, C.c_int, C.POINTER(vp), C.POINTER(vp)]
         _lib = L
     return _lib
 
@@ -110,6 +124,41 @@ def fx_topology_cartesian(nb, bc_lo, bc_hi, order=ORDER_LEX):
     _check(lib().fx_topology_cartesian(i3(*nb), i3(*bc_lo), i3(*bc_hi), order, C.c_void_p(neigh.ctypes.data),
                                        C.c_void_p(coords.ctypes.data)))
     return neigh, coords
+
+
+class Shard:
+    """fx_shard: rank `rank`'s part of a block batch cut into `nranks` contiguous runs (host index logic only; no GPU).
+    Attributes: owned_begin, n_owned, n_ghost, neigh_local int32 [n_local, 6], global_id int64 [n_local],
+    send_items / recv_items int32 [n, 2] (local block, side), send_counts / recv_counts int64 [nranks] (items per peer)."""
+
+    def __init__(self, neigh_global, nranks, rank):
+        neigh_global = np.ascontiguousarray(neigh_global, np.int32)
+        self._h = C.c_void_p()
+        _check(lib().fx_shard_create(C.byref(self._h), neigh_global.shape[0], C.c_void_p(neigh_global.ctypes.data), nranks, rank))
+        v = [C.c_int64() for _ in range(5)]
+        _check(lib().fx_shard_sizes(self._h, *[C.byref(x) for x in v]))
+        self.owned_begin, self.n_owned, self.n_ghost, n_send, n_recv = (int(x.value) for x in v)
+        self.n_local, self.nranks, self.rank = self.n_owned + self.n_ghost, nranks, rank
+        self.neigh_local = np.empty((self.n_local, 6), np.int32)
+        self.global_id = np.empty(self.n_local, np.int64)
+        _check(lib().fx_shard_tables(self._h, C.c_void_p(self.neigh_local.ctypes.data), C.c_void_p(self.global_id.ctypes.data)))
+        self.send_items, self.recv_items = np.empty((n_send, 2), np.int32), np.empty((n_recv, 2), np.int32)
+        self.send_counts, self.recv_counts = np.empty(nranks, np.int64), np.empty(nranks, np.int64)
+        _check(lib().fx_shard_items(self._h, C.c_void_p(self.send_items.ctypes.data), C.c_void_p(self.send_counts.ctypes.data),
+                                    C.c_void_p(self.recv_items.ctypes.data), C.c_void_p(self.recv_counts.ctypes.data)))
+
+    def __del__(self):
+        try:
+            if getattr(self, "_h", None) and self._h.value:
+                lib().fx_shard_destroy(self._h)
+                self._h = C.c_void_p()
+        except Exception:  # interpreter shutdown
+            pass
+
+
+def _ptr(x, dtype=torch.float64):
+    """A device tensor or a raw device address (the stage copies live inside the workspace)."""
+    return C.c_void_p(int(x)) if isinstance(x, int) else _dev(x, dtype)
 
 
 class HydroPlan:
@@ -222,6 +271,30 @@ class HydroPlan:
         """Advance by the device-resident dt (a 1-element float64 CUDA tensor) and overwrite it with the next step's dt."""
         _check(lib().fx_hydro_step(self._h, _dev(U, torch.float64), _dev(dx, torch.float64), float(cfl),
                                    _dev(dt, torch.float64), _stream(stream)))
+
+    def fx_hydro_stage_arrays(self, U, stage):
+        """(address of the array stage `stage` reads, address of the one it writes): U or a stage copy in the workspace."""
+        a, b = C.c_void_p(), C.c_void_p()
+        _check(lib().fx_hydro_stage_arrays(self._h, _dev(U, torch.float64), stage, C.byref(a), C.byref(b)))
+        return int(a.value), int(b.value)
+
+    def fx_hydro_advance_stage(self, U, dx, dt, stage, cfl_next=0.0, dt_next=None, stream=None):
+        """One RK stage; dt a float or a device scalar; dt_next (last stage): device scalar receiving the next time step."""
+        on_dev = isinstance(dt, torch.Tensor)
+        _check(lib().fx_hydro_advance_stage(self._h, _dev(U, torch.float64), _dev(dx, torch.float64), 0.0 if on_dev else float(dt),
+                                            _dev(dt, torch.float64) if on_dev else None, stage, float(cfl_next),
+                                            _dev(dt_next, torch.float64) if dt_next is not None else None, _stream(stream)))
+
+    def fx_halo_item_elems(self, side):
+        return int(lib().fx_halo_item_elems(self._h, side))
+
+    def fx_halo_pack(self, U, items, offsets, buf, stream=None):
+        _check(lib().fx_halo_pack(self._h, _ptr(U), _dev(items, torch.int32), _dev(offsets, torch.int64), items.shape[0],
+                                  _dev(buf, torch.float64), _stream(stream)))
+
+    def fx_halo_unpack(self, U, items, offsets, buf, stream=None):
+        _check(lib().fx_halo_unpack(self._h, _ptr(U), _dev(items, torch.int32), _dev(offsets, torch.int64), items.shape[0],
+                                    _dev(buf, torch.float64), _stream(stream)))
 
     @property
     def interior_shape(self):

@@ -91,6 +91,7 @@ extern "C" int fx_hydro_plan_create(fx_hydro_plan **out, const int block_dims[3]
     return fx_fail(FX_ERR_INVALID_ARG, "plan_create: no active dimension");
   }
   P.nblocks = nblocks;
+  P.nown = nblocks;
   if (fx_relayout(p)) {
     delete p;
     return fx_fail(FX_ERR_INVALID_ARG, "plan_create: padded block too large");
@@ -179,6 +180,12 @@ extern "C" int fx_hydro_plan_set_option(fx_hydro_plan *plan, int key, double val
   case FX_OPT_ZCHAIN:
     if (!(value >= 0.0 && value <= (double)FX_SEG_MAX)) return fx_fail(FX_ERR_INVALID_ARG, "set_option: zchain must be 0 (auto) or 1..%d", (int)FX_SEG_MAX);
     plan->zchain = (int)value;
+    return FX_OK;
+  case FX_OPT_OWNED_BLOCKS:
+    if (!(value >= 0.0 && value <= (double)plan->P.nblocks) || value != floor(value))
+      return fx_fail(FX_ERR_INVALID_ARG, "set_option: owned blocks must be an integer in [0, nblocks]");
+    if (plan->topology_set) return fx_fail(FX_ERR_STATE, "set_option: FX_OPT_OWNED_BLOCKS must be set before the topology");
+    plan->P.nown = (long long)value;
     return FX_OK;
   case FX_OPT_PATH:
     if (value != 0.0 && value != 1.0 && value != 2.0 && value != 3.0) return fx_fail(FX_ERR_INVALID_ARG, "set_option: path must be 0, 1, 2 or 3");
@@ -282,15 +289,16 @@ extern "C" int fx_hydro_plan_set_topology(fx_hydro_plan *plan, const int32_t *ne
     std::vector<int32_t> h((size_t)nb * 6);
     FX_CUDA(cudaMemcpy(h.data(), neigh_dev, h.size() * sizeof(int32_t), cudaMemcpyDeviceToHost));
     const bool zact = plan->P.active[2] != 0;
+    const long long nown = plan->P.nown;  // chains run through owned blocks only; a ghost block ends one (and is its halo)
     auto up = [&](long long b) -> long long {  // the block above b if the link is mutual, else -1
       if (!zact) return -1;
       const long long a = h[b * 6 + 5];
-      return (a >= 0 && a != b && h[a * 6 + 4] == b) ? a : -1;
+      return (a >= 0 && a < nown && a != b && h[a * 6 + 4] == b) ? a : -1;
     };
     auto down = [&](long long b) -> long long {
       if (!zact) return -1;
       const long long a = h[b * 6 + 4];
-      return (a >= 0 && a != b && h[a * 6 + 5] == b) ? a : -1;
+      return (a >= 0 && a < nown && a != b && h[a * 6 + 5] == b) ? a : -1;
     };
     for (long long b = 0; b < nb; ++b)
       for (int f = 0; f < 6; ++f)
@@ -307,7 +315,7 @@ extern "C" int fx_hydro_plan_set_topology(fx_hydro_plan *plan, const int32_t *ne
       const long long slots = (long long)sms * (plan->P.recon == FX_RECON_WENO5 ? 1 : 2);
       double best = 0.0;
       for (int m = 1; m <= FX_SEG_MAX; m *= 2) {
-        const long long nseg = (nb + m - 1) / m;
+        const long long nseg = (nown + m - 1) / m;
         const double cost = (double)((nseg + slots - 1) / slots) * (m + 0.09);
         if (M <= 0 || cost < best) {
           best = cost;
@@ -316,7 +324,7 @@ extern "C" int fx_hydro_plan_set_topology(fx_hydro_plan *plan, const int32_t *ne
       }
     }
     if (plan->P.n[2] > 64) M = 1;
-    for (long long b0 = 0; b0 < nb; ++b0) {
+    for (long long b0 = 0; b0 < nown; ++b0) {
       if (seen[b0]) continue;
       long long start = b0;
       for (long long steps = 0; steps < nb; ++steps) {

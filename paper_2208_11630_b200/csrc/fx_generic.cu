@@ -339,7 +339,7 @@ __global__ void __launch_bounds__(128) fx_k_debug_fluxes(FxParams P, const doubl
 
 int fx_launch_generic_stage(const FxParams &P, const double *X, const double *U0, double *out, const double *dx,
                             double dt, const double *dt_dev, double beta, int first, cudaStream_t st) {
-  const long long nzones = P.nblocks * P.n[0] * P.n[1] * P.n[2];
+  const long long nzones = P.nown * P.n[0] * P.n[1] * P.n[2];  // owned blocks come first
   if (nzones == 0) return FX_OK;
   const unsigned grid = (unsigned)((nzones + 127) / 128);
 #define CALL(RC, RM)                                                                                              \

@@ -199,7 +199,7 @@ __global__ void __launch_bounds__(256) fx_k_compute_dt(FxParams P, const double 
   // 16-byte loads need every zone pair (i even) on a 16-byte boundary: even nx, guard depth and strides, aligned base
   const bool pairs = (nx % 2 == 0) && (P.gd[0] % 2 == 0) && (P.S_j % 2 == 0) && (P.S_v % 2 == 0) &&
                      ((reinterpret_cast<unsigned long long>(U) & 15ull) == 0);
-  for (long long b = blockIdx.x; b < P.nblocks; b += gridDim.x) {
+  for (long long b = blockIdx.x; b < P.nown; b += gridDim.x) {  // owned blocks only (a shard's ghosts are halo sources)
     double idx[3];
 #pragma unroll
     for (int d = 0; d < 3; ++d) idx[d] = P.active[d] ? 1.0 / __ldg(&dx[b * 3 + d]) : 0.0;
@@ -286,7 +286,7 @@ __global__ void __launch_bounds__(256) fx_k_compute_dt(FxParams P, const double 
 
 int fx_launch_compute_dt(const FxParams &P, const double *U, const double *dx, double cfl, double *dt_out,
                          cudaStream_t st) {
-  const long long want = P.nblocks < 1 ? 1 : P.nblocks;
+  const long long want = P.nown < 1 ? 1 : P.nown;
   const long long cap = (long long)fx_sm_count() * 8;
   const int grid = (int)(want > cap ? cap : want);
   fx_k_compute_dt<<<grid, 256, 0, st>>>(P, U, dx, cfl, dt_out);

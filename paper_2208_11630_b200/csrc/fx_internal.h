@@ -14,6 +14,7 @@ struct FxParams {
   int nvars;      // 5 hydro variables + passive mass scalars [B11]
   long long S_j, S_k, S_b, S_v;  // element strides of U[v][b][k][j][i]
   long long nblocks;
+  long long nown;                   // blocks [0, nown) are advanced; [nown, nblocks) are ghost blocks of a shard: halo sources only
   double gamma, gm1, igm1;
   double rho_floor, p_floor, weno_eps;
   int recon, riemann, wavespeed;

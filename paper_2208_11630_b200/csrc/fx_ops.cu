@@ -96,9 +96,43 @@ extern "C" int fx_hydro_plan_get_timing(fx_hydro_plan *plan, double *ms_sum, lon
   return FX_OK;
 }
 
+// Stage s of the step: input X_s, output, beta_s [O6].  The last stage may overwrite U0 in place: its halos come from
+// U1 (RK2) / U2 (RK3), never from U0.
+static void fx_stage_arrays(fx_hydro_plan *plan, double *U, int s, double **X, double **out, double *beta) {
+  double *U1 = plan->stage[0], *U2 = plan->stage[1];
+  const bool last = s == plan->rk - 1;
+  *X = s == 0 ? U : (s == 1 ? U1 : U2);
+  *out = last ? U : (s == 0 ? U1 : U2);
+  *beta = s == 0 ? 1.0 : (plan->rk == 2 ? 0.5 : (s == 1 ? 0.25 : 2.0 / 3.0));
+}
+
+extern "C" int fx_hydro_stage_arrays(fx_hydro_plan *plan, double *U, int stage, double **stage_input, double **stage_output) {
+  int rc = fx_need(plan, false, true, "stage_arrays");
+  if (rc) return rc;
+  if (stage < 0 || stage >= plan->rk || !stage_input || !stage_output) return fx_fail(FX_ERR_INVALID_ARG, "stage_arrays: bad stage or null output");
+  double beta;
+  fx_stage_arrays(plan, U, stage, stage_input, stage_output, &beta);
+  return FX_OK;
+}
+
+extern "C" int fx_hydro_advance_stage(fx_hydro_plan *plan, double *U, const double *dx, double dt, const double *dt_dev, int stage,
+                                      double cfl_next, double *dt_next_dev, void *stream) {
+  int rc = fx_need(plan, true, true, "advance_stage");
+  if (rc) return rc;
+  if (stage < 0 || stage >= plan->rk) return fx_fail(FX_ERR_INVALID_ARG, "advance_stage: stage must be 0 .. rk_order - 1");
+  if (!dt_dev && (!(dt > 0.0) || !isfinite(dt))) return fx_fail(FX_ERR_INVALID_ARG, "advance_stage: dt must be positive and finite");
+  if ((!U || !dx) && plan->P.nblocks > 0) return fx_fail(FX_ERR_INVALID_ARG, "advance_stage: null argument");
+  if (dt_next_dev && stage != plan->rk - 1) return fx_fail(FX_ERR_INVALID_ARG, "advance_stage: the next time step comes out of the last stage only");
+  if (dt_next_dev && (!(cfl_next > 0.0) || !isfinite(cfl_next))) return fx_fail(FX_ERR_INVALID_ARG, "advance_stage: cfl must be positive and finite");
+  if (plan->P.nown == 0) return FX_OK;
+  double *X, *out, beta;
+  fx_stage_arrays(plan, U, stage, &X, &out, &beta);
+  return fx_stage(plan, X, U, out, dx, dt, dt_dev, beta, stage == 0, (cudaStream_t)stream, cfl_next, dt_next_dev);
+}
+
 static int fx_advance_impl(fx_hydro_plan *plan, double *U, const double *dx, double dt, const double *dt_dev,
                            cudaStream_t st, double cfl_next = 0.0, double *dt_next = nullptr) {
-  if (plan->P.nblocks == 0) return FX_OK;
+  if (plan->P.nown == 0) return FX_OK;
   double *U1 = plan->stage[0], *U2 = plan->stage[1];
   // The last stage may overwrite U0 in place: its halos come from U1 (RK2) / U2 (RK3), never from U0.
   int rc = fx_stage(plan, U, U, U1, dx, dt, dt_dev, 1.0, 1, st);  // U1 = U0 - S(U0)
@@ -131,7 +165,7 @@ extern "C" int fx_hydro_step(fx_hydro_plan *plan, double *U, const double *dx, d
   if (rc) return rc;
   if (!dt_inout_dev || ((!U || !dx) && plan->P.nblocks > 0)) return fx_fail(FX_ERR_INVALID_ARG, "step: null argument");
   if (!(cfl > 0.0) || !isfinite(cfl)) return fx_fail(FX_ERR_INVALID_ARG, "step: cfl must be positive and finite");
-  if (plan->P.nblocks == 0) return FX_OK;
+  if (plan->P.nown == 0) return FX_OK;
   // every stage reads dt from dt_inout_dev when it starts; the last CTA of the last stage to finish overwrites it
   return fx_advance_impl(plan, U, dx, 0.0, dt_inout_dev, (cudaStream_t)stream, cfl, dt_inout_dev);
 }

@@ -242,7 +242,7 @@ static int launch_nt(const FxParams &P, const double *X, const double *U0, doubl
   auto kern = fx_k_stage_tile<RECON, RIEMANN, WS, NT, MINB>;
   // (per device and context, and cheap: set on every launch rather than cached per process)
   FX_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
-  kern<<<(unsigned)P.nblocks, NT, g.smem, st>>>(P, X, U0, out, dx, dt, dt_dev, beta, first, g.ntile, g.faces_max, g.nint);
+  kern<<<(unsigned)P.nown, NT, g.smem, st>>>(P, X, U0, out, dx, dt, dt_dev, beta, first, g.ntile, g.faces_max, g.nint);
   FX_LAUNCH_CHECK("stage_tile");
   return FX_OK;
 }

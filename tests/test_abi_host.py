@@ -114,3 +114,36 @@ def test_options_and_state_errors_without_gpu():
     assert L.fx_hydro_compute_dt(h, None, None, 0.3, None, None) == fx.ERR_STATE
     assert L.fx_hydro_plan_set_workspace(h, C.c_void_p(8), 1 << 30) == fx.ERR_WORKSPACE  # misaligned
     assert L.fx_hydro_plan_set_workspace(h, C.c_void_p(256), 16) == fx.ERR_WORKSPACE     # too small
+
+
+def test_shard_partition_lists_agree_between_ranks():
+    """fx_shard_* (host index logic): contiguous runs that cover the order; what rank p sends to q is, item for item and in
+    the same order, what q expects from p (global block id, side); ghosts are exactly the foreign neighbours of the owned
+    blocks; a ghost row names no neighbour; on an irregular table too (one-sided links, outflow, walls)."""
+    import numpy as np
+    from paper_2208_11630_b200 import binding as fx
+    per, out = fx.TOPO_PERIODIC, fx.TOPO_OUTFLOW
+    neigh, coords = fx.fx_topology_cartesian((4, 3, 5), (per, out, per), (per, fx.TOPO_REFLECT, per), fx.ORDER_MORTON)
+    neigh = np.array(neigh, np.int32)
+    neigh[7, 1] = fx.BC_OUTFLOW  # a one-sided cut link
+    N = neigh.shape[0]
+    for world in (1, 2, 3, 7):
+        shards = [fx.Shard(neigh, world, r) for r in range(world)]
+        assert [s.owned_begin for s in shards] == [N * r // world for r in range(world)]
+        assert sum(s.n_owned for s in shards) == N
+        for q, s in enumerate(shards):
+            own = set(range(s.owned_begin, s.owned_begin + s.n_owned))
+            foreign = {int(g) for b in own for g in neigh[b] if g >= 0 and g not in own}
+            assert set(s.global_id[s.n_owned:].tolist()) == foreign and list(s.global_id[:s.n_owned]) == sorted(own)
+            assert (s.neigh_local[s.n_owned:] == fx.BC_OUTFLOW).all()
+            # local table = global table through the numbering
+            back = np.where(s.neigh_local[:s.n_owned] >= 0, s.global_id[np.maximum(s.neigh_local[:s.n_owned], 0)], s.neigh_local[:s.n_owned])
+            assert np.array_equal(back, neigh[s.owned_begin:s.owned_begin + s.n_owned])
+            ro = np.concatenate([[0], np.cumsum(s.recv_counts)])
+            for p, t in enumerate(shards):
+                so = np.concatenate([[0], np.cumsum(t.send_counts)])
+                recv = [(int(s.global_id[b]), int(sd)) for b, sd in s.recv_items[ro[p]:ro[p + 1]]]
+                send = [(int(t.global_id[b]), int(sd)) for b, sd in t.send_items[so[q]:so[q + 1]]]
+                assert recv == send and recv == sorted(set(recv))
+                assert all(b < t.n_owned for b, _ in t.send_items[so[q]:so[q + 1]])
+            assert all(b >= s.n_owned for b, _ in s.recv_items)

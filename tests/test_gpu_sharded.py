@@ -1,0 +1,115 @@
+"""Sharded runs on ONE GPU: the ranks of a 2- and a 3-way partition are emulated in one process (every rank's plan lives on
+the same device, the all_to_all is replaced by copies between the ranks' buffers), so that the pack / unpack kernels, the
+owned / ghost split of the plans (FX_OPT_OWNED_BLOCKS) and the stage-by-stage API are exercised: the union of the ranks'
+owned blocks after RK steps equals the single-plan result BIT FOR BIT, the time step too, and the ghost blocks are
+never written by a stage.  (The rank-to-rank transfer itself is torch.distributed; the host logic is covered with two
+gloo ranks in tests/test_multirank_host.py.)"""
+import numpy as np
+import pytest
+import torch
+
+from paper_2208_11630_b200 import inputs
+from tests.helpers import gpu_plan_for
+
+pytestmark = pytest.mark.gpu
+
+
+def run_sharded(cfg, neigh, coords, world, steps, recon, rk, guard_x, path, nvars=5):
+    from paper_2208_11630_b200 import binding as fx
+    from paper_2208_11630_b200.sharded import ShardedHydro
+    ranks = [ShardedHydro(cfg.block_dims, cfg.nguard, cfg.gamma, recon, cfg.riemann, rk, neigh, r, world, guard_x=guard_x, nvars=nvars)
+             for r in range(world)]
+    for sh in ranks:
+        sh.world = 1  # no process group here: transfer() is done by hand below
+        if path is not None:
+            assert sh.plan.path == path
+    Ui = inputs.block_interiors(cfg, coords)
+    if nvars > 5:
+        Ui = inputs.with_scalars(cfg, coords, Ui, nvars - 5)
+    Us, dxs = [], []
+    dx_all = inputs.dx_array(cfg)
+    for sh in ranks:
+        U = sh.alloc_state(fill=float("nan"))  # ghost blocks start as NaN: only exchanged slabs are ever read
+        gid = sh.shard.global_id[:sh.n_owned]
+        sh.interior(U)[...] = Ui[:, gid].cuda()
+        Us.append(U)
+        dxl = np.ascontiguousarray(dx_all[sh.shard.global_id])
+        dxs.append(torch.from_numpy(dxl).cuda())
+
+    def exchange(stage):
+        for sh, U in zip(ranks, Us):
+            X, _ = sh.plan.fx_hydro_stage_arrays(U, stage)
+            sh.pack(X)
+        torch.cuda.synchronize()
+        for q, sh in enumerate(ranks):  # what all_to_all_single does: rank q's piece of p's send buffer, in rank order
+            ro = 0
+            for p, src in enumerate(ranks):
+                n = sh.recv_splits[p]
+                so = sum(src.send_splits[:q])
+                assert n == src.send_splits[q]
+                sh.recv_buf[ro:ro + n] = src.send_buf[so:so + n]
+                ro += n
+        for sh, U in zip(ranks, Us):
+            X, _ = sh.plan.fx_hydro_stage_arrays(U, stage)
+            sh.unpack(X)
+
+    def global_min(dts):
+        m = torch.stack(dts).min()
+        for d in dts:
+            d.copy_(m)
+
+    dts = [sh.plan.fx_hydro_compute_dt(U, dx, cfg.cfl).clone() for sh, U, dx in zip(ranks, Us, dxs)]
+    global_min(dts)
+    history = [float(dts[0].item())]
+    for _ in range(steps):
+        for s in range(rk):
+            exchange(s)
+            for sh, U, dx, dt in zip(ranks, Us, dxs, dts):
+                if s == rk - 1:
+                    sh.plan.fx_hydro_advance_stage(U, dx, dt, s, cfl_next=cfg.cfl, dt_next=dt)
+                else:
+                    sh.plan.fx_hydro_advance_stage(U, dx, dt, s)
+        global_min(dts)
+        history.append(float(dts[0].item()))
+    out = torch.empty((nvars,) + tuple(Ui.shape[1:]), dtype=torch.float64)
+    for sh, U in zip(ranks, Us):
+        out[:, sh.shard.global_id[:sh.n_owned]] = sh.interior(U).cpu()
+    return out, history, ranks, Us
+
+
+@pytest.mark.parametrize("number,nb,block,recon,rk,guard_x,world,path", [
+    (5, (2, 2, 4), None, 0, 2, 8, 2, 1), (5, (4, 2, 2), None, 1, 3, 4, 3, 1), (5, (2, 2, 2), (8, 8, 8), 0, 2, 4, 2, 0),
+    (5, (2, 2, 2), (8, 8, 8), 1, 3, 4, 2, 2), (2, (4, 4, 1), None, 0, 2, 4, 3, 2)])
+def test_sharded_equals_single_plan_bitwise(number, nb, block, recon, rk, guard_x, world, path):
+    from paper_2208_11630_b200 import binding as fx
+    cfg = inputs.config(number, nb=nb)
+    if block:
+        cfg.block_dims = block
+    bcs = [fx.TOPO_PERIODIC if cfg.block_dims[d] > 1 else fx.TOPO_NONE for d in range(3)]
+    neigh, coords = fx.fx_topology_cartesian(cfg.nb, bcs, bcs, fx.ORDER_MORTON)
+    steps = 3
+    got, hist, ranks, Us = run_sharded(cfg, neigh, coords, world, steps, recon, rk, guard_x, path)
+    # single plan, same order, same layout
+    plan = fx.HydroPlan(cfg.block_dims, cfg.nguard, cfg.nblocks, cfg.gamma, recon, cfg.riemann, rk)
+    if guard_x != cfg.nguard:
+        plan.fx_hydro_plan_set_option(fx.OPT_GUARD_X, guard_x)
+    plan.fx_hydro_plan_set_topology(neigh)
+    plan.fx_hydro_plan_set_workspace()
+    assert plan.path == path
+    U = plan.alloc_state(fill=float("nan"))
+    plan.interior(U)[...] = inputs.block_interiors(cfg, coords).cuda()
+    dx = torch.from_numpy(inputs.dx_array(cfg)).cuda()
+    dt = plan.fx_hydro_compute_dt(U, dx, cfg.cfl).clone()
+    ref_hist = [float(dt.item())]
+    for _ in range(steps):
+        plan.fx_hydro_step(U, dx, cfg.cfl, dt)
+        ref_hist.append(float(dt.item()))
+    assert hist == ref_hist
+    assert torch.equal(got, plan.interior(U).cpu())
+    # every rank has ghosts, they were never written by a stage beyond the exchanged slabs (their cores are still NaN
+    # where no slab reaches: blocks of 16 with slabs of depth 2 or 3 from at most both sides of each dimension)
+    for sh, Ur in zip(ranks, Us):
+        assert sh.shard.n_ghost > 0
+        if cfg.block_dims[0] == 16:
+            core = sh.plan.interior(Ur)[:, sh.n_owned:, 4:12 if cfg.block_dims[2] > 1 else 0:1, 4:12, 4:12]
+            assert torch.isnan(core).all()
