@@ -46,6 +46,8 @@
 #define FXO_BC_OUTFLOW (-1)
 #define FXO_BC_NONE (-2)
 #define FXO_BC_REFLECT (-3) /* reflecting wall [B9]: mirror image of the interior, normal momentum negated */
+#define FXO_NEIGH_COARSER (-4) /* the block behind this face is one level coarser (dx twice as large) [B12] */
+#define FXO_NEIGH_FINER (-5)   /* 2^(ndim-1) blocks one level finer lie behind this face [B12] */
 #define FXO_OPT_RHO_FLOOR 0
 #define FXO_OPT_P_FLOOR 1
 #define FXO_OPT_WENO_EPS 2
@@ -74,6 +76,8 @@ typedef struct fxo_plan {
   double grav[3];
   int wavespeed; /* 0 Einfeldt, 1 Davis [A8] */
   const int32_t *neigh;
+  const int32_t *jump; /* refinement jumps [B12]: [nblocks][6][4], see fxo_plan_set_refinement */
+  double *Fb;          /* scratch: boundary-face fluxes of the blocks with a coarser neighbour [B14] */
   unsigned long long n_nonfinite, n_rho_floor, n_p_floor, n_weno_fb;
 } fxo_plan;
 
@@ -83,6 +87,9 @@ typedef struct fxo_layout {
   int64_t S_j, S_k, S_b, S_v;
   int64_t bytes_per_state;
 } fxo_layout;
+
+double fxo_minmod(double a, double b);
+static void fill_jump_faces(const fxo_plan *p, double *U);
 
 /* ------------------------------------------------------------------ plan */
 
@@ -136,7 +143,10 @@ int fxo_plan_create(fxo_plan **out, const int dims[3], int nguard, int nvars, in
   return FXO_OK;
 }
 
-void fxo_plan_destroy(fxo_plan *p) { free(p); }
+void fxo_plan_destroy(fxo_plan *p) {
+  if (p) free(p->Fb);
+  free(p);
+}
 
 int fxo_plan_layout(const fxo_plan *p, fxo_layout *L) {
   if (!p || !L) return FXO_ERR_INVALID_ARG;
@@ -178,11 +188,33 @@ int fxo_plan_set_topology(fxo_plan *p, const int32_t *neigh) {
       if (!p->active[d]) continue; /* entries of inactive dims are ignored [A26] */
       if (v >= 0) {
         if (v >= p->nblocks) return FXO_ERR_INVALID_ARG;
+      } else if (v == FXO_NEIGH_COARSER || v == FXO_NEIGH_FINER) {
+        if (!p->jump) return FXO_ERR_UNSUPPORTED; /* a jump needs the refinement table [B12] */
+        int nq = v == FXO_NEIGH_COARSER ? 1 : (1 << (p->active[0] + p->active[1] + p->active[2] - 1));
+        for (int q = 0; q < nq; ++q) {
+          int32_t id = p->jump[(b * 6 + f) * 4 + q];
+          if (id < 0 || id >= p->nblocks) return FXO_ERR_INVALID_ARG;
+        }
       } else if (v != FXO_BC_OUTFLOW && v != FXO_BC_REFLECT) {
-        return FXO_ERR_UNSUPPORTED; /* coarse/fine neighbours have no code [A18] */
+        return FXO_ERR_UNSUPPORTED;
       }
     }
   p->neigh = neigh;
+  return FXO_OK;
+}
+
+/* Refinement jumps [B12] ("fine-coarse boundary resolution related API functions of the Grid unit").
+ * Blocks of all levels have the same zone counts; a block one level finer has half the zone width (the caller's dx says
+ * so); neighbours differ by at most one level.  neigh[b][f] = FXO_NEIGH_COARSER: jump[b][f][0] is the coarser block and
+ * jump[b][f][1] says which part of its face this block abuts: bit 0 = upper half along the first transverse dimension,
+ * bit 1 = along the second (transverse dimensions in ascending order; 0 for an inactive one).  neigh[b][f] =
+ * FXO_NEIGH_FINER: jump[b][f][q], q = bit pattern as above, are the finer blocks.  Call before fxo_plan_set_topology.
+ * Needs even block extents and nguard <= n_d / 2 in every active dimension. */
+int fxo_plan_set_refinement(fxo_plan *p, const int32_t *jump) {
+  if (!p) return FXO_ERR_INVALID_ARG;
+  for (int d = 0; d < 3; ++d)
+    if (p->active[d] && (p->n[d] % 2 != 0 || 2 * p->g > p->n[d])) return FXO_ERR_INVALID_ARG;
+  p->jump = jump;
   return FXO_OK;
 }
 
@@ -358,7 +390,127 @@ int fxo_fill_guardcells(fxo_plan *p, double *U) {
             U[v * p->S_v + t] = (v >= 1 && v <= 3 && ((flip >> (v - 1)) & 1u)) ? -x : x;
           }
         }
+  if (p->jump) fill_jump_faces(p, U); /* second pass: restriction / prolongation behind refinement jumps [B12, B13] */
   return FXO_OK;
+}
+
+/* ------------------------------------------- O9 fine-coarse boundaries [B12, B13] */
+
+/* Variable v of the zone at INTERIOR coordinates c (0-based) of block cb, where at most one coordinate may lie outside
+ * [0, n): then the zone is resolved by ONE hop through that face -- the same-level neighbour's interior zone, the clamp
+ * (outflow), the mirror zone (wall; normal momentum negated), or, behind a face with finer neighbours, the RESTRICTION
+ * of their interior zones: the plain mean of the 2^ndim children, summed in the order i fastest, then j, then k [B13].
+ * Behind a face with a coarser neighbour nothing is defined here: returns 0 (and 1 otherwise).  A pure function of
+ * interior data, so fills can run in any order. */
+static int amr_zone(const fxo_plan *p, const double *X, int64_t cb, const int cin[3], int v, double *val) {
+  int c[3] = {cin[0], cin[1], cin[2]};
+  double sign = 1.0;
+  for (int d = 0; d < 3; ++d) {
+    if (c[d] >= 0 && c[d] < p->n[d]) continue;
+    int side = c[d] >= p->n[d];
+    int f = 2 * d + side;
+    int32_t nb = p->neigh[cb * 6 + f];
+    if (nb >= 0) {
+      cb = nb;
+      c[d] += side ? -p->n[d] : p->n[d];
+    } else if (nb == FXO_BC_REFLECT) {
+      c[d] = side ? 2 * p->n[d] - 1 - c[d] : -1 - c[d];
+      if (v == 1 + d) sign = -1.0;
+    } else if (nb == FXO_NEIGH_FINER) {
+      int d1 = d == 0 ? 1 : 0, d2 = d == 2 ? 1 : 2; /* transverse dimensions, ascending */
+      int q = 0, fc[3], cnt[3];
+      int tr[2] = {d1, d2};
+      for (int t = 0; t < 2; ++t) {
+        int e = tr[t];
+        if (!p->active[e]) { fc[e] = 0; cnt[e] = 1; continue; }
+        int half = c[e] >= p->n[e] / 2;
+        q |= half << t;
+        fc[e] = 2 * (c[e] - half * (p->n[e] / 2));
+        cnt[e] = 2;
+      }
+      int m = side ? c[d] - p->n[d] : -1 - c[d]; /* distance behind the face, 0 = adjacent */
+      fc[d] = side ? 2 * m : p->n[d] - 2 - 2 * m;
+      cnt[d] = 2;
+      int64_t fb = p->jump[(cb * 6 + f) * 4 + q];
+      double sum = 0.0;
+      for (int kk = 0; kk < cnt[2]; ++kk)
+        for (int jj = 0; jj < cnt[1]; ++jj)
+          for (int ii = 0; ii < cnt[0]; ++ii)
+            sum += X[v * p->S_v + fb * p->S_b + (int64_t)(fc[2] + kk + p->gd[2]) * p->S_k +
+                     (int64_t)(fc[1] + jj + p->gd[1]) * p->S_j + (fc[0] + ii + p->gd[0])];
+      *val = sum * (1.0 / (double)(cnt[0] * cnt[1] * cnt[2]));
+      return 1;
+    } else if (nb == FXO_NEIGH_COARSER) {
+      return 0;
+    } else {
+      c[d] = side ? p->n[d] - 1 : 0; /* outflow */
+    }
+    break; /* one hop */
+  }
+  *val = sign * X[v * p->S_v + cb * p->S_b + (int64_t)(c[2] + p->gd[2]) * p->S_k + (int64_t)(c[1] + p->gd[1]) * p->S_j +
+                  (c[0] + p->gd[0])];
+  return 1;
+}
+
+/* Face guard zones behind refinement jumps [B12, B13], after the same-level fill: for every block face with finer
+ * neighbours the guard zones are the restriction of the fine interiors; for every face with a coarser neighbour they are
+ * PROLONGED from the parent coarse zone C: q = q_C + sum over active d of sigma_d (1/4) minmod(q_C - q_{C-e_d},
+ * q_{C+e_d} - q_C), sigma_d = +-1 the child's side of C along d, the neighbours of C resolved by amr_zone (a neighbour that
+ * lies behind a coarser jump is not defined: that slope is 0).  Conserved variables, all of them; the children of a zone
+ * average to the zone.  Only zones outside the block in exactly ONE dimension are written (the stage reads no others
+ * [A11]); edge and corner zones next to a jump keep the clamp of the first pass. */
+static void fill_jump_faces(const fxo_plan *p, double *U) {
+#pragma omp parallel for schedule(static)
+  for (int64_t b = 0; b < p->nblocks; ++b)
+    for (int f = 0; f < 6; ++f) {
+      int d = f / 2, side = f & 1;
+      if (!p->active[d]) continue;
+      int32_t code = p->neigh[b * 6 + f];
+      if (code != FXO_NEIGH_COARSER && code != FXO_NEIGH_FINER) continue;
+      int d1 = d == 0 ? 1 : 0, d2 = d == 2 ? 1 : 2;
+      for (int m = 0; m < p->gd[d]; ++m)
+        for (int t2 = 0; t2 < p->n[d2]; ++t2)
+          for (int t1 = 0; t1 < p->n[d1]; ++t1) {
+            int c[3];
+            c[d] = side ? p->n[d] + m : -1 - m;
+            c[d1] = t1;
+            c[d2] = t2;
+            int64_t t = b * p->S_b + (int64_t)(c[2] + p->gd[2]) * p->S_k + (int64_t)(c[1] + p->gd[1]) * p->S_j + (c[0] + p->gd[0]);
+            for (int v = 0; v < p->nvars; ++v) {
+              double val = 0.0;
+              if (code == FXO_NEIGH_FINER) {
+                amr_zone(p, U, b, c, v, &val);
+              } else {
+                int64_t cb = p->jump[(b * 6 + f) * 4 + 0];
+                int qd = p->jump[(b * 6 + f) * 4 + 1];
+                int C[3] = {0, 0, 0};
+                double sg[3] = {0.0, 0.0, 0.0};
+                C[d] = side ? m / 2 : p->n[d] - 1 - m / 2;
+                sg[d] = ((m % 2 == 0) == (side == 0)) ? 1.0 : -1.0; /* the child next to the face is the one on the face's side */
+                int tr[2] = {d1, d2}, tc[2] = {t1, t2};
+                for (int t_ = 0; t_ < 2; ++t_) {
+                  int e = tr[t_];
+                  if (!p->active[e]) continue;
+                  C[e] = ((qd >> t_) & 1) * (p->n[e] / 2) + tc[t_] / 2;
+                  sg[e] = (tc[t_] % 2) ? 1.0 : -1.0;
+                }
+                double qC;
+                amr_zone(p, U, cb, C, v, &qC);
+                val = qC;
+                for (int e = 0; e < 3; ++e) {
+                  if (!p->active[e]) continue;
+                  int Cm[3] = {C[0], C[1], C[2]}, Cp[3] = {C[0], C[1], C[2]};
+                  Cm[e] -= 1;
+                  Cp[e] += 1;
+                  double qm, qp;
+                  if (amr_zone(p, U, cb, Cm, v, &qm) && amr_zone(p, U, cb, Cp, v, &qp))
+                    val += (sg[e] * 0.25) * fxo_minmod(qC - qm, qp - qC);
+                }
+              }
+              U[v * p->S_v + t] = val;
+            }
+          }
+    }
 }
 
 /* ---------------------------------------------------- O2 cons -> prim */
@@ -677,6 +829,35 @@ static void block_stage(fxo_plan *p, const double *X, const double *U0, double *
           face_flux(p, W, p->S_b, cL, d, Fline + nv * f, &hit);
         }
         count_hits(p, hit & (FXO_STATUS_NONFINITE | FXO_STATUS_WENO_FALLBACK), 1);
+        /* flux correction [B14]: at a face with finer neighbours the flux of a coarse face is the mean of the fluxes
+         * of the 2^(ndim-1) fine faces that cover it (computed by the fine blocks from their prolonged guard zones),
+         * so that what leaves the fine blocks enters the coarse one */
+        for (int side = 0; side < 2; ++side)
+          if (p->jump && p->neigh[b * 6 + 2 * d + side] == FXO_NEIGH_FINER) {
+            int lo1 = d == 0 ? 1 : 0, lo2 = d == 2 ? 1 : 2; /* transverse dimensions, ascending */
+            int tc[3];
+            tc[d1] = a1 - p->gd[d1];
+            tc[d2] = a2 - p->gd[d2];
+            int tr[2] = {lo1, lo2}, q = 0, ft[2] = {0, 0}, cnt[2] = {1, 1};
+            for (int t = 0; t < 2; ++t) {
+              int e = tr[t];
+              if (!p->active[e]) continue;
+              int half = tc[e] >= p->n[e] / 2;
+              q |= half << t;
+              ft[t] = 2 * (tc[e] - half * (p->n[e] / 2));
+              cnt[t] = 2;
+            }
+            int64_t fb = p->jump[(b * 6 + 2 * d + side) * 4 + q];
+            int ff = 2 * d + (1 - side); /* the fine block's face that touches ours */
+            int64_t A = (int64_t)p->n[lo1] * p->n[lo2];
+            for (int v = 0; v < nv; ++v) {
+              double sum = 0.0;
+              for (int j2 = 0; j2 < cnt[1]; ++j2)
+                for (int j1 = 0; j1 < cnt[0]; ++j1)
+                  sum += p->Fb[((fb * 6 + ff) * nv + v) * A + (int64_t)(ft[1] + j2) * p->n[lo1] + (ft[0] + j1)];
+              Fline[nv * (side ? p->n[d] : 0) + v] = sum * (1.0 / (double)(cnt[0] * cnt[1]));
+            }
+          }
         for (int f = 0; f < p->n[d]; ++f) {
           int64_t c = base + (int64_t)(p->gd[d] + f) * stride[d];
           for (int v = 0; v < nv; ++v) S[v * p->S_b + c] += r * (Fline[nv * (f + 1) + v] - Fline[nv * f + v]);
@@ -711,6 +892,42 @@ static int run_stage(fxo_plan *p, double *X, const double *U0, double *out, cons
   int rc = fxo_fill_guardcells(p, X); /* O1 on the stage input before every S(.) [A15] */
   if (rc) return rc;
   int fail = 0;
+  if (p->jump) { /* [B14] first the boundary-face fluxes of every block face that has a coarser neighbour */
+    int nmx = p->n[0] > p->n[1] ? p->n[0] : p->n[1];
+    if (p->n[2] > nmx) nmx = p->n[2];
+    if (!p->Fb) p->Fb = (double *)malloc(sizeof(double) * (size_t)p->nblocks * 6 * (size_t)p->nvars * (size_t)nmx * (size_t)nmx);
+    if (!p->Fb) return FXO_ERR_NOMEM;
+#pragma omp parallel
+    {
+      double *W = (double *)malloc(sizeof(double) * (size_t)p->nvars * (size_t)p->S_b);
+#pragma omp for schedule(dynamic, 4)
+      for (int64_t b = 0; b < p->nblocks; ++b) {
+        int any = 0;
+        for (int f = 0; f < 6; ++f) any |= p->active[f / 2] && p->neigh[b * 6 + f] == FXO_NEIGH_COARSER;
+        if (!any || !W) continue;
+        block_prims(p, X, b, W);
+        const int64_t stride[3] = {1, p->S_j, p->S_k};
+        for (int f = 0; f < 6; ++f) {
+          int d = f / 2, side = f & 1;
+          if (!p->active[d] || p->neigh[b * 6 + f] != FXO_NEIGH_COARSER) continue;
+          int lo1 = d == 0 ? 1 : 0, lo2 = d == 2 ? 1 : 2;
+          int64_t A = (int64_t)p->n[lo1] * p->n[lo2];
+          for (int t2 = 0; t2 < p->n[lo2]; ++t2)
+            for (int t1 = 0; t1 < p->n[lo1]; ++t1) {
+              int c[3];
+              c[d] = p->gd[d] + (side ? p->n[d] : 0) - 1; /* left cell of the face */
+              c[lo1] = t1 + p->gd[lo1];
+              c[lo2] = t2 + p->gd[lo2];
+              double Ff[FXO_MAXV];
+              unsigned hit = 0;
+              face_flux(p, W, p->S_b, c[2] * stride[2] + c[1] * stride[1] + c[0], d, Ff, &hit);
+              for (int v = 0; v < p->nvars; ++v) p->Fb[((b * 6 + f) * p->nvars + v) * A + (int64_t)t2 * p->n[lo1] + t1] = Ff[v];
+            }
+        }
+      }
+      free(W);
+    }
+  }
 #pragma omp parallel
   {
     double *W = (double *)malloc(sizeof(double) * (size_t)p->nvars * (size_t)p->S_b);

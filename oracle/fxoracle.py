@@ -19,6 +19,7 @@ _LIB = os.path.join(_HERE, "libfxoracle.so")
 RECON_PLM_MINMOD, RECON_WENO5 = 0, 1
 RIEMANN_HLLE, RIEMANN_HLLC = 0, 1
 BC_OUTFLOW, BC_NONE, BC_REFLECT = -1, -2, -3
+NEIGH_COARSER, NEIGH_FINER = -4, -5
 OPT_GRAVITY_X, OPT_GRAVITY_Y, OPT_GRAVITY_Z = 6, 7, 8
 TOPO_PERIODIC, TOPO_OUTFLOW, TOPO_NONE, TOPO_REFLECT = 0, 1, 2, 3
 ORDER_LEX, ORDER_MORTON = 0, 1
@@ -55,6 +56,7 @@ def lib():
         L.fxo_plan_layout.argtypes = [C.c_void_p, C.POINTER(_Layout)]
         L.fxo_plan_set_option.argtypes = [C.c_void_p, C.c_int, C.c_double]
         L.fxo_plan_set_topology.argtypes = [C.c_void_p, ip]
+        L.fxo_plan_set_refinement.argtypes = [C.c_void_p, ip]
         L.fxo_status.argtypes = [C.c_void_p, C.POINTER(C.c_uint32), C.POINTER(C.c_ulonglong)]
         L.fxo_status_reset.argtypes = [C.c_void_p]
         L.fxo_status_reset.restype = None
@@ -150,6 +152,14 @@ class OraclePlan:
         rc = lib().fxo_plan_set_option(self._h, key, float(value))
         if rc != 0:
             raise ValueError(f"fxo_plan_set_option failed with code {rc}")
+
+    def set_refinement(self, jump):
+        """Refinement-jump table int32 [nblocks, 6, 4] [B12]; before set_topology."""
+        jump = np.ascontiguousarray(jump, np.int32).reshape(self.nblocks, 6, 4)
+        rc = lib().fxo_plan_set_refinement(self._h, jump.ctypes.data_as(C.POINTER(C.c_int32)))
+        if rc != 0:
+            raise ValueError(f"fxo_plan_set_refinement failed with code {rc}")
+        self._jump = jump  # keep alive: the plan borrows it
 
     def set_topology(self, neigh):
         neigh = np.ascontiguousarray(neigh, np.int32).reshape(self.nblocks, 6)

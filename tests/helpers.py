@@ -192,3 +192,88 @@ def cliff_state(cfg, coords, axis, high=1e6):
         shape[ax] = 6
         arr[tuple(s)] = np.array(vals).reshape(shape)
     return np.stack([rho, rho * vel[0], rho * vel[1], rho * vel[2], p / (g - 1) + 0.5 * rho * (vel ** 2).sum(0)])
+
+
+def two_level_grid(nbc, refined, block_dims, periodic=True):
+    """A static 2-level block grid [B12]: the coarse tiling nbc = (cx, cy, cz) of a unit-width-per-coarse-zone domain, the
+    coarse cells in `refined` (a set of (X, Y, Z)) replaced by their 2^ndim children.  Written in numpy from the
+    definition of the tables (include/fx_hydro.h, fxo_plan_set_refinement); used for both sides.
+    Returns dict(neigh int32 [n,6], jump int32 [n,6,4], level int [n], origin float [n,3] (lower corner in coarse zones),
+    dxrel float [n] (zone width in coarse zones: 1 or 1/2), cell [n,3], child [n,3])."""
+    dims = [d for d in range(3) if block_dims[d] > 1]
+    refined = set(tuple(r) for r in refined)
+    blocks = []  # (level, cell, child)
+    for Z in range(nbc[2]):
+        for Y in range(nbc[1]):
+            for X in range(nbc[0]):
+                if (X, Y, Z) in refined:
+                    for cz in range(2 if 2 in dims else 1):
+                        for cy in range(2 if 1 in dims else 1):
+                            for cx in range(2 if 0 in dims else 1):
+                                blocks.append((1, (X, Y, Z), (cx, cy, cz)))
+                else:
+                    blocks.append((0, (X, Y, Z), (0, 0, 0)))
+    ident = {(lv, cell, ch): i for i, (lv, cell, ch) in enumerate(blocks)}
+    n = len(blocks)
+    neigh = np.full((n, 6), -2, np.int32)
+    jump = np.full((n, 6, 4), -1, np.int32)
+    for b, (lv, cell, ch) in enumerate(blocks):
+        for d in dims:
+            tr = [e for e in range(3) if e != d]
+            for side in (0, 1):
+                f = 2 * d + side
+                if lv == 1 and ch[d] == 1 - side:  # the sibling inside the same parent
+                    sib = list(ch)
+                    sib[d] = side
+                    neigh[b, f] = ident[(1, cell, tuple(sib))]
+                    continue
+                nc = list(cell)
+                nc[d] += 1 if side else -1
+                if nc[d] < 0 or nc[d] >= nbc[d]:
+                    if not periodic:
+                        neigh[b, f] = -1  # outflow
+                        continue
+                    nc[d] %= nbc[d]
+                nc = tuple(nc)
+                if lv == 0:
+                    if nc not in refined:
+                        neigh[b, f] = ident[(0, nc, (0, 0, 0))]
+                    else:
+                        neigh[b, f] = -5
+                        for q in range(4):
+                            kid = [0, 0, 0]
+                            kid[d] = 0 if side else 1
+                            ok = True
+                            for t, e in enumerate(tr):
+                                bit = (q >> t) & 1
+                                if e in dims:
+                                    kid[e] = bit
+                                elif bit:
+                                    ok = False
+                            if ok:
+                                jump[b, f, q] = ident[(1, nc, tuple(kid))]
+                else:
+                    if nc in refined:
+                        kid = list(ch)
+                        kid[d] = 0 if side else 1
+                        neigh[b, f] = ident[(1, nc, tuple(kid))]
+                    else:
+                        neigh[b, f] = -4
+                        jump[b, f, 0] = ident[(0, nc, (0, 0, 0))]
+                        jump[b, f, 1] = sum(ch[e] << t for t, e in enumerate(tr) if e in dims)
+    level = np.array([lv for lv, _, _ in blocks])
+    origin = np.array([[cell[d] * block_dims[d] + (ch[d] * block_dims[d] / 2 if lv else 0) for d in range(3)] for lv, cell, ch in blocks], float)
+    return dict(neigh=neigh, jump=jump, level=level, origin=origin, dxrel=np.where(level == 1, 0.5, 1.0),
+                cell=np.array([c for _, c, _ in blocks]), child=np.array([c for _, _, c in blocks]))
+
+
+def amr_zone_centres(grid, block_dims):
+    """Zone-centre coordinates (in coarse zones) of every interior zone: [n, 3, nz, ny, nx]."""
+    n = len(grid["level"])
+    out = np.zeros((n, 3, block_dims[2], block_dims[1], block_dims[0]))
+    for b in range(n):
+        h = grid["dxrel"][b]
+        ax = [grid["origin"][b, d] + (np.arange(block_dims[d]) + 0.5) * (h if block_dims[d] > 1 else 1.0) for d in range(3)]
+        K, J, I = np.meshgrid(ax[2], ax[1], ax[0], indexing="ij")
+        out[b, 0], out[b, 1], out[b, 2] = I, J, K
+    return out
