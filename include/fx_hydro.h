@@ -42,7 +42,8 @@ extern "C" {
 
 enum { FX_RECON_PLM_MINMOD = 0, FX_RECON_WENO5 = 1 };
 enum { FX_RIEMANN_HLLE = 0, FX_RIEMANN_HLLC = 1 };
-enum { FX_BC_OUTFLOW = -1, FX_BC_NONE = -2, FX_BC_REFLECT = -3 };    /* neighbour-table codes */
+enum { FX_BC_OUTFLOW = -1, FX_BC_NONE = -2, FX_BC_REFLECT = -3,        /* neighbour-table codes */
+       FX_NEIGH_COARSER = -4, FX_NEIGH_FINER = -5 };                    /* refinement jumps, see fx_hydro_plan_set_refinement */
 enum { FX_TOPO_PERIODIC = 0, FX_TOPO_OUTFLOW = 1, FX_TOPO_NONE = 2, FX_TOPO_REFLECT = 3 }; /* fx_topology_cartesian bc codes */
 enum { FX_ORDER_LEX = 0, FX_ORDER_MORTON = 1 };
 enum {
@@ -130,9 +131,28 @@ int fx_hydro_plan_set_workspace(fx_hydro_plan *plan, void *workspace_dev, size_t
  * zero-gradient physical boundary, FX_BC_REFLECT a reflecting wall (guard zone -1-m images interior zone m
  * with the momentum normal to the wall negated; reading B9); entries of inactive dimensions are ignored.  The table stays
  * caller-owned and must outlive the plan's use of it.  The call copies it to the host once to validate
- * (synchronises).  Any other negative entry in an active dimension is a coarse/fine relation:
- * FX_ERR_UNSUPPORTED [A18]. */
+ * (synchronises).  FX_NEIGH_COARSER / FX_NEIGH_FINER mark a refinement jump and need fx_hydro_plan_set_refinement first
+ * (FX_ERR_UNSUPPORTED without it, with passive scalars, or in a sharded plan); any other negative entry in an active
+ * dimension: FX_ERR_UNSUPPORTED. */
 int fx_hydro_plan_set_topology(fx_hydro_plan *plan, const int32_t *neigh_dev);
+
+/* Fine-coarse boundaries ("fine-coarse boundary resolution related API functions of the Grid unit"; DESIGN.md
+ * readings B12-B14).  Blocks of all levels have the same zone counts; a block one level finer has half the zone width (the
+ * caller's dx_dev says so); face neighbours differ by at most one level.  jump_dev is int32 [nblocks][6][4], caller-owned:
+ *   neigh[b][f] == FX_NEIGH_COARSER: jump[b][f][0] = the coarser block, jump[b][f][1] = which part of its face block b abuts:
+ *     bit 0 = upper half along the first transverse dimension, bit 1 = along the second (transverse dimensions in
+ *     ascending order; 0 for an inactive one);
+ *   neigh[b][f] == FX_NEIGH_FINER: jump[b][f][q], q = that bit pattern, are the 2^(ndim-1) finer blocks behind the face.
+ * What the library then does, per stage and in fx_fill_guardcells: the face guard zones behind a face with finer
+ * neighbours are the RESTRICTION of their interiors (plain mean of the 2^ndim children); behind a face with a coarser
+ * neighbour they are PROLONGED from the parent coarse zone C, q = q_C + sum_d sigma_d (1/4) minmod(q_C - q_{C-e_d},
+ * q_{C+e_d} - q_C) on the conserved variables (children average to the parent; a neighbour of C that lies behind a coarser
+ * jump gives slope 0); and the flux of a coarse face at a jump is replaced by the mean of the fine face fluxes that cover
+ * it (FLUX CORRECTION: what leaves the fine blocks enters the coarse one).  Edge and corner guard zones next to a jump hold
+ * a clamp (the stage reads none [A11]); fx_guardcell_index_map reports the clamp for zones behind a jump.  Plans with
+ * jumps run on the generic path.  Call before the workspace (which grows by the jump faces' flux buffer) and the
+ * topology.  Needs even block extents and nguard <= n_d / 2 in active dimensions (FX_ERR_INVALID_ARG). */
+int fx_hydro_plan_set_refinement(fx_hydro_plan *plan, const int32_t *jump_dev);
 
 /* Host helper: neighbour table and block coordinates of a regular nb[0] x nb[1] x nb[2] tiling.
  * bc_lo/bc_hi per dimension: FX_TOPO_*; order FX_ORDER_LEX (x fastest) or FX_ORDER_MORTON.

@@ -18,6 +18,7 @@ OK, ERR_INVALID_ARG, ERR_STATE, ERR_UNSUPPORTED, ERR_WORKSPACE, ERR_CUDA = 0, -1
 RECON_PLM_MINMOD, RECON_WENO5 = 0, 1
 RIEMANN_HLLE, RIEMANN_HLLC = 0, 1
 BC_OUTFLOW, BC_NONE, BC_REFLECT = -1, -2, -3
+NEIGH_COARSER, NEIGH_FINER = -4, -5
 TOPO_PERIODIC, TOPO_OUTFLOW, TOPO_NONE, TOPO_REFLECT = 0, 1, 2, 3
 ORDER_LEX, ORDER_MORTON = 0, 1
 OPT_RHO_FLOOR, OPT_P_FLOOR, OPT_WENO_EPS, OPT_WAVESPEED, OPT_PATH, OPT_ZCHAIN = 0, 1, 2, 3, 4, 5
@@ -27,7 +28,7 @@ STATUS_NONFINITE, STATUS_RHO_FLOOR, STATUS_P_FLOOR, STATUS_WENO_FALLBACK = 1, 2,
 EXPORTS = [
     "fx_last_error", "fx_hydro_plan_create", "fx_hydro_plan_destroy", "fx_hydro_plan_layout",
     "fx_hydro_plan_set_option", "fx_hydro_plan_workspace_bytes", "fx_hydro_plan_set_workspace",
-    "fx_hydro_plan_set_topology", "fx_topology_cartesian", "fx_fill_guardcells", "fx_guardcell_index_map",
+    "fx_hydro_plan_set_topology", "fx_hydro_plan_set_refinement", "fx_topology_cartesian", "fx_fill_guardcells", "fx_guardcell_index_map",
     "fx_hydro_compute_dt", "fx_hydro_advance", "fx_hydro_advance_host", "fx_hydro_advance_host_interior", "fx_hydro_advance_devdt", "fx_hydro_step",
     "fx_hydro_status", "fx_hydro_status_reset", "fx_debug_compute_fluxes", "fx_hydro_plan_path",
     "fx_hydro_plan_set_timing", "fx_hydro_plan_get_timing",
@@ -69,6 +70,7 @@ def lib():
         L.fx_hydro_plan_workspace_bytes.restype = C.c_size_t
         L.fx_hydro_plan_set_workspace.argtypes = [vp, vp, C.c_size_t]
         L.fx_hydro_plan_set_topology.argtypes = [vp, vp]
+        L.fx_hydro_plan_set_refinement.argtypes = [vp, vp]
         L.fx_topology_cartesian.argtypes = [i3, i3, i3, C.c_int, vp, vp]
         L.fx_fill_guardcells.argtypes = [vp, vp, vp]
         L.fx_guardcell_index_map.argtypes = [vp, C.c_int64, C.c_int64, vp, vp]
@@ -234,6 +236,12 @@ class HydroPlan:
         _check(lib().fx_hydro_plan_set_workspace(self._h, C.c_void_p(ws.data_ptr()), ws.numel()))
         self._ws = ws
         self._dt = torch.empty(1, dtype=torch.float64, device=self.device)
+
+    def fx_hydro_plan_set_refinement(self, jump):
+        """Refinement-jump table int32 [nblocks, 6, 4] (numpy or tensor) [B12]; before workspace and topology."""
+        t = torch.as_tensor(np.ascontiguousarray(jump, np.int32) if not isinstance(jump, torch.Tensor) else jump).to(self.device).contiguous()
+        _check(lib().fx_hydro_plan_set_refinement(self._h, _dev(t, torch.int32)))
+        self._jump = t  # caller-owned device memory: keep it alive
 
     def fx_hydro_plan_set_topology(self, neigh):
         if not isinstance(neigh, torch.Tensor):

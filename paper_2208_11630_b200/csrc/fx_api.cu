@@ -116,6 +116,7 @@ extern "C" int fx_hydro_plan_create(fx_hydro_plan **out, const int block_dims[3]
 
 extern "C" int fx_hydro_plan_destroy(fx_hydro_plan *plan) {
   if (plan) delete[] plan->seg_host;
+  if (plan) delete[] plan->jump_host;
   if (plan && plan->ev) {
     for (int i = 0; i < 2 * FX_MAX_REC; ++i) cudaEventDestroy(plan->ev[i]);
     delete[] plan->ev;
@@ -198,6 +199,7 @@ extern "C" int fx_hydro_plan_set_option(fx_hydro_plan *plan, int key, double val
 extern "C" int fx_hydro_plan_path(const fx_hydro_plan *plan) {
   if (!plan) return fx_fail(FX_ERR_INVALID_ARG, "plan_path: null plan");
   if (plan->nvars > 5) return 0;  // passive scalars [B11] are carried by the generic path only
+  if (plan->P.has_jumps) return 0;  // refinement jumps [B12-B14]: the generic path reads the interpolated guard zones
   if ((plan->path_option == 0 || plan->path_option == 3) && fx_stage_tma_supported(plan->P))
     return (plan->path_option == 3 && fx_stage_pair_supported(plan->P)) ? 3 : 1;
   // 3-D blocks with PLM: the generic zone kernel, which gathers its halo cells itself, is ahead of the tile kernel
@@ -217,13 +219,18 @@ static size_t fx_seg_bytes(const fx_hydro_plan *plan) {  // room for one segment
   return (((size_t)plan->P.nblocks * FX_SEG_STRIDE * sizeof(int)) + 255) & ~(size_t)255;
 }
 
+static size_t fx_fjump_bytes(const fx_hydro_plan *plan) {  // boundary fluxes at refinement jumps [B14]
+  if (!plan->P.jump) return 0;
+  return (((size_t)plan->P.nblocks * 6 * 5 * (size_t)plan->P.fj_area * sizeof(double)) + 255) & ~(size_t)255;
+}
+
 // The stage copies start `fx_stage_pad` bytes into a 256-byte pad block, so that their interior rows start on a
 // 128-byte boundary like the caller's array should (include/fx_hydro.h, "Layout and DRAM lines").
 static size_t fx_stage_pad(const fx_hydro_plan *plan) { return (128 - ((size_t)plan->P.gd[0] * 8) % 128) % 128; }
 
 extern "C" size_t fx_hydro_plan_workspace_bytes(const fx_hydro_plan *plan) {
   if (!plan) return 0;
-  return (size_t)FX_SCR_WORDS * 8 + 256 + (size_t)(plan->rk - 1) * fx_state_bytes_aligned(plan) + fx_seg_bytes(plan);
+  return (size_t)FX_SCR_WORDS * 8 + 256 + (size_t)(plan->rk - 1) * fx_state_bytes_aligned(plan) + fx_seg_bytes(plan) + fx_fjump_bytes(plan);
 }
 
 // Upload the segment table into its place behind the stage copies (needs both the workspace and the topology).
@@ -254,13 +261,44 @@ extern "C" int fx_hydro_plan_set_workspace(fx_hydro_plan *plan, void *ws, size_t
   char *base = (char *)ws + FX_SCR_WORDS * 8 + fx_stage_pad(plan);
   plan->stage[0] = (double *)base;
   plan->stage[1] = plan->rk == 3 ? (double *)(base + fx_state_bytes_aligned(plan)) : nullptr;
+  plan->P.fjump = plan->P.jump ? (double *)((char *)ws + FX_SCR_WORDS * 8 + 256 + (size_t)(plan->rk - 1) * fx_state_bytes_aligned(plan) +
+                                            fx_seg_bytes(plan))
+                               : nullptr;
   return fx_seg_upload(plan);
 }
 
 // ------------------------------------------------------------------ topology
+// Refinement-jump table [B12]: see include/fx_hydro.h.  A host copy is kept for the validation of the neighbour table.
+extern "C" int fx_hydro_plan_set_refinement(fx_hydro_plan *plan, const int32_t *jump_dev) {
+  if (!plan) return fx_fail(FX_ERR_INVALID_ARG, "set_refinement: null plan");
+  if (plan->topology_set || plan->workspace) return fx_fail(FX_ERR_STATE, "set_refinement: call before the workspace and the topology");
+  for (int d = 0; d < 3; ++d)
+    if (plan->P.active[d] && (plan->P.n[d] % 2 != 0 || 2 * plan->nguard > plan->P.n[d]))
+      return fx_fail(FX_ERR_INVALID_ARG, "set_refinement: needs even block extents and nguard <= n_d / 2 in every active dimension");
+  delete[] plan->jump_host;
+  plan->jump_host = nullptr;
+  plan->P.jump = nullptr;
+  if (!jump_dev) return FX_OK;
+  const size_t n = (size_t)plan->P.nblocks * 24;
+  plan->jump_host = new (std::nothrow) int32_t[n ? n : 1];
+  if (!plan->jump_host) return fx_fail(FX_ERR_INVALID_ARG, "set_refinement: out of host memory");
+  FX_CUDA(cudaMemcpy(plan->jump_host, jump_dev, n * sizeof(int32_t), cudaMemcpyDeviceToHost));
+  plan->P.jump = jump_dev;
+  int a = 1;
+  for (int d = 0; d < 3; ++d) {
+    int f = 1;
+    for (int e = 0; e < 3; ++e)
+      if (e != d) f *= plan->P.n[e];
+    if (f > a) a = f;
+  }
+  plan->P.fj_area = a;
+  return FX_OK;
+}
+
 extern "C" int fx_hydro_plan_set_topology(fx_hydro_plan *plan, const int32_t *neigh_dev) {
   if (!plan) return fx_fail(FX_ERR_INVALID_ARG, "set_topology: null plan");
   const long long nb = plan->P.nblocks;
+  int jumps = 0;
   if (nb > 0) {
     if (!neigh_dev) return fx_fail(FX_ERR_INVALID_ARG, "set_topology: null table");
     std::vector<int32_t> h((size_t)nb * 6);
@@ -271,12 +309,23 @@ extern "C" int fx_hydro_plan_set_topology(fx_hydro_plan *plan, const int32_t *ne
         const int32_t v = h[b * 6 + f];
         if (v >= 0) {
           if (v >= nb) return fx_fail(FX_ERR_INVALID_ARG, "set_topology: block %lld face %d -> id %d out of range", b, f, v);
+        } else if (v == FX_NEIGH_COARSER || v == FX_NEIGH_FINER) {
+          if (!plan->jump_host) return fx_fail(FX_ERR_UNSUPPORTED, "set_topology: block %lld face %d is a refinement jump: call fx_hydro_plan_set_refinement first", b, f);
+          if (plan->nvars > 5) return fx_fail(FX_ERR_UNSUPPORTED, "set_topology: refinement jumps with passive scalars are not supported");
+          if (plan->P.nown != nb) return fx_fail(FX_ERR_UNSUPPORTED, "set_topology: refinement jumps in a sharded plan are not supported");
+          const int nq = v == FX_NEIGH_COARSER ? 1 : (1 << (plan->P.active[0] + plan->P.active[1] + plan->P.active[2] - 1));
+          for (int q = 0; q < nq; ++q) {
+            const int32_t id = plan->jump_host[(b * 6 + f) * 4 + q];
+            if (id < 0 || id >= nb) return fx_fail(FX_ERR_INVALID_ARG, "set_topology: block %lld face %d: jump entry %d = %d out of range", b, f, q, id);
+          }
+          jumps = 1;
         } else if (v != FX_BC_OUTFLOW && v != FX_BC_REFLECT) {
-          return fx_fail(FX_ERR_UNSUPPORTED, "set_topology: block %lld face %d has code %d: coarse/fine neighbours are not supported", b, f, v);
+          return fx_fail(FX_ERR_UNSUPPORTED, "set_topology: block %lld face %d has unknown code %d", b, f, v);
         }
       }
   }
   plan->P.neigh = neigh_dev;
+  plan->P.has_jumps = jumps;
   plan->topology_set = true;
   plan->P.walls = 0;
   // z-chain segments: walk down (-z) from every unvisited block to the start of its chain (or once around a periodic

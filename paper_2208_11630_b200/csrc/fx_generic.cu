@@ -112,6 +112,7 @@ __device__ __forceinline__ long long fx_stencil_cell(const FxParams &P, long lon
   const int side = t >= n;
   const int nb = __ldg(&P.neigh[b * 6 + 2 * D + side]);
   if (nb >= 0) return c + (nb - b) * P.S_b + (long long)(o + (side ? -n : n)) * s;
+  if (nb <= FX_NEIGH_COARSER) return c + o * s;  // a refinement jump [B12]: this block's own guard zone, filled by fx_k_amr_fill
   if (nb == FX_BC_REFLECT) {
     flip = true;
     return c + (long long)((side ? 2 * n - 1 - t : -1 - t) - idx) * s;
@@ -130,10 +131,10 @@ template <int RECON> struct FxScalarShared {
 // Direction D of one zone, in the lean arithmetic of the fused kernel (fx_c2p_v2, fx_recon_cell, fx_riemann_v2: one
 // Newton step on the MUFU seeds instead of IEEE division and square root; same formulas, rounding differs): the 2R+1
 // stencil cells are converted once, cells -1, 0, +1 are reconstructed once each, and the zone's two faces are solved.
-template <int RECON, int RIEMANN, int WS, int D, bool SCALARS>
+template <int RECON, int RIEMANN, int WS, int D, bool SCALARS, bool AMR = false>
 __device__ __forceinline__ unsigned fx_zone_direction(const FxParams &P, const double *__restrict__ X, long long b,
                                                       long long c, int idx, long long s, double rd, double S[5],
-                                                      unsigned &qfb, FxScalarShared<RECON> *sh) {
+                                                      unsigned &qfb, FxScalarShared<RECON> *sh, int tflat = 0) {
   constexpr int R = (RECON == FX_RECON_PLM_MINMOD) ? 2 : 3, r = R - 1;
   constexpr int in = 1 + D, it1 = 1 + (D + 1) % 3, it2 = 1 + (D + 2) % 3;
   constexpr int map[5] = {0, in, it1, it2, 4};
@@ -190,6 +191,16 @@ __device__ __forceinline__ unsigned fx_zone_direction(const FxParams &P, const d
   if (!(fabs(sum) <= 1.79e308)) hit |= FX_STATUS_NONFINITE;
 #pragma unroll
   for (int f = 0; f < 5; ++f) S[map[f]] += rd * (Fp[f] - Fm[f]);
+  if (AMR) {  // the boundary fluxes at refinement jumps, both sides, for the flux correction [B14]
+    if (idx == 0 && __ldg(&P.neigh[b * 6 + 2 * D]) <= FX_NEIGH_COARSER) {
+#pragma unroll
+      for (int f = 0; f < 5; ++f) P.fjump[((b * 6 + 2 * D) * 5 + map[f]) * (long long)P.fj_area + tflat] = Fm[f];
+    }
+    if (idx == P.n[D] - 1 && __ldg(&P.neigh[b * 6 + 2 * D + 1]) <= FX_NEIGH_COARSER) {
+#pragma unroll
+      for (int f = 0; f < 5; ++f) P.fjump[((b * 6 + 2 * D + 1) * 5 + map[f]) * (long long)P.fj_area + tflat] = Fp[f];
+    }
+  }
   if (SCALARS) {
     sh->A[D][0][threadIdx.x] = Am;
     sh->A[D][1][threadIdx.x] = Ap;
@@ -235,7 +246,7 @@ __device__ __forceinline__ double fx_zone_scalar_direction(const FxParams &P, co
 // 5 CTAs 13.9 / 25.9, 6 CTAs (80 registers) 13.5 / 24.7, 8 CTAs (64 registers; its spills reach DRAM: 28.6 GB written
 // for 9.7 GB) 16.3 / 31.0.  WENO5 at config 4 without / with 2 scalars: 3 CTAs 5.5 / 7.8, 4 CTAs 5.5 / 7.4, 5 CTAs
 // 5.6 / 7.3.  (The IEEE-arithmetic version of this kernel: PLM uncapped 38.3, 8 CTAs 30.0; WENO5 uncapped 15.2, 4 CTAs 8.2.)
-template <int RECON, int RIEMANN, int WS, bool SCALARS>
+template <int RECON, int RIEMANN, int WS, bool SCALARS, bool AMR = false>
 __global__ void __launch_bounds__(128, RECON == FX_RECON_PLM_MINMOD ? FX_GENERIC_MINB_PLM : FX_GENERIC_MINB_WENO) fx_k_generic_stage(FxParams P, const double *__restrict__ X,
                                                           const double *U0, double *out,
                                                           const double *__restrict__ dx, double dt,
@@ -264,9 +275,10 @@ __global__ void __launch_bounds__(128, RECON == FX_RECON_PLM_MINMOD ? FX_GENERIC
   const double rd0 = P.active[0] ? dt / __ldg(&dx[b * 3 + 0]) : 0.0;
   const double rd1 = P.active[1] ? dt / __ldg(&dx[b * 3 + 1]) : 0.0;
   const double rd2 = P.active[2] ? dt / __ldg(&dx[b * 3 + 2]) : 0.0;
-  if (P.active[0]) hit |= fx_zone_direction<RECON, RIEMANN, WS, 0, SCALARS>(P, X, b, c, i, 1, rd0, S, qfb, sh);
-  if (P.active[1]) hit |= fx_zone_direction<RECON, RIEMANN, WS, 1, SCALARS>(P, X, b, c, j, P.S_j, rd1, S, qfb, sh);
-  if (P.active[2]) hit |= fx_zone_direction<RECON, RIEMANN, WS, 2, SCALARS>(P, X, b, c, k, P.S_k, rd2, S, qfb, sh);
+  // (tflat: the zone's position on the face, transverse dimensions ascending, first one fastest)
+  if (P.active[0]) hit |= fx_zone_direction<RECON, RIEMANN, WS, 0, SCALARS, AMR>(P, X, b, c, i, 1, rd0, S, qfb, sh, k * ny + j);
+  if (P.active[1]) hit |= fx_zone_direction<RECON, RIEMANN, WS, 1, SCALARS, AMR>(P, X, b, c, j, P.S_j, rd1, S, qfb, sh, k * nx + i);
+  if (P.active[2]) hit |= fx_zone_direction<RECON, RIEMANN, WS, 2, SCALARS, AMR>(P, X, b, c, k, P.S_k, rd2, S, qfb, sh, j * nx + i);
   if (P.grav_on) {  // constant-gravity source of the stage input's own zone [B10]
     const double rho = X[c];
     double gm = 0.0;
@@ -347,6 +359,9 @@ int fx_launch_generic_stage(const FxParams &P, const double *X, const double *U0
     if (P.nvars > 5) {                                                                                          \
       if (P.wavespeed == 0) fx_k_generic_stage<RC, RM, 0, true><<<grid, 128, sizeof(FxScalarShared<RC>), st>>>(P, X, U0, out, dx, dt, dt_dev, beta, first, nzones); \
       else fx_k_generic_stage<RC, RM, 1, true><<<grid, 128, sizeof(FxScalarShared<RC>), st>>>(P, X, U0, out, dx, dt, dt_dev, beta, first, nzones); \
+    } else if (P.has_jumps) {                                                                                   \
+      if (P.wavespeed == 0) fx_k_generic_stage<RC, RM, 0, false, true><<<grid, 128, 0, st>>>(P, X, U0, out, dx, dt, dt_dev, beta, first, nzones); \
+      else fx_k_generic_stage<RC, RM, 1, false, true><<<grid, 128, 0, st>>>(P, X, U0, out, dx, dt, dt_dev, beta, first, nzones); \
     } else {                                                                                                    \
       if (P.wavespeed == 0) fx_k_generic_stage<RC, RM, 0, false><<<grid, 128, 0, st>>>(P, X, U0, out, dx, dt, dt_dev, beta, first, nzones); \
       else fx_k_generic_stage<RC, RM, 1, false><<<grid, 128, 0, st>>>(P, X, U0, out, dx, dt, dt_dev, beta, first, nzones); \

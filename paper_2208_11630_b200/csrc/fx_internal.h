@@ -24,6 +24,10 @@ struct FxParams {
   int walls;                        // some block has a reflecting wall in an active dimension [B9]
   int grav_on;                      // any component of grav is non-zero [B10]
   double grav[3];
+  const int *jump;                  // refinement jumps [B12]: [nblocks][6][4], device; nullptr if none was given
+  int has_jumps;                    // some active face carries FX_NEIGH_COARSER / FX_NEIGH_FINER
+  double *fjump;                    // boundary-face fluxes captured at jump faces [B14]: [nblocks][6][5][fj_area], in the workspace
+  int fj_area;                      // largest face of a block, in zones
   unsigned long long *scratch;      // device scratch block, see FX_SCR_*
 };
 
@@ -50,6 +54,7 @@ struct fx_hydro_plan {
   double *stage[2];     // RK stage copies inside the workspace
   bool topology_set;
   int zchain;           // FX_OPT_ZCHAIN: longest segment (1 .. FX_SEG_MAX)
+  int32_t *jump_host;   // host copy of the refinement-jump table (new[]), or nullptr
   int *seg_host;        // segment table built by set_topology (new[]), nseg_host rows
   int nseg_host;
   bool seg_uploaded;
@@ -83,6 +88,9 @@ int fx_launch_compute_dt(const FxParams &P, const double *U, const double *dx, d
 int fx_launch_generic_stage(const FxParams &P, const double *X, const double *U0, double *out, const double *dx,
                             double dt, const double *dt_dev, double beta, int first, cudaStream_t st);
 int fx_launch_debug_fluxes(const FxParams &P, const double *U, int dir, double *F, cudaStream_t st);
+int fx_launch_amr_fill(const FxParams &P, double *U, int depth, cudaStream_t st);  // face guard zones behind refinement jumps
+int fx_launch_amr_flux_correct(const FxParams &P, double *out, const double *dx, double dt, const double *dt_dev, double beta,
+                               cudaStream_t st);
 bool fx_stage_tma_supported(const FxParams &P);
 bool fx_stage_pair_supported(const FxParams &P);  // the two-zones-per-thread variant: PLM, no wall, no gravity
 bool fx_stage_tile_supported(const FxParams &P);

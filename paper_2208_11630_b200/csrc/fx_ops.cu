@@ -18,7 +18,9 @@ extern "C" int fx_fill_guardcells(fx_hydro_plan *plan, double *U, void *stream) 
   int rc = fx_need(plan, true, false, "fill_guardcells");
   if (rc) return rc;
   if (!U && plan->P.nblocks > 0) return fx_fail(FX_ERR_INVALID_ARG, "fill_guardcells: null U");
-  return fx_launch_fill_guardcells(plan->P, U, (cudaStream_t)stream);
+  rc = fx_launch_fill_guardcells(plan->P, U, (cudaStream_t)stream);
+  if (rc) return rc;
+  return fx_launch_amr_fill(plan->P, U, plan->nguard, (cudaStream_t)stream);  // second pass: the jump faces [B12, B13]
 }
 
 extern "C" int fx_guardcell_index_map(fx_hydro_plan *plan, int64_t b0, int64_t nb, int64_t *src, void *stream) {
@@ -51,6 +53,11 @@ static int fx_stage(fx_hydro_plan *plan, double *X, const double *U0, double *ou
     rc = fx_launch_fill_faces(plan->P, X, 5, st);
     if (rc) return rc;
   }
+  const bool amr = plan->P.has_jumps != 0;  // (generic path)
+  if (amr) {  // the face guard zones behind refinement jumps: restriction / prolongation of the stage input [B12, B13]
+    rc = fx_launch_amr_fill(plan->P, X, plan->P.recon == FX_RECON_WENO5 ? 3 : 2, st);
+    if (rc) return rc;
+  }
   const bool rec = plan->timing && plan->ev && plan->nrec < FX_MAX_REC;
   if (rec) FX_CUDA(cudaEventRecord(plan->ev[2 * plan->nrec], st));
   rc = fused ? (path == 3 ? fx_launch_stage_pair(plan->P, X, U0, out, dx, dt, dt_dev, beta, first, cfl_next, dt_next, st)
@@ -61,6 +68,10 @@ static int fx_stage(fx_hydro_plan *plan, double *X, const double *U0, double *ou
   if (rec) {  // the pair brackets the stage kernel alone (fx_hydro.h), not the reduction pass below
     FX_CUDA(cudaEventRecord(plan->ev[2 * plan->nrec + 1], st));
     ++plan->nrec;
+  }
+  if (amr) {  // coarse face fluxes at the jumps <- the mean of the fine ones [B14]
+    rc = fx_launch_amr_flux_correct(plan->P, out, dx, dt, dt_dev, first ? 1.0 : beta, st);
+    if (rc) return rc;
   }
   if (!fused && dt_next) {  // the generic and tile paths have no fused reduction: a7 as its own pass over the finished state
     rc = fx_launch_compute_dt(plan->P, out, dx, cfl_next, dt_next, st);

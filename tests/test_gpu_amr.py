@@ -1,0 +1,91 @@
+"""GPU <-> oracle parity of the fine-coarse boundary services [B12-B14] on static two-level grids: the face guard zones
+behind refinement jumps bit for bit (restriction, prolongation), advance to the [NS] tolerances, conservation through the
+jumps, uniform state bit for bit."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import fxoracle as fxo
+from tests.helpers import two_level_grid, rel_err
+from tests.test_oracle_amr import GAMMA, GRIDS, amr_plan, cons, dx_of, smooth_field, state_from, totals
+
+pytestmark = pytest.mark.gpu
+
+
+def gpu_amr_plan(grid, dims, g=4, recon=0, riemann=1, rk=2):
+    from paper_2208_11630_b200 import binding as fx
+    plan = fx.HydroPlan(dims, g, len(grid["level"]), GAMMA, recon, riemann, rk)
+    plan.fx_hydro_plan_set_refinement(grid["jump"])
+    plan.fx_hydro_plan_set_topology(grid["neigh"])
+    plan.fx_hydro_plan_set_workspace()
+    assert plan.path == 0
+    return plan
+
+
+class Cfg:
+    gamma = GAMMA
+
+
+@pytest.mark.parametrize("nbc,refined,dims", GRIDS)
+@pytest.mark.parametrize("recon,riemann,rk", [(0, 1, 2), (1, 0, 3), (1, 1, 3)])
+def test_amr_fill_bitwise_and_advance_parity(nbc, refined, dims, recon, riemann, rk):
+    grid = two_level_grid(nbc, refined, dims)
+    oplan = amr_plan(grid, dims, recon=recon, riemann=riemann, rk=rk)
+    gplan = gpu_amr_plan(grid, dims, recon=recon, riemann=riemann, rk=rk)
+    ndim = sum(1 for d in dims if d > 1)
+    L = [nbc[d] * dims[d] for d in range(3)]
+    Uo = state_from(oplan, smooth_field(grid, dims, L))
+    Ud = torch.from_numpy(Uo).cuda()
+    # guard fill: every zone, jump faces included, bit for bit
+    F = Uo.copy()
+    oplan.fill_guardcells(F)
+    Fg = Ud.clone()
+    gplan.fx_fill_guardcells(Fg)
+    assert np.array_equal(Fg.cpu().numpy(), F)
+    assert np.array_equal(gplan.fx_guardcell_index_map().cpu().numpy(), oplan.index_map())
+    dx = dx_of(grid)
+    dxd = torch.from_numpy(dx).cuda()
+    T0 = totals(oplan, grid, Uo, ndim)
+    for step in range(10):
+        dt = oplan.compute_dt(Uo, dx, 0.3)
+        dtg = float(gplan.fx_hydro_compute_dt(Ud, dxd, 0.3).item())
+        assert abs(dtg - dt) <= 1e-14 * dt
+        oplan.advance(Uo, dx, dt)
+        gplan.fx_hydro_advance(Ud, dxd, dt)
+        if step in (0, 9):
+            err = rel_err(Cfg, gplan.interior(Ud).cpu().numpy(), oplan.interior(Uo))
+            assert err <= (1e-12 if step == 0 else 1e-9), (step, err)
+    got = Ud.cpu().numpy()
+    T1 = totals(oplan, grid, got, ndim)
+    scale = np.array([T0[0], 2.4 * T0[0], 2.4 * T0[0], 2.4 * T0[0], T0[4]])
+    assert np.max(np.abs(T1 - T0) / scale) <= 1e-13
+    fo, _ = oplan.status()
+    fg, _ = gplan.fx_hydro_status()
+    assert fo == fg == 0
+
+
+@pytest.mark.parametrize("nbc,refined,dims", GRIDS[1:3])
+def test_amr_uniform_state_bitwise_and_step_api(nbc, refined, dims):
+    grid = two_level_grid(nbc, refined, dims)
+    gplan = gpu_amr_plan(grid, dims)
+    n = len(grid["level"])
+    shape = (n, dims[2], dims[1], dims[0])
+    W = (1.3, 0.4, -0.7, 0.2 if dims[2] > 1 else 0.0, 0.9)
+    oplan = amr_plan(grid, dims)
+    U = torch.from_numpy(state_from(oplan, cons(*[np.full(shape, x) for x in W]))).cuda()
+    U0 = gplan.interior(U).clone()
+    dxd = torch.from_numpy(dx_of(grid)).cuda()
+    dt = gplan.fx_hydro_compute_dt(U, dxd, 0.3).clone()
+    for _ in range(5):
+        gplan.fx_hydro_step(U, dxd, 0.3, dt)
+    assert torch.equal(gplan.interior(U), U0)
+
+
+def test_jumps_need_the_refinement_table():
+    from paper_2208_11630_b200 import binding as fx
+    dims = (8, 8, 8)
+    grid = two_level_grid((3, 3, 3), {(1, 1, 1)}, dims)
+    plan = fx.HydroPlan(dims, 4, len(grid["level"]), GAMMA, 0, 1, 2)
+    with pytest.raises(fx.FxError) as e:
+        plan.fx_hydro_plan_set_topology(grid["neigh"])
+    assert e.value.code == -3  # FX_ERR_UNSUPPORTED
