@@ -198,8 +198,10 @@ extern "C" int fx_hydro_plan_set_option(fx_hydro_plan *plan, int key, double val
 
 extern "C" int fx_hydro_plan_path(const fx_hydro_plan *plan) {
   if (!plan) return fx_fail(FX_ERR_INVALID_ARG, "plan_path: null plan");
-  if (plan->nvars > 5) return 0;  // passive scalars [B11] are carried by the generic path only
   if (plan->P.has_jumps) return 0;  // refinement jumps [B12-B14]: the generic path reads the interpolated guard zones
+  // passive scalars [B11]: behind the fused kernel by the scalar pass where it applies (PLM, same-level neighbours
+  // everywhere, no gravity), else on the generic path
+  if (plan->nvars > 5 && !(plan->path_option == 0 && fx_stage_tma_supported(plan->P) && fx_scalar_pass_supported(plan->P))) return 0;
   if ((plan->path_option == 0 || plan->path_option == 3) && fx_stage_tma_supported(plan->P))
     return (plan->path_option == 3 && fx_stage_pair_supported(plan->P)) ? 3 : 1;
   // 3-D blocks with PLM: the generic zone kernel, which gathers its halo cells itself, is ahead of the tile kernel
@@ -219,6 +221,12 @@ static size_t fx_seg_bytes(const fx_hydro_plan *plan) {  // room for one segment
   return (((size_t)plan->P.nblocks * FX_SEG_STRIDE * sizeof(int)) + 255) & ~(size_t)255;
 }
 
+static size_t fx_fq_bytes(const fx_hydro_plan *plan) {  // scalar pass [B11]: (mass flux, Aq) x 3 low faces per interior zone
+  const FxParams &P = plan->P;
+  if (plan->nvars <= 5 || P.recon != FX_RECON_PLM_MINMOD || P.n[0] != 16 || P.n[1] != 16 || !P.active[2]) return 0;
+  return (((size_t)6 * P.nblocks * P.n[0] * P.n[1] * P.n[2] * sizeof(double)) + 255) & ~(size_t)255;
+}
+
 static size_t fx_fjump_bytes(const fx_hydro_plan *plan) {  // boundary fluxes at refinement jumps [B14]
   if (!plan->P.jump) return 0;
   return (((size_t)plan->P.nblocks * 6 * 5 * (size_t)plan->P.fj_area * sizeof(double)) + 255) & ~(size_t)255;
@@ -230,7 +238,7 @@ static size_t fx_stage_pad(const fx_hydro_plan *plan) { return (128 - ((size_t)p
 
 extern "C" size_t fx_hydro_plan_workspace_bytes(const fx_hydro_plan *plan) {
   if (!plan) return 0;
-  return (size_t)FX_SCR_WORDS * 8 + 256 + (size_t)(plan->rk - 1) * fx_state_bytes_aligned(plan) + fx_seg_bytes(plan) + fx_fjump_bytes(plan);
+  return (size_t)FX_SCR_WORDS * 8 + 256 + (size_t)(plan->rk - 1) * fx_state_bytes_aligned(plan) + fx_seg_bytes(plan) + fx_fjump_bytes(plan) + fx_fq_bytes(plan);
 }
 
 // Upload the segment table into its place behind the stage copies (needs both the workspace and the topology).
@@ -264,6 +272,9 @@ extern "C" int fx_hydro_plan_set_workspace(fx_hydro_plan *plan, void *ws, size_t
   plan->P.fjump = plan->P.jump ? (double *)((char *)ws + FX_SCR_WORDS * 8 + 256 + (size_t)(plan->rk - 1) * fx_state_bytes_aligned(plan) +
                                             fx_seg_bytes(plan))
                                : nullptr;
+  plan->P.fq = fx_fq_bytes(plan) ? (double *)((char *)ws + FX_SCR_WORDS * 8 + 256 + (size_t)(plan->rk - 1) * fx_state_bytes_aligned(plan) +
+                                              fx_seg_bytes(plan) + fx_fjump_bytes(plan))
+                                 : nullptr;
   return fx_seg_upload(plan);
 }
 
@@ -298,7 +309,7 @@ extern "C" int fx_hydro_plan_set_refinement(fx_hydro_plan *plan, const int32_t *
 extern "C" int fx_hydro_plan_set_topology(fx_hydro_plan *plan, const int32_t *neigh_dev) {
   if (!plan) return fx_fail(FX_ERR_INVALID_ARG, "set_topology: null plan");
   const long long nb = plan->P.nblocks;
-  int jumps = 0;
+  int jumps = 0, all_interior = 1;
   if (nb > 0) {
     if (!neigh_dev) return fx_fail(FX_ERR_INVALID_ARG, "set_topology: null table");
     std::vector<int32_t> h((size_t)nb * 6);
@@ -307,6 +318,7 @@ extern "C" int fx_hydro_plan_set_topology(fx_hydro_plan *plan, const int32_t *ne
       for (int f = 0; f < 6; ++f) {
         if (!plan->P.active[f / 2]) continue;
         const int32_t v = h[b * 6 + f];
+        if (v < 0 && b < plan->P.nown) all_interior = 0;
         if (v >= 0) {
           if (v >= nb) return fx_fail(FX_ERR_INVALID_ARG, "set_topology: block %lld face %d -> id %d out of range", b, f, v);
         } else if (v == FX_NEIGH_COARSER || v == FX_NEIGH_FINER) {
@@ -326,6 +338,7 @@ extern "C" int fx_hydro_plan_set_topology(fx_hydro_plan *plan, const int32_t *ne
   }
   plan->P.neigh = neigh_dev;
   plan->P.has_jumps = jumps;
+  plan->P.all_interior = all_interior;
   plan->topology_set = true;
   plan->P.walls = 0;
   // z-chain segments: walk down (-z) from every unvisited block to the start of its chain (or once around a periodic

@@ -24,6 +24,8 @@ struct FxParams {
   int walls;                        // some block has a reflecting wall in an active dimension [B9]
   int grav_on;                      // any component of grav is non-zero [B10]
   double grav[3];
+  double *fq;                       // scalar pass [B11]: mass flux and Aq of every zone's low x, y, z faces, [6][nblocks nz ny nx], in the workspace
+  int all_interior;                 // every active face of every owned block has a same-level neighbour (no physical boundary, no jump)
   const int *jump;                  // refinement jumps [B12]: [nblocks][6][4], device; nullptr if none was given
   int has_jumps;                    // some active face carries FX_NEIGH_COARSER / FX_NEIGH_FINER
   double *fjump;                    // boundary-face fluxes captured at jump faces [B14]: [nblocks][6][5][fj_area], in the workspace
@@ -91,6 +93,9 @@ int fx_launch_debug_fluxes(const FxParams &P, const double *U, int dir, double *
 int fx_launch_amr_fill(const FxParams &P, double *U, int depth, cudaStream_t st);  // face guard zones behind refinement jumps
 int fx_launch_amr_flux_correct(const FxParams &P, double *out, const double *dx, double dt, const double *dt_dev, double beta,
                                cudaStream_t st);
+bool fx_scalar_pass_supported(const FxParams &P);
+int fx_launch_scalar_pass(const FxParams &P, const double *X, const double *U0, double *out, const double *dx, double dt,
+                          const double *dt_dev, double beta, int first, cudaStream_t st);
 bool fx_stage_tma_supported(const FxParams &P);
 bool fx_stage_pair_supported(const FxParams &P);  // the two-zones-per-thread variant: PLM, no wall, no gravity
 bool fx_stage_tile_supported(const FxParams &P);

@@ -60,11 +60,21 @@ static int fx_stage(fx_hydro_plan *plan, double *X, const double *U0, double *ou
   }
   const bool rec = plan->timing && plan->ev && plan->nrec < FX_MAX_REC;
   if (rec) FX_CUDA(cudaEventRecord(plan->ev[2 * plan->nrec], st));
+  // with a scalar pass behind the fused kernel the next time step waits in a scratch word until the pass, which still
+  // reads this step's dt from the device, has been enqueued
+  double *dt_user = dt_next;
+  const bool park_dt = fused && plan->nvars > 5 && dt_next != nullptr;
+  if (park_dt) dt_next = (double *)&plan->P.scratch[FX_SCR_WORDS - 3];
   rc = fused ? (path == 3 ? fx_launch_stage_pair(plan->P, X, U0, out, dx, dt, dt_dev, beta, first, cfl_next, dt_next, st)
                           : fx_launch_stage_tma(plan->P, X, U0, out, dx, dt, dt_dev, beta, first, cfl_next, dt_next, st))
              : (path == 2 ? fx_launch_stage_tile(plan->P, X, U0, out, dx, dt, dt_dev, beta, first, st)
                           : fx_launch_generic_stage(plan->P, X, U0, out, dx, dt, dt_dev, beta, first, st));
   if (rc) return rc;
+  if (fused && plan->nvars > 5) {  // passive scalars [B11] behind the fused kernel: the scalar pass (inside the timing bracket)
+    rc = fx_launch_scalar_pass(plan->P, X, U0, out, dx, dt, dt_dev, beta, first, st);
+    if (rc) return rc;
+    if (park_dt) FX_CUDA(cudaMemcpyAsync(dt_user, dt_next, sizeof(double), cudaMemcpyDeviceToDevice, st));
+  }
   if (rec) {  // the pair brackets the stage kernel alone (fx_hydro.h), not the reduction pass below
     FX_CUDA(cudaEventRecord(plan->ev[2 * plan->nrec + 1], st));
     ++plan->nrec;

@@ -77,13 +77,13 @@ __device__ __forceinline__ void cta_sync() { asm volatile("bar.sync 0, %0;" ::"n
 
 // Riemann flux for direction D (compile-time) from un-rotated primitive states; flux returned in the
 // un-rotated variable order (rho, mx, my, mz, E).
-template <int RIEMANN, int WS, int D>
-__device__ __forceinline__ void flux_dir(const FxParams &P, const double WL[5], const double WR[5], double F[5]) {
+template <int RIEMANN, int WS, int D, bool AQ = false>
+__device__ __forceinline__ void flux_dir(const FxParams &P, const double WL[5], const double WR[5], double F[5], double *Aq = nullptr) {
   constexpr int in = 1 + D, it1 = 1 + (D + 1) % 3, it2 = 1 + (D + 2) % 3;
   const double wl[5] = {WL[0], WL[in], WL[it1], WL[it2], WL[4]};
   const double wr[5] = {WR[0], WR[in], WR[it1], WR[it2], WR[4]};
   double f[5];
-  fx_riemann_v2<RIEMANN, WS>(P, wl, wr, f);
+  fx_riemann_v2<RIEMANN, WS, AQ>(P, wl, wr, f, Aq);
   F[0] = f[0];
   F[in] = f[1];
   F[it1] = f[2];
@@ -93,7 +93,9 @@ __device__ __forceinline__ void flux_dir(const FxParams &P, const double WL[5], 
 
 // EXTRAS: some block of the launch has a reflecting wall [B9] or gravity is on [B10]: the image cells' sign flips
 // and the source term are compiled in only then
-template <int RECON, int RIEMANN, int WS, bool FIRST, bool DTOUT, bool EXTRAS>
+// SCAL: the plan carries passive scalars [B11] and they take the scalar pass (fx_scalar_pass.cu): every zone also leaves the
+// mass flux and the advected-quantity coefficient Aq of its three low faces in P.fq for it
+template <int RECON, int RIEMANN, int WS, bool FIRST, bool DTOUT, bool EXTRAS, bool SCAL = false>
 __global__ void __launch_bounds__(NTHREADS) __maxnreg__(Rc<RECON>::NREG)
 fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ CUtensorMap mXx,
                const __grid_constant__ CUtensorMap mXy, const __grid_constant__ CUtensorMap mU0,
@@ -184,6 +186,8 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
     double rate = 0.0;     // DTOUT: running maximum of (|u_d| + c) / dx_d over this thread's finished zones
     double q[W][5];        // q[m] = primitives of cell c - r + m at tick c
     double qpz[5], Fz[5];  // plus-side z state of cell c-1; z flux of face c-1 (between cells c-2 and c-1)
+    double Aqz = 0.0;      // SCAL: Aq of that face
+    int sq = 0, sk = 0;    // SCAL: plane p is plane sk of the sq-th block of the segment
     {
       // prologue: cells -R .. r straight from global memory (all loads in flight together), the plus-side state
       // of cell 0 and the flux of face 0
@@ -213,7 +217,7 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
       double qm[5], qpm1[5];
       hit |= fx_recon_cell5<RECON>(&w[0], P.weno_eps, qm, qpm1);  // cell -1
       hit |= fx_recon_cell5<RECON>(&w[1], P.weno_eps, qm, qpz);   // cell 0
-      flux_dir<RIEMANN, WS, 2>(P, qpm1, qm, Fz);
+      flux_dir<RIEMANN, WS, 2, SCAL>(P, qpm1, qm, Fz, &Aqz);
 #pragma unroll
       for (int m = 0; m < 2 * r; ++m)
 #pragma unroll
@@ -259,11 +263,11 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
         if (c + r < nz) hit |= h;
       }
       // z: reconstruct cell c, flux of face c (between cells c-1 and c)
-      double Fz_new[5];
+      double Fz_new[5], Aqz_new = 0.0, Aqx = 0.0, Aqy = 0.0;
       {
         double qmz[5], qpz_new[5];
         hit |= fx_recon_cell5<RECON>(q, P.weno_eps, qmz, qpz_new);
-        flux_dir<RIEMANN, WS, 2>(P, qpz, qmz, Fz_new);
+        flux_dir<RIEMANN, WS, 2, SCAL>(P, qpz, qmz, Fz_new, &Aqz_new);
 #pragma unroll
         for (int v = 0; v < 5; ++v) qpz[v] = qpz_new[v];
       }
@@ -272,18 +276,30 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
         double WL[5];
 #pragma unroll
         for (int v = 0; v < 5; ++v) WL[v] = S.Lx[v][j][i];
-        flux_dir<RIEMANN, WS, 0>(P, WL, qmx, Fx);
+        flux_dir<RIEMANN, WS, 0, SCAL>(P, WL, qmx, Fx, &Aqx);
 #pragma unroll
         for (int v = 0; v < 5; ++v) S.Lx[v][j][i] = Fx[v];  // in place: only this thread read the state
 #pragma unroll
         for (int v = 0; v < 5; ++v) WL[v] = S.Ly[v][j][i];
-        flux_dir<RIEMANN, WS, 1>(P, WL, qmy, Fy);
+        flux_dir<RIEMANN, WS, 1, SCAL>(P, WL, qmy, Fy, &Aqy);
 #pragma unroll
         for (int v = 0; v < 5; ++v) S.Ly[v][j][i] = Fy[v];
       }
       if (c < nz) {  // primitives of plane p + 1 (cell c of the window): nobody reads P between barriers B and C
 #pragma unroll
         for (int v = 0; v < 5; ++v) S.P[v][j + R][i + R] = q[r][v];
+      }
+      if (SCAL) {  // mass flux and Aq of the zone's low x, y and z faces, for the scalar pass: fq[6][zone], zones block by block
+        const long long zone = (((long long)S.chain[2 + sq] * nzb + sk) * NY + j) * NX + i;
+        const long long nzt = (long long)P.nblocks * nzb * (NY * NX);
+        P.fq[zone] = Fx[0];
+        P.fq[nzt + zone] = Aqx;
+        P.fq[2 * nzt + zone] = Fy[0];
+        P.fq[3 * nzt + zone] = Aqy;
+        P.fq[4 * nzt + zone] = Fz[0];
+        P.fq[5 * nzt + zone] = Aqz;
+        Aqz = Aqz_new;
+        if (++sk == nzb) { sk = 0; ++sq; }
       }
       cta_sync();  // C: fluxes and the next plane's primitives visible
       {
@@ -525,7 +541,7 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
 }
 
 // ------------------------------------------------------------------ host side: tensor maps and launch
-template <int RECON, int RIEMANN, int WS, bool FIRST, bool DTOUT, bool EXTRAS>
+template <int RECON, int RIEMANN, int WS, bool FIRST, bool DTOUT, bool EXTRAS, bool SCAL = false>
 int launch(const FxParams &P, const double *X, const double *U0, double *out, const double *dx, double dt, const double *dt_dev,
            double beta, double cfl_next, double *dt_next, cudaStream_t st) {
   constexpr int R = Rc<RECON>::R, BW = Rc<RECON>::BW;
@@ -536,7 +552,7 @@ int launch(const FxParams &P, const double *X, const double *U0, double *out, co
   if ((rc = make_map(&mXy, P, X, NX, R))) return rc;
   if ((rc = make_map(&mU0, P, U0, NX, NY))) return rc;
   if ((rc = make_map(&mOut, P, out, NX, NY))) return rc;
-  auto kern = fx_k_stage_tma<RECON, RIEMANN, WS, FIRST, DTOUT, EXTRAS>;
+  auto kern = fx_k_stage_tma<RECON, RIEMANN, WS, FIRST, DTOUT, EXTRAS, SCAL>;
   const int smem = (int)sizeof(Smem<RECON>);
   // (per device and context, and cheap: set on every launch rather than cached per process)
   FX_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
@@ -557,6 +573,13 @@ int launch(const FxParams &P, const double *X, const double *U0, double *out, co
 template <int RECON, int RIEMANN, int WS>
 int launch_ws(const FxParams &P, const double *X, const double *U0, double *out, const double *dx, double dt, const double *dt_dev,
               double beta, int first, double cfl_next, double *dt_next, cudaStream_t st) {
+  if constexpr (RECON == FX_RECON_PLM_MINMOD) {
+    if (P.nvars > 5) {  // with passive scalars: also leave the faces' mass flux and Aq for the scalar pass
+      if (first) return launch<RECON, RIEMANN, WS, true, false, false, true>(P, X, U0, out, dx, dt, dt_dev, beta, 0.0, nullptr, st);
+      if (dt_next) return launch<RECON, RIEMANN, WS, false, true, false, true>(P, X, U0, out, dx, dt, dt_dev, beta, cfl_next, dt_next, st);
+      return launch<RECON, RIEMANN, WS, false, false, false, true>(P, X, U0, out, dx, dt, dt_dev, beta, 0.0, nullptr, st);
+    }
+  }
   if (P.walls || P.grav_on) {
     if (first) return launch<RECON, RIEMANN, WS, true, false, true>(P, X, U0, out, dx, dt, dt_dev, beta, 0.0, nullptr, st);
     if (dt_next) return launch<RECON, RIEMANN, WS, false, true, true>(P, X, U0, out, dx, dt, dt_dev, beta, cfl_next, dt_next, st);
@@ -588,6 +611,7 @@ bool fx_stage_tma_supported(const FxParams &P) {
 int fx_launch_stage_tma(const FxParams &P, const double *X, const double *U0, double *out, const double *dx, double dt,
                         const double *dt_dev, double beta, int first, double cfl_next, double *dt_next, cudaStream_t st) {
   if (!fx_stage_tma_supported(P)) return fx_fail(FX_ERR_UNSUPPORTED, "TMA stage kernel: block shape not supported");
+  if (P.nvars > 5 && !fx_scalar_pass_supported(P)) return fx_fail(FX_ERR_UNSUPPORTED, "TMA stage kernel: passive scalars need the scalar pass");
   if (P.nblocks == 0) return FX_OK;
   if (first && X != U0) return fx_fail(FX_ERR_INVALID_ARG, "TMA stage kernel: the first stage takes U0 from its stage input (X must be U0)");
   if (((uintptr_t)X | (uintptr_t)U0 | (uintptr_t)out) & 15)

@@ -29,7 +29,7 @@ def test_full_size_scalars_sampled_blocks_and_conservation():
     plan.fx_hydro_plan_set_option(fx.OPT_GUARD_X, 8)
     plan.fx_hydro_plan_set_topology(neigh)
     plan.fx_hydro_plan_set_workspace()
-    assert plan.path == 0
+    assert plan.path == 1  # fused kernel + scalar pass (config 5 is periodic, PLM)
     U = plan.alloc_state(fill=float("nan"))
     Ui = plan.interior(U)
     for b0 in range(0, cfg.nblocks, 1024):
