@@ -343,7 +343,7 @@ def run_ours(args, rank, world, local_rank):
         cfg, plan, U, dx, coords = build_workload(args, device)
         zones = cfg.interior_zones
     stages = cfg.rk_order
-    fused = plan.path in (1, 3)
+    fused = plan.path in (1, 3, 4)
     # fused path: one launch per RK stage, the CFL reduction (a7) rides in the last one; tile and generic paths: one
     # stage kernel per stage, then the reduction pass; with passive scalars also their face fill per stage
     launches_per_step = stages if fused else (stages + 1 + (stages if args.scalars else 0))
@@ -420,7 +420,7 @@ def run_ours(args, rank, world, local_rank):
                 "frac": side["frac"], "traffic": traffic, "traffic_source": traffic_src,
                 "roof_ps_per_zone_stage": {"hbm": t_hbm * 1e12, "fp64": t_fp * 1e12 if flops is not None else None},
                 "hbm": hbm, "fp64": fp64,
-                "kernel": {1: "fused stage kernel", 3: "fused stage kernel, pair variant", 2: "tile stage kernel", 0: "generic stage kernel"}[plan.path],
+                "kernel": {1: "fused stage kernel", 3: "fused stage kernel, pair variant", 4: "fused stage kernel on 2 x 2 bundles of 8 x 8 blocks", 2: "tile stage kernel", 0: "generic stage kernel"}[plan.path],
                 "kernel_ms_avg": stage_avg_ms, "kernel_launches_timed": stage_launches,
                 "kernel_share_of_step": stage_ms / ms if ms > 0 else None}
 
@@ -434,7 +434,7 @@ def run_ours(args, rank, world, local_rank):
                                    + (", Davis wave speeds" if args.wavespeed else ""),
                        "interior_zones": zones, "state_bytes": plan.bytes_per_state, "block_order": args.order,
                        "layout": f"x guard depth {plan.gd[0]} (row pitch {plan.S_j * 8} B), y/z guard depth {plan.gd[1]}/{plan.gd[2]}",
-                       "path": {0: "generic", 1: "fused (TMA)", 2: "tile (shared-memory block)", 3: "fused (TMA), two zones per thread"}[plan.path], "l2": "inputs (state) larger than L2; no flush needed",
+                       "path": {0: "generic", 1: "fused (TMA)", 2: "tile (shared-memory block)", 3: "fused (TMA), two zones per thread", 4: "fused (TMA), 2 x 2 bundles of 8 x 8 blocks"}[plan.path], "l2": "inputs (state) larger than L2; no flush needed",
                        "multi_gpu": (f"sharded: tiling {cfg.nb[0]}x{cfg.nb[1]}x{cfg.nb[2]} blocks in {world} contiguous Morton runs, "
                                      f"{sh.shard.n_ghost} ghost blocks on rank 0, cut-face slabs exchanged before every stage "
                                      f"(grouped NCCL send/recv, {sh.send_elems * 8} B sent by rank 0 per stage), dt = all-reduce(min)")

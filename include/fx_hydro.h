@@ -51,13 +51,16 @@ enum {
   FX_OPT_P_FLOOR = 1,   /* primitive pressure floor, default 1e-12 [A7] */
   FX_OPT_WENO_EPS = 2,  /* WENO5-JS epsilon, default 1e-6 [A5] */
   FX_OPT_WAVESPEED = 3, /* 0 = Einfeldt (default), 1 = Davis [A8] */
-  FX_OPT_PATH = 4,      /* 0 = auto: the fused TMA stage kernel for 16 x 16 x nz blocks, else the shared-memory tile kernel
+  FX_OPT_PATH = 4,      /* 0 = auto: the fused TMA stage kernel for 16 x 16 x nz blocks and for 8 x 8 x nz blocks whose topology
+                           groups them completely into 2 x 2 bundles of mutual x / y neighbours (regular tilings with even
+                           counts; no wall, gravity or passive scalar), else the shared-memory tile kernel
                            when the padded block fits a CTA's shared memory (8^3 blocks with WENO5, 2-D, 1-D), else
                            the generic zone kernel (also 3-D PLM blocks that would fit: it is the faster one there, measured);
                            1 = generic; 2 = tile kernel where it fits, else generic; 3 = the fused kernel's
                            two-zones-per-thread variant where it applies (PLM, no wall, no gravity; measured slower
                            than the default, kept for comparison), else as 0.
-                           fx_hydro_plan_path reports the choice (1 fused, 3 its pair variant, 2 tile, 0 generic). */
+                           fx_hydro_plan_path reports the choice (1 fused, 4 fused on bundles of 8 x 8 blocks, 3 the pair variant,
+                           2 tile, 0 generic). */
   FX_OPT_ZCHAIN = 5,    /* fused path: longest chain of z-neighbour blocks one CTA marches through, 1..8; 0 (default) =
                            chosen from the number of blocks and of SMs so that the launch still fills the GPU.
                            Set before fx_hydro_plan_set_topology.  Results do not depend on it (bit for bit). */
@@ -278,7 +281,8 @@ int fx_hydro_stage_arrays(fx_hydro_plan *plan, double *U, int stage, double **st
  * 1 fused and TMA-fed (16 x 16 x nz blocks: halos gathered from neighbour interiors inside the stage kernel,
  * every plane moved by TMA), 2 shared-memory tile kernel (one CTA per block whose padded zones fit its shared
  * memory: halos gathered through the neighbour table, each zone converted once, one Riemann solve per face),
- * 3 the fused kernel with two zones per thread (only on request, FX_OPT_PATH = 3). */
+ * 3 the fused kernel with two zones per thread (only on request, FX_OPT_PATH = 3), 4 the fused kernel marching 2 x 2
+ * bundles of 8 x 8 x nz blocks as one 16 x 16 cross-section (csrc/fx_stage_bundle.cu). */
 int fx_hydro_plan_path(const fx_hydro_plan *plan);
 
 /* Measurement aid: when enabled, fx_hydro_advance brackets every stage-kernel launch (the dominant

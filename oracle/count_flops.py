@@ -36,6 +36,7 @@ CASES = [  # name, block dims, tiling, recon, riemann, rk, wavespeed
     ("3d_weno5_hllc_rk3", (16, 16, 16), (2, 2, 2), 1, 1, 3, 0),
     ("3d_plm_hllc_rk2_davis", (16, 16, 16), (2, 2, 2), 0, 1, 2, 1),
     ("3d_plm_hllc_rk2_8cubed", (8, 8, 8), (2, 2, 2), 0, 1, 2, 0),
+    ("3d_weno5_hllc_rk3_8cubed", (8, 8, 8), (2, 2, 2), 1, 1, 3, 0),
     ("2d_plm_hllc_rk2", (16, 16, 1), (4, 4, 1), 0, 1, 2, 0),
     ("2d_weno5_hllc_rk3", (16, 16, 1), (4, 4, 1), 1, 1, 3, 0),
     ("1d_plm_hlle_rk2", (256, 1, 1), (1, 1, 1), 0, 0, 2, 0),

@@ -117,6 +117,7 @@ extern "C" int fx_hydro_plan_create(fx_hydro_plan **out, const int block_dims[3]
 extern "C" int fx_hydro_plan_destroy(fx_hydro_plan *plan) {
   if (plan) delete[] plan->seg_host;
   if (plan) delete[] plan->jump_host;
+  if (plan) delete[] plan->bseg_host;
   if (plan && plan->ev) {
     for (int i = 0; i < 2 * FX_MAX_REC; ++i) cudaEventDestroy(plan->ev[i]);
     delete[] plan->ev;
@@ -202,6 +203,7 @@ extern "C" int fx_hydro_plan_path(const fx_hydro_plan *plan) {
   // passive scalars [B11]: behind the fused kernel by the scalar pass where it applies (PLM, same-level neighbours
   // everywhere, no gravity), else on the generic path
   if (plan->nvars > 5 && !(plan->path_option == 0 && fx_stage_tma_supported(plan->P) && fx_scalar_pass_supported(plan->P))) return 0;
+  if (plan->path_option == 0 && fx_stage_bundle_supported(plan->P)) return 4;  // 8 x 8 blocks in 2 x 2 bundles
   if ((plan->path_option == 0 || plan->path_option == 3) && fx_stage_tma_supported(plan->P))
     return (plan->path_option == 3 && fx_stage_pair_supported(plan->P)) ? 3 : 1;
   // 3-D blocks with PLM: the generic zone kernel, which gathers its halo cells itself, is ahead of the tile kernel
@@ -249,6 +251,15 @@ static int fx_seg_upload(fx_hydro_plan *plan) {
     FX_CUDA(cudaMemcpy(dst, plan->seg_host, (size_t)plan->nseg_host * FX_SEG_STRIDE * sizeof(int), cudaMemcpyHostToDevice));
   plan->P.seg = dst;
   plan->P.nseg = plan->nseg_host;
+  plan->P.bseg = nullptr;
+  plan->P.nbseg = 0;
+  if (plan->bseg_host && plan->nbseg_host > 0) {  // bundle segments take the place of the (unused: blocks are not 16 wide) block segments
+    FX_CUDA(cudaMemcpy(dst, plan->bseg_host, (size_t)plan->nbseg_host * FX_BSEG_STRIDE * sizeof(int), cudaMemcpyHostToDevice));
+    plan->P.bseg = dst;
+    plan->P.nbseg = plan->nbseg_host;
+    plan->P.seg = nullptr;
+    plan->P.nseg = 0;
+  }
   plan->seg_uploaded = true;
   return FX_OK;
 }
@@ -276,6 +287,95 @@ extern "C" int fx_hydro_plan_set_workspace(fx_hydro_plan *plan, void *ws, size_t
                                               fx_seg_bytes(plan) + fx_fjump_bytes(plan))
                                  : nullptr;
   return fx_seg_upload(plan);
+}
+
+// ------------------------------------------------------------------ bundles of 2 x 2 blocks (fx_stage_bundle.cu)
+// Blocks of 8 x 8 x nz zones: group them into bundles {b00, b10, b01, b11} that name each other as x / y neighbours (every
+// link mutual), then chain bundles whose four blocks lie above each other's.  Succeeds only if EVERY owned block finds its
+// bundle (regular tilings with even counts do, in lexicographic and Morton order: the lowest unbundled id sits at even
+// coordinates); otherwise the plan keeps the tile / generic path.  h: host copy of the neighbour table.
+static int fx_build_bundles(fx_hydro_plan *plan, const std::vector<int32_t> &h) {
+  delete[] plan->bseg_host;
+  plan->bseg_host = nullptr;
+  plan->nbseg_host = 0;
+  const FxParams &P = plan->P;
+  const long long nown = P.nown;
+  if (P.n[0] != 8 || P.n[1] != 8 || !P.active[0] || !P.active[1] || !P.active[2] || nown < 4 || nown % 4 != 0 || P.n[2] > 64) return FX_OK;
+  auto nbr = [&](long long b, int f) -> long long { const long long v = h[b * 6 + f]; return (v >= 0 && v < nown) ? v : -1; };
+  std::vector<int> bundle_of((size_t)nown, -1);
+  std::vector<int> ids;  // 4 per bundle
+  for (long long b = 0; b < nown; ++b) {
+    if (bundle_of[b] >= 0) continue;
+    const long long b10 = nbr(b, 1), b01 = nbr(b, 3);
+    if (b10 < 0 || b01 < 0) return FX_OK;
+    const long long b11 = nbr(b10, 3);
+    if (b11 < 0 || nbr(b01, 1) != b11 || nbr(b10, 0) != b || nbr(b01, 2) != b || nbr(b11, 0) != b01 || nbr(b11, 2) != b10) return FX_OK;
+    const long long q[4] = {b, b10, b01, b11};
+    for (int x = 0; x < 4; ++x)
+      for (int y = x + 1; y < 4; ++y)
+        if (q[x] == q[y]) return FX_OK;  // a periodic direction one block wide
+    for (int x = 0; x < 4; ++x) {
+      if (bundle_of[q[x]] >= 0) return FX_OK;
+      bundle_of[q[x]] = (int)(ids.size() / 4);
+    }
+    for (int x = 0; x < 4; ++x) ids.push_back((int)q[x]);
+  }
+  const int nbun = (int)(ids.size() / 4);
+  // the bundle above / below: all four blocks' z links lead, mutually, to the four blocks of one bundle in the same places
+  auto zlink = [&](int B, int f) -> int {
+    int T = -1;
+    for (int x = 0; x < 4; ++x) {
+      const long long t = nbr(ids[4 * B + x], f);
+      if (t < 0 || nbr(t, f ^ 1) != ids[4 * B + x]) return -1;
+      const int tb = bundle_of[t];
+      if (ids[4 * tb + x] != t || (T >= 0 && tb != T) || tb == B) return -1;
+      T = tb;
+    }
+    return T;
+  };
+  int M = plan->zchain > FX_SEG_MAX ? FX_SEG_MAX : plan->zchain;
+  if (M <= 0) {
+    const long long slots = (long long)fx_sm_count() * (P.recon == FX_RECON_WENO5 ? 1 : 2);
+    double best = 0.0;
+    for (int m = 1; m <= FX_SEG_MAX; m *= 2) {
+      const long long nseg = (nbun + m - 1) / m;
+      const double cost = (double)((nseg + slots - 1) / slots) * (m + 0.09);
+      if (M <= 0 || cost < best) {
+        best = cost;
+        M = m;
+      }
+    }
+  }
+  plan->bseg_host = new (std::nothrow) int[(size_t)nbun * FX_BSEG_STRIDE];
+  if (!plan->bseg_host) return fx_fail(FX_ERR_INVALID_ARG, "set_topology: out of host memory");
+  std::vector<char> seen((size_t)nbun, 0);
+  for (int B0 = 0; B0 < nbun; ++B0) {
+    if (seen[B0]) continue;
+    int start = B0;
+    for (int steps = 0; steps < nbun; ++steps) {
+      const int d = zlink(start, 4);
+      if (d < 0 || seen[d] || d == B0) break;
+      start = d;
+    }
+    int B = start;
+    while (B >= 0 && !seen[B]) {
+      int *row = plan->bseg_host + (size_t)plan->nbseg_host * FX_BSEG_STRIDE;
+      for (int x = 0; x < FX_BSEG_STRIDE; ++x) row[x] = FX_BC_OUTFLOW;
+      int cnt = 0, last = B;
+      for (int x = 0; x < 4; ++x) row[1 + x] = h[(long long)ids[4 * B + x] * 6 + 4];  // below: each block's own -z entry
+      while (B >= 0 && !seen[B] && cnt < M) {
+        seen[B] = 1;
+        for (int x = 0; x < 4; ++x) row[1 + 4 * (1 + cnt) + x] = ids[4 * B + x];
+        ++cnt;
+        last = B;
+        B = zlink(B, 5);
+      }
+      row[0] = cnt;
+      for (int x = 0; x < 4; ++x) row[1 + 4 * (1 + cnt) + x] = h[(long long)ids[4 * last + x] * 6 + 5];  // above
+      ++plan->nbseg_host;
+    }
+  }
+  return FX_OK;
 }
 
 // ------------------------------------------------------------------ topology
@@ -365,6 +465,10 @@ extern "C" int fx_hydro_plan_set_topology(fx_hydro_plan *plan, const int32_t *ne
     for (long long b = 0; b < nb; ++b)
       for (int f = 0; f < 6; ++f)
         if (plan->P.active[f / 2] && h[b * 6 + f] == FX_BC_REFLECT) plan->P.walls = 1;
+    {
+      const int rcb = fx_build_bundles(plan, h);  // 8 x 8 blocks: bundles of 2 x 2 for the fused kernel's 16 x 16 cross-section
+      if (rcb) return rcb;
+    }
     std::vector<char> seen((size_t)nb, 0);
     plan->seg_host = new (std::nothrow) int[(size_t)nb * FX_SEG_STRIDE];
     if (!plan->seg_host) return fx_fail(FX_ERR_INVALID_ARG, "set_topology: out of host memory");

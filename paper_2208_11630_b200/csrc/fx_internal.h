@@ -21,6 +21,8 @@ struct FxParams {
   const int *neigh;                 // [nblocks][6], device
   const int *seg;                   // z-chain segments of the fused kernel: [nseg][FX_SEG_STRIDE], device (in the workspace)
   int nseg;
+  const int *bseg;                  // 8 x 8 blocks: segments of 2 x 2 BUNDLES, [nbseg][FX_BSEG_STRIDE] (same place in the workspace)
+  int nbseg;
   int walls;                        // some block has a reflecting wall in an active dimension [B9]
   int grav_on;                      // any component of grav is non-zero [B10]
   double grav[3];
@@ -37,6 +39,9 @@ struct FxParams {
 // of the fused stage kernel marches through a whole segment.  Row: {count, below, id_0 .. id_{count-1}, above}, where
 // below / above are the z neighbours of the first / last block as the neighbour table gives them (id or FX_BC_OUTFLOW).
 enum { FX_SEG_MAX = 8, FX_SEG_STRIDE = 12 };
+// Bundle segments (fx_stage_bundle.cu): {count, 4 x (FX_SEG_MAX + 2) block ids: the layer below (or each block's own boundary
+// code), the count layers of 2 x 2 blocks (x half + 2 y half), the layer above}; at most 11 ints per block: fits the same area
+enum { FX_BSEG_STRIDE = 44 };
 
 // 64-bit words of the scratch block
 enum {
@@ -58,6 +63,8 @@ struct fx_hydro_plan {
   int zchain;           // FX_OPT_ZCHAIN: longest segment (1 .. FX_SEG_MAX)
   int32_t *jump_host;   // host copy of the refinement-jump table (new[]), or nullptr
   int *seg_host;        // segment table built by set_topology (new[]), nseg_host rows
+  int *bseg_host;       // bundle segments (8 x 8 blocks whose topology bundles completely), nbseg_host rows, or nullptr
+  int nbseg_host;
   int nseg_host;
   bool seg_uploaded;
   // optional per-launch timing of the stage kernels (fx_hydro_plan_set_timing)
@@ -93,6 +100,9 @@ int fx_launch_debug_fluxes(const FxParams &P, const double *U, int dir, double *
 int fx_launch_amr_fill(const FxParams &P, double *U, int depth, cudaStream_t st);  // face guard zones behind refinement jumps
 int fx_launch_amr_flux_correct(const FxParams &P, double *out, const double *dx, double dt, const double *dt_dev, double beta,
                                cudaStream_t st);
+bool fx_stage_bundle_supported(const FxParams &P);
+int fx_launch_stage_bundle(const FxParams &P, const double *X, const double *U0, double *out, const double *dx, double dt,
+                           const double *dt_dev, double beta, int first, double cfl_next, double *dt_next, cudaStream_t st);
 bool fx_scalar_pass_supported(const FxParams &P);
 int fx_launch_scalar_pass(const FxParams &P, const double *X, const double *U0, double *out, const double *dx, double dt,
                           const double *dt_dev, double beta, int first, cudaStream_t st);

@@ -45,7 +45,7 @@ static int fx_stage(fx_hydro_plan *plan, double *X, const double *U0, double *ou
                     const double *dt_dev, double beta, int first, cudaStream_t st, double cfl_next = 0.0,
                     double *dt_next = nullptr) {
   const int path = fx_hydro_plan_path(plan);  // 1 fused TMA kernel (3: its pair variant), 2 shared-memory tile kernel, 0 generic
-  const bool fused = path == 1 || path == 3;
+  const bool fused = path == 1 || path == 3 || path == 4;
   int rc = FX_OK;
   if (path == 0 && plan->nvars > 5) {
     // the generic zone kernel reads the hydro variables' halo cells through the neighbour table, like the other two
@@ -66,6 +66,7 @@ static int fx_stage(fx_hydro_plan *plan, double *X, const double *U0, double *ou
   const bool park_dt = fused && plan->nvars > 5 && dt_next != nullptr;
   if (park_dt) dt_next = (double *)&plan->P.scratch[FX_SCR_WORDS - 3];
   rc = fused ? (path == 3 ? fx_launch_stage_pair(plan->P, X, U0, out, dx, dt, dt_dev, beta, first, cfl_next, dt_next, st)
+                : path == 4 ? fx_launch_stage_bundle(plan->P, X, U0, out, dx, dt, dt_dev, beta, first, cfl_next, dt_next, st)
                           : fx_launch_stage_tma(plan->P, X, U0, out, dx, dt, dt_dev, beta, first, cfl_next, dt_next, st))
              : (path == 2 ? fx_launch_stage_tile(plan->P, X, U0, out, dx, dt, dt_dev, beta, first, st)
                           : fx_launch_generic_stage(plan->P, X, U0, out, dx, dt, dt_dev, beta, first, st));

@@ -78,8 +78,8 @@ def run_sharded(cfg, neigh, coords, world, steps, recon, rk, guard_x, path, nvar
 
 
 @pytest.mark.parametrize("number,nb,block,recon,rk,guard_x,world,path", [
-    (5, (2, 2, 4), None, 0, 2, 8, 2, 1), (5, (4, 2, 2), None, 1, 3, 4, 3, 1), (5, (2, 2, 2), (8, 8, 8), 0, 2, 4, 2, 0),
-    (5, (2, 2, 2), (8, 8, 8), 1, 3, 4, 2, 2), (2, (4, 4, 1), None, 0, 2, 4, 3, 2)])
+    (5, (2, 2, 4), None, 0, 2, 8, 2, 1), (5, (4, 2, 2), None, 1, 3, 4, 3, 1), (5, (2, 2, 2), (8, 8, 8), 0, 2, 4, 2, 4),
+    (5, (2, 2, 2), (8, 8, 8), 1, 3, 4, 2, 4), (5, (3, 2, 2), (8, 8, 8), 0, 2, 4, 2, 0), (2, (4, 4, 1), None, 0, 2, 4, 3, 2)])
 def test_sharded_equals_single_plan_bitwise(number, nb, block, recon, rk, guard_x, world, path):
     from paper_2208_11630_b200 import binding as fx
     cfg = inputs.config(number, nb=nb)
