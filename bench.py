@@ -122,7 +122,7 @@ def max_over_ranks(x: float, world: int, device="cpu") -> float:
 
 
 def whole_job_value(zones_per_rank: int, stages: int, steps: int, ms_max: float, world: int) -> float:
-    """Replicas only: every rank advances its own copy of the workload; value = all zone-updates / max time."""
+    """Weak scaling: every rank advances its own share (equal shares of the grown tiling); value = all zone-updates / max time."""
     return world * zones_per_rank * stages * steps / (ms_max * 1e-3)
 
 

@@ -1,6 +1,6 @@
-"""Host-side logic of the N > 1 bench path, run as 2 gloo ranks on the CPU: the path does not shard across
-GPUs in this round ("replicas only"), so what N > 1 adds is the max-over-ranks timing, the
-whole-job aggregation and the reference arm running on rank 0 alone."""
+"""Host-side logic of the N > 1 bench path, run as 2 gloo ranks on the CPU: the max-over-ranks timing, the whole-job
+aggregation and the reference arm running on rank 0 alone.  (The sharding itself -- partition, slab exchange, stage
+protocol -- is covered by tests/test_sharded_host.py with two gloo ranks and by tests/test_gpu_sharded.py.)"""
 import json
 import os
 import socket
