@@ -49,7 +49,10 @@ enum { FX_ORDER_LEX = 0, FX_ORDER_MORTON = 1 };
 enum {
   FX_OPT_RHO_FLOOR = 0, /* primitive density floor, default 1e-12 [A7] */
   FX_OPT_P_FLOOR = 1,   /* primitive pressure floor, default 1e-12 [A7] */
-  FX_OPT_WENO_EPS = 2,  /* WENO5-JS epsilon, default 1e-6 [A5] */
+  FX_OPT_WENO_EPS = 2,  /* WENO5-JS epsilon, default 1e-6 [A5].  Supported magnitudes: the kernels form the WENO5 weights with one
+                           division (products of the smoothness indicators, ~ (difference)^9): differences of a primitive
+                           between neighbouring zones must stay below ~1e33 in the units used, or the products overflow and
+                           the positivity fallback takes the face (the oracle's quotient form only underflows there) */
   FX_OPT_WAVESPEED = 3, /* 0 = Einfeldt (default), 1 = Davis [A8] */
   FX_OPT_PATH = 4,      /* 0 = auto: the fused TMA stage kernel for 16 x 16 x nz blocks and for 8 x 8 x nz blocks whose topology
                            groups them completely into 2 x 2 bundles of mutual x / y neighbours (regular tilings with even
@@ -122,7 +125,10 @@ int fx_hydro_plan_destroy(fx_hydro_plan *plan);
  * placement is correct; only the traffic differs.  The library places its own stage copies that way. */
 int fx_hydro_plan_layout(const fx_hydro_plan *plan, fx_layout *out);
 
-/* Options; must be set before the first advance.  Unknown key / bad value -> FX_ERR_INVALID_ARG. */
+/* Options.  The physics options (floors, WENO epsilon, wave speeds, gravity) travel with every launch and may be changed
+ * between calls; FX_OPT_GUARD_X before the workspace, FX_OPT_OWNED_BLOCKS, FX_OPT_ZCHAIN and FX_OPT_PATH before the topology
+ * (FX_ERR_STATE afterwards).  Unknown key / bad value (a floor or the WENO epsilon <= 0 or non-finite,
+ * wave speeds not 0 / 1, ...) -> FX_ERR_INVALID_ARG. */
 int fx_hydro_plan_set_option(fx_hydro_plan *plan, int key, double value);
 
 /* Workspace (device, caller-owned, 256-byte aligned): a 256-byte scratch block (dt reduction word,

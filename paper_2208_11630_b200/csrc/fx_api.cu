@@ -181,6 +181,7 @@ extern "C" int fx_hydro_plan_set_option(fx_hydro_plan *plan, int key, double val
   }
   case FX_OPT_ZCHAIN:
     if (!(value >= 0.0 && value <= (double)FX_SEG_MAX)) return fx_fail(FX_ERR_INVALID_ARG, "set_option: zchain must be 0 (auto) or 1..%d", (int)FX_SEG_MAX);
+    if (plan->topology_set) return fx_fail(FX_ERR_STATE, "set_option: FX_OPT_ZCHAIN must be set before the topology (the chains are built there)");
     plan->zchain = (int)value;
     return FX_OK;
   case FX_OPT_OWNED_BLOCKS:
@@ -191,6 +192,7 @@ extern "C" int fx_hydro_plan_set_option(fx_hydro_plan *plan, int key, double val
     return FX_OK;
   case FX_OPT_PATH:
     if (value != 0.0 && value != 1.0 && value != 2.0 && value != 3.0) return fx_fail(FX_ERR_INVALID_ARG, "set_option: path must be 0, 1, 2 or 3");
+    if (plan->topology_set) return fx_fail(FX_ERR_STATE, "set_option: FX_OPT_PATH must be set before the topology (the path's tables are built there)");
     plan->path_option = (int)value;
     return FX_OK;
   default: return fx_fail(FX_ERR_INVALID_ARG, "set_option: unknown key %d", key);

@@ -85,6 +85,134 @@ __global__ void __launch_bounds__(128) fx_k_scalar_pass(const FxParams P, const 
   if (hit) fx_note(P, hit);
 }
 
+
+// ------------------------------------------------------------------ the marching form (16 x 16 x nz blocks)
+// One CTA of 256 threads per block marches through the block's planes; thread (i, j) keeps the abundances X of its column's
+// cells k-2 .. k+2 in registers (the z stencils), the plane's X with its two-deep x / y halo (taken from the neighbour
+// blocks' interiors through the table, like every halo of the fused path) goes through shared memory, double-buffered so
+// that one CTA barrier per plane suffices, and everything a zone needs from HBM in a plane -- the new cell of its window,
+// its halo cells if it sits at the block's edge, the faces' (F_rho, Aq), U0 -- is requested at the top of the iteration,
+// all loads in flight together.  Up to NSC = 4 scalars per launch share the densities and the (F_rho, Aq).  Arithmetic:
+// the expressions of fx_k_scalar_pass, in the same order.
+template <int NSC, bool FIRST>
+__global__ void __launch_bounds__(256) fx_k_scalar_march(const FxParams P, const double *__restrict__ X, const double *U0, double *out,
+                                                         const double *__restrict__ dx, double dt, const double *__restrict__ dt_dev,
+                                                         double beta, int sv0) {
+  __shared__ double XS[2][NSC][20][21];
+  const int b = blockIdx.x, tid = threadIdx.x, i = tid & 15, j = tid >> 4;
+  const int nz = P.n[2];
+  const int g0 = P.gd[0], g1 = P.gd[1], g2 = P.gd[2];
+  int nb[6];
+#pragma unroll
+  for (int f = 0; f < 6; ++f) nb[f] = __ldg(&P.neigh[(long long)b * 6 + f]);
+  if (dt_dev) dt = *dt_dev;
+  const double rd0 = dt / __ldg(&dx[b * 3 + 0]), rd1 = dt / __ldg(&dx[b * 3 + 1]), rd2 = dt / __ldg(&dx[b * 3 + 2]);
+  const long long colo = (long long)(j + g1) * P.S_j + (i + g0);  // this column inside a block's plane
+  const long long nzt = P.nblocks * (long long)nz * 256;
+  const double *Q0 = X + (long long)sv0 * P.S_v;
+  // abundances of the zone at padded offset e: (rho X_s) / max(rho, floor), the reciprocal as the hydro part forms it
+  auto abund = [&](long long e, double x[NSC]) {
+    double rho = X[e];
+    double q[NSC];
+#pragma unroll
+    for (int s = 0; s < NSC; ++s) q[s] = Q0[s * P.S_v + e];
+    if (rho < P.rho_floor) rho = P.rho_floor;
+    const double ri = fx_rcp3(rho);
+#pragma unroll
+    for (int s = 0; s < NSC; ++s) x[s] = q[s] * ri;
+  };
+  auto plane_off = [&](int k) -> long long {  // this column's zone in plane k of the column (k in [-2, nz + 2))
+    const int blk = k < 0 ? nb[4] : (k >= nz ? nb[5] : b);
+    const int kk = k < 0 ? k + nz : (k >= nz ? k - nz : k);
+    return (long long)blk * P.S_b + (long long)(kk + g2) * P.S_k + colo;
+  };
+  double xz[5][NSC];  // X of cells k-2 .. k+2 of this column
+#pragma unroll
+  for (int m = 0; m < 4; ++m) abund(plane_off(m - 2), xz[m]);
+  // the halo cell this thread also provides for each plane (threads in the two outermost columns / rows): where it comes
+  // from inside the neighbour block's plane, and where it goes in the shared plane
+  const bool hx = i < 2 || i >= 14, hy = j < 2 || j >= 14;
+  const int nbx = i < 2 ? nb[0] : nb[1], nby = j < 2 ? nb[2] : nb[3];
+  const long long hxo = (long long)(j + g1) * P.S_j + ((i < 2 ? 14 + i : i - 14) + g0);
+  const long long hyo = (long long)((j < 2 ? 14 + j : j - 14) + g1) * P.S_j + (i + g0);
+  const int hxc = i < 2 ? i : i + 4, hyr = j < 2 ? j : j + 4;
+  unsigned hit = 0;
+#pragma unroll 1
+  for (int k = 0; k < nz; ++k) {
+    const int buf = k & 1;
+    const long long zi = ((long long)b * nz + k) * 256 + tid;
+    // ---- everything from HBM for this plane
+    abund(plane_off(k + 2), xz[4]);
+    double xh[NSC], yh[NSC];
+    if (hx) abund((long long)nbx * P.S_b + (long long)(k + g2) * P.S_k + hxo, xh);
+    if (hy) abund((long long)nby * P.S_b + (long long)(k + g2) * P.S_k + hyo, yh);
+    double F[3][2], A[3][2];
+    {
+      const long long zh[3] = {i < 15 ? zi + 1 : ((long long)nb[1] * nz + k) * 256 + j * 16,
+                               j < 15 ? zi + 16 : ((long long)nb[3] * nz + k) * 256 + i,
+                               k + 1 < nz ? zi + 256 : ((long long)nb[5] * nz) * 256 + tid};
+#pragma unroll
+      for (int d = 0; d < 3; ++d) {
+        const double *fq = P.fq + 2 * d * nzt;
+        F[d][0] = fq[zi];
+        A[d][0] = fq[nzt + zi];
+        F[d][1] = fq[zh[d]];
+        A[d][1] = fq[nzt + zh[d]];
+      }
+    }
+    const long long c = (long long)b * P.S_b + (long long)(k + g2) * P.S_k + colo;
+    double u0[NSC], xs[NSC];
+#pragma unroll
+    for (int s = 0; s < NSC; ++s) {
+      u0[s] = U0[(long long)(sv0 + s) * P.S_v + c];
+      if (!FIRST) xs[s] = Q0[s * P.S_v + c];
+    }
+    // ---- the plane's abundances with their halo into shared memory
+#pragma unroll
+    for (int s = 0; s < NSC; ++s) {
+      XS[buf][s][j + 2][i + 2] = xz[2][s];
+      if (hx) XS[buf][s][j + 2][hxc] = xh[s];
+      if (hy) XS[buf][s][hyr][i + 2] = yh[s];
+    }
+    __syncthreads();
+    auto flux = [&](const double x[5], double rd, const double Fd[2], const double Ad[2]) {
+      double am[3], ap[3];
+#pragma unroll
+      for (int n = 0; n < 3; ++n) fx_plm(x[n], x[n + 1], x[n + 2], am[n], ap[n]);
+      const double Fm = Ad[0] * ap[0] + (Fd[0] - Ad[0]) * am[1];
+      const double Fp = Ad[1] * ap[1] + (Fd[1] - Ad[1]) * am[2];
+      if (!(fabs(Fm + Fp) <= 1.79e308)) hit |= FX_STATUS_NONFINITE;
+      return rd * (Fp - Fm);
+    };
+#pragma unroll
+    for (int s = 0; s < NSC; ++s) {
+      double x[5], Ss = 0.0;
+#pragma unroll
+      for (int m = 0; m < 5; ++m) x[m] = XS[buf][s][j + 2][i + m];
+      Ss += flux(x, rd0, F[0], A[0]);
+#pragma unroll
+      for (int m = 0; m < 5; ++m) x[m] = XS[buf][s][j + m][i + 2];
+      Ss += flux(x, rd1, F[1], A[1]);
+#pragma unroll
+      for (int m = 0; m < 5; ++m) x[m] = xz[m][s];
+      Ss += flux(x, rd2, F[2], A[2]);
+      out[(long long)(sv0 + s) * P.S_v + c] = FIRST ? (u0[s] - Ss) : (u0[s] + beta * ((xs[s] - u0[s]) - Ss));
+    }
+#pragma unroll
+    for (int m = 0; m < 4; ++m)
+#pragma unroll
+      for (int s = 0; s < NSC; ++s) xz[m][s] = xz[m + 1][s];
+  }
+  if (hit) fx_note(P, hit);
+}
+
+template <int NSC>
+static void fx_scalar_march_launch(const FxParams &P, const double *X, const double *U0, double *out, const double *dx, double dt,
+                                   const double *dt_dev, double beta, int first, int sv0, cudaStream_t st) {
+  if (first) fx_k_scalar_march<NSC, true><<<(unsigned)P.nown, 256, 0, st>>>(P, X, U0, out, dx, dt, dt_dev, beta, sv0);
+  else fx_k_scalar_march<NSC, false><<<(unsigned)P.nown, 256, 0, st>>>(P, X, U0, out, dx, dt, dt_dev, beta, sv0);
+}
+
 }  // namespace
 
 bool fx_scalar_pass_supported(const FxParams &P) {
@@ -96,6 +224,17 @@ int fx_launch_scalar_pass(const FxParams &P, const double *X, const double *U0, 
                           const double *dt_dev, double beta, int first, cudaStream_t st) {
   const long long nzones = P.nown * P.n[0] * P.n[1] * P.n[2];
   if (nzones == 0 || P.nvars <= 5) return FX_OK;
+  if (P.n[0] == 16 && P.n[1] == 16 && P.n[2] >= 2) {  // the marching form, up to four scalars per launch
+    for (int sv = 5; sv < P.nvars; sv += 4) {
+      const int n = P.nvars - sv < 4 ? P.nvars - sv : 4;
+      if (n == 4) fx_scalar_march_launch<4>(P, X, U0, out, dx, dt, dt_dev, beta, first, sv, st);
+      else if (n == 3) fx_scalar_march_launch<3>(P, X, U0, out, dx, dt, dt_dev, beta, first, sv, st);
+      else if (n == 2) fx_scalar_march_launch<2>(P, X, U0, out, dx, dt, dt_dev, beta, first, sv, st);
+      else fx_scalar_march_launch<1>(P, X, U0, out, dx, dt, dt_dev, beta, first, sv, st);
+      FX_LAUNCH_CHECK("scalar_march");
+    }
+    return FX_OK;
+  }
   const unsigned grid = (unsigned)((nzones + 127) / 128);
   if (first) fx_k_scalar_pass<true><<<grid, 128, 0, st>>>(P, X, U0, out, dx, dt, dt_dev, beta, nzones);
   else fx_k_scalar_pass<false><<<grid, 128, 0, st>>>(P, X, U0, out, dx, dt, dt_dev, beta, nzones);

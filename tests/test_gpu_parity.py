@@ -231,6 +231,32 @@ def test_pair_variant_of_the_fused_kernel(kw):
     assert wall.path == 1
 
 
+@pytest.mark.parametrize("path", [None, 1])
+def test_weno5_parity_in_cgs_like_units(path):
+    """Large magnitudes: density x 1e7, pressure x 1e25 (velocities then ~ 1e9) -- inside the documented range of the
+    kernels' single-division WENO5 weights (include/fx_hydro.h, FX_OPT_WENO_EPS): same tolerances, no fallback, no flag."""
+    cfg = inputs.config(4, nb=(2, 2, 2))
+    oplan, neigh, coords = oracle_plan_for(cfg)
+    gplan, _, _ = gpu_plan_for(cfg, path=path)
+    Ui = inputs.block_interiors(cfg, coords).numpy().copy()
+    sr, sp = 1e7, 1e25
+    sv = np.sqrt(sp / sr)
+    Ui[0] *= sr
+    Ui[1:4] *= sr * sv
+    Ui[4] *= sp
+    Uh = inputs.embed(cfg, torch.from_numpy(Ui))
+    dx = inputs.dx_array(cfg)
+    Uo, Ud, dxd = Uh.numpy().copy(), Uh.cuda(), torch.from_numpy(dx).cuda()
+    for step in range(3):
+        dt = oplan.compute_dt(Uo, dx, cfg.cfl)
+        dtg = float(gplan.fx_hydro_compute_dt(Ud, dxd, cfg.cfl).item())
+        assert abs(dtg - dt) <= TOL_DT * dt
+        oplan.advance(Uo, dx, dt)
+        gplan.fx_hydro_advance(Ud, dxd, dt)
+    assert rel_err(cfg, gplan.interior(Ud).cpu().numpy(), oplan.interior(Uo)) <= 1e-11
+    assert oplan.status()[0] == 0 and gplan.fx_hydro_status()[0] == 0
+
+
 def test_device_dt_path_equals_host_dt_path():
     cfg, oplan, gplan, Uh, dx = setup(5, (2, 2, 2))
     dxd = torch.from_numpy(dx).cuda()
@@ -449,6 +475,10 @@ def test_x_guard_depth_8_layout(recon, rk, bc, path):
     assert gplan.path == (1 if path is None else 0)
     with pytest.raises(fx.FxError):
         gplan.fx_hydro_plan_set_option(fx.OPT_GUARD_X, 4)
+    for key in (fx.OPT_PATH, fx.OPT_ZCHAIN, fx.OPT_OWNED_BLOCKS):  # what the topology call builds its tables from
+        with pytest.raises(fx.FxError):
+            gplan.fx_hydro_plan_set_option(key, 1)
+    gplan.fx_hydro_plan_set_option(fx.OPT_WAVESPEED, 0)  # a physics option may still change
     rng = np.random.default_rng(41)
     shape = (8, 16, 16, 16)
     rho = 1.0 + 0.3 * rng.random(shape)
