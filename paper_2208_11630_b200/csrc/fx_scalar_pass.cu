@@ -95,7 +95,7 @@ __global__ void __launch_bounds__(128) fx_k_scalar_pass(const FxParams P, const 
 // all loads in flight together.  Up to NSC = 4 scalars per launch share the densities and the (F_rho, Aq).  Arithmetic:
 // the expressions of fx_k_scalar_pass, in the same order.
 template <int NSC, bool FIRST>
-__global__ void __launch_bounds__(256) fx_k_scalar_march(const FxParams P, const double *__restrict__ X, const double *U0, double *out,
+__global__ void __launch_bounds__(256, 2) fx_k_scalar_march(const FxParams P, const double *__restrict__ X, const double *U0, double *out,
                                                          const double *__restrict__ dx, double dt, const double *__restrict__ dt_dev,
                                                          double beta, int sv0) {
   __shared__ double XS[2][NSC][20][21];
@@ -126,40 +126,56 @@ __global__ void __launch_bounds__(256) fx_k_scalar_march(const FxParams P, const
     const int kk = k < 0 ? k + nz : (k >= nz ? k - nz : k);
     return (long long)blk * P.S_b + (long long)(kk + g2) * P.S_k + colo;
   };
-  double xz[5][NSC];  // X of cells k-2 .. k+2 of this column
+  // z direction, carried from plane to plane: X of cells k and k+1, the plus value of cell k, and the scalar flux through
+  // the low z face of cell k (the high face's of the plane before: one evaluation per face)
+  double xw[2][NSC], apc[NSC], Fz[NSC];
+  {
+    double xm2[NSC], xm1[NSC], am, ap;
+    abund(plane_off(-2), xm2);
+    abund(plane_off(-1), xm1);
+    abund(plane_off(0), xw[0]);
+    abund(plane_off(1), xw[1]);
+    const long long z0 = (long long)b * nz * 256 + tid;
+    const double Fl = P.fq[4 * nzt + z0], Al = P.fq[5 * nzt + z0];
 #pragma unroll
-  for (int m = 0; m < 4; ++m) abund(plane_off(m - 2), xz[m]);
+    for (int s = 0; s < NSC; ++s) {
+      double apm;
+      fx_plm(xm2[s], xm1[s], xw[0][s], am, apm);
+      fx_plm(xm1[s], xw[0][s], xw[1][s], am, ap);
+      apc[s] = ap;
+      Fz[s] = Al * apm + (Fl - Al) * am;
+    }
+  }
   // the halo cell this thread also provides for each plane (threads in the two outermost columns / rows): where it comes
   // from inside the neighbour block's plane, and where it goes in the shared plane
   const bool hx = i < 2 || i >= 14, hy = j < 2 || j >= 14;
   const int nbx = i < 2 ? nb[0] : nb[1], nby = j < 2 ? nb[2] : nb[3];
-  const long long hxo = (long long)(j + g1) * P.S_j + ((i < 2 ? 14 + i : i - 14) + g0);
-  const long long hyo = (long long)((j < 2 ? 14 + j : j - 14) + g1) * P.S_j + (i + g0);
+  const long long hxo = (long long)nbx * P.S_b + (long long)(j + g1) * P.S_j + ((i < 2 ? 14 + i : i - 14) + g0);
+  const long long hyo = (long long)nby * P.S_b + (long long)((j < 2 ? 14 + j : j - 14) + g1) * P.S_j + (i + g0);
   const int hxc = i < 2 ? i : i + 4, hyr = j < 2 ? j : j + 4;
+  const long long zxh = i < 15 ? (long long)b * nz * 256 + tid + 1 : (long long)nb[1] * nz * 256 + j * 16;
+  const long long zyh = j < 15 ? (long long)b * nz * 256 + tid + 16 : (long long)nb[3] * nz * 256 + i;
   unsigned hit = 0;
 #pragma unroll 1
   for (int k = 0; k < nz; ++k) {
     const int buf = k & 1;
     const long long zi = ((long long)b * nz + k) * 256 + tid;
     // ---- everything from HBM for this plane
-    abund(plane_off(k + 2), xz[4]);
-    double xh[NSC], yh[NSC];
-    if (hx) abund((long long)nbx * P.S_b + (long long)(k + g2) * P.S_k + hxo, xh);
-    if (hy) abund((long long)nby * P.S_b + (long long)(k + g2) * P.S_k + hyo, yh);
-    double F[3][2], A[3][2];
-    {
-      const long long zh[3] = {i < 15 ? zi + 1 : ((long long)nb[1] * nz + k) * 256 + j * 16,
-                               j < 15 ? zi + 16 : ((long long)nb[3] * nz + k) * 256 + i,
-                               k + 1 < nz ? zi + 256 : ((long long)nb[5] * nz) * 256 + tid};
-#pragma unroll
-      for (int d = 0; d < 3; ++d) {
-        const double *fq = P.fq + 2 * d * nzt;
-        F[d][0] = fq[zi];
-        A[d][0] = fq[nzt + zi];
-        F[d][1] = fq[zh[d]];
-        A[d][1] = fq[nzt + zh[d]];
-      }
-    }
+    double xn[NSC], xh[NSC], yh[NSC];
+    abund(plane_off(k + 2), xn);
+    if (hx) abund((long long)(k + g2) * P.S_k + hxo, xh);
+    if (hy) abund((long long)(k + g2) * P.S_k + hyo, yh);
+    double F[2][2], A[2][2];
+    F[0][0] = P.fq[zi];
+    A[0][0] = P.fq[nzt + zi];
+    F[0][1] = P.fq[zxh + (long long)k * 256];
+    A[0][1] = P.fq[nzt + zxh + (long long)k * 256];
+    F[1][0] = P.fq[2 * nzt + zi];
+    A[1][0] = P.fq[3 * nzt + zi];
+    F[1][1] = P.fq[2 * nzt + zyh + (long long)k * 256];
+    A[1][1] = P.fq[3 * nzt + zyh + (long long)k * 256];
+    const long long zzh = k + 1 < nz ? zi + 256 : (long long)nb[5] * nz * 256 + tid;
+    const double Fzh = P.fq[4 * nzt + zzh], Azh = P.fq[5 * nzt + zzh];
     const long long c = (long long)b * P.S_b + (long long)(k + g2) * P.S_k + colo;
     double u0[NSC], xs[NSC];
 #pragma unroll
@@ -170,7 +186,7 @@ __global__ void __launch_bounds__(256) fx_k_scalar_march(const FxParams P, const
     // ---- the plane's abundances with their halo into shared memory
 #pragma unroll
     for (int s = 0; s < NSC; ++s) {
-      XS[buf][s][j + 2][i + 2] = xz[2][s];
+      XS[buf][s][j + 2][i + 2] = xw[0][s];
       if (hx) XS[buf][s][j + 2][hxc] = xh[s];
       if (hy) XS[buf][s][hyr][i + 2] = yh[s];
     }
@@ -193,15 +209,19 @@ __global__ void __launch_bounds__(256) fx_k_scalar_march(const FxParams P, const
 #pragma unroll
       for (int m = 0; m < 5; ++m) x[m] = XS[buf][s][j + m][i + 2];
       Ss += flux(x, rd1, F[1], A[1]);
-#pragma unroll
-      for (int m = 0; m < 5; ++m) x[m] = xz[m][s];
-      Ss += flux(x, rd2, F[2], A[2]);
+      {  // z: the new face only
+        double amn, apn;
+        fx_plm(xw[0][s], xw[1][s], xn[s], amn, apn);
+        const double Fp = Azh * apc[s] + (Fzh - Azh) * amn;
+        if (!(fabs(Fz[s] + Fp) <= 1.79e308)) hit |= FX_STATUS_NONFINITE;
+        Ss += rd2 * (Fp - Fz[s]);
+        Fz[s] = Fp;
+        apc[s] = apn;
+        xw[0][s] = xw[1][s];
+        xw[1][s] = xn[s];
+      }
       out[(long long)(sv0 + s) * P.S_v + c] = FIRST ? (u0[s] - Ss) : (u0[s] + beta * ((xs[s] - u0[s]) - Ss));
     }
-#pragma unroll
-    for (int m = 0; m < 4; ++m)
-#pragma unroll
-      for (int s = 0; s < NSC; ++s) xz[m][s] = xz[m + 1][s];
   }
   if (hit) fx_note(P, hit);
 }
