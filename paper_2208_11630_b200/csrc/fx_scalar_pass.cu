@@ -87,56 +87,122 @@ __global__ void __launch_bounds__(128) fx_k_scalar_pass(const FxParams P, const 
 
 
 // ------------------------------------------------------------------ the marching form (16 x 16 x nz blocks)
-// One CTA of 256 threads per block marches through the block's planes; thread (i, j) keeps the abundances X of its column's
-// cells k-2 .. k+2 in registers (the z stencils), the plane's X with its two-deep x / y halo (taken from the neighbour
-// blocks' interiors through the table, like every halo of the fused path) goes through shared memory, double-buffered so
-// that one CTA barrier per plane suffices, and everything a zone needs from HBM in a plane -- the new cell of its window,
-// its halo cells if it sits at the block's edge, the faces' (F_rho, Aq), U0 -- is requested at the top of the iteration,
-// all loads in flight together.  Up to NSC = 4 scalars per launch share the densities and the (F_rho, Aq).  Arithmetic:
-// the expressions of fx_k_scalar_pass, in the same order.
+// One CTA of 256 threads per block marches through the block's planes; thread (i, j) carries its column's z stencil in
+// registers (X of cells k and k+1, the plus value of cell k, the flux through the low z face: one evaluation per z face),
+// the plane's X with its two-deep x / y halo (taken from the neighbour blocks' interiors through the table, like every halo
+// of the fused path) goes through shared memory, double-buffered so that one CTA barrier per plane suffices.  What a plane
+// needs from HBM before that barrier -- the new cell of each window (rho, rho X_s), the halo cells' (rho, rho X_s), the
+// faces' (F_rho, Aq) of the x and y directions -- is fetched one plane ahead with cp.async into a two-stage buffer (each
+// thread reads back what it fetched itself, except the high faces' (F_rho, Aq), which are the next zone's low-face values:
+// read from the neighbour's slot after the barrier instead of a second time from memory); U0, the stage input and the z
+// face's (F_rho, Aq) are plain loads issued right after the barrier and consumed at the end of the plane.  Up to NSC = 4
+// scalars per launch share the densities and the (F_rho, Aq).  Arithmetic: the expressions of fx_k_scalar_pass.
+// (Measured, config 5 with 4 scalars, this pass alone: 10.8 ms with every load at the top of the plane and 184 registers
+// (one CTA per SM); 7.4 ms with the z carry and 128 registers (two CTAs); the cp.async form below: see profiles/README.md.)
+template <int NSC>
+struct ScalSmem {
+  double XS[2][NSC][20][20];      // abundances of the plane with halo
+  double raw[2][1 + NSC][256];    // (rho, rho X_s) of the window's new cell, per thread
+  double hal[2][1 + NSC][128];    // (rho, rho X_s) of the halo cells: 64 x-halo cells, 64 y-halo cells
+  double fx[2][2][16][17];        // (F_rho, Aq) of the low x faces of zones i = 0 .. 16 (16: the x+ neighbour's first zone)
+  double fy[2][2][17][16];        // the same along y
+};
+
+__device__ __forceinline__ void cp_async8(void *dst, const void *src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((unsigned)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
 template <int NSC, bool FIRST>
 __global__ void __launch_bounds__(256, 2) fx_k_scalar_march(const FxParams P, const double *__restrict__ X, const double *U0, double *out,
-                                                         const double *__restrict__ dx, double dt, const double *__restrict__ dt_dev,
-                                                         double beta, int sv0) {
-  __shared__ double XS[2][NSC][20][21];
+                                                            const double *__restrict__ dx, double dt, const double *__restrict__ dt_dev,
+                                                            double beta, int sv0) {
+  extern __shared__ __align__(16) unsigned char fx_scal_smem[];
+  ScalSmem<NSC> &S = *reinterpret_cast<ScalSmem<NSC> *>(fx_scal_smem);
   const int b = blockIdx.x, tid = threadIdx.x, i = tid & 15, j = tid >> 4;
   const int nz = P.n[2];
   const int g0 = P.gd[0], g1 = P.gd[1], g2 = P.gd[2];
   int nb[6];
 #pragma unroll
   for (int f = 0; f < 6; ++f) nb[f] = __ldg(&P.neigh[(long long)b * 6 + f]);
-  if (dt_dev) dt = *dt_dev;
-  const double rd0 = dt / __ldg(&dx[b * 3 + 0]), rd1 = dt / __ldg(&dx[b * 3 + 1]), rd2 = dt / __ldg(&dx[b * 3 + 2]);
   const long long colo = (long long)(j + g1) * P.S_j + (i + g0);  // this column inside a block's plane
   const long long nzt = P.nblocks * (long long)nz * 256;
   const double *Q0 = X + (long long)sv0 * P.S_v;
-  // abundances of the zone at padded offset e: (rho X_s) / max(rho, floor), the reciprocal as the hydro part forms it
-  auto abund = [&](long long e, double x[NSC]) {
-    double rho = X[e];
-    double q[NSC];
-#pragma unroll
-    for (int s = 0; s < NSC; ++s) q[s] = Q0[s * P.S_v + e];
-    if (rho < P.rho_floor) rho = P.rho_floor;
-    const double ri = fx_rcp3(rho);
-#pragma unroll
-    for (int s = 0; s < NSC; ++s) x[s] = q[s] * ri;
-  };
   auto plane_off = [&](int k) -> long long {  // this column's zone in plane k of the column (k in [-2, nz + 2))
     const int blk = k < 0 ? nb[4] : (k >= nz ? nb[5] : b);
     const int kk = k < 0 ? k + nz : (k >= nz ? k - nz : k);
     return (long long)blk * P.S_b + (long long)(kk + g2) * P.S_k + colo;
   };
+  // the halo cell this thread also provides for each plane (threads in the two outermost columns / rows): where it comes
+  // from inside the neighbour block's plane, its slot in the staging buffer, and where it goes in the shared plane
+  const bool hx = i < 2 || i >= 14, hy = j < 2 || j >= 14;
+  const long long hxo = (long long)(i < 2 ? nb[0] : nb[1]) * P.S_b + (long long)(j + g1) * P.S_j + ((i < 2 ? 14 + i : i - 14) + g0);
+  const long long hyo = (long long)(j < 2 ? nb[2] : nb[3]) * P.S_b + (long long)((j < 2 ? 14 + j : j - 14) + g1) * P.S_j + (i + g0);
+  const int hxs = j * 4 + (i < 2 ? i : i - 12), hys = 64 + (j < 2 ? j : j - 12) * 16 + i;
+  const int hxc = i < 2 ? i : i + 4, hyr = j < 2 ? j : j + 4;
+  const long long zb = (long long)b * nz * 256 + tid;
+  const long long zxh = (long long)nb[1] * nz * 256 + j * 16, zyh = (long long)nb[3] * nz * 256 + i;
+  // everything plane k needs before its barrier, into stage k & 1
+  auto prefetch = [&](int k) {
+    const int st = k & 1;
+    const long long e = plane_off(k + 2);
+    cp_async8(&S.raw[st][0][tid], X + e);
+#pragma unroll
+    for (int s = 0; s < NSC; ++s) cp_async8(&S.raw[st][1 + s][tid], Q0 + s * P.S_v + e);
+    const long long ko = (long long)(k + g2) * P.S_k;
+    if (hx) {
+      cp_async8(&S.hal[st][0][hxs], X + ko + hxo);
+#pragma unroll
+      for (int s = 0; s < NSC; ++s) cp_async8(&S.hal[st][1 + s][hxs], Q0 + s * P.S_v + ko + hxo);
+    }
+    if (hy) {
+      cp_async8(&S.hal[st][0][hys], X + ko + hyo);
+#pragma unroll
+      for (int s = 0; s < NSC; ++s) cp_async8(&S.hal[st][1 + s][hys], Q0 + s * P.S_v + ko + hyo);
+    }
+    const long long zi = zb + (long long)k * 256;
+    cp_async8(&S.fx[st][0][j][i], P.fq + zi);
+    cp_async8(&S.fx[st][1][j][i], P.fq + nzt + zi);
+    cp_async8(&S.fy[st][0][j][i], P.fq + 2 * nzt + zi);
+    cp_async8(&S.fy[st][1][j][i], P.fq + 3 * nzt + zi);
+    if (i == 15) {
+      cp_async8(&S.fx[st][0][j][16], P.fq + zxh + (long long)k * 256);
+      cp_async8(&S.fx[st][1][j][16], P.fq + nzt + zxh + (long long)k * 256);
+    }
+    if (j == 15) {
+      cp_async8(&S.fy[st][0][16][i], P.fq + 2 * nzt + zyh + (long long)k * 256);
+      cp_async8(&S.fy[st][1][16][i], P.fq + 3 * nzt + zyh + (long long)k * 256);
+    }
+    cp_async_commit();
+  };
+  prefetch(0);
+  if (dt_dev) dt = *dt_dev;
+  const double rd0 = dt / __ldg(&dx[b * 3 + 0]), rd1 = dt / __ldg(&dx[b * 3 + 1]), rd2 = dt / __ldg(&dx[b * 3 + 2]);
+  // abundances: (rho X_s) / max(rho, floor), the reciprocal as the hydro part forms it
+  auto abund = [&](double rho, const double q[NSC], double x[NSC]) {
+    if (rho < P.rho_floor) rho = P.rho_floor;
+    const double ri = fx_rcp3(rho);
+#pragma unroll
+    for (int s = 0; s < NSC; ++s) x[s] = q[s] * ri;
+  };
+  auto abund_at = [&](long long e, double x[NSC]) {
+    const double rho = X[e];
+    double q[NSC];
+#pragma unroll
+    for (int s = 0; s < NSC; ++s) q[s] = Q0[s * P.S_v + e];
+    abund(rho, q, x);
+  };
   // z direction, carried from plane to plane: X of cells k and k+1, the plus value of cell k, and the scalar flux through
-  // the low z face of cell k (the high face's of the plane before: one evaluation per face)
+  // the low z face of cell k (the high face's of the plane before)
   double xw[2][NSC], apc[NSC], Fz[NSC];
   {
     double xm2[NSC], xm1[NSC], am, ap;
-    abund(plane_off(-2), xm2);
-    abund(plane_off(-1), xm1);
-    abund(plane_off(0), xw[0]);
-    abund(plane_off(1), xw[1]);
-    const long long z0 = (long long)b * nz * 256 + tid;
-    const double Fl = P.fq[4 * nzt + z0], Al = P.fq[5 * nzt + z0];
+    abund_at(plane_off(-2), xm2);
+    abund_at(plane_off(-1), xm1);
+    abund_at(plane_off(0), xw[0]);
+    abund_at(plane_off(1), xw[1]);
+    const double Fl = P.fq[4 * nzt + zb], Al = P.fq[5 * nzt + zb];
 #pragma unroll
     for (int s = 0; s < NSC; ++s) {
       double apm;
@@ -146,34 +212,39 @@ __global__ void __launch_bounds__(256, 2) fx_k_scalar_march(const FxParams P, co
       Fz[s] = Al * apm + (Fl - Al) * am;
     }
   }
-  // the halo cell this thread also provides for each plane (threads in the two outermost columns / rows): where it comes
-  // from inside the neighbour block's plane, and where it goes in the shared plane
-  const bool hx = i < 2 || i >= 14, hy = j < 2 || j >= 14;
-  const int nbx = i < 2 ? nb[0] : nb[1], nby = j < 2 ? nb[2] : nb[3];
-  const long long hxo = (long long)nbx * P.S_b + (long long)(j + g1) * P.S_j + ((i < 2 ? 14 + i : i - 14) + g0);
-  const long long hyo = (long long)nby * P.S_b + (long long)((j < 2 ? 14 + j : j - 14) + g1) * P.S_j + (i + g0);
-  const int hxc = i < 2 ? i : i + 4, hyr = j < 2 ? j : j + 4;
-  const long long zxh = i < 15 ? (long long)b * nz * 256 + tid + 1 : (long long)nb[1] * nz * 256 + j * 16;
-  const long long zyh = j < 15 ? (long long)b * nz * 256 + tid + 16 : (long long)nb[3] * nz * 256 + i;
   unsigned hit = 0;
 #pragma unroll 1
   for (int k = 0; k < nz; ++k) {
     const int buf = k & 1;
-    const long long zi = ((long long)b * nz + k) * 256 + tid;
-    // ---- everything from HBM for this plane
-    double xn[NSC], xh[NSC], yh[NSC];
-    abund(plane_off(k + 2), xn);
-    if (hx) abund((long long)(k + g2) * P.S_k + hxo, xh);
-    if (hy) abund((long long)(k + g2) * P.S_k + hyo, yh);
-    double F[2][2], A[2][2];
-    F[0][0] = P.fq[zi];
-    A[0][0] = P.fq[nzt + zi];
-    F[0][1] = P.fq[zxh + (long long)k * 256];
-    A[0][1] = P.fq[nzt + zxh + (long long)k * 256];
-    F[1][0] = P.fq[2 * nzt + zi];
-    A[1][0] = P.fq[3 * nzt + zi];
-    F[1][1] = P.fq[2 * nzt + zyh + (long long)k * 256];
-    A[1][1] = P.fq[3 * nzt + zyh + (long long)k * 256];
+    cp_async_wait_all();  // this thread's part of stage k
+    double xn[NSC];
+    {
+      double q[NSC];
+#pragma unroll
+      for (int s = 0; s < NSC; ++s) q[s] = S.raw[buf][1 + s][tid];
+      abund(S.raw[buf][0][tid], q, xn);
+    }
+#pragma unroll
+    for (int s = 0; s < NSC; ++s) S.XS[buf][s][j + 2][i + 2] = xw[0][s];
+    if (hx) {
+      double q[NSC], xh[NSC];
+#pragma unroll
+      for (int s = 0; s < NSC; ++s) q[s] = S.hal[buf][1 + s][hxs];
+      abund(S.hal[buf][0][hxs], q, xh);
+#pragma unroll
+      for (int s = 0; s < NSC; ++s) S.XS[buf][s][j + 2][hxc] = xh[s];
+    }
+    if (hy) {
+      double q[NSC], yh[NSC];
+#pragma unroll
+      for (int s = 0; s < NSC; ++s) q[s] = S.hal[buf][1 + s][hys];
+      abund(S.hal[buf][0][hys], q, yh);
+#pragma unroll
+      for (int s = 0; s < NSC; ++s) S.XS[buf][s][hyr][i + 2] = yh[s];
+    }
+    __syncthreads();  // plane k's X and (F_rho, Aq) complete; every thread is done with plane k-1 (stage buf ^ 1)
+    if (k + 1 < nz) prefetch(k + 1);
+    const long long zi = zb + (long long)k * 256;
     const long long zzh = k + 1 < nz ? zi + 256 : (long long)nb[5] * nz * 256 + tid;
     const double Fzh = P.fq[4 * nzt + zzh], Azh = P.fq[5 * nzt + zzh];
     const long long c = (long long)b * P.S_b + (long long)(k + g2) * P.S_k + colo;
@@ -183,14 +254,8 @@ __global__ void __launch_bounds__(256, 2) fx_k_scalar_march(const FxParams P, co
       u0[s] = U0[(long long)(sv0 + s) * P.S_v + c];
       if (!FIRST) xs[s] = Q0[s * P.S_v + c];
     }
-    // ---- the plane's abundances with their halo into shared memory
-#pragma unroll
-    for (int s = 0; s < NSC; ++s) {
-      XS[buf][s][j + 2][i + 2] = xw[0][s];
-      if (hx) XS[buf][s][j + 2][hxc] = xh[s];
-      if (hy) XS[buf][s][hyr][i + 2] = yh[s];
-    }
-    __syncthreads();
+    const double F0[2] = {S.fx[buf][0][j][i], S.fx[buf][0][j][i + 1]}, A0[2] = {S.fx[buf][1][j][i], S.fx[buf][1][j][i + 1]};
+    const double F1[2] = {S.fy[buf][0][j][i], S.fy[buf][0][j + 1][i]}, A1[2] = {S.fy[buf][1][j][i], S.fy[buf][1][j + 1][i]};
     auto flux = [&](const double x[5], double rd, const double Fd[2], const double Ad[2]) {
       double am[3], ap[3];
 #pragma unroll
@@ -204,11 +269,11 @@ __global__ void __launch_bounds__(256, 2) fx_k_scalar_march(const FxParams P, co
     for (int s = 0; s < NSC; ++s) {
       double x[5], Ss = 0.0;
 #pragma unroll
-      for (int m = 0; m < 5; ++m) x[m] = XS[buf][s][j + 2][i + m];
-      Ss += flux(x, rd0, F[0], A[0]);
+      for (int m = 0; m < 5; ++m) x[m] = S.XS[buf][s][j + 2][i + m];
+      Ss += flux(x, rd0, F0, A0);
 #pragma unroll
-      for (int m = 0; m < 5; ++m) x[m] = XS[buf][s][j + m][i + 2];
-      Ss += flux(x, rd1, F[1], A[1]);
+      for (int m = 0; m < 5; ++m) x[m] = S.XS[buf][s][j + m][i + 2];
+      Ss += flux(x, rd1, F1, A1);
       {  // z: the new face only
         double amn, apn;
         fx_plm(xw[0][s], xw[1][s], xn[s], amn, apn);
@@ -227,10 +292,15 @@ __global__ void __launch_bounds__(256, 2) fx_k_scalar_march(const FxParams P, co
 }
 
 template <int NSC>
-static void fx_scalar_march_launch(const FxParams &P, const double *X, const double *U0, double *out, const double *dx, double dt,
-                                   const double *dt_dev, double beta, int first, int sv0, cudaStream_t st) {
-  if (first) fx_k_scalar_march<NSC, true><<<(unsigned)P.nown, 256, 0, st>>>(P, X, U0, out, dx, dt, dt_dev, beta, sv0);
-  else fx_k_scalar_march<NSC, false><<<(unsigned)P.nown, 256, 0, st>>>(P, X, U0, out, dx, dt, dt_dev, beta, sv0);
+static int fx_scalar_march_launch(const FxParams &P, const double *X, const double *U0, double *out, const double *dx, double dt,
+                                  const double *dt_dev, double beta, int first, int sv0, cudaStream_t st) {
+  const int smem = (int)sizeof(ScalSmem<NSC>);
+  if (first) FX_CUDA(cudaFuncSetAttribute(fx_k_scalar_march<NSC, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+  else FX_CUDA(cudaFuncSetAttribute(fx_k_scalar_march<NSC, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+  if (first) fx_k_scalar_march<NSC, true><<<(unsigned)P.nown, 256, smem, st>>>(P, X, U0, out, dx, dt, dt_dev, beta, sv0);
+  else fx_k_scalar_march<NSC, false><<<(unsigned)P.nown, 256, smem, st>>>(P, X, U0, out, dx, dt, dt_dev, beta, sv0);
+  FX_LAUNCH_CHECK("scalar_march");
+  return FX_OK;
 }
 
 }  // namespace
@@ -247,11 +317,12 @@ int fx_launch_scalar_pass(const FxParams &P, const double *X, const double *U0, 
   if (P.n[0] == 16 && P.n[1] == 16 && P.n[2] >= 2) {  // the marching form, up to four scalars per launch
     for (int sv = 5; sv < P.nvars; sv += 4) {
       const int n = P.nvars - sv < 4 ? P.nvars - sv : 4;
-      if (n == 4) fx_scalar_march_launch<4>(P, X, U0, out, dx, dt, dt_dev, beta, first, sv, st);
-      else if (n == 3) fx_scalar_march_launch<3>(P, X, U0, out, dx, dt, dt_dev, beta, first, sv, st);
-      else if (n == 2) fx_scalar_march_launch<2>(P, X, U0, out, dx, dt, dt_dev, beta, first, sv, st);
-      else fx_scalar_march_launch<1>(P, X, U0, out, dx, dt, dt_dev, beta, first, sv, st);
-      FX_LAUNCH_CHECK("scalar_march");
+      int rc;
+      if (n == 4) rc = fx_scalar_march_launch<4>(P, X, U0, out, dx, dt, dt_dev, beta, first, sv, st);
+      else if (n == 3) rc = fx_scalar_march_launch<3>(P, X, U0, out, dx, dt, dt_dev, beta, first, sv, st);
+      else if (n == 2) rc = fx_scalar_march_launch<2>(P, X, U0, out, dx, dt, dt_dev, beta, first, sv, st);
+      else rc = fx_scalar_march_launch<1>(P, X, U0, out, dx, dt, dt_dev, beta, first, sv, st);
+      if (rc) return rc;
     }
     return FX_OK;
   }
