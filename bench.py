@@ -279,6 +279,28 @@ def run_reference(args, rank, world):
 
 
 # ------------------------------------------------------------------ roofline inputs (files only; nothing under oracle/ runs here)
+def aux_calls(plan, U, dx, cfg, zones, reps=5):
+    """fx_hydro_compute_dt and fx_fill_guardcells, each alone: average of `reps` launches between CUDA events on the
+    stream they are launched on (the state is larger than L2 at the bench sizes, so no flush), GB/s of algorithmic bytes."""
+    import torch
+    out = {}
+    dt_tmp = torch.empty(1, dtype=torch.float64, device=U.device)
+    guard_zones = plan.nblocks * (plan.np[0] * plan.np[1] * plan.np[2] - cfg.block_dims[0] * cfg.block_dims[1] * cfg.block_dims[2])
+    for name, call, nbytes in (("fx_hydro_compute_dt", lambda: plan.fx_hydro_compute_dt(U, dx, cfg.cfl, dt_tmp), 40.0 * zones),
+                               ("fx_fill_guardcells", lambda: plan.fx_fill_guardcells(U), 16.0 * plan.nvars * guard_zones)):
+        call()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(reps):
+            call()
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / reps
+        out[name] = {"ms": ms, "alg_bytes": nbytes, "GB/s": nbytes / (ms * 1e-3) / 1e9, "launches_timed": reps}
+    return out
+
+
 def algorithmic_flops(cfg, args):
     """Exact fp64 operations per zone and RK stage of this scheme from oracle/flop_counts.json, or None."""
     try:
@@ -441,6 +463,15 @@ def run_ours(args, rank, world, local_rank):
                        if sh is not None else "single"},
             "clocks": clocks, "gpu_launches": launches_per_step * args.steps, "roofline": roofline,
             "status_flags": flags}
+
+    # the two calls of the boundary that are not part of the fused step, each timed alone [SURVEY 8(d)]: the CFL reduction
+    # a7 (reads the 5 hydro variables of the interior zones once: 40 B per zone) and the standalone guard fill a1 (reads one
+    # interior zone and writes one guard zone per guard zone and variable: 16 B per guard zone and variable)
+    if sh is None and rank == 0:
+        try:
+            line["aux"] = aux_calls(plan, U, dx, cfg, zones)
+        except Exception as ex:
+            line["aux"] = {"error": repr(ex)[:200]}
 
     # end to end through the C ABI with HOST buffers (H2D + steps + D2H inside the timed region)
     if not args.no_e2e and sh is not None:
