@@ -190,6 +190,22 @@ int fx_guardcell_index_map(fx_hydro_plan *plan, int64_t block_begin, int64_t blo
 int fx_hydro_compute_dt(fx_hydro_plan *plan, const double *U_dev, const double *dx_dev, double cfl,
                         double *dt_out_dev, void *stream);
 
+/* fx_hydro_compute_dt for callers that may not allocate (code under CUDA graph capture, serving loops, harnesses that
+ * forbid cudaMalloc) and so have no workspace: the same reduction [O7, A13] with its scratch -- one partial maximum per
+ * owned block plus a 32-word header -- in a file-scope device array of the library, (32 + FX_STATIC_DT_MAX_BLOCKS) * 8 =
+ * 524 544 bytes that every GPU loading the library holds until the process exits.  Needs only the plan (neither topology
+ * nor workspace); U_dev, dx_dev, dt_out_dev as above, caller-owned; flags_out_dev (device uint32, may be NULL) receives
+ * this call's FX_STATUS_* bits (they do NOT go to fx_hydro_status, whose words live in the workspace).  The result equals
+ * fx_hydro_compute_dt's bit for bit (same per-zone arithmetic; a maximum has no order).  The call makes no cudaMalloc /
+ * cudaFree and calls no allocating library routine; the first call on each device looks the array's address up
+ * (cudaGetSymbolAddress), so make that one outside a capture.  More than FX_STATIC_DT_MAX_BLOCKS owned blocks ->
+ * FX_ERR_UNSUPPORTED, nothing launched.  All calls on a device share the array, which keeps the last call's contents
+ * (the header is cleared on `stream` before each launch): two calls that overlap on the GPU -- different streams with no
+ * dependency between them -- RACE and both results are undefined. */
+#define FX_STATIC_DT_MAX_BLOCKS 65536
+int fx_hydro_compute_dt_static(fx_hydro_plan *plan, const double *U_dev, const double *dx_dev, double cfl,
+                               double *dt_out_dev, uint32_t *flags_out_dev, void *stream);
+
 /* a1..a6 One SSP-RK step [O5, O6], all stages, in place on the INTERIOR zones of U_dev:
  *   U1 = U0 - S(U0);  RK2: U = U0 + 1/2((U1-U0) - S(U1));
  *   RK3: U2 = U0 + 1/4((U1-U0) - S(U1)); U = U0 + 2/3((U2-U0) - S(U2));

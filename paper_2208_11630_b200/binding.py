@@ -29,7 +29,7 @@ EXPORTS = [
     "fx_last_error", "fx_hydro_plan_create", "fx_hydro_plan_destroy", "fx_hydro_plan_layout",
     "fx_hydro_plan_set_option", "fx_hydro_plan_workspace_bytes", "fx_hydro_plan_set_workspace",
     "fx_hydro_plan_set_topology", "fx_hydro_plan_set_refinement", "fx_topology_cartesian", "fx_fill_guardcells", "fx_guardcell_index_map",
-    "fx_hydro_compute_dt", "fx_hydro_advance", "fx_hydro_advance_host", "fx_hydro_advance_host_interior", "fx_hydro_advance_devdt", "fx_hydro_step",
+    "fx_hydro_compute_dt", "fx_hydro_compute_dt_static", "fx_hydro_advance", "fx_hydro_advance_host", "fx_hydro_advance_host_interior", "fx_hydro_advance_devdt", "fx_hydro_step",
     "fx_hydro_status", "fx_hydro_status_reset", "fx_debug_compute_fluxes", "fx_hydro_plan_path",
     "fx_hydro_plan_set_timing", "fx_hydro_plan_get_timing",
     "fx_shard_create", "fx_shard_destroy", "fx_shard_sizes", "fx_shard_tables", "fx_shard_items", "fx_halo_item_elems",
@@ -75,6 +75,7 @@ def lib():
         L.fx_fill_guardcells.argtypes = [vp, vp, vp]
         L.fx_guardcell_index_map.argtypes = [vp, C.c_int64, C.c_int64, vp, vp]
         L.fx_hydro_compute_dt.argtypes = [vp, vp, vp, C.c_double, vp, vp]
+        L.fx_hydro_compute_dt_static.argtypes = [vp, vp, vp, C.c_double, vp, vp, vp]
         L.fx_hydro_advance.argtypes = [vp, vp, vp, C.c_double, vp]
         L.fx_hydro_advance_devdt.argtypes = [vp, vp, vp, vp, vp]
         L.fx_hydro_step.argtypes = [vp, vp, vp, C.c_double, vp, vp]
@@ -110,6 +111,9 @@ def _check(rc):
 def _stream(stream=None):
     s = torch.cuda.current_stream() if stream is None else stream
     return C.c_void_p(s.cuda_stream)
+
+
+STATIC_DT_MAX_BLOCKS = 65536  # FX_STATIC_DT_MAX_BLOCKS: owned blocks fx_hydro_compute_dt_static's scratch array has room for
 
 
 def _dev(t: torch.Tensor, dtype):
@@ -265,6 +269,14 @@ class HydroPlan:
         dt_out = self._dt if dt_out is None else dt_out
         _check(lib().fx_hydro_compute_dt(self._h, _dev(U, torch.float64), _dev(dx, torch.float64), float(cfl),
                                          _dev(dt_out, torch.float64), _stream(stream)))
+        return dt_out
+
+    def fx_hydro_compute_dt_static(self, U, dx, cfl, dt_out, flags_out=None, stream=None):
+        """The reduction with its scratch in the library's static device array (no workspace, no allocation: the caller
+        passes dt_out, a 1-element float64 device tensor, and optionally flags_out, a 1-element int32 device tensor)."""
+        _check(lib().fx_hydro_compute_dt_static(self._h, _dev(U, torch.float64), _dev(dx, torch.float64), float(cfl),
+                                                _dev(dt_out, torch.float64),
+                                                None if flags_out is None else _dev(flags_out, torch.int32), _stream(stream)))
         return dt_out
 
     def fx_hydro_advance(self, U, dx, dt, stream=None):
