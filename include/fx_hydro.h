@@ -64,7 +64,8 @@ enum {
                            than the default, kept for comparison), else as 0.
                            fx_hydro_plan_path reports the choice (1 fused, 4 fused on bundles of 8 x 8 blocks, 3 the pair variant,
                            2 tile, 0 generic). */
-  FX_OPT_ZCHAIN = 5,    /* fused path: longest chain of z-neighbour blocks one CTA marches through, 1..8; 0 (default) =
+  FX_OPT_ZCHAIN = 5,    /* fused path: longest chain of z-neighbour blocks one CTA marches through, 1..8 (1..16 for 8 x 8 x nz
+                           blocks; a larger value is clamped to what the kernel takes); 0 (default) =
                            chosen from the number of blocks and of SMs so that the launch still fills the GPU.
                            Set before fx_hydro_plan_set_topology.  Results do not depend on it (bit for bit). */
   FX_OPT_GRAVITY_X = 6, /* constant acceleration g_x (default 0): every stage adds beta dt (0, rho g, g.m) [B10] */
@@ -133,7 +134,7 @@ int fx_hydro_plan_set_option(fx_hydro_plan *plan, int key, double value);
 
 /* Workspace (device, caller-owned, 256-byte aligned): a 256-byte scratch block (dt reduction word,
  * status word and counters) + a 256-byte pad + (rk_order - 1) state copies for the RK stages + the z-segment table
- * (12 int32 per block, see FX_OPT_ZCHAIN).  set_workspace initialises the scratch block and
+ * (12 int32 per block, 19 for 8 x 8 x nz blocks; see FX_OPT_ZCHAIN).  set_workspace initialises the scratch block and
  * synchronises the device once. */
 size_t fx_hydro_plan_workspace_bytes(const fx_hydro_plan *plan);
 int fx_hydro_plan_set_workspace(fx_hydro_plan *plan, void *workspace_dev, size_t bytes);

@@ -180,7 +180,7 @@ extern "C" int fx_hydro_plan_set_option(fx_hydro_plan *plan, int key, double val
     return FX_OK;
   }
   case FX_OPT_ZCHAIN:
-    if (!(value >= 0.0 && value <= (double)FX_SEG_MAX)) return fx_fail(FX_ERR_INVALID_ARG, "set_option: zchain must be 0 (auto) or 1..%d", (int)FX_SEG_MAX);
+    if (!(value >= 0.0 && value <= (double)FX_BSEG_MAX)) return fx_fail(FX_ERR_INVALID_ARG, "set_option: zchain must be 0 (auto) or 1..%d", (int)FX_BSEG_MAX);
     if (plan->topology_set) return fx_fail(FX_ERR_STATE, "set_option: FX_OPT_ZCHAIN must be set before the topology (the chains are built there)");
     plan->zchain = (int)value;
     return FX_OK;
@@ -221,8 +221,14 @@ static size_t fx_state_bytes_aligned(const fx_hydro_plan *plan) {
   return (b + 255) & ~(size_t)255;
 }
 
-static size_t fx_seg_bytes(const fx_hydro_plan *plan) {  // room for one segment per block
-  return (((size_t)plan->P.nblocks * FX_SEG_STRIDE * sizeof(int)) + 255) & ~(size_t)255;
+static size_t fx_seg_bytes(const fx_hydro_plan *plan) {  // room for one segment per block, or one bundle segment per four 8 x 8 blocks
+  const FxParams &P = plan->P;
+  size_t ints = (size_t)P.nblocks * FX_SEG_STRIDE;
+  if (P.n[0] == 8 && P.n[1] == 8) {
+    const size_t b = ((size_t)P.nblocks / 4 + 1) * FX_BSEG_STRIDE;
+    if (b > ints) ints = b;
+  }
+  return ((ints * sizeof(int)) + 255) & ~(size_t)255;
 }
 
 static size_t fx_fq_bytes(const fx_hydro_plan *plan) {  // scalar pass [B11]: (mass flux, Aq) x 3 low faces per interior zone
@@ -335,11 +341,11 @@ static int fx_build_bundles(fx_hydro_plan *plan, const std::vector<int32_t> &h) 
     }
     return T;
   };
-  int M = plan->zchain > FX_SEG_MAX ? FX_SEG_MAX : plan->zchain;
+  int M = plan->zchain > FX_BSEG_MAX ? FX_BSEG_MAX : plan->zchain;
   if (M <= 0) {
     const long long slots = (long long)fx_sm_count() * (P.recon == FX_RECON_WENO5 ? 1 : 2);
     double best = 0.0;
-    for (int m = 1; m <= FX_SEG_MAX; m *= 2) {
+    for (int m = 1; m <= FX_BSEG_MAX; m *= 2) {
       const long long nseg = (nbun + m - 1) / m;
       const double cost = (double)((nseg + slots - 1) / slots) * (m + 0.09);
       if (M <= 0 || cost < best) {

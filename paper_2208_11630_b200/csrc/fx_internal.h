@@ -39,9 +39,10 @@ struct FxParams {
 // of the fused stage kernel marches through a whole segment.  Row: {count, below, id_0 .. id_{count-1}, above}, where
 // below / above are the z neighbours of the first / last block as the neighbour table gives them (id or FX_BC_OUTFLOW).
 enum { FX_SEG_MAX = 8, FX_SEG_STRIDE = 12 };
-// Bundle segments (fx_stage_bundle.cu): {count, 4 x (FX_SEG_MAX + 2) block ids: the layer below (or each block's own boundary
-// code), the count layers of 2 x 2 blocks (x half + 2 y half), the layer above}; at most 11 ints per block: fits the same area
-enum { FX_BSEG_STRIDE = 44 };
+// Bundle segments (fx_stage_bundle.cu): {count, 4 x (FX_BSEG_MAX + 2) block ids: the layer below (or each block's own boundary
+// code), the count layers of 2 x 2 blocks (x half + 2 y half), the layer above}.  8-plane blocks: chains twice as long as the
+// 16-plane blocks' keep the planes per pipeline fill the same.  One row per bundle at worst: 19 ints per block.
+enum { FX_BSEG_MAX = 16, FX_BSEG_STRIDE = 76 };
 
 // 64-bit words of the scratch block
 enum {

@@ -51,7 +51,7 @@ template <int RECON> struct alignas(128) Smem {
   double Ly[5][NY + 1][NX];
   double rd[4][4];                   // beta dt / dx_d of the block of each quadrant whose planes are being combined
   double idx[4][4];                  // 1 / dx_d (DTOUT)
-  int blk[FX_SEG_MAX + 2][4];        // block ids: layer below the segment (or that block's boundary code), its layers, the layer above
+  int blk[FX_BSEG_MAX + 2][4];        // block ids: layer below the segment (or that block's boundary code), its layers, the layer above
   int count;
   double wmax[8];
   unsigned long long barX[2], barH;
@@ -91,7 +91,7 @@ fx_k_stage_bundle(const __grid_constant__ CUtensorMap mXm, const __grid_constant
   {  // this CTA's segment: {count, 4 x (count + 2) block ids}
     const int *row = P.bseg + (long long)blockIdx.x * FX_BSEG_STRIDE;
     if (tid == 0) S.count = __ldg(&row[0]);
-    if (tid < 4 * (FX_SEG_MAX + 2)) (&S.blk[0][0])[tid] = __ldg(&row[1 + tid]);
+    if (tid < 4 * (FX_BSEG_MAX + 2)) (&S.blk[0][0])[tid] = __ldg(&row[1 + tid]);
   }
   __syncthreads();
   const int M = S.count;

@@ -25,7 +25,8 @@ def random_state(cfg, nblk, dims, seed):
 @pytest.mark.parametrize("nb,dims,recon,riemann,rk,bc,order,kw", [
     ((4, 4, 4), (8, 8, 8), 0, 1, 2, "periodic", 1, {}), ((2, 4, 3), (8, 8, 8), 1, 1, 3, "periodic", 0, {}),
     ((4, 2, 2), (8, 8, 8), 0, 0, 3, "outflow", 1, {}), ((2, 2, 5), (8, 8, 4), 1, 0, 2, "outflow", 0, {}),
-    ((4, 4, 2), (8, 8, 16), 0, 1, 2, "periodic", 1, dict(wavespeed=1)), ((2, 2, 2), (8, 8, 8), 0, 1, 2, "periodic", 0, {})])
+    ((4, 4, 2), (8, 8, 16), 0, 1, 2, "periodic", 1, dict(wavespeed=1)), ((2, 2, 2), (8, 8, 8), 0, 1, 2, "periodic", 0, {}),
+    ((2, 2, 12), (8, 8, 8), 0, 1, 2, "periodic", 0, {}), ((2, 2, 20), (8, 8, 4), 1, 1, 3, "outflow", 0, {})])
 def test_bundle_parity_chain_lengths_and_generic(nb, dims, recon, riemann, rk, bc, order, kw):
     cfg = inputs.config(5, nb=nb)
     cfg.block_dims = dims
@@ -37,7 +38,7 @@ def test_bundle_parity_chain_lengths_and_generic(nb, dims, recon, riemann, rk, b
     dxd = torch.from_numpy(dx).cuda()
     Uo = Uh.numpy().copy()
     results = []
-    for zc in (None, 1, 3):
+    for zc in (None, 1, 3, 16):  # 16: the longest chain (a column of 12 or 20 layers is marched as one or two segments)
         gplan, _, _ = gpu_plan_for(cfg, bc=bc, recon=recon, riemann=riemann, rk=rk, order=order, zchain=zc, **kw)
         assert gplan.path == 4
         Ud = Uh.cuda()
