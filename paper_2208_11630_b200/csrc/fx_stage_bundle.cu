@@ -49,13 +49,16 @@ template <int RECON> struct alignas(128) Smem {
   double P[5][NP][NP + 1];           // primitives of the plane incl. halo rows / columns
   double Lx[5][NY][NX + 1];
   double Ly[5][NY + 1][NX];
-  double rd[4][4];                   // beta dt / dx_d of the block of each quadrant whose planes are being combined
-  double idx[4][4];                  // 1 / dx_d (DTOUT)
-  int blk[FX_BSEG_MAX + 2][4];        // block ids: layer below the segment (or that block's boundary code), its layers, the layer above
-  int count;
-  double wmax[8];
+  double rd[4][3];                   // beta dt / dx_d of the block of each quadrant whose planes are being combined
+  double idx[4][3];                  // 1 / dx_d (DTOUT)
+  unsigned long long rmax;           // DTOUT: bit pattern of the CTA's maximum of (|u_d| + c) / dx_d
   unsigned long long barX[2], barH;
+  // 115 584 bytes with PLM, the size of fx_stage_tma.cu's: two CTAs per SM (2 x (115 584 + 1024) <= 233 472).  The segment's
+  // block ids stay in global memory (BLK below: read once per plane by one lane, once per layer by a few): with them, the
+  // per-warp maxima and 4-wide rd / idx rows in here the struct was 512 bytes larger and ONE CTA fitted (ncu:
+  // launch__occupancy_limit_shared_mem = 1, 15.8 G zone-updates/s at 8^3).
 };
+static_assert(sizeof(Smem<FX_RECON_PLM_MINMOD>) <= 115712, "PLM: two CTAs per SM need <= 115 712 bytes each");
 
 __device__ __forceinline__ void cta_sync() { asm volatile("bar.sync 0, %0;" ::"n"(NTHREADS) : "memory"); }
 
@@ -88,22 +91,21 @@ fx_k_stage_bundle(const __grid_constant__ CUtensorMap mXm, const __grid_constant
   const int nzb = P.n[2];
   const int g0 = P.gd[0], g1 = P.gd[1], g2 = P.gd[2];
   unsigned hit = 0;
-  {  // this CTA's segment: {count, 4 x (count + 2) block ids}
-    const int *row = P.bseg + (long long)blockIdx.x * FX_BSEG_STRIDE;
-    if (tid == 0) S.count = __ldg(&row[0]);
-    if (tid < 4 * (FX_BSEG_MAX + 2)) (&S.blk[0][0])[tid] = __ldg(&row[1 + tid]);
-  }
+  if (tid == 0) S.rmax = 0ull;
+  // this CTA's segment: {count, 4 x (count + 2) block ids}; block ids of the segment: layer l (0: the layer below, or each block's own boundary code; 1 .. M: its layers; M + 1: above)
+  const int *brow = P.bseg + (long long)blockIdx.x * FX_BSEG_STRIDE + 1;
+#define BLK(l, q) __ldg(&brow[4 * (l) + (q)])
   __syncthreads();
-  const int M = S.count;
+  const int M = __ldg(&brow[-1]);
   const int nz = M * nzb;
   const unsigned zmagic = ((1u << 20) + (unsigned)nzb - 1u) / (unsigned)nzb;
   // where plane Z of quadrant q's column lives: block id and padded k (outflow below / above: clamp [O1])
   auto zmap = [&](int Z, int q, int &bs, int &kp) {
     int qb = Z < 0 ? -1 : (M == 1 ? (int)(Z >= nzb) : (int)(((unsigned)Z * zmagic) >> 20));
     int k = Z - qb * nzb;
-    int id = S.blk[1 + qb][q];
+    int id = BLK(1 + qb, q);
     if (id < 0) {
-      if (qb < 0) { id = S.blk[1][q]; k = 0; } else { id = S.blk[M][q]; k = nzb - 1; }
+      if (qb < 0) { id = BLK(1, q); k = 0; } else { id = BLK(M, q); k = nzb - 1; }
     }
     bs = id;
     kp = k + g2;
@@ -127,10 +129,10 @@ fx_k_stage_bundle(const __grid_constant__ CUtensorMap mXm, const __grid_constant
   auto halo_block = [&]() {
 #pragma unroll
     for (int h = 0; h < 2; ++h) {
-      hbx[0][h] = S.blk[1 + hq][2 * h];      // x-lo side, y half h: quadrant (0, h)
-      hbx[1][h] = S.blk[1 + hq][2 * h + 1];  // x-hi side: quadrant (1, h)
-      hby[0][h] = S.blk[1 + hq][h];          // y-lo side, x half h: quadrant (h, 0)
-      hby[1][h] = S.blk[1 + hq][2 + h];      // y-hi side: quadrant (h, 1)
+      hbx[0][h] = BLK(1 + hq, 2 * h);      // x-lo side, y half h: quadrant (0, h)
+      hbx[1][h] = BLK(1 + hq, 2 * h + 1);  // x-hi side: quadrant (1, h)
+      hby[0][h] = BLK(1 + hq, h);          // y-lo side, x half h: quadrant (h, 0)
+      hby[1][h] = BLK(1 + hq, 2 + h);      // y-hi side: quadrant (h, 1)
       xlo[h] = __ldg(&P.neigh[(long long)hbx[0][h] * 6 + 0]);
       xhi[h] = __ldg(&P.neigh[(long long)hbx[1][h] * 6 + 1]);
       ylo[h] = __ldg(&P.neigh[(long long)hby[0][h] * 6 + 2]);
@@ -152,7 +154,7 @@ fx_k_stage_bundle(const __grid_constant__ CUtensorMap mXm, const __grid_constant
   auto issue_U0 = [&](int p, int layer, int k) {  // plane p of the column = plane k of the layer-th layer
     mbar_expect_tx(&S.barX[(p + 1) & 1], PLANE_BYTES);
 #pragma unroll
-    for (int q = 0; q < 4; ++q) tma_load(&S.U0[p & 1][q][0][0][0], &mU0, &S.barX[(p + 1) & 1], g0, g1, k + g2, S.blk[1 + layer][q]);
+    for (int q = 0; q < 4; ++q) tma_load(&S.U0[p & 1][q][0][0][0], &mU0, &S.barX[(p + 1) & 1], g0, g1, k + g2, BLK(1 + layer, q));
   };
   if (producer) {
     mbar_init(&S.barX[0], FIRST ? 1 : 2); mbar_init(&S.barX[1], FIRST ? 1 : 2);
@@ -310,7 +312,7 @@ fx_k_stage_bundle(const __grid_constant__ CUtensorMap mXm, const __grid_constant
     if (DTOUT) {
 #pragma unroll
       for (int o = 16; o > 0; o >>= 1) rate = fmax(rate, __shfl_xor_sync(0xffffffffu, rate, o));
-      if ((tid & 31) == 0) S.wmax[tid >> 5] = rate;
+      if ((tid & 31) == 0) atomicMax(&S.rmax, (unsigned long long)__double_as_longlong(rate));  // non-negative doubles order like their bits
     }
     cta_sync();  // D
   } else if (tid < NZONE_THREADS + 32) {
@@ -367,7 +369,7 @@ fx_k_stage_bundle(const __grid_constant__ CUtensorMap mXm, const __grid_constant
       if (pk == 0 && lane < 12) {
         // a layer's first plane: the combines of the layer below ended before barrier B, this tick's start after C
         const int qq = lane / 3, d = lane - 3 * qq;
-        const double dxd = __ldg(&dx[(long long)S.blk[1 + pq][qq] * 3 + d]);
+        const double dxd = __ldg(&dx[(long long)BLK(1 + pq, qq) * 3 + d]);
         S.rd[qq][d] = (FIRST ? 1.0 : beta) * dt / dxd;
         if (DTOUT) S.idx[qq][d] = 1.0 / dxd;
       }
@@ -440,7 +442,7 @@ fx_k_stage_bundle(const __grid_constant__ CUtensorMap mXm, const __grid_constant
         if (p >= 1) {
           const int layer = pk >= 1 ? pq : pq - 1, k = (pk >= 1 ? pk - 1 : nzb - 1) + g2;
 #pragma unroll
-          for (int q = 0; q < 4; ++q) tma_store(&mOut, &S.Out[q][0][0][0], g0, g1, k, S.blk[1 + layer][q]);
+          for (int q = 0; q < 4; ++q) tma_store(&mOut, &S.Out[q][0][0][0], g0, g1, k, BLK(1 + layer, q));
           tma_commit();
         }
         if (!FIRST && p + 1 < nz) {
@@ -459,13 +461,10 @@ fx_k_stage_bundle(const __grid_constant__ CUtensorMap mXm, const __grid_constant
     cta_sync();  // D
     if (lane == 0) {
 #pragma unroll
-      for (int q = 0; q < 4; ++q) tma_store(&mOut, &S.Out[q][0][0][0], g0, g1, nzb - 1 + g2, S.blk[M][q]);
+      for (int q = 0; q < 4; ++q) tma_store(&mOut, &S.Out[q][0][0][0], g0, g1, nzb - 1 + g2, BLK(M, q));
       tma_commit();
       if (DTOUT) {
-        double mx = S.wmax[0];
-#pragma unroll
-        for (int w8 = 1; w8 < 8; ++w8) mx = fmax(mx, S.wmax[w8]);
-        atomicMax(&P.scratch[FX_SCR_DTBITS], (unsigned long long)__double_as_longlong(mx));
+        atomicMax(&P.scratch[FX_SCR_DTBITS], S.rmax);
         __threadfence();
         const unsigned long long done = atomicAdd(&P.scratch[FX_SCR_COUNTER], 1ull);
         if (done == gridDim.x - 1) {
