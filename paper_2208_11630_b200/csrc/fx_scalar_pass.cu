@@ -2,7 +2,7 @@
 //
 // A scalar's flux at a face is Aq X_L + (F_rho - Aq) X_R [B11], where the mass flux F_rho and the coefficient Aq come out of
 // the hydro Riemann solve of that face.  The fused kernel (fx_stage_tma.cu, SCAL) leaves both for the three low faces of
-// every zone in P.fq; this kernel, one thread per zone, does what is left for each scalar: X = (rho X) / rho on the 2R+1
+// every zone in P.fq (HLLC: F_rho alone -- there Aq = max(F_rho, 0), the flux being upwind in the sign of S*); this kernel, one thread per zone, does what is left for each scalar: X = (rho X) / rho on the 2R+1
 // cells of each direction's stencil (the reciprocal densities are formed once and serve all scalars), PLM face values of
 // cells -1, 0, +1, the two face fluxes per direction (the high face's F_rho and Aq are the next zone's low-face values,
 // through the neighbour table at a block face), divergence and RK combination.  Expressions and their order are those of
@@ -31,11 +31,12 @@ __device__ __forceinline__ void fx_sp_direction(const FxParams &P, const double 
     ri[m] = fx_rcp3(rho);
   }
   const double *fq = P.fq + 2 * D * nzt;
+  const bool hllc = P.riemann == FX_RIEMANN_HLLC;  // Aq = max(F_rho, 0): not stored
   Flo = fq[zi];
-  Alo = fq[nzt + zi];
+  Alo = hllc ? (Flo > 0.0 ? Flo : 0.0) : fq[nzt + zi];
   const long long zh = idx + 1 < n ? zi + sz : zi - (long long)(n - 1) * sz + (long long)(nhi - b) * per_block;
   Fhi = fq[zh];
-  Ahi = fq[nzt + zh];
+  Ahi = hllc ? (Fhi > 0.0 ? Fhi : 0.0) : fq[nzt + zh];
 }
 
 template <bool FIRST>
@@ -114,7 +115,11 @@ __device__ __forceinline__ void cp_async8(void *dst, const void *src) {
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
-template <int NSC, bool FIRST>
+// HLLC: Aq is F_rho where F_rho > 0 and 0 elsewhere (the flux is upwind in the sign of S*, which is the sign of the mass flux), so
+// the fused kernel leaves F_rho alone for it and this pass reads half the face data.
+__device__ __forceinline__ double fx_aq_hllc(double F) { return F > 0.0 ? F : 0.0; }
+
+template <int NSC, bool FIRST, bool HLLC>
 __global__ void __launch_bounds__(256, 2) fx_k_scalar_march(const FxParams P, const double *__restrict__ X, const double *U0, double *out,
                                                             const double *__restrict__ dx, double dt, const double *__restrict__ dt_dev,
                                                             double beta, int sv0) {
@@ -163,16 +168,16 @@ __global__ void __launch_bounds__(256, 2) fx_k_scalar_march(const FxParams P, co
     }
     const long long zi = zb + (long long)k * 256;
     cp_async8(&S.fx[st][0][j][i], P.fq + zi);
-    cp_async8(&S.fx[st][1][j][i], P.fq + nzt + zi);
+    if (!HLLC) cp_async8(&S.fx[st][1][j][i], P.fq + nzt + zi);
     cp_async8(&S.fy[st][0][j][i], P.fq + 2 * nzt + zi);
-    cp_async8(&S.fy[st][1][j][i], P.fq + 3 * nzt + zi);
+    if (!HLLC) cp_async8(&S.fy[st][1][j][i], P.fq + 3 * nzt + zi);
     if (i == 15) {
       cp_async8(&S.fx[st][0][j][16], P.fq + zxh + (long long)k * 256);
-      cp_async8(&S.fx[st][1][j][16], P.fq + nzt + zxh + (long long)k * 256);
+      if (!HLLC) cp_async8(&S.fx[st][1][j][16], P.fq + nzt + zxh + (long long)k * 256);
     }
     if (j == 15) {
       cp_async8(&S.fy[st][0][16][i], P.fq + 2 * nzt + zyh + (long long)k * 256);
-      cp_async8(&S.fy[st][1][16][i], P.fq + 3 * nzt + zyh + (long long)k * 256);
+      if (!HLLC) cp_async8(&S.fy[st][1][16][i], P.fq + 3 * nzt + zyh + (long long)k * 256);
     }
     cp_async_commit();
   };
@@ -202,7 +207,7 @@ __global__ void __launch_bounds__(256, 2) fx_k_scalar_march(const FxParams P, co
     abund_at(plane_off(-1), xm1);
     abund_at(plane_off(0), xw[0]);
     abund_at(plane_off(1), xw[1]);
-    const double Fl = P.fq[4 * nzt + zb], Al = P.fq[5 * nzt + zb];
+    const double Fl = P.fq[4 * nzt + zb], Al = HLLC ? fx_aq_hllc(Fl) : P.fq[5 * nzt + zb];
 #pragma unroll
     for (int s = 0; s < NSC; ++s) {
       double apm;
@@ -246,7 +251,7 @@ __global__ void __launch_bounds__(256, 2) fx_k_scalar_march(const FxParams P, co
     if (k + 1 < nz) prefetch(k + 1);
     const long long zi = zb + (long long)k * 256;
     const long long zzh = k + 1 < nz ? zi + 256 : (long long)nb[5] * nz * 256 + tid;
-    const double Fzh = P.fq[4 * nzt + zzh], Azh = P.fq[5 * nzt + zzh];
+    const double Fzh = P.fq[4 * nzt + zzh], Azh = HLLC ? fx_aq_hllc(Fzh) : P.fq[5 * nzt + zzh];
     const long long c = (long long)b * P.S_b + (long long)(k + g2) * P.S_k + colo;
     double u0[NSC], xs[NSC];
 #pragma unroll
@@ -254,8 +259,15 @@ __global__ void __launch_bounds__(256, 2) fx_k_scalar_march(const FxParams P, co
       u0[s] = U0[(long long)(sv0 + s) * P.S_v + c];
       if (!FIRST) xs[s] = Q0[s * P.S_v + c];
     }
-    const double F0[2] = {S.fx[buf][0][j][i], S.fx[buf][0][j][i + 1]}, A0[2] = {S.fx[buf][1][j][i], S.fx[buf][1][j][i + 1]};
-    const double F1[2] = {S.fy[buf][0][j][i], S.fy[buf][0][j + 1][i]}, A1[2] = {S.fy[buf][1][j][i], S.fy[buf][1][j + 1][i]};
+    const double F0[2] = {S.fx[buf][0][j][i], S.fx[buf][0][j][i + 1]}, F1[2] = {S.fy[buf][0][j][i], S.fy[buf][0][j + 1][i]};
+    double A0[2], A1[2];
+    if (HLLC) {
+      A0[0] = fx_aq_hllc(F0[0]); A0[1] = fx_aq_hllc(F0[1]);
+      A1[0] = fx_aq_hllc(F1[0]); A1[1] = fx_aq_hllc(F1[1]);
+    } else {
+      A0[0] = S.fx[buf][1][j][i]; A0[1] = S.fx[buf][1][j][i + 1];
+      A1[0] = S.fy[buf][1][j][i]; A1[1] = S.fy[buf][1][j + 1][i];
+    }
     auto flux = [&](const double x[5], double rd, const double Fd[2], const double Ad[2]) {
       double am[3], ap[3];
 #pragma unroll
@@ -291,16 +303,24 @@ __global__ void __launch_bounds__(256, 2) fx_k_scalar_march(const FxParams P, co
   if (hit) fx_note(P, hit);
 }
 
+template <int NSC, bool FIRST, bool HLLC>
+static int fx_scalar_march_launch2(const FxParams &P, const double *X, const double *U0, double *out, const double *dx, double dt,
+                                   const double *dt_dev, double beta, int sv0, cudaStream_t st) {
+  const int smem = (int)sizeof(ScalSmem<NSC>);
+  FX_CUDA(cudaFuncSetAttribute(fx_k_scalar_march<NSC, FIRST, HLLC>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+  fx_k_scalar_march<NSC, FIRST, HLLC><<<(unsigned)P.nown, 256, smem, st>>>(P, X, U0, out, dx, dt, dt_dev, beta, sv0);
+  FX_LAUNCH_CHECK("scalar_march");
+  return FX_OK;
+}
+
 template <int NSC>
 static int fx_scalar_march_launch(const FxParams &P, const double *X, const double *U0, double *out, const double *dx, double dt,
                                   const double *dt_dev, double beta, int first, int sv0, cudaStream_t st) {
-  const int smem = (int)sizeof(ScalSmem<NSC>);
-  if (first) FX_CUDA(cudaFuncSetAttribute(fx_k_scalar_march<NSC, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-  else FX_CUDA(cudaFuncSetAttribute(fx_k_scalar_march<NSC, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-  if (first) fx_k_scalar_march<NSC, true><<<(unsigned)P.nown, 256, smem, st>>>(P, X, U0, out, dx, dt, dt_dev, beta, sv0);
-  else fx_k_scalar_march<NSC, false><<<(unsigned)P.nown, 256, smem, st>>>(P, X, U0, out, dx, dt, dt_dev, beta, sv0);
-  FX_LAUNCH_CHECK("scalar_march");
-  return FX_OK;
+  const bool hllc = P.riemann == FX_RIEMANN_HLLC;
+  if (first) return hllc ? fx_scalar_march_launch2<NSC, true, true>(P, X, U0, out, dx, dt, dt_dev, beta, sv0, st)
+                         : fx_scalar_march_launch2<NSC, true, false>(P, X, U0, out, dx, dt, dt_dev, beta, sv0, st);
+  return hllc ? fx_scalar_march_launch2<NSC, false, true>(P, X, U0, out, dx, dt, dt_dev, beta, sv0, st)
+              : fx_scalar_march_launch2<NSC, false, false>(P, X, U0, out, dx, dt, dt_dev, beta, sv0, st);
 }
 
 }  // namespace

@@ -186,7 +186,8 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
     double rate = 0.0;     // DTOUT: running maximum of (|u_d| + c) / dx_d over this thread's finished zones
     double q[W][5];        // q[m] = primitives of cell c - r + m at tick c
     double qpz[5], Fz[5];  // plus-side z state of cell c-1; z flux of face c-1 (between cells c-2 and c-1)
-    double Aqz = 0.0;      // SCAL: Aq of that face
+    constexpr bool AQS = SCAL && RIEMANN != FX_RIEMANN_HLLC;  // the faces' Aq are needed (HLLC: Aq = max(F_rho, 0))
+    double Aqz = 0.0;      // AQS: Aq of that face
     int sq = 0, sk = 0;    // SCAL: plane p is plane sk of the sq-th block of the segment
     {
       // prologue: cells -R .. r straight from global memory (all loads in flight together), the plus-side state
@@ -217,7 +218,7 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
       double qm[5], qpm1[5];
       hit |= fx_recon_cell5<RECON>(&w[0], P.weno_eps, qm, qpm1);  // cell -1
       hit |= fx_recon_cell5<RECON>(&w[1], P.weno_eps, qm, qpz);   // cell 0
-      flux_dir<RIEMANN, WS, 2, SCAL>(P, qpm1, qm, Fz, &Aqz);
+      flux_dir<RIEMANN, WS, 2, AQS>(P, qpm1, qm, Fz, &Aqz);
 #pragma unroll
       for (int m = 0; m < 2 * r; ++m)
 #pragma unroll
@@ -267,7 +268,7 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
       {
         double qmz[5], qpz_new[5];
         hit |= fx_recon_cell5<RECON>(q, P.weno_eps, qmz, qpz_new);
-        flux_dir<RIEMANN, WS, 2, SCAL>(P, qpz, qmz, Fz_new, &Aqz_new);
+        flux_dir<RIEMANN, WS, 2, AQS>(P, qpz, qmz, Fz_new, &Aqz_new);
 #pragma unroll
         for (int v = 0; v < 5; ++v) qpz[v] = qpz_new[v];
       }
@@ -276,12 +277,12 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
         double WL[5];
 #pragma unroll
         for (int v = 0; v < 5; ++v) WL[v] = S.Lx[v][j][i];
-        flux_dir<RIEMANN, WS, 0, SCAL>(P, WL, qmx, Fx, &Aqx);
+        flux_dir<RIEMANN, WS, 0, AQS>(P, WL, qmx, Fx, &Aqx);
 #pragma unroll
         for (int v = 0; v < 5; ++v) S.Lx[v][j][i] = Fx[v];  // in place: only this thread read the state
 #pragma unroll
         for (int v = 0; v < 5; ++v) WL[v] = S.Ly[v][j][i];
-        flux_dir<RIEMANN, WS, 1, SCAL>(P, WL, qmy, Fy, &Aqy);
+        flux_dir<RIEMANN, WS, 1, AQS>(P, WL, qmy, Fy, &Aqy);
 #pragma unroll
         for (int v = 0; v < 5; ++v) S.Ly[v][j][i] = Fy[v];
       }
@@ -293,11 +294,13 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
         const long long zone = (((long long)S.chain[2 + sq] * nzb + sk) * NY + j) * NX + i;
         const long long nzt = (long long)P.nblocks * nzb * (NY * NX);
         P.fq[zone] = Fx[0];
-        P.fq[nzt + zone] = Aqx;
         P.fq[2 * nzt + zone] = Fy[0];
-        P.fq[3 * nzt + zone] = Aqy;
         P.fq[4 * nzt + zone] = Fz[0];
-        P.fq[5 * nzt + zone] = Aqz;
+        if (RIEMANN != FX_RIEMANN_HLLC) {  // HLLC: Aq = max(F_rho, 0), the pass forms it itself
+          P.fq[nzt + zone] = Aqx;
+          P.fq[3 * nzt + zone] = Aqy;
+          P.fq[5 * nzt + zone] = Aqz;
+        }
         Aqz = Aqz_new;
         if (++sk == nzb) { sk = 0; ++sq; }
       }
