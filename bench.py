@@ -322,9 +322,18 @@ def algorithmic_flops(cfg, args):
 def committed_traffic(cfg, args, plan):
     """dram__bytes_read.sum + dram__bytes_write.sum per stage launch (mean over the stages of a step) from the committed
     `ncu --set full` capture of this workload and path under profiles/, read by metric name; (None, None) if there is none."""
-    if args.nb or args.block or args.scalars or args.wavespeed or args.zchain or plan.gd[0] != 8:
+    per_stage = 1  # captured launches that make up one stage
+    if args.wavespeed or args.zchain:
         return None, None
-    name = f"r2_ncu_config{cfg.number}_path{plan.path}_raw.csv"
+    if args.block == "8,8,8" and args.nb == "64,64,32" and not args.scalars:
+        name = f"r2_ncu_config{cfg.number}_8cubed_path{plan.path}_raw.csv"
+    elif args.nb or args.block or plan.gd[0] != 8:
+        return None, None
+    elif args.scalars:
+        name = f"r2_ncu_config{cfg.number}_scalars{args.scalars}_path{plan.path}_raw.csv"
+        per_stage = 1 + (args.scalars + 3) // 4  # the stage kernel and one scalar-pass launch per four scalars
+    else:
+        name = f"r2_ncu_config{cfg.number}_path{plan.path}_raw.csv"
     path = os.path.join(ROOT, "profiles", name)
     if not os.path.exists(path):
         return None, None
@@ -342,7 +351,8 @@ def committed_traffic(cfg, args, plan):
                 wr = sum(vals) / len(vals)
     if rd is None or wr is None:
         return None, None
-    return rd + wr, f"profiles/{name}: dram__bytes_read.sum + dram__bytes_write.sum, mean over the captured stage launches"
+    return (rd + wr) * per_stage, (f"profiles/{name}: dram__bytes_read.sum + dram__bytes_write.sum, mean over the captured launches"
+                                    + (f" x {per_stage} launches per stage" if per_stage > 1 else ""))
 
 
 # ------------------------------------------------------------------ CUDA arm

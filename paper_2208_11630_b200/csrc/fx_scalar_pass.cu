@@ -99,7 +99,10 @@ __global__ void __launch_bounds__(128) fx_k_scalar_pass(const FxParams P, const 
 // face's (F_rho, Aq) are plain loads issued right after the barrier and consumed at the end of the plane.  Up to NSC = 4
 // scalars per launch share the densities and the (F_rho, Aq).  Arithmetic: the expressions of fx_k_scalar_pass.
 // (Measured, config 5 with 4 scalars, this pass alone: 10.8 ms with every load at the top of the plane and 184 registers
-// (one CTA per SM); 7.4 ms with the z carry and 128 registers (two CTAs); the cp.async form below: see profiles/README.md.)
+// (one CTA per SM); 7.4 ms with the z carry and 128 registers (two CTAs); the cp.async form below 5.1 ms in the first stage
+// and 7.5 ms in the later ones, which also read U0.  Staging U0, the zone's own rho X_s (a four-slot ring) and the z face's
+// F_rho through cp.async as well -- no plain load left in the loop, 114.7 KB, still two CTAs -- was SLOWER (25.6 against
+// 24.0 ms per step): the pass is bound by the load / store unit's instruction rate, not by exposed latency.)
 template <int NSC>
 struct ScalSmem {
   double XS[2][NSC][20][20];      // abundances of the plane with halo
