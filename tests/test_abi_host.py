@@ -78,11 +78,16 @@ def test_layout_matches_oracle_and_closed_form(dims, g, nb):
     assert (L.S_j, L.S_k, L.S_b, L.S_v, L.bytes_per_state) == (o.S_j, o.S_k, o.S_b, o.S_v, o.bytes_per_state)
     npd = [d + 2 * g if d > 1 else d for d in dims]
     assert L.S_b == npd[0] * npd[1] * npd[2] and L.bytes_per_state == 5 * 8 * nb * L.S_b
-    # workspace = 256-byte scratch + 256-byte pad + (rk - 1) state copies (256-byte aligned) + z-segment table (12 ints per block)
+    # workspace = 256-byte scratch + 256-byte pad + (rk - 1) state copies (256-byte aligned) + z-segment table (12 ints per
+    # block; 8 x 8 x nz blocks: room for one 76-int bundle segment per four blocks if that is more)
+    seg_ints = nb * 12
+    if dims[0] == 8 and dims[1] == 8:
+        seg_ints = max(seg_ints, (nb // 4 + 1) * 76)
+    seg = ((seg_ints * 4 + 255) // 256) * 256
     ws = fx.lib().fx_hydro_plan_workspace_bytes(h)
-    assert ws == 512 + ((L.bytes_per_state + 255) // 256) * 256 + ((nb * 12 * 4 + 255) // 256) * 256
+    assert ws == 512 + ((L.bytes_per_state + 255) // 256) * 256 + seg
     rc3, h3 = create(dims, g, nb, rk=3)
-    assert fx.lib().fx_hydro_plan_workspace_bytes(h3) == 512 + 2 * (((L.bytes_per_state + 255) // 256) * 256) + ((nb * 12 * 4 + 255) // 256) * 256
+    assert fx.lib().fx_hydro_plan_workspace_bytes(h3) == 512 + 2 * (((L.bytes_per_state + 255) // 256) * 256) + seg
 
 
 def test_config5_needs_64bit_indexing():
