@@ -23,6 +23,9 @@
  * rho X_s, reconstructed as X_s, and given by each Riemann solver the flux it gives a transverse velocity.  Pinned in
  * tests/test_oracle_scalars.py.
  *
+ * Communication-avoiding step (fxo_hydro_advance_ca, reading B17): one guard fill per step, stages on a
+ * shrinking extension of the interior.  Pinned in tests/test_oracle_ca.py: bit for bit the result of fxo_hydro_advance.
+ *
  * Pins (tests/test_oracle_*.py, -m "not gpu"): see DESIGN.md "Oracle pins".
  * Parity unpinned: none of the routines; the Kelvin-Helmholtz field after 100
  * steps and the config-5 field after 10 steps have no exact solution and are
@@ -995,6 +998,173 @@ int fxo_hydro_advance(fxo_plan *p, double *U, const double *dx, double dt) {
   } else if (!rc) {
     rc = run_stage(p, U1, U, U2, dx, dt, 0.25, 0); /* U2 = U0 + 1/4((U1-U0) - S(U1)) */
     if (!rc) rc = run_stage(p, U2, U, U, dx, dt, 2.0 / 3.0, 0); /* U = U0 + 2/3((U2-U0) - S(U2)) */
+  }
+  free(U1);
+  free(U2);
+  return rc;
+}
+
+/* ------------------------------------------- O10 communication-avoiding step [B17; SURVEY 8(f) NEXT-4]
+ *
+ * The same SSP-RK step with ONE guard fill: O1 fills every guard zone of U0 (edges and corners too) once; stage s of n
+ * then updates the interior EXTENDED by E_s = (n - s) R zones in every active dimension (the whole box, edge and corner
+ * zones of the extension included), R = 2 (PLM) or 3 (WENO5) being the reach of one S(.), reading its stencils in place
+ * from the padded array: the stage input is known on the box extended by E_s + R = E_(s-1) -- the filled U0 for s = 1
+ * (n R <= nguard needed), the previous stage's result after that.  Behind a face with a same-level neighbour the extended
+ * zones are the neighbour's interior zones, updated with the same formula from the same numbers (the blocks must share
+ * dx): they carry what a fill of the stage result would copy there.  Behind a physical boundary that is not so: O1 of the
+ * stage result puts the boundary's IMAGE of the result there (clamp, or mirror with the normal momentum negated), so after
+ * each stage but the last those zones are re-imaged from the block's own zones -- local work, no neighbour is read. */
+
+/* Stage on block b over the interior extended by E zones in every active dimension; stencils in place from X. */
+static void block_stage_ext(fxo_plan *p, const double *X, const double *U0, double *out, int64_t b, const double *dx,
+                            double dt, double beta, int first, int E, double *W, double *S, double *Fline) {
+  const int nv = p->nvars;
+  block_prims(p, X, b, W);
+  const int64_t stride[3] = {1, p->S_j, p->S_k};
+  int lo[3], hi[3];
+  for (int d = 0; d < 3; ++d) {
+    lo[d] = p->gd[d] - (p->active[d] ? E : 0);
+    hi[d] = p->gd[d] + p->n[d] + (p->active[d] ? E : 0);
+  }
+  memset(S, 0, sizeof(double) * (size_t)nv * (size_t)p->S_b);
+  for (int d = 0; d < 3; ++d) {
+    if (!p->active[d]) continue;
+    double r = dt / dx[b * 3 + d];
+    int d1 = (d + 1) % 3, d2 = (d + 2) % 3;
+    int nf = hi[d] - lo[d]; /* zones along d; faces 0 .. nf */
+    for (int a2 = lo[d2]; a2 < hi[d2]; ++a2)
+      for (int a1 = lo[d1]; a1 < hi[d1]; ++a1) {
+        int64_t base = a1 * stride[d1] + a2 * stride[d2];
+        unsigned hit = 0;
+        for (int f = 0; f <= nf; ++f) face_flux(p, W, p->S_b, base + (int64_t)(lo[d] + f - 1) * stride[d], d, Fline + nv * f, &hit);
+        count_hits(p, hit & (FXO_STATUS_NONFINITE | FXO_STATUS_WENO_FALLBACK), 1);
+        for (int f = 0; f < nf; ++f) {
+          int64_t c = base + (int64_t)(lo[d] + f) * stride[d];
+          for (int v = 0; v < nv; ++v) S[v * p->S_b + c] += r * (Fline[nv * (f + 1) + v] - Fline[nv * f + v]);
+        }
+      }
+  }
+  for (int k = lo[2]; k < hi[2]; ++k)
+    for (int j = lo[1]; j < hi[1]; ++j)
+      for (int i = lo[0]; i < hi[0]; ++i) {
+        int64_t c = k * p->S_k + j * p->S_j + i;
+        if (p->grav[0] != 0.0 || p->grav[1] != 0.0 || p->grav[2] != 0.0) {
+          int64_t z = b * p->S_b + c;
+          double rho = X[z], gm = 0.0;
+          for (int d = 0; d < 3; ++d) {
+            S[(1 + d) * p->S_b + c] -= dt * (rho * p->grav[d]);
+            gm += p->grav[d] * X[(1 + d) * p->S_v + z];
+          }
+          S[4 * p->S_b + c] -= dt * gm;
+        }
+        for (int v = 0; v < nv; ++v) {
+          int64_t g = v * p->S_v + b * p->S_b + c;
+          if (first)
+            out[g] = U0[g] - S[v * p->S_b + c];
+          else
+            out[g] = U0[g] + beta * ((X[g] - U0[g]) - S[v * p->S_b + c]);
+        }
+      }
+}
+
+/* Zones of the box (interior + E) that lie behind a PHYSICAL boundary take the boundary's image of the block's own zone:
+ * every coordinate that is out of range on a side without a neighbour is clamped (outflow) or mirrored (wall, that
+ * momentum component negated); coordinates out of range behind a neighbour stay.  Sources are never destinations. */
+static void physical_refill(const fxo_plan *p, double *U, int64_t b, int E) {
+  int lo[3], hi[3];
+  for (int d = 0; d < 3; ++d) {
+    lo[d] = p->gd[d] - (p->active[d] ? E : 0);
+    hi[d] = p->gd[d] + p->n[d] + (p->active[d] ? E : 0);
+  }
+  for (int k = lo[2]; k < hi[2]; ++k)
+    for (int j = lo[1]; j < hi[1]; ++j)
+      for (int i = lo[0]; i < hi[0]; ++i) {
+        int c[3] = {i, j, k};
+        unsigned flip = 0;
+        int moved = 0;
+        for (int d = 0; d < 3; ++d) {
+          if (!p->active[d]) continue;
+          int l = p->gd[d], h = p->gd[d] + p->n[d];
+          int side = c[d] < l ? 0 : (c[d] >= h ? 1 : -1);
+          if (side < 0) continue;
+          int32_t nb = p->neigh[b * 6 + 2 * d + side];
+          if (nb >= 0) continue;
+          if (nb == FXO_BC_REFLECT) {
+            c[d] = side ? 2 * h - 1 - c[d] : 2 * l - 1 - c[d];
+            flip |= 1u << d;
+          } else {
+            c[d] = side ? h - 1 : l;
+          }
+          moved = 1;
+        }
+        if (!moved) continue;
+        int64_t t = b * p->S_b + k * p->S_k + j * p->S_j + i;
+        int64_t s = b * p->S_b + c[2] * p->S_k + c[1] * p->S_j + c[0];
+        for (int v = 0; v < p->nvars; ++v) {
+          double x = U[v * p->S_v + s];
+          U[v * p->S_v + t] = (v >= 1 && v <= 3 && ((flip >> (v - 1)) & 1u)) ? -x : x;
+        }
+      }
+}
+
+static int run_stage_ext(fxo_plan *p, const double *X, const double *U0, double *out, const double *dx, double dt,
+                         double beta, int first, int E) {
+  int fail = 0;
+#pragma omp parallel
+  {
+    double *W = (double *)malloc(sizeof(double) * (size_t)p->nvars * (size_t)p->S_b);
+    double *S = (double *)malloc(sizeof(double) * (size_t)p->nvars * (size_t)p->S_b);
+    int nmax = p->np[0] > p->np[1] ? p->np[0] : p->np[1];
+    if (p->np[2] > nmax) nmax = p->np[2];
+    double *Fl = (double *)malloc(sizeof(double) * (size_t)p->nvars * (size_t)(nmax + 1));
+    if (!W || !S || !Fl) {
+#pragma omp atomic write
+      fail = 1;
+    } else {
+#pragma omp for schedule(dynamic, 4)
+      for (int64_t b = 0; b < p->nblocks; ++b) {
+        block_stage_ext(p, X, U0, out, b, dx, dt, beta, first, E, W, S, Fl);
+        if (E > 0) physical_refill(p, out, b, E);
+      }
+    }
+    free(W);
+    free(S);
+    free(Fl);
+  }
+  return fail ? FXO_ERR_NOMEM : FXO_OK;
+}
+
+/* One SSP-RK step with a single guard fill [B17].  FXO_ERR_UNSUPPORTED: rk_order R > nguard in an active dimension, or
+ * refinement jumps.  The blocks must share dx with their same-level neighbours (not checked). */
+int fxo_hydro_advance_ca(fxo_plan *p, double *U, const double *dx, double dt) {
+  if (!p || (!U && p->nblocks) || (!dx && p->nblocks)) return FXO_ERR_INVALID_ARG;
+  if (!(dt > 0.0) || !isfinite(dt)) return FXO_ERR_INVALID_ARG;
+  if (!p->neigh && p->nblocks > 0) return FXO_ERR_STATE;
+  const int R = p->recon == FXO_RECON_WENO5 ? 3 : 2;
+  if (p->jump) return FXO_ERR_UNSUPPORTED;
+  for (int d = 0; d < 3; ++d)
+    if (p->active[d] && p->rk * R > p->gd[d]) return FXO_ERR_UNSUPPORTED;
+  if (p->nblocks == 0) return FXO_OK;
+  size_t n = (size_t)p->S_v * (size_t)p->nvars;
+  double *U1 = (double *)malloc(sizeof(double) * n);
+  double *U2 = p->rk == 3 ? (double *)malloc(sizeof(double) * n) : NULL;
+  if (!U1 || (p->rk == 3 && !U2)) {
+    free(U1);
+    free(U2);
+    return FXO_ERR_NOMEM;
+  }
+  /* zones outside a stage's box are never read by the next one: poison them so that a wrong reach shows */
+  for (size_t q = 0; q < n; ++q) U1[q] = NAN;
+  if (U2)
+    for (size_t q = 0; q < n; ++q) U2[q] = NAN;
+  int rc = fxo_fill_guardcells(p, U); /* the step's only O1 */
+  if (!rc) rc = run_stage_ext(p, U, U, U1, dx, dt, 1.0, 1, (p->rk - 1) * R);
+  if (!rc && p->rk == 2) {
+    rc = run_stage_ext(p, U1, U, U, dx, dt, 0.5, 0, 0);
+  } else if (!rc) {
+    rc = run_stage_ext(p, U1, U, U2, dx, dt, 0.25, 0, R);
+    if (!rc) rc = run_stage_ext(p, U2, U, U, dx, dt, 2.0 / 3.0, 0, 0);
   }
   free(U1);
   free(U2);

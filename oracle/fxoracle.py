@@ -79,6 +79,7 @@ def lib():
         L.fxo_riemann_flux_nv.restype = None
         L.fxo_euler_step.argtypes = [C.c_void_p, dp, dp, C.c_double]
         L.fxo_hydro_advance.argtypes = [C.c_void_p, dp, dp, C.c_double]
+        L.fxo_hydro_advance_ca.argtypes = [C.c_void_p, dp, dp, C.c_double]
         L.fxo_debug_compute_fluxes.argtypes = [C.c_void_p, dp, C.c_int, dp]
         L.fxo_hydro_compute_dt.argtypes = [C.c_void_p, dp, dp, C.c_double, dp]
         _lib = L
@@ -237,6 +238,13 @@ class OraclePlan:
         rc = lib().fxo_hydro_advance(self._h, _dptr(U), _dptr(dx), float(dt))
         if rc != 0:
             raise ValueError(f"fxo_hydro_advance failed with code {rc}")
+
+    def advance_ca(self, U, dx, dt):
+        """The communication-avoiding step [B17]: one guard fill, stages on a shrinking extension of the interior."""
+        dx = np.ascontiguousarray(dx, np.float64)
+        rc = lib().fxo_hydro_advance_ca(self._h, _dptr(U), _dptr(dx), float(dt))
+        if rc != 0:
+            raise ValueError(f"fxo_hydro_advance_ca failed with code {rc}")
 
     def compute_dt(self, U, dx, cfl):
         dx = np.ascontiguousarray(dx, np.float64)
