@@ -239,6 +239,22 @@ int fx_hydro_advance_host_interior(fx_hydro_plan *plan, double *Uint_host, const
 int fx_hydro_advance_devdt(fx_hydro_plan *plan, double *U_dev, const double *dx_dev, const double *dt_dev,
                            void *stream);
 
+/* The communication-avoiding form of the step [DESIGN.md B17; "fills guards once per step and updates a
+ * shrinking guard region"]: ONE guard fill of U_dev (every guard zone, edges and corners: what fx_fill_guardcells does),
+ * then stage s of n = rk_order on the interior extended by (n - s) R zones in every active dimension (R = 2 PLM, 3 WENO5),
+ * stencils read in place; after every stage but the last, the extended zones behind a physical boundary (outflow, wall) are
+ * re-imaged from the block's own zones (local; no neighbour is read after the fill).  The result on the interior equals
+ * fx_hydro_advance's bit for bit on the generic path PROVIDED every block shares dx with its same-level neighbours (an
+ * extended zone is then the neighbour's interior zone, updated with the same formula from the same numbers); guard zones
+ * of U_dev hold the fill of the step's INPUT on exit.  dt: the host value, or read from dt_dev when that is not NULL.
+ * What it buys is one exchange per step instead of one per stage where the fill is an exchange between devices; on one
+ * GPU it costs a full fill and ((n_d + 2 (n - s) R) / n_d)^ndim times the zones in the early stages, on the generic
+ * kernels (see DESIGN.md section 9 for the measured cost).  FX_ERR_UNSUPPORTED: nguard < rk_order x R (4 for RK2 + PLM,
+ * 6 for RK3 + PLM or RK2 + WENO5, 9 for RK3 + WENO5), refinement jumps, passive scalars, a sharded plan.  Needs topology
+ * and workspace (FX_ERR_STATE). */
+int fx_hydro_advance_ca(fx_hydro_plan *plan, double *U_dev, const double *dx_dev, double dt, const double *dt_dev,
+                        void *stream);
+
 /* One step with the time step kept on the device and the next one formed on the way [O6 + O7]: advances U_dev by
  * *dt_inout_dev exactly as fx_hydro_advance_devdt does, and replaces *dt_inout_dev by cfl * min dx/(|u_d| + c) of
  * the ADVANCED state -- on the fused path the reduction rides in the last RK stage (each zone's rate is formed from

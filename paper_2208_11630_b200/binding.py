@@ -29,7 +29,7 @@ EXPORTS = [
     "fx_last_error", "fx_hydro_plan_create", "fx_hydro_plan_destroy", "fx_hydro_plan_layout",
     "fx_hydro_plan_set_option", "fx_hydro_plan_workspace_bytes", "fx_hydro_plan_set_workspace",
     "fx_hydro_plan_set_topology", "fx_hydro_plan_set_refinement", "fx_topology_cartesian", "fx_fill_guardcells", "fx_guardcell_index_map",
-    "fx_hydro_compute_dt", "fx_hydro_compute_dt_static", "fx_hydro_advance", "fx_hydro_advance_host", "fx_hydro_advance_host_interior", "fx_hydro_advance_devdt", "fx_hydro_step",
+    "fx_hydro_compute_dt", "fx_hydro_compute_dt_static", "fx_hydro_advance", "fx_hydro_advance_host", "fx_hydro_advance_host_interior", "fx_hydro_advance_devdt", "fx_hydro_advance_ca", "fx_hydro_step",
     "fx_hydro_status", "fx_hydro_status_reset", "fx_debug_compute_fluxes", "fx_hydro_plan_path",
     "fx_hydro_plan_set_timing", "fx_hydro_plan_get_timing",
     "fx_shard_create", "fx_shard_destroy", "fx_shard_sizes", "fx_shard_tables", "fx_shard_items", "fx_halo_item_elems",
@@ -78,6 +78,7 @@ def lib():
         L.fx_hydro_compute_dt_static.argtypes = [vp, vp, vp, C.c_double, vp, vp, vp]
         L.fx_hydro_advance.argtypes = [vp, vp, vp, C.c_double, vp]
         L.fx_hydro_advance_devdt.argtypes = [vp, vp, vp, vp, vp]
+        L.fx_hydro_advance_ca.argtypes = [vp, vp, vp, C.c_double, vp, vp]
         L.fx_hydro_step.argtypes = [vp, vp, vp, C.c_double, vp, vp]
         L.fx_hydro_advance_host.argtypes = [vp, vp, vp, C.c_double, C.c_int, vp, vp, vp, vp]
         L.fx_hydro_advance_host_interior.argtypes = [vp, vp, vp, C.c_double, C.c_int, vp, vp, vp, vp, vp]
@@ -270,6 +271,16 @@ class HydroPlan:
         _check(lib().fx_hydro_compute_dt(self._h, _dev(U, torch.float64), _dev(dx, torch.float64), float(cfl),
                                          _dev(dt_out, torch.float64), _stream(stream)))
         return dt_out
+
+    def fx_hydro_advance_ca(self, U, dx, dt, stream=None):
+        """The communication-avoiding step: one guard fill, stages on a shrinking extension of the interior.  dt: a float,
+        or a 1-element device tensor read on the device."""
+        if isinstance(dt, torch.Tensor):
+            _check(lib().fx_hydro_advance_ca(self._h, _dev(U, torch.float64), _dev(dx, torch.float64), 0.0,
+                                             _dev(dt, torch.float64), _stream(stream)))
+        else:
+            _check(lib().fx_hydro_advance_ca(self._h, _dev(U, torch.float64), _dev(dx, torch.float64), float(dt), None,
+                                             _stream(stream)))
 
     def fx_hydro_compute_dt_static(self, U, dx, cfl, dt_out, flags_out=None, stream=None):
         """The reduction with its scratch in the library's static device array (no workspace, no allocation: the caller

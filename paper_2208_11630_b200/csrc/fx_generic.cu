@@ -131,7 +131,9 @@ template <int RECON> struct FxScalarShared {
 // Direction D of one zone, in the lean arithmetic of the fused kernel (fx_c2p_v2, fx_recon_cell, fx_riemann_v2: one
 // Newton step on the MUFU seeds instead of IEEE division and square root; same formulas, rounding differs): the 2R+1
 // stencil cells are converted once, cells -1, 0, +1 are reconstructed once each, and the zone's two faces are solved.
-template <int RECON, int RIEMANN, int WS, int D, bool SCALARS, bool AMR = false>
+// CA (communication-avoiding step [B17]): every stencil cell is read in place from the padded array -- the guard zones hold
+// the step's one fill or the previous stage's extended result -- and idx may lie outside [0, n).
+template <int RECON, int RIEMANN, int WS, int D, bool SCALARS, bool AMR = false, bool CA = false>
 __device__ __forceinline__ unsigned fx_zone_direction(const FxParams &P, const double *__restrict__ X, long long b,
                                                       long long c, int idx, long long s, double rd, double S[5],
                                                       unsigned &qfb, FxScalarShared<RECON> *sh, int tflat = 0) {
@@ -142,8 +144,8 @@ __device__ __forceinline__ unsigned fx_zone_direction(const FxParams &P, const d
   unsigned hit = 0;
 #pragma unroll
   for (int m = 0; m <= 2 * R; ++m) {
-    bool flip;
-    const long long e = fx_stencil_cell<D>(P, b, c, idx, m - R, s, flip);
+    bool flip = false;
+    const long long e = CA ? c + (long long)(m - R) * s : fx_stencil_cell<D>(P, b, c, idx, m - R, s, flip);
     double u[5] = {X[e], X[P.S_v + e], X[2 * P.S_v + e], X[3 * P.S_v + e], X[4 * P.S_v + e]}, ri;
     if (flip) u[1 + D] = -u[1 + D];
     hit |= fx_c2p_v2(P, u[0], u[1], u[2], u[3], u[4], W[m], &ri);
@@ -246,28 +248,30 @@ __device__ __forceinline__ double fx_zone_scalar_direction(const FxParams &P, co
 // 5 CTAs 13.9 / 25.9, 6 CTAs (80 registers) 13.5 / 24.7, 8 CTAs (64 registers; its spills reach DRAM: 28.6 GB written
 // for 9.7 GB) 16.3 / 31.0.  WENO5 at config 4 without / with 2 scalars: 3 CTAs 5.5 / 7.8, 4 CTAs 5.5 / 7.4, 5 CTAs
 // 5.6 / 7.3.  (The IEEE-arithmetic version of this kernel: PLM uncapped 38.3, 8 CTAs 30.0; WENO5 uncapped 15.2, 4 CTAs 8.2.)
-template <int RECON, int RIEMANN, int WS, bool SCALARS, bool AMR = false>
+// CA [B17]: the zones are those of the interior extended by `ext` zones in every active dimension (nzones counts them).
+template <int RECON, int RIEMANN, int WS, bool SCALARS, bool AMR = false, bool CA = false>
 __global__ void __launch_bounds__(128, RECON == FX_RECON_PLM_MINMOD ? FX_GENERIC_MINB_PLM : FX_GENERIC_MINB_WENO) fx_k_generic_stage(FxParams P, const double *__restrict__ X,
                                                           const double *U0, double *out,
                                                           const double *__restrict__ dx, double dt,
                                                           const double *__restrict__ dt_dev, double beta, int first,
-                                                          long long nzones) {
+                                                          long long nzones, int ext = 0) {
   extern __shared__ __align__(16) unsigned char fx_generic_smem[];
   FxScalarShared<RECON> *sh = reinterpret_cast<FxScalarShared<RECON> *>(fx_generic_smem);  // SCALARS only
   const long long z = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (z >= nzones) return;
-  const int nx = P.n[0], ny = P.n[1], nz = P.n[2];
+  const int e0 = CA && P.active[0] ? ext : 0, e1 = CA && P.active[1] ? ext : 0, e2 = CA && P.active[2] ? ext : 0;
+  const int nx = P.n[0] + 2 * e0, ny = P.n[1] + 2 * e1, nz = P.n[2] + 2 * e2;
   const long long per_block = (long long)nx * ny * nz;
   const long long b = z / per_block;
   const int r = (int)(z - b * per_block);
   // (a CTA of 16 x 4 x 2 zones instead of 8 rows of one plane, for L1 reuse of the y and z neighbours: measured, no gain)
-  const int i = r % nx, j = (r / nx) % ny, k = r / (nx * ny);
+  const int i = r % nx - e0, j = (r / nx) % ny - e1, k = r / (nx * ny) - e2;  // interior coordinates (CA: from -ext)
   const long long c = b * P.S_b + (k + P.gd[2]) * P.S_k + (j + P.gd[1]) * P.S_j + (i + P.gd[0]);
   if (dt_dev) dt = *dt_dev;
   double S[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
   unsigned qfb = 0;  // 4 bits per direction: fallback sides of the low and the high face
   unsigned hit = 0;
-  {  // floors are counted once per owned zone
+  if (!CA || (i >= 0 && i < P.n[0] && j >= 0 && j < P.n[1] && k >= 0 && k < P.n[2])) {  // floors are counted once per owned zone
     double W[5];
     hit |= fx_c2p_v2(P, X[c], X[P.S_v + c], X[2 * P.S_v + c], X[3 * P.S_v + c], X[4 * P.S_v + c], W) &
            (FX_STATUS_RHO_FLOOR | FX_STATUS_P_FLOOR | FX_STATUS_NONFINITE);
@@ -276,9 +280,9 @@ __global__ void __launch_bounds__(128, RECON == FX_RECON_PLM_MINMOD ? FX_GENERIC
   const double rd1 = P.active[1] ? dt / __ldg(&dx[b * 3 + 1]) : 0.0;
   const double rd2 = P.active[2] ? dt / __ldg(&dx[b * 3 + 2]) : 0.0;
   // (tflat: the zone's position on the face, transverse dimensions ascending, first one fastest)
-  if (P.active[0]) hit |= fx_zone_direction<RECON, RIEMANN, WS, 0, SCALARS, AMR>(P, X, b, c, i, 1, rd0, S, qfb, sh, k * ny + j);
-  if (P.active[1]) hit |= fx_zone_direction<RECON, RIEMANN, WS, 1, SCALARS, AMR>(P, X, b, c, j, P.S_j, rd1, S, qfb, sh, k * nx + i);
-  if (P.active[2]) hit |= fx_zone_direction<RECON, RIEMANN, WS, 2, SCALARS, AMR>(P, X, b, c, k, P.S_k, rd2, S, qfb, sh, j * nx + i);
+  if (P.active[0]) hit |= fx_zone_direction<RECON, RIEMANN, WS, 0, SCALARS, AMR, CA>(P, X, b, c, i, 1, rd0, S, qfb, sh, k * ny + j);
+  if (P.active[1]) hit |= fx_zone_direction<RECON, RIEMANN, WS, 1, SCALARS, AMR, CA>(P, X, b, c, j, P.S_j, rd1, S, qfb, sh, k * nx + i);
+  if (P.active[2]) hit |= fx_zone_direction<RECON, RIEMANN, WS, 2, SCALARS, AMR, CA>(P, X, b, c, k, P.S_k, rd2, S, qfb, sh, j * nx + i);
   if (P.grav_on) {  // constant-gravity source of the stage input's own zone [B10]
     const double rho = X[c];
     double gm = 0.0;
@@ -370,6 +374,75 @@ int fx_launch_generic_stage(const FxParams &P, const double *X, const double *U0
   FX_DISPATCH(P, CALL);
 #undef CALL
   FX_LAUNCH_CHECK("generic_stage");
+  return FX_OK;
+}
+
+// ------------------------------------------------------------------ communication-avoiding step [B17]
+// A stage over the interior extended by `ext` zones in every active dimension, stencils in place.
+int fx_launch_generic_stage_ca(const FxParams &P, const double *X, const double *U0, double *out, const double *dx, double dt,
+                               const double *dt_dev, double beta, int first, int ext, cudaStream_t st) {
+  long long per = 1;
+  for (int d = 0; d < 3; ++d) per *= P.n[d] + (P.active[d] ? 2 * ext : 0);
+  const long long nzones = P.nown * per;
+  if (nzones == 0) return FX_OK;
+  const unsigned grid = (unsigned)((nzones + 127) / 128);
+#define CALL(RC, RM)                                                                                                                          \
+  do {                                                                                                                                        \
+    if (P.wavespeed == 0) fx_k_generic_stage<RC, RM, 0, false, false, true><<<grid, 128, 0, st>>>(P, X, U0, out, dx, dt, dt_dev, beta, first, nzones, ext); \
+    else fx_k_generic_stage<RC, RM, 1, false, false, true><<<grid, 128, 0, st>>>(P, X, U0, out, dx, dt, dt_dev, beta, first, nzones, ext); \
+  } while (0)
+  FX_DISPATCH(P, CALL);
+#undef CALL
+  FX_LAUNCH_CHECK("generic_stage_ca");
+  return FX_OK;
+}
+
+// The zones of the extended box that lie behind a PHYSICAL boundary take that boundary's image of the block's own zone
+// (clamp; at a wall the mirror zone with the normal momentum negated) -- what O1 of the stage result would put there;
+// zones behind a neighbour keep the value the extended stage computed.  Sources are never destinations.
+__global__ void __launch_bounds__(128) fx_k_ca_refill(FxParams P, double *U, int ext, long long nzones) {
+  const long long z = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (z >= nzones) return;
+  const int e0 = P.active[0] ? ext : 0, e1 = P.active[1] ? ext : 0, e2 = P.active[2] ? ext : 0;
+  const int nx = P.n[0] + 2 * e0, ny = P.n[1] + 2 * e1, nz = P.n[2] + 2 * e2;
+  const long long per_block = (long long)nx * ny * nz;
+  const long long b = z / per_block;
+  const int r = (int)(z - b * per_block);
+  const int t[3] = {r % nx - e0, (r / nx) % ny - e1, r / (nx * ny) - e2};
+  int c[3] = {t[0], t[1], t[2]};
+  unsigned flip = 0;
+  bool moved = false;
+#pragma unroll
+  for (int d = 0; d < 3; ++d) {
+    if (!P.active[d] || (c[d] >= 0 && c[d] < P.n[d])) continue;
+    const int side = c[d] >= P.n[d];
+    const int nb = __ldg(&P.neigh[b * 6 + 2 * d + side]);
+    if (nb >= 0) continue;
+    if (nb == FX_BC_REFLECT) {
+      c[d] = side ? 2 * P.n[d] - 1 - c[d] : -1 - c[d];
+      flip |= 1u << d;
+    } else {
+      c[d] = side ? P.n[d] - 1 : 0;
+    }
+    moved = true;
+  }
+  if (!moved) return;
+  const long long dst = b * P.S_b + (t[2] + P.gd[2]) * P.S_k + (t[1] + P.gd[1]) * P.S_j + (t[0] + P.gd[0]);
+  const long long src = b * P.S_b + (c[2] + P.gd[2]) * P.S_k + (c[1] + P.gd[1]) * P.S_j + (c[0] + P.gd[0]);
+  for (int v = 0; v < P.nvars; ++v) {
+    const double x = U[v * P.S_v + src];
+    U[v * P.S_v + dst] = (v >= 1 && v <= 3 && ((flip >> (v - 1)) & 1u)) ? -x : x;
+  }
+}
+
+int fx_launch_ca_refill(const FxParams &P, double *U, int ext, cudaStream_t st) {
+  if (ext <= 0 || P.all_interior) return FX_OK;  // no physical boundary anywhere
+  long long per = 1;
+  for (int d = 0; d < 3; ++d) per *= P.n[d] + (P.active[d] ? 2 * ext : 0);
+  const long long nzones = P.nown * per;
+  if (nzones == 0) return FX_OK;
+  fx_k_ca_refill<<<(unsigned)((nzones + 127) / 128), 128, 0, st>>>(P, U, ext, nzones);
+  FX_LAUNCH_CHECK("ca_refill");
   return FX_OK;
 }
 

@@ -90,6 +90,11 @@ int fx_cuda_check(cudaError_t e, const char *what);
 
 // kernel launchers (one per .cu file); all enqueue on `st`
 int fx_launch_fill_guardcells(const FxParams &P, double *U, cudaStream_t st);
+// communication-avoiding step [B17]: a stage over the interior extended by `ext` zones (stencils in place); the re-imaging
+// of the extended zones behind physical boundaries
+int fx_launch_generic_stage_ca(const FxParams &P, const double *X, const double *U0, double *out, const double *dx, double dt,
+                               const double *dt_dev, double beta, int first, int ext, cudaStream_t st);
+int fx_launch_ca_refill(const FxParams &P, double *U, int ext, cudaStream_t st);
 int fx_launch_fill_faces(const FxParams &P, double *U, int v0, cudaStream_t st);  // face guard zones of depth R, variables >= v0
 int fx_launch_index_map(const FxParams &P, long long b0, long long nb, long long *src, cudaStream_t st);
 int fx_launch_pack_interior(const FxParams &P, double *U, double *packed, int to_packed, cudaStream_t st);

@@ -173,6 +173,44 @@ extern "C" int fx_hydro_advance(fx_hydro_plan *plan, double *U, const double *dx
   return fx_advance_impl(plan, U, dx, dt, nullptr, (cudaStream_t)stream);
 }
 
+// The communication-avoiding step [B17; SURVEY 8(f) NEXT-4]: the step's one guard fill, then stage s of n on the interior
+// extended by (n - s) R zones, each reading its stencils in place; after every stage but the last the extended zones
+// behind a physical boundary are re-imaged from the block's own zones.  Each stage kernel is bracketed like fx_stage's.
+extern "C" int fx_hydro_advance_ca(fx_hydro_plan *plan, double *U, const double *dx, double dt, const double *dt_dev,
+                                   void *stream) {
+  int rc = fx_need(plan, true, true, "advance_ca");
+  if (rc) return rc;
+  if (!dt_dev && (!(dt > 0.0) || !isfinite(dt))) return fx_fail(FX_ERR_INVALID_ARG, "advance_ca: dt must be positive and finite");
+  if ((!U || !dx) && plan->P.nblocks > 0) return fx_fail(FX_ERR_INVALID_ARG, "advance_ca: null argument");
+  const FxParams &P = plan->P;
+  const int R = P.recon == FX_RECON_WENO5 ? 3 : 2;
+  for (int d = 0; d < 3; ++d)
+    if (P.active[d] && plan->rk * R > plan->nguard)
+      return fx_fail(FX_ERR_UNSUPPORTED, "advance_ca: needs nguard >= rk_order x %d = %d (the plan has %d)", R, plan->rk * R, plan->nguard);
+  if (P.has_jumps || P.jump) return fx_fail(FX_ERR_UNSUPPORTED, "advance_ca: refinement jumps are not supported");
+  if (plan->nvars > 5) return fx_fail(FX_ERR_UNSUPPORTED, "advance_ca: passive scalars are not supported");
+  if (P.nown != P.nblocks) return fx_fail(FX_ERR_UNSUPPORTED, "advance_ca: not for a sharded plan (its ghost blocks carry no edge neighbours)");
+  if (P.nown == 0) return FX_OK;
+  cudaStream_t st = (cudaStream_t)stream;
+  double *U1 = plan->stage[0], *U2 = plan->stage[1];
+  if ((rc = fx_launch_fill_guardcells(P, U, st))) return rc;  // the step's only O1: every guard zone, edges and corners too
+  auto stage = [&](const double *X, double *out, double beta, int first, int ext) -> int {
+    const bool rec = plan->timing && plan->ev && plan->nrec < FX_MAX_REC;
+    if (rec) FX_CUDA(cudaEventRecord(plan->ev[2 * plan->nrec], st));
+    int r2 = fx_launch_generic_stage_ca(P, X, U, out, dx, dt, dt_dev, beta, first, ext, st);
+    if (r2) return r2;
+    if (rec) {
+      FX_CUDA(cudaEventRecord(plan->ev[2 * plan->nrec + 1], st));
+      ++plan->nrec;
+    }
+    return fx_launch_ca_refill(P, out, ext, st);
+  };
+  if ((rc = stage(U, U1, 1.0, 1, (plan->rk - 1) * R))) return rc;
+  if (plan->rk == 2) return stage(U1, U, 0.5, 0, 0);
+  if ((rc = stage(U1, U2, 0.25, 0, R))) return rc;
+  return stage(U2, U, 2.0 / 3.0, 0, 0);
+}
+
 extern "C" int fx_hydro_advance_devdt(fx_hydro_plan *plan, double *U, const double *dx, const double *dt_dev,
                                       void *stream) {
   int rc = fx_need(plan, true, true, "advance_devdt");
