@@ -58,6 +58,8 @@ def parse_args():
     ap.add_argument("--wavespeed", type=int, default=0, help="FX_OPT_WAVESPEED: 0 Einfeldt (the reading the configs are run with [A8]), 1 Davis")
     ap.add_argument("--shard", action="store_true", help="drive the step through ShardedHydro even on one rank (the N > 1 code path with an "
                     "empty exchange; N > 1 always uses it)")
+    ap.add_argument("--ca", action="store_true", help="time the communication-avoiding step (fx_hydro_advance_ca, DESIGN.md B17: one guard fill "
+                    "per step, generic kernels on a shrinking extension of the interior) + fx_hydro_compute_dt instead of fx_hydro_step")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=2)
@@ -235,7 +237,7 @@ def oracle_sample(args, target_seconds=15.0, steps=None, steps_single=0):
     def one_step():
         t = time.perf_counter()
         dt = plan.compute_dt(U, dx, cfg.cfl)
-        plan.advance(U, dx, dt)
+        (plan.advance_ca if getattr(args, "ca", False) else plan.advance)(U, dx, dt)
         return time.perf_counter() - t
 
     t_first = one_step()  # also the warm-up
@@ -257,7 +259,7 @@ def oracle_sample(args, target_seconds=15.0, steps=None, steps_single=0):
             single = None
     return {"value": zs / per_step, "unit": UNIT, "cores": cores, "kind": "oracle", "single_thread": single,
             "sample": f"config {args.config} field on a {nb[0]}x{nb[1]}x{nb[2]}-block periodic sub-tiling "
-                      f"({cfg.interior_zones} zones), {steps} steps of compute_dt + advance, OpenMP over blocks",
+                      f"({cfg.interior_zones} zones), {steps} steps of compute_dt + {'advance_ca' if getattr(args, 'ca', False) else 'advance'}, OpenMP over blocks",
             "ms_per_step": per_step * 1e3, "steps": steps}
 
 
@@ -323,7 +325,7 @@ def committed_traffic(cfg, args, plan):
     """dram__bytes_read.sum + dram__bytes_write.sum per stage launch (mean over the stages of a step) from the committed
     `ncu --set full` capture of this workload and path under profiles/, read by metric name; (None, None) if there is none."""
     per_stage = 1  # captured launches that make up one stage
-    if args.wavespeed or args.zchain:
+    if args.wavespeed or args.zchain or args.ca:
         return None, None
     if args.block == "8,8,8" and args.nb == "64,64,32" and not args.scalars:
         name = f"r2_ncu_config{cfg.number}_8cubed_path{plan.path}_raw.csv"
@@ -385,6 +387,14 @@ def run_ours(args, rank, world, local_rank):
 
         def step():
             sh.step(U, dx, cfg.cfl, dt)  # per stage: slab exchange, then the stage on the owned blocks; dt <- min over ranks
+    elif args.ca:
+        # fill (1 launch), the stages, the local re-imaging of physical boundaries after all but the last, the reduction
+        launches_per_step = 1 + stages + (0 if cfg.bc == "periodic" else stages - 1) + 1
+        dt = plan.fx_hydro_compute_dt(U, dx, cfg.cfl).clone()
+
+        def step():
+            plan.fx_hydro_advance_ca(U, dx, dt)          # one guard fill, then every stage without another
+            plan.fx_hydro_compute_dt(U, dx, cfg.cfl, dt)  # a7 of the advanced state
     else:
         dt = plan.fx_hydro_compute_dt(U, dx, cfg.cfl).clone()  # the first step's dt; stays on the device from here on
 
@@ -452,7 +462,7 @@ def run_ours(args, rank, world, local_rank):
                 "frac": side["frac"], "traffic": traffic, "traffic_source": traffic_src,
                 "roof_ps_per_zone_stage": {"hbm": t_hbm * 1e12, "fp64": t_fp * 1e12 if flops is not None else None},
                 "hbm": hbm, "fp64": fp64,
-                "kernel": {1: "fused stage kernel", 3: "fused stage kernel, pair variant", 4: "fused stage kernel on 2 x 2 bundles of 8 x 8 blocks", 2: "tile stage kernel", 0: "generic stage kernel"}[plan.path],
+                "kernel": "generic stage kernel over the extended interior (communication-avoiding step)" if args.ca else {1: "fused stage kernel", 3: "fused stage kernel, pair variant", 4: "fused stage kernel on 2 x 2 bundles of 8 x 8 blocks", 2: "tile stage kernel", 0: "generic stage kernel"}[plan.path],
                 "kernel_ms_avg": stage_avg_ms, "kernel_launches_timed": stage_launches,
                 "kernel_share_of_step": stage_ms / ms if ms > 0 else None}
 
@@ -466,7 +476,7 @@ def run_ours(args, rank, world, local_rank):
                                    + (", Davis wave speeds" if args.wavespeed else ""),
                        "interior_zones": zones, "state_bytes": plan.bytes_per_state, "block_order": args.order,
                        "layout": f"x guard depth {plan.gd[0]} (row pitch {plan.S_j * 8} B), y/z guard depth {plan.gd[1]}/{plan.gd[2]}",
-                       "path": {0: "generic", 1: "fused (TMA)", 2: "tile (shared-memory block)", 3: "fused (TMA), two zones per thread", 4: "fused (TMA), 2 x 2 bundles of 8 x 8 blocks"}[plan.path], "l2": "inputs (state) larger than L2; no flush needed",
+                       "path": "communication-avoiding step (one guard fill per step; generic kernels on the extended interior)" if args.ca else {0: "generic", 1: "fused (TMA)", 2: "tile (shared-memory block)", 3: "fused (TMA), two zones per thread", 4: "fused (TMA), 2 x 2 bundles of 8 x 8 blocks"}[plan.path], "l2": "inputs (state) larger than L2; no flush needed",
                        "multi_gpu": (f"sharded: tiling {cfg.nb[0]}x{cfg.nb[1]}x{cfg.nb[2]} blocks in {world} contiguous Morton runs, "
                                      f"{sh.shard.n_ghost} ghost blocks on rank 0, cut-face slabs exchanged before every stage "
                                      f"(grouped NCCL send/recv, {sh.send_elems * 8} B sent by rank 0 per stage), dt = all-reduce(min)")
@@ -550,6 +560,10 @@ def run_ours(args, rank, world, local_rank):
 
 def main():
     args = parse_args()
+    if args.ca:
+        args.no_e2e = True  # the end-to-end call (fx_hydro_advance_host_interior) runs the standard step
+        if args.gpus > 1 or args.shard or args.scalars:
+            sys.exit("--ca: single plan, five variables (fx_hydro_advance_ca refuses sharded plans and passive scalars)")
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
