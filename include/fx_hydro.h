@@ -62,8 +62,10 @@ enum {
                            1 = generic; 2 = tile kernel where it fits, else generic; 3 = the fused kernel's
                            two-zones-per-thread variant where it applies (PLM, no wall, no gravity; measured slower
                            than the default, kept for comparison), else as 0.
+                           With refinement jumps (fx_hydro_plan_set_refinement): the generic kernel; under 0 and with 16 x 16 x nz
+                           blocks only the blocks that HAVE a jump face take it, the fused kernel advances the others (5).
                            fx_hydro_plan_path reports the choice (1 fused, 4 fused on bundles of 8 x 8 blocks, 3 the pair variant,
-                           2 tile, 0 generic). */
+                           5 fused + generic at the refinement jumps, 2 tile, 0 generic). */
   FX_OPT_ZCHAIN = 5,    /* fused path: longest chain of z-neighbour blocks one CTA marches through, 1..8 (1..16 for 8 x 8 x nz
                            blocks; a larger value is clamped to what the kernel takes); 0 (default) =
                            chosen from the number of blocks and of SMs so that the launch still fills the GPU.

@@ -118,6 +118,7 @@ extern "C" int fx_hydro_plan_destroy(fx_hydro_plan *plan) {
   if (plan) delete[] plan->seg_host;
   if (plan) delete[] plan->jump_host;
   if (plan) delete[] plan->bseg_host;
+  if (plan) delete[] plan->jlist_host;
   if (plan && plan->ev) {
     for (int i = 0; i < 2 * FX_MAX_REC; ++i) cudaEventDestroy(plan->ev[i]);
     delete[] plan->ev;
@@ -201,7 +202,12 @@ extern "C" int fx_hydro_plan_set_option(fx_hydro_plan *plan, int key, double val
 
 extern "C" int fx_hydro_plan_path(const fx_hydro_plan *plan) {
   if (!plan) return fx_fail(FX_ERR_INVALID_ARG, "plan_path: null plan");
-  if (plan->P.has_jumps) return 0;  // refinement jumps [B12-B14]: the generic path reads the interpolated guard zones
+  if (plan->P.has_jumps) {
+    // refinement jumps [B12-B14]: the generic kernel reads the interpolated guard zones.  Where the fused kernel takes the
+    // block shape, only the blocks that HAVE a jump face go that way (5: fused kernel on the rest, whose faces all have
+    // same-level neighbours or physical boundaries)
+    return (plan->jlist_host && plan->P.jlist && fx_stage_tma_supported(plan->P)) ? 5 : 0;
+  }
   // passive scalars [B11]: behind the fused kernel by the scalar pass where it applies (PLM, same-level neighbours
   // everywhere, no gravity), else on the generic path
   if (plan->nvars > 5 && !(plan->path_option == 0 && fx_stage_tma_supported(plan->P) && fx_scalar_pass_supported(plan->P))) return 0;
@@ -261,6 +267,14 @@ static int fx_seg_upload(fx_hydro_plan *plan) {
   plan->P.nseg = plan->nseg_host;
   plan->P.bseg = nullptr;
   plan->P.nbseg = 0;
+  plan->P.jlist = nullptr;
+  plan->P.njump = 0;
+  if (plan->jlist_host && plan->nseg_host > 0) {  // hybrid AMR path: the jump blocks' ids behind the segments (nseg 12 + njump <= nblocks 12 ints)
+    int *jd = dst + (size_t)plan->nseg_host * FX_SEG_STRIDE;
+    if (plan->njump_host > 0) FX_CUDA(cudaMemcpy(jd, plan->jlist_host, (size_t)plan->njump_host * sizeof(int), cudaMemcpyHostToDevice));
+    plan->P.jlist = jd;
+    plan->P.njump = plan->njump_host;
+  }
   if (plan->bseg_host && plan->nbseg_host > 0) {  // bundle segments take the place of the (unused: blocks are not 16 wide) block segments
     FX_CUDA(cudaMemcpy(dst, plan->bseg_host, (size_t)plan->nbseg_host * FX_BSEG_STRIDE * sizeof(int), cudaMemcpyHostToDevice));
     plan->P.bseg = dst;
@@ -478,6 +492,29 @@ extern "C" int fx_hydro_plan_set_topology(fx_hydro_plan *plan, const int32_t *ne
       if (rcb) return rcb;
     }
     std::vector<char> seen((size_t)nb, 0);
+    // Refinement jumps, hybrid path: where the block shape is the fused kernel's, the blocks WITH a jump face are listed for
+    // the generic kernel (which reads their interpolated guard zones) and taken out of the chains; every face of the others
+    // has a same-level neighbour or a physical boundary, which is all the fused kernel needs.
+    delete[] plan->jlist_host;
+    plan->jlist_host = nullptr;
+    plan->njump_host = 0;
+    {
+      const int Rr = plan->P.recon == FX_RECON_WENO5 ? 3 : 2;
+      const FxParams &Q = plan->P;
+      const bool shape = Q.n[0] == 16 && Q.n[1] == 16 && Q.n[2] >= Rr && Q.active[2] && Q.gd[0] >= Rr && (Q.S_j % 2) == 0 && (Q.gd[0] % 2) == 0;
+      if (jumps && shape && plan->path_option == 0 && plan->nvars == 5 && Q.n[2] <= 64) {
+        plan->jlist_host = new (std::nothrow) int[(size_t)nb];
+        if (!plan->jlist_host) return fx_fail(FX_ERR_INVALID_ARG, "set_topology: out of host memory");
+        for (long long b = 0; b < nown; ++b) {
+          bool jb = false;
+          for (int f = 0; f < 6; ++f) jb |= Q.active[f / 2] && h[b * 6 + f] <= FX_NEIGH_COARSER;
+          if (jb) {
+            plan->jlist_host[plan->njump_host++] = (int)b;
+            seen[b] = 1;  // ends a chain from either side; never starts one
+          }
+        }
+      }
+    }
     plan->seg_host = new (std::nothrow) int[(size_t)nb * FX_SEG_STRIDE];
     if (!plan->seg_host) return fx_fail(FX_ERR_INVALID_ARG, "set_topology: out of host memory");
     // (blocks taller than 64 planes are not chained: the kernel's plane -> block map is exact up to 2^20 / nz planes)

@@ -1,0 +1,117 @@
+"""Refinement jumps with 16 x 16 x nz blocks: the hybrid path (fx_hydro_plan_path = 5) -- the fused TMA kernel on the blocks
+whose faces all have same-level neighbours or physical boundaries, the generic kernel on the blocks that have a jump face
+(it reads their interpolated guard zones), then the flux correction.  Checked against the oracle on static two-level grids
+(<= 1e-12 after one step, <= 1e-9 after ten [NS]), for conservation through the jumps, against the all-generic path, and
+for bitwise independence of the chain length."""
+import numpy as np
+import pytest
+import torch
+
+from tests.helpers import two_level_grid, rel_err
+from tests.test_oracle_amr import GAMMA, amr_plan, cons, dx_of, smooth_field, state_from, totals
+
+pytestmark = pytest.mark.gpu
+
+DIMS = (16, 16, 16)
+CENTRE2 = {(x, y, z) for x in (1, 2) for y in (1, 2) for z in (1, 2)}
+GRIDS16 = [((5, 5, 5), {(2, 2, 2)}, True), ((4, 4, 4), CENTRE2, True), ((4, 4, 3), {(0, 0, 0), (1, 0, 0), (3, 3, 2)}, False)]
+
+
+class Cfg:
+    gamma = GAMMA
+
+
+def gpu_plan(grid, recon=0, riemann=1, rk=2, path=None, zchain=None, dims=DIMS):
+    from paper_2208_11630_b200 import binding as fx
+    plan = fx.HydroPlan(dims, 4, len(grid["level"]), GAMMA, recon, riemann, rk)
+    if path is not None:
+        plan.fx_hydro_plan_set_option(fx.OPT_PATH, path)
+    if zchain is not None:
+        plan.fx_hydro_plan_set_option(fx.OPT_ZCHAIN, zchain)
+    plan.fx_hydro_plan_set_refinement(grid["jump"])
+    plan.fx_hydro_plan_set_topology(grid["neigh"])
+    plan.fx_hydro_plan_set_workspace()
+    return plan
+
+
+@pytest.mark.parametrize("nbc,refined,periodic", GRIDS16)
+@pytest.mark.parametrize("recon,riemann,rk", [(0, 1, 2), (1, 1, 3), (0, 0, 3)])
+def test_hybrid_parity_conservation_and_generic(nbc, refined, periodic, recon, riemann, rk):
+    grid = two_level_grid(nbc, refined, DIMS, periodic=periodic)
+    oplan = amr_plan(grid, DIMS, recon=recon, riemann=riemann, rk=rk)
+    gplan = gpu_plan(grid, recon, riemann, rk)
+    ggen = gpu_plan(grid, recon, riemann, rk, path=1)
+    assert gplan.path == 5 and ggen.path == 0
+    L = [nbc[d] * DIMS[d] for d in range(3)]
+    Uo = state_from(oplan, smooth_field(grid, DIMS, L))
+    Ud, Ug = torch.from_numpy(Uo).cuda(), torch.from_numpy(Uo).cuda()
+    dx = dx_of(grid)
+    dxd = torch.from_numpy(dx).cuda()
+    T0 = totals(oplan, grid, Uo, 3)
+    dts = gplan.fx_hydro_compute_dt(Ud, dxd, 0.3).clone()
+    Us = Ud.clone()
+    for step in range(10):
+        dt = oplan.compute_dt(Uo, dx, 0.3)
+        dtg = float(gplan.fx_hydro_compute_dt(Ud, dxd, 0.3).item())
+        assert abs(dtg - dt) <= 1e-13 * dt
+        oplan.advance(Uo, dx, dt)
+        gplan.fx_hydro_advance(Ud, dxd, dt)
+        ggen.fx_hydro_advance(Ug, dxd, dt)
+        if step < 3:  # fx_hydro_step: same states with the time step kept on the device (the reduction as a pass of its own)
+            assert abs(float(dts.item()) - dt) <= 1e-12 * dt
+            gplan.fx_hydro_step(Us, dxd, 0.3, dts)
+        if step in (0, 9):
+            err = rel_err(Cfg, gplan.interior(Ud).cpu().numpy(), oplan.interior(Uo))
+            assert err <= (1e-12 if step == 0 else 1e-9), (step, err)
+            assert rel_err(Cfg, gplan.interior(Ud).cpu().numpy(), ggen.interior(Ug).cpu().numpy()) <= (1e-12 if step == 0 else 1e-9)
+    if periodic:  # what leaves the fine blocks enters the coarse ones, whichever kernel advanced either
+        T1 = totals(oplan, grid, Ud.cpu().numpy(), 3)
+        scale = np.array([T0[0], 2.4 * T0[0], 2.4 * T0[0], 2.4 * T0[0], T0[4]])
+        assert np.max(np.abs(T1 - T0) / scale) <= 1e-13
+    fo, _ = oplan.status()
+    fg, _ = gplan.fx_hydro_status()
+    assert fo == fg == 0
+
+
+def test_hybrid_uniform_state_bitwise_and_chain_length():
+    grid = two_level_grid((4, 4, 4), CENTRE2, DIMS)
+    n = len(grid["level"])
+    shape = (n,) + DIMS
+    oplan = amr_plan(grid, DIMS)
+    dxd = torch.from_numpy(dx_of(grid)).cuda()
+    W = (1.3, 0.4, -0.7, 0.2, 0.9)
+    Uu = state_from(oplan, cons(*[np.full(shape, x) for x in W]))
+    L = [4 * 16] * 3
+    Usm = state_from(oplan, smooth_field(grid, DIMS, L))
+    results = []
+    for zc in (None, 1, 3, 8):
+        gplan = gpu_plan(grid, zchain=zc)
+        assert gplan.path == 5
+        U = torch.from_numpy(Uu).cuda()
+        U0 = gplan.interior(U).clone()
+        dt = gplan.fx_hydro_compute_dt(U, dxd, 0.3).clone()
+        for _ in range(4):
+            gplan.fx_hydro_step(U, dxd, 0.3, dt)
+        assert torch.equal(gplan.interior(U), U0)
+        V = torch.from_numpy(Usm).cuda()
+        dt = gplan.fx_hydro_compute_dt(V, dxd, 0.3).clone()
+        for _ in range(4):
+            gplan.fx_hydro_step(V, dxd, 0.3, dt)
+        results.append(gplan.interior(V).clone())
+    for r in results[1:]:
+        assert torch.equal(r, results[0])
+
+
+def test_every_block_with_a_jump_face_falls_back_to_generic_everywhere():
+    """A grid whose every block touches a jump leaves the fused kernel nothing: the plan reports the generic path."""
+    grid = two_level_grid((2, 1, 1), {(0, 0, 0)}, DIMS)  # the coarse block sees the refined one through both x faces
+    gplan = gpu_plan(grid)
+    assert gplan.path == 0
+    oplan = amr_plan(grid, DIMS)
+    Uo = state_from(oplan, smooth_field(grid, DIMS, [32, 16, 16]))
+    Ud = torch.from_numpy(Uo).cuda()
+    dx = dx_of(grid)
+    dt = oplan.compute_dt(Uo, dx, 0.3)
+    oplan.advance(Uo, dx, dt)
+    gplan.fx_hydro_advance(Ud, torch.from_numpy(dx).cuda(), dt)
+    assert rel_err(Cfg, gplan.interior(Ud).cpu().numpy(), oplan.interior(Uo)) <= 1e-12
