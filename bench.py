@@ -58,6 +58,8 @@ def parse_args():
     ap.add_argument("--wavespeed", type=int, default=0, help="FX_OPT_WAVESPEED: 0 Einfeldt (the reading the configs are run with [A8]), 1 Davis")
     ap.add_argument("--shard", action="store_true", help="drive the step through ShardedHydro even on one rank (the N > 1 code path with an "
                     "empty exchange; N > 1 always uses it)")
+    ap.add_argument("--amr", action="store_true", help="two-level grid of 16^3 blocks on config 5's domain (7680 blocks, 1736 of them with a "
+                    "refinement jump): the hybrid path (fused kernel + generic kernel at the jumps); --path 1 for all-generic")
     ap.add_argument("--ca", action="store_true", help="time the communication-avoiding step (fx_hydro_advance_ca, DESIGN.md B17: one guard fill "
                     "per step, generic kernels on a shrinking extension of the interior) + fx_hydro_compute_dt instead of fx_hydro_step")
     ap.add_argument("--no-e2e", action="store_true")
@@ -170,6 +172,53 @@ def build_workload(args, device):
         Ui[:, b0:b1] = inputs.with_scalars(cfg, coords[b0:b1], inputs.block_interiors(cfg, coords[b0:b1], device), args.scalars)
     dx = torch.from_numpy(inputs.dx_array(cfg)).to(device)
     return cfg, plan, U, dx, coords
+
+
+AMR_NBC, AMR_LO, AMR_HI = (16, 16, 16), (4, 4, 4), (12, 12, 12)  # --amr: coarse tiling and the refined box (coarse cells)
+
+
+def amr_config(inputs, nbc, nblocks):
+    """What the rest of bench.py reads from a config, for the two-level workload (config 5's scheme and field)."""
+    import types
+    fine = inputs.config(5, nb=tuple(2 * x for x in nbc))
+    return fine, types.SimpleNamespace(
+        number=5, name=f"two-level grid: {nbc[0]}x{nbc[1]}x{nbc[2]} coarse blocks, the central "
+                       f"{AMR_HI[0] - AMR_LO[0]}x{AMR_HI[1] - AMR_LO[1]}x{AMR_HI[2] - AMR_LO[2]} of them refined 2x (config 5's field and scheme)",
+        block_dims=fine.block_dims, nguard=fine.nguard, nb=nbc, bc="periodic", gamma=fine.gamma, recon=fine.recon,
+        riemann=fine.riemann, rk_order=fine.rk_order, cfl=fine.cfl, nblocks=nblocks, ndim=3,
+        interior_zones=nblocks * fine.block_dims[0] * fine.block_dims[1] * fine.block_dims[2])
+
+
+def build_amr_workload(args, device):
+    """--amr: a static two-level grid [DESIGN.md B12-B14] of 16^3 blocks on config 5's domain: 512^3 zones inside the refined
+    box, 256^3 outside; fine blocks hold config 5's field, coarse blocks its 2 x 2 x 2 means."""
+    import numpy as np
+    import torch
+    from paper_2208_11630_b200 import binding as fx
+    from paper_2208_11630_b200 import inputs
+    order = fx.ORDER_MORTON if args.order == "morton" else fx.ORDER_LEX
+    grid = inputs.two_level_tiling(AMR_NBC, AMR_LO, AMR_HI, order)
+    n = len(grid["level"])
+    fine, cfg = amr_config(inputs, AMR_NBC, n)
+    plan = fx.HydroPlan(cfg.block_dims, cfg.nguard, n, cfg.gamma, cfg.recon, cfg.riemann, cfg.rk_order, device=device)
+    plan.fx_hydro_plan_set_option(fx.OPT_PATH, args.path)
+    guard_x = args.guard_x if args.guard_x >= 0 else 8
+    if guard_x != cfg.nguard:
+        plan.fx_hydro_plan_set_option(fx.OPT_GUARD_X, guard_x)
+    if args.zchain:
+        plan.fx_hydro_plan_set_option(fx.OPT_ZCHAIN, args.zchain)
+    plan.fx_hydro_plan_set_refinement(grid["jump"])
+    plan.fx_hydro_plan_set_topology(grid["neigh"])
+    plan.fx_hydro_plan_set_workspace()
+    U = plan.alloc_state(fill=float("nan"))
+    Ui = plan.interior(U)
+    for b0 in range(0, n, 512):
+        b1 = min(n, b0 + 512)
+        Ui[:, b0:b1] = inputs.two_level_interiors(fine, grid, b0, b1, device)
+    dxf = fine.dx
+    dxh = np.where(grid["level"][:, None] == 1, 1.0, 2.0) * np.array(dxf)[None, :]
+    cfg.jump_blocks = int((grid["neigh"] <= inputs.NEIGH_COARSER).any(axis=1).sum())
+    return cfg, plan, U, torch.from_numpy(np.ascontiguousarray(dxh)).to(device), None
 
 
 def shard_factors(world):
@@ -325,7 +374,7 @@ def committed_traffic(cfg, args, plan):
     """dram__bytes_read.sum + dram__bytes_write.sum per stage launch (mean over the stages of a step) from the committed
     `ncu --set full` capture of this workload and path under profiles/, read by metric name; (None, None) if there is none."""
     per_stage = 1  # captured launches that make up one stage
-    if args.wavespeed or args.zchain or args.ca:
+    if args.wavespeed or args.zchain or args.ca or args.amr:
         return None, None
     if args.block == "8,8,8" and args.nb == "64,64,32" and not args.scalars:
         name = f"r2_ncu_config{cfg.number}_8cubed_path{plan.path}_raw.csv"
@@ -374,13 +423,15 @@ def run_ours(args, rank, world, local_rank):
         plan = sh.plan
         zones = sh.n_owned * cfg.block_dims[0] * cfg.block_dims[1] * cfg.block_dims[2]  # this rank's share
     else:
-        cfg, plan, U, dx, coords = build_workload(args, device)
+        cfg, plan, U, dx, coords = build_amr_workload(args, device) if args.amr else build_workload(args, device)
         zones = cfg.interior_zones
     stages = cfg.rk_order
     fused = plan.path in (1, 3, 4)
     # fused path: one launch per RK stage, the CFL reduction (a7) rides in the last one; tile and generic paths: one
     # stage kernel per stage, then the reduction pass; with passive scalars also their face fill per stage
     launches_per_step = stages if fused else (stages + 1 + (stages if args.scalars else 0))
+    if args.amr:  # per stage: guard zones behind the jumps, the stage kernel(s), the flux correction; then the reduction pass
+        launches_per_step = stages * (4 if plan.path == 5 else 3) + 1
     if sh is not None:
         launches_per_step += (int(sh.send_elems > 0) + int(sh.recv_elems > 0)) * stages  # pack + unpack of the cut-face slabs before every stage
         dt = sh.compute_dt(U, dx, cfg.cfl)  # the minimum over the ranks
@@ -462,7 +513,7 @@ def run_ours(args, rank, world, local_rank):
                 "frac": side["frac"], "traffic": traffic, "traffic_source": traffic_src,
                 "roof_ps_per_zone_stage": {"hbm": t_hbm * 1e12, "fp64": t_fp * 1e12 if flops is not None else None},
                 "hbm": hbm, "fp64": fp64,
-                "kernel": "generic stage kernel over the extended interior (communication-avoiding step)" if args.ca else {1: "fused stage kernel", 3: "fused stage kernel, pair variant", 4: "fused stage kernel on 2 x 2 bundles of 8 x 8 blocks", 2: "tile stage kernel", 0: "generic stage kernel"}[plan.path],
+                "kernel": "generic stage kernel over the extended interior (communication-avoiding step)" if args.ca else {5: "fused stage kernel + generic stage kernel at the refinement jumps", 1: "fused stage kernel", 3: "fused stage kernel, pair variant", 4: "fused stage kernel on 2 x 2 bundles of 8 x 8 blocks", 2: "tile stage kernel", 0: "generic stage kernel"}[plan.path],
                 "kernel_ms_avg": stage_avg_ms, "kernel_launches_timed": stage_launches,
                 "kernel_share_of_step": stage_ms / ms if ms > 0 else None}
 
@@ -476,7 +527,7 @@ def run_ours(args, rank, world, local_rank):
                                    + (", Davis wave speeds" if args.wavespeed else ""),
                        "interior_zones": zones, "state_bytes": plan.bytes_per_state, "block_order": args.order,
                        "layout": f"x guard depth {plan.gd[0]} (row pitch {plan.S_j * 8} B), y/z guard depth {plan.gd[1]}/{plan.gd[2]}",
-                       "path": "communication-avoiding step (one guard fill per step; generic kernels on the extended interior)" if args.ca else {0: "generic", 1: "fused (TMA)", 2: "tile (shared-memory block)", 3: "fused (TMA), two zones per thread", 4: "fused (TMA), 2 x 2 bundles of 8 x 8 blocks"}[plan.path], "l2": "inputs (state) larger than L2; no flush needed",
+                       "path": "communication-avoiding step (one guard fill per step; generic kernels on the extended interior)" if args.ca else {0: "generic", 5: f"fused (TMA) on the blocks without a refinement jump + generic on the {getattr(cfg, 'jump_blocks', 0)} blocks with one", 1: "fused (TMA)", 2: "tile (shared-memory block)", 3: "fused (TMA), two zones per thread", 4: "fused (TMA), 2 x 2 bundles of 8 x 8 blocks"}[plan.path], "l2": "inputs (state) larger than L2; no flush needed",
                        "multi_gpu": (f"sharded: tiling {cfg.nb[0]}x{cfg.nb[1]}x{cfg.nb[2]} blocks in {world} contiguous Morton runs, "
                                      f"{sh.shard.n_ghost} ghost blocks on rank 0, cut-face slabs exchanged before every stage "
                                      f"(grouped NCCL send/recv, {sh.send_elems * 8} B sent by rank 0 per stage), dt = all-reduce(min)")
@@ -560,6 +611,10 @@ def run_ours(args, rank, world, local_rank):
 
 def main():
     args = parse_args()
+    if args.amr:
+        args.no_cpu_baseline = True  # (the oracle's two-level runs are in tests/; its timed sample is the uniform workload's)
+        if args.gpus > 1 or args.shard or args.scalars or args.ca or args.nb or args.block or args.config != 5:
+            sys.exit("--amr: single plan, config 5's scheme and field, five variables")
     if args.ca:
         args.no_e2e = True  # the end-to-end call (fx_hydro_advance_host_interior) runs the standard step
         if args.gpus > 1 or args.shard or args.scalars:

@@ -324,3 +324,93 @@ def neighbourhood(cfg: Config, centre, radius: int):
             for ox in rng[0]:
                 out.append([(centre[0] + ox) % cfg.nb[0], (centre[1] + oy) % cfg.nb[1], (centre[2] + oz) % cfg.nb[2]])
     return np.asarray(out, np.int32), tuple(len(r) for r in rng)
+
+
+# ------------------------------------------------------------------ static two-level grids (B12; bench.py --amr)
+NEIGH_COARSER, NEIGH_FINER = -4, -5
+
+
+def two_level_tiling(nbc, lo, hi, order=ORDER_MORTON):
+    """A 3-D periodic two-level block grid: the coarse tiling nbc = (cx, cy, cz), the coarse cells of the box [lo, hi)
+    replaced by their 8 children.  Tables as include/fx_hydro.h defines them: neigh int32 [n, 6] (same-level id,
+    NEIGH_COARSER or NEIGH_FINER), jump int32 [n, 6, 4] (behind NEIGH_FINER the four children that touch the face, index =
+    first transverse half + 2 x second transverse half, transverse dimensions ascending; behind NEIGH_COARSER the coarse
+    block and the index of the quarter of its face this block covers).  Block order: the coarse cells in `order`, a refined
+    cell's children in place, x fastest.  Returns dict(neigh, jump, level [n], fine [n, 3]: the block's coordinates in the
+    FINE tiling (a coarse block: those of its first child))."""
+    nbc, lo, hi = tuple(nbc), tuple(lo), tuple(hi)
+    refined = lambda c: all(lo[d] <= c[d] < hi[d] for d in range(3))  # noqa: E731
+    ident, level, fine = {}, [], []
+    for c in block_coords(nbc, order):
+        c = tuple(int(x) for x in c)
+        if refined(c):
+            for cz in range(2):
+                for cy in range(2):
+                    for cx in range(2):
+                        ident[(c, (cx, cy, cz))] = len(level)
+                        level.append(1)
+                        fine.append((2 * c[0] + cx, 2 * c[1] + cy, 2 * c[2] + cz))
+        else:
+            ident[(c, None)] = len(level)
+            level.append(0)
+            fine.append((2 * c[0], 2 * c[1], 2 * c[2]))
+    n = len(level)
+    neigh = np.empty((n, 6), np.int32)
+    jump = np.full((n, 6, 4), -1, np.int32)
+    for (c, ch), b in ident.items():
+        for d in range(3):
+            t1, t2 = [e for e in range(3) if e != d]
+            for side in (0, 1):
+                f = 2 * d + side
+                if ch is not None and ch[d] != side:  # the sibling inside the same parent
+                    sib = list(ch)
+                    sib[d] = side
+                    neigh[b, f] = ident[(c, tuple(sib))]
+                    continue
+                nc = list(c)
+                nc[d] = (nc[d] + (1 if side else -1)) % nbc[d]
+                nc = tuple(nc)
+                if ch is None:
+                    if not refined(nc):
+                        neigh[b, f] = ident[(nc, None)]
+                    else:
+                        neigh[b, f] = NEIGH_FINER
+                        for q in range(4):
+                            kid = [0, 0, 0]
+                            kid[d] = 1 - side  # the children that touch our face
+                            kid[t1], kid[t2] = q & 1, q >> 1
+                            jump[b, f, q] = ident[(nc, tuple(kid))]
+                else:
+                    if refined(nc):
+                        kid = list(ch)
+                        kid[d] = 1 - side
+                        neigh[b, f] = ident[(nc, tuple(kid))]
+                    else:
+                        neigh[b, f] = NEIGH_COARSER
+                        jump[b, f, 0] = ident[(nc, None)]
+                        jump[b, f, 1] = ch[t1] + 2 * ch[t2]
+    return dict(neigh=neigh, jump=jump, level=np.array(level, np.int32), fine=np.array(fine, np.int32))
+
+
+def two_level_interiors(cfg_fine: Config, grid, b0, b1, device="cpu") -> torch.Tensor:
+    """Conserved interiors [5, b1 - b0, nz, ny, nx] of blocks [b0, b1) of a two_level_tiling whose FINE tiling is cfg_fine's:
+    a fine block holds cfg_fine's field, a coarse block the plain means over the 2 x 2 x 2 fine zones each of its zones
+    covers (input recipe only: a coarse field consistent with the fine one)."""
+    n = cfg_fine.block_dims
+    out = torch.empty((5, b1 - b0, n[2], n[1], n[0]), dtype=torch.float64, device=device)
+    lev, fine = grid["level"][b0:b1], grid["fine"][b0:b1]
+    isf = np.nonzero(lev == 1)[0]
+    if len(isf):
+        out[:, torch.as_tensor(isf, device=device)] = block_interiors(cfg_fine, fine[isf], device)
+    isc = np.nonzero(lev == 0)[0]
+    if len(isc):
+        acc = torch.zeros((5, len(isc), n[2], n[1], n[0]), dtype=torch.float64, device=device)
+        h = [m // 2 for m in n]
+        for cz in range(2):
+            for cy in range(2):
+                for cx in range(2):
+                    kids = block_interiors(cfg_fine, fine[isc] + np.array([cx, cy, cz], np.int32), device)
+                    pooled = kids.reshape(5, len(isc), h[2], 2, h[1], 2, h[0], 2).sum(dim=(3, 5, 7))
+                    acc[:, :, cz * h[2]:(cz + 1) * h[2], cy * h[1]:(cy + 1) * h[1], cx * h[0]:(cx + 1) * h[0]] = pooled
+        out[:, torch.as_tensor(isc, device=device)] = acc * 0.125
+    return out
