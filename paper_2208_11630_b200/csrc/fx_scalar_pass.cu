@@ -136,7 +136,8 @@ __global__ void __launch_bounds__(256, 2) fx_k_scalar_march(const FxParams P, co
   for (int f = 0; f < 6; ++f) nb[f] = __ldg(&P.neigh[(long long)b * 6 + f]);
   const long long colo = (long long)(j + g1) * P.S_j + (i + g0);  // this column inside a block's plane
   const long long nzt = P.nblocks * (long long)nz * 256;
-  const double *Q0 = X + (long long)sv0 * P.S_v;
+  const double *Q0 = X + (long long)sv0 * P.S_v, *U0q = U0 + (long long)sv0 * P.S_v;
+  double *outq = out + (long long)sv0 * P.S_v;
   auto plane_off = [&](int k) -> long long {  // this column's zone in plane k of the column (k in [-2, nz + 2))
     const int blk = k < 0 ? nb[4] : (k >= nz ? nb[5] : b);
     const int kk = k < 0 ? k + nz : (k >= nz ? k - nz : k);
@@ -151,40 +152,57 @@ __global__ void __launch_bounds__(256, 2) fx_k_scalar_march(const FxParams P, co
   const int hxc = i < 2 ? i : i + 4, hyr = j < 2 ? j : j + 4;
   const long long zb = (long long)b * nz * 256 + tid;
   const long long zxh = (long long)nb[1] * nz * 256 + j * 16, zyh = (long long)nb[3] * nz * 256 + i;
-  // everything plane k needs before its barrier, into stage k & 1
-  auto prefetch = [&](int k) {
-    const int st = k & 1;
-    const long long e = plane_off(k + 2);
-    cp_async8(&S.raw[st][0][tid], X + e);
+  // everything plane k needs before its barrier, into stage k & 1.  All addresses are running 64-bit offsets advanced by
+  // one plane per call (the planes are prefetched in turn, k = 0, 1, ...): forming them from k each time cost a quarter of
+  // the loop's instructions (215 of 847 integer instructions per plane were address arithmetic)
+  const long long top0 = plane_off(nz);      // the column's first zone in the block above
+  long long e_pf = plane_off(2);              // new window cell of the plane being prefetched
+  long long ko_pf = (long long)g2 * P.S_k;    // that plane inside a neighbour block (halo cells)
+  long long zi_pf = zb;                       // this thread's zone of that plane in fq
+  const long long dzx = zxh - zb, dzy = zyh - zb;
+  int kp = 0;                                 // the plane being prefetched
+  auto prefetch = [&]() {
+    const int st = kp & 1;
+    {
+      const double *p = Q0 + e_pf;
+      cp_async8(&S.raw[st][0][tid], X + e_pf);
 #pragma unroll
-    for (int s = 0; s < NSC; ++s) cp_async8(&S.raw[st][1 + s][tid], Q0 + s * P.S_v + e);
-    const long long ko = (long long)(k + g2) * P.S_k;
+      for (int s = 0; s < NSC; ++s, p += P.S_v) cp_async8(&S.raw[st][1 + s][tid], p);
+    }
     if (hx) {
-      cp_async8(&S.hal[st][0][hxs], X + ko + hxo);
+      const long long o = ko_pf + hxo;
+      const double *p = Q0 + o;
+      cp_async8(&S.hal[st][0][hxs], X + o);
 #pragma unroll
-      for (int s = 0; s < NSC; ++s) cp_async8(&S.hal[st][1 + s][hxs], Q0 + s * P.S_v + ko + hxo);
+      for (int s = 0; s < NSC; ++s, p += P.S_v) cp_async8(&S.hal[st][1 + s][hxs], p);
     }
     if (hy) {
-      cp_async8(&S.hal[st][0][hys], X + ko + hyo);
+      const long long o = ko_pf + hyo;
+      const double *p = Q0 + o;
+      cp_async8(&S.hal[st][0][hys], X + o);
 #pragma unroll
-      for (int s = 0; s < NSC; ++s) cp_async8(&S.hal[st][1 + s][hys], Q0 + s * P.S_v + ko + hyo);
+      for (int s = 0; s < NSC; ++s, p += P.S_v) cp_async8(&S.hal[st][1 + s][hys], p);
     }
-    const long long zi = zb + (long long)k * 256;
-    cp_async8(&S.fx[st][0][j][i], P.fq + zi);
-    if (!HLLC) cp_async8(&S.fx[st][1][j][i], P.fq + nzt + zi);
-    cp_async8(&S.fy[st][0][j][i], P.fq + 2 * nzt + zi);
-    if (!HLLC) cp_async8(&S.fy[st][1][j][i], P.fq + 3 * nzt + zi);
+    const double *f = P.fq + zi_pf;
+    cp_async8(&S.fx[st][0][j][i], f);
+    if (!HLLC) cp_async8(&S.fx[st][1][j][i], f + nzt);
+    cp_async8(&S.fy[st][0][j][i], f + 2 * nzt);
+    if (!HLLC) cp_async8(&S.fy[st][1][j][i], f + 3 * nzt);
     if (i == 15) {
-      cp_async8(&S.fx[st][0][j][16], P.fq + zxh + (long long)k * 256);
-      if (!HLLC) cp_async8(&S.fx[st][1][j][16], P.fq + nzt + zxh + (long long)k * 256);
+      cp_async8(&S.fx[st][0][j][16], f + dzx);
+      if (!HLLC) cp_async8(&S.fx[st][1][j][16], f + dzx + nzt);
     }
     if (j == 15) {
-      cp_async8(&S.fy[st][0][16][i], P.fq + 2 * nzt + zyh + (long long)k * 256);
-      if (!HLLC) cp_async8(&S.fy[st][1][16][i], P.fq + 3 * nzt + zyh + (long long)k * 256);
+      cp_async8(&S.fy[st][0][16][i], f + dzy + 2 * nzt);
+      if (!HLLC) cp_async8(&S.fy[st][1][16][i], f + dzy + 3 * nzt);
     }
     cp_async_commit();
+    ++kp;
+    e_pf = (kp + 2 == nz) ? top0 : e_pf + P.S_k;
+    ko_pf += P.S_k;
+    zi_pf += 256;
   };
-  prefetch(0);
+  prefetch();
   if (dt_dev) dt = *dt_dev;
   const double rd0 = dt / __ldg(&dx[b * 3 + 0]), rd1 = dt / __ldg(&dx[b * 3 + 1]), rd2 = dt / __ldg(&dx[b * 3 + 2]);
   // abundances: (rho X_s) / max(rho, floor), the reciprocal as the hydro part forms it
@@ -221,8 +239,13 @@ __global__ void __launch_bounds__(256, 2) fx_k_scalar_march(const FxParams P, co
     }
   }
   unsigned hit = 0;
+  int hmax = 0;  // largest upper word (sign cleared) of the results: Inf / NaN anywhere in a flux reaches the result
+  // this thread's zone of the current plane: in fq (zone of the plane above: the z face's data) and in the state arrays
+  const double *fz = P.fq + 4 * nzt + zb;
+  const long long ztop = 4 * nzt + (long long)nb[5] * nz * 256 + tid;
+  long long c = (long long)b * P.S_b + (long long)g2 * P.S_k + colo;
 #pragma unroll 1
-  for (int k = 0; k < nz; ++k) {
+  for (int k = 0; k < nz; ++k, c += P.S_k) {
     const int buf = k & 1;
     cp_async_wait_all();  // this thread's part of stage k
     double xn[NSC];
@@ -251,17 +274,19 @@ __global__ void __launch_bounds__(256, 2) fx_k_scalar_march(const FxParams P, co
       for (int s = 0; s < NSC; ++s) S.XS[buf][s][hyr][i + 2] = yh[s];
     }
     __syncthreads();  // plane k's X and (F_rho, Aq) complete; every thread is done with plane k-1 (stage buf ^ 1)
-    if (k + 1 < nz) prefetch(k + 1);
-    const long long zi = zb + (long long)k * 256;
-    const long long zzh = k + 1 < nz ? zi + 256 : (long long)nb[5] * nz * 256 + tid;
-    const double Fzh = P.fq[4 * nzt + zzh], Azh = HLLC ? fx_aq_hllc(Fzh) : P.fq[5 * nzt + zzh];
-    const long long c = (long long)b * P.S_b + (long long)(k + g2) * P.S_k + colo;
+    if (k + 1 < nz) prefetch();
+    fz = k + 1 < nz ? fz + 256 : P.fq + ztop;
+    const double Fzh = fz[0], Azh = HLLC ? fx_aq_hllc(Fzh) : fz[nzt];
     double u0[NSC], xs[NSC];
+    {
+      const double *pu = U0q + c, *px = Q0 + c;
 #pragma unroll
-    for (int s = 0; s < NSC; ++s) {
-      u0[s] = U0[(long long)(sv0 + s) * P.S_v + c];
-      if (!FIRST) xs[s] = Q0[s * P.S_v + c];
+      for (int s = 0; s < NSC; ++s, pu += P.S_v, px += P.S_v) {
+        u0[s] = *pu;
+        if (!FIRST) xs[s] = *px;
+      }
     }
+    double *po = outq + c;
     const double F0[2] = {S.fx[buf][0][j][i], S.fx[buf][0][j][i + 1]}, F1[2] = {S.fy[buf][0][j][i], S.fy[buf][0][j + 1][i]};
     double A0[2], A1[2];
     if (HLLC) {
@@ -277,32 +302,34 @@ __global__ void __launch_bounds__(256, 2) fx_k_scalar_march(const FxParams P, co
       for (int n = 0; n < 3; ++n) fx_plm(x[n], x[n + 1], x[n + 2], am[n], ap[n]);
       const double Fm = Ad[0] * ap[0] + (Fd[0] - Ad[0]) * am[1];
       const double Fp = Ad[1] * ap[1] + (Fd[1] - Ad[1]) * am[2];
-      if (!(fabs(Fm + Fp) <= 1.79e308)) hit |= FX_STATUS_NONFINITE;
       return rd * (Fp - Fm);
     };
 #pragma unroll
     for (int s = 0; s < NSC; ++s) {
       double x[5], Ss = 0.0;
 #pragma unroll
-      for (int m = 0; m < 5; ++m) x[m] = S.XS[buf][s][j + 2][i + m];
+      for (int m = 0; m < 5; ++m) x[m] = m == 2 ? xw[0][s] : S.XS[buf][s][j + 2][i + m];  // (the centre is in the z window)
       Ss += flux(x, rd0, F0, A0);
 #pragma unroll
-      for (int m = 0; m < 5; ++m) x[m] = S.XS[buf][s][j + m][i + 2];
+      for (int m = 0; m < 5; ++m) x[m] = m == 2 ? xw[0][s] : S.XS[buf][s][j + m][i + 2];
       Ss += flux(x, rd1, F1, A1);
       {  // z: the new face only
         double amn, apn;
         fx_plm(xw[0][s], xw[1][s], xn[s], amn, apn);
         const double Fp = Azh * apc[s] + (Fzh - Azh) * amn;
-        if (!(fabs(Fz[s] + Fp) <= 1.79e308)) hit |= FX_STATUS_NONFINITE;
         Ss += rd2 * (Fp - Fz[s]);
         Fz[s] = Fp;
         apc[s] = apn;
         xw[0][s] = xw[1][s];
         xw[1][s] = xn[s];
       }
-      out[(long long)(sv0 + s) * P.S_v + c] = FIRST ? (u0[s] - Ss) : (u0[s] + beta * ((xs[s] - u0[s]) - Ss));
+      const double res = FIRST ? (u0[s] - Ss) : (u0[s] + beta * ((xs[s] - u0[s]) - Ss));
+      *po = res;
+      po += P.S_v;
+      hmax = max(hmax, __double2hiint(res) & 0x7fffffff);
     }
   }
+  if (hmax >= 0x7ff00000) hit |= FX_STATUS_NONFINITE;
   if (hit) fx_note(P, hit);
 }
 
