@@ -95,14 +95,27 @@ __global__ void __launch_bounds__(128) fx_k_scalar_pass(const FxParams P, const 
 // needs from HBM before that barrier -- the new cell of each window (rho, rho X_s), the halo cells' (rho, rho X_s), the
 // faces' (F_rho, Aq) of the x and y directions -- is fetched one plane ahead with cp.async into a two-stage buffer (each
 // thread reads back what it fetched itself, except the high faces' (F_rho, Aq), which are the next zone's low-face values:
-// read from the neighbour's slot after the barrier instead of a second time from memory); U0, the stage input and the z
-// face's (F_rho, Aq) are plain loads issued right after the barrier and consumed at the end of the plane.  Up to NSC = 4
+// read from the neighbour's slot after the barrier instead of a second time from memory), and so are U0 and the z face's
+// (F_rho, Aq), which only the end of the plane needs but which come from DRAM; the stage input's own zone (fetched two
+// planes earlier as a window cell: an L2 hit) is a plain load issued right after the barrier and used last.  Up to NSC = 4
 // scalars per launch share the densities and the (F_rho, Aq).  Arithmetic: the expressions of fx_k_scalar_pass.
-// (Measured, config 5 with 4 scalars, this pass alone: 10.8 ms with every load at the top of the plane and 184 registers
-// (one CTA per SM); 7.4 ms with the z carry and 128 registers (two CTAs); the cp.async form below 5.1 ms in the first stage
-// and 7.5 ms in the later ones, which also read U0.  Staging U0, the zone's own rho X_s (a four-slot ring) and the z face's
-// F_rho through cp.async as well -- no plain load left in the loop, 114.7 KB, still two CTAs -- was SLOWER (25.6 against
-// 24.0 ms per step): the pass is bound by the load / store unit's instruction rate, not by exposed latency.)
+// Measured, config 5 with 4 scalars, whole step (fused kernel + this pass, two stages):
+//   * every load at the top of the plane, 184 registers, one CTA per SM: this pass alone 10.8 ms per stage; the z carry and
+//     128 registers (two CTAs): 7.4 ms; cp.async staging one plane ahead: 5.1 ms (first stage) / 7.5 ms (later ones) --
+//     24.4 ms per step.  At that point ncu showed as many instructions as the hydro kernel issues (3.5 G per launch, 847
+//     SASS instructions per plane and thread, 215 of them 64-bit address arithmetic), 60 % of the issue slots busy.
+//   * running 64-bit offsets advanced by one plane per prefetch instead of addresses formed from k, the stencil's centre
+//     from the z window, the non-finite test on the result's upper word: 758 instructions, 22.3 ms per step.
+//   * two planes per loop trip (constant staging index, no register moves for the carried values): 666 instructions, but
+//     22.6 ms: no longer bound by the issue rate.  ncu's stall samples: 35 % long-scoreboard, nearly all at the first uses
+//     of U0 and of the z face's F_rho (plain loads issued after the barrier).
+//   * those two staged through cp.async with the rest of the plane (this version): 21.6 ms per step.  Loading them one
+//     plane ahead into registers instead: 24.5 ms (15 spill loads per plane at 128 registers).
+//   * every cell's PLM face values formed once and shared through shared memory (three evaluations per scalar and zone
+//     instead of seven; the cells beyond the block faces by one extra evaluation per warp; single-buffered arrays and two
+//     barriers per plane, since double-buffering them does not fit two CTAs per SM): 640 instructions per plane, 23.3 ms
+//     without and 24.8 ms with the staging above -- the second barrier costs more than the 28 % fewer instructions save;
+//     a ninth warp for the outer cells: 96 registers, 37 spill instructions per plane.  Not kept.
 template <int NSC>
 struct ScalSmem {
   double XS[2][NSC][20][20];      // abundances of the plane with halo
@@ -110,6 +123,7 @@ struct ScalSmem {
   double hal[2][1 + NSC][128];    // (rho, rho X_s) of the halo cells: 64 x-halo cells, 64 y-halo cells
   double fx[2][2][16][17];        // (F_rho, Aq) of the low x faces of zones i = 0 .. 16 (16: the x+ neighbour's first zone)
   double fy[2][2][17][16];        // the same along y
+  double late[2][NSC + 2][256];   // U0 of the plane's zones and the (F_rho, Aq) of their high z faces, per thread
 };
 
 __device__ __forceinline__ void cp_async8(void *dst, const void *src) {
@@ -160,8 +174,9 @@ __global__ void __launch_bounds__(256, 2) fx_k_scalar_march(const FxParams P, co
   long long ko_pf = (long long)g2 * P.S_k;    // that plane inside a neighbour block (halo cells)
   long long zi_pf = zb;                       // this thread's zone of that plane in fq
   const long long dzx = zxh - zb, dzy = zyh - zb;
-  int kp = 0;                                 // the plane being prefetched
-  auto prefetch = [&]() {
+  long long c_pf = (long long)b * P.S_b + (long long)g2 * P.S_k + colo;  // this thread's zone of that plane in the state arrays
+  const long long dztop = 4 * nzt + (long long)nb[5] * nz * 256 + tid;
+  auto prefetch = [&](int kp) {  // called for kp = 0, 1, 2, ... in turn
     const int st = kp & 1;
     {
       const double *p = Q0 + e_pf;
@@ -196,13 +211,21 @@ __global__ void __launch_bounds__(256, 2) fx_k_scalar_march(const FxParams P, co
       cp_async8(&S.fy[st][0][16][i], f + dzy + 2 * nzt);
       if (!HLLC) cp_async8(&S.fy[st][1][16][i], f + dzy + 3 * nzt);
     }
+    {  // what only the end of the plane needs (it comes from DRAM: fetched a plane ahead like the rest)
+      const double *pu = U0q + c_pf;
+#pragma unroll
+      for (int s = 0; s < NSC; ++s, pu += P.S_v) cp_async8(&S.late[st][s][tid], pu);
+      const double *fzh = kp + 1 < nz ? f + 4 * nzt + 256 : P.fq + dztop;
+      cp_async8(&S.late[st][NSC][tid], fzh);
+      if (!HLLC) cp_async8(&S.late[st][NSC + 1][tid], fzh + nzt);
+    }
     cp_async_commit();
-    ++kp;
-    e_pf = (kp + 2 == nz) ? top0 : e_pf + P.S_k;
+    e_pf = (kp + 3 == nz) ? top0 : e_pf + P.S_k;
+    c_pf += P.S_k;
     ko_pf += P.S_k;
     zi_pf += 256;
   };
-  prefetch();
+  prefetch(0);
   if (dt_dev) dt = *dt_dev;
   const double rd0 = dt / __ldg(&dx[b * 3 + 0]), rd1 = dt / __ldg(&dx[b * 3 + 1]), rd2 = dt / __ldg(&dx[b * 3 + 2]);
   // abundances: (rho X_s) / max(rho, floor), the reciprocal as the hydro part forms it
@@ -241,10 +264,8 @@ __global__ void __launch_bounds__(256, 2) fx_k_scalar_march(const FxParams P, co
   unsigned hit = 0;
   int hmax = 0;  // largest upper word (sign cleared) of the results: Inf / NaN anywhere in a flux reaches the result
   // this thread's zone of the current plane: in fq (zone of the plane above: the z face's data) and in the state arrays
-  const double *fz = P.fq + 4 * nzt + zb;
-  const long long ztop = 4 * nzt + (long long)nb[5] * nz * 256 + tid;
   long long c = (long long)b * P.S_b + (long long)g2 * P.S_k + colo;
-#pragma unroll 1
+#pragma unroll 2  // (two planes per trip: the staging buffer's index is a constant, the carried values rotate without moves)
   for (int k = 0; k < nz; ++k, c += P.S_k) {
     const int buf = k & 1;
     cp_async_wait_all();  // this thread's part of stage k
@@ -274,17 +295,13 @@ __global__ void __launch_bounds__(256, 2) fx_k_scalar_march(const FxParams P, co
       for (int s = 0; s < NSC; ++s) S.XS[buf][s][hyr][i + 2] = yh[s];
     }
     __syncthreads();  // plane k's X and (F_rho, Aq) complete; every thread is done with plane k-1 (stage buf ^ 1)
-    if (k + 1 < nz) prefetch();
-    fz = k + 1 < nz ? fz + 256 : P.fq + ztop;
-    const double Fzh = fz[0], Azh = HLLC ? fx_aq_hllc(Fzh) : fz[nzt];
-    double u0[NSC], xs[NSC];
-    {
-      const double *pu = U0q + c, *px = Q0 + c;
+    if (k + 1 < nz) prefetch(k + 1);
+    const double Fzh = S.late[buf][NSC][tid], Azh = HLLC ? fx_aq_hllc(Fzh) : S.late[buf][NSC + 1][tid];
+    double xs[NSC];
+    if (!FIRST) {
+      const double *px = Q0 + c;
 #pragma unroll
-      for (int s = 0; s < NSC; ++s, pu += P.S_v, px += P.S_v) {
-        u0[s] = *pu;
-        if (!FIRST) xs[s] = *px;
-      }
+      for (int s = 0; s < NSC; ++s, px += P.S_v) xs[s] = *px;
     }
     double *po = outq + c;
     const double F0[2] = {S.fx[buf][0][j][i], S.fx[buf][0][j][i + 1]}, F1[2] = {S.fy[buf][0][j][i], S.fy[buf][0][j + 1][i]};
@@ -304,6 +321,7 @@ __global__ void __launch_bounds__(256, 2) fx_k_scalar_march(const FxParams P, co
       const double Fp = Ad[1] * ap[1] + (Fd[1] - Ad[1]) * am[2];
       return rd * (Fp - Fm);
     };
+    double Sv[NSC];
 #pragma unroll
     for (int s = 0; s < NSC; ++s) {
       double x[5], Ss = 0.0;
@@ -323,7 +341,13 @@ __global__ void __launch_bounds__(256, 2) fx_k_scalar_march(const FxParams P, co
         xw[0][s] = xw[1][s];
         xw[1][s] = xn[s];
       }
-      const double res = FIRST ? (u0[s] - Ss) : (u0[s] + beta * ((xs[s] - u0[s]) - Ss));
+      Sv[s] = Ss;
+    }
+#pragma unroll
+    for (int s = 0; s < NSC; ++s) {
+      const double Ss = Sv[s];
+      const double u0 = S.late[buf][s][tid];
+      const double res = FIRST ? (u0 - Ss) : (u0 + beta * ((xs[s] - u0) - Ss));
       *po = res;
       po += P.S_v;
       hmax = max(hmax, __double2hiint(res) & 0x7fffffff);
