@@ -171,12 +171,13 @@ __global__ void __launch_bounds__(256, 2) fx_k_scalar_march(const FxParams P, co
   // the loop's instructions (215 of 847 integer instructions per plane were address arithmetic)
   const long long top0 = plane_off(nz);      // the column's first zone in the block above
   long long e_pf = plane_off(2);              // new window cell of the plane being prefetched
-  long long ko_pf = (long long)g2 * P.S_k;    // that plane inside a neighbour block (halo cells)
-  long long zi_pf = zb;                       // this thread's zone of that plane in fq
   const long long dzx = zxh - zb, dzy = zyh - zb;
-  long long c_pf = (long long)b * P.S_b + (long long)g2 * P.S_k + colo;  // this thread's zone of that plane in the state arrays
+  // (the other offsets of a plane follow from its own-zone offset cpf and from kp: fewer values carried across the loop --
+  // the spilled piece of one of them, reloaded from local memory behind the streaming cp.async traffic, was 10 % of the
+  // stall samples)
+  const long long hxr = hxo - ((long long)b * P.S_b + colo), hyr_o = hyo - ((long long)b * P.S_b + colo);
   const long long dztop = 4 * nzt + (long long)nb[5] * nz * 256 + tid;
-  auto prefetch = [&](int kp) {  // called for kp = 0, 1, 2, ... in turn
+  auto prefetch = [&](int kp, long long cpf) {  // called for kp = 0, 1, 2, ... in turn; cpf: this thread's zone of plane kp
     const int st = kp & 1;
     {
       const double *p = Q0 + e_pf;
@@ -185,20 +186,20 @@ __global__ void __launch_bounds__(256, 2) fx_k_scalar_march(const FxParams P, co
       for (int s = 0; s < NSC; ++s, p += P.S_v) cp_async8(&S.raw[st][1 + s][tid], p);
     }
     if (hx) {
-      const long long o = ko_pf + hxo;
+      const long long o = cpf + hxr;
       const double *p = Q0 + o;
       cp_async8(&S.hal[st][0][hxs], X + o);
 #pragma unroll
       for (int s = 0; s < NSC; ++s, p += P.S_v) cp_async8(&S.hal[st][1 + s][hxs], p);
     }
     if (hy) {
-      const long long o = ko_pf + hyo;
+      const long long o = cpf + hyr_o;
       const double *p = Q0 + o;
       cp_async8(&S.hal[st][0][hys], X + o);
 #pragma unroll
       for (int s = 0; s < NSC; ++s, p += P.S_v) cp_async8(&S.hal[st][1 + s][hys], p);
     }
-    const double *f = P.fq + zi_pf;
+    const double *f = P.fq + zb + ((long long)kp << 8);
     cp_async8(&S.fx[st][0][j][i], f);
     if (!HLLC) cp_async8(&S.fx[st][1][j][i], f + nzt);
     cp_async8(&S.fy[st][0][j][i], f + 2 * nzt);
@@ -212,7 +213,7 @@ __global__ void __launch_bounds__(256, 2) fx_k_scalar_march(const FxParams P, co
       if (!HLLC) cp_async8(&S.fy[st][1][16][i], f + dzy + 3 * nzt);
     }
     {  // what only the end of the plane needs (it comes from DRAM: fetched a plane ahead like the rest)
-      const double *pu = U0q + c_pf;
+      const double *pu = U0q + cpf;
 #pragma unroll
       for (int s = 0; s < NSC; ++s, pu += P.S_v) cp_async8(&S.late[st][s][tid], pu);
       const double *fzh = kp + 1 < nz ? f + 4 * nzt + 256 : P.fq + dztop;
@@ -221,11 +222,8 @@ __global__ void __launch_bounds__(256, 2) fx_k_scalar_march(const FxParams P, co
     }
     cp_async_commit();
     e_pf = (kp + 3 == nz) ? top0 : e_pf + P.S_k;
-    c_pf += P.S_k;
-    ko_pf += P.S_k;
-    zi_pf += 256;
   };
-  prefetch(0);
+  prefetch(0, (long long)b * P.S_b + (long long)g2 * P.S_k + colo);
   if (dt_dev) dt = *dt_dev;
   const double rd0 = dt / __ldg(&dx[b * 3 + 0]), rd1 = dt / __ldg(&dx[b * 3 + 1]), rd2 = dt / __ldg(&dx[b * 3 + 2]);
   // abundances: (rho X_s) / max(rho, floor), the reciprocal as the hydro part forms it
@@ -295,7 +293,7 @@ __global__ void __launch_bounds__(256, 2) fx_k_scalar_march(const FxParams P, co
       for (int s = 0; s < NSC; ++s) S.XS[buf][s][hyr][i + 2] = yh[s];
     }
     __syncthreads();  // plane k's X and (F_rho, Aq) complete; every thread is done with plane k-1 (stage buf ^ 1)
-    if (k + 1 < nz) prefetch(k + 1);
+    if (k + 1 < nz) prefetch(k + 1, c + P.S_k);
     const double Fzh = S.late[buf][NSC][tid], Azh = HLLC ? fx_aq_hllc(Fzh) : S.late[buf][NSC + 1][tid];
     double xs[NSC];
     if (!FIRST) {
