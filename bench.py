@@ -59,7 +59,7 @@ def parse_args():
     ap.add_argument("--shard", action="store_true", help="drive the step through ShardedHydro even on one rank (the N > 1 code path with an "
                     "empty exchange; N > 1 always uses it)")
     ap.add_argument("--amr", action="store_true", help="two-level grid of 16^3 blocks on config 5's domain (7680 blocks, 1736 of them with a "
-                    "refinement jump): the hybrid path (fused kernel + generic kernel at the jumps); --path 1 for all-generic")
+                    "refinement jump): the fused kernel on every block (path 5; the blocks at the jumps read their own guard zones); --path 1 for all-generic")
     ap.add_argument("--ca", action="store_true", help="time the communication-avoiding step (fx_hydro_advance_ca, DESIGN.md B17: one guard fill "
                     "per step, generic kernels on a shrinking extension of the interior) + fx_hydro_compute_dt instead of fx_hydro_step")
     ap.add_argument("--no-e2e", action="store_true")
@@ -431,7 +431,7 @@ def run_ours(args, rank, world, local_rank):
     # stage kernel per stage, then the reduction pass; with passive scalars also their face fill per stage
     launches_per_step = stages if fused else (stages + 1 + (stages if args.scalars else 0))
     if args.amr:  # per stage: guard zones behind the jumps, the stage kernel(s), the flux correction; then the reduction pass
-        launches_per_step = stages * (4 if plan.path == 5 else 3) + 1
+        launches_per_step = stages * 3 + 1
     if sh is not None:
         launches_per_step += (int(sh.send_elems > 0) + int(sh.recv_elems > 0)) * stages  # pack + unpack of the cut-face slabs before every stage
         dt = sh.compute_dt(U, dx, cfg.cfl)  # the minimum over the ranks

@@ -63,9 +63,10 @@ enum {
                            two-zones-per-thread variant where it applies (PLM, no wall, no gravity; measured slower
                            than the default, kept for comparison), else as 0.
                            With refinement jumps (fx_hydro_plan_set_refinement): the generic kernel; under 0 and with 16 x 16 x nz
-                           blocks only the blocks that HAVE a jump face take it, the fused kernel advances the others (5).
+                           blocks the fused kernel (5): a block that HAS a jump face is marched alone, takes its halo behind
+                           the jump from its own interpolated guard zones and stores the jump faces' fluxes for the correction.
                            fx_hydro_plan_path reports the choice (1 fused, 4 fused on bundles of 8 x 8 blocks, 3 the pair variant,
-                           5 fused + generic at the refinement jumps, 2 tile, 0 generic). */
+                           5 fused with refinement jumps, 2 tile, 0 generic). */
   FX_OPT_ZCHAIN = 5,    /* fused path: longest chain of z-neighbour blocks one CTA marches through, 1..8 (1..16 for 8 x 8 x nz
                            blocks; a larger value is clamped to what the kernel takes); 0 (default) =
                            chosen from the number of blocks and of SMs so that the launch still fills the GPU.
@@ -165,7 +166,7 @@ int fx_hydro_plan_set_topology(fx_hydro_plan *plan, const int32_t *neigh_dev);
  * jump gives slope 0); and the flux of a coarse face at a jump is replaced by the mean of the fine face fluxes that cover
  * it (FLUX CORRECTION: what leaves the fine blocks enters the coarse one).  Edge and corner guard zones next to a jump hold
  * a clamp (the stage reads none [A11]); fx_guardcell_index_map reports the clamp for zones behind a jump.  Plans with
- * jumps run on the generic path.  Call before the workspace (which grows by the jump faces' flux buffer) and the
+ * jumps run on the generic path, or on the fused one where the block shape is its (FX_OPT_PATH).  Call before the workspace (which grows by the jump faces' flux buffer) and the
  * topology.  Needs even block extents and nguard <= n_d / 2 in active dimensions (FX_ERR_INVALID_ARG). */
 int fx_hydro_plan_set_refinement(fx_hydro_plan *plan, const int32_t *jump_dev);
 

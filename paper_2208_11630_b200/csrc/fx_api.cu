@@ -204,9 +204,9 @@ extern "C" int fx_hydro_plan_path(const fx_hydro_plan *plan) {
   if (!plan) return fx_fail(FX_ERR_INVALID_ARG, "plan_path: null plan");
   if (plan->P.has_jumps) {
     // refinement jumps [B12-B14]: the generic kernel reads the interpolated guard zones.  Where the fused kernel takes the
-    // block shape, only the blocks that HAVE a jump face go that way (5: fused kernel on the rest, whose faces all have
-    // same-level neighbours or physical boundaries)
-    return (plan->jlist_host && plan->P.jlist && fx_stage_tma_supported(plan->P)) ? 5 : 0;
+    // block shape (5), it advances every block: those WITH a jump face as segments of their own, their halo boxes behind a
+    // jump taken from their own guard zones and the jump faces' fluxes stored for the correction
+    return (plan->jlist_host && fx_stage_tma_supported(plan->P)) ? 5 : 0;
   }
   // passive scalars [B11]: behind the fused kernel by the scalar pass where it applies (PLM, same-level neighbours
   // everywhere, no gravity), else on the generic path
@@ -267,14 +267,7 @@ static int fx_seg_upload(fx_hydro_plan *plan) {
   plan->P.nseg = plan->nseg_host;
   plan->P.bseg = nullptr;
   plan->P.nbseg = 0;
-  plan->P.jlist = nullptr;
-  plan->P.njump = 0;
-  if (plan->jlist_host && plan->nseg_host > 0) {  // hybrid AMR path: the jump blocks' ids behind the segments (nseg 12 + njump <= nblocks 12 ints)
-    int *jd = dst + (size_t)plan->nseg_host * FX_SEG_STRIDE;
-    if (plan->njump_host > 0) FX_CUDA(cudaMemcpy(jd, plan->jlist_host, (size_t)plan->njump_host * sizeof(int), cudaMemcpyHostToDevice));
-    plan->P.jlist = jd;
-    plan->P.njump = plan->njump_host;
-  }
+  plan->P.njump = plan->jlist_host ? plan->njump_host : 0;  // (fused AMR path: the blocks with a jump face are single-block segments)
   if (plan->bseg_host && plan->nbseg_host > 0) {  // bundle segments take the place of the (unused: blocks are not 16 wide) block segments
     FX_CUDA(cudaMemcpy(dst, plan->bseg_host, (size_t)plan->nbseg_host * FX_BSEG_STRIDE * sizeof(int), cudaMemcpyHostToDevice));
     plan->P.bseg = dst;
@@ -492,9 +485,10 @@ extern "C" int fx_hydro_plan_set_topology(fx_hydro_plan *plan, const int32_t *ne
       if (rcb) return rcb;
     }
     std::vector<char> seen((size_t)nb, 0);
-    // Refinement jumps, hybrid path: where the block shape is the fused kernel's, the blocks WITH a jump face are listed for
-    // the generic kernel (which reads their interpolated guard zones) and taken out of the chains; every face of the others
-    // has a same-level neighbour or a physical boundary, which is all the fused kernel needs.
+    // Refinement jumps on the fused path: where the block shape is the fused kernel's, the blocks WITH a jump face are taken
+    // out of the chains and appended as segments of one block (the kernel reads their halo behind a jump from their own
+    // interpolated guard zones and stores the jump faces' fluxes, which it can only attribute to a single-block segment);
+    // every face of the others has a same-level neighbour or a physical boundary.
     delete[] plan->jlist_host;
     plan->jlist_host = nullptr;
     plan->njump_host = 0;
@@ -560,6 +554,16 @@ extern "C" int fx_hydro_plan_set_topology(fx_hydro_plan *plan, const int32_t *ne
         row[2 + cnt] = zact ? h[last * 6 + 5] : -1;
         ++plan->nseg_host;
       }
+    }
+    for (long long q = 0; q < plan->njump_host; ++q) {  // the blocks with a jump face: one segment each
+      const long long b = plan->jlist_host[q];
+      int *row = plan->seg_host + (size_t)plan->nseg_host * FX_SEG_STRIDE;
+      for (int t = 0; t < FX_SEG_STRIDE; ++t) row[t] = -1;
+      row[0] = 1;
+      row[1] = zact ? h[b * 6 + 4] : -1;
+      row[2] = (int)b;
+      row[3] = zact ? h[b * 6 + 5] : -1;
+      ++plan->nseg_host;
     }
   }
   return fx_seg_upload(plan);

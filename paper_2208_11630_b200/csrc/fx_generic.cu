@@ -262,9 +262,8 @@ __global__ void __launch_bounds__(128, RECON == FX_RECON_PLM_MINMOD ? FX_GENERIC
   const int e0 = CA && P.active[0] ? ext : 0, e1 = CA && P.active[1] ? ext : 0, e2 = CA && P.active[2] ? ext : 0;
   const int nx = P.n[0] + 2 * e0, ny = P.n[1] + 2 * e1, nz = P.n[2] + 2 * e2;
   const long long per_block = (long long)nx * ny * nz;
-  const long long bi = z / per_block;
-  const int r = (int)(z - bi * per_block);
-  const long long b = (AMR && P.jlist) ? (long long)__ldg(&P.jlist[bi]) : bi;  // hybrid AMR path: the listed blocks only
+  const long long b = z / per_block;
+  const int r = (int)(z - b * per_block);
   // (a CTA of 16 x 4 x 2 zones instead of 8 rows of one plane, for L1 reuse of the y and z neighbours: measured, no gain)
   const int i = r % nx - e0, j = (r / nx) % ny - e1, k = r / (nx * ny) - e2;  // interior coordinates (CA: from -ext)
   const long long c = b * P.S_b + (k + P.gd[2]) * P.S_k + (j + P.gd[1]) * P.S_j + (i + P.gd[0]);
@@ -356,8 +355,7 @@ __global__ void __launch_bounds__(128) fx_k_debug_fluxes(FxParams P, const doubl
 
 int fx_launch_generic_stage(const FxParams &P, const double *X, const double *U0, double *out, const double *dx,
                             double dt, const double *dt_dev, double beta, int first, cudaStream_t st) {
-  // owned blocks come first; on the hybrid AMR path (P.jlist) the blocks with a jump face only
-  const long long nzones = ((P.has_jumps && P.jlist) ? P.njump : P.nown) * P.n[0] * P.n[1] * P.n[2];
+  const long long nzones = P.nown * P.n[0] * P.n[1] * P.n[2];  // owned blocks come first
   if (nzones == 0) return FX_OK;
   const unsigned grid = (unsigned)((nzones + 127) / 128);
 #define CALL(RC, RM)                                                                                              \

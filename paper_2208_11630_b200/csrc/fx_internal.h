@@ -32,8 +32,7 @@ struct FxParams {
   int has_jumps;                    // some active face carries FX_NEIGH_COARSER / FX_NEIGH_FINER
   double *fjump;                    // boundary-face fluxes captured at jump faces [B14]: [nblocks][6][5][fj_area], in the workspace
   int fj_area;                      // largest face of a block, in zones
-  const int *jlist;                 // hybrid AMR path (fx_hydro_plan_path = 5): ids of the blocks that have a jump face, device (behind the
-  long long njump;                  // segments in the workspace); the fused kernel's segments then cover the other blocks only
+  long long njump;                  // fused AMR path (fx_hydro_plan_path = 5): how many blocks have a jump face (each a segment of its own)
   unsigned long long *scratch;      // device scratch block, see FX_SCR_*
 };
 
@@ -66,7 +65,7 @@ struct fx_hydro_plan {
   int zchain;           // FX_OPT_ZCHAIN: longest segment (1 .. FX_SEG_MAX)
   int32_t *jump_host;   // host copy of the refinement-jump table (new[]), or nullptr
   int *seg_host;        // segment table built by set_topology (new[]), nseg_host rows
-  int *jlist_host;      // blocks with a jump face (hybrid AMR path), njump_host entries, or nullptr
+  int *jlist_host;      // blocks with a jump face (fused AMR path), njump_host entries, or nullptr
   long long njump_host;
   int *bseg_host;       // bundle segments (8 x 8 blocks whose topology bundles completely), nbseg_host rows, or nullptr
   int nbseg_host;

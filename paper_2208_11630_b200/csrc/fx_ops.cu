@@ -41,13 +41,6 @@ extern "C" int fx_hydro_compute_dt(fx_hydro_plan *plan, const double *U, const d
 
 // One stage: out = U0 + beta((X - U0) - S(X)); halos of X come from a K1 fill (generic path) or are
 // gathered from neighbour interiors inside the fused kernel.
-// The generic kernel over ALL owned blocks (path 0): a block list left by set_topology for the hybrid path is not used.
-static FxParams fx_without_jlist(const FxParams &P) {
-  FxParams Q = P;
-  Q.jlist = nullptr;
-  Q.njump = 0;
-  return Q;
-}
 
 static int fx_stage(fx_hydro_plan *plan, double *X, const double *U0, double *out, const double *dx, double dt,
                     const double *dt_dev, double beta, int first, cudaStream_t st, double cfl_next = 0.0,
@@ -56,15 +49,14 @@ static int fx_stage(fx_hydro_plan *plan, double *X, const double *U0, double *ou
   const bool fused = path == 1 || path == 3 || path == 4;
   int rc = FX_OK;
   if (path == 5) {
-    // hybrid AMR path: guard zones behind the jumps, then the fused kernel on the blocks without a jump face and the
-    // generic kernel on those with one (both inside the timing bracket), then the flux correction; the time step of the
-    // finished state, if asked for, as a pass of its own (the fused reduction would miss the listed blocks)
+    // fused AMR path: guard zones behind the jumps, then the fused kernel on every block (the blocks with a jump face read
+    // their own guard zones behind it and store the jump faces' fluxes), then the flux correction; the time step of the
+    // finished state, if asked for, as a pass of its own (the fused reduction would miss the correction)
     const FxParams &P = plan->P;
     if ((rc = fx_launch_amr_fill(P, X, P.recon == FX_RECON_WENO5 ? 3 : 2, st))) return rc;
     const bool rec = plan->timing && plan->ev && plan->nrec < FX_MAX_REC;
     if (rec) FX_CUDA(cudaEventRecord(plan->ev[2 * plan->nrec], st));
     if ((rc = fx_launch_stage_tma(P, X, U0, out, dx, dt, dt_dev, beta, first, 0.0, nullptr, st))) return rc;
-    if ((rc = fx_launch_generic_stage(P, X, U0, out, dx, dt, dt_dev, beta, first, st))) return rc;
     if (rec) {
       FX_CUDA(cudaEventRecord(plan->ev[2 * plan->nrec + 1], st));
       ++plan->nrec;
@@ -95,7 +87,7 @@ static int fx_stage(fx_hydro_plan *plan, double *X, const double *U0, double *ou
                 : path == 4 ? fx_launch_stage_bundle(plan->P, X, U0, out, dx, dt, dt_dev, beta, first, cfl_next, dt_next, st)
                           : fx_launch_stage_tma(plan->P, X, U0, out, dx, dt, dt_dev, beta, first, cfl_next, dt_next, st))
              : (path == 2 ? fx_launch_stage_tile(plan->P, X, U0, out, dx, dt, dt_dev, beta, first, st)
-                          : fx_launch_generic_stage(fx_without_jlist(plan->P), X, U0, out, dx, dt, dt_dev, beta, first, st));
+                          : fx_launch_generic_stage(plan->P, X, U0, out, dx, dt, dt_dev, beta, first, st));
   if (rc) return rc;
   if (fused && plan->nvars > 5) {  // passive scalars [B11] behind the fused kernel: the scalar pass (inside the timing bracket)
     rc = fx_launch_scalar_pass(plan->P, X, U0, out, dx, dt, dt_dev, beta, first, st);

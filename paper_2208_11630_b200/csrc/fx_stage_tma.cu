@@ -91,8 +91,9 @@ __device__ __forceinline__ void flux_dir(const FxParams &P, const double WL[5], 
   F[4] = f[4];
 }
 
-// EXTRAS: some block of the launch has a reflecting wall [B9] or gravity is on [B10]: the image cells' sign flips
-// and the source term are compiled in only then
+// EXTRAS: some block of the launch has a reflecting wall [B9], gravity is on [B10] or some face carries a refinement jump
+// [B12-B14]: the image cells' sign flips, the source term, the halo boxes taken from a block's own (interpolated) guard
+// zones behind a jump and the capture of the jump faces' fluxes are compiled in only then
 // SCAL: the plan carries passive scalars [B11] and they take the scalar pass (fx_scalar_pass.cu): every zone also leaves the
 // mass flux and the advected-quantity coefficient Aq of its three low faces in P.fq for it
 template <int RECON, int RIEMANN, int WS, bool FIRST, bool DTOUT, bool EXTRAS, bool SCAL = false>
@@ -128,7 +129,9 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
     int id = S.chain[2 + qb];
     if (id < 0) {
       const bool wall = EXTRAS && id == FX_BC_REFLECT;
-      if (qb < 0) { id = S.chain[2]; k = wall ? -1 - Z : 0; } else { id = S.chain[1 + M]; k = wall ? nzb - 1 - (Z - nz) : nzb - 1; }
+      // behind a refinement jump [B12]: the block's OWN guard planes, which fx_k_amr_fill has interpolated [B13]
+      const bool own = EXTRAS && id <= FX_NEIGH_COARSER;
+      if (qb < 0) { id = S.chain[2]; k = own ? Z : (wall ? -1 - Z : 0); } else { id = S.chain[1 + M]; k = own ? nzb + (Z - nz) : (wall ? nzb - 1 - (Z - nz) : nzb - 1); }
     }
     bs = id;
     kp = k + g2;
@@ -157,10 +160,13 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
   auto issue_H = [&]() {  // halo cells of interior plane hk of block hb, from the block's x and y neighbours
     const int b = hb, kp = hk + g2;
     mbar_expect_tx(&S.barH, 2 * 5 * NY * BW * 8 + 2 * 5 * R * NX * 8);
-    tma_load(&S.Hx[0][0][0][0], &mXx, &S.barH, g0 + (xlo >= 0 ? NX - BW : 0), g1, kp, xlo >= 0 ? xlo : b);
-    tma_load(&S.Hx[1][0][0][0], &mXx, &S.barH, g0 + (xhi >= 0 ? 0 : NX - BW), g1, kp, xhi >= 0 ? xhi : b);
-    tma_load(&S.Hy[0][0][0][0], &mXy, &S.barH, g0, g1 + (ylo >= 0 ? NY - R : 0), kp, ylo >= 0 ? ylo : b);
-    tma_load(&S.Hy[1][0][0][0], &mXy, &S.barH, g0, g1 + (yhi >= 0 ? 0 : NY - R), kp, yhi >= 0 ? yhi : b);
+    // (a face with a refinement jump [B12]: the block's own guard zones behind it, interpolated by fx_k_amr_fill)
+    const bool jxl = EXTRAS && xlo <= FX_NEIGH_COARSER, jxh = EXTRAS && xhi <= FX_NEIGH_COARSER;
+    const bool jyl = EXTRAS && ylo <= FX_NEIGH_COARSER, jyh = EXTRAS && yhi <= FX_NEIGH_COARSER;
+    tma_load(&S.Hx[0][0][0][0], &mXx, &S.barH, g0 + (xlo >= 0 ? NX - BW : (jxl ? -BW : 0)), g1, kp, xlo >= 0 ? xlo : b);
+    tma_load(&S.Hx[1][0][0][0], &mXx, &S.barH, g0 + (xhi >= 0 ? 0 : (jxh ? NX : NX - BW)), g1, kp, xhi >= 0 ? xhi : b);
+    tma_load(&S.Hy[0][0][0][0], &mXy, &S.barH, g0, g1 + (ylo >= 0 ? NY - R : (jyl ? -R : 0)), kp, ylo >= 0 ? ylo : b);
+    tma_load(&S.Hy[1][0][0][0], &mXy, &S.barH, g0, g1 + (yhi >= 0 ? 0 : (jyh ? NY : NY - R)), kp, yhi >= 0 ? yhi : b);
   };
   auto issue_U0 = [&](int p, int b, int k) {  // plane p of the column = plane k of block b
     // completes on the barrier of tick p + 1, the tick that combines plane p: one wait per tick covers both loads
@@ -189,6 +195,19 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
     constexpr bool AQS = SCAL && RIEMANN != FX_RIEMANN_HLLC;  // the faces' Aq are needed (HLLC: Aq = max(F_rho, 0))
     double Aqz = 0.0;      // AQS: Aq of that face
     int sq = 0, sk = 0;    // SCAL: plane p is plane sk of the sq-th block of the segment
+    // Refinement jumps [B14]: the fluxes through a block's jump faces are stored for the flux correction (both sides of a
+    // jump).  Such a block is a segment of its own (fx_hydro_plan_set_topology keeps it out of the chains), so the planes of
+    // this CTA are the planes of block chain[2]; bit f of cap: face f carries a jump.
+    unsigned cap = 0;
+    if (EXTRAS && P.has_jumps && M == 1) {
+#pragma unroll
+      for (int f = 0; f < 6; ++f) cap |= (__ldg(&P.neigh[(long long)S.chain[2] * 6 + f]) <= FX_NEIGH_COARSER ? 1u : 0u) << f;
+    }
+    auto capture = [&](int f, int tflat, const double F[5]) {
+      double *dst = P.fjump + ((long long)S.chain[2] * 6 + f) * 5 * (long long)P.fj_area + tflat;
+#pragma unroll
+      for (int v = 0; v < 5; ++v) dst[(long long)v * P.fj_area] = F[v];
+    };
     {
       // prologue: cells -R .. r straight from global memory (all loads in flight together), the plus-side state
       // of cell 0 and the flux of face 0
@@ -219,6 +238,7 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
       hit |= fx_recon_cell5<RECON>(&w[0], P.weno_eps, qm, qpm1);  // cell -1
       hit |= fx_recon_cell5<RECON>(&w[1], P.weno_eps, qm, qpz);   // cell 0
       flux_dir<RIEMANN, WS, 2, AQS>(P, qpm1, qm, Fz, &Aqz);
+      if (EXTRAS && (cap & 16u)) capture(4, j * NX + i, Fz);
 #pragma unroll
       for (int m = 0; m < 2 * r; ++m)
 #pragma unroll
@@ -305,6 +325,11 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
         if (++sk == nzb) { sk = 0; ++sq; }
       }
       cta_sync();  // C: fluxes and the next plane's primitives visible
+      if (EXTRAS && cap) {
+        if ((cap & 1u) && i == 0) capture(0, p * NY + j, Fx);
+        if ((cap & 4u) && j == 0) capture(2, p * NX + i, Fy);
+        if ((cap & 32u) && c == nz) capture(5, j * NX + i, Fz_new);
+      }
       {
         // out = [U0 + beta (X - U0)] - sum_d (beta dt/dx_d) (F_d+ - F_d-)
         const double rx = S.rd[0], ry = S.rd[1], rz = S.rd[2];
@@ -377,6 +402,9 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
     constexpr int LV = NY * (NX + 1);                       // per-variable size of the L arrays (272)
     cta_sync();  // A0
     int pk = 0, pq = 0, pb = S.chain[2];  // plane p is plane pk of block pb, the pq-th of the segment
+    // the high x / y face of this lane's row / column carries a refinement jump: its flux is stored [B14]
+    const int ef = isx ? 1 : 3;
+    const bool ecap = EXTRAS && P.has_jumps && M == 1 && __ldg(&P.neigh[(long long)pb * 6 + ef]) <= FX_NEIGH_COARSER;
 
 #pragma unroll 1
     for (int c = 1; c <= nz; ++c) {
@@ -415,6 +443,11 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
         F[4] = f[4];
 #pragma unroll
         for (int v = 0; v < 5; ++v) Lf[v * LV + NX * ld + m * lt] = F[v];
+        if (EXTRAS && ecap) {
+          double *dst = P.fjump + ((long long)pb * 6 + ef) * 5 * (long long)P.fj_area + (c - 1) * NX + m;
+#pragma unroll
+          for (int v = 0; v < 5; ++v) dst[(long long)v * P.fj_area] = F[v];
+        }
       }
       if (pk == 0 && lane < 3) {
         // a block's first plane: the combines of the block below ended before barrier B, this tick's starts after C
@@ -445,8 +478,10 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
     auto halo_off = [&](int t, bool high) -> int {
       int idx;  // cell index inside the box
       // a neighbour's cells; at a reflecting wall this block's own cells in mirrored order [B9]; at outflow its edge cell
-      if (isx) idx = high ? (nhi >= 0 ? t : ((EXTRAS && nhi == FX_BC_REFLECT) ? BW - 1 - t : BW - 1)) : (nlo >= 0 ? BW - R + t : ((EXTRAS && nlo == FX_BC_REFLECT) ? R - 1 - t : 0));
-      else idx = high ? (nhi >= 0 ? t : ((EXTRAS && nhi == FX_BC_REFLECT) ? R - 1 - t : R - 1)) : (nlo >= 0 ? t : ((EXTRAS && nlo == FX_BC_REFLECT) ? R - 1 - t : 0));
+      // (the guard zones behind a refinement jump lie in the box like a neighbour's cells)
+      const bool clo = nlo >= 0 || (EXTRAS && nlo <= FX_NEIGH_COARSER), chi = nhi >= 0 || (EXTRAS && nhi <= FX_NEIGH_COARSER);
+      if (isx) idx = high ? (chi ? t : ((EXTRAS && nhi == FX_BC_REFLECT) ? BW - 1 - t : BW - 1)) : (clo ? BW - R + t : ((EXTRAS && nlo == FX_BC_REFLECT) ? R - 1 - t : 0));
+      else idx = high ? (chi ? t : ((EXTRAS && nhi == FX_BC_REFLECT) ? R - 1 - t : R - 1)) : (clo ? t : ((EXTRAS && nlo == FX_BC_REFLECT) ? R - 1 - t : 0));
       return isx ? ((high ? 5 * HXV : 0) + m * BW + idx) : ((high ? 5 * HYV : 0) + idx * NX + m);
     };
     int hoff[2 * R];
@@ -583,7 +618,7 @@ int launch_ws(const FxParams &P, const double *X, const double *U0, double *out,
       return launch<RECON, RIEMANN, WS, false, false, false, true>(P, X, U0, out, dx, dt, dt_dev, beta, 0.0, nullptr, st);
     }
   }
-  if (P.walls || P.grav_on) {
+  if (P.walls || P.grav_on || P.has_jumps) {  // (the kernel variant that also knows the refinement-jump faces [B12-B14])
     if (first) return launch<RECON, RIEMANN, WS, true, false, true>(P, X, U0, out, dx, dt, dt_dev, beta, 0.0, nullptr, st);
     if (dt_next) return launch<RECON, RIEMANN, WS, false, true, true>(P, X, U0, out, dx, dt, dt_dev, beta, cfl_next, dt_next, st);
     return launch<RECON, RIEMANN, WS, false, false, true>(P, X, U0, out, dx, dt, dt_dev, beta, 0.0, nullptr, st);

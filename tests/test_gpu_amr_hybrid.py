@@ -1,6 +1,7 @@
-"""Refinement jumps with 16 x 16 x nz blocks: the hybrid path (fx_hydro_plan_path = 5) -- the fused TMA kernel on the blocks
-whose faces all have same-level neighbours or physical boundaries, the generic kernel on the blocks that have a jump face
-(it reads their interpolated guard zones), then the flux correction.  Checked against the oracle on static two-level grids
+"""Refinement jumps with 16 x 16 x nz blocks on the fused path (fx_hydro_plan_path = 5): the fused TMA kernel advances every
+block -- those whose faces all have same-level neighbours or physical boundaries in chains, those that have a jump face as
+segments of their own, reading their interpolated guard zones behind the jump and storing the jump faces' fluxes --, then
+the flux correction.  Checked against the oracle on static two-level grids
 (<= 1e-12 after one step, <= 1e-9 after ten [NS]), for conservation through the jumps, against the all-generic path, and
 for bitwise independence of the chain length."""
 import numpy as np
@@ -102,11 +103,11 @@ def test_hybrid_uniform_state_bitwise_and_chain_length():
         assert torch.equal(r, results[0])
 
 
-def test_every_block_with_a_jump_face_falls_back_to_generic_everywhere():
-    """A grid whose every block touches a jump leaves the fused kernel nothing: the plan reports the generic path."""
+def test_a_grid_whose_every_block_has_a_jump_face():
+    """Every block touches a jump: every segment of the fused kernel is a single block that reads its own guard zones."""
     grid = two_level_grid((2, 1, 1), {(0, 0, 0)}, DIMS)  # the coarse block sees the refined one through both x faces
     gplan = gpu_plan(grid)
-    assert gplan.path == 0
+    assert gplan.path == 5
     oplan = amr_plan(grid, DIMS)
     Uo = state_from(oplan, smooth_field(grid, DIMS, [32, 16, 16]))
     Ud = torch.from_numpy(Uo).cuda()
