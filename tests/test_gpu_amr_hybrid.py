@@ -22,9 +22,11 @@ class Cfg:
     gamma = GAMMA
 
 
-def gpu_plan(grid, recon=0, riemann=1, rk=2, path=None, zchain=None, dims=DIMS):
+def gpu_plan(grid, recon=0, riemann=1, rk=2, path=None, zchain=None, dims=DIMS, guard_x=None):
     from paper_2208_11630_b200 import binding as fx
     plan = fx.HydroPlan(dims, 4, len(grid["level"]), GAMMA, recon, riemann, rk)
+    if guard_x is not None:
+        plan.fx_hydro_plan_set_option(fx.OPT_GUARD_X, guard_x)
     if path is not None:
         plan.fx_hydro_plan_set_option(fx.OPT_PATH, path)
     if zchain is not None:
@@ -116,3 +118,24 @@ def test_a_grid_whose_every_block_has_a_jump_face():
     oplan.advance(Uo, dx, dt)
     gplan.fx_hydro_advance(Ud, torch.from_numpy(dx).cuda(), dt)
     assert rel_err(Cfg, gplan.interior(Ud).cpu().numpy(), oplan.interior(Uo)) <= 1e-12
+
+
+@pytest.mark.parametrize("nbc,refined,periodic", GRIDS16[1:])
+@pytest.mark.parametrize("recon,rk", [(0, 2), (1, 3)])
+def test_wide_layout_gives_the_same_bits(nbc, refined, periodic, recon, rk):
+    """FX_OPT_GUARD_X = 8 (256-byte row pitch, the layout bench.py runs): a block's own guard zones behind a jump then start
+    8 zones into a row; three steps equal the compact layout's bit for bit."""
+    grid = two_level_grid(nbc, refined, DIMS, periodic=periodic)
+    oplan = amr_plan(grid, DIMS, recon=recon, rk=rk)
+    L = [nbc[d] * DIMS[d] for d in range(3)]
+    Uo = state_from(oplan, smooth_field(grid, DIMS, L))
+    ga, gb = gpu_plan(grid, recon, 1, rk), gpu_plan(grid, recon, 1, rk, guard_x=8)
+    assert ga.path == 5 and gb.path == 5 and gb.gd == (8, 4, 4)
+    A = torch.from_numpy(Uo).cuda()
+    B = gb.embed(np.ascontiguousarray(oplan.interior(Uo)))
+    dxd = torch.from_numpy(dx_of(grid)).cuda()
+    dta, dtb = ga.fx_hydro_compute_dt(A, dxd, 0.3).clone(), gb.fx_hydro_compute_dt(B, dxd, 0.3).clone()
+    for _ in range(3):
+        ga.fx_hydro_step(A, dxd, 0.3, dta)
+        gb.fx_hydro_step(B, dxd, 0.3, dtb)
+    assert torch.equal(dta, dtb) and torch.equal(ga.interior(A), gb.interior(B))
