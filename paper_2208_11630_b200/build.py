@@ -51,7 +51,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
         f.write("\n".join(log))
     if verbose:
         print("\n".join(log))
-    subprocess.check_call([nvcc, "-shared", "-o", LIB, *objs])  # cudart is linked statically (nvcc default)
+    # (the arch flags again: without them the link step adds a device-link stub for nvcc's default architecture)
+    subprocess.check_call([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", LIB, *objs])  # cudart is linked statically (nvcc default)
     return LIB
 
 
