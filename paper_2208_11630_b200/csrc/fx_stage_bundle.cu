@@ -61,6 +61,11 @@ template <int RECON> struct alignas(128) Smem {
 static_assert(sizeof(Smem<FX_RECON_PLM_MINMOD>) <= 115712, "PLM: two CTAs per SM need <= 115 712 bytes each");
 
 __device__ __forceinline__ void cta_sync() { asm volatile("bar.sync 0, %0;" ::"n"(NTHREADS) : "memory"); }
+// Barrier C has a hardware barrier of its own: the zone threads and the edge warp wait at it, the producer warp only ARRIVES
+// (its halo primitives written, the result plane's store read out) and goes on issuing the next tick's copies; its next wait
+// is barrier B, on barrier 0, which the others reach only after C -- so it is never more than one arrival ahead.
+__device__ __forceinline__ void cta_sync_c() { asm volatile("bar.sync 1, %0;" ::"n"(NTHREADS) : "memory"); }
+__device__ __forceinline__ void cta_arrive_c() { asm volatile("bar.arrive 1, %0;" ::"n"(NTHREADS) : "memory"); }
 
 template <int RIEMANN, int WS, int D>
 __device__ __forceinline__ void flux_dir(const FxParams &P, const double WL[5], const double WR[5], double F[5]) {
@@ -275,7 +280,7 @@ fx_k_stage_bundle(const __grid_constant__ CUtensorMap mXm, const __grid_constant
 #pragma unroll
         for (int v = 0; v < 5; ++v) S.P[v][j + R][i + R] = q[r][v];
       }
-      cta_sync();  // C
+      cta_sync_c();  // C
       {
         const double rx = S.rd[zq][0], ry = S.rd[zq][1], rz = S.rd[zq][2];
         int hmax = 0;
@@ -377,7 +382,7 @@ fx_k_stage_bundle(const __grid_constant__ CUtensorMap mXm, const __grid_constant
         pk = 0;
         ++pq;
       }
-      cta_sync();  // C
+      cta_sync_c();  // C
     }
     cta_sync();  // D
   } else {
@@ -416,6 +421,8 @@ fx_k_stage_bundle(const __grid_constant__ CUtensorMap mXm, const __grid_constant
         for (int v = 0; v < 5; ++v) Pf[v * NP * NPS + pos * pd + (m + R) * pt] = w[v];
       }
       __syncwarp();
+    };
+    auto halo_next = [&](int pl) {  // the single halo slot is free (every lane has read its cells): the next plane's boxes
       if (pl + 1 < nz) {
         if (++hk == nzb) {
           hk = 0;
@@ -430,33 +437,66 @@ fx_k_stage_bundle(const __grid_constant__ CUtensorMap mXm, const __grid_constant
       }
     };
     halo_plane(0);
+    halo_next(0);
     cta_sync();  // A0
     int pk = 0, pq = 0;
+    // The block ids a tick's twelve plane copies need -- rows pq, pq + 1, pq + 2 of the segment table: the layers below, of
+    // and above the plane being combined -- are kept in registers and refreshed when a new layer starts, BEFORE the wait for
+    // barrier B.  Read from the table one by one between the copies (each bulk-copy statement is a memory barrier to the
+    // compiler, so every id was a dependent global load in the issuing lane's path, with hardly any L1 beside two CTAs'
+    // shared memory), they made the producer warp the last to arrive at barrier C: ncu showed the zone warps waiting
+    // there for 13 % of their time.
+    int cid[3][4];
+    auto load_rows = [&]() {
+#pragma unroll
+      for (int a = 0; a < 3; ++a)
+#pragma unroll
+        for (int q = 0; q < 4; ++q) cid[a][q] = BLK(pq + a, q);
+    };
+    auto row_id = [&](int row, int q) -> int {
+      const int a = row - pq;
+      return a == 0 ? cid[0][q] : (a == 1 ? cid[1][q] : cid[2][q]);
+    };
+    load_rows();
 #pragma unroll 1
     for (int c = 1; c <= nz; ++c) {
       const int p = c - 1;
+      if (pk == 0 && c > 1) load_rows();
       mbar_wait(&S.barX[c & 1], ((c - 1) >> 1) & 1);
       cta_sync();  // B
       if (lane == 0) {
-        if (c + 1 <= nz) issue_X(c + 1);
+        if (c + 1 <= nz) {  // issue_X(c + 1) with the cached ids
+          const int Z = c + 1 + r;
+          const int qb = M == 1 ? (int)(Z >= nzb) : (int)(((unsigned)Z * zmagic) >> 20);
+          mbar_expect_tx(&S.barX[(c + 1) & 1], PLANE_BYTES);
+#pragma unroll
+          for (int q = 0; q < 4; ++q) {
+            int id = row_id(1 + qb, q), k = Z - qb * nzb;
+            if (id < 0) { id = BLK(M, q); k = nzb - 1; }  // above the segment: outflow clamps to the top plane [O1]
+            tma_load(&S.ring[Z % NRING][q][0][0][0], &mXm, &S.barX[(c + 1) & 1], g0, g1, k + g2, id);
+          }
+        }
         if (p >= 1) {
           const int layer = pk >= 1 ? pq : pq - 1, k = (pk >= 1 ? pk - 1 : nzb - 1) + g2;
 #pragma unroll
-          for (int q = 0; q < 4; ++q) tma_store(&mOut, &S.Out[q][0][0][0], g0, g1, k, BLK(1 + layer, q));
+          for (int q = 0; q < 4; ++q) tma_store(&mOut, &S.Out[q][0][0][0], g0, g1, k, row_id(1 + layer, q));
           tma_commit();
         }
-        if (!FIRST && p + 1 < nz) {
-          if (pk + 1 < nzb) issue_U0(p + 1, pq, pk + 1);
-          else issue_U0(p + 1, pq + 1, 0);
-        }
       }
+      if (c < nz) halo_plane(c);  // halo of plane p + 1: nobody reads P between barriers B and C
+      if (lane == 0 && p >= 1) tma_wait_read();  // Out is free for the combine after barrier C
+      cta_arrive_c();  // C: what the others wait for is done; the rest of the tick is off their path
+      if (lane == 0 && !FIRST && p + 1 < nz) {  // issue_U0(p + 1, ...): its slot was last read before barrier B
+        const int layer = pk + 1 < nzb ? pq : pq + 1, k = pk + 1 < nzb ? pk + 1 : 0;
+        mbar_expect_tx(&S.barX[(p + 2) & 1], PLANE_BYTES);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) tma_load(&S.U0[(p + 1) & 1][q][0][0][0], &mU0, &S.barX[(p + 2) & 1], g0, g1, k + g2, row_id(1 + layer, q));
+      }
+      if (c < nz) halo_next(c);
       if (++pk == nzb) {
         pk = 0;
         ++pq;
       }
-      if (c < nz) halo_plane(c);
-      if (lane == 0 && p >= 1) tma_wait_read();
-      cta_sync();  // C
     }
     cta_sync();  // D
     if (lane == 0) {
