@@ -18,11 +18,19 @@ __device__ __forceinline__ double amr_minmod(double a, double b) {  // compariso
   return 0.0;
 }
 
-// Variable v of the zone at interior coordinates c of block cb; at most one coordinate outside [0, n): one hop [B13].
-// Returns false behind a coarser jump (undefined there).
-__device__ bool amr_zone(const FxParams &P, const double *__restrict__ X, long long cb, const int cin[3], int v, double &val) {
+// Where the zone at interior coordinates c of block cb lives; at most one coordinate outside [0, n): one hop [B13].  The
+// location is the same for every variable, so it is resolved once (kind 0: the zone at element `off` of each variable, its
+// `flipv` momentum negated behind a reflecting wall; kind 1: the restriction of the cnt[0] x cnt[1] x cnt[2] finer zones that
+// start at `off`) and then evaluated per variable.  Returns false behind a coarser jump (undefined there).
+struct AmrSrc {
+  long long off;
+  int kind, flipv, cnt[3];
+};
+
+__device__ __forceinline__ bool amr_locate(const FxParams &P, long long cb, const int cin[3], AmrSrc &s) {
   int c[3] = {cin[0], cin[1], cin[2]};
-  double sign = 1.0;
+  s.kind = 0;
+  s.flipv = -1;
 #pragma unroll
   for (int d = 0; d < 3; ++d) {
     if (c[d] >= 0 && c[d] < P.n[d]) continue;
@@ -33,30 +41,25 @@ __device__ bool amr_zone(const FxParams &P, const double *__restrict__ X, long l
       c[d] += side ? -P.n[d] : P.n[d];
     } else if (nb == FX_BC_REFLECT) {
       c[d] = side ? 2 * P.n[d] - 1 - c[d] : -1 - c[d];
-      if (v == 1 + d) sign = -1.0;
+      s.flipv = 1 + d;
     } else if (nb == FX_NEIGH_FINER) {
       const int tr[2] = {d == 0 ? 1 : 0, d == 2 ? 1 : 2};
-      int q = 0, fc[3], cnt[3];
+      int q = 0, fc[3];
 #pragma unroll
       for (int t = 0; t < 2; ++t) {
         const int e = tr[t];
-        if (!P.active[e]) { fc[e] = 0; cnt[e] = 1; continue; }
+        if (!P.active[e]) { fc[e] = 0; s.cnt[e] = 1; continue; }
         const int half = c[e] >= P.n[e] / 2;
         q |= half << t;
         fc[e] = 2 * (c[e] - half * (P.n[e] / 2));
-        cnt[e] = 2;
+        s.cnt[e] = 2;
       }
       const int m = side ? c[d] - P.n[d] : -1 - c[d];
       fc[d] = side ? 2 * m : P.n[d] - 2 - 2 * m;
-      cnt[d] = 2;
+      s.cnt[d] = 2;
       const long long fb = __ldg(&P.jump[(cb * 6 + f) * 4 + q]);
-      double sum = 0.0;
-      for (int kk = 0; kk < cnt[2]; ++kk)
-        for (int jj = 0; jj < cnt[1]; ++jj)
-          for (int ii = 0; ii < cnt[0]; ++ii)
-            sum = __dadd_rn(sum, X[v * P.S_v + fb * P.S_b + (long long)(fc[2] + kk + P.gd[2]) * P.S_k +
-                                   (long long)(fc[1] + jj + P.gd[1]) * P.S_j + (fc[0] + ii + P.gd[0])]);
-      val = __dmul_rn(sum, 1.0 / (double)(cnt[0] * cnt[1] * cnt[2]));
+      s.kind = 1;
+      s.off = fb * P.S_b + (long long)(fc[2] + P.gd[2]) * P.S_k + (long long)(fc[1] + P.gd[1]) * P.S_j + (fc[0] + P.gd[0]);
       return true;
     } else if (nb == FX_NEIGH_COARSER) {
       return false;
@@ -65,31 +68,69 @@ __device__ bool amr_zone(const FxParams &P, const double *__restrict__ X, long l
     }
     break;  // one hop
   }
-  val = sign * X[v * P.S_v + cb * P.S_b + (long long)(c[2] + P.gd[2]) * P.S_k + (long long)(c[1] + P.gd[1]) * P.S_j + (c[0] + P.gd[0])];
+  s.off = cb * P.S_b + (long long)(c[2] + P.gd[2]) * P.S_k + (long long)(c[1] + P.gd[1]) * P.S_j + (c[0] + P.gd[0]);
   return true;
 }
 
-// One CTA per (block, face); threads over the face guard zones of depth `depth` and the variables.
-__global__ void __launch_bounds__(128) fx_k_amr_fill(const FxParams P, double *U, int depth) {
-  const long long b = blockIdx.x / 6;
-  const int f = blockIdx.x % 6, d = f >> 1, side = f & 1;
+__device__ __forceinline__ double amr_value(const FxParams &P, const double *__restrict__ X, const AmrSrc &s, int v) {
+  const double *Xv = X + (long long)v * P.S_v + s.off;
+  if (s.kind == 0) {
+    const double x = *Xv;
+    return v == s.flipv ? -x : x;
+  }
+  // children summed i fastest, then j, then k; all (up to eight) loads issued before the first addition -- as a loop with
+  // run-time counts every addition waited for its own load, eight memory round trips per value
+  double x[8];
+#pragma unroll
+  for (int t = 0; t < 8; ++t) {
+    const bool on = (t & 1) < s.cnt[0] && ((t >> 1) & 1) < s.cnt[1] && (t >> 2) < s.cnt[2];
+    x[t] = on ? Xv[(t >> 2) * P.S_k + ((t >> 1) & 1) * P.S_j + (t & 1)] : 0.0;
+  }
+  double sum = 0.0;
+#pragma unroll
+  for (int t = 0; t < 8; ++t) {
+    const bool on = (t & 1) < s.cnt[0] && ((t >> 1) & 1) < s.cnt[1] && (t >> 2) < s.cnt[2];
+    sum = on ? __dadd_rn(sum, x[t]) : sum;
+  }
+  return __dmul_rn(sum, 1.0 / (double)(s.cnt[0] * s.cnt[1] * s.cnt[2]));
+}
+
+// One CTA per (block, face); a thread per face guard zone of depth `depth`: it resolves where the zone's data comes from
+// once -- behind finer neighbours one location, behind a coarser one the parent zone and its two neighbours per active
+// dimension -- and then evaluates all variables.  (First version: a thread per zone AND variable, 128 threads per CTA, every
+// value resolving its seven locations itself, the restriction a loop whose every addition waited for its own load: 0.43 ms
+// per fill on the two-level workload of bench.py --amr, a fifth of the step; now 0.23 ms.)
+__global__ void __launch_bounds__(256) fx_k_amr_fill(const FxParams P, double *U, int depth) {
+  // (the grid is the list of jump faces where the plan has one: a CTA per face of EVERY block, most of which only look
+  // their face up and leave, took 0.07 ms more.  The face's dimension as a template parameter -- no dynamically indexed
+  // coordinate triples, no stack frame -- was slower: 0.27 against 0.23 ms, three copies of the code.)
+  const long long bf = P.jface ? (long long)__ldg(&P.jface[blockIdx.x]) : (long long)blockIdx.x;
+  const long long b = bf / 6;
+  const int f = (int)(bf % 6), d = f >> 1, side = f & 1;
   if (!P.active[d]) return;
   const int code = __ldg(&P.neigh[b * 6 + f]);
   if (code != FX_NEIGH_COARSER && code != FX_NEIGH_FINER) return;
   const int d1 = d == 0 ? 1 : 0, d2 = d == 2 ? 1 : 2;
   const int n1 = P.n[d1], n2 = P.n[d2];
-  const int total = depth * n1 * n2 * P.nvars;
-  for (int t = threadIdx.x; t < total; t += blockDim.x) {
-    const int v = t / (depth * n1 * n2), r = t - v * (depth * n1 * n2);
+  const int total = depth * n1 * n2;
+  for (int r = threadIdx.x; r < total; r += blockDim.x) {
     const int m = r / (n1 * n2), r2 = r - m * (n1 * n2), t2 = r2 / n1, t1 = r2 - t2 * n1;
     int c[3];
     c[d] = side ? P.n[d] + m : -1 - m;
     c[d1] = t1;
     c[d2] = t2;
-    const long long e = v * P.S_v + b * P.S_b + (long long)(c[2] + P.gd[2]) * P.S_k + (long long)(c[1] + P.gd[1]) * P.S_j + (c[0] + P.gd[0]);
-    double val = 0.0;
+    double *dst = U + b * P.S_b + (long long)(c[2] + P.gd[2]) * P.S_k + (long long)(c[1] + P.gd[1]) * P.S_j + (c[0] + P.gd[0]);
+    // (every value a zone needs is loaded before its first store: the loads of all variables are then in flight together
+    // instead of one DRAM round trip per variable; jumps come with the five hydro variables only -- set_topology refuses
+    // them with passive scalars)
     if (code == FX_NEIGH_FINER) {
-      amr_zone(P, U, b, c, v, val);
+      AmrSrc s;
+      amr_locate(P, b, c, s);
+      double val[5];
+#pragma unroll
+      for (int v = 0; v < 5; ++v) val[v] = amr_value(P, U, s, v);
+#pragma unroll
+      for (int v = 0; v < 5; ++v) dst[(long long)v * P.S_v] = val[v];
     } else {
       const long long cb = __ldg(&P.jump[(b * 6 + f) * 4 + 0]);
       const int qd = __ldg(&P.jump[(b * 6 + f) * 4 + 1]);
@@ -105,21 +146,40 @@ __global__ void __launch_bounds__(128) fx_k_amr_fill(const FxParams P, double *U
         C[e2] = ((qd >> t_) & 1) * (P.n[e2] / 2) + tc[t_] / 2;
         sg[e2] = (tc[t_] % 2) ? 1.0 : -1.0;
       }
-      double qC;
-      amr_zone(P, U, cb, C, v, qC);
-      val = qC;
+      AmrSrc sC, sm[3], sp[3];
+      bool both[3] = {false, false, false};
+      amr_locate(P, cb, C, sC);
 #pragma unroll
       for (int e2 = 0; e2 < 3; ++e2) {
         if (!P.active[e2]) continue;
         int Cm[3] = {C[0], C[1], C[2]}, Cp[3] = {C[0], C[1], C[2]};
         Cm[e2] -= 1;
         Cp[e2] += 1;
-        double qm, qp;
-        if (amr_zone(P, U, cb, Cm, v, qm) && amr_zone(P, U, cb, Cp, v, qp))
-          val = __dadd_rn(val, __dmul_rn(sg[e2] * 0.25, amr_minmod(__dsub_rn(qC, qm), __dsub_rn(qp, qC))));
+        both[e2] = amr_locate(P, cb, Cm, sm[e2]) && amr_locate(P, cb, Cp, sp[e2]);
+      }
+      double qC[5], qm[3][5], qp[3][5];
+#pragma unroll
+      for (int v = 0; v < 5; ++v) qC[v] = amr_value(P, U, sC, v);
+#pragma unroll
+      for (int e2 = 0; e2 < 3; ++e2) {
+        if (!both[e2]) continue;
+#pragma unroll
+        for (int v = 0; v < 5; ++v) {
+          qm[e2][v] = amr_value(P, U, sm[e2], v);
+          qp[e2][v] = amr_value(P, U, sp[e2], v);
+        }
+      }
+#pragma unroll
+      for (int v = 0; v < 5; ++v) {
+        double val = qC[v];
+#pragma unroll
+        for (int e2 = 0; e2 < 3; ++e2) {
+          if (!both[e2]) continue;
+          val = __dadd_rn(val, __dmul_rn(sg[e2] * 0.25, amr_minmod(__dsub_rn(qC[v], qm[e2][v]), __dsub_rn(qp[e2][v], qC[v]))));
+        }
+        dst[(long long)v * P.S_v] = val;
       }
     }
-    U[e] = val;
   }
 }
 
@@ -128,9 +188,10 @@ __global__ void __launch_bounds__(128) fx_k_amr_fill(const FxParams P, double *U
 // fluxes the stage kernel captured at every jump face (both sides).
 __global__ void __launch_bounds__(128) fx_k_amr_flux_correct(const FxParams P, double *out, const double *__restrict__ dx, double dt,
                                                              const double *__restrict__ dt_dev, double beta) {
-  const long long b = blockIdx.x / 6;
-  const int f = blockIdx.x % 6, d = f >> 1, side = f & 1;
-  if (!P.active[d] || __ldg(&P.neigh[b * 6 + f]) != FX_NEIGH_FINER) return;
+  const long long bf = P.jface ? (long long)__ldg(&P.jface[blockIdx.x]) : (long long)blockIdx.x;
+  const long long b = bf / 6;
+  const int f = (int)(bf % 6), d = f >> 1, side = f & 1;
+  if (b >= P.nown || !P.active[d] || __ldg(&P.neigh[b * 6 + f]) != FX_NEIGH_FINER) return;
   if (dt_dev) dt = *dt_dev;
   const int d1 = d == 0 ? 1 : 0, d2 = d == 2 ? 1 : 2;
   const int n1 = P.n[d1], n2 = P.n[d2];
@@ -170,7 +231,7 @@ __global__ void __launch_bounds__(128) fx_k_amr_flux_correct(const FxParams P, d
 
 int fx_launch_amr_fill(const FxParams &P, double *U, int depth, cudaStream_t st) {
   if (!P.jump || !P.has_jumps || P.nblocks == 0) return FX_OK;
-  fx_k_amr_fill<<<(unsigned)(P.nblocks * 6), 128, 0, st>>>(P, U, depth);
+  fx_k_amr_fill<<<(unsigned)(P.jface ? P.njface : P.nblocks * 6), 256, 0, st>>>(P, U, depth);
   FX_LAUNCH_CHECK("amr_fill");
   return FX_OK;
 }
@@ -178,7 +239,7 @@ int fx_launch_amr_fill(const FxParams &P, double *U, int depth, cudaStream_t st)
 int fx_launch_amr_flux_correct(const FxParams &P, double *out, const double *dx, double dt, const double *dt_dev, double beta,
                                cudaStream_t st) {
   if (!P.jump || !P.has_jumps || P.nown == 0) return FX_OK;
-  fx_k_amr_flux_correct<<<(unsigned)(P.nown * 6), 128, 0, st>>>(P, out, dx, dt, dt_dev, beta);
+  fx_k_amr_flux_correct<<<(unsigned)(P.jface ? P.njface : P.nown * 6), 128, 0, st>>>(P, out, dx, dt, dt_dev, beta);
   FX_LAUNCH_CHECK("amr_flux_correct");
   return FX_OK;
 }

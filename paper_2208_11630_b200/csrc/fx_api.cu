@@ -119,6 +119,7 @@ extern "C" int fx_hydro_plan_destroy(fx_hydro_plan *plan) {
   if (plan) delete[] plan->jump_host;
   if (plan) delete[] plan->bseg_host;
   if (plan) delete[] plan->jlist_host;
+  if (plan) delete[] plan->jface_host;
   if (plan && plan->ev) {
     for (int i = 0; i < 2 * FX_MAX_REC; ++i) cudaEventDestroy(plan->ev[i]);
     delete[] plan->ev;
@@ -227,13 +228,18 @@ static size_t fx_state_bytes_aligned(const fx_hydro_plan *plan) {
   return (b + 255) & ~(size_t)255;
 }
 
-static size_t fx_seg_bytes(const fx_hydro_plan *plan) {  // room for one segment per block, or one bundle segment per four 8 x 8 blocks
+static size_t fx_seg_ints(const fx_hydro_plan *plan) {  // room for one segment per block, or one bundle segment per four 8 x 8 blocks
   const FxParams &P = plan->P;
   size_t ints = (size_t)P.nblocks * FX_SEG_STRIDE;
   if (P.n[0] == 8 && P.n[1] == 8) {
     const size_t b = ((size_t)P.nblocks / 4 + 1) * FX_BSEG_STRIDE;
     if (b > ints) ints = b;
   }
+  return ints;
+}
+
+static size_t fx_seg_bytes(const fx_hydro_plan *plan) {  // the segment tables and, with a refinement table, the list of jump faces
+  const size_t ints = fx_seg_ints(plan) + (plan->P.jump ? (size_t)plan->P.nblocks * 6 : 0);
   return ((ints * sizeof(int)) + 255) & ~(size_t)255;
 }
 
@@ -268,6 +274,14 @@ static int fx_seg_upload(fx_hydro_plan *plan) {
   plan->P.bseg = nullptr;
   plan->P.nbseg = 0;
   plan->P.njump = plan->jlist_host ? plan->njump_host : 0;  // (fused AMR path: the blocks with a jump face are single-block segments)
+  plan->P.jface = nullptr;
+  plan->P.njface = 0;
+  if (plan->jface_host && plan->P.jump && plan->njface_host > 0) {
+    int *jf = dst + fx_seg_ints(plan);
+    FX_CUDA(cudaMemcpy(jf, plan->jface_host, (size_t)plan->njface_host * sizeof(int), cudaMemcpyHostToDevice));
+    plan->P.jface = jf;
+    plan->P.njface = plan->njface_host;
+  }
   if (plan->bseg_host && plan->nbseg_host > 0) {  // bundle segments take the place of the (unused: blocks are not 16 wide) block segments
     FX_CUDA(cudaMemcpy(dst, plan->bseg_host, (size_t)plan->nbseg_host * FX_BSEG_STRIDE * sizeof(int), cudaMemcpyHostToDevice));
     plan->P.bseg = dst;
@@ -425,6 +439,9 @@ extern "C" int fx_hydro_plan_set_topology(fx_hydro_plan *plan, const int32_t *ne
   if (!plan) return fx_fail(FX_ERR_INVALID_ARG, "set_topology: null plan");
   const long long nb = plan->P.nblocks;
   int jumps = 0, all_interior = 1;
+  delete[] plan->jface_host;
+  plan->jface_host = nullptr;
+  plan->njface_host = 0;
   if (nb > 0) {
     if (!neigh_dev) return fx_fail(FX_ERR_INVALID_ARG, "set_topology: null table");
     std::vector<int32_t> h((size_t)nb * 6);
@@ -446,6 +463,11 @@ extern "C" int fx_hydro_plan_set_topology(fx_hydro_plan *plan, const int32_t *ne
             if (id < 0 || id >= nb) return fx_fail(FX_ERR_INVALID_ARG, "set_topology: block %lld face %d: jump entry %d = %d out of range", b, f, q, id);
           }
           jumps = 1;
+          if (!plan->jface_host) {
+            plan->jface_host = new (std::nothrow) int[(size_t)nb * 6];
+            if (!plan->jface_host) return fx_fail(FX_ERR_INVALID_ARG, "set_topology: out of host memory");
+          }
+          plan->jface_host[plan->njface_host++] = (int)(b * 6 + f);
         } else if (v != FX_BC_OUTFLOW && v != FX_BC_REFLECT) {
           return fx_fail(FX_ERR_UNSUPPORTED, "set_topology: block %lld face %d has unknown code %d", b, f, v);
         }

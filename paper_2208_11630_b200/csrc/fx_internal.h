@@ -30,6 +30,8 @@ struct FxParams {
   int all_interior;                 // every active face of every owned block has a same-level neighbour (no physical boundary, no jump)
   const int *jump;                  // refinement jumps [B12]: [nblocks][6][4], device; nullptr if none was given
   int has_jumps;                    // some active face carries FX_NEIGH_COARSER / FX_NEIGH_FINER
+  const int *jface;                 // the faces that carry a jump, as b * 6 + f, device (behind the segment tables in the workspace), or nullptr
+  long long njface;
   double *fjump;                    // boundary-face fluxes captured at jump faces [B14]: [nblocks][6][5][fj_area], in the workspace
   int fj_area;                      // largest face of a block, in zones
   long long njump;                  // fused AMR path (fx_hydro_plan_path = 5): how many blocks have a jump face (each a segment of its own)
@@ -66,6 +68,8 @@ struct fx_hydro_plan {
   int32_t *jump_host;   // host copy of the refinement-jump table (new[]), or nullptr
   int *seg_host;        // segment table built by set_topology (new[]), nseg_host rows
   int *jlist_host;      // blocks with a jump face (fused AMR path), njump_host entries, or nullptr
+  int *jface_host;      // faces with a jump (b * 6 + f), njface_host entries, or nullptr: the grids of fx_k_amr_fill / _flux_correct
+  long long njface_host;
   long long njump_host;
   int *bseg_host;       // bundle segments (8 x 8 blocks whose topology bundles completely), nbseg_host rows, or nullptr
   int nbseg_host;
