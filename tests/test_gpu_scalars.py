@@ -140,3 +140,30 @@ def test_host_interior_call_carries_the_scalars():
     gplan.fx_hydro_advance_host_interior(Uint, torch.from_numpy(dx), cfg.cfl, nsteps, U_stage, packed, dx_stage)
     got, ref = Uint.numpy(), oplan.interior(Uo)
     assert rel_err(cfg, got[:5], ref[:5]) <= 1e-11 and scalar_err(got, ref) <= 1e-11
+
+
+@pytest.mark.parametrize("nz,g,ns,riemann,rk", [(2, 2, 3, 1, 2), (3, 2, 6, 1, 3), (4, 4, 5, 0, 2), (8, 4, 7, 1, 2), (16, 4, 9, 0, 3)])
+def test_scalar_march_block_heights_and_scalar_counts(nz, g, ns, riemann, rk):
+    """The marching scalar pass on blocks of 16 x 16 x nz zones, down to the two planes its prefetch distance allows (the
+    window's new cell is then always the block above's), with every launch shape: 1 to 4 scalars per launch, several
+    launches per stage, HLLC (F_rho alone handed over) and HLLE (F_rho and Aq)."""
+    cfg = inputs.config(5, nb=(2, 2, 3))
+    cfg.block_dims, cfg.nguard = (16, 16, nz), g
+    kw = dict(riemann=riemann, rk=rk)
+    oplan, neigh, coords = oracle_plan_for(cfg, nvars=5 + ns, **kw)
+    gplan, _, _ = gpu_plan_for(cfg, nvars=5 + ns, **kw)
+    assert gplan.path == 1
+    Uh = inputs.embed(cfg, inputs.with_scalars(cfg, coords, inputs.block_interiors(cfg, coords), ns))
+    rng = np.random.default_rng(7 + nz)
+    dx = inputs.dx_array(cfg) * (1.0 + 0.2 * rng.random((12, 1)))  # a different zone width per block
+    Uo, Ud, dxd = Uh.numpy().copy(), Uh.cuda(), torch.from_numpy(dx).cuda()
+    for step in range(3):
+        dt = oplan.compute_dt(Uo, dx, cfg.cfl)
+        oplan.advance(Uo, dx, dt)
+        gplan.fx_hydro_advance(Ud, dxd, dt)
+        got, ref = gplan.interior(Ud).cpu().numpy(), oplan.interior(Uo)
+        tol = TOL_1 * (1 + 2 * step)
+        assert rel_err(cfg, got[:5], ref[:5]) <= tol and scalar_err(got, ref) <= tol, (step, rel_err(cfg, got[:5], ref[:5]), scalar_err(got, ref))
+    fo, _ = oplan.status()
+    fg, _ = gplan.fx_hydro_status()
+    assert fo == fg
