@@ -139,3 +139,48 @@ def test_wide_layout_gives_the_same_bits(nbc, refined, periodic, recon, rk):
         ga.fx_hydro_step(A, dxd, 0.3, dta)
         gb.fx_hydro_step(B, dxd, 0.3, dtb)
     assert torch.equal(dta, dtb) and torch.equal(ga.interior(A), gb.interior(B))
+
+
+@pytest.mark.parametrize("recon,rk", [(0, 2), (1, 3)])
+def test_jumps_next_to_walls_with_gravity(recon, rk):
+    """Everything the kernel's EXTRAS variant carries at once: refinement jumps on blocks in the corners of a box with
+    reflecting walls, and a constant gravity [B9, B10, B12-B14], against the oracle and the all-generic path."""
+    from oracle import fxoracle as fxo
+    from paper_2208_11630_b200 import binding as fx
+    nbc = (4, 4, 3)
+    grid = two_level_grid(nbc, {(0, 0, 0), (1, 0, 0), (3, 3, 2)}, DIMS, periodic=False)
+    grid["neigh"] = np.where(grid["neigh"] == fxo.BC_OUTFLOW, fxo.BC_REFLECT, grid["neigh"]).astype(np.int32)
+    assert fxo.BC_REFLECT == fx.BC_REFLECT and (grid["neigh"] == fx.BC_REFLECT).any()
+    grav = (0.3, -0.2, 0.5)
+
+    def gplan_with_gravity(path=None):
+        plan = fx.HydroPlan(DIMS, 4, len(grid["level"]), GAMMA, recon, 1, rk)
+        if path is not None:
+            plan.fx_hydro_plan_set_option(fx.OPT_PATH, path)
+        for d in range(3):
+            plan.fx_hydro_plan_set_option(fx.OPT_GRAVITY_X + d, grav[d])
+        plan.fx_hydro_plan_set_refinement(grid["jump"])
+        plan.fx_hydro_plan_set_topology(grid["neigh"])
+        plan.fx_hydro_plan_set_workspace()
+        return plan
+
+    oplan = amr_plan(grid, DIMS, recon=recon, rk=rk)
+    for d in range(3):
+        oplan.set_option(fxo.OPT_GRAVITY_X + d, grav[d])
+    gplan, ggen = gplan_with_gravity(), gplan_with_gravity(path=1)
+    assert gplan.path == 5 and ggen.path == 0
+    Uo = state_from(oplan, smooth_field(grid, DIMS, [nbc[d] * DIMS[d] for d in range(3)]))
+    Ud, Ug = torch.from_numpy(Uo).cuda(), torch.from_numpy(Uo).cuda()
+    dx = dx_of(grid)
+    dxd = torch.from_numpy(dx).cuda()
+    for step in range(4):
+        dt = oplan.compute_dt(Uo, dx, 0.3)
+        oplan.advance(Uo, dx, dt)
+        gplan.fx_hydro_advance(Ud, dxd, dt)
+        ggen.fx_hydro_advance(Ug, dxd, dt)
+        tol = 1e-12 * (1 + 3 * step)
+        assert rel_err(Cfg, gplan.interior(Ud).cpu().numpy(), oplan.interior(Uo)) <= tol
+        assert rel_err(Cfg, gplan.interior(Ud).cpu().numpy(), ggen.interior(Ug).cpu().numpy()) <= tol
+    fo, _ = oplan.status()
+    fg, _ = gplan.fx_hydro_status()
+    assert fo == fg == 0
