@@ -317,6 +317,18 @@ int fx_halo_unpack(fx_hydro_plan *plan, double *U, const int32_t *items_dev, con
 int fx_hydro_advance_stage(fx_hydro_plan *plan, double *U, const double *dx_dev, double dt, const double *dt_dev, int stage,
                            double cfl_next, double *dt_next_dev, void *stream);
 int fx_hydro_stage_arrays(fx_hydro_plan *plan, double *U, int stage, double **stage_input, double **stage_output);
+/* A stage in two parts, so that the exchange of the ghost slabs can overlap the part of the stage that does not need them
+ * ("blocks are independent within a stage once halos are known"): FX_PART_INNER advances the
+ * owned blocks none of whose faces (nor those of the blocks chained with them in z) has a ghost block behind it -- it reads
+ * no ghost zone and may run while the slabs are under way --, FX_PART_BOUNDARY the others, once the ghosts are current.
+ * Both parts of a stage, in either order, equal fx_hydro_advance_stage bit for bit; dt_next_dev is given to BOTH parts of
+ * the last stage (the stage's last CTA finalises the reduction).  Only the fused kernel without passive scalars is split
+ * (fx_hydro_plan_path = 1): on every other path FX_PART_INNER does nothing and FX_PART_BOUNDARY is the whole stage.
+ * fx_hydro_plan_stage_parts: how many owned blocks each part advances (after the topology). */
+enum { FX_PART_INNER = 1, FX_PART_BOUNDARY = 2 };
+int fx_hydro_advance_stage_part(fx_hydro_plan *plan, double *U, const double *dx_dev, double dt, const double *dt_dev, int stage,
+                                int part, double cfl_next, double *dt_next_dev, void *stream);
+int fx_hydro_plan_stage_parts(const fx_hydro_plan *plan, int64_t *inner_blocks, int64_t *boundary_blocks);
 
 /* Which stage kernel fx_hydro_advance will use for this plan: 0 generic (zone kernel that reads its halo cells through
  * the neighbour table; the only path for plans with passive scalars, whose face guard zones it fills first),

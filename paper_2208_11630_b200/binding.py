@@ -18,6 +18,7 @@ OK, ERR_INVALID_ARG, ERR_STATE, ERR_UNSUPPORTED, ERR_WORKSPACE, ERR_CUDA = 0, -1
 RECON_PLM_MINMOD, RECON_WENO5 = 0, 1
 RIEMANN_HLLE, RIEMANN_HLLC = 0, 1
 BC_OUTFLOW, BC_NONE, BC_REFLECT = -1, -2, -3
+PART_INNER, PART_BOUNDARY = 1, 2
 NEIGH_COARSER, NEIGH_FINER = -4, -5
 TOPO_PERIODIC, TOPO_OUTFLOW, TOPO_NONE, TOPO_REFLECT = 0, 1, 2, 3
 ORDER_LEX, ORDER_MORTON = 0, 1
@@ -34,6 +35,7 @@ EXPORTS = [
     "fx_hydro_plan_set_timing", "fx_hydro_plan_get_timing",
     "fx_shard_create", "fx_shard_destroy", "fx_shard_sizes", "fx_shard_tables", "fx_shard_items", "fx_halo_item_elems",
     "fx_halo_pack", "fx_halo_unpack", "fx_hydro_advance_stage", "fx_hydro_stage_arrays",
+    "fx_hydro_advance_stage_part", "fx_hydro_plan_stage_parts",
 ]
 
 
@@ -100,6 +102,8 @@ def lib():
         L.fx_halo_unpack.argtypes = [vp, vp, vp, vp, C.c_int64, vp, vp]
         L.fx_hydro_advance_stage.argtypes = [vp, vp, vp, C.c_double, vp, C.c_int, C.c_double, vp, vp]
         L.fx_hydro_stage_arrays.argtypes = [vp, vp, C.c_int, C.POINTER(vp), C.POINTER(vp)]
+        L.fx_hydro_advance_stage_part.argtypes = [vp, vp, vp, C.c_double, vp, C.c_int, C.c_int, C.c_double, vp, vp]
+        L.fx_hydro_plan_stage_parts.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
         _lib = L
     return _lib
 
@@ -315,6 +319,19 @@ class HydroPlan:
         _check(lib().fx_hydro_advance_stage(self._h, _dev(U, torch.float64), _dev(dx, torch.float64), 0.0 if on_dev else float(dt),
                                             _dev(dt, torch.float64) if on_dev else None, stage, float(cfl_next),
                                             _dev(dt_next, torch.float64) if dt_next is not None else None, _stream(stream)))
+
+    def fx_hydro_advance_stage_part(self, U, dx, dt, stage, part, cfl_next=0.0, dt_next=None, stream=None):
+        """One part (PART_INNER: the owned blocks that read no ghost zone; PART_BOUNDARY: the others) of one RK stage."""
+        on_dev = isinstance(dt, torch.Tensor)
+        _check(lib().fx_hydro_advance_stage_part(self._h, _dev(U, torch.float64), _dev(dx, torch.float64), 0.0 if on_dev else float(dt),
+                                                 _dev(dt, torch.float64) if on_dev else None, stage, part, float(cfl_next),
+                                                 _dev(dt_next, torch.float64) if dt_next is not None else None, _stream(stream)))
+
+    def fx_hydro_plan_stage_parts(self):
+        """(owned blocks advanced by PART_INNER, by PART_BOUNDARY)."""
+        a, b = C.c_int64(0), C.c_int64(0)
+        _check(lib().fx_hydro_plan_stage_parts(self._h, C.byref(a), C.byref(b)))
+        return int(a.value), int(b.value)
 
     def fx_halo_item_elems(self, side):
         return int(lib().fx_halo_item_elems(self._h, side))

@@ -271,6 +271,8 @@ static int fx_seg_upload(fx_hydro_plan *plan) {
     FX_CUDA(cudaMemcpy(dst, plan->seg_host, (size_t)plan->nseg_host * FX_SEG_STRIDE * sizeof(int), cudaMemcpyHostToDevice));
   plan->P.seg = dst;
   plan->P.nseg = plan->nseg_host;
+  plan->P.nseg_all = plan->nseg_host;
+  plan->P.nseg_inner = plan->nseg_inner_host;
   plan->P.bseg = nullptr;
   plan->P.nbseg = 0;
   plan->P.njump = plan->jlist_host ? plan->njump_host : 0;  // (fused AMR path: the blocks with a jump face are single-block segments)
@@ -288,6 +290,8 @@ static int fx_seg_upload(fx_hydro_plan *plan) {
     plan->P.nbseg = plan->nbseg_host;
     plan->P.seg = nullptr;
     plan->P.nseg = 0;
+    plan->P.nseg_all = 0;
+    plan->P.nseg_inner = 0;
   }
   plan->seg_uploaded = true;
   return FX_OK;
@@ -483,6 +487,7 @@ extern "C" int fx_hydro_plan_set_topology(fx_hydro_plan *plan, const int32_t *ne
   delete[] plan->seg_host;
   plan->seg_host = nullptr;
   plan->nseg_host = 0;
+  plan->nseg_inner_host = 0;
   plan->seg_uploaded = false;
   if (nb > 0) {
     std::vector<int32_t> h((size_t)nb * 6);
@@ -575,6 +580,28 @@ extern "C" int fx_hydro_plan_set_topology(fx_hydro_plan *plan, const int32_t *ne
         row[0] = cnt;
         row[2 + cnt] = zact ? h[last * 6 + 5] : -1;
         ++plan->nseg_host;
+      }
+    }
+    // Sharded plans: the segments that touch no ghost block first, so that a stage can be launched in two parts -- those
+    // while the ghost slabs are still under way, the others once they have arrived (fx_hydro_advance_stage_part)
+    plan->nseg_inner_host = plan->nseg_host;
+    if (nown < nb && plan->nseg_host > 0) {
+      std::vector<int> rows((size_t)plan->nseg_host * FX_SEG_STRIDE);
+      memcpy(rows.data(), plan->seg_host, rows.size() * sizeof(int));
+      auto inner = [&](const int *row) {
+        if (row[1] >= nown || row[2 + row[0]] >= nown) return false;  // the z neighbours below / above the segment
+        for (int q = 0; q < row[0]; ++q)
+          for (int f = 0; f < 4; ++f)
+            if (plan->P.active[f / 2] && h[(long long)row[2 + q] * 6 + f] >= nown) return false;
+        return true;
+      };
+      int w = 0;
+      for (int pass = 0; pass < 2; ++pass) {
+        for (int r = 0; r < plan->nseg_host; ++r) {
+          const int *row = rows.data() + (size_t)r * FX_SEG_STRIDE;
+          if (inner(row) == (pass == 0)) memcpy(plan->seg_host + (size_t)w++ * FX_SEG_STRIDE, row, FX_SEG_STRIDE * sizeof(int));
+        }
+        if (pass == 0) plan->nseg_inner_host = w;
       }
     }
     for (long long q = 0; q < plan->njump_host; ++q) {  // the blocks with a jump face: one segment each

@@ -21,6 +21,9 @@ struct FxParams {
   const int *neigh;                 // [nblocks][6], device
   const int *seg;                   // z-chain segments of the fused kernel: [nseg][FX_SEG_STRIDE], device (in the workspace)
   int nseg;
+  int nseg_all;                     // segments of the whole stage (= nseg unless a launch covers a part of them: the fused CFL
+                                    // reduction is finalised by the last CTA of the stage, whichever launch it belongs to)
+  int nseg_inner;                   // sharded plans: the first nseg_inner segments touch no ghost block (fx_hydro_advance_stage_part)
   const int *bseg;                  // 8 x 8 blocks: segments of 2 x 2 BUNDLES, [nbseg][FX_BSEG_STRIDE] (same place in the workspace)
   int nbseg;
   int walls;                        // some block has a reflecting wall in an active dimension [B9]
@@ -74,6 +77,7 @@ struct fx_hydro_plan {
   int *bseg_host;       // bundle segments (8 x 8 blocks whose topology bundles completely), nbseg_host rows, or nullptr
   int nbseg_host;
   int nseg_host;
+  int nseg_inner_host;  // the leading segments none of whose blocks has a ghost block behind a face
   bool seg_uploaded;
   // optional per-launch timing of the stage kernels (fx_hydro_plan_set_timing)
   bool timing;

@@ -42,12 +42,32 @@ extern "C" int fx_hydro_compute_dt(fx_hydro_plan *plan, const double *U, const d
 // One stage: out = U0 + beta((X - U0) - S(X)); halos of X come from a K1 fill (generic path) or are
 // gathered from neighbour interiors inside the fused kernel.
 
+// part (fx_hydro_advance_stage_part): 0 the whole stage; 1 the segments that touch no ghost block; 2 the others.  Only the
+// fused kernel without passive scalars is launched in parts; every other path does nothing for part 1 and all for part 2.
 static int fx_stage(fx_hydro_plan *plan, double *X, const double *U0, double *out, const double *dx, double dt,
                     const double *dt_dev, double beta, int first, cudaStream_t st, double cfl_next = 0.0,
-                    double *dt_next = nullptr) {
+                    double *dt_next = nullptr, int part = 0) {
   const int path = fx_hydro_plan_path(plan);  // 1 fused TMA kernel (3: its pair variant), 2 shared-memory tile kernel, 0 generic
   const bool fused = path == 1 || path == 3 || path == 4;
   int rc = FX_OK;
+  if (part != 0) {
+    if (path == 1 && plan->nvars == 5) {
+      FxParams Q = plan->P;
+      const int ni = Q.nseg_inner;
+      Q.seg = part == 1 ? Q.seg : Q.seg + (size_t)ni * FX_SEG_STRIDE;
+      Q.nseg = part == 1 ? ni : Q.nseg - ni;
+      if (Q.nseg == 0) return FX_OK;
+      const bool rec = plan->timing && plan->ev && plan->nrec < FX_MAX_REC;
+      if (rec) FX_CUDA(cudaEventRecord(plan->ev[2 * plan->nrec], st));
+      if ((rc = fx_launch_stage_tma(Q, X, U0, out, dx, dt, dt_dev, beta, first, cfl_next, dt_next, st))) return rc;
+      if (rec) {
+        FX_CUDA(cudaEventRecord(plan->ev[2 * plan->nrec + 1], st));
+        ++plan->nrec;
+      }
+      return FX_OK;
+    }
+    if (part == 1) return FX_OK;
+  }
   if (path == 5) {
     // fused AMR path: guard zones behind the jumps, then the fused kernel on every block (the blocks with a jump face read
     // their own guard zones behind it and store the jump faces' fluxes), then the flux correction; the time step of the
@@ -168,6 +188,33 @@ extern "C" int fx_hydro_advance_stage(fx_hydro_plan *plan, double *U, const doub
   double *X, *out, beta;
   fx_stage_arrays(plan, U, stage, &X, &out, &beta);
   return fx_stage(plan, X, U, out, dx, dt, dt_dev, beta, stage == 0, (cudaStream_t)stream, cfl_next, dt_next_dev);
+}
+
+extern "C" int fx_hydro_advance_stage_part(fx_hydro_plan *plan, double *U, const double *dx, double dt, const double *dt_dev, int stage,
+                                           int part, double cfl_next, double *dt_next_dev, void *stream) {
+  int rc = fx_need(plan, true, true, "advance_stage_part");
+  if (rc) return rc;
+  if (part != FX_PART_INNER && part != FX_PART_BOUNDARY) return fx_fail(FX_ERR_INVALID_ARG, "advance_stage_part: part must be FX_PART_INNER or FX_PART_BOUNDARY");
+  if (stage < 0 || stage >= plan->rk) return fx_fail(FX_ERR_INVALID_ARG, "advance_stage_part: stage must be 0 .. rk_order - 1");
+  if (!dt_dev && (!(dt > 0.0) || !isfinite(dt))) return fx_fail(FX_ERR_INVALID_ARG, "advance_stage_part: dt must be positive and finite");
+  if ((!U || !dx) && plan->P.nblocks > 0) return fx_fail(FX_ERR_INVALID_ARG, "advance_stage_part: null argument");
+  if (dt_next_dev && stage != plan->rk - 1) return fx_fail(FX_ERR_INVALID_ARG, "advance_stage_part: the next time step comes out of the last stage only");
+  if (dt_next_dev && (!(cfl_next > 0.0) || !isfinite(cfl_next))) return fx_fail(FX_ERR_INVALID_ARG, "advance_stage_part: cfl must be positive and finite");
+  if (plan->P.nown == 0) return FX_OK;
+  double *X, *out, beta;
+  fx_stage_arrays(plan, U, stage, &X, &out, &beta);
+  return fx_stage(plan, X, U, out, dx, dt, dt_dev, beta, stage == 0, (cudaStream_t)stream, cfl_next, dt_next_dev, part);
+}
+
+extern "C" int fx_hydro_plan_stage_parts(const fx_hydro_plan *plan, int64_t *inner_blocks, int64_t *boundary_blocks) {
+  if (!plan || !inner_blocks || !boundary_blocks) return fx_fail(FX_ERR_INVALID_ARG, "stage_parts: null argument");
+  if (!plan->topology_set) return fx_fail(FX_ERR_STATE, "stage_parts: set the topology first");
+  int64_t ni = 0;
+  if (fx_hydro_plan_path(plan) == 1 && plan->nvars == 5 && plan->seg_host)
+    for (int r = 0; r < plan->nseg_inner_host; ++r) ni += plan->seg_host[(size_t)r * FX_SEG_STRIDE];
+  *inner_blocks = ni;
+  *boundary_blocks = plan->P.nown - ni;
+  return FX_OK;
 }
 
 static int fx_advance_impl(fx_hydro_plan *plan, double *U, const double *dx, double dt, const double *dt_dev,

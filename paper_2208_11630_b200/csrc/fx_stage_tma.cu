@@ -565,7 +565,7 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
         atomicMax(&P.scratch[FX_SCR_DTBITS], (unsigned long long)__double_as_longlong(mx));
         __threadfence();
         const unsigned long long done = atomicAdd(&P.scratch[FX_SCR_COUNTER], 1ull);
-        if (done == gridDim.x - 1) {
+        if (done == (unsigned long long)P.nseg_all - 1) {  // the stage's last CTA (the stage may be launched in two parts)
           __threadfence();
           const unsigned long long bits = atomicExch(&P.scratch[FX_SCR_DTBITS], 0ull);
           P.scratch[FX_SCR_COUNTER] = 0ull;

@@ -113,3 +113,88 @@ def test_sharded_equals_single_plan_bitwise(number, nb, block, recon, rk, guard_
         if cfg.block_dims[0] == 16:
             core = sh.plan.interior(Ur)[:, sh.n_owned:, 4:12 if cfg.block_dims[2] > 1 else 0:1, 4:12, 4:12]
             assert torch.isnan(core).all()
+
+
+@pytest.mark.parametrize("recon,rk,guard_x", [(0, 2, 8), (1, 3, 4)])
+def test_stage_in_two_parts_inner_reads_no_ghost(recon, rk, guard_x):
+    """fx_hydro_advance_stage_part: FX_PART_INNER runs BEFORE the exchange with every ghost block of the stage input full of
+    NaN, FX_PART_BOUNDARY after it; the union of the ranks' owned blocks still equals the single plan bit for bit, and so
+    does the time step (the fused reduction is finalised by the stage's last CTA, whichever launch it is in).  The tiling is
+    cut in y with outflow there, so that each rank has blocks away from the cut."""
+    from paper_2208_11630_b200 import binding as fx
+    from paper_2208_11630_b200.sharded import ShardedHydro
+    cfg = inputs.config(5, nb=(4, 4, 2))
+    bcs = [fx.TOPO_PERIODIC, fx.TOPO_OUTFLOW, fx.TOPO_PERIODIC]
+    neigh, coords = fx.fx_topology_cartesian(cfg.nb, bcs, bcs, fx.ORDER_MORTON)
+    world, steps = 2, 3
+    ranks = [ShardedHydro(cfg.block_dims, cfg.nguard, cfg.gamma, recon, cfg.riemann, rk, neigh, r, world, guard_x=guard_x) for r in range(world)]
+    Ui = inputs.block_interiors(cfg, coords)
+    dx_all = inputs.dx_array(cfg)
+    Us, dxs = [], []
+    for sh in ranks:
+        sh.world = 1
+        assert sh.plan.path == 1
+        ni, nbd = sh.plan.fx_hydro_plan_stage_parts()
+        assert ni > 0 and nbd > 0 and ni + nbd == sh.n_owned
+        U = sh.alloc_state(fill=float("nan"))
+        sh.interior(U)[...] = Ui[:, sh.shard.global_id[:sh.n_owned]].cuda()
+        Us.append(U)
+        dxs.append(torch.from_numpy(np.ascontiguousarray(dx_all[sh.shard.global_id])).cuda())
+    dts = [sh.plan.fx_hydro_compute_dt(U, dx, cfg.cfl).clone() for sh, U, dx in zip(ranks, Us, dxs)]
+    m = torch.stack(dts).min()
+    for d in dts:
+        d.copy_(m)
+    hist = [float(m.item())]
+    for _ in range(steps):
+        for s in range(rk):
+            last = s == rk - 1
+            kw = [dict(cfl_next=cfg.cfl, dt_next=dt) if last else {} for dt in dts]
+            for sh, U, dx, dt, k in zip(ranks, Us, dxs, dts, kw):
+                X, _ = sh.plan.fx_hydro_stage_arrays(U, s)
+                # poison the ghost blocks of the stage's input (the array at X: U itself or a stage copy inside the workspace)
+                if X == U.data_ptr():
+                    view = U
+                else:
+                    ws = sh.plan._ws
+                    off = X - ws.data_ptr()
+                    assert 0 < off < ws.numel() and off % 8 == 0
+                    view = ws[off:off + U.numel() * 8].view(torch.float64).view(U.shape)
+                view[:, sh.n_owned:] = float("nan")
+                sh.plan.fx_hydro_advance_stage_part(U, dx, dt, s, fx.PART_INNER, **k)
+            for sh, U in zip(ranks, Us):
+                X, _ = sh.plan.fx_hydro_stage_arrays(U, s)
+                sh.pack(X)
+            torch.cuda.synchronize()
+            for q, sh in enumerate(ranks):
+                ro = 0
+                for p, src in enumerate(ranks):
+                    n = sh.recv_splits[p]
+                    so = sum(src.send_splits[:q])
+                    sh.recv_buf[ro:ro + n] = src.send_buf[so:so + n]
+                    ro += n
+            for sh, U, dx, dt, k in zip(ranks, Us, dxs, dts, kw):
+                X, _ = sh.plan.fx_hydro_stage_arrays(U, s)
+                sh.unpack(X)
+                sh.plan.fx_hydro_advance_stage_part(U, dx, dt, s, fx.PART_BOUNDARY, **k)
+        m = torch.stack(dts).min()
+        for d in dts:
+            d.copy_(m)
+        hist.append(float(m.item()))
+    got = torch.empty((5,) + tuple(Ui.shape[1:]), dtype=torch.float64)
+    for sh, U in zip(ranks, Us):
+        got[:, sh.shard.global_id[:sh.n_owned]] = sh.interior(U).cpu()
+    plan = fx.HydroPlan(cfg.block_dims, cfg.nguard, cfg.nblocks, cfg.gamma, recon, cfg.riemann, rk)
+    if guard_x != cfg.nguard:
+        plan.fx_hydro_plan_set_option(fx.OPT_GUARD_X, guard_x)
+    plan.fx_hydro_plan_set_topology(neigh)
+    plan.fx_hydro_plan_set_workspace()
+    U = plan.alloc_state(fill=float("nan"))
+    plan.interior(U)[...] = Ui.cuda()
+    dx = torch.from_numpy(dx_all).cuda()
+    dt = plan.fx_hydro_compute_dt(U, dx, cfg.cfl).clone()
+    ref_hist = [float(dt.item())]
+    for _ in range(steps):
+        plan.fx_hydro_step(U, dx, cfg.cfl, dt)
+        ref_hist.append(float(dt.item()))
+    assert hist == ref_hist
+    assert torch.equal(got, plan.interior(U).cpu())
