@@ -434,6 +434,8 @@ def run_ours(args, rank, world, local_rank):
         launches_per_step = stages * 3 + 1
     if sh is not None:
         launches_per_step += (int(sh.send_elems > 0) + int(sh.recv_elems > 0)) * stages  # pack + unpack of the cut-face slabs before every stage
+        if sh.overlap:  # a stage in two launches: the blocks away from the cut beside the exchange, the others behind it
+            launches_per_step += stages
         dt = sh.compute_dt(U, dx, cfg.cfl)  # the minimum over the ranks
 
         def step():
@@ -527,10 +529,12 @@ def run_ours(args, rank, world, local_rank):
                                    + (", Davis wave speeds" if args.wavespeed else ""),
                        "interior_zones": zones, "state_bytes": plan.bytes_per_state, "block_order": args.order,
                        "layout": f"x guard depth {plan.gd[0]} (row pitch {plan.S_j * 8} B), y/z guard depth {plan.gd[1]}/{plan.gd[2]}",
-                       "path": "communication-avoiding step (one guard fill per step; generic kernels on the extended interior)" if args.ca else {0: "generic", 5: f"fused (TMA) on the blocks without a refinement jump + generic on the {getattr(cfg, 'jump_blocks', 0)} blocks with one", 1: "fused (TMA)", 2: "tile (shared-memory block)", 3: "fused (TMA), two zones per thread", 4: "fused (TMA), 2 x 2 bundles of 8 x 8 blocks"}[plan.path], "l2": "inputs (state) larger than L2; no flush needed",
+                       "path": "communication-avoiding step (one guard fill per step; generic kernels on the extended interior)" if args.ca else {0: "generic", 5: f"fused (TMA); the {getattr(cfg, 'jump_blocks', 0)} blocks with a refinement jump as single-block segments reading their own guard zones", 1: "fused (TMA)", 2: "tile (shared-memory block)", 3: "fused (TMA), two zones per thread", 4: "fused (TMA), 2 x 2 bundles of 8 x 8 blocks"}[plan.path], "l2": "inputs (state) larger than L2; no flush needed",
                        "multi_gpu": (f"sharded: tiling {cfg.nb[0]}x{cfg.nb[1]}x{cfg.nb[2]} blocks in {world} contiguous Morton runs, "
                                      f"{sh.shard.n_ghost} ghost blocks on rank 0, cut-face slabs exchanged before every stage "
-                                     f"(grouped NCCL send/recv, {sh.send_elems * 8} B sent by rank 0 per stage), dt = all-reduce(min)")
+                                     f"(grouped NCCL send/recv, {sh.send_elems * 8} B sent by rank 0 per stage"
+                                     + (", on a stream of its own beside the stage's launch over the blocks away from the cut" if sh.overlap else "")
+                                     + "), dt = all-reduce(min)")
                        if sh is not None else "single"},
             "clocks": clocks, "gpu_launches": launches_per_step * args.steps, "roofline": roofline,
             "status_flags": flags}

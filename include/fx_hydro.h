@@ -321,7 +321,7 @@ int fx_hydro_stage_arrays(fx_hydro_plan *plan, double *U, int stage, double **st
  * ("blocks are independent within a stage once halos are known"): FX_PART_INNER advances the
  * owned blocks none of whose faces (nor those of the blocks chained with them in z) has a ghost block behind it -- it reads
  * no ghost zone and may run while the slabs are under way --, FX_PART_BOUNDARY the others, once the ghosts are current.
- * Both parts of a stage, in either order, equal fx_hydro_advance_stage bit for bit; dt_next_dev is given to BOTH parts of
+ * Both parts of a stage, in either order or side by side on two streams, equal fx_hydro_advance_stage bit for bit; dt_next_dev is given to BOTH parts of
  * the last stage (the stage's last CTA finalises the reduction).  Only the fused kernel without passive scalars is split
  * (fx_hydro_plan_path = 1): on every other path FX_PART_INNER does nothing and FX_PART_BOUNDARY is the whole stage.
  * fx_hydro_plan_stage_parts: how many owned blocks each part advances (after the topology). */

@@ -556,6 +556,13 @@ extern "C" int fx_hydro_plan_set_topology(fx_hydro_plan *plan, const int32_t *ne
       }
     }
     if (plan->P.n[2] > 64) M = 1;
+    // Sharded plans: a block with a ghost block behind a face is chained only with its like, so that the layers of a
+    // column next to a cut do not drag the rest of it into the part of a stage that waits for the exchange
+    std::vector<char> touch((size_t)nb, 0);
+    if (nown < nb)
+      for (long long b = 0; b < nown; ++b)
+        for (int f = 0; f < 6; ++f)
+          if (plan->P.active[f / 2] && h[b * 6 + f] >= nown) touch[b] = 1;
     for (long long b0 = 0; b0 < nown; ++b0) {
       if (seen[b0]) continue;
       long long start = b0;
@@ -571,7 +578,8 @@ extern "C" int fx_hydro_plan_set_topology(fx_hydro_plan *plan, const int32_t *ne
         int cnt = 0;
         row[1] = zact ? h[b * 6 + 4] : -1;
         long long last = b;
-        while (b >= 0 && !seen[b] && cnt < M) {
+        const char kind = touch[b];
+        while (b >= 0 && !seen[b] && cnt < M && touch[b] == kind) {
           seen[b] = 1;
           row[2 + cnt++] = (int)b;
           last = b;

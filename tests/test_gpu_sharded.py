@@ -198,3 +198,94 @@ def test_stage_in_two_parts_inner_reads_no_ghost(recon, rk, guard_x):
         ref_hist.append(float(dt.item()))
     assert hist == ref_hist
     assert torch.equal(got, plan.interior(U).cpu())
+
+
+def test_overlapped_step_of_two_ranks_in_two_threads():
+    """ShardedHydro.step as the ranks run it -- the exchange on a stream of its own beside FX_PART_INNER, FX_PART_BOUNDARY behind
+    the event -- with the two ranks of a partition driven by two host threads on this GPU (the rank-to-rank transfer and the
+    time-step minimum are replaced by copies between the ranks' buffers at a host barrier; no kernel waits for another
+    rank's): bit for bit the single plan's result and time steps."""
+    import threading
+    from paper_2208_11630_b200 import binding as fx
+    from paper_2208_11630_b200.sharded import ShardedHydro
+    cfg = inputs.config(5, nb=(4, 4, 2))
+    bcs = [fx.TOPO_PERIODIC, fx.TOPO_OUTFLOW, fx.TOPO_PERIODIC]
+    neigh, coords = fx.fx_topology_cartesian(cfg.nb, bcs, bcs, fx.ORDER_MORTON)
+    world, steps = 2, 4
+    ranks = [ShardedHydro(cfg.block_dims, cfg.nguard, cfg.gamma, 0, cfg.riemann, 2, neigh, r, world, guard_x=8) for r in range(world)]
+    assert all(sh.overlap for sh in ranks)
+    Ui = inputs.block_interiors(cfg, coords)
+    dx_all = inputs.dx_array(cfg)
+    bar = threading.Barrier(world)
+    shared_dt = [None] * world
+
+    def make_transfer(q):
+        sh = ranks[q]
+
+        def transfer():
+            torch.cuda.current_stream().synchronize()  # this rank's pack (on its exchange stream) is done
+            bar.wait()
+            ro = 0
+            for p, src in enumerate(ranks):
+                n = sh.recv_splits[p]
+                so = sum(src.send_splits[:q])
+                sh.recv_buf[ro:ro + n].copy_(src.send_buf[so:so + n])
+                ro += n
+            torch.cuda.current_stream().synchronize()
+            bar.wait()  # nobody packs the next stage before everybody has copied this one
+        return transfer
+
+    def make_min(q):
+        def global_min(dt):
+            torch.cuda.synchronize()
+            shared_dt[q] = float(dt.item())
+            bar.wait()
+            dt.fill_(min(shared_dt))
+            bar.wait()
+            return dt
+        return global_min
+
+    results, hists, errors = [None] * world, [None] * world, []
+
+    def run(q):
+        try:
+            sh = ranks[q]
+            sh.transfer, sh._global_min = make_transfer(q), make_min(q)
+            with torch.cuda.stream(torch.cuda.Stream()):
+                U = sh.alloc_state(fill=float("nan"))
+                sh.interior(U)[...] = Ui[:, sh.shard.global_id[:sh.n_owned]].cuda()
+                dx = torch.from_numpy(np.ascontiguousarray(dx_all[sh.shard.global_id])).cuda()
+                dt = sh.compute_dt(U, dx, cfg.cfl)
+                hist = [float(dt.item())]
+                for _ in range(steps):
+                    sh.step(U, dx, cfg.cfl, dt)
+                    hist.append(float(dt.item()))
+                torch.cuda.synchronize()
+                results[q], hists[q] = sh.interior(U).cpu(), hist
+        except Exception as e:  # a failing rank must not leave the other at the barrier
+            errors.append(e)
+            bar.abort()
+
+    threads = [threading.Thread(target=run, args=(q,)) for q in range(world)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join(timeout=120)
+    assert not errors, errors
+    got = torch.empty((5,) + tuple(Ui.shape[1:]), dtype=torch.float64)
+    for sh, r in zip(ranks, results):
+        got[:, sh.shard.global_id[:sh.n_owned]] = r
+    plan = fx.HydroPlan(cfg.block_dims, cfg.nguard, cfg.nblocks, cfg.gamma, 0, cfg.riemann, 2)
+    plan.fx_hydro_plan_set_option(fx.OPT_GUARD_X, 8)
+    plan.fx_hydro_plan_set_topology(neigh)
+    plan.fx_hydro_plan_set_workspace()
+    U = plan.alloc_state(fill=float("nan"))
+    plan.interior(U)[...] = Ui.cuda()
+    dx = torch.from_numpy(dx_all).cuda()
+    dt = plan.fx_hydro_compute_dt(U, dx, cfg.cfl).clone()
+    ref_hist = [float(dt.item())]
+    for _ in range(steps):
+        plan.fx_hydro_step(U, dx, cfg.cfl, dt)
+        ref_hist.append(float(dt.item()))
+    assert hists[0] == ref_hist and hists[1] == ref_hist
+    assert torch.equal(got, plan.interior(U).cpu())
