@@ -230,3 +230,61 @@ def test_mirror_symmetric_patch_gives_mirror_symmetric_flow():
         assert np.allclose(I[0, b], I[0, m][..., ::-1], rtol=1e-13, atol=0)
         assert np.allclose(I[1, b], -I[1, m][..., ::-1], rtol=0, atol=1e-13)
         assert np.allclose(I[4, b], I[4, m][..., ::-1], rtol=1e-13, atol=0)
+
+
+# ---- passive mass scalars through refinement jumps [B11 with B12-B14]: the scalars are conserved variables like the rest,
+# so restriction, prolongation and the flux correction act on rho X_s as they act on a momentum component
+def with_scalars(fields, X):
+    """fields [5, ...] conserved; X: list of abundance arrays -> [5 + ns, ...]."""
+    return np.concatenate([fields, np.stack([fields[0] * x for x in X])])
+
+
+@pytest.mark.parametrize("recon,riemann,rk", [(0, 1, 2), (0, 0, 3), (1, 1, 3)])
+def test_scalar_equal_to_w_is_the_out_of_plane_momentum_bitwise_through_jumps(recon, riemann, rk):
+    """2-D two-level grid, w a smooth field: a scalar with X = w is advected, restricted, prolonged and flux-corrected
+    exactly as m_z is -- rho X stays equal to m_z BIT FOR BIT; and the hydro variables are those of the run without scalars."""
+    dims = (8, 8, 1)
+    grid = two_level_grid((4, 4, 1), {(1, 1, 0), (2, 1, 0)}, dims)
+    f5 = smooth_field(grid, dims, [32, 32, 1])
+    X = amr_zone_centres(grid, dims)
+    w = 0.3 * np.sin(2 * np.pi * X[:, 0] / 32) * np.cos(2 * np.pi * X[:, 1] / 32 + 0.4)
+    f5[3] = f5[0] * w
+    f5[4] = f5[4] + 0.5 * f5[0] * w * w
+    plan5 = amr_plan(grid, dims, recon=recon, riemann=riemann, rk=rk)
+    plan7 = amr_plan(grid, dims, recon=recon, riemann=riemann, rk=rk, nvars=7)
+    U5 = state_from(plan5, f5)
+    U7 = state_from(plan7, with_scalars(f5, [w, np.full_like(w, 0.25)]))
+    dx = dx_of(grid)
+    for _ in range(6):
+        dt = plan5.compute_dt(U5, dx, 0.4)
+        assert dt == plan7.compute_dt(U7, dx, 0.4)
+        plan5.advance(U5, dx, dt)
+        plan7.advance(U7, dx, dt)
+    I5, I7 = plan5.interior(U5), plan7.interior(U7)
+    assert np.array_equal(I7[:5], I5)
+    assert np.array_equal(I7[5], I7[3]) and np.abs(I7[3]).max() > 0.01
+    assert np.max(np.abs(I7[6] - 0.25 * I7[0])) <= 2e-15  # a uniform abundance stays uniform
+    fo, _ = plan7.status()
+    assert fo == 0
+
+
+@pytest.mark.parametrize("nbc,refined,dims,periodic", [((3, 3, 3), {(1, 1, 1)}, (8, 8, 8), True),
+                                                        ((3, 3, 2), {(0, 0, 0), (1, 0, 0), (2, 2, 1)}, (8, 8, 8), True)])
+def test_scalar_mass_is_conserved_through_jumps(nbc, refined, dims, periodic):
+    grid = two_level_grid(nbc, refined, dims, periodic=periodic)
+    L = [nbc[d] * dims[d] for d in range(3)]
+    f5 = smooth_field(grid, dims, L)
+    X = amr_zone_centres(grid, dims)
+    xa = 0.5 + 0.4 * np.sin(2 * np.pi * X[:, 0] / L[0]) * np.cos(2 * np.pi * X[:, 2] / L[2])
+    xb = (np.abs(X[:, 1] - 0.5 * L[1]) < 0.2 * L[1]).astype(float)  # a slab that crosses the refined region
+    plan = amr_plan(grid, dims, nvars=7)
+    U = state_from(plan, with_scalars(f5, [xa, xb]))
+    dx = dx_of(grid)
+    T0 = totals(plan, grid, U, 3)
+    for _ in range(10):
+        plan.advance(U, dx, plan.compute_dt(U, dx, 0.3))
+    T1 = totals(plan, grid, U, 3)
+    for v in (0, 4, 5, 6):
+        assert abs(T1[v] - T0[v]) <= 1e-13 * T0[0], (v, T1[v] - T0[v])
+    I = plan.interior(U)
+    assert np.abs(I[6] - xb * I[0]).max() > 1e-3  # the slab moved
