@@ -166,7 +166,9 @@ int fx_hydro_plan_set_topology(fx_hydro_plan *plan, const int32_t *neigh_dev);
  * jump gives slope 0); and the flux of a coarse face at a jump is replaced by the mean of the fine face fluxes that cover
  * it (FLUX CORRECTION: what leaves the fine blocks enters the coarse one).  Edge and corner guard zones next to a jump hold
  * a clamp (the stage reads none [A11]); fx_guardcell_index_map reports the clamp for zones behind a jump.  Plans with
- * jumps run on the generic path, or on the fused one where the block shape is its (FX_OPT_PATH).  Call before the workspace (which grows by the jump faces' flux buffer) and the
+ * jumps run on the generic path, or on the fused one where the block shape is its (FX_OPT_PATH).  Passive mass scalars
+ * (nvars > 5) go through the jumps like the conserved variables they are -- restricted, prolonged, their fluxes corrected --
+ * on the generic path.  Call before the workspace (which grows by the jump faces' flux buffer) and the
  * topology.  Needs even block extents and nguard <= n_d / 2 in active dimensions (FX_ERR_INVALID_ARG). */
 int fx_hydro_plan_set_refinement(fx_hydro_plan *plan, const int32_t *jump_dev);
 

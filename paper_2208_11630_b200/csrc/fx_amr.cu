@@ -121,16 +121,19 @@ __global__ void __launch_bounds__(256) fx_k_amr_fill(const FxParams P, double *U
     c[d2] = t2;
     double *dst = U + b * P.S_b + (long long)(c[2] + P.gd[2]) * P.S_k + (long long)(c[1] + P.gd[1]) * P.S_j + (c[0] + P.gd[0]);
     // (every value a zone needs is loaded before its first store: the loads of all variables are then in flight together
-    // instead of one DRAM round trip per variable; jumps come with the five hydro variables only -- set_topology refuses
-    // them with passive scalars)
+    // instead of one DRAM round trip per variable)
     if (code == FX_NEIGH_FINER) {
       AmrSrc s;
       amr_locate(P, b, c, s);
-      double val[5];
+      for (int v0 = 0; v0 < P.nvars; v0 += 5) {  // (five variables at a time: the hydro set, then the passive scalars)
+        double val[5];
 #pragma unroll
-      for (int v = 0; v < 5; ++v) val[v] = amr_value(P, U, s, v);
+        for (int v = 0; v < 5; ++v)
+          if (v0 + v < P.nvars) val[v] = amr_value(P, U, s, v0 + v);
 #pragma unroll
-      for (int v = 0; v < 5; ++v) dst[(long long)v * P.S_v] = val[v];
+        for (int v = 0; v < 5; ++v)
+          if (v0 + v < P.nvars) dst[(long long)(v0 + v) * P.S_v] = val[v];
+      }
     } else {
       const long long cb = __ldg(&P.jump[(b * 6 + f) * 4 + 0]);
       const int qd = __ldg(&P.jump[(b * 6 + f) * 4 + 1]);
@@ -157,34 +160,39 @@ __global__ void __launch_bounds__(256) fx_k_amr_fill(const FxParams P, double *U
         Cp[e2] += 1;
         both[e2] = amr_locate(P, cb, Cm, sm[e2]) && amr_locate(P, cb, Cp, sp[e2]);
       }
-      double qC[5], qm[3][5], qp[3][5];
+      for (int v0 = 0; v0 < P.nvars; v0 += 5) {
+        double qC[5], qm[3][5], qp[3][5];
 #pragma unroll
-      for (int v = 0; v < 5; ++v) qC[v] = amr_value(P, U, sC, v);
-#pragma unroll
-      for (int e2 = 0; e2 < 3; ++e2) {
-        if (!both[e2]) continue;
-#pragma unroll
-        for (int v = 0; v < 5; ++v) {
-          qm[e2][v] = amr_value(P, U, sm[e2], v);
-          qp[e2][v] = amr_value(P, U, sp[e2], v);
-        }
-      }
-#pragma unroll
-      for (int v = 0; v < 5; ++v) {
-        double val = qC[v];
+        for (int v = 0; v < 5; ++v)
+          if (v0 + v < P.nvars) qC[v] = amr_value(P, U, sC, v0 + v);
 #pragma unroll
         for (int e2 = 0; e2 < 3; ++e2) {
           if (!both[e2]) continue;
-          val = __dadd_rn(val, __dmul_rn(sg[e2] * 0.25, amr_minmod(__dsub_rn(qC[v], qm[e2][v]), __dsub_rn(qp[e2][v], qC[v]))));
+#pragma unroll
+          for (int v = 0; v < 5; ++v) {
+            if (v0 + v >= P.nvars) continue;
+            qm[e2][v] = amr_value(P, U, sm[e2], v0 + v);
+            qp[e2][v] = amr_value(P, U, sp[e2], v0 + v);
+          }
         }
-        dst[(long long)v * P.S_v] = val;
+#pragma unroll
+        for (int v = 0; v < 5; ++v) {
+          if (v0 + v >= P.nvars) continue;
+          double val = qC[v];
+#pragma unroll
+          for (int e2 = 0; e2 < 3; ++e2) {
+            if (!both[e2]) continue;
+            val = __dadd_rn(val, __dmul_rn(sg[e2] * 0.25, amr_minmod(__dsub_rn(qC[v], qm[e2][v]), __dsub_rn(qp[e2][v], qC[v]))));
+          }
+          dst[(long long)(v0 + v) * P.S_v] = val;
+        }
       }
     }
   }
 }
 
 // Flux correction [B14]: one CTA per (block, face) with finer neighbours; out -= (+-) beta dt/dx (mean of the fine fluxes
-// - the block's own flux) in the zones next to the face.  fjump[((b 6 + f) 5 + v) A + t2 n1 + t1] holds the boundary
+// - the block's own flux) in the zones next to the face.  fjump[((b 6 + f) nvars + v) A + t2 n1 + t1] holds the boundary
 // fluxes the stage kernel captured at every jump face (both sides).
 __global__ void __launch_bounds__(128) fx_k_amr_flux_correct(const FxParams P, double *out, const double *__restrict__ dx, double dt,
                                                              const double *__restrict__ dt_dev, double beta) {
@@ -197,7 +205,8 @@ __global__ void __launch_bounds__(128) fx_k_amr_flux_correct(const FxParams P, d
   const int n1 = P.n[d1], n2 = P.n[d2];
   const long long A = (long long)P.fj_area;
   const double r = beta * (dt / __ldg(&dx[b * 3 + d]));
-  for (int t = threadIdx.x; t < 5 * n1 * n2; t += blockDim.x) {
+  const int nv = P.nvars;  // the passive scalars' fluxes are corrected like the others [B11]
+  for (int t = threadIdx.x; t < nv * n1 * n2; t += blockDim.x) {
     const int v = t / (n1 * n2), r2 = t - v * (n1 * n2), t2 = r2 / n1, t1 = r2 - t2 * n1;
     const int tr[2] = {d1, d2}, tc[2] = {t1, t2};
     int q = 0, ft[2] = {0, 0}, cnt[2] = {1, 1};
@@ -214,9 +223,9 @@ __global__ void __launch_bounds__(128) fx_k_amr_flux_correct(const FxParams P, d
     const int ff = 2 * d + (1 - side);
     double sum = 0.0;
     for (int j2 = 0; j2 < cnt[1]; ++j2)
-      for (int j1 = 0; j1 < cnt[0]; ++j1) sum += P.fjump[((fb * 6 + ff) * 5 + v) * A + (long long)(ft[1] + j2) * n1 + (ft[0] + j1)];
+      for (int j1 = 0; j1 < cnt[0]; ++j1) sum += P.fjump[((fb * 6 + ff) * nv + v) * A + (long long)(ft[1] + j2) * n1 + (ft[0] + j1)];
     const double fbar = sum * (1.0 / (double)(cnt[0] * cnt[1]));
-    const double fown = P.fjump[((b * 6 + f) * 5 + v) * A + (long long)t2 * n1 + t1];
+    const double fown = P.fjump[((b * 6 + f) * nv + v) * A + (long long)t2 * n1 + t1];
     int c[3];
     c[d] = side ? P.n[d] - 1 : 0;
     c[d1] = t1;

@@ -251,7 +251,7 @@ static size_t fx_fq_bytes(const fx_hydro_plan *plan) {  // scalar pass [B11]: (m
 
 static size_t fx_fjump_bytes(const fx_hydro_plan *plan) {  // boundary fluxes at refinement jumps [B14]
   if (!plan->P.jump) return 0;
-  return (((size_t)plan->P.nblocks * 6 * 5 * (size_t)plan->P.fj_area * sizeof(double)) + 255) & ~(size_t)255;
+  return (((size_t)plan->P.nblocks * 6 * (size_t)plan->nvars * (size_t)plan->P.fj_area * sizeof(double)) + 255) & ~(size_t)255;
 }
 
 // The stage copies start `fx_stage_pad` bytes into a 256-byte pad block, so that their interior rows start on a
@@ -459,7 +459,6 @@ extern "C" int fx_hydro_plan_set_topology(fx_hydro_plan *plan, const int32_t *ne
           if (v >= nb) return fx_fail(FX_ERR_INVALID_ARG, "set_topology: block %lld face %d -> id %d out of range", b, f, v);
         } else if (v == FX_NEIGH_COARSER || v == FX_NEIGH_FINER) {
           if (!plan->jump_host) return fx_fail(FX_ERR_UNSUPPORTED, "set_topology: block %lld face %d is a refinement jump: call fx_hydro_plan_set_refinement first", b, f);
-          if (plan->nvars > 5) return fx_fail(FX_ERR_UNSUPPORTED, "set_topology: refinement jumps with passive scalars are not supported");
           if (plan->P.nown != nb) return fx_fail(FX_ERR_UNSUPPORTED, "set_topology: refinement jumps in a sharded plan are not supported");
           const int nq = v == FX_NEIGH_COARSER ? 1 : (1 << (plan->P.active[0] + plan->P.active[1] + plan->P.active[2] - 1));
           for (int q = 0; q < nq; ++q) {

@@ -196,11 +196,11 @@ __device__ __forceinline__ unsigned fx_zone_direction(const FxParams &P, const d
   if (AMR) {  // the boundary fluxes at refinement jumps, both sides, for the flux correction [B14]
     if (idx == 0 && __ldg(&P.neigh[b * 6 + 2 * D]) <= FX_NEIGH_COARSER) {
 #pragma unroll
-      for (int f = 0; f < 5; ++f) P.fjump[((b * 6 + 2 * D) * 5 + map[f]) * (long long)P.fj_area + tflat] = Fm[f];
+      for (int f = 0; f < 5; ++f) P.fjump[((b * 6 + 2 * D) * P.nvars + map[f]) * (long long)P.fj_area + tflat] = Fm[f];
     }
     if (idx == P.n[D] - 1 && __ldg(&P.neigh[b * 6 + 2 * D + 1]) <= FX_NEIGH_COARSER) {
 #pragma unroll
-      for (int f = 0; f < 5; ++f) P.fjump[((b * 6 + 2 * D + 1) * 5 + map[f]) * (long long)P.fj_area + tflat] = Fp[f];
+      for (int f = 0; f < 5; ++f) P.fjump[((b * 6 + 2 * D + 1) * P.nvars + map[f]) * (long long)P.fj_area + tflat] = Fp[f];
     }
   }
   if (SCALARS) {
@@ -214,10 +214,14 @@ __device__ __forceinline__ unsigned fx_zone_direction(const FxParams &P, const d
 }
 
 // One scalar, direction D: r dt/dx (F+ - F-) with flux = Aq X_L + (mass flux - Aq) X_R [B11].
-template <int RECON, int D>
+// AMR: the scalar's fluxes through the block's jump faces are stored with the hydro variables' [B14]; jf = bit 0 / 1: the
+// zone's low / high face along D is such a face, slot = the face's entry of variable sv in P.fjump (for the low face;
+// the high face's is one face further)
+template <int RECON, int D, bool AMR = false>
 __device__ __forceinline__ double fx_zone_scalar_direction(const FxParams &P, const double *__restrict__ Q, long long c,
                                                            long long s, double rd, unsigned qfb,
-                                                           const FxScalarShared<RECON> *sh, unsigned &hit) {
+                                                           const FxScalarShared<RECON> *sh, unsigned &hit, unsigned jf = 0,
+                                                           long long slot = 0) {
   constexpr int RS = (RECON == FX_RECON_PLM_MINMOD) ? 2 : 3;
   double x[2 * RS + 1];
 #pragma unroll
@@ -234,6 +238,10 @@ __device__ __forceinline__ double fx_zone_scalar_direction(const FxParams &P, co
   const double Fm = Am * mL + (sh->F[D][0][threadIdx.x] - Am) * mR;
   const double Fp = Ap * pL + (sh->F[D][1][threadIdx.x] - Ap) * pR;
   if (!(fabs(Fm + Fp) <= 1.79e308)) hit |= FX_STATUS_NONFINITE;
+  if (AMR) {
+    if (jf & 1u) P.fjump[slot] = Fm;
+    if (jf & 2u) P.fjump[slot + (long long)P.nvars * P.fj_area] = Fp;
+  }
   return rd * (Fp - Fm);
 }
 
@@ -299,15 +307,32 @@ __global__ void __launch_bounds__(128, RECON == FX_RECON_PLM_MINMOD ? FX_GENERIC
     const double u0 = U0[g];
     out[g] = first ? (u0 - S[v]) : (u0 + beta * ((X[g] - u0) - S[v]));
   }
+  unsigned jfc = 0;  // AMR with scalars: two bits per direction, the zone's low / high face is a refinement jump of its block
+  if (SCALARS && AMR) {
+    const int id3[3] = {i, j, k};
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+      if (!P.active[d]) continue;
+      if (id3[d] == 0 && __ldg(&P.neigh[b * 6 + 2 * d]) <= FX_NEIGH_COARSER) jfc |= 1u << (2 * d);
+      if (id3[d] == P.n[d] - 1 && __ldg(&P.neigh[b * 6 + 2 * d + 1]) <= FX_NEIGH_COARSER) jfc |= 2u << (2 * d);
+    }
+  }
   if (SCALARS) {
     // passive scalars [B11]: same divergence and combination, no source term
 #pragma unroll 1
     for (int sv = 5; sv < P.nvars; ++sv) {
       const double *Q = X + sv * P.S_v;
       double Ss = 0.0;
-      if (P.active[0]) Ss += fx_zone_scalar_direction<RECON, 0>(P, Q, c, 1, rd0, qfb, sh, hit);
-      if (P.active[1]) Ss += fx_zone_scalar_direction<RECON, 1>(P, Q, c, P.S_j, rd1, qfb, sh, hit);
-      if (P.active[2]) Ss += fx_zone_scalar_direction<RECON, 2>(P, Q, c, P.S_k, rd2, qfb, sh, hit);
+      if (AMR) {
+        const long long A = P.fj_area;
+        if (P.active[0]) Ss += fx_zone_scalar_direction<RECON, 0, true>(P, Q, c, 1, rd0, qfb, sh, hit, jfc & 3u, ((b * 6 + 0) * P.nvars + sv) * A + (k * ny + j));
+        if (P.active[1]) Ss += fx_zone_scalar_direction<RECON, 1, true>(P, Q, c, P.S_j, rd1, qfb, sh, hit, (jfc >> 2) & 3u, ((b * 6 + 2) * P.nvars + sv) * A + (k * nx + i));
+        if (P.active[2]) Ss += fx_zone_scalar_direction<RECON, 2, true>(P, Q, c, P.S_k, rd2, qfb, sh, hit, (jfc >> 4) & 3u, ((b * 6 + 4) * P.nvars + sv) * A + (j * nx + i));
+      } else {
+        if (P.active[0]) Ss += fx_zone_scalar_direction<RECON, 0>(P, Q, c, 1, rd0, qfb, sh, hit);
+        if (P.active[1]) Ss += fx_zone_scalar_direction<RECON, 1>(P, Q, c, P.S_j, rd1, qfb, sh, hit);
+        if (P.active[2]) Ss += fx_zone_scalar_direction<RECON, 2>(P, Q, c, P.S_k, rd2, qfb, sh, hit);
+      }
       const long long g = sv * P.S_v + c;
       const double u0 = U0[g];
       out[g] = first ? (u0 - Ss) : (u0 + beta * ((Q[c] - u0) - Ss));
@@ -360,7 +385,10 @@ int fx_launch_generic_stage(const FxParams &P, const double *X, const double *U0
   const unsigned grid = (unsigned)((nzones + 127) / 128);
 #define CALL(RC, RM)                                                                                              \
   do {                                                                                                          \
-    if (P.nvars > 5) {                                                                                          \
+    if (P.nvars > 5 && P.has_jumps) {                                                                           \
+      if (P.wavespeed == 0) fx_k_generic_stage<RC, RM, 0, true, true><<<grid, 128, sizeof(FxScalarShared<RC>), st>>>(P, X, U0, out, dx, dt, dt_dev, beta, first, nzones); \
+      else fx_k_generic_stage<RC, RM, 1, true, true><<<grid, 128, sizeof(FxScalarShared<RC>), st>>>(P, X, U0, out, dx, dt, dt_dev, beta, first, nzones); \
+    } else if (P.nvars > 5) {                                                                                   \
       if (P.wavespeed == 0) fx_k_generic_stage<RC, RM, 0, true><<<grid, 128, sizeof(FxScalarShared<RC>), st>>>(P, X, U0, out, dx, dt, dt_dev, beta, first, nzones); \
       else fx_k_generic_stage<RC, RM, 1, true><<<grid, 128, sizeof(FxScalarShared<RC>), st>>>(P, X, U0, out, dx, dt, dt_dev, beta, first, nzones); \
     } else if (P.has_jumps) {                                                                                   \

@@ -204,7 +204,7 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
       for (int f = 0; f < 6; ++f) cap |= (__ldg(&P.neigh[(long long)S.chain[2] * 6 + f]) <= FX_NEIGH_COARSER ? 1u : 0u) << f;
     }
     auto capture = [&](int f, int tflat, const double F[5]) {
-      double *dst = P.fjump + ((long long)S.chain[2] * 6 + f) * 5 * (long long)P.fj_area + tflat;
+      double *dst = P.fjump + ((long long)S.chain[2] * 6 + f) * P.nvars * (long long)P.fj_area + tflat;
 #pragma unroll
       for (int v = 0; v < 5; ++v) dst[(long long)v * P.fj_area] = F[v];
     };
@@ -444,7 +444,7 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
 #pragma unroll
         for (int v = 0; v < 5; ++v) Lf[v * LV + NX * ld + m * lt] = F[v];
         if (EXTRAS && ecap) {
-          double *dst = P.fjump + ((long long)pb * 6 + ef) * 5 * (long long)P.fj_area + (c - 1) * NX + m;
+          double *dst = P.fjump + ((long long)pb * 6 + ef) * P.nvars * (long long)P.fj_area + (c - 1) * NX + m;
 #pragma unroll
           for (int v = 0; v < 5; ++v) dst[(long long)v * P.fj_area] = F[v];
         }

@@ -89,3 +89,65 @@ def test_jumps_need_the_refinement_table():
     with pytest.raises(fx.FxError) as e:
         plan.fx_hydro_plan_set_topology(grid["neigh"])
     assert e.value.code == -3  # FX_ERR_UNSUPPORTED
+
+
+@pytest.mark.parametrize("nbc,refined,dims", [GRIDS[1], GRIDS[2], ((3, 3, 2), {(0, 0, 0), (2, 2, 1)}, (16, 16, 16))])
+@pytest.mark.parametrize("recon,riemann,rk,ns", [(0, 1, 2, 2), (1, 0, 3, 1), (0, 0, 3, 6)])
+def test_passive_scalars_through_jumps(nbc, refined, dims, recon, riemann, rk, ns):
+    """Passive mass scalars on a two-level grid [B11 with B12-B14] (generic path): guard fill of all variables bit for bit,
+    advance to the [NS] tolerances, the scalars' fluxes corrected at the jumps (scalar mass conserved), hydro variables those
+    of the plan without scalars (bit for bit with PLM + HLLC)."""
+    from paper_2208_11630_b200 import binding as fx
+    from tests.test_oracle_amr import amr_zone_centres, with_scalars
+    grid = two_level_grid(nbc, refined, dims)
+    n = len(grid["level"])
+    oplan = amr_plan(grid, dims, recon=recon, riemann=riemann, rk=rk, nvars=5 + ns)
+
+    def gplan_for(nvars, path=None):
+        plan = fx.HydroPlan(dims, 4, n, GAMMA, recon, riemann, rk, nvars=nvars)
+        if path is not None:
+            plan.fx_hydro_plan_set_option(fx.OPT_PATH, path)
+        plan.fx_hydro_plan_set_refinement(grid["jump"])
+        plan.fx_hydro_plan_set_topology(grid["neigh"])
+        plan.fx_hydro_plan_set_workspace()
+        assert plan.path == 0
+        return plan
+
+    gplan, g5 = gplan_for(5 + ns), gplan_for(5, path=1)
+    ndim = sum(1 for d in dims if d > 1)
+    L = [nbc[d] * dims[d] for d in range(3)]
+    f5 = smooth_field(grid, dims, L)
+    X = amr_zone_centres(grid, dims)
+    ab = [0.5 + 0.4 * np.sin(2 * np.pi * (s + 1) * X[:, s % ndim] / L[s % ndim] + 0.3 * s) for s in range(ns)]
+    ab[0] = (np.abs(X[:, 1] - 0.5 * L[1]) < 0.2 * L[1]).astype(float)  # a slab that crosses the refined region
+    Uo = state_from(oplan, with_scalars(f5, ab))
+    Ud = torch.from_numpy(Uo).cuda()
+    U5 = torch.from_numpy(np.ascontiguousarray(Uo[:5])).cuda()
+    F = Uo.copy()
+    oplan.fill_guardcells(F)
+    Fg = Ud.clone()
+    gplan.fx_fill_guardcells(Fg)
+    assert np.array_equal(Fg.cpu().numpy(), F)
+    dx = dx_of(grid)
+    dxd = torch.from_numpy(dx).cuda()
+    T0 = totals(oplan, grid, Uo, ndim)
+    for step in range(10):
+        dt = oplan.compute_dt(Uo, dx, 0.3)
+        oplan.advance(Uo, dx, dt)
+        gplan.fx_hydro_advance(Ud, dxd, dt)
+        g5.fx_hydro_advance(U5, dxd, dt)
+        if step in (0, 9):
+            got, ref = gplan.interior(Ud).cpu().numpy(), oplan.interior(Uo)
+            tol = 1e-12 if step == 0 else 1e-9
+            assert rel_err(Cfg, got[:5], ref[:5]) <= tol
+            assert float((np.abs(got[5:] - ref[5:]) / ref[0]).max()) <= tol
+    if recon == 0 and riemann == 1:
+        assert torch.equal(gplan.interior(Ud)[:5], g5.interior(U5))
+    else:  # (WENO5, HLLE: the kernel variant with scalars contracts some products differently -- rounding, not bits)
+        assert rel_err(Cfg, gplan.interior(Ud)[:5].cpu().numpy(), g5.interior(U5).cpu().numpy()) <= 1e-12
+    T1 = totals(oplan, grid, Ud.cpu().numpy(), ndim)
+    for v in [0, 4] + list(range(5, 5 + ns)):
+        assert abs(T1[v] - T0[v]) <= 1e-13 * T0[0], (v, T1[v] - T0[v])
+    fo, _ = oplan.status()
+    fg, _ = gplan.fx_hydro_status()
+    assert fo == fg == 0
