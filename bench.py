@@ -58,6 +58,10 @@ def parse_args():
     ap.add_argument("--wavespeed", type=int, default=0, help="FX_OPT_WAVESPEED: 0 Einfeldt (the reading the configs are run with [A8]), 1 Davis")
     ap.add_argument("--shard", action="store_true", help="drive the step through ShardedHydro even on one rank (the N > 1 code path with an "
                     "empty exchange; N > 1 always uses it)")
+    ap.add_argument("--one-rank-of", type=int, default=0, metavar="N", help="rank 0 of an N-way partition of the N-fold tiling, ALONE on this GPU: "
+                    "its stage launches (two parts side by side), pack and unpack as the rank runs them, the transfer replaced by a device "
+                    "copy of the same bytes and the dt all-reduce left out -- what one rank's kernels cost, not a multi-GPU measurement")
+    ap.add_argument("--no-overlap", action="store_true", help="sharded runs: the exchange in front of an undivided stage instead of beside its first part")
     ap.add_argument("--amr", action="store_true", help="two-level grid of 16^3 blocks on config 5's domain (7680 blocks, 1736 of them with a "
                     "refinement jump): the fused kernel on every block (path 5; the blocks at the jumps read their own guard zones); --path 1 for all-generic")
     ap.add_argument("--ca", action="store_true", help="time the communication-avoiding step (fx_hydro_advance_ca, DESIGN.md B17: one guard fill "
@@ -251,7 +255,7 @@ def build_sharded_workload(args, device, rank, world):
     neigh, coords = fx.fx_topology_cartesian(cfg.nb, bcs, bcs, fx.ORDER_MORTON if args.order == "morton" else fx.ORDER_LEX)
     guard_x = args.guard_x if args.guard_x >= 0 else (8 if (cfg.block_dims[0] == 16 and cfg.nguard == 4) else cfg.nguard)
     sh = ShardedHydro(cfg.block_dims, cfg.nguard, cfg.gamma, cfg.recon, cfg.riemann, cfg.rk_order, neigh, rank, world, device=device,
-                      guard_x=guard_x, nvars=5 + args.scalars, zchain=args.zchain, wavespeed=args.wavespeed)
+                      guard_x=guard_x, nvars=5 + args.scalars, zchain=args.zchain, wavespeed=args.wavespeed, overlap=not args.no_overlap)
     U = sh.alloc_state(fill=float("nan"))
     gid = sh.shard.global_id
     Ui = sh.interior(U)
@@ -418,8 +422,12 @@ def run_ours(args, rank, world, local_rank):
     if world > 1:
         dist.init_process_group("nccl", device_id=device)
     sh = None
-    if world > 1 or args.shard:
-        cfg, sh, U, dx = build_sharded_workload(args, device, rank, world)
+    if world > 1 or args.shard or args.one_rank_of > 1:
+        cfg, sh, U, dx = build_sharded_workload(args, device, rank, args.one_rank_of if args.one_rank_of > 1 else world)
+        if args.one_rank_of > 1:
+            n = min(sh.send_elems, sh.recv_elems)
+            sh.transfer = lambda: sh.recv_buf[:n].copy_(sh.send_buf[:n])  # the slabs' bytes moved once, on the device
+            sh._global_min = lambda d: d
         plan = sh.plan
         zones = sh.n_owned * cfg.block_dims[0] * cfg.block_dims[1] * cfg.block_dims[2]  # this rank's share
     else:
@@ -530,11 +538,12 @@ def run_ours(args, rank, world, local_rank):
                        "interior_zones": zones, "state_bytes": plan.bytes_per_state, "block_order": args.order,
                        "layout": f"x guard depth {plan.gd[0]} (row pitch {plan.S_j * 8} B), y/z guard depth {plan.gd[1]}/{plan.gd[2]}",
                        "path": "communication-avoiding step (one guard fill per step; generic kernels on the extended interior)" if args.ca else {0: "generic", 5: f"fused (TMA); the {getattr(cfg, 'jump_blocks', 0)} blocks with a refinement jump as single-block segments reading their own guard zones", 1: "fused (TMA)", 2: "tile (shared-memory block)", 3: "fused (TMA), two zones per thread", 4: "fused (TMA), 2 x 2 bundles of 8 x 8 blocks"}[plan.path], "l2": "inputs (state) larger than L2; no flush needed",
-                       "multi_gpu": (f"sharded: tiling {cfg.nb[0]}x{cfg.nb[1]}x{cfg.nb[2]} blocks in {world} contiguous Morton runs, "
+                       "multi_gpu": (f"sharded: tiling {cfg.nb[0]}x{cfg.nb[1]}x{cfg.nb[2]} blocks in {args.one_rank_of if args.one_rank_of > 1 else world} contiguous Morton runs, "
                                      f"{sh.shard.n_ghost} ghost blocks on rank 0, cut-face slabs exchanged before every stage "
                                      f"(grouped NCCL send/recv, {sh.send_elems * 8} B sent by rank 0 per stage"
                                      + (", on a stream of its own beside the stage's launch over the blocks away from the cut" if sh.overlap else "")
-                                     + "), dt = all-reduce(min)")
+                                     + "), dt = all-reduce(min)"
+                                     + (f"; ONE RANK OF {args.one_rank_of} ALONE on this GPU (transfer replaced by a device copy, no all-reduce): not a multi-GPU measurement" if args.one_rank_of > 1 else ""))
                        if sh is not None else "single"},
             "clocks": clocks, "gpu_launches": launches_per_step * args.steps, "roofline": roofline,
             "status_flags": flags}
