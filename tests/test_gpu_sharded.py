@@ -289,3 +289,34 @@ def test_overlapped_step_of_two_ranks_in_two_threads():
         ref_hist.append(float(dt.item()))
     assert hists[0] == ref_hist and hists[1] == ref_hist
     assert torch.equal(got, plan.interior(U).cpu())
+
+
+@pytest.mark.parametrize("number,nb,block,recon,path", [(5, (2, 2, 2), None, 0, 1), (5, (2, 2, 2), (8, 8, 8), 1, 4), (2, (2, 2, 1), None, 0, 2),
+                                                        (5, (2, 2, 2), (6, 5, 4), 0, 0)])
+def test_stage_parts_on_every_path_equal_the_whole_stage(number, nb, block, recon, path):
+    """fx_hydro_advance_stage_part on a plan of its own (no ghost block: everything is 'inner' on the fused path) and on the
+    paths that are not split (FX_PART_INNER does nothing, FX_PART_BOUNDARY is the stage): both parts = fx_hydro_advance_stage."""
+    from paper_2208_11630_b200 import binding as fx
+    cfg = inputs.config(number, nb=nb)
+    if block:
+        cfg.block_dims = block
+    n = cfg.nb[0] * cfg.nb[1] * cfg.nb[2]
+    a, neigh, coords = gpu_plan_for(cfg, recon=recon, rk=2)
+    b, _, _ = gpu_plan_for(cfg, recon=recon, rk=2)
+    assert a.path == path
+    ni, nbd = a.fx_hydro_plan_stage_parts()
+    assert (ni, nbd) == ((n, 0) if path == 1 else (0, n))
+    Uh = inputs.embed(cfg, inputs.block_interiors(cfg, coords))
+    Ua, Ub = Uh.cuda(), Uh.cuda()
+    dx = torch.from_numpy(inputs.dx_array(cfg)).cuda()
+    dta, dtb = a.fx_hydro_compute_dt(Ua, dx, cfg.cfl).clone(), b.fx_hydro_compute_dt(Ub, dx, cfg.cfl).clone()
+    for _ in range(2):
+        for s in range(2):
+            kwa = dict(cfl_next=cfg.cfl, dt_next=dta) if s == 1 else {}
+            kwb = dict(cfl_next=cfg.cfl, dt_next=dtb) if s == 1 else {}
+            a.fx_hydro_advance_stage(Ua, dx, dta, s, **kwa)
+            b.fx_hydro_advance_stage_part(Ub, dx, dtb, s, fx.PART_BOUNDARY if s == 0 else fx.PART_INNER, **kwb)  # either order
+            b.fx_hydro_advance_stage_part(Ub, dx, dtb, s, fx.PART_INNER if s == 0 else fx.PART_BOUNDARY, **kwb)
+    assert torch.equal(dta, dtb) and torch.equal(a.interior(Ua), b.interior(Ub))
+    with pytest.raises(fx.FxError):
+        b.fx_hydro_advance_stage_part(Ub, dx, dtb, 0, 3)
