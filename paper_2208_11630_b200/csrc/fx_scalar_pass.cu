@@ -378,7 +378,8 @@ static int fx_scalar_march_launch(const FxParams &P, const double *X, const doub
 }  // namespace
 
 bool fx_scalar_pass_supported(const FxParams &P) {
-  return P.nvars > 5 && P.recon == FX_RECON_PLM_MINMOD && P.all_interior && !P.grav_on && !P.walls && P.fq != nullptr &&
+  // (no ghost block either: a zone's high-face data are the NEXT zone's low-face values, and nobody writes a ghost block's)
+  return P.nvars > 5 && P.recon == FX_RECON_PLM_MINMOD && P.all_interior && P.nown == P.nblocks && !P.grav_on && !P.walls && P.fq != nullptr &&
          P.active[0] && P.active[1] && P.active[2];
 }
 

@@ -77,6 +77,31 @@ def run_sharded(cfg, neigh, coords, world, steps, recon, rk, guard_x, path, nvar
     return out, history, ranks, Us
 
 
+def test_sharded_with_passive_scalars_equals_single_plan():
+    """Passive scalars in a sharded plan ride on the generic path (the scalar pass behind the fused kernel reads a zone's
+    high-face data from the next zone's low face, which nobody computes for a ghost block): owned blocks and time steps
+    equal the single plan's on the same path bit for bit."""
+    from paper_2208_11630_b200 import binding as fx
+    cfg = inputs.config(5, nb=(2, 2, 4))
+    bcs = [fx.TOPO_PERIODIC] * 3
+    neigh, coords = fx.fx_topology_cartesian(cfg.nb, bcs, bcs, fx.ORDER_MORTON)
+    got, hist, ranks, Us = run_sharded(cfg, neigh, coords, 2, 3, 0, 2, 4, 0, nvars=7)
+    plan = fx.HydroPlan(cfg.block_dims, cfg.nguard, cfg.nblocks, cfg.gamma, 0, cfg.riemann, 2, nvars=7)
+    plan.fx_hydro_plan_set_option(fx.OPT_PATH, 1)
+    plan.fx_hydro_plan_set_topology(neigh)
+    plan.fx_hydro_plan_set_workspace()
+    U = plan.alloc_state(fill=float("nan"))
+    plan.interior(U)[...] = inputs.with_scalars(cfg, coords, inputs.block_interiors(cfg, coords), 2).cuda()
+    dx = torch.from_numpy(inputs.dx_array(cfg)).cuda()
+    dt = plan.fx_hydro_compute_dt(U, dx, cfg.cfl).clone()
+    ref_hist = [float(dt.item())]
+    for _ in range(3):
+        plan.fx_hydro_step(U, dx, cfg.cfl, dt)
+        ref_hist.append(float(dt.item()))
+    assert hist == ref_hist
+    assert torch.equal(got, plan.interior(U).cpu())
+
+
 @pytest.mark.parametrize("number,nb,block,recon,rk,guard_x,world,path", [
     (5, (2, 2, 4), None, 0, 2, 8, 2, 1), (5, (4, 2, 2), None, 1, 3, 4, 3, 1), (5, (2, 2, 2), (8, 8, 8), 0, 2, 4, 2, 4),
     (5, (2, 2, 2), (8, 8, 8), 1, 3, 4, 2, 4), (5, (3, 2, 2), (8, 8, 8), 0, 2, 4, 2, 0), (2, (4, 4, 1), None, 0, 2, 4, 3, 2)])
