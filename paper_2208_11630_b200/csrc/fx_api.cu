@@ -246,7 +246,9 @@ static size_t fx_seg_bytes(const fx_hydro_plan *plan) {  // the segment tables a
 static size_t fx_fq_bytes(const fx_hydro_plan *plan) {  // scalar pass [B11]: (mass flux, Aq) x 3 low faces per interior zone
   const FxParams &P = plan->P;
   if (plan->nvars <= 5 || P.recon != FX_RECON_PLM_MINMOD || P.n[0] != 16 || P.n[1] != 16 || !P.active[2]) return 0;
-  return (((size_t)6 * P.nblocks * P.n[0] * P.n[1] * P.n[2] * sizeof(double)) + 255) & ~(size_t)255;
+  // + the high faces of the blocks at a physical boundary or a cut: (mass flux, Aq) x 3 directions x a face of 16 x max(nz, 16) zones
+  const size_t area = (size_t)16 * (P.n[2] > 16 ? P.n[2] : 16);
+  return (((size_t)6 * P.nblocks * (P.n[0] * P.n[1] * P.n[2] + area) * sizeof(double)) + 255) & ~(size_t)255;
 }
 
 static size_t fx_fjump_bytes(const fx_hydro_plan *plan) {  // boundary fluxes at refinement jumps [B14]
@@ -319,6 +321,8 @@ extern "C" int fx_hydro_plan_set_workspace(fx_hydro_plan *plan, void *ws, size_t
   plan->P.fq = fx_fq_bytes(plan) ? (double *)((char *)ws + FX_SCR_WORDS * 8 + 256 + (size_t)(plan->rk - 1) * fx_state_bytes_aligned(plan) +
                                               fx_seg_bytes(plan) + fx_fjump_bytes(plan))
                                  : nullptr;
+  plan->P.fqb_area = 16 * (plan->P.n[2] > 16 ? plan->P.n[2] : 16);
+  plan->P.fqb = plan->P.fq ? plan->P.fq + (size_t)6 * plan->P.nblocks * plan->P.n[0] * plan->P.n[1] * plan->P.n[2] : nullptr;
   return fx_seg_upload(plan);
 }
 

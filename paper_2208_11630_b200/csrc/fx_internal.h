@@ -30,6 +30,8 @@ struct FxParams {
   int grav_on;                      // any component of grav is non-zero [B10]
   double grav[3];
   double *fq;                       // scalar pass [B11]: mass flux and Aq of every zone's low x, y, z faces, [6][nblocks nz ny nx], in the workspace
+  double *fqb;                      // the same for the HIGH face of a block that has no owned same-level block behind it (a physical
+  int fqb_area;                     // boundary, a ghost block): [2 (F_rho, Aq)][3][nblocks][fqb_area], behind fq; the 17th face's solve
   int all_interior;                 // every active face of every owned block has a same-level neighbour (no physical boundary, no jump)
   const int *jump;                  // refinement jumps [B12]: [nblocks][6][4], device; nullptr if none was given
   int has_jumps;                    // some active face carries FX_NEIGH_COARSER / FX_NEIGH_FINER

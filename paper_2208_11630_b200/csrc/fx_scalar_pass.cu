@@ -5,9 +5,12 @@
 // every zone in P.fq (HLLC: F_rho alone -- there Aq = max(F_rho, 0), the flux being upwind in the sign of S*); this kernel, one thread per zone, does what is left for each scalar: X = (rho X) / rho on the 2R+1
 // cells of each direction's stencil (the reciprocal densities are formed once and serve all scalars), PLM face values of
 // cells -1, 0, +1, the two face fluxes per direction (the high face's F_rho and Aq are the next zone's low-face values,
-// through the neighbour table at a block face), divergence and RK combination.  Expressions and their order are those of
-// the generic kernel's scalar loop (fx_generic.cu), which remains the path for WENO5, physical boundaries and gravity.
-// Applies to: PLM, every face of every block with a same-level neighbour (periodic tilings), no gravity.
+// through the neighbour table at a block face -- or, where no owned same-level block lies behind a block's high face (a
+// physical boundary, a ghost block of a sharded plan), the fused kernel's own solve of that face, which it leaves in P.fqb),
+// divergence and RK combination.  Halo abundances behind an outflow boundary are the block's edge cell's, behind a wall its
+// mirror cells' [B9, B11].  Expressions and their order are those of the generic kernel's scalar loop (fx_generic.cu),
+// which remains the path for WENO5 and refinement jumps.
+// Applies to: PLM, 16 x 16 x nz blocks, no refinement jump (fx_scalar_pass_supported).
 #include "fx_physics.cuh"
 
 namespace {
@@ -152,31 +155,48 @@ __global__ void __launch_bounds__(256, 2) fx_k_scalar_march(const FxParams P, co
   const long long nzt = P.nblocks * (long long)nz * 256;
   const double *Q0 = X + (long long)sv0 * P.S_v, *U0q = U0 + (long long)sv0 * P.S_v;
   double *outq = out + (long long)sv0 * P.S_v;
-  auto plane_off = [&](int k) -> long long {  // this column's zone in plane k of the column (k in [-2, nz + 2))
-    const int blk = k < 0 ? nb[4] : (k >= nz ? nb[5] : b);
-    const int kk = k < 0 ? k + nz : (k >= nz ? k - nz : k);
+  // this column's zone in plane k of the column (k in [-2, nz + 2)): the z neighbour's planes, or behind a physical
+  // boundary this block's own edge plane (outflow) / mirror plane (wall: scalars and density are copied unchanged [B11])
+  auto plane_off = [&](int k) -> long long {
+    int blk = b, kk = k;
+    if (k < 0) {
+      if (nb[4] >= 0) { blk = nb[4]; kk = k + nz; } else kk = nb[4] == FX_BC_REFLECT ? -1 - k : 0;
+    } else if (k >= nz) {
+      if (nb[5] >= 0) { blk = nb[5]; kk = k - nz; } else kk = nb[5] == FX_BC_REFLECT ? 2 * nz - 1 - k : nz - 1;
+    }
     return (long long)blk * P.S_b + (long long)(kk + g2) * P.S_k + colo;
   };
   // the halo cell this thread also provides for each plane (threads in the two outermost columns / rows): where it comes
   // from inside the neighbour block's plane, its slot in the staging buffer, and where it goes in the shared plane
   const bool hx = i < 2 || i >= 14, hy = j < 2 || j >= 14;
-  const long long hxo = (long long)(i < 2 ? nb[0] : nb[1]) * P.S_b + (long long)(j + g1) * P.S_j + ((i < 2 ? 14 + i : i - 14) + g0);
-  const long long hyo = (long long)(j < 2 ? nb[2] : nb[3]) * P.S_b + (long long)((j < 2 ? 14 + j : j - 14) + g1) * P.S_j + (i + g0);
+  // (behind a physical boundary: the block's own edge cell, or its mirror cells at a wall)
+  const int nxs = i < 2 ? nb[0] : nb[1], nys = j < 2 ? nb[2] : nb[3];
+  const int xi = i < 2 ? (nxs >= 0 ? 14 + i : (nxs == FX_BC_REFLECT ? 1 - i : 0)) : (nxs >= 0 ? i - 14 : (nxs == FX_BC_REFLECT ? 29 - i : 15));
+  const int yj = j < 2 ? (nys >= 0 ? 14 + j : (nys == FX_BC_REFLECT ? 1 - j : 0)) : (nys >= 0 ? j - 14 : (nys == FX_BC_REFLECT ? 29 - j : 15));
+  const long long hxo = (long long)(nxs >= 0 ? nxs : b) * P.S_b + (long long)(j + g1) * P.S_j + (xi + g0);
+  const long long hyo = (long long)(nys >= 0 ? nys : b) * P.S_b + (long long)(yj + g1) * P.S_j + (i + g0);
   const int hxs = j * 4 + (i < 2 ? i : i - 12), hys = 64 + (j < 2 ? j : j - 12) * 16 + i;
   const int hxc = i < 2 ? i : i + 4, hyr = j < 2 ? j : j + 4;
   const long long zb = (long long)b * nz * 256 + tid;
-  const long long zxh = (long long)nb[1] * nz * 256 + j * 16, zyh = (long long)nb[3] * nz * 256 + i;
   // everything plane k needs before its barrier, into stage k & 1.  All addresses are running 64-bit offsets advanced by
   // one plane per call (the planes are prefetched in turn, k = 0, 1, ...): forming them from k each time cost a quarter of
   // the loop's instructions (215 of 847 integer instructions per plane were address arithmetic)
-  const long long top0 = plane_off(nz);      // the column's first zone in the block above
   long long e_pf = plane_off(2);              // new window cell of the plane being prefetched
-  const long long dzx = zxh - zb, dzy = zyh - zb;
+  const long long top0 = plane_off(nz), top1 = plane_off(nz + 1);  // the two planes beyond the block's top
   // (the other offsets of a plane follow from its own-zone offset cpf and from kp: fewer values carried across the loop --
   // the spilled piece of one of them, reloaded from local memory behind the streaming cp.async traffic, was 10 % of the
   // stall samples)
   const long long hxr = hxo - ((long long)b * P.S_b + colo), hyr_o = hyo - ((long long)b * P.S_b + colo);
-  const long long dztop = 4 * nzt + (long long)nb[5] * nz * 256 + tid;
+  // a zone's HIGH-face data are the next zone's low-face values; behind a block face: the neighbour block's, if that is an
+  // owned same-level block -- else (physical boundary, ghost block) what the fused kernel's 17th-face solve left in P.fqb
+  // Resolved once per thread: where the data of plane 0 are (x: thread i = 15 of row j; y: thread j = 15 of column i), how
+  // far apart two planes' are (256 zones in the neighbour block, 16 on a stored face), and for z the block's top face.
+  auto owned = [&](int h) { return h >= 0 && h < P.nown; };
+  const long long fqbc = 3 * P.nblocks * (long long)P.fqb_area;  // (F_rho -> Aq in P.fqb)
+  const bool ox = owned(nb[1]), oy = owned(nb[3]), oz = owned(nb[5]);
+  const double *const hsx = ox ? P.fq + (long long)nb[1] * nz * 256 + j * 16 : P.fqb + (long long)b * P.fqb_area + j;
+  const double *const hsy = oy ? P.fq + 2 * nzt + (long long)nb[3] * nz * 256 + i : P.fqb + (P.nblocks + b) * (long long)P.fqb_area + i;
+  const double *const hsz = oz ? P.fq + 4 * nzt + (long long)nb[5] * nz * 256 + tid : P.fqb + (2 * P.nblocks + b) * (long long)P.fqb_area + tid;
   auto prefetch = [&](int kp, long long cpf) {  // called for kp = 0, 1, 2, ... in turn; cpf: this thread's zone of plane kp
     const int st = kp & 1;
     {
@@ -205,23 +225,26 @@ __global__ void __launch_bounds__(256, 2) fx_k_scalar_march(const FxParams P, co
     cp_async8(&S.fy[st][0][j][i], f + 2 * nzt);
     if (!HLLC) cp_async8(&S.fy[st][1][j][i], f + 3 * nzt);
     if (i == 15) {
-      cp_async8(&S.fx[st][0][j][16], f + dzx);
-      if (!HLLC) cp_async8(&S.fx[st][1][j][16], f + dzx + nzt);
+      const double *h = hsx + kp * (ox ? 256 : 16);
+      cp_async8(&S.fx[st][0][j][16], h);
+      if (!HLLC) cp_async8(&S.fx[st][1][j][16], h + (ox ? nzt : fqbc));
     }
     if (j == 15) {
-      cp_async8(&S.fy[st][0][16][i], f + dzy + 2 * nzt);
-      if (!HLLC) cp_async8(&S.fy[st][1][16][i], f + dzy + 3 * nzt);
+      const double *h = hsy + kp * (oy ? 256 : 16);
+      cp_async8(&S.fy[st][0][16][i], h);
+      if (!HLLC) cp_async8(&S.fy[st][1][16][i], h + (oy ? nzt : fqbc));
     }
     {  // what only the end of the plane needs (it comes from DRAM: fetched a plane ahead like the rest)
       const double *pu = U0q + cpf;
 #pragma unroll
       for (int s = 0; s < NSC; ++s, pu += P.S_v) cp_async8(&S.late[st][s][tid], pu);
-      const double *fzh = kp + 1 < nz ? f + 4 * nzt + 256 : P.fq + dztop;
+      const bool top = kp + 1 >= nz;
+      const double *fzh = top ? hsz : f + 4 * nzt + 256;
       cp_async8(&S.late[st][NSC][tid], fzh);
-      if (!HLLC) cp_async8(&S.late[st][NSC + 1][tid], fzh + nzt);
+      if (!HLLC) cp_async8(&S.late[st][NSC + 1][tid], fzh + ((top && !oz) ? fqbc : nzt));
     }
     cp_async_commit();
-    e_pf = (kp + 3 == nz) ? top0 : e_pf + P.S_k;
+    e_pf = kp + 3 == nz ? top0 : (kp + 3 == nz + 1 ? top1 : e_pf + P.S_k);  // (beyond the block's top: wherever those planes live)
   };
   prefetch(0, (long long)b * P.S_b + (long long)g2 * P.S_k + colo);
   if (dt_dev) dt = *dt_dev;
@@ -378,9 +401,11 @@ static int fx_scalar_march_launch(const FxParams &P, const double *X, const doub
 }  // namespace
 
 bool fx_scalar_pass_supported(const FxParams &P) {
-  // (no ghost block either: a zone's high-face data are the NEXT zone's low-face values, and nobody writes a ghost block's)
-  return P.nvars > 5 && P.recon == FX_RECON_PLM_MINMOD && P.all_interior && P.nown == P.nblocks && !P.grav_on && !P.walls && P.fq != nullptr &&
-         P.active[0] && P.active[1] && P.active[2];
+  // The marching form serves 16 x 16 x nz blocks with same-level neighbours, physical boundaries (outflow, walls) and ghost
+  // blocks behind their faces (the high-face data behind such a face are the fused kernel's own 17th-face solve, P.fqb);
+  // gravity acts on the hydro variables only [B11].  Refinement jumps: generic path.
+  return P.nvars > 5 && P.recon == FX_RECON_PLM_MINMOD && !P.has_jumps && P.fq != nullptr && P.fqb != nullptr && P.n[0] == 16 &&
+         P.n[1] == 16 && P.n[2] >= 2 && P.active[0] && P.active[1] && P.active[2];
 }
 
 int fx_launch_scalar_pass(const FxParams &P, const double *X, const double *U0, double *out, const double *dx, double dt,

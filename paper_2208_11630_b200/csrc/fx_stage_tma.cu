@@ -105,6 +105,7 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
                double cfl_next, double *dt_next) {  // dt_next may be dt_dev (fx_hydro_step): read at the start, written by the last CTA
   constexpr int r = Rc<RECON>::r, R = Rc<RECON>::R, W = 2 * r + 1, NP = Rc<RECON>::NP, BW = Rc<RECON>::BW;
   constexpr int NRING = Rc<RECON>::NRING;
+  constexpr bool AQS = SCAL && RIEMANN != FX_RIEMANN_HLLC;  // the faces' Aq are needed (HLLC: Aq = max(F_rho, 0))
   extern __shared__ __align__(1024) unsigned char fx_smem_raw[];  // TMA destinations need 128-byte alignment
   Smem<RECON> &S = *reinterpret_cast<Smem<RECON> *>(fx_smem_raw);
   const int tid = threadIdx.x;
@@ -192,7 +193,6 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
     double rate = 0.0;     // DTOUT: running maximum of (|u_d| + c) / dx_d over this thread's finished zones
     double q[W][5];        // q[m] = primitives of cell c - r + m at tick c
     double qpz[5], Fz[5];  // plus-side z state of cell c-1; z flux of face c-1 (between cells c-2 and c-1)
-    constexpr bool AQS = SCAL && RIEMANN != FX_RIEMANN_HLLC;  // the faces' Aq are needed (HLLC: Aq = max(F_rho, 0))
     double Aqz = 0.0;      // AQS: Aq of that face
     int sq = 0, sk = 0;    // SCAL: plane p is plane sk of the sq-th block of the segment
     // Refinement jumps [B14]: the fluxes through a block's jump faces are stored for the flux correction (both sides of a
@@ -383,6 +383,15 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
 #pragma unroll
         for (int v = 0; v < 5; ++v) q[m][v] = q[m + 1][v];
     }
+    if (SCAL) {  // the segment's top face has no owned block above it: its mass flux (the last one carried) goes where the
+                 // scalar pass looks for it.  (Behind the loop: inside it the few registers this needs spilled loop values.)
+      const int ab = S.chain[2 + M];
+      if (ab < 0 || ab >= P.nown) {
+        const long long t = ((2 * P.nblocks + S.chain[1 + M]) * (long long)P.fqb_area) + j * NX + i;
+        P.fqb[t] = Fz[0];
+        if (AQS) P.fqb[t + 3 * P.nblocks * (long long)P.fqb_area] = Aqz;
+      }
+    }
     if (DTOUT) {
 #pragma unroll
       for (int o = 16; o > 0; o >>= 1) rate = fmax(rate, __shfl_xor_sync(0xffffffffu, rate, o));
@@ -405,6 +414,10 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
     // the high x / y face of this lane's row / column carries a refinement jump: its flux is stored [B14]
     const int ef = isx ? 1 : 3;
     const bool ecap = EXTRAS && P.has_jumps && M == 1 && __ldg(&P.neigh[(long long)pb * 6 + ef]) <= FX_NEIGH_COARSER;
+    // SCAL: no owned same-level block behind that face (a physical boundary, a ghost block): the scalar pass takes the face's
+    // mass flux (and Aq) from P.fqb, where this warp leaves it -- nobody else computes it
+    auto no_owner = [&](int blk) { const int h = __ldg(&P.neigh[(long long)blk * 6 + ef]); return h < 0 || h >= P.nown; };
+    bool ebnd = SCAL && no_owner(pb);
 
 #pragma unroll 1
     for (int c = 1; c <= nz; ++c) {
@@ -433,8 +446,13 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
         for (int v = 0; v < 5; ++v) WL[v] = Lf[v * LV + NX * ld + m * lt];
         const double wl[5] = {WL[0], isx ? WL[1] : WL[2], isx ? WL[2] : WL[3], isx ? WL[3] : WL[1], WL[4]};
         const double wr[5] = {qm16[0], isx ? qm16[1] : qm16[2], isx ? qm16[2] : qm16[3], isx ? qm16[3] : qm16[1], qm16[4]};
-        double f[5];
-        fx_riemann_v2<RIEMANN, WS>(P, wl, wr, f);
+        double f[5], Aqe = 0.0;
+        fx_riemann_v2<RIEMANN, WS, AQS>(P, wl, wr, f, &Aqe);
+        if (SCAL && ebnd) {
+          const long long t = (((isx ? 0 : 1) * P.nblocks + pb) * (long long)P.fqb_area) + pk * NX + m;
+          P.fqb[t] = f[0];
+          if (AQS) P.fqb[t + 3 * P.nblocks * (long long)P.fqb_area] = Aqe;
+        }
         double F[5];
         F[0] = f[0];
         F[1] = isx ? f[1] : f[3];
@@ -459,6 +477,7 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
         pk = 0;
         ++pq;
         pb = S.chain[2 + pq];
+        if (SCAL && c < nz) ebnd = no_owner(pb);
       }
       cta_sync();  // C
     }
@@ -613,6 +632,11 @@ int launch_ws(const FxParams &P, const double *X, const double *U0, double *out,
               double beta, int first, double cfl_next, double *dt_next, cudaStream_t st) {
   if constexpr (RECON == FX_RECON_PLM_MINMOD) {
     if (P.nvars > 5) {  // with passive scalars: also leave the faces' mass flux and Aq for the scalar pass
+      if (P.walls || P.grav_on) {
+        if (first) return launch<RECON, RIEMANN, WS, true, false, true, true>(P, X, U0, out, dx, dt, dt_dev, beta, 0.0, nullptr, st);
+        if (dt_next) return launch<RECON, RIEMANN, WS, false, true, true, true>(P, X, U0, out, dx, dt, dt_dev, beta, cfl_next, dt_next, st);
+        return launch<RECON, RIEMANN, WS, false, false, true, true>(P, X, U0, out, dx, dt, dt_dev, beta, 0.0, nullptr, st);
+      }
       if (first) return launch<RECON, RIEMANN, WS, true, false, false, true>(P, X, U0, out, dx, dt, dt_dev, beta, 0.0, nullptr, st);
       if (dt_next) return launch<RECON, RIEMANN, WS, false, true, false, true>(P, X, U0, out, dx, dt, dt_dev, beta, cfl_next, dt_next, st);
       return launch<RECON, RIEMANN, WS, false, false, false, true>(P, X, U0, out, dx, dt, dt_dev, beta, 0.0, nullptr, st);

@@ -44,7 +44,7 @@ def test_advance_1_and_10_steps(number, nb, ns, kw):
     cfg, oplan, gplan, Uh, dx = setup(number, nb, ns, **kw)
     # scalars follow the fused kernel in the scalar pass where it applies (3-D 16 x 16 blocks, PLM, same-level neighbours on
     # every face), else they ride on the generic path
-    fused = cfg.block_dims == (16, 16, 16) and kw.get("recon", cfg.recon) == 0 and kw.get("bc", cfg.bc) == "periodic"
+    fused = cfg.block_dims == (16, 16, 16) and kw.get("recon", cfg.recon) == 0  # (physical boundaries included)
     assert gplan.path == (1 if fused else 0)
     Uo = Uh.numpy().copy()
     Ud = Uh.cuda()
@@ -167,3 +167,37 @@ def test_scalar_march_block_heights_and_scalar_counts(nz, g, ns, riemann, rk):
     fo, _ = oplan.status()
     fg, _ = gplan.fx_hydro_status()
     assert fo == fg
+
+
+@pytest.mark.parametrize("riemann,rk", [(1, 2), (0, 3)])
+def test_scalars_in_a_closed_box_with_gravity_on_the_fused_path(riemann, rk):
+    """Reflecting walls on every face and a constant gravity, with three scalars: the fused kernel's EXTRAS + SCAL variant and
+    the marching pass with its mirrored halo cells and the walls' high faces taken from the 17th-face solves [B9, B10, B11]."""
+    from oracle import fxoracle as fxo
+    from paper_2208_11630_b200 import binding as fx
+    cfg, oplan, gplan, Uh, dx = setup(5, (2, 2, 2), 3, bc="reflect", riemann=riemann, rk=rk)
+    grav = (0.4, -0.3, 0.6)
+    for d in range(3):
+        oplan.set_option(fxo.OPT_GRAVITY_X + d, grav[d])
+    # (options go in before the topology: a fresh plan)
+    gplan = fx.HydroPlan(cfg.block_dims, cfg.nguard, 8, cfg.gamma, cfg.recon, riemann, rk, nvars=8)
+    for d in range(3):
+        gplan.fx_hydro_plan_set_option(fx.OPT_GRAVITY_X + d, grav[d])
+    bcs = [fx.TOPO_REFLECT] * 3
+    neigh, _ = fx.fx_topology_cartesian((2, 2, 2), bcs, bcs, fx.ORDER_LEX)
+    gplan.fx_hydro_plan_set_topology(neigh)
+    gplan.fx_hydro_plan_set_workspace()
+    assert gplan.path == 1
+    Uo, Ud, dxd = Uh.numpy().copy(), Uh.cuda(), torch.from_numpy(dx).cuda()
+    T0 = [float(gplan.interior(Ud)[v].sum(dtype=torch.float64)) for v in (0, 5, 6, 7)]
+    for step in range(10):
+        dt = oplan.compute_dt(Uo, dx, cfg.cfl)
+        oplan.advance(Uo, dx, dt)
+        gplan.fx_hydro_advance(Ud, dxd, dt)
+        if step in (0, 9):
+            got, ref = gplan.interior(Ud).cpu().numpy(), oplan.interior(Uo)
+            tol = TOL_1 if step == 0 else TOL_10
+            assert rel_err(cfg, got[:5], ref[:5]) <= tol and scalar_err(got, ref) <= tol, (step, rel_err(cfg, got[:5], ref[:5]), scalar_err(got, ref))
+    T1 = [float(gplan.interior(Ud)[v].sum(dtype=torch.float64)) for v in (0, 5, 6, 7)]
+    for a, b in zip(T0, T1):  # nothing leaves a closed box
+        assert abs(a - b) <= 1e-13 * T0[0]

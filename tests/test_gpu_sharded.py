@@ -78,16 +78,15 @@ def run_sharded(cfg, neigh, coords, world, steps, recon, rk, guard_x, path, nvar
 
 
 def test_sharded_with_passive_scalars_equals_single_plan():
-    """Passive scalars in a sharded plan ride on the generic path (the scalar pass behind the fused kernel reads a zone's
-    high-face data from the next zone's low face, which nobody computes for a ghost block): owned blocks and time steps
-    equal the single plan's on the same path bit for bit."""
+    """Passive scalars in a sharded plan on the fused kernel + scalar pass: a zone's high-face data behind a cut are not the
+    ghost block's (nobody computes those) but the fused kernel's own solve of that face, left in P.fqb -- owned blocks and
+    time steps equal the single plan's bit for bit.  (The first sharded run with scalars had read the ghost block's.)"""
     from paper_2208_11630_b200 import binding as fx
     cfg = inputs.config(5, nb=(2, 2, 4))
     bcs = [fx.TOPO_PERIODIC] * 3
     neigh, coords = fx.fx_topology_cartesian(cfg.nb, bcs, bcs, fx.ORDER_MORTON)
-    got, hist, ranks, Us = run_sharded(cfg, neigh, coords, 2, 3, 0, 2, 4, 0, nvars=7)
+    got, hist, ranks, Us = run_sharded(cfg, neigh, coords, 2, 3, 0, 2, 4, 1, nvars=7)
     plan = fx.HydroPlan(cfg.block_dims, cfg.nguard, cfg.nblocks, cfg.gamma, 0, cfg.riemann, 2, nvars=7)
-    plan.fx_hydro_plan_set_option(fx.OPT_PATH, 1)
     plan.fx_hydro_plan_set_topology(neigh)
     plan.fx_hydro_plan_set_workspace()
     U = plan.alloc_state(fill=float("nan"))
@@ -98,7 +97,7 @@ def test_sharded_with_passive_scalars_equals_single_plan():
     for _ in range(3):
         plan.fx_hydro_step(U, dx, cfg.cfl, dt)
         ref_hist.append(float(dt.item()))
-    assert hist == ref_hist
+    assert plan.path == 1 and hist == ref_hist
     assert torch.equal(got, plan.interior(U).cpu())
 
 
