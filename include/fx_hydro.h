@@ -112,8 +112,8 @@ const char *fx_last_error(void);
  * advected quantity (for HLLC: the upwind X_s times the mass flux); no floor, no source term, not in the time step;
  * copied unchanged into guard zones (walls included).  Plans with ns > 0 run on the fused kernel followed by the scalar pass
  * (fx_hydro_plan_path = 1: the stage kernel leaves every face's mass flux and scalar coefficient, a second kernel advances the
- * scalars) where that applies -- 16 x 16 x nz blocks, PLM, no refinement jump; physical boundaries, gravity and the ghost
- * blocks of a sharded plan included -- and on the generic path (0) otherwise;
+ * scalars) where that applies -- 16 x 16 x nz blocks, PLM; physical boundaries, gravity, the ghost blocks of a sharded plan
+ * and refinement jumps (then fx_hydro_plan_path = 5) included -- and on the generic path (0) otherwise;
  * recon FX_RECON_*; riemann FX_RIEMANN_*; rk_order 2 or 3 (SSP-RK).
  * FX_ERR_INVALID_ARG: a dim < 1; no active dim; nguard < 2 (PLM) or < 3 (WENO5); nguard > an active
  * block dim; gamma <= 1; nblocks < 0; unknown enum; nvars < 5.  FX_ERR_UNSUPPORTED: nvars > FX_MAX_NVARS. */
@@ -168,7 +168,7 @@ int fx_hydro_plan_set_topology(fx_hydro_plan *plan, const int32_t *neigh_dev);
  * a clamp (the stage reads none [A11]); fx_guardcell_index_map reports the clamp for zones behind a jump.  Plans with
  * jumps run on the generic path, or on the fused one where the block shape is its (FX_OPT_PATH).  Passive mass scalars
  * (nvars > 5) go through the jumps like the conserved variables they are -- restricted, prolonged, their fluxes corrected --
- * on the generic path.  Call before the workspace (which grows by the jump faces' flux buffer) and the
+ * on either path.  Call before the workspace (which grows by the jump faces' flux buffer) and the
  * topology.  Needs even block extents and nguard <= n_d / 2 in active dimensions (FX_ERR_INVALID_ARG). */
 int fx_hydro_plan_set_refinement(fx_hydro_plan *plan, const int32_t *jump_dev);
 

@@ -207,7 +207,7 @@ extern "C" int fx_hydro_plan_path(const fx_hydro_plan *plan) {
     // refinement jumps [B12-B14]: the generic kernel reads the interpolated guard zones.  Where the fused kernel takes the
     // block shape (5), it advances every block: those WITH a jump face as segments of their own, their halo boxes behind a
     // jump taken from their own guard zones and the jump faces' fluxes stored for the correction
-    return (plan->jlist_host && fx_stage_tma_supported(plan->P)) ? 5 : 0;
+    return (plan->jlist_host && fx_stage_tma_supported(plan->P) && (plan->nvars == 5 || fx_scalar_pass_supported(plan->P))) ? 5 : 0;
   }
   // passive scalars [B11]: behind the fused kernel by the scalar pass where it applies (PLM, same-level neighbours
   // everywhere, no gravity), else on the generic path
@@ -526,7 +526,8 @@ extern "C" int fx_hydro_plan_set_topology(fx_hydro_plan *plan, const int32_t *ne
       const int Rr = plan->P.recon == FX_RECON_WENO5 ? 3 : 2;
       const FxParams &Q = plan->P;
       const bool shape = Q.n[0] == 16 && Q.n[1] == 16 && Q.n[2] >= Rr && Q.active[2] && Q.gd[0] >= Rr && (Q.S_j % 2) == 0 && (Q.gd[0] % 2) == 0;
-      if (jumps && shape && plan->path_option == 0 && plan->nvars == 5 && Q.n[2] <= 64) {
+      // (with passive scalars: where the scalar pass can follow the fused kernel, i.e. PLM)
+      if (jumps && shape && plan->path_option == 0 && (plan->nvars == 5 || Q.recon == FX_RECON_PLM_MINMOD) && Q.n[2] <= 64) {
         plan->jlist_host = new (std::nothrow) int[(size_t)nb];
         if (!plan->jlist_host) return fx_fail(FX_ERR_INVALID_ARG, "set_topology: out of host memory");
         for (long long b = 0; b < nown; ++b) {

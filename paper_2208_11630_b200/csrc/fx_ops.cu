@@ -77,6 +77,7 @@ static int fx_stage(fx_hydro_plan *plan, double *X, const double *U0, double *ou
     const bool rec = plan->timing && plan->ev && plan->nrec < FX_MAX_REC;
     if (rec) FX_CUDA(cudaEventRecord(plan->ev[2 * plan->nrec], st));
     if ((rc = fx_launch_stage_tma(P, X, U0, out, dx, dt, dt_dev, beta, first, 0.0, nullptr, st))) return rc;
+    if (plan->nvars > 5 && (rc = fx_launch_scalar_pass(P, X, U0, out, dx, dt, dt_dev, beta, first, st))) return rc;  // [B11]
     if (rec) {
       FX_CUDA(cudaEventRecord(plan->ev[2 * plan->nrec + 1], st));
       ++plan->nrec;

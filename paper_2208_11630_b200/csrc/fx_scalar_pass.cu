@@ -139,7 +139,10 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 // the fused kernel leaves F_rho alone for it and this pass reads half the face data.
 __device__ __forceinline__ double fx_aq_hllc(double F) { return F > 0.0 ? F : 0.0; }
 
-template <int NSC, bool FIRST, bool HLLC>
+// AMRS: the plan has refinement jumps [B12-B14]: behind a jump face the halo abundances are the block's own guard zones'
+// (interpolated by fx_k_amr_fill for every variable) and the scalars' fluxes through the jump faces are stored with the
+// hydro variables' for the flux correction.
+template <int NSC, bool FIRST, bool HLLC, bool AMRS = false>
 __global__ void __launch_bounds__(256, 2) fx_k_scalar_march(const FxParams P, const double *__restrict__ X, const double *U0, double *out,
                                                             const double *__restrict__ dx, double dt, const double *__restrict__ dt_dev,
                                                             double beta, int sv0) {
@@ -160,9 +163,11 @@ __global__ void __launch_bounds__(256, 2) fx_k_scalar_march(const FxParams P, co
   auto plane_off = [&](int k) -> long long {
     int blk = b, kk = k;
     if (k < 0) {
-      if (nb[4] >= 0) { blk = nb[4]; kk = k + nz; } else kk = nb[4] == FX_BC_REFLECT ? -1 - k : 0;
+      if (nb[4] >= 0) { blk = nb[4]; kk = k + nz; }
+      else if (!(AMRS && nb[4] <= FX_NEIGH_COARSER)) kk = nb[4] == FX_BC_REFLECT ? -1 - k : 0;  // (a jump: the own guard plane k)
     } else if (k >= nz) {
-      if (nb[5] >= 0) { blk = nb[5]; kk = k - nz; } else kk = nb[5] == FX_BC_REFLECT ? 2 * nz - 1 - k : nz - 1;
+      if (nb[5] >= 0) { blk = nb[5]; kk = k - nz; }
+      else if (!(AMRS && nb[5] <= FX_NEIGH_COARSER)) kk = nb[5] == FX_BC_REFLECT ? 2 * nz - 1 - k : nz - 1;
     }
     return (long long)blk * P.S_b + (long long)(kk + g2) * P.S_k + colo;
   };
@@ -171,8 +176,11 @@ __global__ void __launch_bounds__(256, 2) fx_k_scalar_march(const FxParams P, co
   const bool hx = i < 2 || i >= 14, hy = j < 2 || j >= 14;
   // (behind a physical boundary: the block's own edge cell, or its mirror cells at a wall)
   const int nxs = i < 2 ? nb[0] : nb[1], nys = j < 2 ? nb[2] : nb[3];
-  const int xi = i < 2 ? (nxs >= 0 ? 14 + i : (nxs == FX_BC_REFLECT ? 1 - i : 0)) : (nxs >= 0 ? i - 14 : (nxs == FX_BC_REFLECT ? 29 - i : 15));
-  const int yj = j < 2 ? (nys >= 0 ? 14 + j : (nys == FX_BC_REFLECT ? 1 - j : 0)) : (nys >= 0 ? j - 14 : (nys == FX_BC_REFLECT ? 29 - j : 15));
+  const bool jx = AMRS && nxs <= FX_NEIGH_COARSER, jy = AMRS && nys <= FX_NEIGH_COARSER;  // a jump: the own guard zones behind the face
+  const int xi = jx ? (i < 2 ? i - 2 : i + 2)
+                    : (i < 2 ? (nxs >= 0 ? 14 + i : (nxs == FX_BC_REFLECT ? 1 - i : 0)) : (nxs >= 0 ? i - 14 : (nxs == FX_BC_REFLECT ? 29 - i : 15)));
+  const int yj = jy ? (j < 2 ? j - 2 : j + 2)
+                    : (j < 2 ? (nys >= 0 ? 14 + j : (nys == FX_BC_REFLECT ? 1 - j : 0)) : (nys >= 0 ? j - 14 : (nys == FX_BC_REFLECT ? 29 - j : 15)));
   const long long hxo = (long long)(nxs >= 0 ? nxs : b) * P.S_b + (long long)(j + g1) * P.S_j + (xi + g0);
   const long long hyo = (long long)(nys >= 0 ? nys : b) * P.S_b + (long long)(yj + g1) * P.S_j + (i + g0);
   const int hxs = j * 4 + (i < 2 ? i : i - 12), hys = 64 + (j < 2 ? j : j - 12) * 16 + i;
@@ -282,6 +290,17 @@ __global__ void __launch_bounds__(256, 2) fx_k_scalar_march(const FxParams P, co
       Fz[s] = Al * apm + (Fl - Al) * am;
     }
   }
+  // AMRS: which of this zone column's faces are jump faces of the block (bit f: face f; z faces at the first / last plane)
+  unsigned cap = 0;
+  if (AMRS) {
+    cap = (i == 0 && nb[0] <= FX_NEIGH_COARSER ? 1u : 0u) | (i == 15 && nb[1] <= FX_NEIGH_COARSER ? 2u : 0u) |
+          (j == 0 && nb[2] <= FX_NEIGH_COARSER ? 4u : 0u) | (j == 15 && nb[3] <= FX_NEIGH_COARSER ? 8u : 0u) |
+          (nb[4] <= FX_NEIGH_COARSER ? 16u : 0u) | (nb[5] <= FX_NEIGH_COARSER ? 32u : 0u);
+    if (cap & 16u) {
+#pragma unroll
+      for (int s = 0; s < NSC; ++s) P.fjump[(((long long)b * 6 + 4) * P.nvars + sv0 + s) * P.fj_area + tid] = Fz[s];
+    }
+  }
   unsigned hit = 0;
   int hmax = 0;  // largest upper word (sign cleared) of the results: Inf / NaN anywhere in a flux reaches the result
   // this thread's zone of the current plane: in fq (zone of the plane above: the z face's data) and in the state arrays
@@ -334,12 +353,18 @@ __global__ void __launch_bounds__(256, 2) fx_k_scalar_march(const FxParams P, co
       A0[0] = S.fx[buf][1][j][i]; A0[1] = S.fx[buf][1][j][i + 1];
       A1[0] = S.fy[buf][1][j][i]; A1[1] = S.fy[buf][1][j + 1][i];
     }
-    auto flux = [&](const double x[5], double rd, const double Fd[2], const double Ad[2]) {
+    // (AMRS: face f0 / f0 + 1 of the block is the zone's low / high face and a jump: the fluxes are stored [B14])
+    auto flux = [&](const double x[5], double rd, const double Fd[2], const double Ad[2], int f0, int t, int sv) {
       double am[3], ap[3];
 #pragma unroll
       for (int n = 0; n < 3; ++n) fx_plm(x[n], x[n + 1], x[n + 2], am[n], ap[n]);
       const double Fm = Ad[0] * ap[0] + (Fd[0] - Ad[0]) * am[1];
       const double Fp = Ad[1] * ap[1] + (Fd[1] - Ad[1]) * am[2];
+      if (AMRS && ((cap >> f0) & 3u)) {
+        double *dst = P.fjump + (((long long)b * 6 + f0) * P.nvars + sv) * P.fj_area + t;
+        if ((cap >> f0) & 1u) dst[0] = Fm;
+        if ((cap >> f0) & 2u) dst[(long long)P.nvars * P.fj_area] = Fp;
+      }
       return rd * (Fp - Fm);
     };
     double Sv[NSC];
@@ -348,14 +373,15 @@ __global__ void __launch_bounds__(256, 2) fx_k_scalar_march(const FxParams P, co
       double x[5], Ss = 0.0;
 #pragma unroll
       for (int m = 0; m < 5; ++m) x[m] = m == 2 ? xw[0][s] : S.XS[buf][s][j + 2][i + m];  // (the centre is in the z window)
-      Ss += flux(x, rd0, F0, A0);
+      Ss += flux(x, rd0, F0, A0, 0, k * 16 + j, sv0 + s);
 #pragma unroll
       for (int m = 0; m < 5; ++m) x[m] = m == 2 ? xw[0][s] : S.XS[buf][s][j + m][i + 2];
-      Ss += flux(x, rd1, F1, A1);
+      Ss += flux(x, rd1, F1, A1, 2, k * 16 + i, sv0 + s);
       {  // z: the new face only
         double amn, apn;
         fx_plm(xw[0][s], xw[1][s], xn[s], amn, apn);
         const double Fp = Azh * apc[s] + (Fzh - Azh) * amn;
+        if (AMRS && (cap & 32u) && k == nz - 1) P.fjump[(((long long)b * 6 + 5) * P.nvars + sv0 + s) * P.fj_area + tid] = Fp;
         Ss += rd2 * (Fp - Fz[s]);
         Fz[s] = Fp;
         apc[s] = apn;
@@ -382,6 +408,12 @@ template <int NSC, bool FIRST, bool HLLC>
 static int fx_scalar_march_launch2(const FxParams &P, const double *X, const double *U0, double *out, const double *dx, double dt,
                                    const double *dt_dev, double beta, int sv0, cudaStream_t st) {
   const int smem = (int)sizeof(ScalSmem<NSC>);
+  if (P.has_jumps) {
+    FX_CUDA(cudaFuncSetAttribute(fx_k_scalar_march<NSC, FIRST, HLLC, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    fx_k_scalar_march<NSC, FIRST, HLLC, true><<<(unsigned)P.nown, 256, smem, st>>>(P, X, U0, out, dx, dt, dt_dev, beta, sv0);
+    FX_LAUNCH_CHECK("scalar_march");
+    return FX_OK;
+  }
   FX_CUDA(cudaFuncSetAttribute(fx_k_scalar_march<NSC, FIRST, HLLC>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
   fx_k_scalar_march<NSC, FIRST, HLLC><<<(unsigned)P.nown, 256, smem, st>>>(P, X, U0, out, dx, dt, dt_dev, beta, sv0);
   FX_LAUNCH_CHECK("scalar_march");
@@ -403,8 +435,8 @@ static int fx_scalar_march_launch(const FxParams &P, const double *X, const doub
 bool fx_scalar_pass_supported(const FxParams &P) {
   // The marching form serves 16 x 16 x nz blocks with same-level neighbours, physical boundaries (outflow, walls) and ghost
   // blocks behind their faces (the high-face data behind such a face are the fused kernel's own 17th-face solve, P.fqb);
-  // gravity acts on the hydro variables only [B11].  Refinement jumps: generic path.
-  return P.nvars > 5 && P.recon == FX_RECON_PLM_MINMOD && !P.has_jumps && P.fq != nullptr && P.fqb != nullptr && P.n[0] == 16 &&
+  // gravity acts on the hydro variables only [B11]; refinement jumps (AMRS variant) on the fused AMR path.
+  return P.nvars > 5 && P.recon == FX_RECON_PLM_MINMOD && (!P.has_jumps || P.fjump != nullptr) && P.fq != nullptr && P.fqb != nullptr && P.n[0] == 16 &&
          P.n[1] == 16 && P.n[2] >= 2 && P.active[0] && P.active[1] && P.active[2];
 }
 

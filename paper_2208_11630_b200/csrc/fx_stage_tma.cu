@@ -632,7 +632,7 @@ int launch_ws(const FxParams &P, const double *X, const double *U0, double *out,
               double beta, int first, double cfl_next, double *dt_next, cudaStream_t st) {
   if constexpr (RECON == FX_RECON_PLM_MINMOD) {
     if (P.nvars > 5) {  // with passive scalars: also leave the faces' mass flux and Aq for the scalar pass
-      if (P.walls || P.grav_on) {
+      if (P.walls || P.grav_on || P.has_jumps) {
         if (first) return launch<RECON, RIEMANN, WS, true, false, true, true>(P, X, U0, out, dx, dt, dt_dev, beta, 0.0, nullptr, st);
         if (dt_next) return launch<RECON, RIEMANN, WS, false, true, true, true>(P, X, U0, out, dx, dt, dt_dev, beta, cfl_next, dt_next, st);
         return launch<RECON, RIEMANN, WS, false, false, true, true>(P, X, U0, out, dx, dt, dt_dev, beta, 0.0, nullptr, st);
