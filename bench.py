@@ -204,7 +204,8 @@ def build_amr_workload(args, device):
     grid = inputs.two_level_tiling(AMR_NBC, AMR_LO, AMR_HI, order)
     n = len(grid["level"])
     fine, cfg = amr_config(inputs, AMR_NBC, n)
-    plan = fx.HydroPlan(cfg.block_dims, cfg.nguard, n, cfg.gamma, cfg.recon, cfg.riemann, cfg.rk_order, device=device)
+    ns = getattr(args, "scalars", 0)
+    plan = fx.HydroPlan(cfg.block_dims, cfg.nguard, n, cfg.gamma, cfg.recon, cfg.riemann, cfg.rk_order, nvars=5 + ns, device=device)
     plan.fx_hydro_plan_set_option(fx.OPT_PATH, args.path)
     guard_x = args.guard_x if args.guard_x >= 0 else 8
     if guard_x != cfg.nguard:
@@ -218,7 +219,9 @@ def build_amr_workload(args, device):
     Ui = plan.interior(U)
     for b0 in range(0, n, 512):
         b1 = min(n, b0 + 512)
-        Ui[:, b0:b1] = inputs.two_level_interiors(fine, grid, b0, b1, device)
+        Ui[:5, b0:b1] = inputs.two_level_interiors(fine, grid, b0, b1, device)
+        for s in range(ns):  # --scalars: abundances that follow the density field (a throughput workload: any smooth bounded field does)
+            Ui[5 + s, b0:b1] = Ui[0, b0:b1] * (0.5 + 0.4 * torch.sin((s + 1.0) * Ui[0, b0:b1]))
     dxf = fine.dx
     dxh = np.where(grid["level"][:, None] == 1, 1.0, 2.0) * np.array(dxf)[None, :]
     cfg.jump_blocks = int((grid["neigh"] <= inputs.NEIGH_COARSER).any(axis=1).sum())
@@ -438,8 +441,8 @@ def run_ours(args, rank, world, local_rank):
     # fused path: one launch per RK stage, the CFL reduction (a7) rides in the last one; tile and generic paths: one
     # stage kernel per stage, then the reduction pass; with passive scalars also their face fill per stage
     launches_per_step = stages if fused else (stages + 1 + (stages if args.scalars else 0))
-    if args.amr:  # per stage: guard zones behind the jumps, the stage kernel(s), the flux correction; then the reduction pass
-        launches_per_step = stages * 3 + 1
+    if args.amr:  # per stage: guard zones behind the jumps, the stage kernel (and the scalar pass), the flux correction; then the reduction pass
+        launches_per_step = stages * (3 + (args.scalars + 3) // 4) + 1
     if sh is not None:
         launches_per_step += (int(sh.send_elems > 0) + int(sh.recv_elems > 0)) * stages  # pack + unpack of the cut-face slabs before every stage
         if sh.overlap:  # a stage in two launches: the blocks away from the cut beside the exchange, the others behind it
@@ -626,8 +629,10 @@ def main():
     args = parse_args()
     if args.amr:
         args.no_cpu_baseline = True  # (the oracle's two-level runs are in tests/; its timed sample is the uniform workload's)
-        if args.gpus > 1 or args.shard or args.scalars or args.ca or args.nb or args.block or args.config != 5:
-            sys.exit("--amr: single plan, config 5's scheme and field, five variables")
+        if args.gpus > 1 or args.shard or args.ca or args.nb or args.block or args.config != 5:
+            sys.exit("--amr: single plan, config 5's scheme and field")
+        if args.scalars:
+            args.no_e2e = True  # (the end-to-end line is the five-variable workload's)
     if args.ca:
         args.no_e2e = True  # the end-to-end call (fx_hydro_advance_host_interior) runs the standard step
         if args.gpus > 1 or args.shard or args.scalars:
