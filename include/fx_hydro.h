@@ -137,8 +137,11 @@ int fx_hydro_plan_set_option(fx_hydro_plan *plan, int key, double value);
 
 /* Workspace (device, caller-owned, 256-byte aligned): a 256-byte scratch block (dt reduction word,
  * status word and counters) + a 256-byte pad + (rk_order - 1) state copies for the RK stages + the z-segment table
- * (12 int32 per block, 19 for 8 x 8 x nz blocks; see FX_OPT_ZCHAIN).  set_workspace initialises the scratch block and
- * synchronises the device once. */
+ * (12 int32 per block, 19 for 8 x 8 x nz blocks; see FX_OPT_ZCHAIN); with a refinement table also the list of jump faces
+ * (6 int32 per block) and the jump faces' flux buffer (6 faces x nvars x the largest face, per block); with passive scalars
+ * on 16 x 16 x nz blocks and PLM also what the fused kernel hands the scalar pass (6 doubles per zone and 6 per zone of a
+ * block face of 16 x max(nz, 16)).  fx_hydro_plan_workspace_bytes is the authority.  set_workspace initialises the scratch
+ * block and synchronises the device once. */
 size_t fx_hydro_plan_workspace_bytes(const fx_hydro_plan *plan);
 int fx_hydro_plan_set_workspace(fx_hydro_plan *plan, void *workspace_dev, size_t bytes);
 
