@@ -103,7 +103,8 @@ __device__ __forceinline__ double amr_value(const FxParams &P, const double *__r
 __global__ void __launch_bounds__(256) fx_k_amr_fill(const FxParams P, double *U, int depth) {
   // (the grid is the list of jump faces where the plan has one: a CTA per face of EVERY block, most of which only look
   // their face up and leave, took 0.07 ms more.  The face's dimension as a template parameter -- no dynamically indexed
-  // coordinate triples, no stack frame -- was slower: 0.27 against 0.23 ms, three copies of the code.)
+  // coordinate triples -- was slower both ways: as three branches of this kernel 0.27 against 0.23 ms, as three launches
+  // over a list sorted by dimension 0.17 + 0.13 + 0.12 ms (165 registers, a third of the CTAs each).)
   const long long bf = P.jface ? (long long)__ldg(&P.jface[blockIdx.x]) : (long long)blockIdx.x;
   const long long b = bf / 6;
   const int f = (int)(bf % 6), d = f >> 1, side = f & 1;
