@@ -170,6 +170,23 @@ __device__ __forceinline__ void fx_slab_geometry(const FxParams &P, int side, in
   if (side & 1) o[d] += P.n[d] - R;
 }
 
+// The copy of one slab with its extents known at compile time (16-wide blocks, depth 2: the PLM slabs of the fused path) and
+// two doubles per thread: the element -> (v, k, j, i) decode is shifts and masks instead of three integer divisions per
+// element, which were most of the kernel's instructions (0.51 ms per step for 126 MB of slabs each way on rank 0 of 8).
+template <bool PACK, int E0, int E1, int E2>
+__device__ __forceinline__ void fx_slab_copy_fixed(const FxParams &P, double *U, int b, const int o[3], double *dst) {
+  constexpr int H0 = E0 / 2, PER = H0 * E1 * E2;  // pairs per row, per variable
+  const int total = PER * P.nvars;
+  for (int t = threadIdx.x; t < total; t += blockDim.x) {
+    const int v = t / PER, c = t - v * PER;
+    const int k = c / (H0 * E1), r2 = c - k * (H0 * E1);
+    const int j = r2 / H0, i = 2 * (r2 - j * H0);
+    const long long a = (long long)v * P.S_v + (long long)b * P.S_b + (long long)(k + o[2]) * P.S_k + (long long)(j + o[1]) * P.S_j + (i + o[0]);
+    double2 *p = reinterpret_cast<double2 *>(U + a), *q = reinterpret_cast<double2 *>(dst) + t;
+    if (PACK) *q = *p; else *p = *q;
+  }
+}
+
 template <bool PACK>
 __global__ void __launch_bounds__(256) fx_k_halo_slabs(const FxParams P, double *U, const int *__restrict__ items,
                                                        const long long *__restrict__ offsets, int R, double *buf) {
@@ -177,9 +194,19 @@ __global__ void __launch_bounds__(256) fx_k_halo_slabs(const FxParams P, double 
   const int b = items[2 * it], side = items[2 * it + 1];
   int e[3], o[3];
   fx_slab_geometry(P, side, R, e, o);
+  double *dst = buf + offsets[it];
+  // the fixed-extent form needs 16-byte aligned pairs: even origins and strides (even guard depths), an aligned array and slot
+  const bool pairs = R == 2 && P.n[0] == 16 && P.n[1] == 16 && P.n[2] == 16 && !((o[0] | P.S_j) & 1) &&
+                     !(((unsigned long long)U | (unsigned long long)dst) & 15);
+  if (pairs) {
+    const int d = side >> 1;
+    if (d == 0) fx_slab_copy_fixed<PACK, 2, 16, 16>(P, U, b, o, dst);
+    else if (d == 1) fx_slab_copy_fixed<PACK, 16, 2, 16>(P, U, b, o, dst);
+    else fx_slab_copy_fixed<PACK, 16, 16, 2>(P, U, b, o, dst);
+    return;
+  }
   const int per_var = e[0] * e[1] * e[2];
   const int total = per_var * P.nvars;
-  double *dst = buf + offsets[it];
   for (int t = threadIdx.x; t < total; t += blockDim.x) {
     const int v = t / per_var, c = t - v * per_var;
     const int k = c / (e[0] * e[1]), r2 = c - k * e[0] * e[1];
