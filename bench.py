@@ -643,6 +643,10 @@ def main():
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.impl != "reference":
         # started plainly with --gpus N: launch the N ranks ourselves (one process per GPU, NCCL), as the driver's torchrun would
         import socket
+        import torch
+        if torch.cuda.device_count() < args.gpus:
+            sys.exit(f"bench.py --gpus {args.gpus}: this machine has {torch.cuda.device_count()} GPU(s); one process per GPU is needed "
+                     "(`--one-rank-of N` times one rank of an N-way partition alone)")
         sk = socket.socket()
         sk.bind(("127.0.0.1", 0))
         port = sk.getsockname()[1]
