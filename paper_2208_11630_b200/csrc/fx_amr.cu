@@ -95,12 +95,14 @@ __device__ __forceinline__ double amr_value(const FxParams &P, const double *__r
   return __dmul_rn(sum, 1.0 / (double)(s.cnt[0] * s.cnt[1] * s.cnt[2]));
 }
 
-// One CTA per (block, face); a thread per face guard zone of depth `depth`: it resolves where the zone's data comes from
-// once -- behind finer neighbours one location, behind a coarser one the parent zone and its two neighbours per active
-// dimension -- and then evaluates all variables.  (First version: a thread per zone AND variable, 128 threads per CTA, every
-// value resolving its seven locations itself, the restriction a loop whose every addition waited for its own load: 0.43 ms
-// per fill on the two-level workload of bench.py --amr, a fifth of the step; now 0.23 ms.)
-__global__ void __launch_bounds__(256) fx_k_amr_fill(const FxParams P, double *U, int depth) {
+// CTAs of 64 threads per (block, face).  Behind finer neighbours a thread per face guard zone of depth `depth` (the zones
+// split over the grid's y extent): it resolves the one location its data comes from and evaluates all variables.  Behind a
+// coarser neighbour a thread per parent zone (below).  (First version: a thread per zone AND variable, 128 threads per CTA,
+// every value resolving its seven locations itself, the restriction a loop whose every addition waited for its own load:
+// 0.43 ms per fill on the two-level workload of bench.py --amr, a fifth of the step; a thread per guard zone on both sides,
+// 256 threads: 0.23 ms; a thread per parent zone in 256-thread CTAs: 188 registers, one CTA per SM with two busy warps,
+// 0.29 ms; 64-thread CTAs held to 128 registers, eight per SM: 0.11 ms.)
+__global__ void __launch_bounds__(64, 8) fx_k_amr_fill(const FxParams P, double *U, int depth) {
   // (the grid is the list of jump faces where the plan has one: a CTA per face of EVERY block, most of which only look
   // their face up and leave, took 0.07 ms more.  The face's dimension as a template parameter -- no dynamically indexed
   // coordinate triples -- was slower both ways: as three branches of this kernel 0.27 against 0.23 ms, as three launches
@@ -113,17 +115,17 @@ __global__ void __launch_bounds__(256) fx_k_amr_fill(const FxParams P, double *U
   if (code != FX_NEIGH_COARSER && code != FX_NEIGH_FINER) return;
   const int d1 = d == 0 ? 1 : 0, d2 = d == 2 ? 1 : 2;
   const int n1 = P.n[d1], n2 = P.n[d2];
-  const int total = depth * n1 * n2;
-  for (int r = threadIdx.x; r < total; r += blockDim.x) {
-    const int m = r / (n1 * n2), r2 = r - m * (n1 * n2), t2 = r2 / n1, t1 = r2 - t2 * n1;
-    int c[3];
-    c[d] = side ? P.n[d] + m : -1 - m;
-    c[d1] = t1;
-    c[d2] = t2;
-    double *dst = U + b * P.S_b + (long long)(c[2] + P.gd[2]) * P.S_k + (long long)(c[1] + P.gd[1]) * P.S_j + (c[0] + P.gd[0]);
-    // (every value a zone needs is loaded before its first store: the loads of all variables are then in flight together
-    // instead of one DRAM round trip per variable)
-    if (code == FX_NEIGH_FINER) {
+  if (code == FX_NEIGH_FINER) {
+    const int total = depth * n1 * n2;
+    for (int r = threadIdx.x + blockDim.x * blockIdx.y; r < total; r += blockDim.x * gridDim.y) {
+      const int m = r / (n1 * n2), r2 = r - m * (n1 * n2), t2 = r2 / n1, t1 = r2 - t2 * n1;
+      int c[3];
+      c[d] = side ? P.n[d] + m : -1 - m;
+      c[d1] = t1;
+      c[d2] = t2;
+      double *dst = U + b * P.S_b + (long long)(c[2] + P.gd[2]) * P.S_k + (long long)(c[1] + P.gd[1]) * P.S_j + (c[0] + P.gd[0]);
+      // (every value a zone needs is loaded before its first store: the loads of all variables are then in flight together
+      // instead of one DRAM round trip per variable)
       AmrSrc s;
       amr_locate(P, b, c, s);
       for (int v0 = 0; v0 < P.nvars; v0 += 5) {  // (five variables at a time: the hydro set, then the passive scalars)
@@ -135,47 +137,68 @@ __global__ void __launch_bounds__(256) fx_k_amr_fill(const FxParams P, double *U
         for (int v = 0; v < 5; ++v)
           if (v0 + v < P.nvars) dst[(long long)(v0 + v) * P.S_v] = val[v];
       }
-    } else {
-      const long long cb = __ldg(&P.jump[(b * 6 + f) * 4 + 0]);
-      const int qd = __ldg(&P.jump[(b * 6 + f) * 4 + 1]);
-      int C[3] = {0, 0, 0};
-      double sg[3] = {0.0, 0.0, 0.0};
-      C[d] = side ? m / 2 : P.n[d] - 1 - m / 2;
-      sg[d] = ((m % 2 == 0) == (side == 0)) ? 1.0 : -1.0;
-      const int tr[2] = {d1, d2}, tc[2] = {t1, t2};
+    }
+    return;
+  }
+  if (blockIdx.y) return;  // (the grid's y extent splits the restriction faces' zones only)
+  // Behind a coarser neighbour: a thread per PARENT zone of the neighbour.  The (up to eight) guard zones it covers share
+  // the parent's value, its two neighbours per active dimension and so the limited slopes; only the signs of the quarter
+  // offsets differ.  (A thread per guard zone resolved the same seven locations and loaded the same values eight times over:
+  // 2400 warp instructions per 32 zones, 0.23 ms per fill of the two-level workload.)
+  const long long cb = __ldg(&P.jump[(b * 6 + f) * 4 + 0]);
+  const int qd = __ldg(&P.jump[(b * 6 + f) * 4 + 1]);
+  const int a1 = P.active[d1] ? 2 : 1, a2 = P.active[d2] ? 2 : 1;  // children per parent across the face
+  const int p1n = n1 / a1, p2n = n2 / a2, pmn = (depth + 1) / 2;
+  for (int r = threadIdx.x; r < pmn * p1n * p2n; r += blockDim.x) {
+    const int mc = r / (p1n * p2n), r2 = r - mc * (p1n * p2n), p2 = r2 / p1n, p1 = r2 - p2 * p1n;
+    int C[3] = {0, 0, 0};
+    C[d] = side ? mc : P.n[d] - 1 - mc;
+    if (P.active[d1]) C[d1] = ((qd >> 0) & 1) * (P.n[d1] / 2) + p1;
+    if (P.active[d2]) C[d2] = ((qd >> 1) & 1) * (P.n[d2] / 2) + p2;
+    AmrSrc sC, sm[3], sp[3];
+    bool both[3] = {false, false, false};
+    amr_locate(P, cb, C, sC);
 #pragma unroll
-      for (int t_ = 0; t_ < 2; ++t_) {
-        const int e2 = tr[t_];
-        if (!P.active[e2]) continue;
-        C[e2] = ((qd >> t_) & 1) * (P.n[e2] / 2) + tc[t_] / 2;
-        sg[e2] = (tc[t_] % 2) ? 1.0 : -1.0;
-      }
-      AmrSrc sC, sm[3], sp[3];
-      bool both[3] = {false, false, false};
-      amr_locate(P, cb, C, sC);
+    for (int e2 = 0; e2 < 3; ++e2) {
+      if (!P.active[e2]) continue;
+      int Cm[3] = {C[0], C[1], C[2]}, Cp[3] = {C[0], C[1], C[2]};
+      Cm[e2] -= 1;
+      Cp[e2] += 1;
+      both[e2] = amr_locate(P, cb, Cm, sm[e2]) && amr_locate(P, cb, Cp, sp[e2]);
+    }
+    for (int v0 = 0; v0 < P.nvars; v0 += 5) {
+      double qC[5], qm[3][5], qp[3][5];
+#pragma unroll
+      for (int v = 0; v < 5; ++v)
+        if (v0 + v < P.nvars) qC[v] = amr_value(P, U, sC, v0 + v);
 #pragma unroll
       for (int e2 = 0; e2 < 3; ++e2) {
-        if (!P.active[e2]) continue;
-        int Cm[3] = {C[0], C[1], C[2]}, Cp[3] = {C[0], C[1], C[2]};
-        Cm[e2] -= 1;
-        Cp[e2] += 1;
-        both[e2] = amr_locate(P, cb, Cm, sm[e2]) && amr_locate(P, cb, Cp, sp[e2]);
+        if (!both[e2]) continue;
+#pragma unroll
+        for (int v = 0; v < 5; ++v) {
+          if (v0 + v >= P.nvars) continue;
+          qm[e2][v] = amr_value(P, U, sm[e2], v0 + v);
+          qp[e2][v] = amr_value(P, U, sp[e2], v0 + v);
+        }
       }
-      for (int v0 = 0; v0 < P.nvars; v0 += 5) {
-        double qC[5], qm[3][5], qp[3][5];
+      double sl[3][5];  // the limited slopes, per dimension and variable
+#pragma unroll
+      for (int e2 = 0; e2 < 3; ++e2)
 #pragma unroll
         for (int v = 0; v < 5; ++v)
-          if (v0 + v < P.nvars) qC[v] = amr_value(P, U, sC, v0 + v);
-#pragma unroll
-        for (int e2 = 0; e2 < 3; ++e2) {
-          if (!both[e2]) continue;
-#pragma unroll
-          for (int v = 0; v < 5; ++v) {
-            if (v0 + v >= P.nvars) continue;
-            qm[e2][v] = amr_value(P, U, sm[e2], v0 + v);
-            qp[e2][v] = amr_value(P, U, sp[e2], v0 + v);
-          }
-        }
+          sl[e2][v] = (both[e2] && v0 + v < P.nvars) ? amr_minmod(__dsub_rn(qC[v], qm[e2][v]), __dsub_rn(qp[e2][v], qC[v])) : 0.0;
+      for (int ch = 0; ch < 2 * a1 * a2; ++ch) {
+        const int b1 = ch % a1, b2 = (ch / a1) % a2, mm = ch / (a1 * a2), m = 2 * mc + mm;
+        if (m >= depth) continue;
+        int c[3];
+        double sg[3] = {0.0, 0.0, 0.0};
+        c[d] = side ? P.n[d] + m : -1 - m;
+        c[d1] = a1 * p1 + b1;
+        c[d2] = a2 * p2 + b2;
+        sg[d] = ((mm == 0) == (side == 0)) ? 1.0 : -1.0;
+        if (P.active[d1]) sg[d1] = b1 ? 1.0 : -1.0;
+        if (P.active[d2]) sg[d2] = b2 ? 1.0 : -1.0;
+        double *dst = U + b * P.S_b + (long long)(c[2] + P.gd[2]) * P.S_k + (long long)(c[1] + P.gd[1]) * P.S_j + (c[0] + P.gd[0]);
 #pragma unroll
         for (int v = 0; v < 5; ++v) {
           if (v0 + v >= P.nvars) continue;
@@ -183,7 +206,7 @@ __global__ void __launch_bounds__(256) fx_k_amr_fill(const FxParams P, double *U
 #pragma unroll
           for (int e2 = 0; e2 < 3; ++e2) {
             if (!both[e2]) continue;
-            val = __dadd_rn(val, __dmul_rn(sg[e2] * 0.25, amr_minmod(__dsub_rn(qC[v], qm[e2][v]), __dsub_rn(qp[e2][v], qC[v]))));
+            val = __dadd_rn(val, __dmul_rn(sg[e2] * 0.25, sl[e2][v]));
           }
           dst[(long long)(v0 + v) * P.S_v] = val;
         }
@@ -241,7 +264,7 @@ __global__ void __launch_bounds__(128) fx_k_amr_flux_correct(const FxParams P, d
 
 int fx_launch_amr_fill(const FxParams &P, double *U, int depth, cudaStream_t st) {
   if (!P.jump || !P.has_jumps || P.nblocks == 0) return FX_OK;
-  fx_k_amr_fill<<<(unsigned)(P.jface ? P.njface : P.nblocks * 6), 256, 0, st>>>(P, U, depth);
+  fx_k_amr_fill<<<dim3((unsigned)(P.jface ? P.njface : P.nblocks * 6), 4), 64, 0, st>>>(P, U, depth);
   FX_LAUNCH_CHECK("amr_fill");
   return FX_OK;
 }
