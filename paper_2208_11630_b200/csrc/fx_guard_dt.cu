@@ -191,7 +191,8 @@ int fx_launch_index_map(const FxParams &P, long long b0, long long nb, long long
 // the scratch words for the next call.  HBM-bound: one 40 B/zone read pass.
 __global__ void __launch_bounds__(256) fx_k_compute_dt(FxParams P, const double *__restrict__ U,
                                                        const double *__restrict__ dx, double cfl,
-                                                       double *__restrict__ dt_out) {
+                                                       double *__restrict__ dt_out, const int *__restrict__ jface,
+                                                       long long njface) {
   const unsigned nx = P.n[0], ny = P.n[1];
   const unsigned per_block = nx * ny * (unsigned)P.n[2];
   double rate = 0.0;  // max of (|u_d| + c) / dx_d
@@ -199,7 +200,18 @@ __global__ void __launch_bounds__(256) fx_k_compute_dt(FxParams P, const double 
   // 16-byte loads need every zone pair (i even) on a 16-byte boundary: even nx, guard depth and strides, aligned base
   const bool pairs = (nx % 2 == 0) && (P.gd[0] % 2 == 0) && (P.S_j % 2 == 0) && (P.S_v % 2 == 0) &&
                      ((reinterpret_cast<unsigned long long>(U) & 15ull) == 0);
-  for (long long b = blockIdx.x; b < P.nown; b += gridDim.x) {  // owned blocks only (a shard's ghosts are halo sources)
+  // (jface: only the owned blocks with a finer neighbour, each at the first such face of the jump-face list)
+  const long long nit = jface ? njface : P.nown;
+  for (long long it = blockIdx.x; it < nit; it += gridDim.x) {  // owned blocks only (a shard's ghosts are halo sources)
+    long long b = it;
+    if (jface) {
+      const int bf = __ldg(&jface[it]);
+      b = bf / 6;
+      const int f = bf % 6;
+      bool mine = b < P.nown && __ldg(&P.neigh[b * 6 + f]) == FX_NEIGH_FINER;
+      for (int g = 0; g < f; ++g) mine = mine && __ldg(&P.neigh[b * 6 + g]) != FX_NEIGH_FINER;
+      if (!mine) continue;
+    }
     double idx[3];
 #pragma unroll
     for (int d = 0; d < 3; ++d) idx[d] = P.active[d] ? 1.0 / __ldg(&dx[b * 3 + d]) : 0.0;
@@ -289,7 +301,17 @@ int fx_launch_compute_dt(const FxParams &P, const double *U, const double *dx, d
   const long long want = P.nown < 1 ? 1 : P.nown;
   const long long cap = (long long)fx_sm_count() * 8;
   const int grid = (int)(want > cap ? cap : want);
-  fx_k_compute_dt<<<grid, 256, 0, st>>>(P, U, dx, cfl, dt_out);
+  fx_k_compute_dt<<<grid, 256, 0, st>>>(P, U, dx, cfl, dt_out, nullptr, 0);
   FX_LAUNCH_CHECK("compute_dt");
+  return FX_OK;
+}
+
+int fx_launch_compute_dt_corrected(const FxParams &P, const double *U, const double *dx, double cfl, double *dt_out,
+                                   cudaStream_t st) {
+  const long long want = P.njface < 1 ? 1 : P.njface;
+  const long long cap = (long long)fx_sm_count() * 8;
+  const int grid = (int)(want > cap ? cap : want);
+  fx_k_compute_dt<<<grid, 256, 0, st>>>(P, U, dx, cfl, dt_out, P.jface, P.jface ? P.njface : 0);
+  FX_LAUNCH_CHECK("compute_dt_corrected");
   return FX_OK;
 }

@@ -37,6 +37,8 @@ struct FxParams {
   int has_jumps;                    // some active face carries FX_NEIGH_COARSER / FX_NEIGH_FINER
   const int *jface;                 // the faces that carry a jump, as b * 6 + f, device (behind the segment tables in the workspace), or nullptr
   long long njface;
+  int dt_defer;                     // fused AMR path, last stage: the stage kernel leaves the CFL maximum of the blocks the flux correction
+                                    // does not touch in the scratch word; fx_launch_compute_dt_corrected adds the others and writes dt
   double *fjump;                    // boundary-face fluxes captured at jump faces [B14]: [nblocks][6][5][fj_area], in the workspace
   int fj_area;                      // largest face of a block, in zones
   long long njump;                  // fused AMR path (fx_hydro_plan_path = 5): how many blocks have a jump face (each a segment of its own)
@@ -113,6 +115,10 @@ int fx_launch_index_map(const FxParams &P, long long b0, long long nb, long long
 int fx_launch_pack_interior(const FxParams &P, double *U, double *packed, int to_packed, cudaStream_t st);
 int fx_launch_compute_dt(const FxParams &P, const double *U, const double *dx, double cfl, double *dt_out,
                          cudaStream_t st);
+// the same over the owned blocks with a finer neighbour only (the blocks the flux correction changes), on top of the maximum
+// a stage kernel launched with P.dt_defer left in the scratch word
+int fx_launch_compute_dt_corrected(const FxParams &P, const double *U, const double *dx, double cfl, double *dt_out,
+                                   cudaStream_t st);
 int fx_launch_generic_stage(const FxParams &P, const double *X, const double *U0, double *out, const double *dx,
                             double dt, const double *dt_dev, double beta, int first, cudaStream_t st);
 int fx_launch_debug_fluxes(const FxParams &P, const double *U, int dir, double *F, cudaStream_t st);

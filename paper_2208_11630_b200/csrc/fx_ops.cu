@@ -71,18 +71,23 @@ static int fx_stage(fx_hydro_plan *plan, double *X, const double *U0, double *ou
   if (path == 5) {
     // fused AMR path: guard zones behind the jumps, then the fused kernel on every block (the blocks with a jump face read
     // their own guard zones behind it and store the jump faces' fluxes), then the flux correction; the time step of the
-    // finished state, if asked for, as a pass of its own (the fused reduction would miss the correction)
+    // finished state, if asked for: the stage kernel's fused reduction over the blocks the correction does not touch, then
+    // a pass over the corrected blocks (a first stage, which has no fused reduction: a pass over every block)
     const FxParams &P = plan->P;
     if ((rc = fx_launch_amr_fill(P, X, P.recon == FX_RECON_WENO5 ? 3 : 2, st))) return rc;
     const bool rec = plan->timing && plan->ev && plan->nrec < FX_MAX_REC;
     if (rec) FX_CUDA(cudaEventRecord(plan->ev[2 * plan->nrec], st));
-    if ((rc = fx_launch_stage_tma(P, X, U0, out, dx, dt, dt_dev, beta, first, 0.0, nullptr, st))) return rc;
+    const bool fuse_dt = dt_next && !first && P.jface && P.njface > 0;
+    FxParams Pd = P;
+    Pd.dt_defer = fuse_dt ? 1 : 0;
+    if ((rc = fx_launch_stage_tma(Pd, X, U0, out, dx, dt, dt_dev, beta, first, cfl_next, fuse_dt ? dt_next : nullptr, st))) return rc;
     if (plan->nvars > 5 && (rc = fx_launch_scalar_pass(P, X, U0, out, dx, dt, dt_dev, beta, first, st))) return rc;  // [B11]
     if (rec) {
       FX_CUDA(cudaEventRecord(plan->ev[2 * plan->nrec + 1], st));
       ++plan->nrec;
     }
     if ((rc = fx_launch_amr_flux_correct(P, out, dx, dt, dt_dev, first ? 1.0 : beta, st))) return rc;
+    if (fuse_dt) return fx_launch_compute_dt_corrected(P, out, dx, cfl_next, dt_next, st);
     if (dt_next) return fx_launch_compute_dt(P, out, dx, cfl_next, dt_next, st);
     return FX_OK;
   }

@@ -581,14 +581,22 @@ fx_k_stage_tma(const __grid_constant__ CUtensorMap mXm, const __grid_constant__ 
         double mx = S.wmax[0];
 #pragma unroll
         for (int w8 = 1; w8 < 8; ++w8) mx = fmax(mx, S.wmax[w8]);
-        atomicMax(&P.scratch[FX_SCR_DTBITS], (unsigned long long)__double_as_longlong(mx));
-        __threadfence();
-        const unsigned long long done = atomicAdd(&P.scratch[FX_SCR_COUNTER], 1ull);
-        if (done == (unsigned long long)P.nseg_all - 1) {  // the stage's last CTA (the stage may be launched in two parts)
+        if (EXTRAS && P.dt_defer) {
+          // fused AMR path: the flux correction still changes the blocks with a finer neighbour (each a segment of its own);
+          // the others' maximum waits in the scratch word for fx_launch_compute_dt_corrected, which writes the time step
+          bool corr = false;
+          for (int f = 0; f < 6; ++f) corr |= __ldg(&P.neigh[(long long)S.chain[2] * 6 + f]) == FX_NEIGH_FINER;
+          if (!corr) atomicMax(&P.scratch[FX_SCR_DTBITS], (unsigned long long)__double_as_longlong(mx));
+        } else {
+          atomicMax(&P.scratch[FX_SCR_DTBITS], (unsigned long long)__double_as_longlong(mx));
           __threadfence();
-          const unsigned long long bits = atomicExch(&P.scratch[FX_SCR_DTBITS], 0ull);
-          P.scratch[FX_SCR_COUNTER] = 0ull;
-          *dt_next = cfl_next / __longlong_as_double((long long)bits);
+          const unsigned long long done = atomicAdd(&P.scratch[FX_SCR_COUNTER], 1ull);
+          if (done == (unsigned long long)P.nseg_all - 1) {  // the stage's last CTA (the stage may be launched in two parts)
+            __threadfence();
+            const unsigned long long bits = atomicExch(&P.scratch[FX_SCR_DTBITS], 0ull);
+            P.scratch[FX_SCR_COUNTER] = 0ull;
+            *dt_next = cfl_next / __longlong_as_double((long long)bits);
+          }
         }
       }
       tma_wait_all();

@@ -60,7 +60,7 @@ def test_hybrid_parity_conservation_and_generic(nbc, refined, periodic, recon, r
         oplan.advance(Uo, dx, dt)
         gplan.fx_hydro_advance(Ud, dxd, dt)
         ggen.fx_hydro_advance(Ug, dxd, dt)
-        if step < 3:  # fx_hydro_step: same states with the time step kept on the device (the reduction as a pass of its own)
+        if step < 3:  # fx_hydro_step: same states with the time step kept on the device (the reduction fused but for the corrected blocks)
             assert abs(float(dts.item()) - dt) <= 1e-12 * dt
             gplan.fx_hydro_step(Us, dxd, 0.3, dts)
         if step in (0, 9):
@@ -184,3 +184,41 @@ def test_jumps_next_to_walls_with_gravity(recon, rk):
     fo, _ = oplan.status()
     fg, _ = gplan.fx_hydro_status()
     assert fo == fg == 0
+
+
+@pytest.mark.parametrize("recon,rk", [(0, 2), (1, 3)])
+def test_step_time_step_wherever_the_fastest_zone_sits(recon, rk):
+    """fx_hydro_step on the fused path forms the next time step in two pieces: the last stage kernel's own reduction over the
+    blocks the flux correction leaves alone, then a pass over the corrected blocks (those with a finer neighbour).  With the
+    fastest zone (a hot block) put in a corrected block, in a fine block behind a jump, or far from any jump, the step's dt
+    equals fx_hydro_compute_dt of the state it produced and the oracle's [B7, B14]."""
+    from paper_2208_11630_b200.binding import NEIGH_FINER, NEIGH_COARSER
+    grid = two_level_grid((4, 4, 4), CENTRE2, DIMS)
+    neigh = np.asarray(grid["neigh"]).reshape(-1, 6)
+    corrected = [b for b in range(len(neigh)) if (neigh[b] == NEIGH_FINER).any()]
+    fine = [b for b in range(len(neigh)) if (neigh[b] == NEIGH_COARSER).any()]
+    plain = [b for b in range(len(neigh)) if b not in corrected and b not in fine]
+    assert corrected and fine and plain
+    oplan = amr_plan(grid, DIMS, recon=recon, rk=rk)
+    gplan = gpu_plan(grid, recon, 1, rk)
+    assert gplan.path == 5
+    dx = dx_of(grid)
+    dxd = torch.from_numpy(dx).cuda()
+    prim = smooth_field(grid, DIMS, [64, 64, 64])
+    seen = []
+    for hot in (corrected[0], corrected[-1], fine[0], plain[0], plain[-1]):
+        Uo = state_from(oplan, prim)
+        Io = oplan.interior(Uo)
+        Io[4, hot] *= 6.0  # total energy: a hot block, the largest sound speed by far
+        Ud = torch.from_numpy(Uo).cuda()
+        dts = gplan.fx_hydro_compute_dt(Ud, dxd, 0.3).clone()
+        dt = oplan.compute_dt(Uo, dx, 0.3)
+        assert abs(float(dts.item()) - dt) <= 1e-13 * dt
+        oplan.advance(Uo, dx, dt)
+        gplan.fx_hydro_step(Ud, dxd, 0.3, dts)
+        after = float(gplan.fx_hydro_compute_dt(Ud, dxd, 0.3).item())
+        assert abs(float(dts.item()) - after) <= 1e-14 * after, (hot, float(dts.item()), after)
+        dto = oplan.compute_dt(Uo, dx, 0.3)
+        assert abs(float(dts.item()) - dto) <= 1e-12 * dto
+        seen.append(after)
+    assert len({round(s / seen[0], 6) for s in seen}) > 1  # (the fastest zone really moved with the hot block)
